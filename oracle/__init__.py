@@ -1,0 +1,156 @@
+"""fp64 CPU oracle of the GAMER-2 patch-group hydro solver -- TEST INFRASTRUCTURE, not the product.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
+this package.  It never imports paper_1712_07070_b200 (and is never imported by it).
+The arithmetic lives in hydro_oracle.c (plain C, gcc); this file only marshals numpy arrays.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+from . import build as _build
+
+MHM, CTU = 1, 2
+PLM, PPM = 1, 2
+ROE, HLLC, HLLE = 1, 2, 3
+GMINMOD, VANLEER, VANALBADA = 1, 2, 3
+
+PS, NG, NP = 16, 3, 22
+
+
+class Opts(ctypes.Structure):
+    _fields_ = [
+        ("limiter", ctypes.c_int),
+        ("theta", ctypes.c_double),
+        ("n_scalar", ctypes.c_int),
+        ("dual_energy", ctypes.c_int),
+        ("de_xi", ctypes.c_double),
+        ("min_dens", ctypes.c_double),
+        ("min_pres", ctypes.c_double),
+        ("min_temp", ctypes.c_double),
+        ("remedy_first_order", ctypes.c_int),
+    ]
+
+
+class Stats(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_int64) for n in (
+        "n_riemann", "n_riemann_final", "n_roe_fallback", "n_pred_revert",
+        "n_first_order", "n_dual_fix", "n_floor", "n_unphysical")]
+
+    def as_dict(self):
+        return {n: int(getattr(self, n)) for n, _ in self._fields_}
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = ctypes.CDLL(_build.build())
+        assert _lib.oracle_sizeof_opts() == ctypes.sizeof(Opts)
+        assert _lib.oracle_sizeof_stats() == ctypes.sizeof(Stats)
+        _lib.oracle_limited_slope.restype = ctypes.c_double
+        _lib.oracle_limited_slope.argtypes = [ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_double]
+    return _lib
+
+
+def make_opts(limiter=GMINMOD, theta=0.0, n_scalar=0, dual_energy=False, de_xi=1e-2,
+              min_dens=0.0, min_pres=0.0, min_temp=0.0, remedy_first_order=False):
+    return Opts(limiter, theta, n_scalar, int(dual_energy), de_xi, min_dens, min_pres, min_temp,
+                int(remedy_first_order))
+
+
+def _p(a):
+    return a.ctypes.data_as(ctypes.c_void_p) if a is not None else None
+
+
+def _c64(a):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a
+
+
+def set_threads(n):
+    os.environ["OMP_NUM_THREADS"] = str(n)
+
+
+def fluid_advance(u_in, dt, dh, gamma, scheme, recon, riemann, opts=None, want_flux=True):
+    """u_in: [G, NV, 22, 22, 22] -> dict(out [G,NV,16,16,16], flux [G,3,3,NV,16,16], speed [G], stats)."""
+    u_in = _c64(u_in)
+    g, nv = u_in.shape[0], u_in.shape[1]
+    assert u_in.shape[2:] == (NP, NP, NP)
+    if opts is None:
+        opts = make_opts()
+    assert nv == 5 + opts.n_scalar
+    out = np.empty((g, nv, PS, PS, PS), dtype=np.float64)
+    flux = np.empty((g, 3, 3, nv, PS, PS), dtype=np.float64) if want_flux else None
+    speed = np.empty((g,), dtype=np.float64)
+    st = Stats()
+    rc = lib().oracle_fluid_advance(_p(u_in), _p(out), _p(flux), _p(speed), ctypes.c_int64(g),
+                                    ctypes.c_double(dt), ctypes.c_double(dh), ctypes.c_double(gamma),
+                                    int(scheme), int(recon), int(riemann), ctypes.byref(opts), ctypes.byref(st))
+    if rc != 0:
+        raise ValueError(f"oracle_fluid_advance returned {rc}")
+    return {"out": out, "flux": flux, "speed": speed, "stats": st.as_dict()}
+
+
+def cfl_dt(u, dh, gamma, cfl, scheme, opts=None):
+    """u: [G, NV, 16,16,16] -> (dt, group_speed[G])"""
+    u = _c64(u)
+    g = u.shape[0]
+    if opts is None:
+        opts = make_opts(n_scalar=u.shape[1] - 5)
+    speed = np.empty((g,), dtype=np.float64)
+    dt = ctypes.c_double(0.0)
+    rc = lib().oracle_cfl_dt(_p(u), ctypes.c_int64(g), ctypes.c_double(dh), ctypes.c_double(gamma),
+                             ctypes.c_double(cfl), int(scheme), ctypes.byref(opts), _p(speed), ctypes.byref(dt))
+    if rc != 0:
+        raise ValueError(f"oracle_cfl_dt returned {rc}")
+    return dt.value, speed
+
+
+def riemann(solver, axis, UL, UR, gamma, n_scalar=0):
+    UL, UR = _c64(UL), _c64(UR)
+    F = np.zeros(5 + n_scalar)
+    fb = ctypes.c_int(0)
+    lib().oracle_riemann(int(solver), int(axis), _p(UL), _p(UR), ctypes.c_double(gamma), int(n_scalar),
+                         _p(F), ctypes.byref(fb))
+    return F, fb.value
+
+
+def roe_decomposition(UL, UR, gamma):
+    UL, UR = _c64(UL), _c64(UR)
+    alpha, lam, K = np.zeros(5), np.zeros(5), np.zeros((5, 5))
+    lib().oracle_roe_decomposition(_p(UL), _p(UR), ctypes.c_double(gamma), _p(alpha), _p(lam), _p(K))
+    return alpha, lam, K
+
+
+def limited_slope(limiter, theta, dL, dR):
+    return lib().oracle_limited_slope(int(limiter), float(theta), float(dL), float(dR))
+
+
+def face_values(recon, w5, limiter=GMINMOD, theta=None):
+    if theta is None:
+        theta = 2.0 if recon == PPM else 1.0
+    w5 = _c64(w5)
+    wm, wp = ctypes.c_double(0), ctypes.c_double(0)
+    lib().oracle_face_values(int(recon), int(limiter), ctypes.c_double(theta), _p(w5),
+                             ctypes.byref(wm), ctypes.byref(wp))
+    return wm.value, wp.value
+
+
+def trace_cell(recon, gamma, W, wm, wp, dt_over_dh):
+    W, wm, wp = _c64(W), _c64(wm), _c64(wp)
+    ns = W.shape[0] - 5
+    tm, tp = np.zeros_like(W), np.zeros_like(W)
+    lib().oracle_trace_cell(int(recon), ctypes.c_double(gamma), int(ns), _p(W), _p(wm), _p(wp),
+                            ctypes.c_double(dt_over_dh), _p(tm), _p(tp))
+    return tm, tp
+
+
+def close_cell(U, gamma, opts):
+    U = _c64(U).copy()
+    st = Stats()
+    ok = lib().oracle_close_cell(_p(U), ctypes.c_double(gamma), ctypes.byref(opts), ctypes.byref(st))
+    return U, bool(ok), st.as_dict()

@@ -1,0 +1,115 @@
+"""Pins for slope limiters, PLM/PPM face values and characteristic tracing (oracle O2, O3, O4-CTU(a))."""
+import math
+
+import numpy as np
+import pytest
+
+PLM, PPM = 1, 2
+
+
+def test_generalized_minmod_closed_forms(oracle_mod):
+    o = oracle_mod
+    assert o.limited_slope(1, 1.0, 1.0, 3.0) == 1.0          # theta=1: plain minmod
+    assert o.limited_slope(1, 1.0, -3.0, -1.0) == -1.0
+    assert o.limited_slope(1, 2.0, 1.0, 3.0) == 2.0          # theta=2: min(2, 2, 6)
+    assert o.limited_slope(1, 2.0, 1.0, 1.5) == 1.25         # centred slope wins
+    assert o.limited_slope(1, 1.5, 1.0, 100.0) == 1.5
+    for th in (1.0, 1.5, 2.0):
+        assert o.limited_slope(1, th, 1.0, -1.0) == 0.0      # extremum
+        assert o.limited_slope(1, th, 0.0, 1.0) == 0.0       # tie at zero -> 0
+        assert o.limited_slope(1, th, 0.7, 0.7) == pytest.approx(0.7, rel=1e-15)
+    assert o.limited_slope(2, 0, 1.0, 3.0) == pytest.approx(1.5)        # van Leer: harmonic mean
+    assert o.limited_slope(3, 0, 1.0, 3.0) == pytest.approx(12.0 / 10.0)  # van Albada
+    assert o.limited_slope(2, 0, 1.0, -3.0) == 0.0 and o.limited_slope(3, 0, -1.0, 3.0) == 0.0
+
+
+@pytest.mark.parametrize("recon", [PLM, PPM])
+def test_linear_data_reproduced_exactly(oracle_mod, recon):
+    a, b = 0.75, -0.125       # exactly representable
+    w = np.array([a + b * i for i in range(-2, 3)])
+    wm, wp = oracle_mod.face_values(recon, w)
+    assert wm == a - 0.5 * b and wp == a + 0.5 * b
+
+
+def test_ppm_interface_value_is_exact_for_cubic_cell_averages(oracle_mod):
+    """Colella & Woodward (1984) eq. 1.6 is fourth order: exact for cell averages of a cubic, when the
+    limiter is inactive (gentle monotone profile)."""
+    c0, c1, c2, c3 = 1.0, 0.5, 0.02, 0.003
+
+    def avg(i):   # cell average of the cubic over [i-1/2, i+1/2]
+        F = lambda x: c0 * x + c1 * x ** 2 / 2 + c2 * x ** 3 / 3 + c3 * x ** 4 / 4
+        return F(i + 0.5) - F(i - 0.5)
+
+    w = np.array([avg(i) for i in range(-2, 3)])
+    wm, wp = oracle_mod.face_values(PPM, w)
+    point = lambda x: c0 + c1 * x + c2 * x ** 2 + c3 * x ** 3
+    # the gen.-minmod(2) slope equals the centred difference here, which is what eq. 1.6 assumes
+    assert wp == pytest.approx(point(0.5), abs=2e-15 + 0.0)
+    assert wm == pytest.approx(point(-0.5), abs=2e-15 + 0.0)
+
+
+@pytest.mark.parametrize("recon", [PLM, PPM])
+def test_face_values_monotone_and_extrema_flattened(oracle_mod, recon):
+    rng = np.random.default_rng(5)
+    for _ in range(300):
+        w = np.sort(rng.uniform(0, 1, 5)) if rng.uniform() < 0.5 else rng.uniform(0, 1, 5)
+        wm, wp = oracle_mod.face_values(recon, w)
+        lo, hi = min(w[1], w[2], w[3]), max(w[1], w[2], w[3])
+        assert lo - 1e-15 <= wm <= hi + 1e-15 and lo - 1e-15 <= wp <= hi + 1e-15
+        if (w[3] - w[2]) * (w[2] - w[1]) <= 0:
+            assert wm == w[2] and wp == w[2]
+        # the parabola through (wm, w, wp) has no interior extremum
+        if recon == PPM:
+            d, w6 = wp - wm, 6 * (w[2] - 0.5 * (wm + wp))
+            assert abs(w6) <= abs(d) * (1 + 1e-12) + 1e-15
+
+
+def _eig(rho, vn, p, gamma):
+    c = math.sqrt(gamma * p / rho)
+    R = np.array([[1, -c / rho, 0, 0, c * c], [1, 0, 0, 0, 0], [0, 0, 1, 0, 0], [0, 0, 0, 1, 0],
+                  [1, c / rho, 0, 0, c * c]], dtype=float)
+    lam = np.array([vn - c, vn, vn, vn, vn + c])
+    return lam, R
+
+
+@pytest.mark.parametrize("recon", [PLM, PPM])
+def test_tracing_with_zero_dt_returns_untraced(oracle_mod, recon):
+    W = np.array([1.0, 0.3, -0.2, 0.1, 0.8])
+    wm, wp = W - np.array([0.05, 0.01, 0.02, -0.01, 0.03]), W + np.array([0.04, 0.01, 0.02, -0.01, 0.03])
+    tm, tp = oracle_mod.trace_cell(recon, 1.4, W, wm, wp, 0.0)
+    assert np.array_equal(tm, wm) and np.array_equal(tp, wp)
+
+
+@pytest.mark.parametrize("recon", [PLM, PPM])
+@pytest.mark.parametrize("vn", [0.3, -0.3, 2.5, -2.5])
+def test_single_wave_tracing_is_domain_of_dependence_average(oracle_mod, recon, vn):
+    """If the in-cell profile varies along ONE eigenvector r_a, the traced face state must be the
+    average of that profile over the wave's domain of dependence [face - lambda_a dt, face]
+    (Colella & Woodward 1984 eq. 1.12; Colella 1990) -- computed here by direct quadrature."""
+    gamma, lam_r = 5.0 / 3.0, 0.4
+    W = np.array([1.3, vn, 0.2, -0.1, 0.9])
+    lam, R = _eig(W[0], vn, W[4], gamma)
+    for a in range(5):
+        r = R[a]
+        if recon == PLM:
+            slope, curv = 0.02, 0.0
+        else:
+            slope, curv = 0.02, 0.006
+        # profile W(xi) = W + r * (slope*(xi-1/2) + curv*((xi-1/2)^2 - 1/12)), xi in [0,1]; mean = W
+        prof = lambda xi: slope * (xi - 0.5) + curv * ((xi - 0.5) ** 2 - 1.0 / 12.0)
+        wm, wp = W + r * prof(0.0), W + r * prof(1.0)
+        tm, tp = oracle_mod.trace_cell(recon, gamma, W, wm, wp, lam_r)
+        y = lam[a] * lam_r
+
+        def mean(x0, x1):
+            xs = np.linspace(x0, x1, 20001)
+            return np.trapezoid(prof(xs), xs) / (x1 - x0)
+
+        # A wave that does not move toward a face stays averaged over the reference domain (that of
+        # the fastest wave toward that face), as in Colella & Woodward's reference-state form.
+        yp = y if y > 0 else max(lam[4] * lam_r, 0.0)
+        ym = -y if y < 0 else max(-lam[0] * lam_r, 0.0)
+        exp_p = W + r * (mean(1.0 - yp, 1.0) if yp > 0 else prof(1.0))
+        exp_m = W + r * (mean(0.0, ym) if ym > 0 else prof(0.0))
+        assert np.allclose(tp, exp_p, atol=1e-10), (a, tp, exp_p)
+        assert np.allclose(tm, exp_m, atol=1e-10), (a, tm, exp_m)
