@@ -1,0 +1,274 @@
+"""Whole-step pins of the oracle (oracle/hydro_oracle.c): invariants and special cases that the
+paper and the mathematics fix.  CPU only."""
+import itertools
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from helpers import oracle_run, oracle_step
+from paper_1712_07070_b200 import inputs
+
+MHM, CTU = 1, 2
+PLM, PPM = 1, 2
+ROE, HLLC, HLLE = 1, 2, 3
+COMBOS = list(itertools.product((MHM, CTU), (PLM, PPM), (ROE, HLLC, HLLE)))
+G53 = 5.0 / 3.0
+
+
+def _turb(n=32, seed=1712, mach=1.0, entropy=False):
+    return inputs.turbulence_field(n, seed, kmax=4, gamma=G53, mach=mach, entropy=entropy)
+
+
+def _dt(oracle, field, dh, gamma, cfl, scheme, opts=None):
+    u = inputs.interior(inputs.pack_periodic(field)).contiguous().numpy()
+    return oracle.cfl_dt(u, dh, gamma, cfl, scheme, opts)[0]
+
+
+@pytest.mark.parametrize("scheme,recon,solver", COMBOS)
+def test_conservation_on_periodic_box(oracle_mod, scheme, recon, solver):
+    """conservation to machine precision (pure hydro, closed domain)."""
+    f = _turb()
+    dh = 1.0 / 32
+    dt = _dt(oracle_mod, f, dh, G53, 0.4, scheme)
+    new, r = oracle_step(oracle_mod, f, dt, dh, G53, scheme, recon, solver)
+    assert r["stats"]["n_unphysical"] == 0
+    for v in range(5):
+        s0, s1 = math.fsum(f[v].flatten().tolist()), math.fsum(new[v].flatten().tolist())
+        scale = math.fsum(f[v].abs().flatten().tolist()) + 1.0
+        assert abs(s1 - s0) <= 1e-13 * scale, (v, s0, s1)
+    assert (new - f).abs().max() > 1e-3       # and something did happen
+
+
+@pytest.mark.parametrize("scheme,recon,solver", [(MHM, PLM, ROE), (CTU, PPM, HLLC), (MHM, PPM, HLLE)])
+def test_boundary_fluxes_of_neighbouring_groups_are_bitwise_equal(oracle_mod, scheme, recon, solver):
+    """the flux through a face shared by two groups is computed twice and must agree
+    bit for bit; also the mid-plane (p=1) equals the difference form of the update."""
+    f = _turb()
+    dh = 1.0 / 32
+    dt = _dt(oracle_mod, f, dh, G53, 0.4, scheme)
+    _, r = oracle_step(oracle_mod, f, dt, dh, G53, scheme, recon, solver)
+    fl = r["flux"].reshape(2, 2, 2, 3, 3, 5, 16, 16)      # [gz,gy,gx,axis,plane,...]
+    for gz, gy, gx in itertools.product(range(2), repeat=3):
+        assert np.array_equal(fl[gz, gy, gx, 0, 2], fl[gz, gy, (gx + 1) % 2, 0, 0])
+        assert np.array_equal(fl[gz, gy, gx, 1, 2], fl[gz, (gy + 1) % 2, gx, 1, 0])
+        assert np.array_equal(fl[gz, gy, gx, 2, 2], fl[(gz + 1) % 2, gy, gx, 2, 0])
+
+
+@pytest.mark.parametrize("scheme,recon,solver", [(MHM, PLM, HLLE), (CTU, PLM, ROE)])
+def test_flux_out_reproduces_update_of_a_boundary_slab(oracle_mod, scheme, recon, solver):
+    """Sum over a half-group slab: d(sum U)/dt = -(flux through its faces)/dh.  With periodic y,z
+    sums over a whole x-slab [0,8) of the 32^3 box, only the x-planes 0 and 8 contribute."""
+    f = _turb()
+    dh = 1.0 / 32
+    dt = _dt(oracle_mod, f, dh, G53, 0.4, scheme)
+    new, r = oracle_step(oracle_mod, f, dt, dh, G53, scheme, recon, solver)
+    fl = r["flux"].reshape(2, 2, 2, 3, 3, 5, 16, 16)
+    for v in range(5):
+        dsum = (new[v, :, :, 0:8] - f[v, :, :, 0:8]).sum().item()
+        fin = fl[:, :, 0, 0, 0, v].sum()       # x-plane 0 of the gx=0 groups
+        fout = fl[:, :, 0, 0, 1, v].sum()      # x-plane 8
+        assert dsum == pytest.approx(-(dt / dh) * (fout - fin), rel=1e-9, abs=1e-11)
+
+
+@pytest.mark.parametrize("scheme,recon,solver", COMBOS)
+def test_uniform_state_is_bitwise_invariant(oracle_mod, scheme, recon, solver):
+    n = 16
+    one = torch.ones((n, n, n), dtype=torch.float64)
+    f = inputs.prim_to_cons(1.3 * one, 0.7 * one, -0.45 * one, 0.3 * one, 0.9 * one, G53)
+    new, _ = oracle_step(oracle_mod, f, 0.01, 1.0 / n, G53, scheme, recon, solver)
+    assert torch.equal(new, f)
+
+
+@pytest.mark.parametrize("scheme,recon,solver", COMBOS)
+def test_cyclic_permutation_symmetry(oracle_mod, scheme, recon, solver):
+    """Relabel the axes (x,y,z) -> (y,z,x): the solver must commute with it (<= 1e-13: the three-term
+    sums re-associate, so not bitwise)."""
+    f = _turb(seed=99)
+    dh, dt = 1.0 / 32, 0.004
+    new, _ = oracle_step(oracle_mod, f, dt, dh, G53, scheme, recon, solver)
+    # P: array [z,y,x] -> [x,z,y] i.e. the old x axis becomes the new z axis, old z -> new y, old y -> new x
+    def P(a):
+        b = a.permute(0, 3, 1, 2).contiguous()
+        # momentum: new (mx', my', mz') = components along new axes = old (my, mz, mx)
+        return torch.stack([b[0], b[2], b[3], b[1], b[4]], dim=0)
+    newP, _ = oracle_step(oracle_mod, P(f), dt, dh, G53, scheme, recon, solver)
+    ref = P(new)
+    assert (newP - ref).abs().max().item() <= 1e-13 * ref.abs().max().item()
+
+
+@pytest.mark.parametrize("scheme,recon,solver", [(MHM, PLM, ROE), (CTU, PPM, HLLC), (CTU, PLM, HLLE), (MHM, PPM, HLLC)])
+def test_mirror_symmetry(oracle_mod, scheme, recon, solver):
+    f = _turb(seed=5)
+    dh, dt = 1.0 / 32, 0.004
+    new, _ = oracle_step(oracle_mod, f, dt, dh, G53, scheme, recon, solver)
+    def M(a):
+        b = torch.flip(a, dims=[3]).clone()
+        b[1] = -b[1]
+        return b
+    newM, _ = oracle_step(oracle_mod, M(f), dt, dh, G53, scheme, recon, solver)
+    assert (newM - M(new)).abs().max().item() <= 1e-13 * new.abs().max().item()
+
+
+@pytest.mark.parametrize("scheme,recon,solver", COMBOS)
+def test_one_dimensional_data_stay_one_dimensional_bitwise(oracle_mod, scheme, recon, solver):
+    f = inputs.sod_field(32, 1.4)
+    new, _ = oracle_step(oracle_mod, f, 0.2 / 32, 1.0 / 32, 1.4, scheme, recon, solver)
+    assert torch.equal(new, new[:, :1, :1, :].expand_as(new))
+    assert new[2].abs().max() == 0 and new[3].abs().max() == 0
+
+
+def _minmod(a, b):
+    return np.where(a * b > 0, np.sign(a) * np.minimum(np.abs(a), np.abs(b)), 0.0)
+
+
+@pytest.mark.parametrize("scheme,solver", [(MHM, ROE), (MHM, HLLC), (CTU, ROE), (CTU, HLLC)])
+def test_contact_advection_reduces_to_second_order_upwind_advection(oracle_mod, scheme, solver):
+    """Uniform v and P, varying rho: the Euler system reduces to linear advection of rho.  Roe and
+    HLLC resolve a moving contact exactly, so MHM+PLM (and CTU+PLM in 1-D) must equal the textbook
+    second-order upwind (MUSCL/Fromm-type) scheme  rho_i - nu (r_{i+1/2} - r_{i-1/2}),
+    r_{i+1/2} = rho_i + (1-nu)/2 * minmod slope   (Toro 2009 sect. 13.4; van Leer 1979)."""
+    n = 32
+    x = (np.arange(n) + 0.5) / n
+    rho1 = 1.0 + 0.3 * np.sin(2 * np.pi * x) + 0.2 * (np.abs(x - 0.5) < 0.2)
+    rho = torch.from_numpy(rho1)[None, None, :].expand(16, 16, n).contiguous()
+    one = torch.ones_like(rho)
+    v = 0.8
+    f = inputs.prim_to_cons(rho, v * one, 0 * one, 0 * one, one, 1.4)
+    dh, dt = 1.0 / n, 0.3 / n / v * 1.0
+    nu = v * dt / dh
+    new, _ = oracle_step(oracle_mod, f, dt, dh, 1.4, scheme, PLM, solver)
+    s = _minmod(rho1 - np.roll(rho1, 1), np.roll(rho1, -1) - rho1)
+    face = rho1 + 0.5 * (1 - nu) * s
+    ref = rho1 - nu * (face - np.roll(face, 1))
+    assert np.abs(new[0, 3, 5].numpy() - ref).max() <= 2e-14
+    # velocity and pressure stay uniform
+    assert np.abs(new[1, 3, 5].numpy() / new[0, 3, 5].numpy() - v).max() <= 1e-13
+
+
+def test_mhm_three_d_contact_advection_closed_form(oracle_mod):
+    """Same reduction in 3-D for the unsplit MUSCL-Hancock scheme: the half-step predictor adds
+    -(1/2) sum_d nu_d slope_d to every face value (Toro 2009 sect. 16.5)."""
+    n = 16
+    f0 = inputs.blob_field(n, G53, v=(0.9, -0.6, 0.4))
+    rho = f0[0].numpy()
+    vel = (0.9, -0.6, 0.4)
+    dh, dt = 1.0 / n, 0.25 / n
+    new, _ = oracle_step(oracle_mod, f0, dt, dh, G53, MHM, PLM, HLLC)
+    ax = {0: 2, 1: 1, 2: 0}      # direction -> array axis
+    slopes = {d: _minmod(rho - np.roll(rho, 1, ax[d]), np.roll(rho, -1, ax[d]) - rho) for d in range(3)}
+    half = -0.5 * sum(vel[d] * dt / dh * slopes[d] for d in range(3))
+    ref = rho.copy()
+    for d in range(3):
+        nu = vel[d] * dt / dh
+        if vel[d] > 0:
+            face = rho + 0.5 * slopes[d] + half                 # value at i+1/2 from cell i
+            ref -= nu * (face - np.roll(face, 1, ax[d]))
+        else:
+            face = rho - 0.5 * slopes[d] + half                 # value at i-1/2 from cell i
+            ref -= nu * (np.roll(face, -1, ax[d]) - face)
+    assert np.abs(new[0].numpy() - ref).max() <= 5e-14
+
+
+@pytest.mark.parametrize("recon", [PLM, PPM])
+def test_ctu_one_d_contact_advection_uses_domain_of_dependence_average(oracle_mod, recon):
+    """CTU in 1-D: the face value is the average of the reconstructed profile over [x_f - v dt, x_f]
+    (Colella 1990).  For PPM the profile is the monotonised parabola, integrated here in closed form
+    from the oracle's own (separately pinned) face values."""
+    n = 32
+    x = (np.arange(n) + 0.5) / n
+    rho1 = 1.0 + 0.3 * np.sin(2 * np.pi * x) + 0.1 * np.sin(6 * np.pi * x)
+    rho = torch.from_numpy(rho1)[None, None, :].expand(16, 16, n).contiguous()
+    one = torch.ones_like(rho)
+    v = 0.7
+    f = inputs.prim_to_cons(rho, v * one, 0 * one, 0 * one, one, 1.4)
+    dh, dt = 1.0 / n, 0.4 / n
+    nu = v * dt / dh
+    new, _ = oracle_step(oracle_mod, f, dt, dh, 1.4, CTU, recon, HLLC)
+    face = np.empty(n)
+    for i in range(n):
+        w5 = np.array([rho1[(i + m) % n] for m in range(-2, 3)])
+        wm, wp = oracle_mod.face_values(recon, w5)
+        d, w6 = wp - wm, (6 * (rho1[i] - 0.5 * (wm + wp)) if recon == PPM else 0.0)
+        face[i] = wp - 0.5 * nu * (d - (1 - 2.0 / 3.0 * nu) * w6)
+    ref = rho1 - nu * (face - np.roll(face, 1))
+    assert np.abs(new[0, 2, 7].numpy() - ref).max() <= 2e-14
+
+
+@pytest.mark.parametrize("scheme,recon,solver", COMBOS)
+def test_sod_converges_to_exact_solution(oracle_mod, scheme, recon, solver):
+    """BASELINE.json config 1 data; exact solution from Toro's iterative procedure (tests/exact_riemann.py,
+    itself pinned to the printed values in tests/golden/sod_exact.txt).  The periodic wrap adds a
+    mirrored tube at x=0; until t=0.12 the two wave fans do not meet."""
+    import exact_riemann as er
+    t_end, gamma = 0.12, 1.4
+    errs = []
+    for n in (64, 128):
+        f = inputs.sod_field(n, gamma, nyz=16)
+        cfl = 0.4 if scheme == CTU else 0.8
+        out, nsteps = oracle_run(oracle_mod, f, t_end, 1.0 / n, gamma, cfl, scheme, recon, solver)
+        x = (np.arange(n) + 0.5) / n
+        rho_ex = np.empty(n)
+        mid = (x > 0.25) & (x < 0.75)
+        rho_ex[mid] = er.sample(1, 0, 1, 0.125, 0, 0.1, gamma, (x[mid] - 0.5) / t_end)[0]
+        xs = np.where(x[~mid] > 0.5, x[~mid] - 1.0, x[~mid])
+        rho_ex[~mid] = er.sample(0.125, 0, 0.1, 1, 0, 1, gamma, xs / t_end)[0]
+        rho = out[0, 3, 4].numpy()
+        errs.append(np.abs(rho - rho_ex).mean())
+        if n == 128:
+            # plateaus between tail/contact and contact/shock, within 2 % at N=128
+            ps, us = er.star_state(1, 0, 1, 0.125, 0, 0.1, gamma)
+            xl = 0.5 + 0.5 * (-0.0702728126 + us) * t_end
+            xr = 0.5 + 0.5 * (us + 1.7521557320) * t_end
+            assert rho[int(xl * n)] == pytest.approx(0.4263194282, rel=0.02)
+            assert rho[int(xr * n)] == pytest.approx(0.2655737117, rel=0.02)
+    order = math.log(errs[0] / errs[1], 2.0)
+    assert errs[1] < 1.2e-2 and order >= 0.7, (errs, order)
+
+
+@pytest.mark.parametrize("scheme,recon,cfl", [(MHM, PLM, 1.0), (MHM, PPM, 1.0), (CTU, PLM, 0.5), (CTU, PPM, 0.5)])
+def test_stable_at_the_stated_cfl_limit(oracle_mod, scheme, recon, cfl):
+    """CTU needs C_CFL <= 0.5, the others support C_CFL <= 1.0 (with their own Eq. 1 / 2)."""
+    f = inputs.blob_field(16, G53)
+    lo, hi = f[0].min().item(), f[0].max().item()
+    out, n = oracle_run(oracle_mod, f, 1e9, 1.0 / 16, G53, cfl, scheme, recon, HLLC, max_steps=60)
+    assert n == 60 and torch.isfinite(out).all()
+    assert out[0].min().item() >= lo - 0.02 and out[0].max().item() <= hi + 0.02
+
+
+@pytest.mark.parametrize("scheme,recon", [(MHM, PLM), (CTU, PLM), (MHM, PPM), (CTU, PPM)])
+def test_ghost_footprint(oracle_mod, scheme, recon):
+    """CTU+PPM needs 3 ghost zones.  PLM variants must ignore ghost layer 3; no variant
+    reads the triple-corner ghosts; PPM must read layer 3."""
+    f = _turb(n=16, seed=3)
+    p = inputs.pack_periodic(f).numpy()
+    dt, dh = 0.002, 1.0 / 16
+    base = oracle_mod.fluid_advance(p, dt, dh, G53, scheme, recon, HLLC)
+    q = p.copy()
+    outer = np.ones((22, 22, 22), dtype=bool)
+    outer[1:21, 1:21, 1:21] = False
+    q[:, :, outer] *= 1.5                      # outermost ghost layer (layer 3)
+    r = oracle_mod.fluid_advance(q, dt, dh, G53, scheme, recon, HLLC)
+    same = np.array_equal(r["out"], base["out"]) and np.array_equal(r["flux"], base["flux"])
+    assert same == (recon == PLM)
+    q = p.copy()
+    idx = np.arange(22)
+    gh = (idx < 3) | (idx >= 19)
+    corner = gh[:, None, None] & gh[None, :, None] & gh[None, None, :]
+    q[:, :, corner] *= 1.5
+    r = oracle_mod.fluid_advance(q, dt, dh, G53, scheme, recon, HLLC)
+    assert np.array_equal(r["out"], base["out"]) and np.array_equal(r["flux"], base["flux"])
+
+
+def test_riemann_solves_per_cell(oracle_mod):
+    """PAPER.md L90 / L521: MHM needs 3 and CTU 6 Riemann solves per cell.  Per group the final pass is
+    3*17*16*16 faces (3/cell once shared faces are counted once); CTU adds the first pass on the
+    faces of the cells [-1,16]^3."""
+    p = inputs.pack_periodic(_turb(n=16)).numpy()
+    a = oracle_mod.fluid_advance(p, 0.002, 1.0 / 16, G53, MHM, PLM, HLLC)["stats"]
+    b = oracle_mod.fluid_advance(p, 0.002, 1.0 / 16, G53, CTU, PLM, HLLC)["stats"]
+    assert a["n_riemann"] == a["n_riemann_final"] == 3 * 17 * 16 * 16
+    assert 3 * 16 ** 3 * 16 // 17 <= 3 * 16 ** 3                      # shared faces: 16 of 17 unique
+    assert b["n_riemann_final"] == 3 * 17 * 16 * 16
+    assert b["n_riemann"] - b["n_riemann_final"] == 3 * 17 * 18 * 18
