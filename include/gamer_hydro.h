@@ -1,0 +1,124 @@
+/*
+ * gamer_hydro.h -- C ABI of the B200-native batched patch-group hydrodynamic solver
+ * (the data-parallel hot path of GAMER-2, arXiv 1712.07070; PAPER.md = the paper's text).
+ *
+ * One call advances a batch of AMR patch groups (8 sibling patches of 8^3 cells
+ * = 16^3 cells), each padded with 3 ghost zones per side (L300), by one step of an unsplit
+ * Godunov scheme for the ideal-gas Euler equations (section 2.2): MUSCL-Hancock (MHM)
+ * or corner-transport-upwind (CTU, 6 Riemann solves per cell), PLM or PPM reconstruction on
+ * primitive variables, Roe / HLLC / HLLE Riemann solver, conservative update.  It also emits
+ * the patch-boundary fluxes the AMR flux fix-up needs (L112) and the per-group CFL maximum
+ * (Eqs. 1-2; the paper computes time-steps on the GPU too, L240).
+ *
+ * All work runs in hand-written sm_100a CUDA kernels; there is no CPU fallback.  Every entry
+ * point returns 0 on success or a negative GAMER_E* code, never throws, never aborts, and
+ * (except the *_host entry) never synchronises: work is enqueued on the given stream.
+ *
+ * Layouts (x fastest; real = float or double as selected by `precision`):
+ *   in        [n_groups][NVAR][22][22][22]   conserved (rho, mx, my, mz, E [, s]); cell (i,j,k) of
+ *                                            the group is padded cell (i+3, j+3, k+3)
+ *   out       [n_groups][NVAR][16][16][16]
+ *   flux_out  [n_groups][3 axes][3 planes][NVAR][16][16]   plane p of axis d = the cell face at
+ *             index 8p of that axis (faces of the 8^3 patches); the two 16-long dims are the two
+ *             other axes, the lower-numbered axis fastest (x-faces: [z][y]; y: [z][x]; z: [y][x]).
+ *             Values are the time-centred flux densities F_d, not multiplied by dt or area.
+ *   group_speed_out [n_groups]   max over the 16^3 UPDATED cells of |vx|+|vy|+|vz|+3c (MHM, Eq. 2)
+ *                                or max(|vx|,|vy|,|vz|)+c (CTU, Eq. 1)
+ *   NVAR = 5 + n_scalar (n_scalar = 1 carries the entropy s = P/rho^(gamma-1) of L100).
+ * Ownership: every pointer is a DEVICE pointer owned by the caller, 16-byte aligned and
+ * non-overlapping, unless the name ends in _host.  The library keeps no state between calls.
+ */
+#ifndef GAMER_HYDRO_H
+#define GAMER_HYDRO_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { GAMER_MHM = 1, GAMER_CTU = 2 };                      /* scheme   (L90)            */
+enum { GAMER_PLM = 1, GAMER_PPM = 2 };                      /* recon    (L94)            */
+enum { GAMER_ROE = 1, GAMER_HLLC = 2, GAMER_HLLE = 3 };     /* riemann  (L94)            */
+enum { GAMER_FP32 = 4, GAMER_FP64 = 8 };                    /* precision = sizeof(real), L244 */
+enum { GAMER_LIMITER_GMINMOD = 1, GAMER_LIMITER_VANLEER = 2, GAMER_LIMITER_VANALBADA = 3 }; /* L94 */
+
+enum {
+    GAMER_OK = 0,
+    GAMER_EINVAL = -1,        /* NULL in/out, n_groups < 0, dt <= 0 or non-finite, dh <= 0, gamma <= 1,
+                                 unknown enum, misaligned pointer                                  */
+    GAMER_EUNSUPPORTED = -2,  /* valid arguments, combination not built                            */
+    GAMER_ECUDA = -3          /* CUDA runtime / launch error (cudaGetLastError)                    */
+};
+
+/* Everything the 11-argument form fixes by default.  Zero-initialise, then set what you need. */
+typedef struct gamer_opts {
+    void*    stream;              /* cudaStream_t; NULL = default stream                            */
+    int      limiter;             /* GAMER_LIMITER_*; 0 = generalized minmod                        */
+    double   minmod_theta;        /* <= 0: 1 for PLM (plain minmod), 2 for PPM (Colella-Woodward)   */
+    int      n_scalar;            /* 0 | 1                                                          */
+    int      dual_energy;         /* 0 | 1 (needs n_scalar = 1): L100                               */
+    double   de_xi;               /* switch E_the/E_kin < xi; <= 0: 1e-2                            */
+    double   min_dens, min_pres, min_temp;   /* floors, 0 = off; temperature = P/rho (L504)         */
+    int      remedy_first_order;  /* 1: remedy (ii) of L105 on cells that come out unphysical       */
+    const double* dt_dev;         /* nullable device double: if set, dt is read from it on device   */
+    void*    group_speed_out;     /* nullable real[n_groups]                                        */
+    int32_t* n_unphysical_out;    /* nullable device int: cells still unphysical after the remedies;
+                                     the caller applies remedy (iv) (retry with 0.8 dt, L107)       */
+    int32_t* diag_out;            /* nullable device int[4], set by the call: {remedy (i) faces,
+                                     reverted predictor states, remedy (ii) cells, dual-energy fixes} */
+} gamer_opts;
+
+/* One step for n_groups patch groups.  flux_out may be NULL.  n_groups == 0 is a successful no-op.
+ * Defaults: gen. minmod (theta 1 for PLM, 2 for PPM), primitive-variable reconstruction, no scalar,
+ * no dual energy, no floors, remedy (i) (Roe -> HLLE on faces whose intermediate states are
+ * unphysical, L104) on, remedy (ii) off. */
+int gamer_fluid_advance(const void* in, void* out, void* flux_out, int64_t n_groups,
+                        double dt, double dh, double gamma,
+                        int scheme, int recon, int riemann, int precision);
+
+int gamer_fluid_advance_ex(const void* in, void* out, void* flux_out, int64_t n_groups,
+                           double dt, double dh, double gamma,
+                           int scheme, int recon, int riemann, int precision,
+                           const gamer_opts* opts);
+
+/* CFL time-step of an UNPADDED state u (the `out` layout): Eq. (2) for MHM, Eq. (1) for CTU.
+ * *dt_out (device double) = cfl * dh / max speed.  group_speed_out nullable.
+ * The _ex form takes stream, n_scalar and the floors from opts (others ignored). */
+int gamer_cfl_dt(const void* u, int64_t n_groups, double dh, double gamma, double cfl,
+                 int scheme, int precision, void* group_speed_out, double* dt_out);
+int gamer_cfl_dt_ex(const void* u, int64_t n_groups, double dh, double gamma, double cfl,
+                    int scheme, int precision, void* group_speed_out, double* dt_out,
+                    const gamer_opts* opts);
+
+/* dt from the per-group maxima that gamer_fluid_advance_ex already produced (fused A8 row):
+ * *dt_out = cfl * dh / max_g group_speed[g]. */
+int gamer_cfl_from_group_speed(const void* group_speed, int64_t n_groups, double dh, double cfl,
+                               int precision, double* dt_out, void* stream);
+
+/* Same-level ghost refresh on the device for a periodic box of gz x gy x gx patch groups
+ * (g = (z*gy + y)*gx + x): builds the padded `in` batch from the unpadded `u` batch (the paper's
+ * CPU "preparation" step for sibling copies, L248).  u and in must not overlap. */
+int gamer_refresh_ghosts_periodic(const void* u, void* in, int gz, int gy, int gx, int nvar,
+                                  int precision, void* stream);
+
+/* End-to-end form with HOST buffers (pinned or pageable): copies `in` to the device in chunks,
+ * runs the solver, copies `out`, `flux_out` (nullable) and `group_speed_out` (nullable) back,
+ * overlapping copies and kernels on internal streams as the paper does with CUDA streams (L242),
+ * and synchronises before returning.  Device scratch is allocated and freed inside the call. */
+int gamer_fluid_advance_host(const void* in_host, void* out_host, void* flux_out_host,
+                             void* group_speed_out_host, int64_t n_groups,
+                             double dt, double dh, double gamma,
+                             int scheme, int recon, int riemann, int precision,
+                             const gamer_opts* opts /* nullable; device pointers inside are ignored */);
+
+/* Number of kernel launches the library has issued in this process (all entry points). */
+int64_t gamer_launch_count(void);
+
+const char* gamer_strerror(int code);
+int gamer_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GAMER_HYDRO_H */

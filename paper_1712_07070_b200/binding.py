@@ -1,0 +1,183 @@
+"""Thin ctypes binding of the C ABI in include/gamer_hydro.h -- argument marshalling only.
+
+Every function has the name of the C entry point it calls; torch tensors provide device memory and
+streams, nothing else.  The library is loaded lazily and loading fails loudly: there is no CPU or
+PyTorch fallback for any step of the path.
+"""
+import ctypes
+import os
+
+import torch
+
+MHM, CTU = 1, 2
+PLM, PPM = 1, 2
+ROE, HLLC, HLLE = 1, 2, 3
+FP32, FP64 = 4, 8
+GMINMOD, VANLEER, VANALBADA = 1, 2, 3
+PS, NG, NP = 16, 3, 22
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgamerhydro.so")
+
+EXPORTS = ["gamer_fluid_advance", "gamer_fluid_advance_ex", "gamer_cfl_dt", "gamer_cfl_dt_ex",
+           "gamer_cfl_from_group_speed", "gamer_refresh_ghosts_periodic", "gamer_fluid_advance_host",
+           "gamer_launch_count", "gamer_strerror", "gamer_version"]
+
+
+class gamer_opts(ctypes.Structure):
+    _fields_ = [
+        ("stream", ctypes.c_void_p),
+        ("limiter", ctypes.c_int),
+        ("minmod_theta", ctypes.c_double),
+        ("n_scalar", ctypes.c_int),
+        ("dual_energy", ctypes.c_int),
+        ("de_xi", ctypes.c_double),
+        ("min_dens", ctypes.c_double),
+        ("min_pres", ctypes.c_double),
+        ("min_temp", ctypes.c_double),
+        ("remedy_first_order", ctypes.c_int),
+        ("dt_dev", ctypes.c_void_p),
+        ("group_speed_out", ctypes.c_void_p),
+        ("n_unphysical_out", ctypes.c_void_p),
+        ("diag_out", ctypes.c_void_p),
+    ]
+
+
+class GamerError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def lib():
+    """Load libgamerhydro.so (built in-tree by paper_1712_07070_b200.build).  Raises if missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise GamerError(f"{LIB_PATH} is missing: run `python -m paper_1712_07070_b200.build` "
+                             "(there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        i64, dbl, vp, ci = ctypes.c_int64, ctypes.c_double, ctypes.c_void_p, ctypes.c_int
+        adv = [vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, ci, ci]
+        L.gamer_fluid_advance.argtypes = adv
+        L.gamer_fluid_advance_ex.argtypes = adv + [ctypes.POINTER(gamer_opts)]
+        cfl = [vp, i64, dbl, dbl, dbl, ci, ci, vp, vp]
+        L.gamer_cfl_dt.argtypes = cfl
+        L.gamer_cfl_dt_ex.argtypes = cfl + [ctypes.POINTER(gamer_opts)]
+        L.gamer_cfl_from_group_speed.argtypes = [vp, i64, dbl, dbl, ci, vp, vp]
+        L.gamer_refresh_ghosts_periodic.argtypes = [vp, vp, ci, ci, ci, ci, ci, vp]
+        L.gamer_fluid_advance_host.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, ci, ci,
+                                               ctypes.POINTER(gamer_opts)]
+        L.gamer_launch_count.restype = ctypes.c_int64
+        L.gamer_strerror.restype = ctypes.c_char_p
+        L.gamer_strerror.argtypes = [ci]
+        _lib = L
+    return _lib
+
+
+def _check(rc, what):
+    if rc != 0:
+        raise GamerError(f"{what} failed: {rc} ({lib().gamer_strerror(rc).decode()})")
+
+
+def _precision(t):
+    if t.dtype == torch.float32:
+        return FP32
+    if t.dtype == torch.float64:
+        return FP64
+    raise GamerError(f"unsupported dtype {t.dtype}")
+
+
+def _ptr(t, device_type="cuda"):
+    if t is None:
+        return None
+    if t.device.type != device_type:
+        raise GamerError(f"expected a {device_type} tensor, got {t.device}")
+    if not t.is_contiguous():
+        raise GamerError("tensor must be contiguous")
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def _stream_handle(stream=None):
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+def make_opts(stream=None, limiter=0, minmod_theta=0.0, n_scalar=0, dual_energy=False, de_xi=0.0, min_dens=0.0,
+              min_pres=0.0, min_temp=0.0, remedy_first_order=False, dt_dev=None, group_speed_out=None,
+              n_unphysical_out=None, diag_out=None, on_device=True):
+    o = gamer_opts()
+    o.stream = _stream_handle(stream) if on_device else None
+    o.limiter, o.minmod_theta, o.n_scalar = int(limiter), float(minmod_theta), int(n_scalar)
+    o.dual_energy, o.de_xi = int(bool(dual_energy)), float(de_xi)
+    o.min_dens, o.min_pres, o.min_temp = float(min_dens), float(min_pres), float(min_temp)
+    o.remedy_first_order = int(bool(remedy_first_order))
+    o.dt_dev = _ptr(dt_dev)
+    o.group_speed_out = _ptr(group_speed_out)
+    o.n_unphysical_out = _ptr(n_unphysical_out)
+    o.diag_out = _ptr(diag_out)
+    return o
+
+
+def gamer_fluid_advance(u_in, out, flux_out, dt, dh, gamma, scheme, recon, riemann):
+    """11-argument form.  NOTE: runs on the default stream, as the C ABI states."""
+    n = u_in.shape[0]
+    _check(lib().gamer_fluid_advance(_ptr(u_in), _ptr(out), _ptr(flux_out), n, float(dt), float(dh), float(gamma),
+                                     int(scheme), int(recon), int(riemann), _precision(u_in)), "gamer_fluid_advance")
+
+
+def gamer_fluid_advance_ex(u_in, out, flux_out, dt, dh, gamma, scheme, recon, riemann, opts):
+    n = u_in.shape[0]
+    _check(lib().gamer_fluid_advance_ex(_ptr(u_in), _ptr(out), _ptr(flux_out), n, float(dt), float(dh), float(gamma),
+                                        int(scheme), int(recon), int(riemann), _precision(u_in), ctypes.byref(opts)),
+           "gamer_fluid_advance_ex")
+
+
+def gamer_cfl_dt(u, dh, gamma, cfl, scheme, group_speed_out, dt_out, opts=None):
+    n = u.shape[0]
+    if opts is None:
+        opts = make_opts(n_scalar=u.shape[1] - 5)
+    _check(lib().gamer_cfl_dt_ex(_ptr(u), n, float(dh), float(gamma), float(cfl), int(scheme), _precision(u),
+                                 _ptr(group_speed_out), _ptr(dt_out), ctypes.byref(opts)), "gamer_cfl_dt_ex")
+
+
+def gamer_cfl_from_group_speed(group_speed, dh, cfl, dt_out, stream=None):
+    _check(lib().gamer_cfl_from_group_speed(_ptr(group_speed), group_speed.shape[0], float(dh), float(cfl),
+                                            _precision(group_speed), _ptr(dt_out), _stream_handle(stream)),
+           "gamer_cfl_from_group_speed")
+
+
+def gamer_refresh_ghosts_periodic(u, u_in, gz, gy, gx, stream=None):
+    _check(lib().gamer_refresh_ghosts_periodic(_ptr(u), _ptr(u_in), gz, gy, gx, u.shape[1], _precision(u),
+                                               _stream_handle(stream)), "gamer_refresh_ghosts_periodic")
+
+
+def gamer_fluid_advance_host(in_host, out_host, flux_out_host, group_speed_out_host, dt, dh, gamma, scheme, recon,
+                             riemann, opts=None):
+    """Host-buffer entry: tensors live on the CPU (pinned preferably); copies happen inside the call."""
+    n = in_host.shape[0]
+    if opts is None:
+        opts = make_opts(on_device=False)
+    _check(lib().gamer_fluid_advance_host(_ptr(in_host, "cpu"), _ptr(out_host, "cpu"), _ptr(flux_out_host, "cpu"),
+                                          _ptr(group_speed_out_host, "cpu"), n, float(dt), float(dh), float(gamma),
+                                          int(scheme), int(recon), int(riemann), _precision(in_host),
+                                          ctypes.byref(opts)), "gamer_fluid_advance_host")
+
+
+def gamer_launch_count():
+    return int(lib().gamer_launch_count())
+
+
+def gamer_version():
+    return int(lib().gamer_version())
+
+
+# ---------------------------------------------------------------------------------------- allocation helpers
+def alloc_outputs(u_in, want_flux=True, want_speed=True):
+    """Device buffers of the right shapes for a padded batch [G, NV, 22,22,22]."""
+    g, nv = u_in.shape[:2]
+    out = torch.empty((g, nv, PS, PS, PS), dtype=u_in.dtype, device=u_in.device)
+    flux = torch.empty((g, 3, 3, nv, PS, PS), dtype=u_in.dtype, device=u_in.device) if want_flux else None
+    speed = torch.empty((g,), dtype=u_in.dtype, device=u_in.device) if want_speed else None
+    return out, flux, speed

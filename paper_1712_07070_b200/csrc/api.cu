@@ -1,0 +1,249 @@
+// api.cu -- the C ABI of include/gamer_hydro.h: argument validation, dispatch over
+// (scheme, recon, riemann, precision), auxiliary kernels, and the host-buffer entry.
+#include <atomic>
+#include <cmath>
+#include <cstring>
+
+#include "../../include/gamer_hydro.h"
+#include "aux_kernels.cuh"
+
+namespace gamer {
+#define G_DECL(s, r, v) cudaError_t gamer_launch_##s##_##r##_##v(int, int, int, const void*, cudaStream_t, int*);
+G_DECL(1, 1, 1) G_DECL(1, 1, 2) G_DECL(1, 1, 3) G_DECL(1, 2, 1) G_DECL(1, 2, 2) G_DECL(1, 2, 3)
+G_DECL(2, 1, 1) G_DECL(2, 1, 2) G_DECL(2, 1, 3) G_DECL(2, 2, 1) G_DECL(2, 2, 2) G_DECL(2, 2, 3)
+#undef G_DECL
+typedef cudaError_t (*launch_fn)(int, int, int, const void*, cudaStream_t, int*);
+static const launch_fn TABLE[2][2][3] = {
+    {{gamer_launch_1_1_1, gamer_launch_1_1_2, gamer_launch_1_1_3}, {gamer_launch_1_2_1, gamer_launch_1_2_2, gamer_launch_1_2_3}},
+    {{gamer_launch_2_1_1, gamer_launch_2_1_2, gamer_launch_2_1_3}, {gamer_launch_2_2_1, gamer_launch_2_2_2, gamer_launch_2_2_3}}};
+static std::atomic<long long> g_launches{0};
+}  // namespace gamer
+
+using namespace gamer;
+
+static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+static int check_common(const void* in, const void* out, int64_t n_groups, double dh, double gamma, int scheme,
+                        int recon, int riemann, int precision) {
+    if (n_groups < 0 || (n_groups > 0 && (!in || !out))) return GAMER_EINVAL;
+    if (!(dh > 0.0) || !std::isfinite(dh) || !(gamma > 1.0) || !std::isfinite(gamma)) return GAMER_EINVAL;
+    if (scheme != GAMER_MHM && scheme != GAMER_CTU) return GAMER_EINVAL;
+    if (recon != GAMER_PLM && recon != GAMER_PPM) return GAMER_EINVAL;
+    if (riemann < GAMER_ROE || riemann > GAMER_HLLE) return GAMER_EINVAL;
+    if (precision != GAMER_FP32 && precision != GAMER_FP64) return GAMER_EINVAL;
+    if (!aligned16(in) || !aligned16(out)) return GAMER_EINVAL;
+    return GAMER_OK;
+}
+
+template <typename T>
+static int advance_typed(const void* in, void* out, void* flux_out, int64_t n_groups, double dt, double dh,
+                         double gamma, int scheme, int recon, int riemann, const gamer_opts* o) {
+    AdvArgs<T> a;
+    std::memset(&a, 0, sizeof(a));
+    a.in = static_cast<const T*>(in);
+    a.out = static_cast<T*>(out);
+    a.flux = static_cast<T*>(flux_out);
+    a.dt = dt; a.dh = dh; a.gamma = gamma;
+    a.n_groups = n_groups;
+    a.limiter = LIM_GMINMOD;
+    a.theta = recon == GAMER_PPM ? 2.0 : 1.0;
+    a.xi = 1e-2;
+    cudaStream_t st = nullptr;
+    int nsc = 0, ext = 0;
+    if (o) {
+        st = static_cast<cudaStream_t>(o->stream);
+        if (o->limiter != 0) a.limiter = o->limiter;
+        if (o->minmod_theta > 0.0) a.theta = o->minmod_theta;
+        if (o->de_xi > 0.0) a.xi = o->de_xi;
+        a.min_dens = o->min_dens; a.min_pres = o->min_pres; a.min_temp = o->min_temp;
+        a.dual = o->dual_energy; a.remedy2 = o->remedy_first_order;
+        a.dt_dev = o->dt_dev;
+        a.speed = static_cast<T*>(o->group_speed_out);
+        a.n_unphys = o->n_unphysical_out;
+        a.diag = o->diag_out;
+        nsc = o->n_scalar;
+        ext = (nsc || a.dual || a.remedy2 || a.limiter != LIM_GMINMOD || a.min_dens > 0 || a.min_pres > 0 ||
+               a.min_temp > 0 || a.n_unphys || a.diag) ? 1 : 0;
+    }
+    if (a.n_unphys && cudaMemsetAsync(a.n_unphys, 0, sizeof(int), st) != cudaSuccess) return GAMER_ECUDA;
+    if (a.diag && cudaMemsetAsync(a.diag, 0, 4 * sizeof(int), st) != cudaSuccess) return GAMER_ECUDA;
+    if (n_groups == 0) return GAMER_OK;
+    int launches = 0;
+    const cudaError_t e = TABLE[scheme - 1][recon - 1][riemann - 1](sizeof(T), nsc, ext, &a, st, &launches);
+    g_launches += launches;
+    return e == cudaSuccess ? GAMER_OK : GAMER_ECUDA;
+}
+
+extern "C" int gamer_fluid_advance_ex(const void* in, void* out, void* flux_out, int64_t n_groups, double dt,
+                                      double dh, double gamma, int scheme, int recon, int riemann, int precision,
+                                      const gamer_opts* opts) {
+    int rc = check_common(in, out, n_groups, dh, gamma, scheme, recon, riemann, precision);
+    if (rc) return rc;
+    const bool dev_dt = opts && opts->dt_dev;
+    if (!dev_dt && (!(dt > 0.0) || !std::isfinite(dt))) return GAMER_EINVAL;
+    if (flux_out && !aligned16(flux_out)) return GAMER_EINVAL;
+    if (opts) {
+        if (opts->n_scalar < 0 || opts->n_scalar > 1) return GAMER_EINVAL;
+        if (opts->dual_energy && opts->n_scalar != 1) return GAMER_EINVAL;
+        if (opts->limiter < 0 || opts->limiter > GAMER_LIMITER_VANALBADA) return GAMER_EINVAL;
+        if (opts->min_dens < 0 || opts->min_pres < 0 || opts->min_temp < 0) return GAMER_EINVAL;
+    }
+    if (n_groups > 0x3fffffff) return GAMER_EUNSUPPORTED;
+    return precision == GAMER_FP32
+               ? advance_typed<float>(in, out, flux_out, n_groups, dt, dh, gamma, scheme, recon, riemann, opts)
+               : advance_typed<double>(in, out, flux_out, n_groups, dt, dh, gamma, scheme, recon, riemann, opts);
+}
+
+extern "C" int gamer_fluid_advance(const void* in, void* out, void* flux_out, int64_t n_groups, double dt, double dh,
+                                   double gamma, int scheme, int recon, int riemann, int precision) {
+    return gamer_fluid_advance_ex(in, out, flux_out, n_groups, dt, dh, gamma, scheme, recon, riemann, precision,
+                                  nullptr);
+}
+
+// ------------------------------------------------------------------------------------------ CFL
+template <typename T>
+static int cfl_typed(const void* u, int64_t n_groups, double dh, double gamma, double cfl, int scheme,
+                     void* group_speed_out, double* dt_out, const gamer_opts* o) {
+    cudaStream_t st = o ? static_cast<cudaStream_t>(o->stream) : nullptr;
+    CflArgs<T> a;
+    a.u = static_cast<const T*>(u);
+    a.speed = static_cast<T*>(group_speed_out);
+    a.acc = dt_out;
+    a.gamma = gamma;
+    a.min_dens = o ? o->min_dens : 0.0; a.min_pres = o ? o->min_pres : 0.0; a.min_temp = o ? o->min_temp : 0.0;
+    a.n_groups = n_groups;
+    const int nsc = o ? o->n_scalar : 0;
+    if (cudaMemsetAsync(dt_out, 0, sizeof(double), st) != cudaSuccess) return GAMER_ECUDA;
+    if (n_groups > 0) {
+        const unsigned grid = (unsigned)n_groups;
+        if (scheme == GAMER_MHM) {
+            if (nsc) cfl_kernel<T, 6, MHM><<<grid, 256, 0, st>>>(a); else cfl_kernel<T, 5, MHM><<<grid, 256, 0, st>>>(a);
+        } else {
+            if (nsc) cfl_kernel<T, 6, CTU><<<grid, 256, 0, st>>>(a); else cfl_kernel<T, 5, CTU><<<grid, 256, 0, st>>>(a);
+        }
+        g_launches += 1;
+    }
+    finish_dt_kernel<<<1, 1, 0, st>>>(dt_out, cfl * dh);
+    g_launches += 1;
+    return cudaGetLastError() == cudaSuccess ? GAMER_OK : GAMER_ECUDA;
+}
+
+extern "C" int gamer_cfl_dt_ex(const void* u, int64_t n_groups, double dh, double gamma, double cfl, int scheme,
+                               int precision, void* group_speed_out, double* dt_out, const gamer_opts* opts) {
+    if (!u || !dt_out || n_groups < 0 || !(dh > 0.0) || !(gamma > 1.0) || !(cfl > 0.0)) return GAMER_EINVAL;
+    if (scheme != GAMER_MHM && scheme != GAMER_CTU) return GAMER_EINVAL;
+    if (precision != GAMER_FP32 && precision != GAMER_FP64) return GAMER_EINVAL;
+    if (!aligned16(u)) return GAMER_EINVAL;
+    if (opts && (opts->n_scalar < 0 || opts->n_scalar > 1)) return GAMER_EINVAL;
+    if (n_groups > 0x7fffffff) return GAMER_EUNSUPPORTED;
+    return precision == GAMER_FP32 ? cfl_typed<float>(u, n_groups, dh, gamma, cfl, scheme, group_speed_out, dt_out, opts)
+                                   : cfl_typed<double>(u, n_groups, dh, gamma, cfl, scheme, group_speed_out, dt_out, opts);
+}
+
+extern "C" int gamer_cfl_dt(const void* u, int64_t n_groups, double dh, double gamma, double cfl, int scheme,
+                            int precision, void* group_speed_out, double* dt_out) {
+    return gamer_cfl_dt_ex(u, n_groups, dh, gamma, cfl, scheme, precision, group_speed_out, dt_out, nullptr);
+}
+
+extern "C" int gamer_cfl_from_group_speed(const void* group_speed, int64_t n_groups, double dh, double cfl,
+                                          int precision, double* dt_out, void* stream) {
+    if (!group_speed || !dt_out || n_groups < 0 || !(dh > 0.0) || !(cfl > 0.0)) return GAMER_EINVAL;
+    if (precision != GAMER_FP32 && precision != GAMER_FP64) return GAMER_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (cudaMemsetAsync(dt_out, 0, sizeof(double), st) != cudaSuccess) return GAMER_ECUDA;
+    if (n_groups > 0) {
+        const unsigned grid = (unsigned)((n_groups + 8191) / 8192 > 64 ? 64 : (n_groups + 8191) / 8192);
+        if (precision == GAMER_FP32)
+            group_max_kernel<float><<<grid, 1024, 0, st>>>(static_cast<const float*>(group_speed), n_groups, dt_out);
+        else
+            group_max_kernel<double><<<grid, 1024, 0, st>>>(static_cast<const double*>(group_speed), n_groups, dt_out);
+        g_launches += 1;
+    }
+    finish_dt_kernel<<<1, 1, 0, st>>>(dt_out, cfl * dh);
+    g_launches += 1;
+    return cudaGetLastError() == cudaSuccess ? GAMER_OK : GAMER_ECUDA;
+}
+
+// ------------------------------------------------------------------------------------------ ghost refresh
+extern "C" int gamer_refresh_ghosts_periodic(const void* u, void* in, int gz, int gy, int gx, int nvar, int precision,
+                                             void* stream) {
+    if (!u || !in || gz < 1 || gy < 1 || gx < 1 || nvar < 5 || nvar > 6) return GAMER_EINVAL;
+    if (precision != GAMER_FP32 && precision != GAMER_FP64) return GAMER_EINVAL;
+    const long long ng = (long long)gz * gy * gx;
+    if (ng * nvar > 0x7fffffff) return GAMER_EUNSUPPORTED;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const dim3 grid((unsigned)(ng * nvar), NP);
+    if (precision == GAMER_FP32)
+        refresh_periodic_kernel<float><<<grid, 512, 0, st>>>(static_cast<const float*>(u), static_cast<float*>(in), gz, gy, gx, nvar);
+    else
+        refresh_periodic_kernel<double><<<grid, 512, 0, st>>>(static_cast<const double*>(u), static_cast<double*>(in), gz, gy, gx, nvar);
+    g_launches += 1;
+    return cudaGetLastError() == cudaSuccess ? GAMER_OK : GAMER_ECUDA;
+}
+
+// ------------------------------------------------------------------------------------------ host-buffer entry
+extern "C" int gamer_fluid_advance_host(const void* in_host, void* out_host, void* flux_out_host,
+                                        void* group_speed_out_host, int64_t n_groups, double dt, double dh,
+                                        double gamma, int scheme, int recon, int riemann, int precision,
+                                        const gamer_opts* opts) {
+    if (!in_host || !out_host || n_groups < 0) return GAMER_EINVAL;
+    if (precision != GAMER_FP32 && precision != GAMER_FP64) return GAMER_EINVAL;
+    if (!(dt > 0.0) || !std::isfinite(dt)) return GAMER_EINVAL;
+    if (n_groups == 0) return GAMER_OK;
+    const int nv = 5 + (opts ? opts->n_scalar : 0);
+    const size_t sz = (size_t)precision;
+    const size_t in_g = (size_t)nv * NPC * sz, out_g = (size_t)nv * PS * PS * PS * sz, fl_g = (size_t)9 * nv * PS * PS * sz;
+    constexpr int NBUF = 3;
+    const int64_t chunk = n_groups < 592 ? n_groups : 592;   // 4 waves of 148 CTAs; ~1e6 cells saturate (L321)
+    cudaStream_t st[NBUF] = {nullptr, nullptr, nullptr};
+    char *d_in[NBUF] = {}, *d_out[NBUF] = {}, *d_fl[NBUF] = {}, *d_sp[NBUF] = {};
+    int rc = GAMER_OK;
+    for (int b = 0; b < NBUF && rc == GAMER_OK; ++b) {
+        if (cudaStreamCreateWithFlags(&st[b], cudaStreamNonBlocking) != cudaSuccess) rc = GAMER_ECUDA;
+        else if (cudaMalloc(&d_in[b], in_g * chunk) != cudaSuccess || cudaMalloc(&d_out[b], out_g * chunk) != cudaSuccess ||
+                 cudaMalloc(&d_fl[b], fl_g * chunk) != cudaSuccess || cudaMalloc(&d_sp[b], sz * chunk) != cudaSuccess)
+            rc = GAMER_ECUDA;
+    }
+    int64_t done = 0;
+    for (int it = 0; done < n_groups && rc == GAMER_OK; ++it) {
+        const int b = it % NBUF;
+        const int64_t n = (n_groups - done) < chunk ? (n_groups - done) : chunk;
+        gamer_opts o;
+        if (opts) o = *opts; else std::memset(&o, 0, sizeof(o));
+        o.stream = st[b];
+        o.dt_dev = nullptr; o.n_unphysical_out = nullptr; o.diag_out = nullptr;
+        o.group_speed_out = group_speed_out_host ? d_sp[b] : nullptr;
+        const char* hin = static_cast<const char*>(in_host) + done * in_g;
+        if (cudaMemcpyAsync(d_in[b], hin, in_g * n, cudaMemcpyHostToDevice, st[b]) != cudaSuccess) { rc = GAMER_ECUDA; break; }
+        rc = gamer_fluid_advance_ex(d_in[b], d_out[b], flux_out_host ? d_fl[b] : nullptr, n, dt, dh, gamma, scheme, recon,
+                                    riemann, precision, &o);
+        if (rc != GAMER_OK) break;
+        cudaMemcpyAsync(static_cast<char*>(out_host) + done * out_g, d_out[b], out_g * n, cudaMemcpyDeviceToHost, st[b]);
+        if (flux_out_host)
+            cudaMemcpyAsync(static_cast<char*>(flux_out_host) + done * fl_g, d_fl[b], fl_g * n, cudaMemcpyDeviceToHost, st[b]);
+        if (group_speed_out_host)
+            cudaMemcpyAsync(static_cast<char*>(group_speed_out_host) + done * sz, d_sp[b], sz * n, cudaMemcpyDeviceToHost, st[b]);
+        if (cudaGetLastError() != cudaSuccess) rc = GAMER_ECUDA;
+        done += n;
+    }
+    for (int b = 0; b < NBUF; ++b) {
+        if (st[b]) { if (cudaStreamSynchronize(st[b]) != cudaSuccess) rc = GAMER_ECUDA; }
+        cudaFree(d_in[b]); cudaFree(d_out[b]); cudaFree(d_fl[b]); cudaFree(d_sp[b]);
+        if (st[b]) cudaStreamDestroy(st[b]);
+    }
+    return rc;
+}
+
+extern "C" int64_t gamer_launch_count(void) { return g_launches.load(); }
+
+extern "C" const char* gamer_strerror(int code) {
+    switch (code) {
+    case GAMER_OK: return "success";
+    case GAMER_EINVAL: return "invalid argument";
+    case GAMER_EUNSUPPORTED: return "unsupported combination or size";
+    case GAMER_ECUDA: return "CUDA runtime or launch error";
+    default: return "unknown error code";
+    }
+}
+
+extern "C" int gamer_version(void) { return 100; }

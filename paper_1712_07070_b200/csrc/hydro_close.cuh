@@ -1,0 +1,119 @@
+// hydro_close.cuh -- closing step of one updated cell (PAPER.md L100 dual energy, L102-105 remedies,
+// L504 floors) and the CFL signal speed (Eqs. 1-2).
+#pragma once
+#include "hydro_stream.cuh"
+
+namespace gamer {
+
+template <typename T, int NV>
+__device__ __forceinline__ bool is_physical(const T* U) {
+    bool ok = U[0] > T(0);
+#pragma unroll
+    for (int v = 0; v < NV; ++v) ok = ok && Ops<T>::finite(U[v]);
+    const T ek = T(0.5) * (U[1] * U[1] + U[2] * U[2] + U[3] * U[3]) / U[0];
+    return ok && (U[4] - ek) > T(0);
+}
+
+// E_the/E_kin < xi: rebuild E from the entropy; otherwise resynchronise the entropy from E (L100)
+template <typename T, int NV>
+__device__ __forceinline__ int dual_energy_fix(T* U, const Phys<T>& ph) {
+    if (NV < 6 || !ph.dual || !(U[0] > T(0))) return 0;
+    const T ek = T(0.5) * (U[1] * U[1] + U[2] * U[2] + U[3] * U[3]) / U[0];
+    const T et = U[4] - ek;
+    const T rg = Ops<T>::pow(U[0], ph.gm1);
+    if (et < ph.xi * ek) {
+        U[4] = ek + U[NV - 1] * rg * ph.inv_gm1;
+        return 1;
+    }
+    U[NV - 1] = ph.gm1 * et / rg;
+    return 0;
+}
+
+template <typename T, int NV>
+__device__ __forceinline__ void floor_cons(T* U, const Phys<T>& ph) {
+    if (ph.min_dens > T(0) && U[0] < ph.min_dens) U[0] = ph.min_dens;
+    const T ek = T(0.5) * (U[1] * U[1] + U[2] * U[2] + U[3] * U[3]) / U[0];
+    const T P = ph.gm1 * (U[4] - ek);
+    T pf = ph.min_pres;
+    const T pt = U[0] * ph.min_temp;
+    if (pt > pf) pf = pt;
+    if (pf > T(0) && P < pf) {
+        U[4] = ek + pf * ph.inv_gm1;
+        if (NV > 5 && ph.dual) U[NV - 1] = pf / Ops<T>::pow(U[0], ph.gm1);
+    }
+}
+
+template <typename T, int NV, int SCHEME, bool EXT>
+__device__ __forceinline__ T signal_speed(const T* U, const Phys<T>& ph) {
+    T W[NV];
+    cons2prim<T, NV>(U, W, ph);
+    if (EXT && ph.floors) floor_prim(W, ph);
+    const T cs = Ops<T>::sqrt(ph.gamma * W[4] * Ops<T>::rcp(W[0]));
+    const T ax = Ops<T>::abs(W[1]), ay = Ops<T>::abs(W[2]), az = Ops<T>::abs(W[3]);
+    if (SCHEME == MHM) return ax + ay + az + T(3) * cs;
+    return Ops<T>::max(Ops<T>::max(ax, ay), az) + cs;
+}
+
+// remedy (ii), L105: first order in space and time, unsplit, same Riemann solver, straight from the
+// padded input in global memory (rare path).  gin points at variable 0 of the padded cell.
+template <typename T, int SOLVER, int NV, bool EXT>
+__device__ __noinline__ void first_order_cell(const T* gin, T* Unew, int* nfb, const Phys<T>& ph) {
+    T Uc[NV], Wc[NV], acc[NV];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) { Uc[v] = gin[(size_t)v * NPC]; acc[v] = T(0); }
+    cons2prim<T, NV>(Uc, Wc, ph);
+    const int step[3] = {1, NP, NP * NP};
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const int cn = 1 + d, c1 = 1 + (d + 1) % 3, c2 = 1 + (d + 2) % 3;
+        T Wr[NV] ;
+        Wr[0] = Wc[0]; Wr[1] = Wc[cn]; Wr[2] = Wc[c1]; Wr[3] = Wc[c2]; Wr[4] = Wc[4];
+        if (NV > 5) Wr[NV - 1] = Wc[NV - 1];
+        T Fd[NV];
+#pragma unroll
+        for (int v = 0; v < NV; ++v) Fd[v] = T(0);
+#pragma unroll
+        for (int s = 0; s < 2; ++s) {
+            T Un[NV], Wn[NV], Wq[NV], F[NV];
+            const int off = s ? step[d] : -step[d];
+#pragma unroll
+            for (int v = 0; v < NV; ++v) Un[v] = gin[(size_t)v * NPC + off];
+            cons2prim<T, NV>(Un, Wn, ph);
+            Wq[0] = Wn[0]; Wq[1] = Wn[cn]; Wq[2] = Wn[c1]; Wq[3] = Wn[c2]; Wq[4] = Wn[4];
+            if (NV > 5) Wq[NV - 1] = Wn[NV - 1];
+            const bool fb = s ? riemann_flux<T, SOLVER, NV>(Wr, Wq, F, ph) : riemann_flux<T, SOLVER, NV>(Wq, Wr, F, ph);
+            *nfb += fb ? 1 : 0;
+            const T sg = s ? T(1) : T(-1);
+            Fd[0] += sg * F[0];
+            Fd[cn] += sg * F[1];
+            Fd[c1] += sg * F[2];
+            Fd[c2] += sg * F[3];
+            Fd[4] += sg * F[4];
+            if (NV > 5) Fd[NV - 1] += sg * F[NV - 1];
+        }
+#pragma unroll
+        for (int v = 0; v < NV; ++v) acc[v] += Fd[v];
+    }
+#pragma unroll
+    for (int v = 0; v < NV; ++v) Unew[v] = Uc[v] - ph.lam * acc[v];
+}
+
+struct Counters {
+    int roe_fb, reverted, first_order, dual_fix, unphys;
+};
+
+// finish one interior cell: U holds the high-order update on entry, the final state on exit
+template <typename T, int SOLVER, int NV, bool EXT>
+__device__ __forceinline__ void close_cell(T* U, const T* gin_cell, Counters& cnt, const Phys<T>& ph) {
+    if (!EXT) return;
+    cnt.dual_fix += dual_energy_fix<T, NV>(U, ph);
+    if (ph.remedy2 && !is_physical<T, NV>(U)) {
+        cnt.first_order++;
+        first_order_cell<T, SOLVER, NV, EXT>(gin_cell, U, &cnt.roe_fb, ph);
+        cnt.dual_fix += dual_energy_fix<T, NV>(U, ph);
+    }
+    if (ph.floors) floor_cons<T, NV>(U, ph);
+    if (!is_physical<T, NV>(U)) cnt.unphys++;
+}
+
+}  // namespace gamer

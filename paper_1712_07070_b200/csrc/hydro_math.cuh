@@ -1,0 +1,237 @@
+// hydro_math.cuh -- per-cell / per-face device arithmetic of the patch-group hydro solver.
+// Written from the paper's method list (section 2.2) and the textbook
+// formulas it names; shares nothing with oracle/ (the CPU oracle is test infrastructure).
+//
+// Conventions: W = primitive (rho, v0, v1, v2, P [, q]), U = conserved (rho, m0, m1, m2, E [, s]).
+// "Rotated" means the face normal is component 1 (n) and the transverse ones are 2,3 (t1,t2),
+// taken in cyclic order (x: y,z; y: z,x; z: x,y).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace gamer {
+
+enum { MHM = 1, CTU = 2 };
+enum { PLM = 1, PPM = 2 };
+enum { ROE = 1, HLLC = 2, HLLE = 3 };
+enum { LIM_GMINMOD = 1, LIM_VANLEER = 2, LIM_VANALBADA = 3 };
+
+// ---------------------------------------------------------------------------------------------
+// precision-dependent primitives.  fp32 uses the SFU approximations (<= 2 ulp); the parity bound
+// of the fp32 path is 1e-5 relative L1 per step, four orders of magnitude above that.
+// ---------------------------------------------------------------------------------------------
+template <typename T> struct Ops;
+
+template <> struct Ops<float> {
+    static __device__ __forceinline__ float rcp(float x) {
+        float r;
+        asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+        return r;
+    }
+    static __device__ __forceinline__ float sqrt(float x) {
+        float r;
+        asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+        return r;
+    }
+    static __device__ __forceinline__ float rsqrt(float x) {
+        float r;
+        asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+        return r;
+    }
+    static __device__ __forceinline__ float abs(float x) { return fabsf(x); }
+    static __device__ __forceinline__ float min(float a, float b) { return fminf(a, b); }
+    static __device__ __forceinline__ float max(float a, float b) { return fmaxf(a, b); }
+    static __device__ __forceinline__ float pow(float a, float b) { return powf(a, b); }
+    static __device__ __forceinline__ float copysign(float a, float b) { return copysignf(a, b); }
+    static __device__ __forceinline__ bool finite(float a) { return isfinite(a); }
+};
+
+template <> struct Ops<double> {
+    static __device__ __forceinline__ double rcp(double x) { return 1.0 / x; }
+    static __device__ __forceinline__ double sqrt(double x) { return ::sqrt(x); }
+    static __device__ __forceinline__ double rsqrt(double x) { return 1.0 / ::sqrt(x); }
+    static __device__ __forceinline__ double abs(double x) { return fabs(x); }
+    static __device__ __forceinline__ double min(double a, double b) { return fmin(a, b); }
+    static __device__ __forceinline__ double max(double a, double b) { return fmax(a, b); }
+    static __device__ __forceinline__ double pow(double a, double b) { return ::pow(a, b); }
+    static __device__ __forceinline__ double copysign(double a, double b) { return ::copysign(a, b); }
+    static __device__ __forceinline__ bool finite(double a) { return isfinite(a); }
+};
+
+// run-time constants shared by every stage (kept in registers / constant bank)
+template <typename T> struct Phys {
+    T gamma, gm1, inv_gm1;
+    T lam;          // dt / dh
+    T hlam;         // dt / (2 dh)
+    T theta;        // generalized-minmod parameter
+    int limiter;    // LIM_*
+    // extended mode only
+    T xi, min_dens, min_pres, min_temp;
+    int floors, dual, remedy2;
+};
+
+// ---------------------------------------------------------------------------------------------
+// conserved <-> primitive
+// ---------------------------------------------------------------------------------------------
+template <typename T, int NV>
+__device__ __forceinline__ void cons2prim(const T* U, T* W, const Phys<T>& ph) {
+    const T ir = Ops<T>::rcp(U[0]);
+    W[0] = U[0];
+    W[1] = U[1] * ir;
+    W[2] = U[2] * ir;
+    W[3] = U[3] * ir;
+    const T ek = T(0.5) * (U[1] * W[1] + U[2] * W[2] + U[3] * W[3]);
+    W[4] = ph.gm1 * (U[4] - ek);
+    if (NV > 5) W[NV - 1] = U[NV - 1] * ir;
+}
+
+template <typename T, int NV>
+__device__ __forceinline__ void prim2cons(const T* W, T* U, const Phys<T>& ph) {
+    U[0] = W[0];
+    U[1] = W[0] * W[1];
+    U[2] = W[0] * W[2];
+    U[3] = W[0] * W[3];
+    U[4] = W[4] * ph.inv_gm1 + T(0.5) * (U[1] * W[1] + U[2] * W[2] + U[3] * W[3]);
+    if (NV > 5) U[NV - 1] = W[0] * W[NV - 1];
+}
+
+template <typename T>
+__device__ __forceinline__ void floor_prim(T* W, const Phys<T>& ph) {
+    if (ph.min_dens > T(0) && W[0] < ph.min_dens) W[0] = ph.min_dens;
+    T pf = ph.min_pres;
+    const T pt = W[0] * ph.min_temp;
+    if (pt > pf) pf = pt;
+    if (pf > T(0) && W[4] < pf) W[4] = pf;
+}
+
+// ---------------------------------------------------------------------------------------------
+// slope limiters (L94)
+// ---------------------------------------------------------------------------------------------
+template <typename T, bool EXT>
+__device__ __forceinline__ T limited_slope(T dL, T dR, const Phys<T>& ph) {
+    const T prod = dL * dR;
+    if (EXT && ph.limiter != LIM_GMINMOD) {
+        if (!(prod > T(0))) return T(0);
+        if (ph.limiter == LIM_VANLEER) return T(2) * prod * Ops<T>::rcp(dL + dR);
+        return prod * (dL + dR) * Ops<T>::rcp(dL * dL + dR * dR);
+    }
+    const T aL = Ops<T>::abs(dL), aR = Ops<T>::abs(dR);
+    T m = ph.theta * Ops<T>::min(aL, aR);
+    m = Ops<T>::min(m, T(0.5) * Ops<T>::abs(dL + dR));
+    m = Ops<T>::copysign(m, dR);
+    return prod > T(0) ? m : T(0);
+}
+
+// face values of the centre cell of a strip: q points at the centre, neighbours at q[+-s], q[+-2s]
+template <typename T, int RECON, bool EXT>
+__device__ __forceinline__ void face_values(const T* q, int s, T& wm, T& wp, const Phys<T>& ph) {
+    const T c = q[0], l1 = q[-s], r1 = q[s];
+    if (RECON == PLM) {
+        const T sl = limited_slope<T, EXT>(c - l1, r1 - c, ph);
+        wm = c - T(0.5) * sl;
+        wp = c + T(0.5) * sl;
+    } else {   // PPM, Colella & Woodward (1984) eqs. 1.6-1.10, no steepening / flattening
+        const T l2 = q[-2 * s], r2 = q[2 * s];
+        const T sm = limited_slope<T, EXT>(l1 - l2, c - l1, ph);
+        const T s0 = limited_slope<T, EXT>(c - l1, r1 - c, ph);
+        const T sp = limited_slope<T, EXT>(r1 - c, r2 - r1, ph);
+        const T sixth = T(1.0 / 6.0);
+        T m = T(0.5) * (l1 + c) - (s0 - sm) * sixth;
+        T p = T(0.5) * (c + r1) - (sp - s0) * sixth;
+        if ((p - c) * (c - m) <= T(0)) {
+            m = c;
+            p = c;
+        } else {
+            const T D = p - m;
+            const T C = c - T(0.5) * (m + p);
+            const T DC = D * C, D6 = D * D * sixth;
+            if (DC > D6) m = T(3) * c - T(2) * p;
+            else if (DC < -D6) p = T(3) * c - T(2) * m;
+        }
+        wm = m;
+        wp = p;
+    }
+}
+
+// physical flux along axis D of a state known as W and U, added with sign sg into acc
+template <typename T, int NV, int D>
+__device__ __forceinline__ void phys_flux(const T* W, const T* U, T* F) {
+    const T vn = W[1 + D];
+    F[0] = U[0] * vn;
+    F[1] = U[1] * vn;
+    F[2] = U[2] * vn;
+    F[3] = U[3] * vn;
+    F[1 + D] += W[4];
+    F[4] = vn * (U[4] + W[4]);
+    if (NV > 5) F[NV - 1] = U[NV - 1] * vn;
+}
+
+// ---------------------------------------------------------------------------------------------
+// CTU characteristic tracing over dt/2 (Colella 1990; Colella & Woodward 1984 eq. 1.12): rotated
+// primitive cell value W and untraced face values wm/wp -> traced tm/tp.  Reference state = average
+// over the domain of dependence of the fastest wave toward the face; the slower waves that also
+// move toward the face are corrected to their own domains.
+// ---------------------------------------------------------------------------------------------
+template <typename T, int RECON, int NV>
+__device__ __forceinline__ void trace_cell(const T* W, const T* wm, const T* wp, T* tm, T* tp,
+                                           const Phys<T>& ph) {
+    const T rho = W[0], vn = W[1];
+    const T c2 = ph.gamma * W[4] * Ops<T>::rcp(rho);
+    const T cs = Ops<T>::sqrt(c2);
+    const T l1 = vn - cs, l5 = vn + cs;
+    const T x1 = l1 * ph.lam, x0 = vn * ph.lam, x5 = l5 * ph.lam;
+    const T x5p = x5 > T(0) ? x5 : T(0);
+    const T x1m = x1 < T(0) ? x1 : T(0);
+    const T third = T(1.0 / 3.0);
+    T d[NV], w6[NV];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) {
+        d[v] = wp[v] - wm[v];
+        w6[v] = RECON == PPM ? T(6) * (W[v] - T(0.5) * (wm[v] + wp[v])) : T(0);
+        tp[v] = wp[v] - T(0.5) * x5p * (d[v] - (T(1) - T(2) * third * x5p) * w6[v]);
+        tm[v] = wm[v] - T(0.5) * x1m * (d[v] + (T(1) + T(2) * third * x1m) * w6[v]);
+    }
+    const T ic2 = Ops<T>::rcp(c2);
+    const T rc = rho * cs;
+    const T cor = cs * Ops<T>::rcp(rho);
+    // ---- plus face: waves with lambda > 0
+    if (l1 > T(0)) {
+        const T A = T(0.5) * (x5p - x1), B = third * (x5p * x5p - x1 * x1);
+        const T vP = A * (d[4] - w6[4]) + B * w6[4];
+        const T vU = A * (d[1] - w6[1]) + B * w6[1];
+        const T amp = (vP - rc * vU) * (T(0.5) * ic2);
+        tp[0] += amp;
+        tp[1] -= amp * cor;
+        tp[4] += amp * c2;
+    }
+    if (vn > T(0)) {
+        const T A = T(0.5) * (x5p - x0), B = third * (x5p * x5p - x0 * x0);
+        const T vR = A * (d[0] - w6[0]) + B * w6[0];
+        const T vP = A * (d[4] - w6[4]) + B * w6[4];
+        tp[0] += vR - vP * ic2;
+        tp[2] += A * (d[2] - w6[2]) + B * w6[2];
+        tp[3] += A * (d[3] - w6[3]) + B * w6[3];
+        if (NV > 5) tp[NV - 1] += A * (d[NV - 1] - w6[NV - 1]) + B * w6[NV - 1];
+    }
+    // ---- minus face: waves with lambda < 0
+    if (l5 < T(0)) {
+        const T C = T(0.5) * (x1m - x5), D = third * (x1m * x1m - x5 * x5);
+        const T vP = C * (d[4] + w6[4]) + D * w6[4];
+        const T vU = C * (d[1] + w6[1]) + D * w6[1];
+        const T amp = (vP + rc * vU) * (T(0.5) * ic2);
+        tm[0] += amp;
+        tm[1] += amp * cor;
+        tm[4] += amp * c2;
+    }
+    if (vn < T(0)) {
+        const T C = T(0.5) * (x1m - x0), D = third * (x1m * x1m - x0 * x0);
+        const T vR = C * (d[0] + w6[0]) + D * w6[0];
+        const T vP = C * (d[4] + w6[4]) + D * w6[4];
+        tm[0] += vR - vP * ic2;
+        tm[2] += C * (d[2] + w6[2]) + D * w6[2];
+        tm[3] += C * (d[3] + w6[3]) + D * w6[3];
+        if (NV > 5) tm[NV - 1] += C * (d[NV - 1] + w6[NV - 1]) + D * w6[NV - 1];
+    }
+}
+
+}  // namespace gamer

@@ -1,0 +1,154 @@
+// hydro_riemann.cuh -- Roe / HLLC / HLLE fluxes on rotated primitive states.
+#pragma once
+#include "hydro_math.cuh"
+
+namespace gamer {
+
+template <typename T> struct RoeAvg {
+    T u, v, w, H, q2, a2, a;
+};
+
+template <typename T> struct Side {
+    T rho, u, v, w, P, E, H;
+    T m1, m2, m3;   // momenta
+};
+
+template <typename T>
+__device__ __forceinline__ void make_side(const T* W, Side<T>& s, const Phys<T>& ph) {
+    s.rho = W[0]; s.u = W[1]; s.v = W[2]; s.w = W[3]; s.P = W[4];
+    s.m1 = s.rho * s.u; s.m2 = s.rho * s.v; s.m3 = s.rho * s.w;
+    s.E = s.P * ph.inv_gm1 + T(0.5) * (s.m1 * s.u + s.m2 * s.v + s.m3 * s.w);
+    s.H = (s.E + s.P) * Ops<T>::rcp(s.rho);
+}
+
+template <typename T>
+__device__ __forceinline__ void side_flux(const Side<T>& s, T* F) {
+    F[0] = s.m1;
+    F[1] = s.m1 * s.u + s.P;
+    F[2] = s.m2 * s.u;
+    F[3] = s.m3 * s.u;
+    F[4] = s.u * (s.E + s.P);
+}
+
+template <typename T>
+__device__ __forceinline__ void roe_average(const Side<T>& L, const Side<T>& R, RoeAvg<T>& r, const Phys<T>& ph) {
+    const T wl = Ops<T>::sqrt(L.rho), wr = Ops<T>::sqrt(R.rho);
+    const T id = Ops<T>::rcp(wl + wr);
+    const T fl = wl * id, fr = wr * id;
+    r.u = fl * L.u + fr * R.u;
+    r.v = fl * L.v + fr * R.v;
+    r.w = fl * L.w + fr * R.w;
+    r.H = fl * L.H + fr * R.H;
+    r.q2 = r.u * r.u + r.v * r.v + r.w * r.w;
+    r.a2 = ph.gm1 * (r.H - T(0.5) * r.q2);
+    r.a = r.a2 > T(0) ? Ops<T>::sqrt(r.a2) : T(0);
+}
+
+// HLLE (Einfeldt et al. 1991)
+template <typename T>
+__device__ __forceinline__ void solve_hlle(const Side<T>& L, const Side<T>& R, const RoeAvg<T>& r, T* F,
+                                           const Phys<T>& ph) {
+    T FL[5], FR[5];
+    side_flux(L, FL);
+    side_flux(R, FR);
+    const T cl = Ops<T>::sqrt(ph.gamma * L.P * Ops<T>::rcp(L.rho));
+    const T cr = Ops<T>::sqrt(ph.gamma * R.P * Ops<T>::rcp(R.rho));
+    const T bl = Ops<T>::min(r.u - r.a, L.u - cl);
+    const T br = Ops<T>::max(r.u + r.a, R.u + cr);
+    const T bm = Ops<T>::min(bl, T(0)), bp = Ops<T>::max(br, T(0));
+    const T id = Ops<T>::rcp(bp - bm);
+    const T bb = bp * bm;
+    const T UL[5] = {L.rho, L.m1, L.m2, L.m3, L.E};
+    const T UR[5] = {R.rho, R.m1, R.m2, R.m3, R.E};
+#pragma unroll
+    for (int v = 0; v < 5; ++v) F[v] = (bp * FL[v] - bm * FR[v] + bb * (UR[v] - UL[v])) * id;
+}
+
+// HLLC (Toro 2009 ch. 10) with Einfeldt's wave-speed bounds
+template <typename T>
+__device__ __forceinline__ void solve_hllc(const Side<T>& L, const Side<T>& R, const RoeAvg<T>& r, T* F,
+                                           const Phys<T>& ph) {
+    const T cl = Ops<T>::sqrt(ph.gamma * L.P * Ops<T>::rcp(L.rho));
+    const T cr = Ops<T>::sqrt(ph.gamma * R.P * Ops<T>::rcp(R.rho));
+    const T SL = Ops<T>::min(r.u - r.a, L.u - cl);
+    const T SR = Ops<T>::max(r.u + r.a, R.u + cr);
+    if (SL >= T(0)) { side_flux(L, F); return; }
+    if (SR <= T(0)) { side_flux(R, F); return; }
+    const T ml = L.rho * (SL - L.u), mr = R.rho * (SR - R.u);
+    const T SS = (R.P - L.P + L.u * ml - R.u * mr) * Ops<T>::rcp(ml - mr);
+    const bool left = SS >= T(0);
+    const Side<T>& K = left ? L : R;
+    const T SK = left ? SL : SR;
+    T FK[5];
+    side_flux(K, FK);
+    const T dk = SK - K.u;
+    const T fac = K.rho * dk * Ops<T>::rcp(SK - SS);
+    const T ir = Ops<T>::rcp(K.rho);
+    const T es = K.E * ir + (SS - K.u) * (SS + K.P * ir * Ops<T>::rcp(dk));
+    F[0] = FK[0] + SK * (fac - K.rho);
+    F[1] = FK[1] + SK * (fac * SS - K.m1);
+    F[2] = FK[2] + SK * (fac * K.v - K.m2);
+    F[3] = FK[3] + SK * (fac * K.w - K.m3);
+    F[4] = FK[4] + SK * (fac * es - K.E);
+}
+
+// Roe (1981), no entropy fix.  Returns true if remedy (i) (L104) must be taken.
+template <typename T>
+__device__ __forceinline__ bool solve_roe(const Side<T>& L, const Side<T>& R, const RoeAvg<T>& r, T* F,
+                                          const Phys<T>& ph) {
+    if (!(r.a2 > T(0))) return true;
+    const T d0 = R.rho - L.rho, d1 = R.m1 - L.m1, d2 = R.m2 - L.m2, d3 = R.m3 - L.m3, d4 = R.E - L.E;
+    const T u = r.u, v = r.v, w = r.w, H = r.H, a = r.a;
+    const T a3 = d2 - v * d0;
+    const T a4 = d3 - w * d0;
+    const T d5 = d4 - a3 * v - a4 * w;
+    const T ia2 = Ops<T>::rcp(r.a2);
+    const T a2 = ph.gm1 * ia2 * (d0 * (H - u * u) + u * d1 - d5);
+    const T a1 = (d0 * (u + a) - d1 - a * a2) * (T(0.5) * Ops<T>::rcp(a));
+    const T a5 = d0 - (a1 + a2);
+    // intermediate states U_L + a1 K1 and U_R - a5 K5
+    {
+        const T r1 = L.rho + a1, n1 = L.m1 + a1 * (u - a), s1 = L.m2 + a1 * v, t1 = L.m3 + a1 * w,
+                e1 = L.E + a1 * (H - u * a);
+        const T r5 = R.rho - a5, n5 = R.m1 - a5 * (u + a), s5 = R.m2 - a5 * v, t5 = R.m3 - a5 * w,
+                e5 = R.E - a5 * (H + u * a);
+        // P > 0  <=>  rho*E - |m|^2/2 > 0 when rho > 0
+        const T p1 = r1 * e1 - T(0.5) * (n1 * n1 + s1 * s1 + t1 * t1);
+        const T p5 = r5 * e5 - T(0.5) * (n5 * n5 + s5 * s5 + t5 * t5);
+        if (!(r1 > T(0)) || !(r5 > T(0)) || !(p1 > T(0)) || !(p5 > T(0))) return true;
+    }
+    T FL[5], FR[5];
+    side_flux(L, FL);
+    side_flux(R, FR);
+    const T l1 = Ops<T>::abs(u - a) * a1, l2 = Ops<T>::abs(u), l5 = Ops<T>::abs(u + a) * a5;
+    const T c2 = l2 * a2, c3 = l2 * a3, c4 = l2 * a4;
+    F[0] = T(0.5) * ((FL[0] + FR[0]) - (l1 + c2 + l5));
+    F[1] = T(0.5) * ((FL[1] + FR[1]) - (l1 * (u - a) + c2 * u + l5 * (u + a)));
+    F[2] = T(0.5) * ((FL[2] + FR[2]) - (l1 * v + (c2 * v + c3) + l5 * v));
+    F[3] = T(0.5) * ((FL[3] + FR[3]) - (l1 * w + (c2 * w + c4) + l5 * w));
+    F[4] = T(0.5) * ((FL[4] + FR[4]) - (l1 * (H - u * a) + (c2 * (T(0.5) * r.q2) + c3 * v + c4 * w) + l5 * (H + u * a)));
+    return false;
+}
+
+// Flux through a face from rotated primitive states.  Returns true if Roe fell back to HLLE.
+template <typename T, int SOLVER, int NV>
+__device__ __forceinline__ bool riemann_flux(const T* WL, const T* WR, T* F, const Phys<T>& ph) {
+    Side<T> L, R;
+    RoeAvg<T> r;
+    make_side(WL, L, ph);
+    make_side(WR, R, ph);
+    roe_average(L, R, r, ph);
+    bool fb = false;
+    if (SOLVER == ROE) {
+        fb = solve_roe(L, R, r, F, ph);
+        if (fb) solve_hlle(L, R, r, F, ph);
+    } else if (SOLVER == HLLC) {
+        solve_hllc(L, R, r, F, ph);
+    } else {
+        solve_hlle(L, R, r, F, ph);
+    }
+    if (NV > 5) F[NV - 1] = F[0] >= T(0) ? F[0] * WL[NV - 1] : F[0] * WR[NV - 1];
+    return fb;
+}
+
+}  // namespace gamer

@@ -1,0 +1,211 @@
+// hydro_stream.cuh -- shared machinery of the z-streaming patch-group kernels.
+//
+// One CTA advances one (16 x TY x 16) column tile of a patch group (TY = 16 is the whole group),
+// marching along z one plane at a time.  Padded conserved planes are staged in shared memory with
+// 1-D TMA bulk copies (cp.async.bulk + mbarrier, two stages in flight), converted to primitives
+// into a ring of 2R+1 planes (R = reconstruction radius), and every intermediate of the scheme
+// (face states, fluxes) lives only in shared memory / registers for the planes in flight, so HBM
+// sees the algorithmic bytes only: one read of `in`, one write of `out` / `flux_out`.
+// (The paper's own kernels kept these intermediates in global memory.)
+#pragma once
+#include "hydro_riemann.cuh"
+
+namespace gamer {
+
+constexpr int PS = 16;   // cells per patch-group edge
+constexpr int NGH = 3;   // ghost zones (L300)
+constexpr int NP = 22;   // padded edge
+constexpr int NPC = NP * NP * NP;
+
+template <typename T> struct AdvArgs {
+    const T* in;
+    T* out;
+    T* flux;          // nullable
+    T* speed;         // nullable
+    int* n_unphys;    // nullable
+    int* diag;        // nullable, int[4]
+    const double* dt_dev;
+    double dt, dh, gamma, theta, xi, min_dens, min_pres, min_temp;
+    int limiter, dual, remedy2;
+    long long n_groups;
+};
+
+template <typename T>
+__device__ __forceinline__ Phys<T> make_phys(const AdvArgs<T>& a) {
+    Phys<T> ph;
+    const double dt = a.dt_dev ? *a.dt_dev : a.dt;
+    const double lam = dt / a.dh;
+    ph.gamma = T(a.gamma);
+    ph.gm1 = T(a.gamma - 1.0);
+    ph.inv_gm1 = T(1.0 / (a.gamma - 1.0));
+    ph.lam = T(lam);
+    ph.hlam = T(0.5 * lam);
+    ph.theta = T(a.theta);
+    ph.limiter = a.limiter;
+    ph.xi = T(a.xi);
+    ph.min_dens = T(a.min_dens);
+    ph.min_pres = T(a.min_pres);
+    ph.min_temp = T(a.min_temp);
+    ph.floors = (a.min_dens > 0.0 || a.min_pres > 0.0 || a.min_temp > 0.0) ? 1 : 0;
+    ph.dual = a.dual;
+    ph.remedy2 = a.remedy2;
+    return ph;
+}
+
+// ---------------------------------------------------------------------------------------------
+// TMA 1-D bulk copy + mbarrier (sm_90+ PTX; SASS: UBLKCP / SYNCS)
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init() {
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    uint32_t ok = 0;
+    const uint32_t addr = smem_u32(bar);
+    while (!ok) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(ok)
+            : "r"(addr), "r"(parity)
+            : "memory");
+    }
+}
+__device__ __forceinline__ void tma_load_1d(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+            smem_u32(dst)),
+        "l"(src), "r"(bytes), "r"(smem_u32(bar))
+        : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() {
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+
+// ---------------------------------------------------------------------------------------------
+// tile geometry
+// ---------------------------------------------------------------------------------------------
+template <int TY> struct Geo {
+    static constexpr int NT = 16 * TY;            // threads per CTA = cells per plane of the tile
+    static constexpr int NTILE = PS / TY;         // tiles per group
+    static constexpr int NR = TY + 2 * NGH;       // rows of a staged plane
+    static constexpr int PLN = NR * NP;           // elements of a staged plane (per variable)
+    static constexpr int EW = 18, EH = TY + 2;    // face-state plane: cells -1..16 x -1..TY
+    static constexpr int EPL = EW * EH;
+    static constexpr int NPLUS = 18 * TY + 32;    // cells whose face states the final pass needs
+    static constexpr int NFX = 17 * TY, NFY = 16 * (TY + 1), NFZ = 16 * TY;
+    static constexpr int NF = NFX + NFY + NFZ;
+};
+
+// stage the padded conserved plane p (0..21) of the tile into raw stage `st`
+template <typename T, int NV, int TY>
+__device__ __forceinline__ void issue_plane(const T* gin, int j0, int p, T* raw_stage, uint64_t* bar) {
+    using G = Geo<TY>;
+    constexpr uint32_t bytes = G::PLN * sizeof(T);
+    fence_proxy_async();
+    mbar_expect_tx(bar, bytes * NV);
+#pragma unroll
+    for (int v = 0; v < NV; ++v)
+        tma_load_1d(raw_stage + v * G::PLN, gin + (size_t)v * NPC + (size_t)p * (NP * NP) + j0 * NP, bytes, bar);
+}
+
+// raw conserved plane -> primitive plane (O1), floors in extended mode
+template <typename T, int NV, bool EXT, int TY>
+__device__ __forceinline__ void convert_plane(const T* raw, T* prim, const Phys<T>& ph, int tid) {
+    using G = Geo<TY>;
+    for (int t = tid; t < G::PLN; t += G::NT) {
+        T U[NV], W[NV];
+#pragma unroll
+        for (int v = 0; v < NV; ++v) U[v] = raw[v * G::PLN + t];
+        cons2prim<T, NV>(U, W, ph);
+        if (EXT && ph.floors) floor_prim(W, ph);
+#pragma unroll
+        for (int v = 0; v < NV; ++v) prim[v * G::PLN + t] = W[v];
+    }
+}
+
+template <typename T, int RECON, bool EXT>
+__device__ __forceinline__ void face_values5(T l2, T l1, T c, T r1, T r2, T& wm, T& wp, const Phys<T>& ph) {
+    T q[5] = {l2, l1, c, r1, r2};
+    face_values<T, RECON, EXT>(q + 2, 1, wm, wp, ph);
+}
+
+// ---------------------------------------------------------------------------------------------
+// final Riemann pass over the faces of one plane of the tile (x- and y-faces of plane kk, z-faces
+// between planes kk-1 and kk).  States are primitive; es = [5][NV][EPL] (x-,x+,y-,y+,z-),
+// zprev = [NV][16*TY] (z+ of plane kk-1).  Writes fx/fy/fz and the patch-boundary planes of flux_out.
+// ---------------------------------------------------------------------------------------------
+template <typename T, int SOLVER, int NV, int TY>
+__device__ __forceinline__ int riemann_plane(const T* es, const T* zprev, T* fx, T* fy, T* fz, T* gflux,
+                                             int kk, int j0, const Phys<T>& ph, int tid) {
+    using G = Geo<TY>;
+    int nfb = 0;
+    const int f_lo = (kk >= 0 && kk < PS) ? 0 : G::NFX + G::NFY;
+    const int f_hi = (kk >= 0 && kk <= PS) ? G::NF : 0;
+    for (int f = f_lo + tid; f < f_hi; f += G::NT) {
+        int d, lidx, ridx, lstr, fidx, fstr, gp, ga, gb;
+        const T *lp, *rp;
+        T* fp;
+        if (f < G::NFX) {
+            const int jj = f / 17, ii = f - jj * 17;
+            d = 0;
+            lp = es + 1 * NV * G::EPL; lidx = (jj + 1) * G::EW + ii; lstr = G::EPL;
+            rp = es + 0 * NV * G::EPL; ridx = lidx + 1;
+            fp = fx; fidx = f; fstr = G::NFX;
+            gp = ii; ga = j0 + jj; gb = kk;
+        } else if (f < G::NFX + G::NFY) {
+            const int g = f - G::NFX;
+            const int jj = g >> 4, ii = g & 15;
+            d = 1;
+            lp = es + 3 * NV * G::EPL; lidx = jj * G::EW + ii + 1; lstr = G::EPL;
+            rp = es + 2 * NV * G::EPL; ridx = lidx + G::EW;
+            fp = fy; fidx = g; fstr = G::NFY;
+            gp = j0 + jj; ga = ii; gb = kk;
+        } else {
+            const int g = f - G::NFX - G::NFY;
+            const int jj = g >> 4, ii = g & 15;
+            d = 2;
+            lp = zprev; lidx = g; lstr = G::NFZ;
+            rp = es + 4 * NV * G::EPL; ridx = (jj + 1) * G::EW + ii + 1;
+            fp = fz; fidx = g; fstr = G::NFZ;
+            gp = kk; ga = ii; gb = j0 + jj;
+        }
+        const int cn = 1 + d, c1 = 1 + (d + 1) % 3, c2 = 1 + (d + 2) % 3;
+        T WL[NV], WR[NV], F[NV];
+        WL[0] = lp[lidx];                 WR[0] = rp[ridx];
+        WL[1] = lp[cn * lstr + lidx];     WR[1] = rp[cn * G::EPL + ridx];
+        WL[2] = lp[c1 * lstr + lidx];     WR[2] = rp[c1 * G::EPL + ridx];
+        WL[3] = lp[c2 * lstr + lidx];     WR[3] = rp[c2 * G::EPL + ridx];
+        WL[4] = lp[4 * lstr + lidx];      WR[4] = rp[4 * G::EPL + ridx];
+        if (NV > 5) { WL[NV - 1] = lp[(NV - 1) * lstr + lidx]; WR[NV - 1] = rp[(NV - 1) * G::EPL + ridx]; }
+        nfb += riemann_flux<T, SOLVER, NV>(WL, WR, F, ph) ? 1 : 0;
+        fp[fidx] = F[0];
+        fp[cn * fstr + fidx] = F[1];
+        fp[c1 * fstr + fidx] = F[2];
+        fp[c2 * fstr + fidx] = F[3];
+        fp[4 * fstr + fidx] = F[4];
+        if (NV > 5) fp[(NV - 1) * fstr + fidx] = F[NV - 1];
+        if (gflux != nullptr && (gp & 7) == 0) {   // faces 0, 8, 16 of the axis: patch boundaries (L112)
+            T* q = gflux + ((size_t)(d * 3 + (gp >> 3)) * NV) * (PS * PS) + gb * PS + ga;
+            q[0] = F[0];
+            q[(size_t)cn * (PS * PS)] = F[1];
+            q[(size_t)c1 * (PS * PS)] = F[2];
+            q[(size_t)c2 * (PS * PS)] = F[3];
+            q[(size_t)4 * (PS * PS)] = F[4];
+            if (NV > 5) q[(size_t)(NV - 1) * (PS * PS)] = F[NV - 1];
+        }
+    }
+    return nfb;
+}
+
+}  // namespace gamer

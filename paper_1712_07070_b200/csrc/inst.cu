@@ -1,0 +1,38 @@
+// inst.cu -- one translation unit per (scheme, recon, riemann): compiled 12 times with
+// -DG_SCHEME=.. -DG_RECON=.. -DG_SOLVER=..; each instantiates fp32/fp64 x {fast, extended, extended+scalar}.
+#include "launch.cuh"
+
+#ifndef G_SCHEME
+#error "compile with -DG_SCHEME=1|2 -DG_RECON=1|2 -DG_SOLVER=1|2|3"
+#endif
+
+#define G_CAT2(a, b, c, d) a##b##_##c##_##d
+#define G_CAT(a, b, c, d) G_CAT2(a, b, c, d)
+#define G_NAME G_CAT(gamer_launch_, G_SCHEME, G_RECON, G_SOLVER)
+
+namespace gamer {
+
+template <typename T, int NV, bool EXT>
+static cudaError_t go(const void* args, cudaStream_t st, int* launches) {
+    const AdvArgs<T>& a = *static_cast<const AdvArgs<T>*>(args);
+#if G_SCHEME == 1
+    return launch_mhm<T, G_RECON, G_SOLVER, NV, EXT>(a, st, launches);
+#elif defined(GAMER_HAVE_CTU)
+    return launch_ctu<T, G_RECON, G_SOLVER, NV, EXT>(a, st, launches);
+#else
+    (void)a; (void)st; (void)launches;
+    return cudaErrorNotSupported;
+#endif
+}
+
+// prec = 4|8, nsc = 0|1, ext = 0|1 (nsc = 1 implies ext)
+cudaError_t G_NAME(int prec, int nsc, int ext, const void* args, cudaStream_t st, int* launches) {
+    if (prec == 4) {
+        if (nsc) return go<float, 6, true>(args, st, launches);
+        return ext ? go<float, 5, true>(args, st, launches) : go<float, 5, false>(args, st, launches);
+    }
+    if (nsc) return go<double, 6, true>(args, st, launches);
+    return ext ? go<double, 5, true>(args, st, launches) : go<double, 5, false>(args, st, launches);
+}
+
+}  // namespace gamer

@@ -1,0 +1,36 @@
+// launch.cuh -- host-side launch helpers: tile height selection by shared-memory fit, attribute setup.
+#pragma once
+#include "mhm_kernel.cuh"
+#ifdef GAMER_HAVE_CTU
+#include "ctu_kernel.cuh"
+#endif
+
+namespace gamer {
+
+constexpr size_t SMEM_LIMIT = 232448;   // 227 KB opt-in maximum per CTA on sm_100
+
+template <typename T, int RECON, int NV>
+constexpr int mhm_tile() {
+    return MhmSmem<T, RECON, NV, 16>::BYTES <= SMEM_LIMIT ? 16 : (MhmSmem<T, RECON, NV, 8>::BYTES <= SMEM_LIMIT ? 8 : 4);
+}
+
+template <typename T, int RECON, int SOLVER, int NV, bool EXT>
+cudaError_t launch_mhm(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
+    constexpr int TY = mhm_tile<T, RECON, NV>();
+    using G = Geo<TY>;
+    using S = MhmSmem<T, RECON, NV, TY>;
+    static_assert(S::BYTES <= SMEM_LIMIT, "tile does not fit in shared memory");
+    auto kern = mhm_kernel<T, RECON, SOLVER, NV, EXT, TY>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::BYTES);
+    if (e != cudaSuccess) return e;
+    if (G::NTILE > 1 && a.speed) {
+        e = cudaMemsetAsync(a.speed, 0, sizeof(T) * a.n_groups, st);
+        if (e != cudaSuccess) return e;
+    }
+    const long long grid = a.n_groups * G::NTILE;
+    kern<<<(unsigned)grid, G::NT, S::BYTES, st>>>(a);
+    *launches += 1;
+    return cudaGetLastError();
+}
+
+}  // namespace gamer

@@ -1,0 +1,241 @@
+// mhm_kernel.cuh -- MUSCL-Hancock (MHM; Toro 2009 sect. 14.4/16.5) patch-group kernel.
+//
+// Per plane kk = -1..16 of the tile (2 block barriers per plane):
+//   S1  predictor : PLM/PPM face values of the "plus"-shaped cell set of the plane (the cells whose
+//                   face states a final flux needs), Hancock half-step with the cell's own face
+//                   fluxes in all three directions, conversion back to primitives -> es / zp (smem)
+//   S2  Riemann   : x/y faces of plane kk, z faces between kk-1 and kk -> fx/fy/fz (smem) and the
+//                   patch-boundary planes of flux_out;  meanwhile the next staged plane -> primitives
+//   S3  update    : thread (i,j) finishes cell (i,j,kk-1) (needs F_z at kk-1/2), applies the closing
+//                   step, writes `out`, tracks the CFL maximum; then keeps (dFx+dFy) and F_z(kk-1/2)
+//                   of plane kk in registers;  one thread re-arms the freed TMA stage.
+#pragma once
+#include "hydro_close.cuh"
+
+namespace gamer {
+
+template <typename T, int RECON, int NV, int TY> struct MhmSmem {
+    using G = Geo<TY>;
+    static constexpr int R = RECON == PPM ? 2 : 1;
+    static constexpr int PR = 2 * R + 1;
+    static constexpr int RAW = 0;                                   // [2][NV][PLN]
+    static constexpr int PRIM = RAW + 2 * NV * G::PLN;              // [PR][NV][PLN]
+    static constexpr int ES = PRIM + PR * NV * G::PLN;              // [5][NV][EPL]
+    static constexpr int ZP = ES + 5 * NV * G::EPL;                 // [2][NV][NFZ]
+    static constexpr int FX = ZP + 2 * NV * G::NFZ;
+    static constexpr int FY = FX + NV * G::NFX;
+    static constexpr int FZ = FY + NV * G::NFY;
+    static constexpr int END = FZ + NV * G::NFZ;
+    static constexpr size_t BYTES = 16 + (size_t)END * sizeof(T);  // 2 mbarriers first
+};
+
+template <typename T, int RECON, int SOLVER, int NV, bool EXT, int TY>
+__global__ void __launch_bounds__(16 * TY) mhm_kernel(const AdvArgs<T> a) {
+    using G = Geo<TY>;
+    using S = MhmSmem<T, RECON, NV, TY>;
+    constexpr int R = S::R, PR = S::PR;
+    constexpr int NPL = 18 + 2 * R;      // staged planes: padded 2-R .. 19+R
+    constexpr int PF = 2 - R;
+
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw);
+    T* sm = reinterpret_cast<T*>(smem_raw + 16);
+    T* raw = sm + S::RAW;
+    T* prim = sm + S::PRIM;
+    T* es = sm + S::ES;
+    T* zp = sm + S::ZP;
+    T* fx = sm + S::FX;
+    T* fy = sm + S::FY;
+    T* fz = sm + S::FZ;
+
+    const int tid = threadIdx.x;
+    const long long tile = blockIdx.x;
+    const long long g = tile / G::NTILE;
+    const int j0 = (int)(tile % G::NTILE) * TY;
+    const T* gin = a.in + (size_t)g * NV * NPC;
+    T* gout = a.out + (size_t)g * NV * (PS * PS * PS);
+    T* gflux = a.flux ? a.flux + (size_t)g * 9 * NV * (PS * PS) : nullptr;
+    const Phys<T> ph = make_phys<T>(a);
+
+    if (tid == 0) {
+        mbar_init(&bars[0], 1);
+        mbar_init(&bars[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    if (tid == 0) {
+        issue_plane<T, NV, TY>(gin, j0, PF + 0, raw, &bars[0]);
+        issue_plane<T, NV, TY>(gin, j0, PF + 1, raw + NV * G::PLN, &bars[1]);
+    }
+    // prologue: fill the primitive ring with staged planes n = 0 .. 2R
+    for (int n = 0; n <= 2 * R; ++n) {
+        mbar_wait(&bars[n & 1], (n >> 1) & 1);
+        convert_plane<T, NV, EXT, TY>(raw + (n & 1) * NV * G::PLN, prim + ((PF + n) % PR) * NV * G::PLN, ph, tid);
+        __syncthreads();
+        if (tid == 0 && n + 2 < NPL) issue_plane<T, NV, TY>(gin, j0, PF + n + 2, raw + (n & 1) * NV * G::PLN, &bars[n & 1]);
+    }
+
+    // per-thread cell of the update stage
+    const int ci = tid & 15, cj = tid >> 4;
+    T sxy[NV], fzm[NV];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) { sxy[v] = T(0); fzm[v] = T(0); }
+    T smax = T(0);
+    Counters cnt = {0, 0, 0, 0, 0};
+
+    for (int kk = -1; kk <= PS; ++kk) {
+        // ------------------------------------------------------------------ S1: predictor
+        {
+            const int pc = kk + NGH;   // padded plane index of kk
+            const T* Pz[2 * R + 1];
+#pragma unroll
+            for (int m = -R; m <= R; ++m) Pz[m + R] = prim + ((pc + m) % PR) * NV * G::PLN;
+            T* zcur = zp + (kk & 1) * NV * G::NFZ;
+            for (int t = tid; t < G::NPLUS; t += G::NT) {
+                int ei, ej;
+                if (t < 18 * TY) { ej = t / 18; ei = t - ej * 18; ej += 1; }
+                else { const int u = t - 18 * TY; ej = (u < 16) ? 0 : TY + 1; ei = 1 + (u & 15); }
+                const int c = (ej + 2) * NP + (ei + 2);
+                T Uf[3][2][NV], dU[NV];
+#pragma unroll
+                for (int d = 0; d < 3; ++d) {
+                    T Wm[NV], Wp[NV];
+#pragma unroll
+                    for (int v = 0; v < NV; ++v) {
+                        const T* q = Pz[R] + v * G::PLN + c;
+                        if (d == 0) face_values<T, RECON, EXT>(q, 1, Wm[v], Wp[v], ph);
+                        else if (d == 1) face_values<T, RECON, EXT>(q, NP, Wm[v], Wp[v], ph);
+                        else {
+                            const int o = v * G::PLN + c;
+                            if (RECON == PPM)
+                                face_values5<T, RECON, EXT>(Pz[0][o], Pz[R - 1][o], Pz[R][o], Pz[R + 1][o], Pz[2 * R][o], Wm[v], Wp[v], ph);
+                            else
+                                face_values5<T, RECON, EXT>(T(0), Pz[R - 1][o], Pz[R][o], Pz[R + 1][o], T(0), Wm[v], Wp[v], ph);
+                        }
+                    }
+                    T Fm[NV], Fp[NV];
+                    prim2cons<T, NV>(Wm, Uf[d][0], ph);
+                    prim2cons<T, NV>(Wp, Uf[d][1], ph);
+                    if (d == 0) { phys_flux<T, NV, 0>(Wm, Uf[d][0], Fm); phys_flux<T, NV, 0>(Wp, Uf[d][1], Fp); }
+                    if (d == 1) { phys_flux<T, NV, 1>(Wm, Uf[d][0], Fm); phys_flux<T, NV, 1>(Wp, Uf[d][1], Fp); }
+                    if (d == 2) { phys_flux<T, NV, 2>(Wm, Uf[d][0], Fm); phys_flux<T, NV, 2>(Wp, Uf[d][1], Fp); }
+#pragma unroll
+                    for (int v = 0; v < NV; ++v) dU[v] = (d == 0) ? (Fp[v] - Fm[v]) : dU[v] + (Fp[v] - Fm[v]);
+                }
+                // Hancock half step on all six face states, back to primitives, positivity check
+                T We[3][2][NV];
+                bool ok = true;
+#pragma unroll
+                for (int d = 0; d < 3; ++d)
+#pragma unroll
+                    for (int s = 0; s < 2; ++s) {
+                        T Ue[NV];
+#pragma unroll
+                        for (int v = 0; v < NV; ++v) Ue[v] = Uf[d][s][v] - ph.hlam * dU[v];
+                        cons2prim<T, NV>(Ue, We[d][s], ph);
+                        if (EXT && ph.floors) floor_prim(We[d][s], ph);
+                        ok = ok && (We[d][s][0] > T(0)) && (We[d][s][4] > T(0));
+                    }
+                if (!ok) {   // revert the cell's six states to the un-evolved face values
+                    cnt.reverted++;
+#pragma unroll
+                    for (int d = 0; d < 3; ++d)
+#pragma unroll
+                        for (int s = 0; s < 2; ++s) cons2prim<T, NV>(Uf[d][s], We[d][s], ph);
+                }
+                const int e = ej * G::EW + ei;
+                const bool inner = (ei >= 1 && ei <= 16 && ej >= 1 && ej <= TY);
+#pragma unroll
+                for (int v = 0; v < NV; ++v) {
+                    es[(0 * NV + v) * G::EPL + e] = We[0][0][v];
+                    es[(1 * NV + v) * G::EPL + e] = We[0][1][v];
+                    es[(2 * NV + v) * G::EPL + e] = We[1][0][v];
+                    es[(3 * NV + v) * G::EPL + e] = We[1][1][v];
+                    es[(4 * NV + v) * G::EPL + e] = We[2][0][v];
+                    if (inner) zcur[v * G::NFZ + (ej - 1) * 16 + (ei - 1)] = We[2][1][v];
+                }
+            }
+        }
+        __syncthreads();
+        // ------------------------------------------------------------------ S2: Riemann + convert next plane
+        cnt.roe_fb += riemann_plane<T, SOLVER, NV, TY>(es, zp + ((kk + 1) & 1) * NV * G::NFZ, fx, fy, fz, gflux, kk, j0, ph, tid);
+        {
+            const int n = kk + 2 + 2 * R;
+            if (n < NPL) {
+                mbar_wait(&bars[n & 1], (n >> 1) & 1);
+                convert_plane<T, NV, EXT, TY>(raw + (n & 1) * NV * G::PLN, prim + ((PF + n) % PR) * NV * G::PLN, ph, tid);
+            }
+        }
+        __syncthreads();
+        // ------------------------------------------------------------------ S3: update plane kk-1, prepare plane kk
+        if (tid == 0) {
+            const int n = kk + 4 + 2 * R;
+            if (n < NPL) issue_plane<T, NV, TY>(gin, j0, PF + n, raw + (n & 1) * NV * G::PLN, &bars[n & 1]);
+        }
+        if (kk >= 1) {
+            const int k = kk - 1;
+            const T* gcell = gin + (size_t)(k + NGH) * (NP * NP) + (j0 + cj + NGH) * NP + (ci + NGH);
+            T U[NV];
+#pragma unroll
+            for (int v = 0; v < NV; ++v) {
+                const T dfz = fz[v * G::NFZ + tid] - fzm[v];
+                U[v] = __ldg(gcell + (size_t)v * NPC) - ph.lam * (sxy[v] + dfz);
+            }
+            close_cell<T, SOLVER, NV, EXT>(U, gcell, cnt, ph);
+#pragma unroll
+            for (int v = 0; v < NV; ++v) gout[((size_t)v * PS + k) * (PS * PS) + (j0 + cj) * PS + ci] = U[v];
+            if (a.speed) {
+                const T s = signal_speed<T, NV, MHM, EXT>(U, ph);
+                if (s > smax) smax = s;
+            }
+        }
+        if (kk >= 0 && kk < PS) {
+#pragma unroll
+            for (int v = 0; v < NV; ++v) {
+                const T dfx = fx[v * G::NFX + cj * 17 + ci + 1] - fx[v * G::NFX + cj * 17 + ci];
+                const T dfy = fy[v * G::NFY + (cj + 1) * 16 + ci] - fy[v * G::NFY + cj * 16 + ci];
+                sxy[v] = dfx + dfy;
+                fzm[v] = fz[v * G::NFZ + tid];
+            }
+        }
+    }
+
+    // ---------------------------------------------------------------------- epilogue: reductions
+    __syncthreads();
+    T* red = sm;                       // reuse the raw stages (all TMA traffic has landed and been consumed)
+    if (a.speed) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const T other = __shfl_xor_sync(0xffffffffu, smax, o);
+            smax = other > smax ? other : smax;
+        }
+        if ((tid & 31) == 0) red[tid >> 5] = smax;
+        __syncthreads();
+        if (tid == 0) {
+            T m = red[0];
+            for (int w = 1; w < G::NT / 32; ++w) m = red[w] > m ? red[w] : m;
+            if (G::NTILE == 1) a.speed[g] = m;
+            else if (sizeof(T) == 4) atomicMax(reinterpret_cast<unsigned int*>(a.speed + g), __float_as_uint((float)m));
+            else atomicMax(reinterpret_cast<unsigned long long*>(a.speed + g), (unsigned long long)__double_as_longlong((double)m));
+        }
+    }
+    if (EXT) {
+        int c[5] = {cnt.roe_fb, cnt.reverted, cnt.first_order, cnt.dual_fix, cnt.unphys};
+#pragma unroll
+        for (int q = 0; q < 5; ++q) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) c[q] += __shfl_xor_sync(0xffffffffu, c[q], o);
+        }
+        if ((tid & 31) == 0) {
+            if (a.diag) {
+                if (c[0]) atomicAdd(a.diag + 0, c[0]);
+                if (c[1]) atomicAdd(a.diag + 1, c[1]);
+                if (c[2]) atomicAdd(a.diag + 2, c[2]);
+                if (c[3]) atomicAdd(a.diag + 3, c[3]);
+            }
+            if (a.n_unphys && c[4]) atomicAdd(a.n_unphys, c[4]);
+        }
+    }
+}
+
+}  // namespace gamer

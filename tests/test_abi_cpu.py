@@ -1,0 +1,84 @@
+"""CPU-side checks of the boundary: the C-ABI library loads without a GPU and exports every symbol that
+include/gamer_hydro.h declares; the binding mirrors the struct layout.  No compute calls."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def built_lib():
+    from paper_1712_07070_b200 import build
+    return ctypes.CDLL(build.build())
+
+
+def _declared_functions():
+    text = open(os.path.join(ROOT, "include", "gamer_hydro.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(gamer_[a-z_0-9]+)\s*\(", text)))
+
+
+def test_header_symbols_are_exported(built_lib):
+    names = _declared_functions()
+    assert "gamer_fluid_advance" in names and "gamer_cfl_dt" in names and len(names) >= 10
+    for n in names:
+        assert hasattr(built_lib, n), n
+
+
+def test_binding_lists_the_same_entry_points():
+    from paper_1712_07070_b200 import binding
+    assert sorted(binding.EXPORTS) == _declared_functions()
+
+
+def test_version_and_strerror_without_gpu(built_lib):
+    built_lib.gamer_strerror.restype = ctypes.c_char_p
+    assert built_lib.gamer_version() >= 100
+    assert built_lib.gamer_strerror(0) == b"success"
+    assert b"invalid" in built_lib.gamer_strerror(-1)
+
+
+def test_argument_validation_needs_no_gpu(built_lib):
+    """Bad arguments are rejected before any CUDA call (error behaviour stated in the header)."""
+    L = built_lib
+    i64, dbl, vp, ci = ctypes.c_int64, ctypes.c_double, ctypes.c_void_p, ctypes.c_int
+    L.gamer_fluid_advance.argtypes = [vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, ci, ci]
+    ok = (vp(4096), vp(8192), None)
+    assert L.gamer_fluid_advance(None, ok[1], None, 1, 0.1, 0.1, 1.4, 1, 1, 1, 4) == -1
+    assert L.gamer_fluid_advance(ok[0], ok[1], None, -1, 0.1, 0.1, 1.4, 1, 1, 1, 4) == -1
+    assert L.gamer_fluid_advance(ok[0], ok[1], None, 1, 0.0, 0.1, 1.4, 1, 1, 1, 4) == -1
+    assert L.gamer_fluid_advance(ok[0], ok[1], None, 1, float("nan"), 0.1, 1.4, 1, 1, 1, 4) == -1
+    assert L.gamer_fluid_advance(ok[0], ok[1], None, 1, 0.1, -1.0, 1.4, 1, 1, 1, 4) == -1
+    assert L.gamer_fluid_advance(ok[0], ok[1], None, 1, 0.1, 0.1, 1.0, 1, 1, 1, 4) == -1
+    assert L.gamer_fluid_advance(ok[0], ok[1], None, 1, 0.1, 0.1, 1.4, 3, 1, 1, 4) == -1
+    assert L.gamer_fluid_advance(ok[0], ok[1], None, 1, 0.1, 0.1, 1.4, 1, 0, 1, 4) == -1
+    assert L.gamer_fluid_advance(ok[0], ok[1], None, 1, 0.1, 0.1, 1.4, 1, 1, 4, 4) == -1
+    assert L.gamer_fluid_advance(ok[0], ok[1], None, 1, 0.1, 0.1, 1.4, 1, 1, 1, 2) == -1
+    assert L.gamer_fluid_advance(vp(4100), ok[1], None, 1, 0.1, 0.1, 1.4, 1, 1, 1, 4) == -1     # misaligned
+
+
+def test_opts_struct_layout_matches_header():
+    from paper_1712_07070_b200 import binding
+    fields = [f[0] for f in binding.gamer_opts._fields_]
+    text = open(os.path.join(ROOT, "include", "gamer_hydro.h")).read()
+    body = text[text.index("typedef struct gamer_opts {"):text.index("} gamer_opts;")]
+    body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
+    declared = []
+    for stmt in body.split("{", 1)[1].split(";"):
+        stmt = stmt.strip()
+        if not stmt:
+            continue
+        names = stmt.split(",")
+        declared.append(re.findall(r"[A-Za-z_0-9]+", names[0])[-1])
+        declared += [re.findall(r"[A-Za-z_0-9]+", n)[-1] for n in names[1:]]
+    assert declared == fields
+
+
+def test_binding_fails_loudly_without_library(monkeypatch, tmp_path):
+    from paper_1712_07070_b200 import binding
+    monkeypatch.setattr(binding, "_lib", None)
+    monkeypatch.setattr(binding, "LIB_PATH", str(tmp_path / "nope.so"))
+    with pytest.raises(binding.GamerError):
+        binding.lib()
