@@ -1,0 +1,330 @@
+#!/usr/bin/env python
+"""bench.py -- hydro cell-updates/s of the patch-group solver on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--scheme mhm|ctu] [--recon plm|ppm] [--riemann roe|hllc|hlle] [--precision fp32|fp64]
+                    [--groups G]
+
+A "step" is one pass of the whole hot path over one batch: gamer_fluid_advance_ex (stage, primitives,
+reconstruction, predictor, Riemann, update, boundary fluxes, fused per-group CFL maximum) followed by
+gamer_cfl_from_group_speed (dt for the next step).  Default workload = BASELINE.json configs[3]:
+32,768 patch groups (512^3 cells) of seeded Mach-1 log-normal turbulence, gamma = 5/3, fp32 MHM+PLM+Roe.
+Inputs (7 GB) are far larger than L2 (126 MB), so no L2 flush is needed between iterations.
+For N > 1 every rank owns its own 32,768 groups (weak scaling; groups are independent, the only exchange
+is the max-reduction of one scalar for dt).
+
+--impl reference times the fp64 CPU oracle (oracle/, test infrastructure) on a bounded sample.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+SCHEMES = {"mhm": 1, "ctu": 2}
+RECONS = {"plm": 1, "ppm": 2}
+SOLVERS = {"roe": 1, "hllc": 2, "hlle": 3}
+CELLS = 4096
+
+# algorithmic HBM bytes per cell update: padded read + interior write + 9 flux planes
+#   PLM needs 5*20^3 values in, PPM 5*22^3; out 5*16^3; flux 9*5*16^2; + 1 speed value per group
+def algorithmic_bytes_per_cell(recon, sz, nv=5):
+    n_in = nv * (20 ** 3 if recon == 1 else 22 ** 3)
+    return (n_in + nv * CELLS + 9 * nv * 256 + 1) * sz / CELLS
+
+
+# counted SASS FLOPs per cell update (FMA = 2; profiles/r01_flops.md), used for the ALU roofline
+FLOPS_PER_CELL = {}
+
+
+def load_flops():
+    p = os.path.join(ROOT, "profiles", "flops_per_cell.json")
+    if os.path.exists(p):
+        FLOPS_PER_CELL.update(json.load(open(p)))
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return d.get("hbm_gbs", 6650.0), d.get("sm_max_mhz", 1965.0), "measured"
+    return 6650.0, 1965.0, "fallback"
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.stop_flag = index, [], False
+
+    def run(self):
+        while not self.stop_flag:
+            try:
+                r = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                    "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5)
+                parts = [x.strip() for x in r.stdout.strip().split(",")]
+                if len(parts) >= 6:
+                    self.samples.append(parts)
+            except Exception:
+                pass
+            time.sleep(0.1)
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        mhz = sorted(float(s[0]) for s in self.samples)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(s[2 + i].lower().startswith("active") for s in self.samples)]
+        return {"sm_mhz": mhz[len(mhz) // 2], "sm_max_mhz": float(self.samples[0][1]), "reasons": reasons,
+                "samples": len(mhz)}
+
+
+def reference_arm(args):
+    """The fp64 CPU oracle, as it stands, on a bounded sample of the same workload (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import numpy as np
+    import torch
+    import oracle
+    from paper_1712_07070_b200 import inputs
+    scheme, recon, solver = SCHEMES[args.scheme], RECONS[args.recon], SOLVERS[args.riemann]
+    n_sample = 512                                                      # 2.1e6 cells, the paper's saturation size
+    f = inputs.turbulence_field(128, 7070, kmax=16, gamma=5.0 / 3.0)     # 512 groups of the same field family
+    padded = inputs.pack_periodic(f)
+    if args.precision == "fp32":
+        padded = padded.to(torch.float32).to(torch.float64)
+    p = padded.numpy()
+    dh = 1.0 / 512
+    dt = oracle.cfl_dt(inputs.interior(padded).contiguous().numpy(), dh, 5.0 / 3.0, 0.4, scheme)[0]
+    cores = os.cpu_count()
+    for _ in range(max(1, min(args.warmup, 1))):
+        oracle.fluid_advance(p, dt, dh, 5.0 / 3.0, scheme, recon, solver)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        r = oracle.fluid_advance(p, dt, dh, 5.0 / 3.0, scheme, recon, solver)
+        oracle.cfl_dt(r["out"], dh, 5.0 / 3.0, 0.4, scheme)
+    el = time.perf_counter() - t0
+    value = n_sample * CELLS * args.steps / el
+    sample = f"{n_sample} of 32768 patch groups (128^3 cells of the same field family), {args.steps} steps"
+    line = {"impl": "reference", "metric": "hydro cell-updates/sec", "value": value, "unit": "cells/s",
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": el / args.steps * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(args, n_sample),
+            "cpu_baseline": {"value": value, "unit": "cells/s", "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": "cells/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(args, groups):
+    return {"workload": "BASELINE.json configs[3]: seeded Mach-1 log-normal turbulence, gamma=5/3, 16^3 patch groups + 3 ghosts",
+            "patch_groups_per_gpu": groups, "cells_per_gpu": groups * CELLS,
+            "scheme": args.scheme.upper(), "recon": args.recon.upper(), "riemann": args.riemann.upper(),
+            "precision": args.precision, "parallelism": f"dp{args.gpus} (independent patch-group shards)",
+            "l2": "inputs (>= 7 GB at full size) exceed the 126 MB L2; no flush needed"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--scheme", default="mhm", choices=list(SCHEMES))
+    ap.add_argument("--recon", default="plm", choices=list(RECONS))
+    ap.add_argument("--riemann", default="roe", choices=list(SOLVERS))
+    ap.add_argument("--precision", default="fp32", choices=["fp32", "fp64"])
+    ap.add_argument("--groups", type=int, default=32768, help="patch groups per GPU (must be a cube of an integer)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        if args.steps > 5:
+            args.steps = 5
+        return reference_arm(args)
+
+    import torch
+    import torch.distributed as dist
+    from paper_1712_07070_b200 import binding as gb
+    from paper_1712_07070_b200 import inputs
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    gb.lib()                                      # fail loudly if the CUDA library is missing
+    load_flops()
+
+    scheme, recon, solver = SCHEMES[args.scheme], RECONS[args.recon], SOLVERS[args.riemann]
+    dtype = torch.float32 if args.precision == "fp32" else torch.float64
+    sz = 4 if dtype == torch.float32 else 8
+    gside = round(args.groups ** (1.0 / 3.0))
+    assert gside ** 3 == args.groups, "--groups must be a cube"
+    n = gside * PS_CELLS
+    gamma, dh, cfl = 5.0 / 3.0, 1.0 / n, (0.4 if scheme == 2 else 0.5)
+
+    # ---- synthetic input, built on the device (seed differs per rank: every rank owns its own box)
+    field = inputs.turbulence_field(n, 7070 + rank, kmax=16, gamma=gamma, device=dev)
+    u_in = inputs.pack_periodic(field, dtype=dtype)
+    del field
+    torch.cuda.empty_cache()
+    out, flux, speed = gb.alloc_outputs(u_in)
+    dt_dev = torch.zeros(1, dtype=torch.float64, device=dev)
+    gb.gamer_cfl_dt(inputs.interior(u_in[:64]).contiguous(), dh, gamma, cfl, scheme, None, dt_dev)   # a valid first dt
+    stream = torch.cuda.current_stream()
+    opts = gb.make_opts(stream=stream, dt_dev=dt_dev, group_speed_out=speed)
+
+    def step():
+        gb.gamer_fluid_advance_ex(u_in, out, flux, 1.0, dh, gamma, scheme, recon, solver, opts)
+        gb.gamer_cfl_from_group_speed(speed, dh, cfl, dt_dev, stream)
+        if world > 1:
+            dist.all_reduce(dt_dev, op=dist.ReduceOp.MIN)        # the one exchange: 1 scalar
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    l0 = gb.gamer_launch_count()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    kev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    ev[0].record(stream)
+    for i in range(args.steps):
+        kev[i][0].record(stream)
+        gb.gamer_fluid_advance_ex(u_in, out, flux, 1.0, dh, gamma, scheme, recon, solver, opts)
+        kev[i][1].record(stream)
+        gb.gamer_cfl_from_group_speed(speed, dh, cfl, dt_dev, stream)
+        if world > 1:
+            dist.all_reduce(dt_dev, op=dist.ReduceOp.MIN)
+        ev[i + 1].record(stream)
+    barrier()
+    launches = gb.gamer_launch_count() - l0
+    sampler.stop_flag = True
+    total_ms = ev[0].elapsed_time(ev[-1])
+    kern_ms = sum(a.elapsed_time(b) for a, b in kev) / args.steps
+    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms = t.item()
+    cells = args.groups * CELLS
+    value = world * cells * args.steps / (total_ms * 1e-3)
+    finite = bool(torch.isfinite(out).all().item()) and bool(torch.isfinite(dt_dev).all().item())
+
+    # ---- extra: the same loop with the device-side periodic ghost refresh included (NEXT-1 row)
+    refresh_value = None
+    if world == 1:
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        nref = max(2, min(5, args.steps))
+        a0.record(stream)
+        for _ in range(nref):
+            step()
+            gb.gamer_refresh_ghosts_periodic(out, u_in, gside, gside, gside, stream)
+        a1.record(stream)
+        torch.cuda.synchronize()
+        refresh_value = cells * nref / (a0.elapsed_time(a1) * 1e-3)
+        finite = finite and bool(torch.isfinite(u_in).all().item())
+
+    # ---- e2e: host buffers through the C ABI, copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        ge = min(args.groups, 8192)
+        h_in = torch.empty((ge,) + tuple(u_in.shape[1:]), dtype=dtype, pin_memory=True)
+        h_in.copy_(u_in[:ge])
+        h_out = torch.empty((ge,) + tuple(out.shape[1:]), dtype=dtype, pin_memory=True)
+        h_flux = torch.empty((ge,) + tuple(flux.shape[1:]), dtype=dtype, pin_memory=True)
+        h_speed = torch.empty((ge,), dtype=dtype, pin_memory=True)
+        dt_host = float(dt_dev.item())
+        torch.cuda.synchronize()
+        gb.gamer_fluid_advance_host(h_in, h_out, h_flux, h_speed, dt_host, dh, gamma, scheme, recon, solver)
+        ne = 3
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(ne):
+            gb.gamer_fluid_advance_host(h_in, h_out, h_flux, h_speed, dt_host, dh, gamma, scheme, recon, solver)
+            dt_host = cfl * dh / float(h_speed.max())
+        el = time.perf_counter() - t0
+        tt = torch.tensor([el], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        e2e = {"value": world * ge * CELLS * ne / tt.item(), "unit": "cells/s",
+               "h2d_bytes_per_step": h_in.numel() * sz,
+               "d2h_bytes_per_step": (h_out.numel() + h_flux.numel() + h_speed.numel()) * sz,
+               "patch_groups_per_step": ge, "steps": ne,
+               "api": "gamer_fluid_advance_host (pinned host buffers, chunked H2D -> kernel -> D2H on 3 streams)"}
+        del h_in, h_out, h_flux, h_speed
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    hbm_peak, sm_max, which = peaks()
+    bpc = algorithmic_bytes_per_cell(recon, sz)
+    key = f"{args.scheme}_{args.recon}_{args.riemann}_{args.precision}"
+    fpc = FLOPS_PER_CELL.get(key)
+    lanes = 128 if sz == 4 else 64
+    alu_peak = 148 * lanes * 2 * sm_max * 1e6 / 1e12          # TFLOP/s, DESIGN.md "Rooflines"
+    hbm_ach = bpc * cells / (kern_ms * 1e-3) / 1e9
+    roofline = {"kernel": "mhm_kernel" if scheme == 1 else "ctu_kernel"}
+    if fpc:
+        ach = fpc * cells / (kern_ms * 1e-3) / 1e12
+        roofline.update({"bound": "alu", "achieved": ach, "peak": alu_peak, "unit": "TFLOP/s", "frac": ach / alu_peak,
+                         "flops_per_cell": fpc, "peak_source": f"148 SMs x {lanes} lanes x 2 x {sm_max} MHz"})
+    else:
+        roofline.update({"bound": "hbm", "achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_ach / hbm_peak})
+    tr = FLOPS_PER_CELL.get(key + "_dram_bytes_per_cell")
+    roofline["traffic"] = tr * cells if tr else None
+    roofline["hbm"] = {"achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_ach / hbm_peak,
+                       "bytes_per_cell": bpc, "peak_source": which}
+    roofline["kernel_ms"] = kern_ms
+
+    cpu = None
+    if not args.no_cpu:
+        import oracle
+        ns = 1024
+        sample = u_in[:ns].to(torch.float64).cpu().numpy()
+        dtv = float(dt_dev.item())
+        oracle.fluid_advance(sample[:64], dtv, dh, gamma, scheme, recon, solver)
+        t0 = time.perf_counter()
+        reps = 0
+        while time.perf_counter() - t0 < 10.0 and reps < 50:
+            r = oracle.fluid_advance(sample, dtv, dh, gamma, scheme, recon, solver)
+            oracle.cfl_dt(r["out"], dh, gamma, cfl, scheme)
+            reps += 1
+        el = time.perf_counter() - t0
+        cpu = {"value": ns * CELLS * reps / el, "unit": "cells/s", "cores": os.cpu_count(), "kind": "oracle",
+               "sample": f"first {ns} of {args.groups} patch groups, {reps} passes, OpenMP over groups"}
+
+    line = {"metric": "hydro cell-updates/sec", "value": value, "unit": "cells/s", "n_gpus": world,
+            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32" if sz == 4 else "f64", "data": "synthetic",
+            "config": workload_config(args, args.groups), "clocks": sampler.summary(), "e2e": e2e,
+            "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
+            "with_ghost_refresh": refresh_value, "outputs_finite": finite,
+            "paper_context": "P100-PCIe fp32 ~2e8 cells/s incl. PCIe (PAPER.md L318-320); other hardware, not a target"}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+PS_CELLS = 16
+
+if __name__ == "__main__":
+    main()

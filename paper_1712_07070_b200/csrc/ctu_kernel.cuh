@@ -1,0 +1,327 @@
+// ctu_kernel.cuh -- corner-transport-upwind, 6 Riemann solves per cell (Colella 1990,
+// "similar to ATHENA", Stone et al. 2008; C_CFL <= 0.5, L168) as a z-streaming patch-group kernel.
+//
+// Iteration kk = -1..17 works on three planes at once (4 block barriers per iteration):
+//   T    (kk)   : PLM/PPM face values + characteristic tracing over dt/2 of every cell of plane kk
+//                 (18 x (TY+2) cells, three directions)                         -> ts[kk&1]
+//   R1z  (kk)   : first-pass z flux H* at kk-1/2 from ts[(kk-1)&1].z+ and ts[kk&1].z-  -> f1z[kk&1]
+//                 (meanwhile the next staged plane is converted to primitives)
+//   C    (kk-1) : transverse flux-gradient correction (coefficient dt/2dh, conserved variables) of
+//                 the face states of plane kk-1, in place, using F*x,G*y of plane kk-1 and H* at
+//                 kk-3/2, kk-1/2; corrected z+ also saved to zp[(kk-1)&1]
+//   R1xy (kk)   : first-pass F*x, G*y of plane kk (overwrite those of kk-1, now consumed)
+//   R2   (kk-1) : final Riemann pass of plane kk-1 (x, y faces; z faces at kk-3/2)  -> fx/fy/fz, flux_out
+//   U    (kk-2) : conservative update + closing step of plane kk-2 (thread-owned cell, registers)
+#pragma once
+#include "hydro_close.cuh"
+
+namespace gamer {
+
+template <typename T, int RECON, int NV, int TY> struct CtuSmem {
+    using G = Geo<TY>;
+    static constexpr int R = RECON == PPM ? 2 : 1;
+    static constexpr int PR = 2 * R + 1;
+    static constexpr int NF1X = 17 * G::EH, NF1Y = 18 * (G::EH - 1);
+    static constexpr int RAW = 0;                                   // [2][NV][PLN]
+    static constexpr int PRIM = RAW + 2 * NV * G::PLN;              // [PR][NV][PLN]
+    static constexpr int TS = PRIM + PR * NV * G::PLN;              // [2][6][NV][EPL]
+    static constexpr int F1X = TS + 2 * 6 * NV * G::EPL;            // [NV][NF1X]
+    static constexpr int F1Y = F1X + NV * NF1X;                     // [NV][NF1Y]
+    static constexpr int F1Z = F1Y + NV * NF1Y;                     // [2][NV][EPL]
+    static constexpr int ZP = F1Z + 2 * NV * G::EPL;                // [2][NV][NFZ]
+    static constexpr int FX = ZP + 2 * NV * G::NFZ;
+    static constexpr int FY = FX + NV * G::NFX;
+    static constexpr int FZ = FY + NV * G::NFY;
+    static constexpr int END = FZ + NV * G::NFZ;
+    static constexpr size_t BYTES = 16 + (size_t)END * sizeof(T);
+};
+
+// one first-pass Riemann solve: rotated loads from two state arrays, unrotated store
+template <typename T, int SOLVER, int NV>
+__device__ __forceinline__ int first_pass_face(const T* lp, int lidx, const T* rp, int ridx, int sstr, T* fp,
+                                               int fidx, int fstr, int d, const Phys<T>& ph) {
+    const int cn = 1 + d, c1 = 1 + (d + 1) % 3, c2 = 1 + (d + 2) % 3;
+    T WL[NV], WR[NV], F[NV];
+    WL[0] = lp[lidx];               WR[0] = rp[ridx];
+    WL[1] = lp[cn * sstr + lidx];   WR[1] = rp[cn * sstr + ridx];
+    WL[2] = lp[c1 * sstr + lidx];   WR[2] = rp[c1 * sstr + ridx];
+    WL[3] = lp[c2 * sstr + lidx];   WR[3] = rp[c2 * sstr + ridx];
+    WL[4] = lp[4 * sstr + lidx];    WR[4] = rp[4 * sstr + ridx];
+    if (NV > 5) { WL[NV - 1] = lp[(NV - 1) * sstr + lidx]; WR[NV - 1] = rp[(NV - 1) * sstr + ridx]; }
+    const int fb = riemann_flux<T, SOLVER, NV>(WL, WR, F, ph) ? 1 : 0;
+    fp[fidx] = F[0];
+    fp[cn * fstr + fidx] = F[1];
+    fp[c1 * fstr + fidx] = F[2];
+    fp[c2 * fstr + fidx] = F[3];
+    fp[4 * fstr + fidx] = F[4];
+    if (NV > 5) fp[(NV - 1) * fstr + fidx] = F[NV - 1];
+    return fb;
+}
+
+template <typename T, int RECON, int SOLVER, int NV, bool EXT, int TY, int NT>
+__global__ void __launch_bounds__(NT) ctu_kernel(const AdvArgs<T> a) {
+    using G = Geo<TY>;
+    using S = CtuSmem<T, RECON, NV, TY>;
+    constexpr int R = S::R, PR = S::PR;
+    constexpr int NPL = 18 + 2 * R;
+    constexpr int PF = 2 - R;
+    constexpr int EPL = G::EPL, EW = G::EW;
+
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw);
+    T* sm = reinterpret_cast<T*>(smem_raw + 16);
+    T* raw = sm + S::RAW;
+    T* prim = sm + S::PRIM;
+    T* ts = sm + S::TS;
+    T* f1x = sm + S::F1X;
+    T* f1y = sm + S::F1Y;
+    T* f1z = sm + S::F1Z;
+    T* zp = sm + S::ZP;
+    T* fx = sm + S::FX;
+    T* fy = sm + S::FY;
+    T* fz = sm + S::FZ;
+
+    const int tid = threadIdx.x;
+    const long long tile = blockIdx.x;
+    const long long g = tile / G::NTILE;
+    const int j0 = (int)(tile % G::NTILE) * TY;
+    const T* gin = a.in + (size_t)g * NV * NPC;
+    T* gout = a.out + (size_t)g * NV * (PS * PS * PS);
+    T* gflux = a.flux ? a.flux + (size_t)g * 9 * NV * (PS * PS) : nullptr;
+    const Phys<T> ph = make_phys<T>(a);
+
+    if (tid == 0) {
+        mbar_init(&bars[0], 1);
+        mbar_init(&bars[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    if (tid == 0) {
+        issue_plane<T, NV, TY>(gin, j0, PF + 0, raw, &bars[0]);
+        issue_plane<T, NV, TY>(gin, j0, PF + 1, raw + NV * G::PLN, &bars[1]);
+    }
+    for (int n = 0; n <= 2 * R; ++n) {
+        mbar_wait(&bars[n & 1], (n >> 1) & 1);
+        convert_plane<T, NV, EXT, TY, NT>(raw + (n & 1) * NV * G::PLN, prim + ((PF + n) % PR) * NV * G::PLN, ph, tid);
+        __syncthreads();
+        if (tid == 0 && n + 2 < NPL) issue_plane<T, NV, TY>(gin, j0, PF + n + 2, raw + (n & 1) * NV * G::PLN, &bars[n & 1]);
+    }
+
+    const bool owner = tid < G::NFZ;           // threads that own a cell column of the update
+    const int ci = tid & 15, cj = (tid >> 4) % TY;
+    T sxy[NV], fzm[NV];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) { sxy[v] = T(0); fzm[v] = T(0); }
+    T smax = T(0);
+    Counters cnt = {0, 0, 0, 0, 0};
+
+    for (int kk = -1; kk <= PS + 1; ++kk) {
+        T* tcur = ts + (kk & 1) * 6 * NV * EPL;            // plane kk
+        T* tprev = ts + ((kk + 1) & 1) * 6 * NV * EPL;     // plane kk-1
+        const int m = kk - 1;
+        // ------------------------------------------------------------------ T(kk)
+        if (kk <= PS) {
+            const int pc = kk + NGH;
+            const T* Pz[2 * R + 1];
+#pragma unroll
+            for (int q = -R; q <= R; ++q) Pz[q + R] = prim + ((pc + q) % PR) * NV * G::PLN;
+            for (int t = tid; t < EPL; t += NT) {
+                const int ej = t / EW, ei = t - ej * EW;
+                const int c = (ej + 2) * NP + (ei + 2);
+                T Wc[NV];
+#pragma unroll
+                for (int v = 0; v < NV; ++v) Wc[v] = Pz[R][v * G::PLN + c];
+#pragma unroll
+                for (int d = 0; d < 3; ++d) {
+                    const int cn = 1 + d, c1 = 1 + (d + 1) % 3, c2 = 1 + (d + 2) % 3;
+                    T wm[NV], wp[NV];
+#pragma unroll
+                    for (int v = 0; v < NV; ++v) {
+                        const T* q = Pz[R] + v * G::PLN + c;
+                        if (d == 0) face_values<T, RECON, EXT>(q, 1, wm[v], wp[v], ph);
+                        else if (d == 1) face_values<T, RECON, EXT>(q, NP, wm[v], wp[v], ph);
+                        else {
+                            const int o = v * G::PLN + c;
+                            if (RECON == PPM)
+                                face_values5<T, RECON, EXT>(Pz[0][o], Pz[R - 1][o], Pz[R][o], Pz[R + 1][o], Pz[2 * R][o], wm[v], wp[v], ph);
+                            else
+                                face_values5<T, RECON, EXT>(T(0), Pz[R - 1][o], Pz[R][o], Pz[R + 1][o], T(0), wm[v], wp[v], ph);
+                        }
+                    }
+                    // rotate so that the traced axis is "n"
+                    T Wr[NV], rm[NV], rp[NV], tm[NV], tp[NV];
+                    Wr[0] = Wc[0]; Wr[1] = Wc[cn]; Wr[2] = Wc[c1]; Wr[3] = Wc[c2]; Wr[4] = Wc[4];
+                    rm[0] = wm[0]; rm[1] = wm[cn]; rm[2] = wm[c1]; rm[3] = wm[c2]; rm[4] = wm[4];
+                    rp[0] = wp[0]; rp[1] = wp[cn]; rp[2] = wp[c1]; rp[3] = wp[c2]; rp[4] = wp[4];
+                    if (NV > 5) { Wr[NV - 1] = Wc[NV - 1]; rm[NV - 1] = wm[NV - 1]; rp[NV - 1] = wp[NV - 1]; }
+                    trace_cell<T, RECON, NV>(Wr, rm, rp, tm, tp, ph);
+                    if (EXT && ph.floors) { floor_prim(tm, ph); floor_prim(tp, ph); }
+                    if (!(tm[0] > T(0) && tm[4] > T(0) && tp[0] > T(0) && tp[4] > T(0))) {
+                        cnt.reverted++;
+#pragma unroll
+                        for (int v = 0; v < NV; ++v) { tm[v] = rm[v]; tp[v] = rp[v]; }
+                    }
+                    T* sm_ = tcur + (2 * d) * NV * EPL + t;
+                    T* sp_ = tcur + (2 * d + 1) * NV * EPL + t;
+                    sm_[0] = tm[0];        sp_[0] = tp[0];
+                    sm_[cn * EPL] = tm[1]; sp_[cn * EPL] = tp[1];
+                    sm_[c1 * EPL] = tm[2]; sp_[c1 * EPL] = tp[2];
+                    sm_[c2 * EPL] = tm[3]; sp_[c2 * EPL] = tp[3];
+                    sm_[4 * EPL] = tm[4];  sp_[4 * EPL] = tp[4];
+                    if (NV > 5) { sm_[(NV - 1) * EPL] = tm[NV - 1]; sp_[(NV - 1) * EPL] = tp[NV - 1]; }
+                }
+            }
+        }
+        __syncthreads();
+        // ------------------------------------------------------------------ R1z(kk) + convert
+        if (kk >= 0 && kk <= PS) {
+            T* hz = f1z + (kk & 1) * NV * EPL;
+            for (int t = tid; t < EPL; t += NT)
+                cnt.roe_fb += first_pass_face<T, SOLVER, NV>(tprev + 5 * NV * EPL, t, tcur + 4 * NV * EPL, t, EPL, hz, t, EPL, 2, ph);
+        }
+        {
+            const int n = kk + 2 + 2 * R;
+            if (n < NPL) {
+                mbar_wait(&bars[n & 1], (n >> 1) & 1);
+                convert_plane<T, NV, EXT, TY, NT>(raw + (n & 1) * NV * G::PLN, prim + ((PF + n) % PR) * NV * G::PLN, ph, tid);
+            }
+        }
+        __syncthreads();
+        // ------------------------------------------------------------------ C(kk-1)
+        if (m >= -1 && m <= PS) {
+            const bool mid = (m >= 0 && m < PS);            // x/y states are needed only in planes 0..15
+            const T* hlo = f1z + (m & 1) * NV * EPL;        // H* at m-1/2
+            const T* hhi = f1z + (kk & 1) * NV * EPL;       // H* at m+1/2
+            T* zsave = zp + (m & 1) * NV * G::NFZ;
+            for (int t = tid; t < G::NPLUS; t += NT) {
+                int ei, ej;
+                if (t < 18 * TY) { ej = t / 18; ei = t - ej * 18; ej += 1; }
+                else { const int u = t - 18 * TY; ej = (u < 16) ? 0 : TY + 1; ei = 1 + (u & 15); }
+                const int e = ej * EW + ei;
+                const bool rowin = (ej >= 1 && ej <= TY), colin = (ei >= 1 && ei <= 16);
+                T gx[NV], gy[NV], gz[NV];     // flux differences across the cell in x, y, z
+#pragma unroll
+                for (int v = 0; v < NV; ++v) {
+                    gx[v] = colin ? f1x[v * S::NF1X + ej * 17 + ei] - f1x[v * S::NF1X + ej * 17 + ei - 1] : T(0);
+                    gy[v] = rowin ? f1y[v * S::NF1Y + ej * 18 + ei] - f1y[v * S::NF1Y + (ej - 1) * 18 + ei] : T(0);
+                    gz[v] = mid ? hhi[v * EPL + e] - hlo[v * EPL + e] : T(0);
+                }
+#pragma unroll
+                for (int d = 0; d < 3; ++d) {
+                    const bool need = (d == 0) ? (rowin && mid) : (d == 1) ? (colin && mid) : (rowin && colin);
+                    if (!need) continue;
+                    const T* g1 = (d == 0) ? gy : (d == 1) ? gz : gx;     // d1 = (d+1)%3
+                    const T* g2 = (d == 0) ? gz : (d == 1) ? gx : gy;     // d2 = (d+2)%3
+#pragma unroll
+                    for (int s = 0; s < 2; ++s) {
+                        T* sp_ = tprev + (2 * d + s) * NV * EPL + e;
+                        T W[NV], U[NV], Wn[NV];
+#pragma unroll
+                        for (int v = 0; v < NV; ++v) W[v] = sp_[v * EPL];
+                        prim2cons<T, NV>(W, U, ph);
+#pragma unroll
+                        for (int v = 0; v < NV; ++v) U[v] = U[v] - ph.hlam * g1[v] - ph.hlam * g2[v];
+                        cons2prim<T, NV>(U, Wn, ph);
+                        if (EXT && ph.floors) floor_prim(Wn, ph);
+                        const bool ok = Wn[0] > T(0) && Wn[4] > T(0);
+                        if (!ok) cnt.reverted++;
+#pragma unroll
+                        for (int v = 0; v < NV; ++v) {
+                            const T val = ok ? Wn[v] : W[v];
+                            if (d == 2 && s == 1) zsave[v * G::NFZ + (ej - 1) * 16 + (ei - 1)] = val;
+                            else sp_[v * EPL] = val;
+                        }
+                    }
+                }
+            }
+        }
+        __syncthreads();
+        // ------------------------------------------------------------------ R1xy(kk) + R2(kk-1)
+        if (kk <= PS) {
+            for (int t = tid; t < S::NF1X + S::NF1Y; t += NT) {
+                if (t < S::NF1X) {
+                    const int ej = t / 17, ei = t - ej * 17;
+                    const int l = ej * EW + ei;
+                    cnt.roe_fb += first_pass_face<T, SOLVER, NV>(tcur + 1 * NV * EPL, l, tcur + 0 * NV * EPL, l + 1, EPL, f1x, t, S::NF1X, 0, ph);
+                } else {
+                    const int u = t - S::NF1X;      // = ej*18 + ei, ej in [0, EH-1)
+                    cnt.roe_fb += first_pass_face<T, SOLVER, NV>(tcur + 3 * NV * EPL, u, tcur + 2 * NV * EPL, u + EW, EPL, f1y, u, S::NF1Y, 1, ph);
+                }
+            }
+        }
+        if (m >= 0) cnt.roe_fb += riemann_plane<T, SOLVER, NV, TY, NT>(tprev, zp + ((m + 1) & 1) * NV * G::NFZ, fx, fy, fz, gflux, m, j0, ph, tid);
+        __syncthreads();
+        // ------------------------------------------------------------------ U(kk-2)
+        if (tid == 0) {
+            const int n = kk + 4 + 2 * R;
+            if (n < NPL) issue_plane<T, NV, TY>(gin, j0, PF + n, raw + (n & 1) * NV * G::PLN, &bars[n & 1]);
+        }
+        if (owner) {
+            if (m >= 1) {
+                const int k = m - 1;
+                const T* gcell = gin + (size_t)(k + NGH) * (NP * NP) + (j0 + cj + NGH) * NP + (ci + NGH);
+                T U[NV];
+#pragma unroll
+                for (int v = 0; v < NV; ++v) {
+                    const T dfz = fz[v * G::NFZ + tid] - fzm[v];
+                    U[v] = __ldg(gcell + (size_t)v * NPC) - ph.lam * (sxy[v] + dfz);
+                }
+                close_cell<T, SOLVER, NV, EXT>(U, gcell, cnt, ph);
+#pragma unroll
+                for (int v = 0; v < NV; ++v) gout[((size_t)v * PS + k) * (PS * PS) + (j0 + cj) * PS + ci] = U[v];
+                if (a.speed) {
+                    const T s = signal_speed<T, NV, CTU, EXT>(U, ph);
+                    if (s > smax) smax = s;
+                }
+            }
+            if (m >= 0 && m < PS) {
+#pragma unroll
+                for (int v = 0; v < NV; ++v) {
+                    const T dfx = fx[v * G::NFX + cj * 17 + ci + 1] - fx[v * G::NFX + cj * 17 + ci];
+                    const T dfy = fy[v * G::NFY + (cj + 1) * 16 + ci] - fy[v * G::NFY + cj * 16 + ci];
+                    sxy[v] = dfx + dfy;
+                    fzm[v] = fz[v * G::NFZ + tid];
+                }
+            }
+        }
+    }
+
+    // ---------------------------------------------------------------------- epilogue: reductions
+    __syncthreads();
+    T* red = sm;
+    if (a.speed) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const T other = __shfl_xor_sync(0xffffffffu, smax, o);
+            smax = other > smax ? other : smax;
+        }
+        if ((tid & 31) == 0) red[tid >> 5] = smax;
+        __syncthreads();
+        if (tid == 0) {
+            T mx = red[0];
+            for (int w = 1; w < NT / 32; ++w) mx = red[w] > mx ? red[w] : mx;
+            if (G::NTILE == 1) a.speed[g] = mx;
+            else if (sizeof(T) == 4) atomicMax(reinterpret_cast<unsigned int*>(a.speed + g), __float_as_uint((float)mx));
+            else atomicMax(reinterpret_cast<unsigned long long*>(a.speed + g), (unsigned long long)__double_as_longlong((double)mx));
+        }
+    }
+    if (EXT) {
+        int c[5] = {cnt.roe_fb, cnt.reverted, cnt.first_order, cnt.dual_fix, cnt.unphys};
+#pragma unroll
+        for (int q = 0; q < 5; ++q) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) c[q] += __shfl_xor_sync(0xffffffffu, c[q], o);
+        }
+        if ((tid & 31) == 0) {
+            if (a.diag) {
+                if (c[0]) atomicAdd(a.diag + 0, c[0]);
+                if (c[1]) atomicAdd(a.diag + 1, c[1]);
+                if (c[2]) atomicAdd(a.diag + 2, c[2]);
+                if (c[3]) atomicAdd(a.diag + 3, c[3]);
+            }
+            if (a.n_unphys && c[4]) atomicAdd(a.n_unphys, c[4]);
+        }
+    }
+}
+
+}  // namespace gamer

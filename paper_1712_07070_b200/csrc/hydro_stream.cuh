@@ -120,10 +120,10 @@ __device__ __forceinline__ void issue_plane(const T* gin, int j0, int p, T* raw_
 }
 
 // raw conserved plane -> primitive plane (O1), floors in extended mode
-template <typename T, int NV, bool EXT, int TY>
+template <typename T, int NV, bool EXT, int TY, int NT = Geo<TY>::NT>
 __device__ __forceinline__ void convert_plane(const T* raw, T* prim, const Phys<T>& ph, int tid) {
     using G = Geo<TY>;
-    for (int t = tid; t < G::PLN; t += G::NT) {
+    for (int t = tid; t < G::PLN; t += NT) {
         T U[NV], W[NV];
 #pragma unroll
         for (int v = 0; v < NV; ++v) U[v] = raw[v * G::PLN + t];
@@ -145,14 +145,14 @@ __device__ __forceinline__ void face_values5(T l2, T l1, T c, T r1, T r2, T& wm,
 // between planes kk-1 and kk).  States are primitive; es = [5][NV][EPL] (x-,x+,y-,y+,z-),
 // zprev = [NV][16*TY] (z+ of plane kk-1).  Writes fx/fy/fz and the patch-boundary planes of flux_out.
 // ---------------------------------------------------------------------------------------------
-template <typename T, int SOLVER, int NV, int TY>
+template <typename T, int SOLVER, int NV, int TY, int NT = Geo<TY>::NT>
 __device__ __forceinline__ int riemann_plane(const T* es, const T* zprev, T* fx, T* fy, T* fz, T* gflux,
                                              int kk, int j0, const Phys<T>& ph, int tid) {
     using G = Geo<TY>;
     int nfb = 0;
     const int f_lo = (kk >= 0 && kk < PS) ? 0 : G::NFX + G::NFY;
     const int f_hi = (kk >= 0 && kk <= PS) ? G::NF : 0;
-    for (int f = f_lo + tid; f < f_hi; f += G::NT) {
+    for (int f = f_lo + tid; f < f_hi; f += NT) {
         int d, lidx, ridx, lstr, fidx, fstr, gp, ga, gb;
         const T *lp, *rp;
         T* fp;

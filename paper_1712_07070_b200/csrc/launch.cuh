@@ -33,4 +33,31 @@ cudaError_t launch_mhm(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
     return cudaGetLastError();
 }
 
+#ifdef GAMER_HAVE_CTU
+template <typename T, int RECON, int NV>
+constexpr int ctu_tile() {
+    return CtuSmem<T, RECON, NV, 16>::BYTES <= SMEM_LIMIT ? 16 : (CtuSmem<T, RECON, NV, 8>::BYTES <= SMEM_LIMIT ? 8 : 4);
+}
+
+template <typename T, int RECON, int SOLVER, int NV, bool EXT>
+cudaError_t launch_ctu(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
+    constexpr int TY = ctu_tile<T, RECON, NV>();
+    constexpr int NT = (sizeof(T) == 4 ? 32 : 16) * TY < 128 ? 128 : (sizeof(T) == 4 ? 32 : 16) * TY;
+    using G = Geo<TY>;
+    using S = CtuSmem<T, RECON, NV, TY>;
+    static_assert(S::BYTES <= SMEM_LIMIT, "tile does not fit in shared memory");
+    auto kern = ctu_kernel<T, RECON, SOLVER, NV, EXT, TY, NT>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::BYTES);
+    if (e != cudaSuccess) return e;
+    if (G::NTILE > 1 && a.speed) {
+        e = cudaMemsetAsync(a.speed, 0, sizeof(T) * a.n_groups, st);
+        if (e != cudaSuccess) return e;
+    }
+    const long long grid = a.n_groups * G::NTILE;
+    kern<<<(unsigned)grid, NT, S::BYTES, st>>>(a);
+    *launches += 1;
+    return cudaGetLastError();
+}
+#endif
+
 }  // namespace gamer
