@@ -172,11 +172,11 @@ extern "C" int gamer_refresh_ghosts_periodic(const void* u, void* in, int gz, in
     const long long ng = (long long)gz * gy * gx;
     if (ng * nvar > 0x7fffffff) return GAMER_EUNSUPPORTED;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    const dim3 grid((unsigned)(ng * nvar), NP);
+    const unsigned grid = (unsigned)(ng * nvar);
     if (precision == GAMER_FP32)
-        refresh_periodic_kernel<float><<<grid, 512, 0, st>>>(static_cast<const float*>(u), static_cast<float*>(in), gz, gy, gx, nvar);
+        refresh_periodic_kernel<float><<<grid, 256, 0, st>>>(static_cast<const float*>(u), static_cast<float*>(in), gz, gy, gx, nvar);
     else
-        refresh_periodic_kernel<double><<<grid, 512, 0, st>>>(static_cast<const double*>(u), static_cast<double*>(in), gz, gy, gx, nvar);
+        refresh_periodic_kernel<double><<<grid, 256, 0, st>>>(static_cast<const double*>(u), static_cast<double*>(in), gz, gy, gx, nvar);
     g_launches += 1;
     return cudaGetLastError() == cudaSuccess ? GAMER_OK : GAMER_ECUDA;
 }

@@ -95,23 +95,39 @@ __global__ void __launch_bounds__(1024) group_max_kernel(const T* speed, long lo
 __global__ void finish_dt_kernel(double* acc, double cfl_dh) { *acc = cfl_dh / *acc; }
 
 // padded `in` batch from the unpadded `u` batch of a periodic box of gz x gy x gx groups.
-// grid = (n_groups*nvar, 22 planes), 512 threads cover the 22 x 22 plane.
+// One CTA per (group, variable): 256 threads own two (row, column) positions of the 22 x 22 plane each and
+// walk the 22 planes; the wrapped source offset splits into a per-thread (x,y) part computed once and a
+// per-plane (z) part that is uniform over the CTA.  Writes are fully contiguous (a padded variable block is
+// 10,648 consecutive elements), reads are 16-element rows of the neighbours' unpadded blocks.
 template <typename T>
-__global__ void __launch_bounds__(512) refresh_periodic_kernel(const T* __restrict__ u, T* __restrict__ in, int gz,
+__global__ void __launch_bounds__(256) refresh_periodic_kernel(const T* __restrict__ u, T* __restrict__ in, int gz,
                                                                int gy, int gx, int nvar) {
-    const int t = threadIdx.x;
-    if (t >= NP * NP) return;
     const long long gv = blockIdx.x;
     const long long g = gv / nvar;
-    const int v = (int)(gv % nvar);
-    const int pk = blockIdx.y, pj = t / NP, pi = t - pj * NP;
+    const int v = (int)(gv - g * nvar);
     const int bx = (int)(g % gx), by = (int)((g / gx) % gy), bz = (int)(g / ((long long)gx * gy));
-    int x = bx * PS + pi - NGH, y = by * PS + pj - NGH, z = bz * PS + pk - NGH;
-    const int nx = gx * PS, ny = gy * PS, nz = gz * PS;
-    x = (x + nx) % nx; y = (y + ny) % ny; z = (z + nz) % nz;
-    const long long sg = ((long long)(z / PS) * gy + (y / PS)) * gx + (x / PS);
-    const T val = u[((size_t)sg * nvar + v) * (PS * PS * PS) + ((z % PS) * PS + (y % PS)) * PS + (x % PS)];
-    in[((size_t)g * nvar + v) * NPC + ((size_t)pk * NP + pj) * NP + pi] = val;
+    const size_t gstride = (size_t)nvar * (PS * PS * PS);
+    size_t offxy[2];
+    bool live[2];
+#pragma unroll
+    for (int r = 0; r < 2; ++r) {
+        const int t = threadIdx.x + r * 256;
+        live[r] = t < NP * NP;
+        const int pj = t / NP, pi = t - pj * NP;
+        int sx = bx, lx = pi - NGH, sy = by, ly = pj - NGH;
+        if (lx < 0) { lx += PS; sx = sx == 0 ? gx - 1 : sx - 1; } else if (lx >= PS) { lx -= PS; sx = sx == gx - 1 ? 0 : sx + 1; }
+        if (ly < 0) { ly += PS; sy = sy == 0 ? gy - 1 : sy - 1; } else if (ly >= PS) { ly -= PS; sy = sy == gy - 1 ? 0 : sy + 1; }
+        offxy[r] = ((size_t)sy * gx + sx) * gstride + (size_t)v * (PS * PS * PS) + ly * PS + lx;
+    }
+    T* dst = in + ((size_t)g * nvar + v) * NPC;
+    for (int pk = 0; pk < NP; ++pk) {
+        int sz = bz, lz = pk - NGH;
+        if (lz < 0) { lz += PS; sz = sz == 0 ? gz - 1 : sz - 1; } else if (lz >= PS) { lz -= PS; sz = sz == gz - 1 ? 0 : sz + 1; }
+        const size_t offz = (size_t)sz * gy * gx * gstride + (size_t)lz * (PS * PS);
+#pragma unroll
+        for (int r = 0; r < 2; ++r)
+            if (live[r]) dst[pk * (NP * NP) + threadIdx.x + r * 256] = __ldg(u + offz + offxy[r]);
+    }
 }
 
 }  // namespace gamer

@@ -116,8 +116,10 @@ __device__ __forceinline__ T limited_slope(T dL, T dR, const Phys<T>& ph) {
         return prod * (dL + dR) * Ops<T>::rcp(dL * dL + dR * dR);
     }
     const T aL = Ops<T>::abs(dL), aR = Ops<T>::abs(dR);
-    T m = ph.theta * Ops<T>::min(aL, aR);
-    m = Ops<T>::min(m, T(0.5) * Ops<T>::abs(dL + dR));
+    T m = Ops<T>::min(aL, aR);
+    // theta == 1 (plain minmod): |dL+dR|/2 >= min(|dL|,|dR|) holds exactly in floating point for equal
+    // signs (rounding is monotonic), so the centred term can never win and is skipped
+    if (ph.theta != T(1)) m = Ops<T>::min(ph.theta * m, T(0.5) * Ops<T>::abs(dL + dR));
     m = Ops<T>::copysign(m, dR);
     return prod > T(0) ? m : T(0);
 }

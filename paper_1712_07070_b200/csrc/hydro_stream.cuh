@@ -208,4 +208,69 @@ __device__ __forceinline__ int riemann_plane(const T* es, const T* zprev, T* fx,
     return nfb;
 }
 
+// ---------------------------------------------------------------------------------------------
+// Rotated storage (used by the MHM kernel): a face-state array of axis d holds (rho, v_d, v_{d+1},
+// v_{d+2}, P [, q]) -- the producer rotates at compile time -- and the flux array holds the rotated flux,
+// so the Riemann stage needs no per-face rotation arithmetic.  Face f of the flat list (x: 17*TY, y:
+// 16*(TY+1), z: 16*TY) reads its left / right state at offsets lo / ro from `es` (variable stride EPL)
+// and writes F[k*NF + f].  rot_index(d, v) = position of natural variable v in the rotation of axis d.
+// ---------------------------------------------------------------------------------------------
+__host__ __device__ constexpr int rot_index(int d, int v) { return (v >= 1 && v <= 3) ? 1 + ((v - 1 - d + 3) % 3) : v; }
+__host__ __device__ constexpr int nat_index(int d, int k) { return (k >= 1 && k <= 3) ? 1 + ((k - 1 + d) % 3) : k; }
+
+// packed (lo | ro << 16) descriptor of face f; z faces get lo relative to the z+ buffer of parity 0
+template <int NV, int TY>
+__device__ __forceinline__ unsigned face_descriptor(int f, int zp_off) {
+    using G = Geo<TY>;
+    int lo, ro;
+    if (f < G::NFX) {
+        const int jj = f / 17, ii = f - jj * 17;
+        lo = 1 * NV * G::EPL + (jj + 1) * G::EW + ii;
+        ro = 0 * NV * G::EPL + (jj + 1) * G::EW + ii + 1;
+    } else if (f < G::NFX + G::NFY) {
+        const int g = f - G::NFX;
+        const int jj = g >> 4, ii = g & 15;
+        lo = 3 * NV * G::EPL + jj * G::EW + ii + 1;
+        ro = 2 * NV * G::EPL + (jj + 1) * G::EW + ii + 1;
+    } else {
+        const int g = f - G::NFX - G::NFY;
+        const int jj = g >> 4, ii = g & 15;
+        lo = zp_off + (jj + 1) * G::EW + ii + 1;
+        ro = 4 * NV * G::EPL + (jj + 1) * G::EW + ii + 1;
+    }
+    return (unsigned)lo | ((unsigned)ro << 16);
+}
+
+template <typename T, int SOLVER, int NV, int TY>
+__device__ __forceinline__ int riemann_face_rot(const T* es, T* fl, T* gflux, unsigned desc, int f, int zpar_off,
+                                                int kk, int j0, const Phys<T>& ph) {
+    using G = Geo<TY>;
+    const bool isz = f >= G::NFX + G::NFY;
+    const int lo = (int)(desc & 0xffffu) + (isz ? zpar_off : 0);
+    const int ro = (int)(desc >> 16);
+    T WL[NV], WR[NV], F[NV];
+#pragma unroll
+    for (int k = 0; k < NV; ++k) { WL[k] = es[k * G::EPL + lo]; WR[k] = es[k * G::EPL + ro]; }
+    const int fb = riemann_flux<T, SOLVER, NV>(WL, WR, F, ph) ? 1 : 0;
+#pragma unroll
+    for (int k = 0; k < NV; ++k) fl[k * G::NF + f] = F[k];
+    if (gflux != nullptr) {   // faces 0, 8, 16 of the axis are patch boundaries
+        int d, gp, ga, gb;
+        if (f < G::NFX) { const int jj = f / 17, ii = f - jj * 17; d = 0; gp = ii; ga = j0 + jj; gb = kk; }
+        else if (!isz) { const int g = f - G::NFX; d = 1; gp = j0 + (g >> 4); ga = g & 15; gb = kk; }
+        else { const int g = f - G::NFX - G::NFY; d = 2; gp = kk; ga = g & 15; gb = j0 + (g >> 4); }
+        if ((gp & 7) == 0) {
+            T* q = gflux + ((size_t)(d * 3 + (gp >> 3)) * NV) * (PS * PS) + gb * PS + ga;
+            const int cn = 1 + d, c1 = 1 + (d + 1) % 3, c2 = 1 + (d + 2) % 3;
+            q[0] = F[0];
+            q[(size_t)cn * (PS * PS)] = F[1];
+            q[(size_t)c1 * (PS * PS)] = F[2];
+            q[(size_t)c2 * (PS * PS)] = F[3];
+            q[(size_t)4 * (PS * PS)] = F[4];
+            if (NV > 5) q[(size_t)(NV - 1) * (PS * PS)] = F[NV - 1];
+        }
+    }
+    return fb;
+}
+
 }  // namespace gamer

@@ -1,5 +1,6 @@
 // launch.cuh -- host-side launch helpers: tile height selection by shared-memory fit, attribute setup.
 #pragma once
+#include <cstdlib>
 #include "mhm_kernel.cuh"
 #ifdef GAMER_HAVE_CTU
 #include "ctu_kernel.cuh"
@@ -20,7 +21,10 @@ cudaError_t launch_mhm(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
     using G = Geo<TY>;
     using S = MhmSmem<T, RECON, NV, TY>;
     static_assert(S::BYTES <= SMEM_LIMIT, "tile does not fit in shared memory");
-    auto kern = mhm_kernel<T, RECON, SOLVER, NV, EXT, TY>;
+    // 320 threads = the 320 predictor cells of a plane (one each), 800 faces = 2.5 rounds; see DESIGN.md
+    constexpr int NT = TY == 16 ? 320 : G::NT < 128 ? 128 : G::NT;
+    constexpr int MINB = (sizeof(T) == 4 && TY == 16 && NV == 5 && RECON == PLM) ? 2 : 1;
+    auto kern = mhm_kernel<T, RECON, SOLVER, NV, EXT, TY, NT, MINB>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::BYTES);
     if (e != cudaSuccess) return e;
     if (G::NTILE > 1 && a.speed) {
@@ -28,7 +32,7 @@ cudaError_t launch_mhm(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
         if (e != cudaSuccess) return e;
     }
     const long long grid = a.n_groups * G::NTILE;
-    kern<<<(unsigned)grid, G::NT, S::BYTES, st>>>(a);
+    kern<<<(unsigned)grid, NT, S::BYTES, st>>>(a);
     *launches += 1;
     return cudaGetLastError();
 }
@@ -39,9 +43,8 @@ constexpr int ctu_tile() {
     return CtuSmem<T, RECON, NV, 16>::BYTES <= SMEM_LIMIT ? 16 : (CtuSmem<T, RECON, NV, 8>::BYTES <= SMEM_LIMIT ? 8 : 4);
 }
 
-template <typename T, int RECON, int SOLVER, int NV, bool EXT>
-cudaError_t launch_ctu(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
-    constexpr int TY = ctu_tile<T, RECON, NV>();
+template <typename T, int RECON, int SOLVER, int NV, bool EXT, int TY>
+cudaError_t launch_ctu_ty(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
     constexpr int NT = (sizeof(T) == 4 ? 32 : 16) * TY < 128 ? 128 : (sizeof(T) == 4 ? 32 : 16) * TY;
     using G = Geo<TY>;
     using S = CtuSmem<T, RECON, NV, TY>;
@@ -57,6 +60,18 @@ cudaError_t launch_ctu(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
     kern<<<(unsigned)grid, NT, S::BYTES, st>>>(a);
     *launches += 1;
     return cudaGetLastError();
+}
+
+template <typename T, int RECON, int SOLVER, int NV, bool EXT>
+cudaError_t launch_ctu(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
+    constexpr int TY = ctu_tile<T, RECON, NV>();
+#ifdef GAMER_EXPERIMENT_TY
+    if constexpr (TY == 16 && !EXT && sizeof(T) == 4) {
+        static const char* env = getenv("GAMER_CTU_TY");
+        if (env && env[0] == '8') return launch_ctu_ty<T, RECON, SOLVER, NV, EXT, 8>(a, st, launches);
+    }
+#endif
+    return launch_ctu_ty<T, RECON, SOLVER, NV, EXT, TY>(a, st, launches);
 }
 #endif
 

@@ -21,16 +21,14 @@ template <typename T, int RECON, int NV, int TY> struct MhmSmem {
     static constexpr int RAW = 0;                                   // [2][NV][PLN]
     static constexpr int PRIM = RAW + 2 * NV * G::PLN;              // [PR][NV][PLN]
     static constexpr int ES = PRIM + PR * NV * G::PLN;              // [5][NV][EPL]
-    static constexpr int ZP = ES + 5 * NV * G::EPL;                 // [2][NV][NFZ]
-    static constexpr int FX = ZP + 2 * NV * G::NFZ;
-    static constexpr int FY = FX + NV * G::NFX;
-    static constexpr int FZ = FY + NV * G::NFY;
-    static constexpr int END = FZ + NV * G::NFZ;
+    static constexpr int ZP = ES + 5 * NV * G::EPL;                 // [2][NV][EPL]  z+ of planes kk, kk-1
+    static constexpr int FL = ZP + 2 * NV * G::EPL;                 // [NV][NF]      rotated fluxes, flat face list
+    static constexpr int END = FL + NV * G::NF;
     static constexpr size_t BYTES = 16 + (size_t)END * sizeof(T);  // 2 mbarriers first
 };
 
-template <typename T, int RECON, int SOLVER, int NV, bool EXT, int TY>
-__global__ void __launch_bounds__(16 * TY) mhm_kernel(const AdvArgs<T> a) {
+template <typename T, int RECON, int SOLVER, int NV, bool EXT, int TY, int NT, int MINB>
+__global__ void __launch_bounds__(NT, MINB) mhm_kernel(const AdvArgs<T> a) {
     using G = Geo<TY>;
     using S = MhmSmem<T, RECON, NV, TY>;
     constexpr int R = S::R, PR = S::PR;
@@ -43,10 +41,7 @@ __global__ void __launch_bounds__(16 * TY) mhm_kernel(const AdvArgs<T> a) {
     T* raw = sm + S::RAW;
     T* prim = sm + S::PRIM;
     T* es = sm + S::ES;
-    T* zp = sm + S::ZP;
-    T* fx = sm + S::FX;
-    T* fy = sm + S::FY;
-    T* fz = sm + S::FZ;
+    T* fl = sm + S::FL;
 
     const int tid = threadIdx.x;
     const long long tile = blockIdx.x;
@@ -70,13 +65,23 @@ __global__ void __launch_bounds__(16 * TY) mhm_kernel(const AdvArgs<T> a) {
     // prologue: fill the primitive ring with staged planes n = 0 .. 2R
     for (int n = 0; n <= 2 * R; ++n) {
         mbar_wait(&bars[n & 1], (n >> 1) & 1);
-        convert_plane<T, NV, EXT, TY>(raw + (n & 1) * NV * G::PLN, prim + ((PF + n) % PR) * NV * G::PLN, ph, tid);
+        convert_plane<T, NV, EXT, TY, NT>(raw + (n & 1) * NV * G::PLN, prim + ((PF + n) % PR) * NV * G::PLN, ph, tid);
         __syncthreads();
         if (tid == 0 && n + 2 < NPL) issue_plane<T, NV, TY>(gin, j0, PF + n + 2, raw + (n & 1) * NV * G::PLN, &bars[n & 1]);
     }
 
     // per-thread cell of the update stage
-    const int ci = tid & 15, cj = tid >> 4;
+    const bool owner = tid < G::NFZ;               // threads that own a cell column of the update stage
+    const int ci = tid & 15, cj = (tid >> 4) % TY;
+    // the convert stage starts at the warps that get fewer Riemann faces, to balance the barrier interval
+    constexpr int CROT = (G::NF % NT) == 0 ? 0 : ((G::NF % NT + 31) / 32) * 32 % NT;
+    const int ctid = (tid + NT - CROT) % NT;
+    // loop-invariant face descriptors of this thread's Riemann rounds (f = tid + r*NT)
+    constexpr int NROUND = (G::NF + NT - 1) / NT;
+    constexpr int ZOFF = 5 * NV * G::EPL;          // offset of the z+ buffers relative to es
+    unsigned fdesc[NROUND];
+#pragma unroll
+    for (int r = 0; r < NROUND; ++r) fdesc[r] = face_descriptor<NV, TY>(tid + r * NT < G::NF ? tid + r * NT : 0, ZOFF);
     T sxy[NV], fzm[NV];
 #pragma unroll
     for (int v = 0; v < NV; ++v) { sxy[v] = T(0); fzm[v] = T(0); }
@@ -90,8 +95,8 @@ __global__ void __launch_bounds__(16 * TY) mhm_kernel(const AdvArgs<T> a) {
             const T* Pz[2 * R + 1];
 #pragma unroll
             for (int m = -R; m <= R; ++m) Pz[m + R] = prim + ((pc + m) % PR) * NV * G::PLN;
-            T* zcur = zp + (kk & 1) * NV * G::NFZ;
-            for (int t = tid; t < G::NPLUS; t += G::NT) {
+            T* zcur = es + ZOFF + (kk & 1) * NV * G::EPL;
+            for (int t = tid; t < G::NPLUS; t += NT) {
                 int ei, ej;
                 if (t < 18 * TY) { ej = t / 18; ei = t - ej * 18; ej += 1; }
                 else { const int u = t - 18 * TY; ej = (u < 16) ? 0 : TY + 1; ei = 1 + (u & 15); }
@@ -144,26 +149,36 @@ __global__ void __launch_bounds__(16 * TY) mhm_kernel(const AdvArgs<T> a) {
                         for (int s = 0; s < 2; ++s) cons2prim<T, NV>(Uf[d][s], We[d][s], ph);
                 }
                 const int e = ej * G::EW + ei;
-                const bool inner = (ei >= 1 && ei <= 16 && ej >= 1 && ej <= TY);
+                // rotated storage: array of axis d holds (rho, v_d, v_{d+1}, v_{d+2}, P [, q])
 #pragma unroll
-                for (int v = 0; v < NV; ++v) {
-                    es[(0 * NV + v) * G::EPL + e] = We[0][0][v];
-                    es[(1 * NV + v) * G::EPL + e] = We[0][1][v];
-                    es[(2 * NV + v) * G::EPL + e] = We[1][0][v];
-                    es[(3 * NV + v) * G::EPL + e] = We[1][1][v];
-                    es[(4 * NV + v) * G::EPL + e] = We[2][0][v];
-                    if (inner) zcur[v * G::NFZ + (ej - 1) * 16 + (ei - 1)] = We[2][1][v];
+                for (int k = 0; k < NV; ++k) {
+                    es[(0 * NV + k) * G::EPL + e] = We[0][0][nat_index(0, k)];
+                    es[(1 * NV + k) * G::EPL + e] = We[0][1][nat_index(0, k)];
+                    es[(2 * NV + k) * G::EPL + e] = We[1][0][nat_index(1, k)];
+                    es[(3 * NV + k) * G::EPL + e] = We[1][1][nat_index(1, k)];
+                    es[(4 * NV + k) * G::EPL + e] = We[2][0][nat_index(2, k)];
+                    zcur[k * G::EPL + e] = We[2][1][nat_index(2, k)];
                 }
             }
         }
         __syncthreads();
         // ------------------------------------------------------------------ S2: Riemann + convert next plane
-        cnt.roe_fb += riemann_plane<T, SOLVER, NV, TY>(es, zp + ((kk + 1) & 1) * NV * G::NFZ, fx, fy, fz, gflux, kk, j0, ph, tid);
+        {
+            const int f_lo = (kk >= 0 && kk < PS) ? 0 : G::NFX + G::NFY;
+            const int f_hi = (kk >= 0 && kk <= PS) ? G::NF : 0;
+            const int zpar = ((kk + 1) & 1) * NV * G::EPL;      // z+ states of plane kk-1
+#pragma unroll
+            for (int r = 0; r < NROUND; ++r) {
+                const int f = tid + r * NT;
+                if (f >= f_lo && f < f_hi)
+                    cnt.roe_fb += riemann_face_rot<T, SOLVER, NV, TY>(es, fl, gflux, fdesc[r], f, zpar, kk, j0, ph);
+            }
+        }
         {
             const int n = kk + 2 + 2 * R;
             if (n < NPL) {
                 mbar_wait(&bars[n & 1], (n >> 1) & 1);
-                convert_plane<T, NV, EXT, TY>(raw + (n & 1) * NV * G::PLN, prim + ((PF + n) % PR) * NV * G::PLN, ph, tid);
+                convert_plane<T, NV, EXT, TY, NT>(raw + (n & 1) * NV * G::PLN, prim + ((PF + n) % PR) * NV * G::PLN, ph, ctid);
             }
         }
         __syncthreads();
@@ -172,13 +187,13 @@ __global__ void __launch_bounds__(16 * TY) mhm_kernel(const AdvArgs<T> a) {
             const int n = kk + 4 + 2 * R;
             if (n < NPL) issue_plane<T, NV, TY>(gin, j0, PF + n, raw + (n & 1) * NV * G::PLN, &bars[n & 1]);
         }
-        if (kk >= 1) {
+        if (owner && kk >= 1) {
             const int k = kk - 1;
             const T* gcell = gin + (size_t)(k + NGH) * (NP * NP) + (j0 + cj + NGH) * NP + (ci + NGH);
             T U[NV];
 #pragma unroll
             for (int v = 0; v < NV; ++v) {
-                const T dfz = fz[v * G::NFZ + tid] - fzm[v];
+                const T dfz = fl[rot_index(2, v) * G::NF + G::NFX + G::NFY + tid] - fzm[v];
                 U[v] = __ldg(gcell + (size_t)v * NPC) - ph.lam * (sxy[v] + dfz);
             }
             close_cell<T, SOLVER, NV, EXT>(U, gcell, cnt, ph);
@@ -189,13 +204,15 @@ __global__ void __launch_bounds__(16 * TY) mhm_kernel(const AdvArgs<T> a) {
                 if (s > smax) smax = s;
             }
         }
-        if (kk >= 0 && kk < PS) {
+        if (owner && kk >= 0 && kk < PS) {
 #pragma unroll
             for (int v = 0; v < NV; ++v) {
-                const T dfx = fx[v * G::NFX + cj * 17 + ci + 1] - fx[v * G::NFX + cj * 17 + ci];
-                const T dfy = fy[v * G::NFY + (cj + 1) * 16 + ci] - fy[v * G::NFY + cj * 16 + ci];
+                const T* px = fl + rot_index(0, v) * G::NF + cj * 17 + ci;
+                const T* py = fl + rot_index(1, v) * G::NF + G::NFX + cj * 16 + ci;
+                const T dfx = px[1] - px[0];
+                const T dfy = py[16] - py[0];
                 sxy[v] = dfx + dfy;
-                fzm[v] = fz[v * G::NFZ + tid];
+                fzm[v] = fl[rot_index(2, v) * G::NF + G::NFX + G::NFY + tid];
             }
         }
     }
@@ -213,7 +230,7 @@ __global__ void __launch_bounds__(16 * TY) mhm_kernel(const AdvArgs<T> a) {
         __syncthreads();
         if (tid == 0) {
             T m = red[0];
-            for (int w = 1; w < G::NT / 32; ++w) m = red[w] > m ? red[w] : m;
+            for (int w = 1; w < NT / 32; ++w) m = red[w] > m ? red[w] : m;
             if (G::NTILE == 1) a.speed[g] = m;
             else if (sizeof(T) == 4) atomicMax(reinterpret_cast<unsigned int*>(a.speed + g), __float_as_uint((float)m));
             else atomicMax(reinterpret_cast<unsigned long long*>(a.speed + g), (unsigned long long)__double_as_longlong((double)m));
