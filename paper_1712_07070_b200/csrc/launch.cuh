@@ -38,6 +38,9 @@ cudaError_t launch_mhm(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
 }
 
 #ifdef GAMER_HAVE_CTU
+#ifndef CTU_NT_OVERRIDE
+#define CTU_NT_OVERRIDE 0
+#endif
 template <typename T, int RECON, int NV>
 constexpr int ctu_tile() {
     return CtuSmem<T, RECON, NV, 16>::BYTES <= SMEM_LIMIT ? 16 : (CtuSmem<T, RECON, NV, 8>::BYTES <= SMEM_LIMIT ? 8 : 4);
@@ -45,7 +48,7 @@ constexpr int ctu_tile() {
 
 template <typename T, int RECON, int SOLVER, int NV, bool EXT, int TY>
 cudaError_t launch_ctu_ty(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
-    constexpr int NT = (sizeof(T) == 4 ? 32 : 16) * TY < 128 ? 128 : (sizeof(T) == 4 ? 32 : 16) * TY;
+    constexpr int NT = CTU_NT_OVERRIDE > 0 ? CTU_NT_OVERRIDE : ((sizeof(T) == 8 ? 48 : 32) * TY < 128 ? 128 : (sizeof(T) == 8 ? 48 : 32) * TY);
     using G = Geo<TY>;
     using S = CtuSmem<T, RECON, NV, TY>;
     static_assert(S::BYTES <= SMEM_LIMIT, "tile does not fit in shared memory");

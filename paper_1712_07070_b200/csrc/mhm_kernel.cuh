@@ -88,13 +88,19 @@ __global__ void __launch_bounds__(NT, MINB) mhm_kernel(const AdvArgs<T> a) {
     T smax = T(0);
     Counters cnt = {0, 0, 0, 0, 0};
 
-    for (int kk = -1; kk <= PS; ++kk) {
+    int slot0 = (NGH - 1 - R) % PR;      // ring slot of the lowest plane the predictor of plane kk reads
+    for (int kk = -1; kk <= PS; ++kk, slot0 = (slot0 + 1 == PR) ? 0 : slot0 + 1) {
         // ------------------------------------------------------------------ S1: predictor
         {
             const int pc = kk + NGH;   // padded plane index of kk
             const T* Pz[2 * R + 1];
 #pragma unroll
-            for (int m = -R; m <= R; ++m) Pz[m + R] = prim + ((pc + m) % PR) * NV * G::PLN;
+            for (int m = 0; m <= 2 * R; ++m) {
+                int sl = slot0 + m;
+                if (sl >= PR) sl -= PR;
+                Pz[m] = prim + sl * NV * G::PLN;
+            }
+            (void)pc;
             T* zcur = es + ZOFF + (kk & 1) * NV * G::EPL;
             for (int t = tid; t < G::NPLUS; t += NT) {
                 int ei, ej;
@@ -118,14 +124,20 @@ __global__ void __launch_bounds__(NT, MINB) mhm_kernel(const AdvArgs<T> a) {
                                 face_values5<T, RECON, EXT>(T(0), Pz[R - 1][o], Pz[R][o], Pz[R + 1][o], T(0), Wm[v], Wp[v], ph);
                         }
                     }
-                    T Fm[NV], Fp[NV];
                     prim2cons<T, NV>(Wm, Uf[d][0], ph);
                     prim2cons<T, NV>(Wp, Uf[d][1], ph);
-                    if (d == 0) { phys_flux<T, NV, 0>(Wm, Uf[d][0], Fm); phys_flux<T, NV, 0>(Wp, Uf[d][1], Fp); }
-                    if (d == 1) { phys_flux<T, NV, 1>(Wm, Uf[d][0], Fm); phys_flux<T, NV, 1>(Wp, Uf[d][1], Fp); }
-                    if (d == 2) { phys_flux<T, NV, 2>(Wm, Uf[d][0], Fm); phys_flux<T, NV, 2>(Wp, Uf[d][1], Fp); }
+                    // F_d(W+) - F_d(W-), each difference formed as one product and one fused multiply-add
+                    const T vm = Wm[1 + d], vp = Wp[1 + d];
+                    T dF[NV];
 #pragma unroll
-                    for (int v = 0; v < NV; ++v) dU[v] = (d == 0) ? (Fp[v] - Fm[v]) : dU[v] + (Fp[v] - Fm[v]);
+                    for (int v = 0; v < NV; ++v) {
+                        const T am = (v == 4) ? Uf[d][0][4] + Wm[4] : Uf[d][0][v];
+                        const T ap = (v == 4) ? Uf[d][1][4] + Wp[4] : Uf[d][1][v];
+                        dF[v] = ap * vp - am * vm;
+                    }
+                    dF[1 + d] += Wp[4] - Wm[4];
+#pragma unroll
+                    for (int v = 0; v < NV; ++v) dU[v] = (d == 0) ? dF[v] : dU[v] + dF[v];
                 }
                 // Hancock half step on all six face states, back to primitives, positivity check
                 T We[3][2][NV];
