@@ -44,8 +44,8 @@ def build(force=False, verbose=False):
                 cmd = [NVCC, *FLAGS, "-DG_SCHEME=%d" % s, "-DG_RECON=%d" % r, "-DG_SOLVER=%d" % v]
                 if have_ctu:
                     cmd.append("-DGAMER_HAVE_CTU")
-                if os.environ.get("GAMER_EXPERIMENT_TY"):
-                    cmd.append("-DGAMER_EXPERIMENT_TY")
+                if os.environ.get("GAMER_EXTRA_DEFS"):
+                    cmd += os.environ["GAMER_EXTRA_DEFS"].split()
                 if verbose:
                     cmd += ["-Xptxas", "-v"]
                 jobs.append((cmd + ["-c", os.path.join(CSRC, "inst.cu"), "-o", o], o))

@@ -286,42 +286,7 @@ __global__ void __launch_bounds__(NT) ctu_kernel(const AdvArgs<T> a) {
         }
     }
 
-    // ---------------------------------------------------------------------- epilogue: reductions
-    __syncthreads();
-    T* red = sm;
-    if (a.speed) {
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            const T other = __shfl_xor_sync(0xffffffffu, smax, o);
-            smax = other > smax ? other : smax;
-        }
-        if ((tid & 31) == 0) red[tid >> 5] = smax;
-        __syncthreads();
-        if (tid == 0) {
-            T mx = red[0];
-            for (int w = 1; w < NT / 32; ++w) mx = red[w] > mx ? red[w] : mx;
-            if (G::NTILE == 1) a.speed[g] = mx;
-            else if (sizeof(T) == 4) atomicMax(reinterpret_cast<unsigned int*>(a.speed + g), __float_as_uint((float)mx));
-            else atomicMax(reinterpret_cast<unsigned long long*>(a.speed + g), (unsigned long long)__double_as_longlong((double)mx));
-        }
-    }
-    if (EXT) {
-        int c[5] = {cnt.roe_fb, cnt.reverted, cnt.first_order, cnt.dual_fix, cnt.unphys};
-#pragma unroll
-        for (int q = 0; q < 5; ++q) {
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) c[q] += __shfl_xor_sync(0xffffffffu, c[q], o);
-        }
-        if ((tid & 31) == 0) {
-            if (a.diag) {
-                if (c[0]) atomicAdd(a.diag + 0, c[0]);
-                if (c[1]) atomicAdd(a.diag + 1, c[1]);
-                if (c[2]) atomicAdd(a.diag + 2, c[2]);
-                if (c[3]) atomicAdd(a.diag + 3, c[3]);
-            }
-            if (a.n_unphys && c[4]) atomicAdd(a.n_unphys, c[4]);
-        }
-    }
+    block_epilogue<T, NT, G::NTILE, EXT>(a, g, smax, cnt, sm, tid);
 }
 
 }  // namespace gamer

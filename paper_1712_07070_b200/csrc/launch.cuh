@@ -68,12 +68,6 @@ cudaError_t launch_ctu_ty(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
 template <typename T, int RECON, int SOLVER, int NV, bool EXT>
 cudaError_t launch_ctu(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
     constexpr int TY = ctu_tile<T, RECON, NV>();
-#ifdef GAMER_EXPERIMENT_TY
-    if constexpr (TY == 16 && !EXT && sizeof(T) == 4) {
-        static const char* env = getenv("GAMER_CTU_TY");
-        if (env && env[0] == '8') return launch_ctu_ty<T, RECON, SOLVER, NV, EXT, 8>(a, st, launches);
-    }
-#endif
     return launch_ctu_ty<T, RECON, SOLVER, NV, EXT, TY>(a, st, launches);
 }
 #endif
