@@ -183,3 +183,40 @@ def test_config5_full_size_sampled(dev, oracle_mod):
     assert torch.isfinite(out).all() and (out[:, 0] > 0).all() and nun == 0
     ek = 0.5 * (out[:, 1] ** 2 + out[:, 2] ** 2 + out[:, 3] ** 2) / out[:, 0]
     assert ((out[:, 4] - ek) > 0).all()
+
+
+def test_config3_two_level_sedov_flux_correction(dev, oracle_mod):
+    """BASELINE.json config 3 at full size: coarse 256 x 256 x 128 cells (2048 groups) + the central half refined
+    by 2 (2048 fine groups), Sedov blast (E = 1 in the central 2x2x2 fine cells, ambient rho = 1, P = 1e-5),
+    MHM+PLM+HLLE through the extended entry with a tiny pressure floor; one coarse step and two fine steps, every
+    batch compared with the oracle, and the composite grid conserved to round-off after restriction + flux
+    correction with the GPU's flux_out."""
+    import amr_harness as amr
+    uc, uf, region, dh_c = amr.sedov_two_level(128, 256, 256, gamma=G53, device=dev)
+    kw = dict(min_pres=1e-10)
+
+    def gpu_solver(p, dt, dh):
+        out, flux, speed, nun, diag = gpu_ex(p.contiguous(), dt, dh, G53, gb.MHM, gb.PLM, gb.HLLE, **kw)
+        assert nun == 0
+        return out, flux
+
+    tot0 = amr.composite_total(uc, uf, region, dh_c)
+    # blast cells: P = (gamma-1) E / (8 dv) with dv = (dh_c/2)^3; the fine level sets the step (Eq. 2, C = 0.4)
+    pb = (G53 - 1.0) / (8 * (0.5 * dh_c) ** 3)
+    dt_c = 2 * 0.4 * (0.5 * dh_c) / (3.0 * math.sqrt(G53 * pb))
+    uc1, uf1, rec = amr.two_level_step(gpu_solver, uc, uf, region, dh_c, dt_c)
+    tot1 = amr.composite_total(uc1, uf1, region, dh_c)
+    assert ((tot1 - tot0).abs() / (tot0.abs() + 1e-9)).max().item() <= 1e-12
+    assert torch.isfinite(uc1).all() and torch.isfinite(uf1).all()
+    n_groups = 0
+    for name, (p, out, flux) in rec.items():
+        dt, dh = (dt_c, dh_c) if name == "coarse" else (0.5 * dt_c, 0.5 * dh_c)
+        n_groups += p.shape[0]
+        ref = oracle_mod.fluid_advance(p.cpu().numpy(), dt, dh, G53, gb.MHM, gb.PLM, gb.HLLE, oracle_mod.make_opts(**kw))
+        err = rel_l1(out.cpu().numpy(), ref["out"], G53)
+        assert max(err.values()) <= 1e-12, (name, err)
+        fe = np.abs(flux.cpu().numpy() - ref["flux"]).sum() / np.abs(ref["flux"]).sum()
+        assert fe <= 1e-12, (name, fe)
+    assert n_groups == 2048 + 2 * 2048
+    # the blast did move energy inside the fine level
+    assert (uf1[4] - uf[4]).abs().max().item() > 1.0
