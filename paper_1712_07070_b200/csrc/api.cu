@@ -62,7 +62,8 @@ static int advance_typed(const void* in, void* out, void* flux_out, int64_t n_gr
         a.n_unphys = o->n_unphysical_out;
         a.diag = o->diag_out;
         nsc = o->n_scalar;
-        ext = (nsc || a.dual || a.remedy2 || a.limiter != LIM_GMINMOD || a.min_dens > 0 || a.min_pres > 0 ||
+        const bool custom_theta = a.theta != (recon == GAMER_PPM ? 2.0 : 1.0);   // fast kernels fix theta at compile time
+        ext = (nsc || a.dual || a.remedy2 || a.limiter != LIM_GMINMOD || custom_theta || a.min_dens > 0 || a.min_pres > 0 ||
                a.min_temp > 0 || a.n_unphys || a.diag) ? 1 : 0;
     }
     if (a.n_unphys && cudaMemsetAsync(a.n_unphys, 0, sizeof(int), st) != cudaSuccess) return GAMER_ECUDA;

@@ -138,8 +138,8 @@ __global__ void __launch_bounds__(NT) ctu_kernel(const AdvArgs<T> a) {
 #pragma unroll
                     for (int v = 0; v < NV; ++v) {
                         const T* q = Pz[R] + v * G::PLN + c;
-                        if (d == 0) face_values<T, RECON, EXT>(q, 1, wm[v], wp[v], ph);
-                        else if (d == 1) face_values<T, RECON, EXT>(q, NP, wm[v], wp[v], ph);
+                        if (d == 0) face_values<T, RECON, EXT, fixed_theta(EXT, RECON)>(q, 1, wm[v], wp[v], ph);
+                        else if (d == 1) face_values<T, RECON, EXT, fixed_theta(EXT, RECON)>(q, NP, wm[v], wp[v], ph);
                         else {
                             const int o = v * G::PLN + c;
                             if (RECON == PPM)

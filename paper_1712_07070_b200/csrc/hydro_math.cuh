@@ -44,6 +44,12 @@ template <> struct Ops<float> {
     static __device__ __forceinline__ float pow(float a, float b) { return powf(a, b); }
     static __device__ __forceinline__ float copysign(float a, float b) { return copysignf(a, b); }
     static __device__ __forceinline__ bool finite(float a) { return isfinite(a); }
+    // min(|a|,|b|) if a and b have the same sign, else 0 (one FMNMX.XORSIGN + one FMNMX)
+    static __device__ __forceinline__ float minabs_same_sign(float a, float b) {
+        float r;
+        asm("min.xorsign.abs.f32 %0, %1, %2;" : "=f"(r) : "f"(a), "f"(b));
+        return fmaxf(r, 0.0f);
+    }
 };
 
 template <> struct Ops<double> {
@@ -56,6 +62,10 @@ template <> struct Ops<double> {
     static __device__ __forceinline__ double pow(double a, double b) { return ::pow(a, b); }
     static __device__ __forceinline__ double copysign(double a, double b) { return ::copysign(a, b); }
     static __device__ __forceinline__ bool finite(double a) { return isfinite(a); }
+    static __device__ __forceinline__ double minabs_same_sign(double a, double b) {
+        const double m = fmin(fabs(a), fabs(b));
+        return a * b > 0.0 ? m : 0.0;
+    }
 };
 
 // run-time constants shared by every stage (kept in registers / constant bank)
@@ -107,36 +117,42 @@ __device__ __forceinline__ void floor_prim(T* W, const Phys<T>& ph) {
 // ---------------------------------------------------------------------------------------------
 // slope limiters (L94)
 // ---------------------------------------------------------------------------------------------
-template <typename T, bool EXT>
+// THETA = 1 or 2 fixes the generalized-minmod parameter at compile time (the defaults of the 11-argument form:
+// 1 for PLM, 2 for PPM); THETA = 0 reads ph.theta / ph.limiter at run time (extended mode).
+// The sign test "dL*dR > 0" is taken on the sign bits (min.xorsign.abs in fp32): it differs from the product
+// only when the product underflows, where the slope is below 1e-19 of the data either way.
+template <typename T, bool EXT, int THETA = 0>
 __device__ __forceinline__ T limited_slope(T dL, T dR, const Phys<T>& ph) {
-    const T prod = dL * dR;
-    if (EXT && ph.limiter != LIM_GMINMOD) {
+    if (THETA == 0 && EXT && ph.limiter != LIM_GMINMOD) {
+        const T prod = dL * dR;
         if (!(prod > T(0))) return T(0);
         if (ph.limiter == LIM_VANLEER) return T(2) * prod * Ops<T>::rcp(dL + dR);
         return prod * (dL + dR) * Ops<T>::rcp(dL * dL + dR * dR);
     }
-    const T aL = Ops<T>::abs(dL), aR = Ops<T>::abs(dR);
-    T m = Ops<T>::min(aL, aR);
+    T m = Ops<T>::minabs_same_sign(dL, dR);
     // theta == 1 (plain minmod): |dL+dR|/2 >= min(|dL|,|dR|) holds exactly in floating point for equal
     // signs (rounding is monotonic), so the centred term can never win and is skipped
-    if (ph.theta != T(1)) m = Ops<T>::min(ph.theta * m, T(0.5) * Ops<T>::abs(dL + dR));
-    m = Ops<T>::copysign(m, dR);
-    return prod > T(0) ? m : T(0);
+    if (THETA == 2) m = Ops<T>::min(m + m, T(0.5) * Ops<T>::abs(dL + dR));
+    else if (THETA == 0 && ph.theta != T(1)) m = Ops<T>::min(ph.theta * m, T(0.5) * Ops<T>::abs(dL + dR));
+    return Ops<T>::copysign(m, dR);
 }
 
+// compile-time theta of the fast (non-extended) kernels: the 11-argument defaults, theta = 1 (PLM) / 2 (PPM)
+__host__ __device__ constexpr int fixed_theta(bool ext, int recon) { return ext ? 0 : (recon == PLM ? 1 : 2); }
+
 // face values of the centre cell of a strip: q points at the centre, neighbours at q[+-s], q[+-2s]
-template <typename T, int RECON, bool EXT>
+template <typename T, int RECON, bool EXT, int THETA = 0>
 __device__ __forceinline__ void face_values(const T* q, int s, T& wm, T& wp, const Phys<T>& ph) {
     const T c = q[0], l1 = q[-s], r1 = q[s];
     if (RECON == PLM) {
-        const T sl = limited_slope<T, EXT>(c - l1, r1 - c, ph);
+        const T sl = limited_slope<T, EXT, THETA>(c - l1, r1 - c, ph);
         wm = c - T(0.5) * sl;
         wp = c + T(0.5) * sl;
     } else {   // PPM, Colella & Woodward (1984) eqs. 1.6-1.10, no steepening / flattening
         const T l2 = q[-2 * s], r2 = q[2 * s];
-        const T sm = limited_slope<T, EXT>(l1 - l2, c - l1, ph);
-        const T s0 = limited_slope<T, EXT>(c - l1, r1 - c, ph);
-        const T sp = limited_slope<T, EXT>(r1 - c, r2 - r1, ph);
+        const T sm = limited_slope<T, EXT, THETA>(l1 - l2, c - l1, ph);
+        const T s0 = limited_slope<T, EXT, THETA>(c - l1, r1 - c, ph);
+        const T sp = limited_slope<T, EXT, THETA>(r1 - c, r2 - r1, ph);
         const T sixth = T(1.0 / 6.0);
         T m = T(0.5) * (l1 + c) - (s0 - sm) * sixth;
         T p = T(0.5) * (c + r1) - (sp - s0) * sixth;

@@ -5,7 +5,7 @@
 namespace gamer {
 
 template <typename T> struct RoeAvg {
-    T u, v, w, H, q2, a2, a;
+    T u, v, w, H, q2, a2, a, ia;   // ia = 1/a (0 if a2 <= 0)
 };
 
 template <typename T> struct Side {
@@ -41,7 +41,8 @@ __device__ __forceinline__ void roe_average(const Side<T>& L, const Side<T>& R, 
     r.H = fl * L.H + fr * R.H;
     r.q2 = r.u * r.u + r.v * r.v + r.w * r.w;
     r.a2 = ph.gm1 * (r.H - T(0.5) * r.q2);
-    r.a = r.a2 > T(0) ? Ops<T>::sqrt(r.a2) : T(0);
+    r.ia = r.a2 > T(0) ? Ops<T>::rsqrt(r.a2) : T(0);
+    r.a = r.a2 * r.ia;
 }
 
 // HLLE (Einfeldt et al. 1991)
@@ -93,6 +94,11 @@ __device__ __forceinline__ void solve_hllc(const Side<T>& L, const Side<T>& R, c
 }
 
 // Roe (1981), no entropy fix.  Returns true if remedy (i) (L104) must be taken.
+// The flux is evaluated in the one-sided form  F = F_L + sum_{lambda_k<0} lambda_k alpha_k K_k  (u~ >= 0)  or
+// F = F_R - sum_{lambda_k>0} lambda_k alpha_k K_k  (u~ < 0), which equals the symmetric form
+// (F_L+F_R)/2 - sum |lambda_k| alpha_k K_k / 2 because F_R - F_L = sum lambda_k alpha_k K_k holds identically for
+// Roe averages; only the acoustic wave on the far side of the contact can then contribute, so the dissipation
+// of the three lambda = u~ waves never has to be formed.
 template <typename T>
 __device__ __forceinline__ bool solve_roe(const Side<T>& L, const Side<T>& R, const RoeAvg<T>& r, T* F,
                                           const Phys<T>& ph) {
@@ -102,31 +108,33 @@ __device__ __forceinline__ bool solve_roe(const Side<T>& L, const Side<T>& R, co
     const T a3 = d2 - v * d0;
     const T a4 = d3 - w * d0;
     const T d5 = d4 - a3 * v - a4 * w;
-    const T ia2 = Ops<T>::rcp(r.a2);
-    const T a2 = ph.gm1 * ia2 * (d0 * (H - u * u) + u * d1 - d5);
-    const T a1 = (d0 * (u + a) - d1 - a * a2) * (T(0.5) * Ops<T>::rcp(a));
+    const T a2 = ph.gm1 * r.ia * r.ia * (d0 * (H - u * u) + u * d1 - d5);
+    const T up = u + a, um = u - a;
+    const T a1 = (d0 * up - d1 - a * a2) * (T(0.5) * r.ia);
     const T a5 = d0 - (a1 + a2);
+    const T ua = u * a;
+    const T Hm = H - ua, Hp = H + ua;
     // intermediate states U_L + a1 K1 and U_R - a5 K5
     {
-        const T r1 = L.rho + a1, n1 = L.m1 + a1 * (u - a), s1 = L.m2 + a1 * v, t1 = L.m3 + a1 * w,
-                e1 = L.E + a1 * (H - u * a);
-        const T r5 = R.rho - a5, n5 = R.m1 - a5 * (u + a), s5 = R.m2 - a5 * v, t5 = R.m3 - a5 * w,
-                e5 = R.E - a5 * (H + u * a);
+        const T r1 = L.rho + a1, n1 = L.m1 + a1 * um, s1 = L.m2 + a1 * v, t1 = L.m3 + a1 * w, e1 = L.E + a1 * Hm;
+        const T r5 = R.rho - a5, n5 = R.m1 - a5 * up, s5 = R.m2 - a5 * v, t5 = R.m3 - a5 * w, e5 = R.E - a5 * Hp;
         // P > 0  <=>  rho*E - |m|^2/2 > 0 when rho > 0
         const T p1 = r1 * e1 - T(0.5) * (n1 * n1 + s1 * s1 + t1 * t1);
         const T p5 = r5 * e5 - T(0.5) * (n5 * n5 + s5 * s5 + t5 * t5);
         if (!(r1 > T(0)) || !(r5 > T(0)) || !(p1 > T(0)) || !(p5 > T(0))) return true;
     }
-    T FL[5], FR[5];
-    side_flux(L, FL);
-    side_flux(R, FR);
-    const T l1 = Ops<T>::abs(u - a) * a1, l2 = Ops<T>::abs(u), l5 = Ops<T>::abs(u + a) * a5;
-    const T c2 = l2 * a2, c3 = l2 * a3, c4 = l2 * a4;
-    F[0] = T(0.5) * ((FL[0] + FR[0]) - (l1 + c2 + l5));
-    F[1] = T(0.5) * ((FL[1] + FR[1]) - (l1 * (u - a) + c2 * u + l5 * (u + a)));
-    F[2] = T(0.5) * ((FL[2] + FR[2]) - (l1 * v + (c2 * v + c3) + l5 * v));
-    F[3] = T(0.5) * ((FL[3] + FR[3]) - (l1 * w + (c2 * w + c4) + l5 * w));
-    F[4] = T(0.5) * ((FL[4] + FR[4]) - (l1 * (H - u * a) + (c2 * (T(0.5) * r.q2) + c3 * v + c4 * w) + l5 * (H + u * a)));
+    const bool pos = u >= T(0);
+    const T rho = pos ? L.rho : R.rho, un = pos ? L.u : R.u, P = pos ? L.P : R.P, E = pos ? L.E : R.E;
+    const T m1 = pos ? L.m1 : R.m1, m2 = pos ? L.m2 : R.m2, m3 = pos ? L.m3 : R.m3;
+    (void)rho;
+    const T cm = Ops<T>::min(um, T(0)) * a1, cp = Ops<T>::max(up, T(0)) * a5;
+    const T cf = pos ? cm : -cp;
+    const T Kn = pos ? um : up, K4 = pos ? Hm : Hp;
+    F[0] = m1 + cf;
+    F[1] = (m1 * un + P) + cf * Kn;
+    F[2] = m2 * un + cf * v;
+    F[3] = m3 * un + cf * w;
+    F[4] = un * (E + P) + cf * K4;
     return false;
 }
 

@@ -137,7 +137,7 @@ __device__ __forceinline__ void convert_plane(const T* raw, T* prim, const Phys<
 template <typename T, int RECON, bool EXT>
 __device__ __forceinline__ void face_values5(T l2, T l1, T c, T r1, T r2, T& wm, T& wp, const Phys<T>& ph) {
     T q[5] = {l2, l1, c, r1, r2};
-    face_values<T, RECON, EXT>(q + 2, 1, wm, wp, ph);
+    face_values<T, RECON, EXT, fixed_theta(EXT, RECON)>(q + 2, 1, wm, wp, ph);
 }
 
 // ---------------------------------------------------------------------------------------------

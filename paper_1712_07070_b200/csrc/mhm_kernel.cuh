@@ -114,8 +114,8 @@ __global__ void __launch_bounds__(NT, MINB) mhm_kernel(const AdvArgs<T> a) {
 #pragma unroll
                     for (int v = 0; v < NV; ++v) {
                         const T* q = Pz[R] + v * G::PLN + c;
-                        if (d == 0) face_values<T, RECON, EXT>(q, 1, Wm[v], Wp[v], ph);
-                        else if (d == 1) face_values<T, RECON, EXT>(q, NP, Wm[v], Wp[v], ph);
+                        if (d == 0) face_values<T, RECON, EXT, fixed_theta(EXT, RECON)>(q, 1, Wm[v], Wp[v], ph);
+                        else if (d == 1) face_values<T, RECON, EXT, fixed_theta(EXT, RECON)>(q, NP, Wm[v], Wp[v], ph);
                         else {
                             const int o = v * G::PLN + c;
                             if (RECON == PPM)
