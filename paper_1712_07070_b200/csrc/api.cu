@@ -69,6 +69,7 @@ static int advance_typed(const void* in, void* out, void* flux_out, int64_t n_gr
     if (a.n_unphys && cudaMemsetAsync(a.n_unphys, 0, sizeof(int), st) != cudaSuccess) return GAMER_ECUDA;
     if (a.diag && cudaMemsetAsync(a.diag, 0, 4 * sizeof(int), st) != cudaSuccess) return GAMER_ECUDA;
     if (n_groups == 0) return GAMER_OK;
+    fill_phys(a);
     int launches = 0;
     const cudaError_t e = TABLE[scheme - 1][recon - 1][riemann - 1](sizeof(T), nsc, ext, &a, st, &launches);
     g_launches += launches;

@@ -28,13 +28,15 @@ template <typename T> struct AdvArgs {
     double dt, dh, gamma, theta, xi, min_dens, min_pres, min_temp;
     int limiter, dual, remedy2;
     long long n_groups;
+    Phys<T> ph;       // the run-time constants in the kernel's precision, filled on the host (fill_phys)
 };
 
+// host side: every constant of the step in the kernel's precision, so that device code reads them straight
+// from the kernel-parameter constant bank (no per-use double -> T conversion, no registers)
 template <typename T>
-__device__ __forceinline__ Phys<T> make_phys(const AdvArgs<T>& a) {
-    Phys<T> ph;
-    const double dt = a.dt_dev ? *a.dt_dev : a.dt;
-    const double lam = dt / a.dh;
+inline void fill_phys(AdvArgs<T>& a) {
+    Phys<T>& ph = a.ph;
+    const double lam = a.dt / a.dh;
     ph.gamma = T(a.gamma);
     ph.gm1 = T(a.gamma - 1.0);
     ph.inv_gm1 = T(1.0 / (a.gamma - 1.0));
@@ -49,6 +51,17 @@ __device__ __forceinline__ Phys<T> make_phys(const AdvArgs<T>& a) {
     ph.floors = (a.min_dens > 0.0 || a.min_pres > 0.0 || a.min_temp > 0.0) ? 1 : 0;
     ph.dual = a.dual;
     ph.remedy2 = a.remedy2;
+}
+
+// device side: the host-filled constants; only dt/dh comes from memory when dt lives on the device
+template <typename T>
+__device__ __forceinline__ Phys<T> make_phys(const AdvArgs<T>& a) {
+    Phys<T> ph = a.ph;
+    if (a.dt_dev) {
+        const double lam = *a.dt_dev / a.dh;
+        ph.lam = T(lam);
+        ph.hlam = T(0.5 * lam);
+    }
     return ph;
 }
 

@@ -12,27 +12,32 @@ constexpr size_t SMEM_LIMIT = 232448;   // 227 KB opt-in maximum per CTA on sm_1
 
 template <typename T, int RECON, int NV>
 constexpr int mhm_tile() {
-    return MhmSmem<T, RECON, NV, 16>::BYTES <= SMEM_LIMIT ? 16 : (MhmSmem<T, RECON, NV, 8>::BYTES <= SMEM_LIMIT ? 8 : 4);
+    return MhmGeo<T, RECON, NV, 16>::BYTES <= SMEM_LIMIT ? 16 : (MhmGeo<T, RECON, NV, 8>::BYTES <= SMEM_LIMIT ? 8 : 4);
 }
 
 template <typename T, int RECON, int SOLVER, int NV, bool EXT>
 cudaError_t launch_mhm(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
+#ifndef MHM_MINB3
+#define MHM_MINB3 1
+#endif
+#ifdef MHM_TY_OVERRIDE
+    constexpr int TY = MHM_TY_OVERRIDE;
+#else
     constexpr int TY = mhm_tile<T, RECON, NV>();
-    using G = Geo<TY>;
-    using S = MhmSmem<T, RECON, NV, TY>;
-    static_assert(S::BYTES <= SMEM_LIMIT, "tile does not fit in shared memory");
-    // 320 threads = the 320 predictor cells of a plane (one each), 800 faces = 2.5 rounds; see DESIGN.md
-    constexpr int NT = TY == 16 ? 320 : G::NT < 128 ? 128 : G::NT;
-    constexpr int MINB = (sizeof(T) == 4 && TY == 16 && NV == 5 && RECON == PLM) ? 2 : 1;
-    auto kern = mhm_kernel<T, RECON, SOLVER, NV, EXT, TY, NT, MINB>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::BYTES);
+#endif
+    using G = MhmGeo<T, RECON, NV, TY>;
+    static_assert(G::BYTES <= SMEM_LIMIT, "tile does not fit in shared memory");
+    // two CTAs per SM when two tiles (plus the 1 KB the driver reserves per CTA) fit in the 228 KB of an SM
+    constexpr int MINB = (MHM_MINB3 && 3 * (G::BYTES + 1024) <= 233472 && G::NT <= 192) ? 3 : (2 * (G::BYTES + 1024) <= 233472) ? 2 : 1;
+    auto kern = mhm_kernel<T, RECON, SOLVER, NV, EXT, TY, MINB>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::BYTES);
     if (e != cudaSuccess) return e;
     if (G::NTILE > 1 && a.speed) {
         e = cudaMemsetAsync(a.speed, 0, sizeof(T) * a.n_groups, st);
         if (e != cudaSuccess) return e;
     }
     const long long grid = a.n_groups * G::NTILE;
-    kern<<<(unsigned)grid, NT, S::BYTES, st>>>(a);
+    kern<<<(unsigned)grid, G::NT, G::BYTES, st>>>(a);
     *launches += 1;
     return cudaGetLastError();
 }

@@ -1,56 +1,196 @@
 // mhm_kernel.cuh -- MUSCL-Hancock (MHM; Toro 2009 sect. 14.4/16.5) patch-group kernel.
 //
-// Per plane kk = -1..16 of the tile (2 block barriers per plane):
-//   S1  predictor : PLM/PPM face values of the "plus"-shaped cell set of the plane (the cells whose
-//                   face states a final flux needs), Hancock half-step with the cell's own face
-//                   fluxes in all three directions, conversion back to primitives -> es / zp (smem)
-//   S2  Riemann   : x/y faces of plane kk, z faces between kk-1 and kk -> fx/fy/fz (smem) and the
-//                   patch-boundary planes of flux_out;  meanwhile the next staged plane -> primitives
-//   S3  update    : thread (i,j) finishes cell (i,j,kk-1) (needs F_z at kk-1/2), applies the closing
-//                   step, writes `out`, tracks the CFL maximum; then keeps (dFx+dFy) and F_z(kk-1/2)
-//                   of plane kk in registers;  one thread re-arms the freed TMA stage.
+// One CTA advances one (16 x TY x 16) column tile of a patch group, marching along z, ONE block barrier
+// per plane.  Thread roles (fixed for the whole kernel):
+//   interior (16*TY threads) : cell (i, j) of the tile.  Per plane kk it runs the predictor of its cell
+//        (PLM/PPM face values, Hancock half step, R6 of DESIGN.md), keeps the z+ / z- states and the
+//        x-, y- states in registers, publishes only x+ and y+ to shared memory, and solves the three
+//        Riemann problems at its own lower faces (i-1/2, j-1/2, kk-1/2).  It finishes cell (i, j, kk-1)
+//        from registers plus the two neighbour fluxes (i+1/2, j+1/2) read from shared memory.
+//   x-halo (2*TY threads)    : cells (-1, j) [publish x+] and (16, j) [solve face 15 1/2].
+//   y-halo (32 threads)      : cells (i, -1) [publish y+] and (i, TY) [solve face TY - 1/2].
+//   halo warps also turn each staged conserved plane (TMA 1-D bulk copies, two stages) into primitives
+//   in a ring of 2R+2 planes, one plane ahead of the predictor.
+// Face states and fluxes in shared memory are double-buffered by plane parity, which is what lets a
+// single __syncthreads per plane separate "publish" from "consume":
+//   iteration kk:  predictor(kk), z-Riemann(kk-1/2), convert(plane kk+2+R)  | barrier |
+//                  x/y-Riemann(kk), update of plane kk-1, TMA issue for the freed stage.
+// All threads run the same loop body (one copy of the predictor and of each of the three Riemann solves, so
+// the code stays inside the 32 KB instruction cache and a face shared by two groups gets bit-identical
+// fluxes from both); roles only switch parts of it off.
 #pragma once
 #include "hydro_close.cuh"
 
 namespace gamer {
 
-template <typename T, int RECON, int NV, int TY> struct MhmSmem {
-    using G = Geo<TY>;
-    static constexpr int R = RECON == PPM ? 2 : 1;
-    static constexpr int PR = 2 * R + 1;
-    static constexpr int RAW = 0;                                   // [2][NV][PLN]
-    static constexpr int PRIM = RAW + 2 * NV * G::PLN;              // [PR][NV][PLN]
-    static constexpr int ES = PRIM + PR * NV * G::PLN;              // [5][NV][EPL]
-    static constexpr int ZP = ES + 5 * NV * G::EPL;                 // [2][NV][EPL]  z+ of planes kk, kk-1
-    static constexpr int FL = ZP + 2 * NV * G::EPL;                 // [NV][NF]      rotated fluxes, flat face list
-    static constexpr int END = FL + NV * G::NF;
-    static constexpr size_t BYTES = 16 + (size_t)END * sizeof(T);  // 2 mbarriers first
+template <typename T> struct alignas(16) Vec4 {
+    T a, b, c, d;
 };
 
-template <typename T, int RECON, int SOLVER, int NV, bool EXT, int TY, int NT, int MINB>
-__global__ void __launch_bounds__(NT, MINB) mhm_kernel(const AdvArgs<T> a) {
-    using G = Geo<TY>;
-    using S = MhmSmem<T, RECON, NV, TY>;
-    constexpr int R = S::R, PR = S::PR;
-    constexpr int NPL = 18 + 2 * R;      // staged planes: padded 2-R .. 19+R
+template <typename T, int RECON, int NV, int TY> struct MhmGeo {
+    static constexpr int R = RECON == PPM ? 2 : 1;
+    static constexpr int RING = 2 * R + 2;
+    static constexpr int NI = 16 * TY;                          // interior threads
+    static constexpr int NXH = 2 * TY, NYH = 32;                // halo threads
+    static constexpr int NT = ((NI + NXH + NYH + 31) / 32) * 32;
+    static constexpr int NCV = NT - NI;                         // threads that convert planes
+    static constexpr int NTILE = PS / TY;
+    static constexpr int NR = TY + 2 * NGH, PLN = NR * NP;      // staged plane
+    static constexpr int NSX = 17 * TY, NSY = 16 * (TY + 1);    // x+ states / x fluxes, y+ states / y fluxes
+    static constexpr int BLK = (NSX + NSY) * NV;                // one buffer of states (or of fluxes)
+    static constexpr int RAW = 0;                               // [2][NV][PLN]
+    static constexpr int PRIM = RAW + 2 * NV * PLN;             // [RING][NV][PLN]
+    static constexpr int ST = PRIM + RING * NV * PLN;           // [2] x [Vec4 NSX | (NV-4) NSX | Vec4 NSY | (NV-4) NSY]
+    static constexpr int FL = ST + 2 * BLK;                     // same shape, fluxes in natural variable order
+    static constexpr int END = FL + 2 * BLK;
+    static constexpr size_t BYTES = 16 + (size_t)END * sizeof(T);   // 2 mbarriers first
+    static_assert((NV * PLN) % 4 == 0 && NSX % 4 == 0 && NSY % 4 == 0, "16-byte alignment of the Vec4 arrays");
+};
+
+// five (six) values of one face <-> shared memory: one Vec4 + NV-4 scalars; n = entries of the array
+template <typename T, int NV>
+__device__ __forceinline__ void put_state(T* blk, int n, int idx, const T* W) {
+    Vec4<T> q;
+    q.a = W[0]; q.b = W[1]; q.c = W[2]; q.d = W[3];
+    reinterpret_cast<Vec4<T>*>(blk)[idx] = q;
+#pragma unroll
+    for (int v = 4; v < NV; ++v) blk[v * n + idx] = W[v];
+}
+template <typename T, int NV>
+__device__ __forceinline__ void get_state(const T* blk, int n, int idx, T* W) {
+    const Vec4<T> q = reinterpret_cast<const Vec4<T>*>(blk)[idx];
+    W[0] = q.a; W[1] = q.b; W[2] = q.c; W[3] = q.d;
+#pragma unroll
+    for (int v = 4; v < NV; ++v) W[v] = blk[v * n + idx];
+}
+
+
+// ---------------------------------------------------------------------------------------------
+// predictor pieces (DESIGN R6)
+// ---------------------------------------------------------------------------------------------
+// Face values of one cell in all three directions -> conserved face states Uf[d][s] and the sum over d of
+// F_d(W+) - F_d(W-).  Pz[m] points at variable 0 of this cell in the primitive plane kk-R+m.
+template <typename T, int RECON, int NV, bool EXT, int PLN>
+__device__ __forceinline__ void mhm_face_states(const T* const* Pz, const Phys<T>& ph, T (&Uf)[3][2][NV], T (&dU)[NV]) {
+    constexpr int R = RECON == PPM ? 2 : 1;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        T Wm[NV], Wp[NV];
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+            const T* q = Pz[R] + v * PLN;
+            if (d == 0) face_values<T, RECON, EXT, fixed_theta(EXT, RECON)>(q, 1, Wm[v], Wp[v], ph);
+            else if (d == 1) face_values<T, RECON, EXT, fixed_theta(EXT, RECON)>(q, NP, Wm[v], Wp[v], ph);
+            else {
+                const int o = v * PLN;
+                if (RECON == PPM)
+                    face_values5<T, RECON, EXT>(Pz[0][o], Pz[R - 1][o], Pz[R][o], Pz[R + 1][o], Pz[2 * R][o], Wm[v], Wp[v], ph);
+                else
+                    face_values5<T, RECON, EXT>(T(0), Pz[R - 1][o], Pz[R][o], Pz[R + 1][o], T(0), Wm[v], Wp[v], ph);
+            }
+        }
+        prim2cons<T, NV>(Wm, Uf[d][0], ph);
+        prim2cons<T, NV>(Wp, Uf[d][1], ph);
+        // dU += F_d(W+) - F_d(W-), accumulated term by term with fused multiply-adds
+        const T vm = Wm[1 + d], vp = Wp[1 + d];
+        {
+            const T dm = Uf[d][1][1 + d] - Uf[d][0][1 + d];      // mass flux = momentum along d
+            dU[0] = (d == 0) ? dm : dU[0] + dm;
+        }
+#pragma unroll
+        for (int v = 1; v < NV; ++v) {
+            const T am = (v == 4) ? Uf[d][0][4] + Wm[4] : Uf[d][0][v];
+            const T ap = (v == 4) ? Uf[d][1][4] + Wp[4] : Uf[d][1][v];
+            T acc = (d == 0) ? ap * vp : dU[v] + ap * vp;
+            acc = acc - am * vm;
+            dU[v] = acc;
+        }
+        dU[1 + d] += Wp[4] - Wm[4];
+    }
+}
+
+// Hancock half step of one face state.  full: evolved primitives -> We (floors applied in extended mode);
+// !full: only the positivity of the evolved state is tested (no division), We is left untouched.  A state
+// that no Riemann solver of this thread consumes still decides the revert of R6.  floors = false in the
+// reverting pass (the un-evolved face values are taken as they are).
+template <typename T, int NV, bool EXT>
+__device__ __forceinline__ bool mhm_evolve(const T* Uf, const T* dU, T* We, bool full, bool floors, const Phys<T>& ph) {
+    T Ue[NV];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) Ue[v] = Uf[v] - ph.hlam * dU[v];
+    if (full || (EXT && ph.floors)) {
+        cons2prim<T, NV>(Ue, We, ph);
+        if (EXT && ph.floors && floors) floor_prim(We, ph);
+        return (We[0] > T(0)) && (We[4] > T(0));
+    }
+    const T pe = Ue[0] * Ue[4] - T(0.5) * (Ue[1] * Ue[1] + Ue[2] * Ue[2] + Ue[3] * Ue[3]);
+    return (Ue[0] > T(0)) && (pe > T(0));
+}
+
+// per-thread constants of the cell column this thread owns
+template <typename T> struct MhmCell {
+    int cidx;            // cell inside a staged plane
+    int sx_own, sy_own;  // slot of the x+ (y+) state of the left (lower) neighbour = slot of the own lower-face flux
+    int fxo, fyo, fzo;   // offsets into the group's flux_out of this thread's patch-boundary faces, -1 if none
+    const T* gin_cell;   // padded cell (ei, ej, interior plane 0) of variable 0 in `in`
+    T* gout_cell;        // cell (ei, ej, plane 0) of variable 0 in `out`
+    T* gflux;            // flux_out of this group (nullable)
+};
+
+template <typename T, int RECON, int SOLVER, int NV, bool EXT, int TY, int MINB>
+__global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY>::NT), MINB) mhm_kernel(const AdvArgs<T> a) {
+    using G = MhmGeo<T, RECON, NV, TY>;
+    constexpr int R = G::R, RING = G::RING, NT = G::NT, NI = G::NI, PLN = G::PLN, S = NV * G::PLN;
+    constexpr int NPL = 18 + 2 * R;      // staged planes: padded PF .. PF+NPL-1
     constexpr int PF = 2 - R;
+    constexpr int PSQ = PS * PS;
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw);
     T* sm = reinterpret_cast<T*>(smem_raw + 16);
-    T* raw = sm + S::RAW;
-    T* prim = sm + S::PRIM;
-    T* es = sm + S::ES;
-    T* fl = sm + S::FL;
+    T* raw = sm + G::RAW;
+    T* prim = sm + G::PRIM;
 
     const int tid = threadIdx.x;
     const long long tile = blockIdx.x;
     const long long g = tile / G::NTILE;
     const int j0 = (int)(tile % G::NTILE) * TY;
     const T* gin = a.in + (size_t)g * NV * NPC;
-    T* gout = a.out + (size_t)g * NV * (PS * PS * PS);
-    T* gflux = a.flux ? a.flux + (size_t)g * 9 * NV * (PS * PS) : nullptr;
     const Phys<T> ph = make_phys<T>(a);
+
+    // ---- role of this thread: cell (ei, ej) of the tile, ei in -1..16, ej in -1..TY
+    // role: 0 = interior, 1 = x-low, 2 = x-high, 4 = y-low, 8 = y-high, 16 = padding thread (conversion only)
+    const bool interior = tid < NI;
+    int ei = 0, ej = 0, role = 16;
+    if (interior) {
+        // a warp holds rows w and w + TY/2: the two 16-lane halves then fall in disjoint shared-memory banks
+        role = 0;
+        ei = tid & 15;
+        ej = (tid >> 5) + ((tid >> 4) & 1) * (TY / 2);
+    } else if (tid < NI + G::NXH) {
+        const int u = tid - NI;
+        role = u >= TY ? 2 : 1;
+        ei = role == 2 ? PS : -1;
+        ej = role == 2 ? u - TY : u;
+    } else if (tid < NI + G::NXH + G::NYH) {
+        const int u = tid - NI - G::NXH;
+        role = u >= 16 ? 8 : 4;
+        ei = u & 15;
+        ej = role == 8 ? TY : -1;
+    }
+    const bool pub_x = (role & ~1) == 0, pub_y = (role & ~4) == 0;      // publishes x+ / y+
+    const bool own_x = (role & ~2) == 0, own_y = (role & ~8) == 0;      // solves its lower x / y face
+    const int gj = j0 + ej;
+    MhmCell<T> c;
+    c.cidx = (ej + NGH) * NP + (ei + NGH);
+    c.sx_own = ej * 17 + ei;
+    c.sy_own = ej * 16 + ei;
+    c.gflux = a.flux ? a.flux + (size_t)g * 9 * NV * PSQ : nullptr;
+    c.fxo = (c.gflux && own_x && (ei & 7) == 0) ? ((0 * 3 + (ei >> 3)) * NV) * PSQ + gj : -1;
+    c.fyo = (c.gflux && own_y && (gj & 7) == 0) ? ((1 * 3 + (gj >> 3)) * NV) * PSQ + ei : -1;
+    c.fzo = (c.gflux && interior) ? (2 * 3 * NV) * PSQ + gj * PS + ei : -1;
+    c.gin_cell = gin + (size_t)NGH * (NP * NP) + (gj + NGH) * NP + (ei + NGH);
+    c.gout_cell = a.out + (size_t)g * NV * (PS * PSQ) + gj * PS + ei;
 
     if (tid == 0) {
         mbar_init(&bars[0], 1);
@@ -58,174 +198,182 @@ __global__ void __launch_bounds__(NT, MINB) mhm_kernel(const AdvArgs<T> a) {
         mbar_fence_init();
     }
     __syncthreads();
-    if (tid == 0) {
+    if (tid == NI) {
         issue_plane<T, NV, TY>(gin, j0, PF + 0, raw, &bars[0]);
-        issue_plane<T, NV, TY>(gin, j0, PF + 1, raw + NV * G::PLN, &bars[1]);
+        issue_plane<T, NV, TY>(gin, j0, PF + 1, raw + S, &bars[1]);
     }
-    // prologue: fill the primitive ring with staged planes n = 0 .. 2R
+    // prologue: staged planes n = 0 .. 2R (what the predictor of plane -1 reads), all threads convert
     for (int n = 0; n <= 2 * R; ++n) {
         mbar_wait(&bars[n & 1], (n >> 1) & 1);
-        convert_plane<T, NV, EXT, TY, NT>(raw + (n & 1) * NV * G::PLN, prim + ((PF + n) % PR) * NV * G::PLN, ph, tid);
+        convert_plane<T, NV, EXT, TY, NT>(raw + (n & 1) * S, prim + n * S, ph, tid);
         __syncthreads();
-        if (tid == 0 && n + 2 < NPL) issue_plane<T, NV, TY>(gin, j0, PF + n + 2, raw + (n & 1) * NV * G::PLN, &bars[n & 1]);
+        if (tid == NI && n + 2 < NPL) issue_plane<T, NV, TY>(gin, j0, PF + n + 2, raw + (n & 1) * S, &bars[n & 1]);
     }
 
-    // per-thread cell of the update stage
-    const bool owner = tid < G::NFZ;               // threads that own a cell column of the update stage
-    const int ci = tid & 15, cj = (tid >> 4) % TY;
-    // the convert stage starts at the warps that get fewer Riemann faces, to balance the barrier interval
-    constexpr int CROT = (G::NF % NT) == 0 ? 0 : ((G::NF % NT + 31) / 32) * 32 % NT;
-    const int ctid = (tid + NT - CROT) % NT;
-    // loop-invariant face descriptors of this thread's Riemann rounds (f = tid + r*NT)
-    constexpr int NROUND = (G::NF + NT - 1) / NT;
-    constexpr int ZOFF = 5 * NV * G::EPL;          // offset of the z+ buffers relative to es
-    unsigned fdesc[NROUND];
+    T zplus[NV];                    // z+ state of the plane below (rotated for z)
+    T fzl[NV];                      // z flux at kk-3/2 (natural variable order)
 #pragma unroll
-    for (int r = 0; r < NROUND; ++r) fdesc[r] = face_descriptor<NV, TY>(tid + r * NT < G::NF ? tid + r * NT : 0, ZOFF);
-    T sxy[NV], fzm[NV];
-#pragma unroll
-    for (int v = 0; v < NV; ++v) { sxy[v] = T(0); fzm[v] = T(0); }
+    for (int v = 0; v < NV; ++v) { zplus[v] = T(1); fzl[v] = T(0); }
     T smax = T(0);
     Counters cnt = {0, 0, 0, 0, 0};
+    // Q[m] = ring slot (offset into prim) of staged plane kk+1+m; Q[2R+1] is the slot the next plane goes to
+    int Q[RING];
+#pragma unroll
+    for (int m = 0; m < RING; ++m) Q[m] = m * S;
 
-    int slot0 = (NGH - 1 - R) % PR;      // ring slot of the lowest plane the predictor of plane kk reads
-    for (int kk = -1; kk <= PS; ++kk, slot0 = (slot0 + 1 == PR) ? 0 : slot0 + 1) {
-        // ------------------------------------------------------------------ S1: predictor
-        {
-            const int pc = kk + NGH;   // padded plane index of kk
+#pragma unroll 1
+    for (int kk = -1; kk <= PS; ++kk) {
+        const bool mid = kk >= 0 && kk < PS;
+        const int par = kk & 1;
+        T* st_x = sm + G::ST + par * G::BLK;
+        T* st_y = st_x + NV * G::NSX;
+        T* fl_x = sm + G::FL + par * G::BLK;
+        T* fl_y = fl_x + NV * G::NSX;
+        T xminus[NV], yminus[NV], fzn[NV];
+        // ------------------------------------------------------------------ predictor of plane kk
+        if (interior || (mid && role != 16)) {
             const T* Pz[2 * R + 1];
 #pragma unroll
-            for (int m = 0; m <= 2 * R; ++m) {
-                int sl = slot0 + m;
-                if (sl >= PR) sl -= PR;
-                Pz[m] = prim + sl * NV * G::PLN;
+            for (int m = 0; m <= 2 * R; ++m) Pz[m] = prim + Q[m] + c.cidx;
+            // Pass 0 evolves the six face states over dt/2; if one of them comes out unphysical the whole
+            // predictor is redone with a zero increment (pass 1), which yields the un-evolved face values (R6).
+            // A loop (not a branch that keeps everything alive) so that each conserved face state dies as soon
+            // as it has been evolved; x+ / y+ go to shared memory at once, pass 1 simply overwrites them.
+            T zminus[NV], znew[NV];
+#pragma unroll 1
+            for (int pass = 0; pass < 2; ++pass) {
+                T Uf[3][2][NV], dU[NV], We[NV];
+                mhm_face_states<T, RECON, NV, EXT, PLN>(Pz, ph, Uf, dU);
+                if (pass) {
+#pragma unroll
+                    for (int v = 0; v < NV; ++v) dU[v] = T(0);
+                }
+                const bool fl_ok = pass == 0;
+                bool ok = mhm_evolve<T, NV, EXT>(Uf[0][1], dU, We, mid && pub_x, fl_ok, ph);
+                if (mid && pub_x) {
+                    T rot[NV];
+#pragma unroll
+                    for (int k = 0; k < NV; ++k) rot[k] = We[nat_index(0, k)];
+                    put_state<T, NV>(st_x, G::NSX, c.sx_own + 1, rot);
+                }
+                ok = mhm_evolve<T, NV, EXT>(Uf[1][1], dU, We, mid && pub_y, fl_ok, ph) && ok;
+                if (mid && pub_y) {
+                    T rot[NV];
+#pragma unroll
+                    for (int k = 0; k < NV; ++k) rot[k] = We[nat_index(1, k)];
+                    put_state<T, NV>(st_y, G::NSY, c.sy_own + 16, rot);
+                }
+                ok = mhm_evolve<T, NV, EXT>(Uf[0][0], dU, We, mid && own_x, fl_ok, ph) && ok;
+#pragma unroll
+                for (int k = 0; k < NV; ++k) xminus[k] = We[nat_index(0, k)];
+                ok = mhm_evolve<T, NV, EXT>(Uf[1][0], dU, We, mid && own_y, fl_ok, ph) && ok;
+#pragma unroll
+                for (int k = 0; k < NV; ++k) yminus[k] = We[nat_index(1, k)];
+                ok = mhm_evolve<T, NV, EXT>(Uf[2][0], dU, We, interior && kk >= 0, fl_ok, ph) && ok;
+#pragma unroll
+                for (int k = 0; k < NV; ++k) zminus[k] = We[nat_index(2, k)];
+                ok = mhm_evolve<T, NV, EXT>(Uf[2][1], dU, We, interior && kk < PS, fl_ok, ph) && ok;
+#pragma unroll
+                for (int k = 0; k < NV; ++k) znew[k] = We[nat_index(2, k)];
+                if (ok || pass) break;
+                cnt.reverted++;
             }
-            (void)pc;
-            T* zcur = es + ZOFF + (kk & 1) * NV * G::EPL;
-            for (int t = tid; t < G::NPLUS; t += NT) {
-                int ei, ej;
-                if (t < 18 * TY) { ej = t / 18; ei = t - ej * 18; ej += 1; }
-                else { const int u = t - 18 * TY; ej = (u < 16) ? 0 : TY + 1; ei = 1 + (u & 15); }
-                const int c = (ej + 2) * NP + (ei + 2);
-                T Uf[3][2][NV], dU[NV];
+            if (interior) {
+                // ------------------------------------------------------------ z face kk-1/2
+                if (kk >= 0) {
+                    T F[NV];
+                    cnt.roe_fb += riemann_flux<T, SOLVER, NV>(zplus, zminus, F, ph) ? 1 : 0;
 #pragma unroll
-                for (int d = 0; d < 3; ++d) {
-                    T Wm[NV], Wp[NV];
+                    for (int v = 0; v < NV; ++v) fzn[v] = F[rot_index(2, v)];
+                    if (c.fzo >= 0 && (kk & 7) == 0) {
+                        T* q = c.gflux + c.fzo + (kk >> 3) * NV * PSQ;
 #pragma unroll
-                    for (int v = 0; v < NV; ++v) {
-                        const T* q = Pz[R] + v * G::PLN + c;
-                        if (d == 0) face_values<T, RECON, EXT, fixed_theta(EXT, RECON)>(q, 1, Wm[v], Wp[v], ph);
-                        else if (d == 1) face_values<T, RECON, EXT, fixed_theta(EXT, RECON)>(q, NP, Wm[v], Wp[v], ph);
-                        else {
-                            const int o = v * G::PLN + c;
-                            if (RECON == PPM)
-                                face_values5<T, RECON, EXT>(Pz[0][o], Pz[R - 1][o], Pz[R][o], Pz[R + 1][o], Pz[2 * R][o], Wm[v], Wp[v], ph);
-                            else
-                                face_values5<T, RECON, EXT>(T(0), Pz[R - 1][o], Pz[R][o], Pz[R + 1][o], T(0), Wm[v], Wp[v], ph);
-                        }
+                        for (int v = 0; v < NV; ++v) q[v * PSQ] = fzn[v];
                     }
-                    prim2cons<T, NV>(Wm, Uf[d][0], ph);
-                    prim2cons<T, NV>(Wp, Uf[d][1], ph);
-                    // F_d(W+) - F_d(W-), each difference formed as one product and one fused multiply-add
-                    const T vm = Wm[1 + d], vp = Wp[1 + d];
-                    T dF[NV];
-#pragma unroll
-                    for (int v = 0; v < NV; ++v) {
-                        const T am = (v == 4) ? Uf[d][0][4] + Wm[4] : Uf[d][0][v];
-                        const T ap = (v == 4) ? Uf[d][1][4] + Wp[4] : Uf[d][1][v];
-                        dF[v] = ap * vp - am * vm;
-                    }
-                    dF[1 + d] += Wp[4] - Wm[4];
-#pragma unroll
-                    for (int v = 0; v < NV; ++v) dU[v] = (d == 0) ? dF[v] : dU[v] + dF[v];
                 }
-                // Hancock half step on all six face states, back to primitives, positivity check
-                T We[3][2][NV];
-                bool ok = true;
 #pragma unroll
-                for (int d = 0; d < 3; ++d)
-#pragma unroll
-                    for (int s = 0; s < 2; ++s) {
-                        T Ue[NV];
-#pragma unroll
-                        for (int v = 0; v < NV; ++v) Ue[v] = Uf[d][s][v] - ph.hlam * dU[v];
-                        cons2prim<T, NV>(Ue, We[d][s], ph);
-                        if (EXT && ph.floors) floor_prim(We[d][s], ph);
-                        ok = ok && (We[d][s][0] > T(0)) && (We[d][s][4] > T(0));
-                    }
-                if (!ok) {   // revert the cell's six states to the un-evolved face values
-                    cnt.reverted++;
-#pragma unroll
-                    for (int d = 0; d < 3; ++d)
-#pragma unroll
-                        for (int s = 0; s < 2; ++s) cons2prim<T, NV>(Uf[d][s], We[d][s], ph);
-                }
-                const int e = ej * G::EW + ei;
-                // rotated storage: array of axis d holds (rho, v_d, v_{d+1}, v_{d+2}, P [, q])
-#pragma unroll
-                for (int k = 0; k < NV; ++k) {
-                    es[(0 * NV + k) * G::EPL + e] = We[0][0][nat_index(0, k)];
-                    es[(1 * NV + k) * G::EPL + e] = We[0][1][nat_index(0, k)];
-                    es[(2 * NV + k) * G::EPL + e] = We[1][0][nat_index(1, k)];
-                    es[(3 * NV + k) * G::EPL + e] = We[1][1][nat_index(1, k)];
-                    es[(4 * NV + k) * G::EPL + e] = We[2][0][nat_index(2, k)];
-                    zcur[k * G::EPL + e] = We[2][1][nat_index(2, k)];
-                }
+                for (int k = 0; k < NV; ++k) zplus[k] = znew[k];
             }
         }
-        __syncthreads();
-        // ------------------------------------------------------------------ S2: Riemann + convert next plane
-        {
-            const int f_lo = (kk >= 0 && kk < PS) ? 0 : G::NFX + G::NFY;
-            const int f_hi = (kk >= 0 && kk <= PS) ? G::NF : 0;
-            const int zpar = ((kk + 1) & 1) * NV * G::EPL;      // z+ states of plane kk-1
-#pragma unroll
-            for (int r = 0; r < NROUND; ++r) {
-                const int f = tid + r * NT;
-                if (f >= f_lo && f < f_hi)
-                    cnt.roe_fb += riemann_face_rot<T, SOLVER, NV, TY>(es, fl, gflux, fdesc[r], f, zpar, kk, j0, ph);
-            }
-        }
+        // ------------------------------------------------------------------ halo warps: next plane -> primitives
         {
             const int n = kk + 2 + 2 * R;
-            if (n < NPL) {
+            if (!interior && n < NPL) {
                 mbar_wait(&bars[n & 1], (n >> 1) & 1);
-                convert_plane<T, NV, EXT, TY, NT>(raw + (n & 1) * NV * G::PLN, prim + ((PF + n) % PR) * NV * G::PLN, ph, ctid);
+                convert_plane<T, NV, EXT, TY, G::NCV>(raw + (n & 1) * S, prim + Q[2 * R + 1], ph, tid - NI);
             }
         }
         __syncthreads();
-        // ------------------------------------------------------------------ S3: update plane kk-1, prepare plane kk
-        if (tid == 0) {
+        if (tid == NI) {
             const int n = kk + 4 + 2 * R;
-            if (n < NPL) issue_plane<T, NV, TY>(gin, j0, PF + n, raw + (n & 1) * NV * G::PLN, &bars[n & 1]);
+            if (n < NPL) issue_plane<T, NV, TY>(gin, j0, PF + n, raw + (n & 1) * S, &bars[n & 1]);
         }
-        if (owner && kk >= 1) {
-            const int k = kk - 1;
-            const T* gcell = gin + (size_t)(k + NGH) * (NP * NP) + (j0 + cj + NGH) * NP + (ci + NGH);
-            T U[NV];
+        // ------------------------------------------------------------------ conserved input of cell (ei, ej, kk-1)
+        const bool upd = interior && kk >= 1;
+        const T* gcell = c.gin_cell + (kk - 1) * (NP * NP);
+        T U[NV];
+        if (upd) {
 #pragma unroll
-            for (int v = 0; v < NV; ++v) {
-                const T dfz = fl[rot_index(2, v) * G::NF + G::NFX + G::NFY + tid] - fzm[v];
-                U[v] = __ldg(gcell + (size_t)v * NPC) - ph.lam * (sxy[v] + dfz);
+            for (int v = 0; v < NV; ++v) U[v] = __ldg(gcell + (size_t)v * NPC);
+        }
+        // ------------------------------------------------------------------ x and y faces of plane kk
+        if (mid && own_x) {
+            T WL[NV], F[NV], fn[NV];
+            get_state<T, NV>(st_x, G::NSX, c.sx_own, WL);
+            cnt.roe_fb += riemann_flux<T, SOLVER, NV>(WL, xminus, F, ph) ? 1 : 0;
+#pragma unroll
+            for (int v = 0; v < NV; ++v) fn[v] = F[rot_index(0, v)];
+            put_state<T, NV>(fl_x, G::NSX, c.sx_own, fn);
+            if (c.fxo >= 0) {
+                T* q = c.gflux + c.fxo + kk * PS;
+#pragma unroll
+                for (int v = 0; v < NV; ++v) q[v * PSQ] = fn[v];
             }
-            close_cell<T, SOLVER, NV, EXT>(U, gcell, cnt, ph);
+        }
+        if (mid && own_y) {
+            T WL[NV], F[NV], fn[NV];
+            get_state<T, NV>(st_y, G::NSY, c.sy_own, WL);
+            cnt.roe_fb += riemann_flux<T, SOLVER, NV>(WL, yminus, F, ph) ? 1 : 0;
 #pragma unroll
-            for (int v = 0; v < NV; ++v) gout[((size_t)v * PS + k) * (PS * PS) + (j0 + cj) * PS + ci] = U[v];
+            for (int v = 0; v < NV; ++v) fn[v] = F[rot_index(1, v)];
+            put_state<T, NV>(fl_y, G::NSY, c.sy_own, fn);
+            if (c.fyo >= 0) {
+                T* q = c.gflux + c.fyo + kk * PS;
+#pragma unroll
+                for (int v = 0; v < NV; ++v) q[v * PSQ] = fn[v];
+            }
+        }
+        // ------------------------------------------------------------------ finish cell (ei, ej, kk-1)
+        if (upd) {   // its four x/y fluxes were published before the barrier
+            const T* pl_x = sm + G::FL + (par ^ 1) * G::BLK;
+            const T* pl_y = pl_x + NV * G::NSX;
+            T fl[NV], fr[NV], fd[NV], fu[NV];
+            get_state<T, NV>(pl_x, G::NSX, c.sx_own, fl);
+            get_state<T, NV>(pl_x, G::NSX, c.sx_own + 1, fr);
+            get_state<T, NV>(pl_y, G::NSY, c.sy_own, fd);
+            get_state<T, NV>(pl_y, G::NSY, c.sy_own + 16, fu);
+#pragma unroll
+            for (int v = 0; v < NV; ++v)
+                U[v] = U[v] - ph.lam * (((fr[v] - fl[v]) + (fu[v] - fd[v])) + (fzn[v] - fzl[v]));
+            close_cell<T, SOLVER, NV, EXT>(U, gcell, cnt, ph);
+            T* o = c.gout_cell + (kk - 1) * PSQ;
+#pragma unroll
+            for (int v = 0; v < NV; ++v) o[(size_t)v * (PS * PSQ)] = U[v];
             if (a.speed) {
                 const T s = signal_speed<T, NV, MHM, EXT>(U, ph);
                 if (s > smax) smax = s;
             }
         }
-        if (owner && kk >= 0 && kk < PS) {
+        if (interior && kk >= 0) {
 #pragma unroll
-            for (int v = 0; v < NV; ++v) {
-                const T* px = fl + rot_index(0, v) * G::NF + cj * 17 + ci;
-                const T* py = fl + rot_index(1, v) * G::NF + G::NFX + cj * 16 + ci;
-                const T dfx = px[1] - px[0];
-                const T dfy = py[16] - py[0];
-                sxy[v] = dfx + dfy;
-                fzm[v] = fl[rot_index(2, v) * G::NF + G::NFX + G::NFY + tid];
-            }
+            for (int v = 0; v < NV; ++v) fzl[v] = fzn[v];
+        }
+        // rotate the ring: the slot of the lowest plane is the one the plane after next is converted into
+        {
+            const int q0 = Q[0];
+#pragma unroll
+            for (int m = 0; m + 1 < RING; ++m) Q[m] = Q[m + 1];
+            Q[RING - 1] = q0;
         }
     }
 
