@@ -37,7 +37,7 @@ def algorithmic_bytes_per_cell(recon, sz, nv=5):
     return (n_in + nv * CELLS + 9 * nv * 256 + 1) * sz / CELLS
 
 
-# counted SASS FLOPs per cell update (FMA = 2; profiles/r01_flops.md), used for the ALU roofline
+# counted SASS FLOPs per cell update (FMA = 2; profiles/flops_per_cell.json from the ncu captures), used for the ALU roofline
 FLOPS_PER_CELL = {}
 
 
@@ -292,6 +292,15 @@ def main():
                          "flops_per_cell": fpc, "peak_source": f"148 SMs x {lanes} lanes x 2 x {sm_max} MHz"})
     else:
         roofline.update({"bound": "hbm", "achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_ach / hbm_peak})
+    ipc = FLOPS_PER_CELL.get(key + "_inst_per_cell")
+    if ipc:      # instruction-issue view of the same launch: warp instructions per second against 1 / clock / SM sub-partition
+        issue_peak = 148 * 4 * sm_max * 1e6 / 1e9
+        issue_ach = ipc / 32.0 * cells / (kern_ms * 1e-3) / 1e9
+        roofline["issue"] = {"achieved": issue_ach, "peak": issue_peak, "unit": "G warp-inst/s", "frac": issue_ach / issue_peak,
+                             "warp_inst_x32_per_cell": ipc,
+                             "note": "FP32 adds/multiplies count 1 FLOP but take the same issue slot as an FMA, and compares, "
+                                     "selects, min/max and shared-memory traffic take slots too: the FMA-only peak is not "
+                                     "reachable by this instruction mix (DESIGN.md section 6)"}
     tr = FLOPS_PER_CELL.get(key + "_dram_bytes_per_cell")
     roofline["traffic"] = tr * cells if tr else None
     roofline["hbm"] = {"achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_ach / hbm_peak,

@@ -131,10 +131,8 @@ __device__ __forceinline__ bool mhm_evolve(const T* Uf, const T* dU, T* We, bool
 template <typename T> struct MhmCell {
     int cidx;            // cell inside a staged plane
     int sx_own, sy_own;  // slot of the x+ (y+) state of the left (lower) neighbour = slot of the own lower-face flux
-    int fxo, fyo, fzo;   // offsets into the group's flux_out of this thread's patch-boundary faces, -1 if none
-    const T* gin_cell;   // padded cell (ei, ej, interior plane 0) of variable 0 in `in`
-    T* gout_cell;        // cell (ei, ej, plane 0) of variable 0 in `out`
-    T* gflux;            // flux_out of this group (nullable)
+    int gin_off;         // padded cell (ei, ej, interior plane 0) of variable 0, relative to the group's `in`
+    int out_off;         // cell (ei, ej) inside a 16 x 16 plane of `out` (also of a z plane of flux_out)
 };
 
 template <typename T, int RECON, int SOLVER, int NV, bool EXT, int TY, int MINB>
@@ -185,12 +183,14 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY>::NT), MINB) mhm_kern
     c.cidx = (ej + NGH) * NP + (ei + NGH);
     c.sx_own = ej * 17 + ei;
     c.sy_own = ej * 16 + ei;
-    c.gflux = a.flux ? a.flux + (size_t)g * 9 * NV * PSQ : nullptr;
-    c.fxo = (c.gflux && own_x && (ei & 7) == 0) ? ((0 * 3 + (ei >> 3)) * NV) * PSQ + gj : -1;
-    c.fyo = (c.gflux && own_y && (gj & 7) == 0) ? ((1 * 3 + (gj >> 3)) * NV) * PSQ + ei : -1;
-    c.fzo = (c.gflux && interior) ? (2 * 3 * NV) * PSQ + gj * PS + ei : -1;
-    c.gin_cell = gin + (size_t)NGH * (NP * NP) + (gj + NGH) * NP + (ei + NGH);
-    c.gout_cell = a.out + (size_t)g * NV * (PS * PSQ) + gj * PS + ei;
+    c.gin_off = NGH * (NP * NP) + (gj + NGH) * NP + (ei + NGH);
+    c.out_off = gj * PS + ei;
+    T* gout = a.out + (size_t)g * NV * (PS * PSQ);
+    T* gflux = a.flux ? a.flux + (size_t)g * 9 * NV * PSQ : nullptr;     // block-uniform
+    // patch-boundary x / y faces are copied from shared memory to flux_out by the halo warps,
+    // one plane late, when those warps would otherwise idle: faces i = 0, 8, 16 (x) and rows with gj = 0 mod 8 (y)
+    const int hid = tid - NI;
+    const int yrow0 = (8 - (j0 & 7)) & 7;      // first tile row whose lower face is a patch boundary
 
     if (tid == 0) {
         mbar_init(&bars[0], 1);
@@ -285,8 +285,8 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY>::NT), MINB) mhm_kern
                     cnt.roe_fb += riemann_flux<T, SOLVER, NV>(zplus, zminus, F, ph) ? 1 : 0;
 #pragma unroll
                     for (int v = 0; v < NV; ++v) fzn[v] = F[rot_index(2, v)];
-                    if (c.fzo >= 0 && (kk & 7) == 0) {
-                        T* q = c.gflux + c.fzo + (kk >> 3) * NV * PSQ;
+                    if (gflux != nullptr && (kk & 7) == 0) {      // block-uniform: a real branch
+                        T* q = gflux + (2 * 3 + (kk >> 3)) * NV * PSQ + c.out_off;
 #pragma unroll
                         for (int v = 0; v < NV; ++v) q[v * PSQ] = fzn[v];
                     }
@@ -310,7 +310,7 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY>::NT), MINB) mhm_kern
         }
         // ------------------------------------------------------------------ conserved input of cell (ei, ej, kk-1)
         const bool upd = interior && kk >= 1;
-        const T* gcell = c.gin_cell + (kk - 1) * (NP * NP);
+        const T* gcell = gin + c.gin_off + (kk - 1) * (NP * NP);
         T U[NV];
         if (upd) {
 #pragma unroll
@@ -324,11 +324,6 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY>::NT), MINB) mhm_kern
 #pragma unroll
             for (int v = 0; v < NV; ++v) fn[v] = F[rot_index(0, v)];
             put_state<T, NV>(fl_x, G::NSX, c.sx_own, fn);
-            if (c.fxo >= 0) {
-                T* q = c.gflux + c.fxo + kk * PS;
-#pragma unroll
-                for (int v = 0; v < NV; ++v) q[v * PSQ] = fn[v];
-            }
         }
         if (mid && own_y) {
             T WL[NV], F[NV], fn[NV];
@@ -337,8 +332,26 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY>::NT), MINB) mhm_kern
 #pragma unroll
             for (int v = 0; v < NV; ++v) fn[v] = F[rot_index(1, v)];
             put_state<T, NV>(fl_y, G::NSY, c.sy_own, fn);
-            if (c.fyo >= 0) {
-                T* q = c.gflux + c.fyo + kk * PS;
+        }
+        // ------------------------------------------------------------------ halo warps: boundary fluxes of plane kk-1
+        if (!interior && kk >= 1 && gflux != nullptr) {
+            const T* pl_x = sm + G::FL + (par ^ 1) * G::BLK;
+            const T* pl_y = pl_x + NV * G::NSX;
+            constexpr int NXF = 3 * TY, NYF = 3 * 16;
+            for (int f = hid; f < NXF + NYF; f += G::NCV) {
+                T fn[NV];
+                T* q;
+                if (f < NXF) {
+                    const int p = f / TY, j = f - p * TY;
+                    get_state<T, NV>(pl_x, G::NSX, j * 17 + 8 * p, fn);
+                    q = gflux + ((0 * 3 + p) * NV) * PSQ + (kk - 1) * PS + (j0 + j);
+                } else {
+                    const int h = f - NXF, r = h >> 4, i = h & 15;
+                    const int j = yrow0 + 8 * r;
+                    if (j > TY) continue;
+                    get_state<T, NV>(pl_y, G::NSY, j * 16 + i, fn);
+                    q = gflux + ((1 * 3 + ((j0 + j) >> 3)) * NV) * PSQ + (kk - 1) * PS + i;
+                }
 #pragma unroll
                 for (int v = 0; v < NV; ++v) q[v * PSQ] = fn[v];
             }
@@ -356,7 +369,7 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY>::NT), MINB) mhm_kern
             for (int v = 0; v < NV; ++v)
                 U[v] = U[v] - ph.lam * (((fr[v] - fl[v]) + (fu[v] - fd[v])) + (fzn[v] - fzl[v]));
             close_cell<T, SOLVER, NV, EXT>(U, gcell, cnt, ph);
-            T* o = c.gout_cell + (kk - 1) * PSQ;
+            T* o = gout + c.out_off + (kk - 1) * PSQ;
 #pragma unroll
             for (int v = 0; v < NV; ++v) o[(size_t)v * (PS * PSQ)] = U[v];
             if (a.speed) {
