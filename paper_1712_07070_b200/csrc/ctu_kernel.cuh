@@ -58,6 +58,54 @@ __device__ __forceinline__ int first_pass_face(const T* lp, int lidx, const T* r
     return fb;
 }
 
+// T stage for one cell t of the 18 x (TY+2) face-state plane and one direction D: PLM/PPM face values of
+// every variable along D, characteristic tracing over dt/2 (R7), revert of an unphysical pair (R8), store.
+template <typename T, int RECON, int NV, bool EXT, int TY, int D>
+__device__ __forceinline__ void ctu_trace_dir(const T* const* Pz, int t, T* tcur, const Phys<T>& ph, Counters& cnt) {
+    using G = Geo<TY>;
+    constexpr int R = RECON == PPM ? 2 : 1;
+    constexpr int EPL = G::EPL, EW = G::EW;
+    constexpr int cn = 1 + D, c1 = 1 + (D + 1) % 3, c2 = 1 + (D + 2) % 3;
+    const int ej = t / EW, ei = t - ej * EW;
+    const int c = (ej + 2) * NP + (ei + 2);
+    T wm[NV], wp[NV], Wc[NV];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) {
+        const T* q = Pz[R] + v * G::PLN + c;
+        Wc[v] = q[0];
+        if (D == 0) face_values<T, RECON, EXT, fixed_theta(EXT, RECON)>(q, 1, wm[v], wp[v], ph);
+        else if (D == 1) face_values<T, RECON, EXT, fixed_theta(EXT, RECON)>(q, NP, wm[v], wp[v], ph);
+        else {
+            const int o = v * G::PLN + c;
+            if (RECON == PPM)
+                face_values5<T, RECON, EXT>(Pz[0][o], Pz[R - 1][o], Pz[R][o], Pz[R + 1][o], Pz[2 * R][o], wm[v], wp[v], ph);
+            else
+                face_values5<T, RECON, EXT>(T(0), Pz[R - 1][o], Pz[R][o], Pz[R + 1][o], T(0), wm[v], wp[v], ph);
+        }
+    }
+    // rotate so that the traced axis is "n"
+    T Wr[NV], rm[NV], rp[NV], tm[NV], tp[NV];
+    Wr[0] = Wc[0]; Wr[1] = Wc[cn]; Wr[2] = Wc[c1]; Wr[3] = Wc[c2]; Wr[4] = Wc[4];
+    rm[0] = wm[0]; rm[1] = wm[cn]; rm[2] = wm[c1]; rm[3] = wm[c2]; rm[4] = wm[4];
+    rp[0] = wp[0]; rp[1] = wp[cn]; rp[2] = wp[c1]; rp[3] = wp[c2]; rp[4] = wp[4];
+    if (NV > 5) { Wr[NV - 1] = Wc[NV - 1]; rm[NV - 1] = wm[NV - 1]; rp[NV - 1] = wp[NV - 1]; }
+    trace_cell<T, RECON, NV>(Wr, rm, rp, tm, tp, ph);
+    if (EXT && ph.floors) { floor_prim(tm, ph); floor_prim(tp, ph); }
+    if (!(tm[0] > T(0) && tm[4] > T(0) && tp[0] > T(0) && tp[4] > T(0))) {
+        cnt.reverted++;
+#pragma unroll
+        for (int v = 0; v < NV; ++v) { tm[v] = rm[v]; tp[v] = rp[v]; }
+    }
+    T* sm_ = tcur + (2 * D) * NV * EPL + t;
+    T* sp_ = tcur + (2 * D + 1) * NV * EPL + t;
+    sm_[0] = tm[0];        sp_[0] = tp[0];
+    sm_[cn * EPL] = tm[1]; sp_[cn * EPL] = tp[1];
+    sm_[c1 * EPL] = tm[2]; sp_[c1 * EPL] = tp[2];
+    sm_[c2 * EPL] = tm[3]; sp_[c2 * EPL] = tp[3];
+    sm_[4 * EPL] = tm[4];  sp_[4 * EPL] = tp[4];
+    if (NV > 5) { sm_[(NV - 1) * EPL] = tm[NV - 1]; sp_[(NV - 1) * EPL] = tp[NV - 1]; }
+}
+
 template <typename T, int RECON, int SOLVER, int NV, bool EXT, int TY, int NT>
 __global__ void __launch_bounds__(NT) ctu_kernel(const AdvArgs<T> a) {
     using G = Geo<TY>;
@@ -120,56 +168,17 @@ __global__ void __launch_bounds__(NT) ctu_kernel(const AdvArgs<T> a) {
         T* tprev = ts + ((kk + 1) & 1) * 6 * NV * EPL;     // plane kk-1
         const int m = kk - 1;
         // ------------------------------------------------------------------ T(kk)
+        // work item = (direction, cell): 3 * EPL items spread over all NT threads
         if (kk <= PS) {
             const int pc = kk + NGH;
             const T* Pz[2 * R + 1];
 #pragma unroll
             for (int q = -R; q <= R; ++q) Pz[q + R] = prim + ((pc + q) % PR) * NV * G::PLN;
-            for (int t = tid; t < EPL; t += NT) {
-                const int ej = t / EW, ei = t - ej * EW;
-                const int c = (ej + 2) * NP + (ei + 2);
-                T Wc[NV];
-#pragma unroll
-                for (int v = 0; v < NV; ++v) Wc[v] = Pz[R][v * G::PLN + c];
-#pragma unroll
-                for (int d = 0; d < 3; ++d) {
-                    const int cn = 1 + d, c1 = 1 + (d + 1) % 3, c2 = 1 + (d + 2) % 3;
-                    T wm[NV], wp[NV];
-#pragma unroll
-                    for (int v = 0; v < NV; ++v) {
-                        const T* q = Pz[R] + v * G::PLN + c;
-                        if (d == 0) face_values<T, RECON, EXT, fixed_theta(EXT, RECON)>(q, 1, wm[v], wp[v], ph);
-                        else if (d == 1) face_values<T, RECON, EXT, fixed_theta(EXT, RECON)>(q, NP, wm[v], wp[v], ph);
-                        else {
-                            const int o = v * G::PLN + c;
-                            if (RECON == PPM)
-                                face_values5<T, RECON, EXT>(Pz[0][o], Pz[R - 1][o], Pz[R][o], Pz[R + 1][o], Pz[2 * R][o], wm[v], wp[v], ph);
-                            else
-                                face_values5<T, RECON, EXT>(T(0), Pz[R - 1][o], Pz[R][o], Pz[R + 1][o], T(0), wm[v], wp[v], ph);
-                        }
-                    }
-                    // rotate so that the traced axis is "n"
-                    T Wr[NV], rm[NV], rp[NV], tm[NV], tp[NV];
-                    Wr[0] = Wc[0]; Wr[1] = Wc[cn]; Wr[2] = Wc[c1]; Wr[3] = Wc[c2]; Wr[4] = Wc[4];
-                    rm[0] = wm[0]; rm[1] = wm[cn]; rm[2] = wm[c1]; rm[3] = wm[c2]; rm[4] = wm[4];
-                    rp[0] = wp[0]; rp[1] = wp[cn]; rp[2] = wp[c1]; rp[3] = wp[c2]; rp[4] = wp[4];
-                    if (NV > 5) { Wr[NV - 1] = Wc[NV - 1]; rm[NV - 1] = wm[NV - 1]; rp[NV - 1] = wp[NV - 1]; }
-                    trace_cell<T, RECON, NV>(Wr, rm, rp, tm, tp, ph);
-                    if (EXT && ph.floors) { floor_prim(tm, ph); floor_prim(tp, ph); }
-                    if (!(tm[0] > T(0) && tm[4] > T(0) && tp[0] > T(0) && tp[4] > T(0))) {
-                        cnt.reverted++;
-#pragma unroll
-                        for (int v = 0; v < NV; ++v) { tm[v] = rm[v]; tp[v] = rp[v]; }
-                    }
-                    T* sm_ = tcur + (2 * d) * NV * EPL + t;
-                    T* sp_ = tcur + (2 * d + 1) * NV * EPL + t;
-                    sm_[0] = tm[0];        sp_[0] = tp[0];
-                    sm_[cn * EPL] = tm[1]; sp_[cn * EPL] = tp[1];
-                    sm_[c1 * EPL] = tm[2]; sp_[c1 * EPL] = tp[2];
-                    sm_[c2 * EPL] = tm[3]; sp_[c2 * EPL] = tp[3];
-                    sm_[4 * EPL] = tm[4];  sp_[4 * EPL] = tp[4];
-                    if (NV > 5) { sm_[(NV - 1) * EPL] = tm[NV - 1]; sp_[(NV - 1) * EPL] = tp[NV - 1]; }
-                }
+            for (int item = tid; item < 3 * EPL; item += NT) {
+                const int d = item / EPL, t = item - d * EPL;
+                if (d == 0) ctu_trace_dir<T, RECON, NV, EXT, TY, 0>(Pz, t, tcur, ph, cnt);
+                else if (d == 1) ctu_trace_dir<T, RECON, NV, EXT, TY, 1>(Pz, t, tcur, ph, cnt);
+                else ctu_trace_dir<T, RECON, NV, EXT, TY, 2>(Pz, t, tcur, ph, cnt);
             }
         }
         __syncthreads();

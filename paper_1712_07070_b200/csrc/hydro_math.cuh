@@ -154,20 +154,18 @@ __device__ __forceinline__ void face_values(const T* q, int s, T& wm, T& wp, con
         const T s0 = limited_slope<T, EXT, THETA>(c - l1, r1 - c, ph);
         const T sp = limited_slope<T, EXT, THETA>(r1 - c, r2 - r1, ph);
         const T sixth = T(1.0 / 6.0);
-        T m = T(0.5) * (l1 + c) - (s0 - sm) * sixth;
-        T p = T(0.5) * (c + r1) - (sp - s0) * sixth;
-        if ((p - c) * (c - m) <= T(0)) {
-            m = c;
-            p = c;
-        } else {
-            const T D = p - m;
-            const T C = c - T(0.5) * (m + p);
-            const T DC = D * C, D6 = D * D * sixth;
-            if (DC > D6) m = T(3) * c - T(2) * p;
-            else if (DC < -D6) p = T(3) * c - T(2) * m;
-        }
-        wm = m;
-        wp = p;
+        const T m = T(0.5) * (l1 + c) - (s0 - sm) * sixth;
+        const T p = T(0.5) * (c + r1) - (sp - s0) * sixth;
+        // Monotonisation (CW84 eq. 1.10) written without branches.  With dm = c - m, dp = p - c:
+        //   (p-c)(c-m) <= 0                      <=>  dm, dp of opposite sign (or one is 0)  ->  dm = dp = 0
+        //   (p-m)(c-(m+p)/2) >  (p-m)^2/6        <=>  |dm| > 2|dp|                            ->  dm = 2 dp
+        //   (p-m)(c-(m+p)/2) < -(p-m)^2/6        <=>  |dp| > 2|dm|                            ->  dp = 2 dm
+        // i.e. dm <- sign * min(|dm|, 2|dp|), dp <- sign * min(|dp|, 2|dm|), both 0 for opposite signs.
+        const T dm = c - m, dp = p - c;
+        const T am = Ops<T>::minabs_same_sign(dm, dp + dp);
+        const T ap = Ops<T>::minabs_same_sign(dp, dm + dm);
+        wm = c - Ops<T>::copysign(am, dm);
+        wp = c + Ops<T>::copysign(ap, dp);
     }
 }
 

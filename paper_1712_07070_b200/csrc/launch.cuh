@@ -72,7 +72,11 @@ cudaError_t launch_ctu_ty(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
 
 template <typename T, int RECON, int SOLVER, int NV, bool EXT>
 cudaError_t launch_ctu(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
+#ifdef CTU_TY_OVERRIDE
+    constexpr int TY = (sizeof(T) == 4 && CtuSmem<T, RECON, NV, CTU_TY_OVERRIDE>::BYTES <= SMEM_LIMIT) ? CTU_TY_OVERRIDE : ctu_tile<T, RECON, NV>();
+#else
     constexpr int TY = ctu_tile<T, RECON, NV>();
+#endif
     return launch_ctu_ty<T, RECON, SOLVER, NV, EXT, TY>(a, st, launches);
 }
 #endif
