@@ -15,21 +15,27 @@ constexpr int mhm_tile() {
     return MhmGeo<T, RECON, NV, 16>::BYTES <= SMEM_LIMIT ? 16 : (MhmGeo<T, RECON, NV, 8>::BYTES <= SMEM_LIMIT ? 8 : 4);
 }
 
+constexpr size_t SM_SMEM = 233472;      // 228 KB of shared memory per SM, 1 KB of it reserved per resident CTA
+constexpr int ctas_by_smem(size_t bytes) { return (int)(SM_SMEM / (bytes + 1024)); }
+
 template <typename T, int RECON, int SOLVER, int NV, bool EXT>
 cudaError_t launch_mhm(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
-#ifndef MHM_MINB3
-#define MHM_MINB3 1
-#endif
 #ifdef MHM_TY_OVERRIDE
     constexpr int TY = MHM_TY_OVERRIDE;
 #else
     constexpr int TY = mhm_tile<T, RECON, NV>();
 #endif
-    using G = MhmGeo<T, RECON, NV, TY>;
+    // two TMA landing stages unless dropping to one lets a second CTA share the SM
+    constexpr int C2 = ctas_by_smem(MhmGeo<T, RECON, NV, TY, 2>::BYTES), C1 = ctas_by_smem(MhmGeo<T, RECON, NV, TY, 1>::BYTES);
+#ifdef MHM_FORCE_NSTG2
+    constexpr int NSTG = 2;
+#else
+    constexpr int NSTG = (C1 >= 2 && C2 < 2) ? 1 : 2;
+#endif
+    using G = MhmGeo<T, RECON, NV, TY, NSTG>;
     static_assert(G::BYTES <= SMEM_LIMIT, "tile does not fit in shared memory");
-    // two CTAs per SM when two tiles (plus the 1 KB the driver reserves per CTA) fit in the 228 KB of an SM
-    constexpr int MINB = (MHM_MINB3 && 3 * (G::BYTES + 1024) <= 233472 && G::NT <= 192) ? 3 : (2 * (G::BYTES + 1024) <= 233472) ? 2 : 1;
-    auto kern = mhm_kernel<T, RECON, SOLVER, NV, EXT, TY, MINB>;
+    constexpr int MINB = ctas_by_smem(G::BYTES) >= 2 ? 2 : 1;
+    auto kern = mhm_kernel<T, RECON, SOLVER, NV, EXT, TY, NSTG, MINB>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::BYTES);
     if (e != cudaSuccess) return e;
     if (G::NTILE > 1 && a.speed) {

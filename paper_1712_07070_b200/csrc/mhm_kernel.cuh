@@ -27,7 +27,7 @@ template <typename T> struct alignas(16) Vec4 {
     T a, b, c, d;
 };
 
-template <typename T, int RECON, int NV, int TY> struct MhmGeo {
+template <typename T, int RECON, int NV, int TY, int NSTG = 2> struct MhmGeo {
     static constexpr int R = RECON == PPM ? 2 : 1;
     static constexpr int RING = 2 * R + 2;
     static constexpr int NI = 16 * TY;                          // interior threads
@@ -38,8 +38,8 @@ template <typename T, int RECON, int NV, int TY> struct MhmGeo {
     static constexpr int NR = TY + 2 * NGH, PLN = NR * NP;      // staged plane
     static constexpr int NSX = 17 * TY, NSY = 16 * (TY + 1);    // x+ states / x fluxes, y+ states / y fluxes
     static constexpr int BLK = (NSX + NSY) * NV;                // one buffer of states (or of fluxes)
-    static constexpr int RAW = 0;                               // [2][NV][PLN]
-    static constexpr int PRIM = RAW + 2 * NV * PLN;             // [RING][NV][PLN]
+    static constexpr int RAW = 0;                               // [NSTG][NV][PLN]  TMA landing stages
+    static constexpr int PRIM = RAW + NSTG * NV * PLN;          // [RING][NV][PLN]
     static constexpr int ST = PRIM + RING * NV * PLN;           // [2] x [Vec4 NSX | (NV-4) NSX | Vec4 NSY | (NV-4) NSY]
     static constexpr int FL = ST + 2 * BLK;                     // same shape, fluxes in natural variable order
     static constexpr int END = FL + 2 * BLK;
@@ -135,9 +135,9 @@ template <typename T> struct MhmCell {
     int out_off;         // cell (ei, ej) inside a 16 x 16 plane of `out` (also of a z plane of flux_out)
 };
 
-template <typename T, int RECON, int SOLVER, int NV, bool EXT, int TY, int MINB>
-__global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY>::NT), MINB) mhm_kernel(const AdvArgs<T> a) {
-    using G = MhmGeo<T, RECON, NV, TY>;
+template <typename T, int RECON, int SOLVER, int NV, bool EXT, int TY, int NSTG, int MINB>
+__global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG>::NT), MINB) mhm_kernel(const AdvArgs<T> a) {
+    using G = MhmGeo<T, RECON, NV, TY, NSTG>;
     constexpr int R = G::R, RING = G::RING, NT = G::NT, NI = G::NI, PLN = G::PLN, S = NV * G::PLN;
     constexpr int NPL = 18 + 2 * R;      // staged planes: padded PF .. PF+NPL-1
     constexpr int PF = 2 - R;
@@ -200,14 +200,14 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY>::NT), MINB) mhm_kern
     __syncthreads();
     if (tid == NI) {
         issue_plane<T, NV, TY>(gin, j0, PF + 0, raw, &bars[0]);
-        issue_plane<T, NV, TY>(gin, j0, PF + 1, raw + S, &bars[1]);
+        if (NSTG > 1) issue_plane<T, NV, TY>(gin, j0, PF + 1, raw + S, &bars[1]);
     }
     // prologue: staged planes n = 0 .. 2R (what the predictor of plane -1 reads), all threads convert
     for (int n = 0; n <= 2 * R; ++n) {
-        mbar_wait(&bars[n & 1], (n >> 1) & 1);
-        convert_plane<T, NV, EXT, TY, NT>(raw + (n & 1) * S, prim + n * S, ph, tid);
+        mbar_wait(&bars[n % NSTG], (n / NSTG) & 1);
+        convert_plane<T, NV, EXT, TY, NT>(raw + (n % NSTG) * S, prim + n * S, ph, tid);
         __syncthreads();
-        if (tid == NI && n + 2 < NPL) issue_plane<T, NV, TY>(gin, j0, PF + n + 2, raw + (n & 1) * S, &bars[n & 1]);
+        if (tid == NI && n + NSTG < NPL) issue_plane<T, NV, TY>(gin, j0, PF + n + NSTG, raw + (n % NSTG) * S, &bars[n % NSTG]);
     }
 
     T zplus[NV];                    // z+ state of the plane below (rotated for z)
@@ -299,14 +299,14 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY>::NT), MINB) mhm_kern
         {
             const int n = kk + 2 + 2 * R;
             if (!interior && n < NPL) {
-                mbar_wait(&bars[n & 1], (n >> 1) & 1);
-                convert_plane<T, NV, EXT, TY, G::NCV>(raw + (n & 1) * S, prim + Q[2 * R + 1], ph, tid - NI);
+                mbar_wait(&bars[n % NSTG], (n / NSTG) & 1);
+                convert_plane<T, NV, EXT, TY, G::NCV>(raw + (n % NSTG) * S, prim + Q[2 * R + 1], ph, tid - NI);
             }
         }
         __syncthreads();
-        if (tid == NI) {
-            const int n = kk + 4 + 2 * R;
-            if (n < NPL) issue_plane<T, NV, TY>(gin, j0, PF + n, raw + (n & 1) * S, &bars[n & 1]);
+        if (tid == NI) {      // the stage the plane above came from is free again
+            const int n = kk + 2 + 2 * R + NSTG;
+            if (n < NPL) issue_plane<T, NV, TY>(gin, j0, PF + n, raw + (n % NSTG) * S, &bars[n % NSTG]);
         }
         // ------------------------------------------------------------------ conserved input of cell (ei, ej, kk-1)
         const bool upd = interior && kk >= 1;
