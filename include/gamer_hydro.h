@@ -102,6 +102,24 @@ int gamer_cfl_from_group_speed(const void* group_speed, int64_t n_groups, double
 int gamer_refresh_ghosts_periodic(const void* u, void* in, int gz, int gy, int gx, int nvar,
                                   int precision, void* stream);
 
+/* Device-resident step with the same-level ghost refresh FUSED into the staging loads (SURVEY 8(f) NEXT-1,
+ * PAPER.md L248 "preparation" + L274 Fig. 3): `u` is the UNPADDED state of the whole batch,
+ * u[n_groups][NVAR][16][16][16] (the `out` layout), and nbr[n_groups][27] (device int32) names, for every group,
+ * the group that holds each of its 27 same-level neighbours, index (dz+1)*9 + (dy+1)*3 + (dx+1) with
+ * d* in {-1,0,+1} (entry 13 = the group itself); every entry must be in [0, n_groups).  The kernel gathers each
+ * padded plane from those groups directly, so no padded copy of the batch exists in memory; results are
+ * bit-identical to gamer_refresh_ghosts_periodic / a host gather followed by gamer_fluid_advance_ex.
+ * u and out must not overlap (every group reads its neighbours' old state).  opts may be NULL.
+ * Supported: scheme = GAMER_MHM (any recon / riemann / precision, all opts except remedy_first_order);
+ * anything else returns GAMER_EUNSUPPORTED -- use the refresh + gamer_fluid_advance_ex pair there. */
+int gamer_fluid_advance_resident(const void* u, const int32_t* nbr, void* out, void* flux_out, int64_t n_groups,
+                                 double dt, double dh, double gamma,
+                                 int scheme, int recon, int riemann, int precision,
+                                 const gamer_opts* opts);
+
+/* Fills nbr[gz*gy*gx][27] (device int32) for a periodic box of gz x gy x gx groups, g = (z*gy + y)*gx + x. */
+int gamer_neighbors_periodic(int32_t* nbr, int gz, int gy, int gx, void* stream);
+
 /* End-to-end form with HOST buffers (pinned or pageable): copies `in` to the device in chunks,
  * runs the solver, copies `out`, `flux_out` (nullable) and `group_speed_out` (nullable) back,
  * overlapping copies and kernels on internal streams as the paper does with CUDA streams (L242),

@@ -20,7 +20,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libgamerhydro.so")
 
 EXPORTS = ["gamer_fluid_advance", "gamer_fluid_advance_ex", "gamer_cfl_dt", "gamer_cfl_dt_ex",
-           "gamer_cfl_from_group_speed", "gamer_refresh_ghosts_periodic", "gamer_fluid_advance_host",
+           "gamer_cfl_from_group_speed", "gamer_refresh_ghosts_periodic", "gamer_fluid_advance_resident",
+           "gamer_neighbors_periodic", "gamer_fluid_advance_host",
            "gamer_launch_count", "gamer_strerror", "gamer_version"]
 
 
@@ -67,6 +68,8 @@ def lib():
         L.gamer_cfl_dt_ex.argtypes = cfl + [ctypes.POINTER(gamer_opts)]
         L.gamer_cfl_from_group_speed.argtypes = [vp, i64, dbl, dbl, ci, vp, vp]
         L.gamer_refresh_ghosts_periodic.argtypes = [vp, vp, ci, ci, ci, ci, ci, vp]
+        L.gamer_fluid_advance_resident.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, ci, ci, ctypes.POINTER(gamer_opts)]
+        L.gamer_neighbors_periodic.argtypes = [vp, ci, ci, ci, vp]
         L.gamer_fluid_advance_host.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, ci, ci,
                                                ctypes.POINTER(gamer_opts)]
         L.gamer_launch_count.restype = ctypes.c_int64
@@ -151,6 +154,24 @@ def gamer_cfl_from_group_speed(group_speed, dh, cfl, dt_out, stream=None):
 def gamer_refresh_ghosts_periodic(u, u_in, gz, gy, gx, stream=None):
     _check(lib().gamer_refresh_ghosts_periodic(_ptr(u), _ptr(u_in), gz, gy, gx, u.shape[1], _precision(u),
                                                _stream_handle(stream)), "gamer_refresh_ghosts_periodic")
+
+
+def gamer_fluid_advance_resident(u, nbr, out, flux_out, dt, dh, gamma, scheme, recon, riemann, opts=None):
+    """Unpadded state + same-level neighbour table in, unpadded state out: the ghost refresh is fused into the kernel."""
+    if nbr.dtype != torch.int32 or tuple(nbr.shape) != (u.shape[0], 27):
+        raise GamerError("nbr must be an int32 tensor of shape [n_groups, 27]")
+    if opts is None:
+        opts = make_opts()
+    _check(lib().gamer_fluid_advance_resident(_ptr(u), _ptr(nbr), _ptr(out), _ptr(flux_out), u.shape[0], float(dt), float(dh),
+                                              float(gamma), int(scheme), int(recon), int(riemann), _precision(u),
+                                              ctypes.byref(opts)), "gamer_fluid_advance_resident")
+
+
+def gamer_neighbors_periodic(gz, gy, gx, device, stream=None):
+    """[gz*gy*gx, 27] int32 neighbour table of a periodic box of groups."""
+    nbr = torch.empty((gz * gy * gx, 27), dtype=torch.int32, device=device)
+    _check(lib().gamer_neighbors_periodic(_ptr(nbr), gz, gy, gx, _stream_handle(stream)), "gamer_neighbors_periodic")
+    return nbr
 
 
 def gamer_fluid_advance_host(in_host, out_host, flux_out_host, group_speed_out_host, dt, dh, gamma, scheme, recon,

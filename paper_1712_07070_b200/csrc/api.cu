@@ -37,9 +37,11 @@ static int check_common(const void* in, const void* out, int64_t n_groups, doubl
 
 template <typename T>
 static int advance_typed(const void* in, void* out, void* flux_out, int64_t n_groups, double dt, double dh,
-                         double gamma, int scheme, int recon, int riemann, const gamer_opts* o) {
+                         double gamma, int scheme, int recon, int riemann, const gamer_opts* o,
+                         const int32_t* nbr = nullptr) {
     AdvArgs<T> a;
     std::memset(&a, 0, sizeof(a));
+    a.nbr = nbr;
     a.in = static_cast<const T*>(in);
     a.out = static_cast<T*>(out);
     a.flux = static_cast<T*>(flux_out);
@@ -100,6 +102,39 @@ extern "C" int gamer_fluid_advance(const void* in, void* out, void* flux_out, in
                                    double gamma, int scheme, int recon, int riemann, int precision) {
     return gamer_fluid_advance_ex(in, out, flux_out, n_groups, dt, dh, gamma, scheme, recon, riemann, precision,
                                   nullptr);
+}
+
+extern "C" int gamer_fluid_advance_resident(const void* u, const int32_t* nbr, void* out, void* flux_out, int64_t n_groups,
+                                            double dt, double dh, double gamma, int scheme, int recon, int riemann,
+                                            int precision, const gamer_opts* opts) {
+    int rc = check_common(u, out, n_groups, dh, gamma, scheme, recon, riemann, precision);
+    if (rc) return rc;
+    if (n_groups > 0 && !nbr) return GAMER_EINVAL;
+    const bool dev_dt = opts && opts->dt_dev;
+    if (!dev_dt && (!(dt > 0.0) || !std::isfinite(dt))) return GAMER_EINVAL;
+    if (flux_out && !aligned16(flux_out)) return GAMER_EINVAL;
+    if (opts) {
+        if (opts->n_scalar < 0 || opts->n_scalar > 1) return GAMER_EINVAL;
+        if (opts->dual_energy && opts->n_scalar != 1) return GAMER_EINVAL;
+        if (opts->limiter < 0 || opts->limiter > GAMER_LIMITER_VANALBADA) return GAMER_EINVAL;
+        if (opts->min_dens < 0 || opts->min_pres < 0 || opts->min_temp < 0) return GAMER_EINVAL;
+        if (opts->remedy_first_order) return GAMER_EUNSUPPORTED;   // remedy (ii) re-reads the padded slab
+    }
+    if (scheme != GAMER_MHM) return GAMER_EUNSUPPORTED;
+    if (n_groups > 0x3fffffff / 27) return GAMER_EUNSUPPORTED;
+    if (u == out) return GAMER_EINVAL;
+    return precision == GAMER_FP32
+               ? advance_typed<float>(u, out, flux_out, n_groups, dt, dh, gamma, scheme, recon, riemann, opts, nbr)
+               : advance_typed<double>(u, out, flux_out, n_groups, dt, dh, gamma, scheme, recon, riemann, opts, nbr);
+}
+
+extern "C" int gamer_neighbors_periodic(int32_t* nbr, int gz, int gy, int gx, void* stream) {
+    if (!nbr || gz < 1 || gy < 1 || gx < 1) return GAMER_EINVAL;
+    const long long n = (long long)gz * gy * gx * 27;
+    if (n > 0x7fffffff) return GAMER_EUNSUPPORTED;
+    neighbors_periodic_kernel<<<(unsigned)((n + 255) / 256), 256, 0, static_cast<cudaStream_t>(stream)>>>(nbr, gz, gy, gx);
+    g_launches += 1;
+    return cudaGetLastError() == cudaSuccess ? GAMER_OK : GAMER_ECUDA;
 }
 
 // ------------------------------------------------------------------------------------------ CFL

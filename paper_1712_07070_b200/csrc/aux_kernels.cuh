@@ -130,4 +130,17 @@ __global__ void __launch_bounds__(256) refresh_periodic_kernel(const T* __restri
     }
 }
 
+// neighbour table of a periodic box of gz x gy x gx groups: nbr[g][(dz+1)*9 + (dy+1)*3 + (dx+1)]
+__global__ void neighbors_periodic_kernel(int* __restrict__ nbr, int gz, int gy, int gx) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long ng = (long long)gz * gy * gx;
+    if (i >= ng * 27) return;
+    const long long g = i / 27;
+    const int k = (int)(i - g * 27);
+    const int dx = k % 3 - 1, dy = (k / 3) % 3 - 1, dz = k / 9 - 1;
+    const int bx = (int)(g % gx), by = (int)((g / gx) % gy), bz = (int)(g / ((long long)gx * gy));
+    const int sx = (bx + dx + gx) % gx, sy = (by + dy + gy) % gy, sz = (bz + dz + gz) % gz;
+    nbr[i] = (int)(((long long)sz * gy + sy) * gx + sx);
+}
+
 }  // namespace gamer

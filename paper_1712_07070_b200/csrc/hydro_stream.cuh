@@ -25,6 +25,7 @@ template <typename T> struct AdvArgs {
     int* n_unphys;    // nullable
     int* diag;        // nullable, int[4]
     const double* dt_dev;
+    const int* nbr;   // nullable: [n_groups][27] same-level neighbour table => `in` is the UNPADDED state (fused refresh)
     double dt, dh, gamma, theta, xi, min_dens, min_pres, min_temp;
     int limiter, dual, remedy2;
     long long n_groups;
@@ -140,6 +141,91 @@ __device__ __forceinline__ void convert_plane(const T* raw, T* prim, const Phys<
         T U[NV], W[NV];
 #pragma unroll
         for (int v = 0; v < NV; ++v) U[v] = raw[v * G::PLN + t];
+        cons2prim<T, NV>(U, W, ph);
+        if (EXT && ph.floors) floor_prim(W, ph);
+#pragma unroll
+        for (int v = 0; v < NV; ++v) prim[v * G::PLN + t] = W[v];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Fused ghost refresh: the padded plane is gathered straight from the
+// unpadded state of the group and of its same-level neighbours with cp.async (LDGSTS), so no padded copy of the
+// batch ever exists in HBM.  Staged rows are 24 wide with the 16 interior cells at columns 4..19 (16-byte aligned
+// for the wide copies), ghosts at 1..3 and 20..22.  nb = the 27 neighbour group indices of this group.
+// ---------------------------------------------------------------------------------------------
+constexpr int FW = 24;   // row stride of a staged plane in fused mode
+
+__device__ __forceinline__ void cp_async_16(void* dst, const void* src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
+}
+template <int BYTES> __device__ __forceinline__ void cp_async_small(void* dst, const void* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(smem_u32(dst)), "l"(src), "n"(BYTES) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+// wait until at most N of this thread's committed copy groups are still in flight
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// One copy of the gather of a padded plane: destination element inside the landing stage, source element inside a
+// group's plane z (v*16^3 + y*16 + x), which in-plane neighbour (dy*3 + dx) holds it, and whether it is a 16-byte
+// copy.  The list is the same for every plane, so it is built once per CTA (fused_copy_table) and each thread
+// issues the same few entries for every plane.
+template <typename T, int NV, int TY> struct FusedCopies {
+    static constexpr int CE = 16 / (int)sizeof(T);          // elements per 16-byte copy
+    static constexpr int OPS = PS / CE + 2 * NGH;           // copies per row and variable
+    static constexpr int N = Geo<TY>::NR * NV * OPS;
+};
+
+template <typename T, int NV, int TY>
+__device__ __forceinline__ void fused_copy_table(int2* tab, int j0, int tid, int nthr) {
+    using G = Geo<TY>;
+    using F = FusedCopies<T, NV, TY>;
+    constexpr int PS3 = PS * PS * PS;
+    for (int it = tid; it < F::N; it += nthr) {
+        const int op = it % F::OPS, rv = it / F::OPS;
+        const int r = rv % G::NR, v = rv / G::NR;
+        const int py = j0 + r;
+        const int dy = py < NGH ? 0 : (py < NGH + PS ? 1 : 2);
+        const int yy = (py + PS - NGH) & (PS - 1);
+        int dx, xx, col, wide;
+        if (op < PS / F::CE) { dx = 1; xx = op * F::CE; col = 4 + xx; wide = 1; }
+        else {
+            const int q = op - PS / F::CE;
+            dx = q < NGH ? 0 : 2;
+            xx = q < NGH ? PS - NGH + q : q - NGH;
+            col = q < NGH ? 1 + q : 4 + PS + (q - NGH);
+            wide = 0;
+        }
+        tab[it] = make_int2((v * G::NR + r) * FW + col, (v * PS3 + yy * PS + xx) | ((dy * 3 + dx) << 20) | (wide << 24));
+    }
+}
+
+// every thread issues its entries of the list for padded plane p (0..21) and commits them as one group
+template <typename T, int NV, int TY>
+__device__ __forceinline__ void stage_plane_fused(const T* u, const int* nb, const int2* tab, int p, T* raw_stage, int tid, int nthr) {
+    using F = FusedCopies<T, NV, TY>;
+    constexpr int PS3 = PS * PS * PS;
+    const int dz = p < NGH ? 0 : (p < NGH + PS ? 1 : 2);
+    const int zoff = ((p + PS - NGH) & (PS - 1)) * (PS * PS);
+    const int* nbz = nb + dz * 9;
+    for (int it = tid; it < F::N; it += nthr) {
+        const int2 d = tab[it];
+        const T* src = u + (size_t)nbz[(d.y >> 20) & 15] * NV * PS3 + ((d.y & 0xfffff) + zoff);
+        if (d.y >> 24) cp_async_16(raw_stage + d.x, src);
+        else cp_async_small<(int)sizeof(T)>(raw_stage + d.x, src);
+    }
+    cp_async_commit();
+}
+
+// raw conserved plane in the fused layout -> primitive plane in the standard [NV][NR*22] layout
+template <typename T, int NV, bool EXT, int TY, int NT>
+__device__ __forceinline__ void convert_plane_fused(const T* raw, T* prim, const Phys<T>& ph, int tid) {
+    using G = Geo<TY>;
+    for (int t = tid; t < G::PLN; t += NT) {
+        const int r = t / NP, cx = t - r * NP;
+        T U[NV], W[NV];
+#pragma unroll
+        for (int v = 0; v < NV; ++v) U[v] = raw[(v * G::NR + r) * FW + cx + 1];
         cons2prim<T, NV>(U, W, ph);
         if (EXT && ph.floors) floor_prim(W, ph);
 #pragma unroll

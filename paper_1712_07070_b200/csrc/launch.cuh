@@ -18,24 +18,24 @@ constexpr int mhm_tile() {
 constexpr size_t SM_SMEM = 233472;      // 228 KB of shared memory per SM, 1 KB of it reserved per resident CTA
 constexpr int ctas_by_smem(size_t bytes) { return (int)(SM_SMEM / (bytes + 1024)); }
 
-template <typename T, int RECON, int SOLVER, int NV, bool EXT>
-cudaError_t launch_mhm(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
+template <typename T, int RECON, int SOLVER, int NV, bool EXT, bool FUSED>
+cudaError_t launch_mhm_f(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
 #ifdef MHM_TY_OVERRIDE
     constexpr int TY = MHM_TY_OVERRIDE;
 #else
     constexpr int TY = mhm_tile<T, RECON, NV>();
 #endif
-    // two TMA landing stages unless dropping to one lets a second CTA share the SM
-    constexpr int C2 = ctas_by_smem(MhmGeo<T, RECON, NV, TY, 2>::BYTES), C1 = ctas_by_smem(MhmGeo<T, RECON, NV, TY, 1>::BYTES);
+    // two landing stages unless dropping to one lets a second CTA share the SM
+    constexpr int C2 = ctas_by_smem(MhmGeo<T, RECON, NV, TY, 2, FUSED>::BYTES), C1 = ctas_by_smem(MhmGeo<T, RECON, NV, TY, 1, FUSED>::BYTES);
 #ifdef MHM_FORCE_NSTG2
     constexpr int NSTG = 2;
 #else
-    constexpr int NSTG = (C1 >= 2 && C2 < 2) ? 1 : 2;
+    constexpr int NSTG = (!FUSED && C1 >= 2 && C2 < 2) ? 1 : 2;      // the fused gather is pipelined over two stages
 #endif
-    using G = MhmGeo<T, RECON, NV, TY, NSTG>;
+    using G = MhmGeo<T, RECON, NV, TY, NSTG, FUSED>;
     static_assert(G::BYTES <= SMEM_LIMIT, "tile does not fit in shared memory");
     constexpr int MINB = ctas_by_smem(G::BYTES) >= 2 ? 2 : 1;
-    auto kern = mhm_kernel<T, RECON, SOLVER, NV, EXT, TY, NSTG, MINB>;
+    auto kern = mhm_kernel<T, RECON, SOLVER, NV, EXT, TY, NSTG, MINB, FUSED>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::BYTES);
     if (e != cudaSuccess) return e;
     if (G::NTILE > 1 && a.speed) {
@@ -46,6 +46,13 @@ cudaError_t launch_mhm(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
     kern<<<(unsigned)grid, G::NT, G::BYTES, st>>>(a);
     *launches += 1;
     return cudaGetLastError();
+}
+
+// a.nbr set => `in` is the unpadded state and the ghost refresh is fused into the staging loads
+template <typename T, int RECON, int SOLVER, int NV, bool EXT>
+cudaError_t launch_mhm(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
+    return a.nbr ? launch_mhm_f<T, RECON, SOLVER, NV, EXT, true>(a, st, launches)
+                 : launch_mhm_f<T, RECON, SOLVER, NV, EXT, false>(a, st, launches);
 }
 
 #ifdef GAMER_HAVE_CTU

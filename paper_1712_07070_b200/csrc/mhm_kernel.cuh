@@ -27,7 +27,7 @@ template <typename T> struct alignas(16) Vec4 {
     T a, b, c, d;
 };
 
-template <typename T, int RECON, int NV, int TY, int NSTG = 2> struct MhmGeo {
+template <typename T, int RECON, int NV, int TY, int NSTG = 2, bool FUSED = false> struct MhmGeo {
     static constexpr int R = RECON == PPM ? 2 : 1;
     static constexpr int RING = 2 * R + 2;
     static constexpr int NI = 16 * TY;                          // interior threads
@@ -38,12 +38,15 @@ template <typename T, int RECON, int NV, int TY, int NSTG = 2> struct MhmGeo {
     static constexpr int NR = TY + 2 * NGH, PLN = NR * NP;      // staged plane
     static constexpr int NSX = 17 * TY, NSY = 16 * (TY + 1);    // x+ states / x fluxes, y+ states / y fluxes
     static constexpr int BLK = (NSX + NSY) * NV;                // one buffer of states (or of fluxes)
-    static constexpr int RAW = 0;                               // [NSTG][NV][PLN]  TMA landing stages
-    static constexpr int PRIM = RAW + NSTG * NV * PLN;          // [RING][NV][PLN]
+    static constexpr int RSTG = NV * (FUSED ? NR * FW : PLN);   // one landing stage (fused refresh: 24-wide rows)
+    static constexpr int RAW = 0;                               // [NSTG][RSTG]  TMA / cp.async landing stages
+    static constexpr int PRIM = RAW + NSTG * RSTG;              // [RING][NV][PLN]
     static constexpr int ST = PRIM + RING * NV * PLN;           // [2] x [Vec4 NSX | (NV-4) NSX | Vec4 NSY | (NV-4) NSY]
     static constexpr int FL = ST + 2 * BLK;                     // same shape, fluxes in natural variable order
     static constexpr int END = FL + 2 * BLK;
-    static constexpr size_t BYTES = 16 + (size_t)END * sizeof(T);   // 2 mbarriers first
+    static constexpr int NCOPY = FUSED ? FusedCopies<T, NV, TY>::N : 0;                   // fused refresh: copy list
+    static constexpr size_t BYTES = 16 + (size_t)END * sizeof(T) + (FUSED ? 128 + 8 * (size_t)NCOPY : 0);   // 2 mbarriers
+                                                                // first; neighbour table and copy list last
     static_assert((NV * PLN) % 4 == 0 && NSX % 4 == 0 && NSY % 4 == 0, "16-byte alignment of the Vec4 arrays");
 };
 
@@ -135,9 +138,10 @@ template <typename T> struct MhmCell {
     int out_off;         // cell (ei, ej) inside a 16 x 16 plane of `out` (also of a z plane of flux_out)
 };
 
-template <typename T, int RECON, int SOLVER, int NV, bool EXT, int TY, int NSTG, int MINB>
-__global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG>::NT), MINB) mhm_kernel(const AdvArgs<T> a) {
-    using G = MhmGeo<T, RECON, NV, TY, NSTG>;
+template <typename T, int RECON, int SOLVER, int NV, bool EXT, int TY, int NSTG, int MINB, bool FUSED>
+__global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED>::NT), MINB) mhm_kernel(const AdvArgs<T> a) {
+    using G = MhmGeo<T, RECON, NV, TY, NSTG, FUSED>;
+    constexpr int RS = G::RSTG;
     constexpr int R = G::R, RING = G::RING, NT = G::NT, NI = G::NI, PLN = G::PLN, S = NV * G::PLN;
     constexpr int NPL = 18 + 2 * R;      // staged planes: padded PF .. PF+NPL-1
     constexpr int PF = 2 - R;
@@ -153,7 +157,14 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG>::NT), MINB) mh
     const long long tile = blockIdx.x;
     const long long g = tile / G::NTILE;
     const int j0 = (int)(tile % G::NTILE) * TY;
-    const T* gin = a.in + (size_t)g * NV * NPC;
+    // padded mode: this group's padded slab; fused mode: the whole unpadded batch (neighbours are read too)
+    const T* gin = FUSED ? a.in : a.in + (size_t)g * NV * NPC;
+    int* nb = reinterpret_cast<int*>(smem_raw + 16 + G::END * sizeof(T));      // fused mode: 27 neighbour groups
+    int2* ctab = reinterpret_cast<int2*>(smem_raw + 16 + G::END * sizeof(T) + 128);
+    if (FUSED) {
+        if (tid < 27) nb[tid] = a.nbr[g * 27 + tid];
+        fused_copy_table<T, NV, TY>(ctab, j0, tid, NT);
+    }
     const Phys<T> ph = make_phys<T>(a);
 
     // ---- role of this thread: cell (ei, ej) of the tile, ei in -1..16, ej in -1..TY
@@ -198,16 +209,28 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG>::NT), MINB) mh
         mbar_fence_init();
     }
     __syncthreads();
-    if (tid == NI) {
+    if (FUSED) {      // every thread issues a few copies of each plane (cp.async groups are per thread)
+        stage_plane_fused<T, NV, TY>(gin, nb, ctab, PF + 0, raw, tid, NT);
+        stage_plane_fused<T, NV, TY>(gin, nb, ctab, PF + 1, raw + RS, tid, NT);
+    } else if (tid == NI) {
         issue_plane<T, NV, TY>(gin, j0, PF + 0, raw, &bars[0]);
-        if (NSTG > 1) issue_plane<T, NV, TY>(gin, j0, PF + 1, raw + S, &bars[1]);
+        if (NSTG > 1) issue_plane<T, NV, TY>(gin, j0, PF + 1, raw + RS, &bars[1]);
     }
     // prologue: staged planes n = 0 .. 2R (what the predictor of plane -1 reads), all threads convert
     for (int n = 0; n <= 2 * R; ++n) {
-        mbar_wait(&bars[n % NSTG], (n / NSTG) & 1);
-        convert_plane<T, NV, EXT, TY, NT>(raw + (n % NSTG) * S, prim + n * S, ph, tid);
+        if (FUSED) {
+            cp_async_wait<0>();
+            __syncthreads();
+            convert_plane_fused<T, NV, EXT, TY, NT>(raw + (n % NSTG) * RS, prim + n * S, ph, tid);
+        } else {
+            mbar_wait(&bars[n % NSTG], (n / NSTG) & 1);
+            convert_plane<T, NV, EXT, TY, NT>(raw + (n % NSTG) * RS, prim + n * S, ph, tid);
+        }
         __syncthreads();
-        if (tid == NI && n + NSTG < NPL) issue_plane<T, NV, TY>(gin, j0, PF + n + NSTG, raw + (n % NSTG) * S, &bars[n % NSTG]);
+        if (n + NSTG < NPL) {
+            if (FUSED) stage_plane_fused<T, NV, TY>(gin, nb, ctab, PF + n + NSTG, raw + (n % NSTG) * RS, tid, NT);
+            else if (tid == NI) issue_plane<T, NV, TY>(gin, j0, PF + n + NSTG, raw + (n % NSTG) * RS, &bars[n % NSTG]);
+        }
     }
 
     T zplus[NV];                    // z+ state of the plane below (rotated for z)
@@ -299,22 +322,32 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG>::NT), MINB) mh
         {
             const int n = kk + 2 + 2 * R;
             if (!interior && n < NPL) {
-                mbar_wait(&bars[n % NSTG], (n / NSTG) & 1);
-                convert_plane<T, NV, EXT, TY, G::NCV>(raw + (n % NSTG) * S, prim + Q[2 * R + 1], ph, tid - NI);
+                if (FUSED) {      // this plane's copies were waited for before the previous barrier
+                    convert_plane_fused<T, NV, EXT, TY, G::NCV>(raw + (n % NSTG) * RS, prim + Q[2 * R + 1], ph, tid - NI);
+                } else {
+                    mbar_wait(&bars[n % NSTG], (n / NSTG) & 1);
+                    convert_plane<T, NV, EXT, TY, G::NCV>(raw + (n % NSTG) * RS, prim + Q[2 * R + 1], ph, tid - NI);
+                }
             }
         }
+        if (FUSED) cp_async_wait<0>();      // the plane issued one barrier ago: visible to the converting warps after this one
         __syncthreads();
-        if (tid == NI) {      // the stage the plane above came from is free again
+        {      // the stage the plane above came from is free again
             const int n = kk + 2 + 2 * R + NSTG;
-            if (n < NPL) issue_plane<T, NV, TY>(gin, j0, PF + n, raw + (n % NSTG) * S, &bars[n % NSTG]);
+            if (n < NPL) {
+                if (FUSED) stage_plane_fused<T, NV, TY>(gin, nb, ctab, PF + n, raw + (n % NSTG) * RS, tid, NT);
+                else if (tid == NI) issue_plane<T, NV, TY>(gin, j0, PF + n, raw + (n % NSTG) * RS, &bars[n % NSTG]);
+            }
         }
         // ------------------------------------------------------------------ conserved input of cell (ei, ej, kk-1)
         const bool upd = interior && kk >= 1;
-        const T* gcell = gin + c.gin_off + (kk - 1) * (NP * NP);
+        // padded mode: cell of the padded slab; fused mode: cell of this group's unpadded state
+        const T* gcell = FUSED ? gin + (size_t)g * NV * (PS * PSQ) + c.out_off + (kk - 1) * PSQ
+                               : gin + c.gin_off + (kk - 1) * (NP * NP);
         T U[NV];
         if (upd) {
 #pragma unroll
-            for (int v = 0; v < NV; ++v) U[v] = __ldg(gcell + (size_t)v * NPC);
+            for (int v = 0; v < NV; ++v) U[v] = __ldg(gcell + (size_t)v * (FUSED ? PS * PSQ : NPC));
         }
         // ------------------------------------------------------------------ x and y faces of plane kk
         if (mid && own_x) {
