@@ -152,15 +152,13 @@ __device__ __forceinline__ void convert_plane(const T* raw, T* prim, const Phys<
 // Fused ghost refresh: the padded plane is gathered straight from the
 // unpadded state of the group and of its same-level neighbours with cp.async (LDGSTS), so no padded copy of the
 // batch ever exists in HBM.  Staged rows are 24 wide with the 16 interior cells at columns 4..19 (16-byte aligned
-// for the wide copies), ghosts at 1..3 and 20..22.  nb = the 27 neighbour group indices of this group.
+// for the wide copies), ghosts at 1..3 and 20..22 (columns 0 and 23 receive a fourth, unused neighbour cell so that
+// the ghost cells travel as aligned 16-byte chunks too).  nb = the 27 neighbour group indices of this group.
 // ---------------------------------------------------------------------------------------------
 constexpr int FW = 24;   // row stride of a staged plane in fused mode
 
 __device__ __forceinline__ void cp_async_16(void* dst, const void* src) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
-}
-template <int BYTES> __device__ __forceinline__ void cp_async_small(void* dst, const void* src) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(smem_u32(dst)), "l"(src), "n"(BYTES) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 // wait until at most N of this thread's committed copy groups are still in flight
@@ -172,7 +170,9 @@ template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile(
 // issues the same few entries for every plane.
 template <typename T, int NV, int TY> struct FusedCopies {
     static constexpr int CE = 16 / (int)sizeof(T);          // elements per 16-byte copy
-    static constexpr int OPS = PS / CE + 2 * NGH;           // copies per row and variable
+    static constexpr int GC = 4 / CE;                       // copies per ghost side: the 3 ghost cells travel as the
+                                                            // aligned 4-element chunk that contains them
+    static constexpr int OPS = PS / CE + 2 * GC;            // copies per row and variable, all 16 bytes wide
     static constexpr int N = Geo<TY>::NR * NV * OPS;
 };
 
@@ -187,16 +187,11 @@ __device__ __forceinline__ void fused_copy_table(int2* tab, int j0, int tid, int
         const int py = j0 + r;
         const int dy = py < NGH ? 0 : (py < NGH + PS ? 1 : 2);
         const int yy = (py + PS - NGH) & (PS - 1);
-        int dx, xx, col, wide;
-        if (op < PS / F::CE) { dx = 1; xx = op * F::CE; col = 4 + xx; wide = 1; }
-        else {
-            const int q = op - PS / F::CE;
-            dx = q < NGH ? 0 : 2;
-            xx = q < NGH ? PS - NGH + q : q - NGH;
-            col = q < NGH ? 1 + q : 4 + PS + (q - NGH);
-            wide = 0;
-        }
-        tab[it] = make_int2((v * G::NR + r) * FW + col, (v * PS3 + yy * PS + xx) | ((dy * 3 + dx) << 20) | (wide << 24));
+        int dx, xx, col;
+        if (op < PS / F::CE) { dx = 1; xx = op * F::CE; col = 4 + xx; }                      // interior cells
+        else if (op < PS / F::CE + F::GC) { dx = 0; xx = PS - 4 + (op - PS / F::CE) * F::CE; col = xx - (PS - 4); }   // x' 12..15 -> cols 0..3
+        else { dx = 2; xx = (op - PS / F::CE - F::GC) * F::CE; col = 4 + PS + xx; }           // x' 0..3 -> cols 20..23
+        tab[it] = make_int2((v * G::NR + r) * FW + col, (v * PS3 + yy * PS + xx) | ((dy * 3 + dx) << 20));
     }
 }
 
@@ -210,9 +205,8 @@ __device__ __forceinline__ void stage_plane_fused(const T* u, const int* nb, con
     const int* nbz = nb + dz * 9;
     for (int it = tid; it < F::N; it += nthr) {
         const int2 d = tab[it];
-        const T* src = u + (size_t)nbz[(d.y >> 20) & 15] * NV * PS3 + ((d.y & 0xfffff) + zoff);
-        if (d.y >> 24) cp_async_16(raw_stage + d.x, src);
-        else cp_async_small<(int)sizeof(T)>(raw_stage + d.x, src);
+        const T* src = u + (size_t)nbz[d.y >> 20] * NV * PS3 + ((d.y & 0xfffff) + zoff);
+        cp_async_16(raw_stage + d.x, src);
     }
     cp_async_commit();
 }
