@@ -244,9 +244,9 @@ def main():
         refresh_value = cells * nref / (a0.elapsed_time(a1) * 1e-3)
         finite = finite and bool(torch.isfinite(u_in).all().item())
     # ---- extra: the fused form of the same loop (gamer_fluid_advance_resident: unpadded state + neighbour table,
-    # ghost zones gathered inside the solver; MHM only) -- two unpadded buffers ping-pong, no padded batch is touched
+    # ghost zones gathered inside the solver) -- two unpadded buffers ping-pong, no padded batch is touched
     fused_value = None
-    if world == 1 and scheme == 1:
+    if world == 1:
         nbr = gb.gamer_neighbors_periodic(gside, gside, gside, dev)
         ua, ub = out, torch.empty_like(out)
         nref = max(2, min(5, args.steps))

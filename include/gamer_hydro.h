@@ -110,8 +110,8 @@ int gamer_refresh_ghosts_periodic(const void* u, void* in, int gz, int gy, int g
  * padded plane from those groups directly, so no padded copy of the batch exists in memory; results are
  * bit-identical to gamer_refresh_ghosts_periodic / a host gather followed by gamer_fluid_advance_ex.
  * u and out must not overlap (every group reads its neighbours' old state).  opts may be NULL.
- * Supported: scheme = GAMER_MHM (any recon / riemann / precision, all opts except remedy_first_order);
- * anything else returns GAMER_EUNSUPPORTED -- use the refresh + gamer_fluid_advance_ex pair there. */
+ * All schemes, reconstructions, solvers and precisions; all opts except remedy_first_order (remedy (ii)
+ * re-reads the padded slab), which returns GAMER_EUNSUPPORTED -- use the refresh + gamer_fluid_advance_ex pair there. */
 int gamer_fluid_advance_resident(const void* u, const int32_t* nbr, void* out, void* flux_out, int64_t n_groups,
                                  double dt, double dh, double gamma,
                                  int scheme, int recon, int riemann, int precision,

@@ -120,7 +120,6 @@ extern "C" int gamer_fluid_advance_resident(const void* u, const int32_t* nbr, v
         if (opts->min_dens < 0 || opts->min_pres < 0 || opts->min_temp < 0) return GAMER_EINVAL;
         if (opts->remedy_first_order) return GAMER_EUNSUPPORTED;   // remedy (ii) re-reads the padded slab
     }
-    if (scheme != GAMER_MHM) return GAMER_EUNSUPPORTED;
     if (n_groups > 0x3fffffff / 27) return GAMER_EUNSUPPORTED;
     if (u == out) return GAMER_EINVAL;
     return precision == GAMER_FP32

@@ -17,13 +17,14 @@
 
 namespace gamer {
 
-template <typename T, int RECON, int NV, int TY> struct CtuSmem {
+template <typename T, int RECON, int NV, int TY, bool FUSED = false> struct CtuSmem {
     using G = Geo<TY>;
     static constexpr int R = RECON == PPM ? 2 : 1;
     static constexpr int PR = 2 * R + 1;
     static constexpr int NF1X = 17 * G::EH, NF1Y = 18 * (G::EH - 1);
     static constexpr int RAW = 0;                                   // [2][NV][PLN]
-    static constexpr int PRIM = RAW + 2 * NV * G::PLN;              // [PR][NV][PLN]
+    static constexpr int RSTG = NV * (FUSED ? G::NR * FW : G::PLN); // one landing stage (fused refresh: 24-wide rows)
+    static constexpr int PRIM = RAW + 2 * RSTG;                     // [PR][NV][PLN]
     static constexpr int TS = PRIM + PR * NV * G::PLN;              // [2][6][NV][EPL]
     static constexpr int F1X = TS + 2 * 6 * NV * G::EPL;            // [NV][NF1X]
     static constexpr int F1Y = F1X + NV * NF1X;                     // [NV][NF1Y]
@@ -33,7 +34,7 @@ template <typename T, int RECON, int NV, int TY> struct CtuSmem {
     static constexpr int FY = FX + NV * G::NFX;
     static constexpr int FZ = FY + NV * G::NFY;
     static constexpr int END = FZ + NV * G::NFZ;
-    static constexpr size_t BYTES = 16 + (size_t)END * sizeof(T);
+    static constexpr size_t BYTES = 16 + (size_t)END * sizeof(T) + (FUSED ? 128 : 0);   // + neighbour table
 };
 
 // one first-pass Riemann solve: rotated loads from two state arrays, unrotated store
@@ -106,10 +107,11 @@ __device__ __forceinline__ void ctu_trace_dir(const T* const* Pz, int t, T* tcur
     if (NV > 5) { sm_[(NV - 1) * EPL] = tm[NV - 1]; sp_[(NV - 1) * EPL] = tp[NV - 1]; }
 }
 
-template <typename T, int RECON, int SOLVER, int NV, bool EXT, int TY, int NT>
+template <typename T, int RECON, int SOLVER, int NV, bool EXT, int TY, int NT, bool FUSED>
 __global__ void __launch_bounds__(NT) ctu_kernel(const AdvArgs<T> a) {
     using G = Geo<TY>;
-    using S = CtuSmem<T, RECON, NV, TY>;
+    using S = CtuSmem<T, RECON, NV, TY, FUSED>;
+    constexpr int RS = S::RSTG;
     constexpr int R = S::R, PR = S::PR;
     constexpr int NPL = 18 + 2 * R;
     constexpr int PF = 2 - R;
@@ -133,7 +135,12 @@ __global__ void __launch_bounds__(NT) ctu_kernel(const AdvArgs<T> a) {
     const long long tile = blockIdx.x;
     const long long g = tile / G::NTILE;
     const int j0 = (int)(tile % G::NTILE) * TY;
-    const T* gin = a.in + (size_t)g * NV * NPC;
+    // padded mode: this group's padded slab; fused mode (a.nbr set): the whole unpadded batch, ghost zones gathered
+    // from the same-level neighbours inside the kernel (hydro_stream.cuh "Fused ghost refresh")
+    const T* gin = FUSED ? a.in : a.in + (size_t)g * NV * NPC;
+    int* nb = reinterpret_cast<int*>(smem_raw + 16 + S::END * sizeof(T));
+    const int2* ctab = nullptr;      // copy list decoded on the fly: a table would cost the fp64 variants a tile size
+    if (FUSED && tid < 27) nb[tid] = a.nbr[g * 27 + tid];
     T* gout = a.out + (size_t)g * NV * (PS * PS * PS);
     T* gflux = a.flux ? a.flux + (size_t)g * 9 * NV * (PS * PS) : nullptr;
     const Phys<T> ph = make_phys<T>(a);
@@ -144,15 +151,27 @@ __global__ void __launch_bounds__(NT) ctu_kernel(const AdvArgs<T> a) {
         mbar_fence_init();
     }
     __syncthreads();
-    if (tid == 0) {
+    if (FUSED) {
+        stage_plane_fused<T, NV, TY>(gin, nb, ctab, j0, PF + 0, raw, tid, NT);
+        stage_plane_fused<T, NV, TY>(gin, nb, ctab, j0, PF + 1, raw + RS, tid, NT);
+    } else if (tid == 0) {
         issue_plane<T, NV, TY>(gin, j0, PF + 0, raw, &bars[0]);
-        issue_plane<T, NV, TY>(gin, j0, PF + 1, raw + NV * G::PLN, &bars[1]);
+        issue_plane<T, NV, TY>(gin, j0, PF + 1, raw + RS, &bars[1]);
     }
     for (int n = 0; n <= 2 * R; ++n) {
-        mbar_wait(&bars[n & 1], (n >> 1) & 1);
-        convert_plane<T, NV, EXT, TY, NT>(raw + (n & 1) * NV * G::PLN, prim + ((PF + n) % PR) * NV * G::PLN, ph, tid);
+        if (FUSED) {
+            cp_async_wait<0>();
+            __syncthreads();
+            convert_plane_fused<T, NV, EXT, TY, NT>(raw + (n & 1) * RS, prim + ((PF + n) % PR) * NV * G::PLN, ph, tid);
+        } else {
+            mbar_wait(&bars[n & 1], (n >> 1) & 1);
+            convert_plane<T, NV, EXT, TY, NT>(raw + (n & 1) * RS, prim + ((PF + n) % PR) * NV * G::PLN, ph, tid);
+        }
         __syncthreads();
-        if (tid == 0 && n + 2 < NPL) issue_plane<T, NV, TY>(gin, j0, PF + n + 2, raw + (n & 1) * NV * G::PLN, &bars[n & 1]);
+        if (n + 2 < NPL) {
+            if (FUSED) stage_plane_fused<T, NV, TY>(gin, nb, ctab, j0, PF + n + 2, raw + (n & 1) * RS, tid, NT);
+            else if (tid == 0) issue_plane<T, NV, TY>(gin, j0, PF + n + 2, raw + (n & 1) * RS, &bars[n & 1]);
+        }
     }
 
     const bool owner = tid < G::NFZ;           // threads that own a cell column of the update
@@ -181,6 +200,7 @@ __global__ void __launch_bounds__(NT) ctu_kernel(const AdvArgs<T> a) {
                 else ctu_trace_dir<T, RECON, NV, EXT, TY, 2>(Pz, t, tcur, ph, cnt);
             }
         }
+        if (FUSED) cp_async_wait<0>();      // this thread's share of the plane converted below
         __syncthreads();
         // ------------------------------------------------------------------ R1z(kk) + convert
         if (kk >= 0 && kk <= PS) {
@@ -191,8 +211,12 @@ __global__ void __launch_bounds__(NT) ctu_kernel(const AdvArgs<T> a) {
         {
             const int n = kk + 2 + 2 * R;
             if (n < NPL) {
-                mbar_wait(&bars[n & 1], (n >> 1) & 1);
-                convert_plane<T, NV, EXT, TY, NT>(raw + (n & 1) * NV * G::PLN, prim + ((PF + n) % PR) * NV * G::PLN, ph, tid);
+                if (FUSED) {      // copies waited for before the barrier above
+                    convert_plane_fused<T, NV, EXT, TY, NT>(raw + (n & 1) * RS, prim + ((PF + n) % PR) * NV * G::PLN, ph, tid);
+                } else {
+                    mbar_wait(&bars[n & 1], (n >> 1) & 1);
+                    convert_plane<T, NV, EXT, TY, NT>(raw + (n & 1) * RS, prim + ((PF + n) % PR) * NV * G::PLN, ph, tid);
+                }
             }
         }
         __syncthreads();
@@ -261,19 +285,23 @@ __global__ void __launch_bounds__(NT) ctu_kernel(const AdvArgs<T> a) {
         if (m >= 0) cnt.roe_fb += riemann_plane<T, SOLVER, NV, TY, NT>(tprev, zp + ((m + 1) & 1) * NV * G::NFZ, fx, fy, fz, gflux, m, j0, ph, tid);
         __syncthreads();
         // ------------------------------------------------------------------ U(kk-2)
-        if (tid == 0) {
+        {
             const int n = kk + 4 + 2 * R;
-            if (n < NPL) issue_plane<T, NV, TY>(gin, j0, PF + n, raw + (n & 1) * NV * G::PLN, &bars[n & 1]);
+            if (n < NPL) {
+                if (FUSED) stage_plane_fused<T, NV, TY>(gin, nb, ctab, j0, PF + n, raw + (n & 1) * RS, tid, NT);
+                else if (tid == 0) issue_plane<T, NV, TY>(gin, j0, PF + n, raw + (n & 1) * RS, &bars[n & 1]);
+            }
         }
         if (owner) {
             if (m >= 1) {
                 const int k = m - 1;
-                const T* gcell = gin + (size_t)(k + NGH) * (NP * NP) + (j0 + cj + NGH) * NP + (ci + NGH);
+                const T* gcell = FUSED ? gin + (size_t)g * NV * (PS * PS * PS) + (size_t)k * (PS * PS) + (j0 + cj) * PS + ci
+                                       : gin + (size_t)(k + NGH) * (NP * NP) + (j0 + cj + NGH) * NP + (ci + NGH);
                 T U[NV];
 #pragma unroll
                 for (int v = 0; v < NV; ++v) {
                     const T dfz = fz[v * G::NFZ + tid] - fzm[v];
-                    U[v] = __ldg(gcell + (size_t)v * NPC) - ph.lam * (sxy[v] + dfz);
+                    U[v] = __ldg(gcell + (size_t)v * (FUSED ? PS * PS * PS : NPC)) - ph.lam * (sxy[v] + dfz);
                 }
                 close_cell<T, SOLVER, NV, EXT>(U, gcell, cnt, ph);
 #pragma unroll

@@ -176,35 +176,40 @@ template <typename T, int NV, int TY> struct FusedCopies {
     static constexpr int N = Geo<TY>::NR * NV * OPS;
 };
 
+// entry `it` of the copy list: .x = destination element in the landing stage, .y = source element | in-plane neighbour << 20
 template <typename T, int NV, int TY>
-__device__ __forceinline__ void fused_copy_table(int2* tab, int j0, int tid, int nthr) {
+__device__ __forceinline__ int2 fused_copy_desc(int it, int j0) {
     using G = Geo<TY>;
     using F = FusedCopies<T, NV, TY>;
     constexpr int PS3 = PS * PS * PS;
-    for (int it = tid; it < F::N; it += nthr) {
-        const int op = it % F::OPS, rv = it / F::OPS;
-        const int r = rv % G::NR, v = rv / G::NR;
-        const int py = j0 + r;
-        const int dy = py < NGH ? 0 : (py < NGH + PS ? 1 : 2);
-        const int yy = (py + PS - NGH) & (PS - 1);
-        int dx, xx, col;
-        if (op < PS / F::CE) { dx = 1; xx = op * F::CE; col = 4 + xx; }                      // interior cells
-        else if (op < PS / F::CE + F::GC) { dx = 0; xx = PS - 4 + (op - PS / F::CE) * F::CE; col = xx - (PS - 4); }   // x' 12..15 -> cols 0..3
-        else { dx = 2; xx = (op - PS / F::CE - F::GC) * F::CE; col = 4 + PS + xx; }           // x' 0..3 -> cols 20..23
-        tab[it] = make_int2((v * G::NR + r) * FW + col, (v * PS3 + yy * PS + xx) | ((dy * 3 + dx) << 20));
-    }
+    const int op = it % F::OPS, rv = it / F::OPS;
+    const int r = rv % G::NR, v = rv / G::NR;
+    const int py = j0 + r;
+    const int dy = py < NGH ? 0 : (py < NGH + PS ? 1 : 2);
+    const int yy = (py + PS - NGH) & (PS - 1);
+    int dx, xx, col;
+    if (op < PS / F::CE) { dx = 1; xx = op * F::CE; col = 4 + xx; }                      // interior cells
+    else if (op < PS / F::CE + F::GC) { dx = 0; xx = PS - 4 + (op - PS / F::CE) * F::CE; col = xx - (PS - 4); }   // x' 12..15 -> cols 0..3
+    else { dx = 2; xx = (op - PS / F::CE - F::GC) * F::CE; col = 4 + PS + xx; }           // x' 0..3 -> cols 20..23
+    return make_int2((v * G::NR + r) * FW + col, (v * PS3 + yy * PS + xx) | ((dy * 3 + dx) << 20));
 }
 
-// every thread issues its entries of the list for padded plane p (0..21) and commits them as one group
 template <typename T, int NV, int TY>
-__device__ __forceinline__ void stage_plane_fused(const T* u, const int* nb, const int2* tab, int p, T* raw_stage, int tid, int nthr) {
+__device__ __forceinline__ void fused_copy_table(int2* tab, int j0, int tid, int nthr) {
+    for (int it = tid; it < FusedCopies<T, NV, TY>::N; it += nthr) tab[it] = fused_copy_desc<T, NV, TY>(it, j0);
+}
+
+// every thread issues its entries of the list for padded plane p (0..21) and commits them as one group;
+// tab == nullptr: the entries are decoded on the fly (CTU, where the list would cost a tile size in shared memory)
+template <typename T, int NV, int TY>
+__device__ __forceinline__ void stage_plane_fused(const T* u, const int* nb, const int2* tab, int j0, int p, T* raw_stage, int tid, int nthr) {
     using F = FusedCopies<T, NV, TY>;
     constexpr int PS3 = PS * PS * PS;
     const int dz = p < NGH ? 0 : (p < NGH + PS ? 1 : 2);
     const int zoff = ((p + PS - NGH) & (PS - 1)) * (PS * PS);
     const int* nbz = nb + dz * 9;
     for (int it = tid; it < F::N; it += nthr) {
-        const int2 d = tab[it];
+        const int2 d = tab ? tab[it] : fused_copy_desc<T, NV, TY>(it, j0);
         const T* src = u + (size_t)nbz[d.y >> 20] * NV * PS3 + ((d.y & 0xfffff) + zoff);
         cp_async_16(raw_stage + d.x, src);
     }

@@ -59,18 +59,19 @@ cudaError_t launch_mhm(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
 #ifndef CTU_NT_OVERRIDE
 #define CTU_NT_OVERRIDE 0
 #endif
-template <typename T, int RECON, int NV>
+template <typename T, int RECON, int NV, bool FUSED>
 constexpr int ctu_tile() {
-    return CtuSmem<T, RECON, NV, 16>::BYTES <= SMEM_LIMIT ? 16 : (CtuSmem<T, RECON, NV, 8>::BYTES <= SMEM_LIMIT ? 8 : 4);
+    return CtuSmem<T, RECON, NV, 16, FUSED>::BYTES <= SMEM_LIMIT ? 16 : (CtuSmem<T, RECON, NV, 8, FUSED>::BYTES <= SMEM_LIMIT ? 8 : 4);
 }
 
-template <typename T, int RECON, int SOLVER, int NV, bool EXT, int TY>
-cudaError_t launch_ctu_ty(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
+template <typename T, int RECON, int SOLVER, int NV, bool EXT, bool FUSED>
+cudaError_t launch_ctu_f(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
+    constexpr int TY = ctu_tile<T, RECON, NV, FUSED>();
     constexpr int NT = CTU_NT_OVERRIDE > 0 ? CTU_NT_OVERRIDE : ((sizeof(T) == 8 ? 48 : 32) * TY < 128 ? 128 : (sizeof(T) == 8 ? 48 : 32) * TY);
     using G = Geo<TY>;
-    using S = CtuSmem<T, RECON, NV, TY>;
+    using S = CtuSmem<T, RECON, NV, TY, FUSED>;
     static_assert(S::BYTES <= SMEM_LIMIT, "tile does not fit in shared memory");
-    auto kern = ctu_kernel<T, RECON, SOLVER, NV, EXT, TY, NT>;
+    auto kern = ctu_kernel<T, RECON, SOLVER, NV, EXT, TY, NT, FUSED>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::BYTES);
     if (e != cudaSuccess) return e;
     if (G::NTILE > 1 && a.speed) {
@@ -83,14 +84,11 @@ cudaError_t launch_ctu_ty(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
     return cudaGetLastError();
 }
 
+// a.nbr set => `in` is the unpadded state and the ghost refresh is fused into the staging loads
 template <typename T, int RECON, int SOLVER, int NV, bool EXT>
 cudaError_t launch_ctu(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
-#ifdef CTU_TY_OVERRIDE
-    constexpr int TY = (sizeof(T) == 4 && CtuSmem<T, RECON, NV, CTU_TY_OVERRIDE>::BYTES <= SMEM_LIMIT) ? CTU_TY_OVERRIDE : ctu_tile<T, RECON, NV>();
-#else
-    constexpr int TY = ctu_tile<T, RECON, NV>();
-#endif
-    return launch_ctu_ty<T, RECON, SOLVER, NV, EXT, TY>(a, st, launches);
+    return a.nbr ? launch_ctu_f<T, RECON, SOLVER, NV, EXT, true>(a, st, launches)
+                 : launch_ctu_f<T, RECON, SOLVER, NV, EXT, false>(a, st, launches);
 }
 #endif
 

@@ -210,8 +210,8 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED>::NT), M
     }
     __syncthreads();
     if (FUSED) {      // every thread issues a few copies of each plane (cp.async groups are per thread)
-        stage_plane_fused<T, NV, TY>(gin, nb, ctab, PF + 0, raw, tid, NT);
-        stage_plane_fused<T, NV, TY>(gin, nb, ctab, PF + 1, raw + RS, tid, NT);
+        stage_plane_fused<T, NV, TY>(gin, nb, ctab, j0, PF + 0, raw, tid, NT);
+        stage_plane_fused<T, NV, TY>(gin, nb, ctab, j0, PF + 1, raw + RS, tid, NT);
     } else if (tid == NI) {
         issue_plane<T, NV, TY>(gin, j0, PF + 0, raw, &bars[0]);
         if (NSTG > 1) issue_plane<T, NV, TY>(gin, j0, PF + 1, raw + RS, &bars[1]);
@@ -228,7 +228,7 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED>::NT), M
         }
         __syncthreads();
         if (n + NSTG < NPL) {
-            if (FUSED) stage_plane_fused<T, NV, TY>(gin, nb, ctab, PF + n + NSTG, raw + (n % NSTG) * RS, tid, NT);
+            if (FUSED) stage_plane_fused<T, NV, TY>(gin, nb, ctab, j0, PF + n + NSTG, raw + (n % NSTG) * RS, tid, NT);
             else if (tid == NI) issue_plane<T, NV, TY>(gin, j0, PF + n + NSTG, raw + (n % NSTG) * RS, &bars[n % NSTG]);
         }
     }
@@ -335,7 +335,7 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED>::NT), M
         {      // the stage the plane above came from is free again
             const int n = kk + 2 + 2 * R + NSTG;
             if (n < NPL) {
-                if (FUSED) stage_plane_fused<T, NV, TY>(gin, nb, ctab, PF + n, raw + (n % NSTG) * RS, tid, NT);
+                if (FUSED) stage_plane_fused<T, NV, TY>(gin, nb, ctab, j0, PF + n, raw + (n % NSTG) * RS, tid, NT);
                 else if (tid == NI) issue_plane<T, NV, TY>(gin, j0, PF + n, raw + (n % NSTG) * RS, &bars[n % NSTG]);
             }
         }

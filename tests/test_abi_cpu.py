@@ -57,10 +57,13 @@ def test_argument_validation_needs_no_gpu(built_lib):
     assert L.gamer_fluid_advance(ok[0], ok[1], None, 1, 0.1, 0.1, 1.4, 1, 1, 4, 4) == -1
     assert L.gamer_fluid_advance(ok[0], ok[1], None, 1, 0.1, 0.1, 1.4, 1, 1, 1, 2) == -1
     assert L.gamer_fluid_advance(vp(4100), ok[1], None, 1, 0.1, 0.1, 1.4, 1, 1, 1, 4) == -1     # misaligned
-    # fused-refresh entry: no neighbour table, CTU (not built for it), in-place update
-    L.gamer_fluid_advance_resident.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, ci, ci, vp]
+    # fused-refresh entry: no neighbour table, remedy (ii) (needs the padded slab), in-place update
+    from paper_1712_07070_b200 import binding as gb
+    L.gamer_fluid_advance_resident.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, ci, ci, ctypes.POINTER(gb.gamer_opts)]
     assert L.gamer_fluid_advance_resident(ok[0], None, ok[1], None, 1, 0.1, 0.1, 1.4, 1, 1, 1, 4, None) == -1
-    assert L.gamer_fluid_advance_resident(ok[0], vp(16384), ok[1], None, 1, 0.1, 0.1, 1.4, 2, 1, 1, 4, None) == -2
+    o = gb.gamer_opts()
+    o.remedy_first_order = 1
+    assert L.gamer_fluid_advance_resident(ok[0], vp(16384), ok[1], None, 1, 0.1, 0.1, 1.4, 2, 1, 1, 4, ctypes.byref(o)) == -2
     assert L.gamer_fluid_advance_resident(ok[0], vp(16384), ok[0], None, 1, 0.1, 0.1, 1.4, 1, 1, 1, 4, None) == -1
     L.gamer_neighbors_periodic.argtypes = [vp, ci, ci, ci, vp]
     assert L.gamer_neighbors_periodic(None, 1, 1, 1, None) == -1
