@@ -154,3 +154,24 @@ def close_cell(U, gamma, opts):
     st = Stats()
     ok = lib().oracle_close_cell(_p(U), ctypes.c_double(gamma), ctypes.byref(opts), ctypes.byref(st))
     return U, bool(ok), st.as_dict()
+
+
+def restrict(fine, coarse, parent):
+    """PAPER.md L112 restriction in the group layout: fine [Gf,NV,16,16,16] -> octants of coarse [Gc,NV,16,16,16]
+    (modified in place and returned); parent[g] = coarse group * 8 + octant."""
+    fine = _c64(fine)
+    assert coarse.dtype == np.float64 and coarse.flags["C_CONTIGUOUS"]
+    parent = np.ascontiguousarray(parent, dtype=np.int32)
+    lib().oracle_restrict(_p(fine), _p(coarse), _p(parent), ctypes.c_int64(fine.shape[0]), int(fine.shape[1]))
+    return coarse
+
+
+def flux_correct(coarse, coarse_flux, fine_flux_avg, table, lam):
+    """PAPER.md L112 flux correction of the coarse cells next to coarse-fine boundaries (coarse modified in place);
+    table [n, 8] int32 as documented in hydro_oracle.c."""
+    assert coarse.dtype == np.float64 and coarse.flags["C_CONTIGUOUS"]
+    coarse_flux, fine_flux_avg = _c64(coarse_flux), _c64(fine_flux_avg)
+    table = np.ascontiguousarray(table, dtype=np.int32)
+    lib().oracle_flux_correct(_p(coarse), _p(coarse_flux), _p(fine_flux_avg), _p(table), ctypes.c_int64(table.shape[0]),
+                              int(coarse.shape[1]), ctypes.c_double(lam))
+    return coarse

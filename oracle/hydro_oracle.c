@@ -956,3 +956,76 @@ int oracle_close_cell(double *U, double gamma, const orc_opts *opts, orc_stats *
 
 int oracle_sizeof_opts(void) { return (int)sizeof(orc_opts); }
 int oracle_sizeof_stats(void) { return (int)sizeof(orc_stats); }
+
+/* ------------------------------------------------------------------------------------------------
+ * The two fix-up operations of PAPER.md L112 between a refined patch group and the coarse level, in the
+ * patch-group layout of the solver.  Plain loops, fp64.
+ *
+ * Restriction: "the data of fine patches are averaged to replace the data of their parent coarse cells".
+ * fine[n_fine][nv][16][16][16], coarse[..][nv][16][16][16]; parent[g] = coarse group * 8 + octant,
+ * octant = oz*4 + oy*2 + ox: fine group g covers the 8^3 coarse cells of that octant.  The eight children of a
+ * coarse cell are summed in the order (dz, dy, dx) = (0,0,0), (0,0,1), (0,1,0), ... and multiplied by 1/8.
+ * ---------------------------------------------------------------------------------------------- */
+int oracle_restrict(const double *fine, double *coarse, const int32_t *parent, int64_t n_fine, int nv)
+{
+    for (int64_t g = 0; g < n_fine; ++g) {
+        const int64_t cg = parent[g] >> 3;
+        const int oz = (parent[g] >> 2) & 1, oy = (parent[g] >> 1) & 1, ox = parent[g] & 1;
+        for (int v = 0; v < nv; ++v) {
+            const double *f = fine + ((size_t)g * nv + v) * 4096;
+            double *c = coarse + ((size_t)cg * nv + v) * 4096;
+            for (int k = 0; k < 8; ++k)
+                for (int j = 0; j < 8; ++j)
+                    for (int i = 0; i < 8; ++i) {
+                        double s = 0.0;
+                        for (int dz = 0; dz < 2; ++dz)
+                            for (int dy = 0; dy < 2; ++dy)
+                                for (int dx = 0; dx < 2; ++dx)
+                                    s = s + f[((2 * k + dz) * 16 + (2 * j + dy)) * 16 + (2 * i + dx)];
+                        c[((oz * 8 + k) * 16 + (oy * 8 + j)) * 16 + (ox * 8 + i)] = 0.125 * s;
+                    }
+        }
+    }
+    return 0;
+}
+
+/* Flux correction: "the coarse-grid fluxes across the coarse-fine boundaries are replaced by the fine-grid fluxes
+ * averaged in space and time" -- applied as a correction of the coarse cells next to the boundary.
+ * One table entry = one outer face of a fine group that is a coarse-fine boundary (16 x 16 fine faces = 8 x 8 coarse):
+ *   e[0] fine group   e[1] axis d   e[2] side (0: the group's low face, flux plane 0; 1: high face, plane 2)
+ *   e[3] coarse group whose flux_out holds the coarse flux there, e[4] its plane (0,1,2),
+ *   e[5] (b0 << 8) | a0 : origin of the 8 x 8 quadrant in that 16 x 16 plane (b = slower, a = faster remaining axis)
+ *   e[6] coarse group that owns the coarse cells on the other side of the face,
+ *   e[7] (z << 16) | (y << 8) | x : the cell of the 8 x 8 patch with b = a = 0 (its coordinate along d is the layer).
+ * fine_flux_avg = time average over the coarse step of the fine flux_out; lam = dt_coarse / dh_coarse.
+ * U_cell += sgn * lam * (avg2x2(F_fine) - F_coarse), sgn = -1 on side 0 (the face is the cell's upper face), +1 on
+ * side 1; avg2x2 = 0.25 * (((f00 + f01) + f10) + f11).  Entries are applied in the order axis 0 side 0, axis 0
+ * side 1, axis 1 side 0, ... (within such a pass no two entries touch the same cell). */
+int oracle_flux_correct(double *coarse, const double *coarse_flux, const double *fine_flux_avg, const int32_t *tab,
+                        int64_t n_entries, int nv, double lam)
+{
+    for (int pass = 0; pass < 6; ++pass)
+        for (int64_t n = 0; n < n_entries; ++n) {
+            const int32_t *e = tab + 8 * n;
+            const int d = e[1], side = e[2];
+            if (d * 2 + side != pass) continue;
+            const double sgn = side ? 1.0 : -1.0;
+            const int b0 = e[5] >> 8, a0 = e[5] & 255;
+            const int z0 = e[7] >> 16, y0 = (e[7] >> 8) & 255, x0 = e[7] & 255;
+            for (int v = 0; v < nv; ++v) {
+                const double *ff = fine_flux_avg + ((((size_t)e[0] * 3 + d) * 3 + (side ? 2 : 0)) * nv + v) * 256;
+                const double *fc = coarse_flux + ((((size_t)e[3] * 3 + d) * 3 + e[4]) * nv + v) * 256;
+                double *c = coarse + ((size_t)e[6] * nv + v) * 4096;
+                for (int b = 0; b < 8; ++b)
+                    for (int a = 0; a < 8; ++a) {
+                        const double favg = 0.25 * (((ff[(2 * b) * 16 + 2 * a] + ff[(2 * b) * 16 + 2 * a + 1]) +
+                                                     ff[(2 * b + 1) * 16 + 2 * a]) + ff[(2 * b + 1) * 16 + 2 * a + 1]);
+                        const double corr = lam * (favg - fc[(b0 + b) * 16 + (a0 + a)]);
+                        int z = z0, y = y0, x = x0;
+                        if (d == 0) { z += b; y += a; } else if (d == 1) { z += b; x += a; } else { y += b; x += a; }
+                        c[(z * 16 + y) * 16 + x] += sgn * corr;
+                    }
+            }
+        }
+    return 0;
+}

@@ -69,8 +69,11 @@ def restrict(uf):
     return 0.125 * sum(uf[:, a::2, b::2, d::2] for a in (0, 1) for b in (0, 1) for d in (0, 1))
 
 
-def two_level_step(solver, uc, uf, region, dh_c, dt_c):
-    """Returns (uc_new after fix-up, uf_new, records) where records holds every padded batch / output for parity."""
+def two_level_step(solver, uc, uf, region, dh_c, dt_c, fixup=None):
+    """Returns (uc_new after fix-up, uf_new, records) where records holds every padded batch / output for parity.
+    fixup = None: restriction and flux correction are done right here on the global arrays (torch); otherwise
+    fixup(uc1, uf, flux_c, [flux_f of each sub-step], region, dt_c / dh_c) -> corrected uc1 (group-layout
+    implementations: the oracle's C functions or the CUDA library, see fixup_in_group_layout)."""
     z0, z1, y0, y1, x0, x1 = region
     rec = {}
     cdims = inputs.group_dims(uc)
@@ -80,17 +83,21 @@ def two_level_step(solver, uc, uf, region, dh_c, dt_c):
     uc1 = inputs.unpack(out_c, *cdims)
     fsum = {}
     fdims = None
+    fine_fluxes = []
     for sub in (0, 1):
         w = 0.5 * sub
         uc_t = (1.0 - w) * uc + w * uc1                      # linear in time
         pf, fdims = pack_fine(uf, uc_t, region)
         out_f, flux_f = solver(pf, 0.5 * dt_c, 0.5 * dh_c)
         rec["fine%d" % sub] = (pf, out_f, flux_f)
+        fine_fluxes.append(flux_f)
         uf = inputs.unpack(out_f, *fdims)
         for axis, n in ((0, fdims[2]), (1, fdims[1]), (2, fdims[0])):
             for side, (gi, pl) in (("lo", (0, 0)), ("hi", (n - 1, 2))):
                 p = 0.5 * avg2x2(face_plane(flux_f, fdims, axis, gi, pl))   # time average over the two sub-steps
                 fsum[(axis, side)] = fsum.get((axis, side), 0) + p
+    if fixup is not None:
+        return fixup(uc1, uf, flux_c, fine_fluxes, region, dt_c / dh_c), uf, rec
     # ---- fix-up 1: restriction (L112)
     uc1 = uc1.clone()
     uc1[:, z0:z1, y0:y1, x0:x1] = restrict(uf)
@@ -147,3 +154,69 @@ def composite_total(uc, uf, region, dh_c):
     mask = torch.ones(uc.shape[1:], dtype=torch.bool, device=uc.device)
     mask[z0:z1, y0:y1, x0:x1] = False
     return (uc[:, mask].sum(dim=1) * dh_c ** 3 + uf.sum(dim=(1, 2, 3)) * (0.5 * dh_c) ** 3)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# group-layout description of the same two-level grid, for the fix-up entry points of the library and of the oracle
+# ---------------------------------------------------------------------------------------------------------------
+def to_groups(field):
+    """[NV, nz, ny, nx] -> [G, NV, 16, 16, 16], g = (gz*Gy + gy)*Gx + gx (inverse of inputs.unpack)."""
+    nv, nz, ny, nx = field.shape
+    w = field.reshape(nv, nz // PS, PS, ny // PS, PS, nx // PS, PS)
+    return w.permute(1, 3, 5, 0, 2, 4, 6).reshape(-1, nv, PS, PS, PS).contiguous()
+
+
+def region_tables(region, cshape):
+    """parent [Gf] and coarse-fine face table [n, 8] (int32; layout documented in include/gamer_hydro.h,
+    gamer_flux_correct) of a box-shaped refined region of a periodic coarse level."""
+    z0, z1, y0, y1, x0, x1 = region
+    nz, ny, nx = cshape
+    gcy, gcx = ny // PS, nx // PS
+    fz, fy, fx = (z1 - z0) // 8, (y1 - y0) // 8, (x1 - x0) // 8          # fine groups per axis
+
+    def cgroup(Z, Y, X):
+        return ((Z // PS) * gcy + Y // PS) * gcx + X // PS
+
+    parent, table = [], []
+    for a in range(fz):
+        for b in range(fy):
+            for c in range(fx):
+                g = (a * fy + b) * fx + c
+                Z, Y, X = z0 + 8 * a, y0 + 8 * b, x0 + 8 * c              # coarse cell at the group's origin
+                parent.append(cgroup(Z, Y, X) * 8 + ((Z % PS) // 8) * 4 + ((Y % PS) // 8) * 2 + (X % PS) // 8)
+                for d, idx, n_idx, lo, hi, n_ax in ((0, c, fx, x0, x1, nx), (1, b, fy, y0, y1, ny), (2, a, fz, z0, z1, nz)):
+                    for side in (0, 1):
+                        if idx != (0 if side == 0 else n_idx - 1):
+                            continue
+                        face = lo if side == 0 else hi                    # coarse face index along d
+                        cell = (face - 1) % n_ax if side == 0 else face % n_ax
+                        pos_f = [Z, Y, X]
+                        pos_c = [Z, Y, X]
+                        pos_f[2 - d] = face % n_ax                        # a cell whose lower face is `face`
+                        pos_c[2 - d] = cell
+                        plane = (face % PS) // 8
+                        if d == 0:
+                            b0, a0 = Z % PS, Y % PS
+                        elif d == 1:
+                            b0, a0 = Z % PS, X % PS
+                        else:
+                            b0, a0 = Y % PS, X % PS
+                        table.append([g, d, side, cgroup(*pos_f), plane, (b0 << 8) | a0, cgroup(*pos_c),
+                                      ((pos_c[0] % PS) << 16) | ((pos_c[1] % PS) << 8) | (pos_c[2] % PS)])
+    return torch.tensor(parent, dtype=torch.int32), torch.tensor(table, dtype=torch.int32).reshape(-1, 8)
+
+
+def fixup_in_group_layout(restrict_fn, accumulate_fn, correct_fn):
+    """Adapter for two_level_step(fixup=...): restrict_fn(fine_groups, coarse_groups, parent) -> coarse_groups;
+    accumulate_fn(acc_or_None, flux, weight) -> acc; correct_fn(coarse_groups, coarse_flux, fine_flux_avg, table, lam)
+    -> coarse_groups.  All arrays are torch tensors in the solver's group layouts."""
+    def fixup(uc1, uf, flux_c, fine_fluxes, region, lam):
+        parent, table = region_tables(region, uc1.shape[1:])
+        cdims = inputs.group_dims(uc1)
+        cg = restrict_fn(to_groups(uf), to_groups(uc1), parent.to(uc1.device))
+        acc = None
+        for f in fine_fluxes:
+            acc = accumulate_fn(acc, f, 1.0 / len(fine_fluxes))
+        cg = correct_fn(cg, flux_c, acc, table.to(uc1.device), lam)
+        return inputs.unpack(cg, *cdims)
+    return fixup

@@ -45,3 +45,53 @@ def test_flux_correction_conserves_composite_grid(oracle_mod):
         uc2, uf2, _ = amr.two_level_step(no_flux, uc2, uf2, region, dh_c, dt_c)
     t1 = amr.composite_total(uc2, uf2, region, dh_c)
     assert ((t1 - t0).abs() / scale)[4].item() > 1e-9
+
+
+def test_oracle_fixup_functions_in_group_layout(oracle_mod):
+    """Pins oracle.restrict / oracle.flux_correct (the C loops the CUDA fix-up kernels are compared with):
+    (a) restriction = the block mean (numpy reshape, an independent formulation), exact for a linear field, and it
+    conserves the sum; (b) with them in place of the harness's own global-array fix-up the two-level step gives the
+    same coarse level to round-off and conserves the composite grid (L112)."""
+    import numpy as np
+    rng = np.random.default_rng(5)
+    fine = rng.standard_normal((16, 5, 16, 16, 16))
+    coarse = np.zeros((2, 5, 16, 16, 16))
+    parent = np.arange(16, dtype=np.int32)                       # fine group g -> octant g of coarse group g // 8
+    oracle_mod.restrict(fine, coarse, parent)
+    for g in range(16):
+        oz, oy, ox = (g >> 2) & 1, (g >> 1) & 1, g & 1
+        blk = fine[g].reshape(5, 8, 2, 8, 2, 8, 2).mean(axis=(2, 4, 6))
+        got = coarse[g >> 3][:, oz * 8:oz * 8 + 8, oy * 8:oy * 8 + 8, ox * 8:ox * 8 + 8]
+        assert np.abs(got - blk).max() <= 2e-15      # summation order differs from numpy.mean
+    assert abs(coarse.sum() * 8 - fine.sum()) <= 1e-10
+    z, y, x = np.meshgrid(np.arange(16.0), np.arange(16.0), np.arange(16.0), indexing="ij")
+    lin = (1.0 + 2.0 * z - 3.0 * y + 0.5 * x)[None, None]
+    c1 = np.zeros((1, 1, 16, 16, 16))
+    oracle_mod.restrict(lin, c1, np.array([5], dtype=np.int32))  # octant (1, 0, 1)
+    zc, yc, xc = np.meshgrid(np.arange(8.0), np.arange(8.0), np.arange(8.0), indexing="ij")
+    assert np.abs(c1[0, 0, 8:, :8, 8:] - (1.0 + 2.0 * (2 * zc + 0.5) - 3.0 * (2 * yc + 0.5) + 0.5 * (2 * xc + 0.5))).max() <= 1e-13
+    assert c1[0, 0, :8].max() == 0.0                              # nothing outside the octant is touched
+
+    uc, uf, region, dh_c = amr.sedov_two_level(32, 64, 64, e_blast=5.7e-5, p_amb=1.0)
+    uf = torch.roll(uf, shifts=(0, 0, 31), dims=(1, 2, 3))
+    z0, z1, y0, y1, x0, x1 = region
+    uc[:, z0:z1, y0:y1, x0:x1] = amr.restrict(uf)
+    opts = oracle_mod.make_opts(min_pres=1e-10)
+
+    def solver(p, dt, dh):
+        r = oracle_mod.fluid_advance(p.numpy(), dt, dh, G53, MHM, PLM, HLLE, opts)
+        return torch.from_numpy(r["out"]), torch.from_numpy(r["flux"])
+
+    fix = amr.fixup_in_group_layout(
+        lambda f, c, par: torch.from_numpy(oracle_mod.restrict(f.numpy(), c.numpy().copy(), par.numpy())),
+        lambda acc, f, w: (w * f if acc is None else acc + w * f),
+        lambda c, fc, ff, tab, lam: torch.from_numpy(oracle_mod.flux_correct(c.numpy().copy(), fc.numpy(), ff.numpy(), tab.numpy(), lam)))
+    dt_c = 0.3 * dh_c / 12.0
+    tot0 = amr.composite_total(uc, uf, region, dh_c)
+    ua, fa, _ = amr.two_level_step(solver, uc, uf, region, dh_c, dt_c)
+    ub, fb, _ = amr.two_level_step(solver, uc, uf, region, dh_c, dt_c, fixup=fix)
+    assert torch.equal(fa, fb)
+    assert ((ua - ub).abs().amax(dim=(1, 2, 3)) <= 1e-14 * ua.abs().amax(dim=(1, 2, 3))).all()
+    assert (ua - uc).abs().max().item() > 1e-6
+    tot1 = amr.composite_total(ub, fb, region, dh_c)
+    assert ((tot1 - tot0).abs() / (tot0.abs() + 1e-6)).max().item() <= 1e-12
