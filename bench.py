@@ -262,6 +262,32 @@ def main():
         finite = finite and bool(torch.isfinite(ua).all().item())
         del ub, nbr
 
+    # ---- extra: the L112 fix-up kernels (NEXT-2) on this batch taken as a fine level: restriction of all groups into
+    # groups/8 parent groups, and the time-averaging pass over flux_out; both are pure HBM streams
+    fixup = None
+    if world == 1 and args.groups >= 64:
+        nf = (args.groups // 8) * 8
+        parent = torch.arange(nf, dtype=torch.int32, device=dev)          # fine g -> octant g % 8 of coarse g // 8
+        coarse = torch.empty((nf // 8,) + tuple(out.shape[1:]), dtype=dtype, device=dev)
+        acc = torch.empty_like(flux)
+        gb.gamer_restrict(out[:nf], coarse, parent, stream)
+        gb.gamer_flux_accumulate(acc, flux, 0.5, True, stream)
+        b0, b1, b2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        b0.record(stream)
+        for _ in range(5):
+            gb.gamer_restrict(out[:nf], coarse, parent, stream)
+        b1.record(stream)
+        for _ in range(5):
+            gb.gamer_flux_accumulate(acc, flux, 0.5, False, stream)
+        b2.record(stream)
+        torch.cuda.synchronize()
+        rb = (out[:nf].numel() + coarse.numel()) * sz
+        ab = 3 * flux.numel() * sz
+        fixup = {"restrict_GBs": rb * 5 / (b0.elapsed_time(b1) * 1e-3) / 1e9, "restrict_bytes": rb,
+                 "flux_accumulate_GBs": ab * 5 / (b1.elapsed_time(b2) * 1e-3) / 1e9, "flux_accumulate_bytes": ab,
+                 "hbm_peak_GBs": peaks()[0]}
+        del coarse, acc, parent
+
     # ---- e2e: host buffers through the C ABI, copies inside the timed region
     e2e = None
     if not args.no_e2e:
@@ -348,7 +374,7 @@ def main():
             "dtype": "f32" if sz == 4 else "f64", "data": "synthetic",
             "config": workload_config(args, args.groups), "clocks": sampler.summary(), "e2e": e2e,
             "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
-            "with_ghost_refresh": refresh_value, "with_fused_ghost_refresh": fused_value, "outputs_finite": finite,
+            "with_ghost_refresh": refresh_value, "with_fused_ghost_refresh": fused_value, "fixup_kernels": fixup, "outputs_finite": finite,
             "paper_context": "P100-PCIe fp32 ~2e8 cells/s incl. PCIe (PAPER.md L318-320); other hardware, not a target"}
     print(json.dumps(line), flush=True)
     if world > 1:

@@ -120,6 +120,34 @@ int gamer_fluid_advance_resident(const void* u, const int32_t* nbr, void* out, v
 /* Fills nbr[gz*gy*gx][27] (device int32) for a periodic box of gz x gy x gx groups, g = (z*gy + y)*gx + x. */
 int gamer_neighbors_periodic(int32_t* nbr, int gz, int gy, int gx, void* stream);
 
+/* ---- The two fix-up operations between a refined level and its parent level,
+ * on the same patch-group layouts as the solver.  All pointers are device pointers; nothing is allocated.
+ *
+ * Restriction: fine[n_fine][nvar][16][16][16] -> the octants of coarse[..][nvar][16][16][16] that the fine groups
+ * cover; parent[g] (device int32) = coarse group * 8 + octant, octant = oz*4 + oy*2 + ox.  Each coarse cell becomes
+ * 1/8 of the sum of its eight children, added in the order (dz,dy,dx) = (0,0,0), (0,0,1), (0,1,0), ... */
+int gamer_restrict(const void* fine, void* coarse, const int32_t* parent, int64_t n_fine, int nvar, int precision,
+                   void* stream);
+
+/* acc = (init ? 0 : acc) + weight * flux over n_groups flux_out batches ([n_groups][3][3][nvar][16][16]): the time
+ * average of the fine level's flux_out over its sub-steps (weight = dt_sub / dt_coarse). */
+int gamer_flux_accumulate(void* acc, const void* flux, double weight, int64_t n_groups, int nvar, int init,
+                          int precision, void* stream);
+
+/* Flux correction of the coarse cells next to coarse-fine boundaries:
+ *   U_cell += sgn * lam * (avg2x2(fine_flux_avg) - coarse_flux),   lam = dt_coarse / dh_coarse,
+ * avg2x2 = 0.25 * (((f00 + f01) + f10) + f11) over the 2 x 2 fine faces of a coarse face.  table[n_entries][8]
+ * (device int32), one entry per outer face of a fine group that is a coarse-fine boundary (8 x 8 coarse faces):
+ *   [0] fine group  [1] axis d  [2] side: 0 = the group's low face (its flux plane 0, sgn = -1: the face is the upper
+ *   face of the corrected cells), 1 = high face (plane 2, sgn = +1)  [3] coarse group whose flux_out holds the coarse
+ *   flux of that face  [4] its plane (0,1,2)  [5] (b0 << 8) | a0 = origin of the 8 x 8 quadrant inside that 16 x 16
+ *   plane (b = slower, a = faster remaining axis)  [6] coarse group that owns the corrected cells
+ *   [7] (z << 16) | (y << 8) | x = the corrected cell with b = a = 0 (its coordinate along d is the cell layer).
+ * The entries are applied in six passes (axis 0 side 0, axis 0 side 1, axis 1 side 0, ...); inside a pass no two
+ * entries may touch the same cell, so the result does not depend on the execution order (bitwise reproducible). */
+int gamer_flux_correct(void* coarse, const void* coarse_flux, const void* fine_flux_avg, const int32_t* table,
+                       int64_t n_entries, int nvar, double lam, int precision, void* stream);
+
 /* End-to-end form with HOST buffers (pinned or pageable): copies `in` to the device in chunks,
  * runs the solver, copies `out`, `flux_out` (nullable) and `group_speed_out` (nullable) back,
  * overlapping copies and kernels on internal streams as the paper does with CUDA streams (L242),

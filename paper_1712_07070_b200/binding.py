@@ -21,7 +21,8 @@ LIB_PATH = os.path.join(_HERE, "libgamerhydro.so")
 
 EXPORTS = ["gamer_fluid_advance", "gamer_fluid_advance_ex", "gamer_cfl_dt", "gamer_cfl_dt_ex",
            "gamer_cfl_from_group_speed", "gamer_refresh_ghosts_periodic", "gamer_fluid_advance_resident",
-           "gamer_neighbors_periodic", "gamer_fluid_advance_host",
+           "gamer_neighbors_periodic", "gamer_restrict", "gamer_flux_accumulate", "gamer_flux_correct",
+           "gamer_fluid_advance_host",
            "gamer_launch_count", "gamer_strerror", "gamer_version"]
 
 
@@ -70,6 +71,9 @@ def lib():
         L.gamer_refresh_ghosts_periodic.argtypes = [vp, vp, ci, ci, ci, ci, ci, vp]
         L.gamer_fluid_advance_resident.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, ci, ci, ctypes.POINTER(gamer_opts)]
         L.gamer_neighbors_periodic.argtypes = [vp, ci, ci, ci, vp]
+        L.gamer_restrict.argtypes = [vp, vp, vp, i64, ci, ci, vp]
+        L.gamer_flux_accumulate.argtypes = [vp, vp, dbl, i64, ci, ci, ci, vp]
+        L.gamer_flux_correct.argtypes = [vp, vp, vp, vp, i64, ci, dbl, ci, vp]
         L.gamer_fluid_advance_host.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, ci, ci,
                                                ctypes.POINTER(gamer_opts)]
         L.gamer_launch_count.restype = ctypes.c_int64
@@ -172,6 +176,29 @@ def gamer_neighbors_periodic(gz, gy, gx, device, stream=None):
     nbr = torch.empty((gz * gy * gx, 27), dtype=torch.int32, device=device)
     _check(lib().gamer_neighbors_periodic(_ptr(nbr), gz, gy, gx, _stream_handle(stream)), "gamer_neighbors_periodic")
     return nbr
+
+
+def gamer_restrict(fine, coarse, parent, stream=None):
+    """PAPER.md L112 restriction: fine [Gf,NV,16,16,16] into the octants of coarse [Gc,NV,16,16,16] (in place)."""
+    if parent.dtype != torch.int32 or parent.shape[0] != fine.shape[0]:
+        raise GamerError("parent must be an int32 tensor of length n_fine")
+    _check(lib().gamer_restrict(_ptr(fine), _ptr(coarse), _ptr(parent), fine.shape[0], fine.shape[1], _precision(fine),
+                                _stream_handle(stream)), "gamer_restrict")
+
+
+def gamer_flux_accumulate(acc, flux, weight, init, stream=None):
+    """acc = (init ? 0 : acc) + weight * flux for flux_out batches [G,3,3,NV,16,16]."""
+    _check(lib().gamer_flux_accumulate(_ptr(acc), _ptr(flux), float(weight), flux.shape[0], flux.shape[3], int(bool(init)),
+                                       _precision(flux), _stream_handle(stream)), "gamer_flux_accumulate")
+
+
+def gamer_flux_correct(coarse, coarse_flux, fine_flux_avg, table, lam, stream=None):
+    """PAPER.md L112 flux correction of the coarse cells next to coarse-fine boundaries (coarse modified in place)."""
+    if table.dtype != torch.int32 or table.dim() != 2 or table.shape[1] != 8:
+        raise GamerError("table must be an int32 tensor of shape [n_entries, 8]")
+    _check(lib().gamer_flux_correct(_ptr(coarse), _ptr(coarse_flux), _ptr(fine_flux_avg), _ptr(table), table.shape[0],
+                                    coarse.shape[1], float(lam), _precision(coarse), _stream_handle(stream)),
+           "gamer_flux_correct")
 
 
 def gamer_fluid_advance_host(in_host, out_host, flux_out_host, group_speed_out_host, dt, dh, gamma, scheme, recon,

@@ -217,6 +217,56 @@ extern "C" int gamer_refresh_ghosts_periodic(const void* u, void* in, int gz, in
     return cudaGetLastError() == cudaSuccess ? GAMER_OK : GAMER_ECUDA;
 }
 
+// ------------------------------------------------------------------------------------------ coarse-fine fix-up
+extern "C" int gamer_restrict(const void* fine, void* coarse, const int32_t* parent, int64_t n_fine, int nvar,
+                              int precision, void* stream) {
+    if (n_fine < 0 || nvar < 1 || nvar > 6 || (precision != GAMER_FP32 && precision != GAMER_FP64)) return GAMER_EINVAL;
+    if (n_fine > 0 && (!fine || !coarse || !parent)) return GAMER_EINVAL;
+    if (n_fine == 0) return GAMER_OK;
+    if (n_fine * nvar > 0x7fffffff) return GAMER_EUNSUPPORTED;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const unsigned grid = (unsigned)(n_fine * nvar);
+    if (precision == GAMER_FP32) restrict_kernel<float><<<grid, 512, 0, st>>>(static_cast<const float*>(fine), static_cast<float*>(coarse), parent, nvar);
+    else restrict_kernel<double><<<grid, 512, 0, st>>>(static_cast<const double*>(fine), static_cast<double*>(coarse), parent, nvar);
+    g_launches += 1;
+    return cudaGetLastError() == cudaSuccess ? GAMER_OK : GAMER_ECUDA;
+}
+
+extern "C" int gamer_flux_accumulate(void* acc, const void* flux, double weight, int64_t n_groups, int nvar, int init,
+                                     int precision, void* stream) {
+    if (n_groups < 0 || nvar < 1 || nvar > 6 || (precision != GAMER_FP32 && precision != GAMER_FP64)) return GAMER_EINVAL;
+    if (n_groups > 0 && (!acc || !flux)) return GAMER_EINVAL;
+    if (!std::isfinite(weight)) return GAMER_EINVAL;
+    if (n_groups == 0) return GAMER_OK;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const long long n = (long long)n_groups * 9 * nvar * PS * PS;
+    const unsigned grid = (unsigned)((n + 1023) / 1024 > 148 * 8 ? 148 * 8 : (n + 1023) / 1024);
+    if (precision == GAMER_FP32) flux_accumulate_kernel<float><<<grid, 256, 0, st>>>(static_cast<float*>(acc), static_cast<const float*>(flux), (float)weight, n, init);
+    else flux_accumulate_kernel<double><<<grid, 256, 0, st>>>(static_cast<double*>(acc), static_cast<const double*>(flux), weight, n, init);
+    g_launches += 1;
+    return cudaGetLastError() == cudaSuccess ? GAMER_OK : GAMER_ECUDA;
+}
+
+extern "C" int gamer_flux_correct(void* coarse, const void* coarse_flux, const void* fine_flux_avg, const int32_t* table,
+                                  int64_t n_entries, int nvar, double lam, int precision, void* stream) {
+    if (n_entries < 0 || nvar < 1 || nvar > 6 || (precision != GAMER_FP32 && precision != GAMER_FP64)) return GAMER_EINVAL;
+    if (n_entries > 0 && (!coarse || !coarse_flux || !fine_flux_avg || !table)) return GAMER_EINVAL;
+    if (!std::isfinite(lam)) return GAMER_EINVAL;
+    if (n_entries == 0) return GAMER_OK;
+    if (n_entries > 0x7fffffff) return GAMER_EUNSUPPORTED;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    for (int pass = 0; pass < 6; ++pass) {
+        if (precision == GAMER_FP32)
+            flux_correct_kernel<float><<<(unsigned)n_entries, 64, 0, st>>>(static_cast<float*>(coarse), static_cast<const float*>(coarse_flux),
+                                                                          static_cast<const float*>(fine_flux_avg), table, nvar, (float)lam, pass);
+        else
+            flux_correct_kernel<double><<<(unsigned)n_entries, 64, 0, st>>>(static_cast<double*>(coarse), static_cast<const double*>(coarse_flux),
+                                                                           static_cast<const double*>(fine_flux_avg), table, nvar, lam, pass);
+        g_launches += 1;
+    }
+    return cudaGetLastError() == cudaSuccess ? GAMER_OK : GAMER_ECUDA;
+}
+
 // ------------------------------------------------------------------------------------------ host-buffer entry
 extern "C" int gamer_fluid_advance_host(const void* in_host, void* out_host, void* flux_out_host,
                                         void* group_speed_out_host, int64_t n_groups, double dt, double dh,

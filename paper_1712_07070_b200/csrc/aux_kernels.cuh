@@ -143,4 +143,63 @@ __global__ void neighbors_periodic_kernel(int* __restrict__ nbr, int gz, int gy,
     nbr[i] = (int)(((long long)sz * gy + sy) * gx + sx);
 }
 
+// ---------------------------------------------------------------------------------------------
+// fix-up between a refined patch group and the coarse level
+// ---------------------------------------------------------------------------------------------
+// restriction: one CTA per (fine group, variable), one thread per coarse cell of the 8^3 octant; the eight children
+// are added in the order (dz, dy, dx) = (0,0,0), (0,0,1), ... and scaled by 1/8
+template <typename T>
+__global__ void __launch_bounds__(512) restrict_kernel(const T* __restrict__ fine, T* __restrict__ coarse,
+                                                       const int* __restrict__ parent, int nvar) {
+    const long long gv = blockIdx.x;
+    const long long g = gv / nvar;
+    const int v = (int)(gv - g * nvar);
+    const int par = parent[g];
+    const int oz = (par >> 2) & 1, oy = (par >> 1) & 1, ox = par & 1;
+    const int t = threadIdx.x, i = t & 7, j = (t >> 3) & 7, k = t >> 6;
+    const T* f = fine + ((size_t)g * nvar + v) * (PS * PS * PS) + ((2 * k) * PS + 2 * j) * PS + 2 * i;
+    T s = T(0);
+#pragma unroll
+    for (int dz = 0; dz < 2; ++dz)
+#pragma unroll
+        for (int dy = 0; dy < 2; ++dy) {
+            // two neighbouring fine cells in one vector load
+            const T a = f[(dz * PS + dy) * PS], b = f[(dz * PS + dy) * PS + 1];
+            s = s + a;
+            s = s + b;
+        }
+    coarse[((size_t)(par >> 3) * nvar + v) * (PS * PS * PS) + ((oz * 8 + k) * PS + (oy * 8 + j)) * PS + (ox * 8 + i)] = T(0.125) * s;
+}
+
+// acc = (init ? 0 : acc) + w * flux, elementwise (time average of the fine flux_out over the sub-steps)
+template <typename T>
+__global__ void flux_accumulate_kernel(T* __restrict__ acc, const T* __restrict__ flux, T w, long long n, int init) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+        acc[i] = init ? w * flux[i] : acc[i] + w * flux[i];
+}
+
+// flux correction: one CTA per table entry (an 8 x 8 patch of coarse faces), thread = coarse face; only the entries
+// of pass = axis * 2 + side act, so no two CTAs of a launch touch the same cell and the result is order-independent
+template <typename T>
+__global__ void __launch_bounds__(64) flux_correct_kernel(T* __restrict__ coarse, const T* __restrict__ coarse_flux,
+                                                          const T* __restrict__ fine_flux_avg, const int* __restrict__ tab,
+                                                          int nvar, T lam, int pass) {
+    const int* e = tab + 8 * (size_t)blockIdx.x;
+    const int d = e[1], side = e[2];
+    if (d * 2 + side != pass) return;
+    const T sgn = side ? T(1) : T(-1);
+    const int b0 = e[5] >> 8, a0 = e[5] & 255;
+    const int b = threadIdx.x >> 3, a = threadIdx.x & 7;
+    int z = e[7] >> 16, y = (e[7] >> 8) & 255, x = e[7] & 255;
+    if (d == 0) { z += b; y += a; } else if (d == 1) { z += b; x += a; } else { y += b; x += a; }
+    for (int v = 0; v < nvar; ++v) {
+        const T* ff = fine_flux_avg + ((((size_t)e[0] * 3 + d) * 3 + (side ? 2 : 0)) * nvar + v) * (PS * PS) + (2 * b) * PS + 2 * a;
+        const T* fc = coarse_flux + ((((size_t)e[3] * 3 + d) * 3 + e[4]) * nvar + v) * (PS * PS);
+        T* c = coarse + ((size_t)e[6] * nvar + v) * (PS * PS * PS) + (z * PS + y) * PS + x;
+        const T favg = T(0.25) * (((ff[0] + ff[1]) + ff[PS]) + ff[PS + 1]);
+        const T corr = lam * (favg - fc[(b0 + b) * PS + (a0 + a)]);
+        *c += sgn * corr;
+    }
+}
+
 }  // namespace gamer

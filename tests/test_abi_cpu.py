@@ -65,6 +65,16 @@ def test_argument_validation_needs_no_gpu(built_lib):
     o.remedy_first_order = 1
     assert L.gamer_fluid_advance_resident(ok[0], vp(16384), ok[1], None, 1, 0.1, 0.1, 1.4, 2, 1, 1, 4, ctypes.byref(o)) == -2
     assert L.gamer_fluid_advance_resident(ok[0], vp(16384), ok[0], None, 1, 0.1, 0.1, 1.4, 1, 1, 1, 4, None) == -1
+    L.gamer_restrict.argtypes = [vp, vp, vp, i64, ci, ci, vp]
+    assert L.gamer_restrict(None, ok[1], vp(64), 1, 5, 4, None) == -1
+    assert L.gamer_restrict(ok[0], ok[1], vp(64), 1, 7, 4, None) == -1
+    assert L.gamer_restrict(ok[0], ok[1], vp(64), 0, 5, 4, None) == 0
+    L.gamer_flux_accumulate.argtypes = [vp, vp, dbl, i64, ci, ci, ci, vp]
+    assert L.gamer_flux_accumulate(ok[0], None, 0.5, 1, 5, 1, 4, None) == -1
+    assert L.gamer_flux_accumulate(ok[0], ok[1], float("inf"), 1, 5, 1, 4, None) == -1
+    L.gamer_flux_correct.argtypes = [vp, vp, vp, vp, i64, ci, dbl, ci, vp]
+    assert L.gamer_flux_correct(ok[0], ok[1], vp(16384), None, 1, 5, 0.1, 4, None) == -1
+    assert L.gamer_flux_correct(ok[0], ok[1], vp(16384), vp(64), 0, 5, 0.1, 4, None) == 0
     L.gamer_neighbors_periodic.argtypes = [vp, ci, ci, ci, vp]
     assert L.gamer_neighbors_periodic(None, 1, 1, 1, None) == -1
     assert L.gamer_neighbors_periodic(vp(4096), 0, 1, 1, None) == -1

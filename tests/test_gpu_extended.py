@@ -265,3 +265,88 @@ def test_fused_ghost_refresh_entry_is_bitwise_the_padded_path(dev, scheme, recon
         assert torch.equal(fl[bz, by, bx, 0, 2], fl[bz, by, (bx + 1) % gx, 0, 0])
         assert torch.equal(fl[bz, by, bx, 1, 2], fl[bz, (by + 1) % gy, bx, 1, 0])
         assert torch.equal(fl[bz, by, bx, 2, 2], fl[(bz + 1) % gz, by, bx, 2, 0])
+
+
+def _gpu_fixup():
+    """two_level_step(fixup=...) adapter that runs restriction, flux averaging and flux correction in the library."""
+    import amr_harness as amr
+
+    def restrict_fn(fine, coarse, parent):
+        coarse = coarse.clone()
+        gb.gamer_restrict(fine, coarse, parent)
+        return coarse
+
+    def accumulate_fn(acc, flux, w):
+        init = acc is None
+        acc = torch.empty_like(flux) if init else acc
+        gb.gamer_flux_accumulate(acc, flux.contiguous(), w, init)
+        return acc
+
+    def correct_fn(coarse, coarse_flux, fine_avg, table, lam):
+        gb.gamer_flux_correct(coarse, coarse_flux.contiguous(), fine_avg, table, lam)
+        return coarse
+
+    return amr.fixup_in_group_layout(restrict_fn, accumulate_fn, correct_fn)
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+def test_fixup_kernels_match_oracle(dev, oracle_mod, dtype):
+    """gamer_restrict / gamer_flux_accumulate / gamer_flux_correct against the
+    oracle's C loops on random data, with the tables of a box-shaped refined region that touches the periodic wrap
+    (so corrected cells and coarse fluxes come from other groups than the parents).  fp64: the same operations in
+    the same order -> identical bits; fp32: 1e-6 of the scale."""
+    import amr_harness as amr
+    region = (0, 16, 8, 24, 24, 48)                  # coarse cells; z starts at the periodic boundary
+    cshape = (32, 32, 48)
+    parent, table = amr.region_tables(region, cshape)
+    n_c, n_f = (32 // 16) * (32 // 16) * (48 // 16), parent.shape[0]
+    assert n_f == 2 * 2 * 3 and table.shape[0] == 2 * (2 * 2 + 2 * 3 + 2 * 3)
+    g = torch.Generator().manual_seed(11)
+    fine = torch.randn((n_f, 5, 16, 16, 16), generator=g, dtype=torch.float64).to(dtype)
+    coarse = torch.randn((n_c, 5, 16, 16, 16), generator=g, dtype=torch.float64).to(dtype)
+    cflux = torch.randn((n_c, 3, 3, 5, 16, 16), generator=g, dtype=torch.float64).to(dtype)
+    ff = [torch.randn((n_f, 3, 3, 5, 16, 16), generator=g, dtype=torch.float64).to(dtype) for _ in range(2)]
+    lam = 0.37
+    ref = oracle_mod.restrict(fine.double().numpy(), coarse.double().numpy().copy(), parent.numpy())
+    favg = 0.5 * ff[0].double().numpy() + 0.5 * ff[1].double().numpy()
+    ref = oracle_mod.flux_correct(ref, cflux.double().numpy(), favg, table.numpy(), lam)
+    c_gpu = coarse.to(dev).clone()
+    gb.gamer_restrict(fine.to(dev), c_gpu, parent.to(dev))
+    acc = torch.empty_like(ff[0], device=dev)
+    gb.gamer_flux_accumulate(acc, ff[0].to(dev), 0.5, True)
+    gb.gamer_flux_accumulate(acc, ff[1].to(dev), 0.5, False)
+    gb.gamer_flux_correct(c_gpu, cflux.to(dev), acc, table.to(dev), lam)
+    torch.cuda.synchronize()
+    got = c_gpu.cpu().double().numpy()
+    assert np.abs(ref - coarse.double().numpy()).max() > 0.1          # the fix-up did change cells
+    if dtype == torch.float64:
+        assert np.array_equal(got, ref)
+        assert np.array_equal(acc.cpu().numpy(), favg)
+    else:
+        assert np.abs(got - ref).max() <= 1e-6 * np.abs(ref).max()
+    # cells outside the refined octants and the corrected layers are untouched
+    untouched = (ref == coarse.double().numpy())
+    assert np.array_equal(got[untouched], coarse.double().numpy()[untouched])
+
+
+def test_config3_with_gpu_fixup(dev):
+    """Config 3 (reduced to 64 x 128 x 128 coarse cells) with the whole L112 fix-up on the GPU: same coarse level as
+    the harness's global-array fix-up to round-off, composite grid conserved to 1e-12."""
+    import amr_harness as amr
+    uc, uf, region, dh_c = amr.sedov_two_level(64, 128, 128, gamma=G53, device=dev)
+    kw = dict(min_pres=1e-10)
+
+    def gpu_solver(p, dt, dh):
+        out, flux, speed, nun, diag = gpu_ex(p.contiguous(), dt, dh, G53, gb.MHM, gb.PLM, gb.HLLE, **kw)
+        return out, flux
+
+    pb = (G53 - 1.0) / (8 * (0.5 * dh_c) ** 3)
+    dt_c = 2 * 0.4 * (0.5 * dh_c) / (3.0 * math.sqrt(G53 * pb))
+    tot0 = amr.composite_total(uc, uf, region, dh_c)
+    ua, fa, _ = amr.two_level_step(gpu_solver, uc, uf, region, dh_c, dt_c)
+    ub, fb, _ = amr.two_level_step(gpu_solver, uc, uf, region, dh_c, dt_c, fixup=_gpu_fixup())
+    torch.cuda.synchronize()
+    assert torch.equal(fa, fb)
+    assert ((ua - ub).abs().amax(dim=(1, 2, 3)) <= 1e-13 * (ua.abs().amax(dim=(1, 2, 3)) + 1e-30)).all()
+    tot1 = amr.composite_total(ub, fb, region, dh_c)
+    assert ((tot1 - tot0).abs() / (tot0.abs() + 1e-6)).max().item() <= 1e-12      # total momentum is 0: absolute bound there
