@@ -175,3 +175,51 @@ def flux_correct(coarse, coarse_flux, fine_flux_avg, table, lam):
     lib().oracle_flux_correct(_p(coarse), _p(coarse_flux), _p(fine_flux_avg), _p(table), ctypes.c_int64(table.shape[0]),
                               int(coarse.shape[1]), ctypes.c_double(lam))
     return coarse
+
+
+PERIODIC, OUTFLOW, REFLECTING = 0, 1, 2
+
+
+def fill_ghosts(field, bc=((PERIODIC, PERIODIC),) * 3):
+    """Same-level "preparation" step with the standard boundary conditions of L98 on a uniform level:
+    field [NV, nz, ny, nx] (conserved; variable 1, 2, 3 = x, y, z momentum) -> padded groups [G, NV, 22, 22, 22],
+    g = (gz*Gy + gy)*Gx + gx.  bc = ((x_lo, x_hi), (y_lo, y_hi), (z_lo, z_hi)); a ghost cell c outside [0, n) takes
+    the value of cell  c mod n (periodic),  the nearest cell inside (outflow, zero gradient),  or the mirror cell
+    -1-c / 2n-1-c with the momentum normal to that face negated (reflecting).  Plain per-axis index tables."""
+    field = np.asarray(field)
+    nv, nz, ny, nx = field.shape
+    n_ax = {0: nx, 1: ny, 2: nz}
+    src, flip = {}, {}
+    for ax in range(3):
+        n = n_ax[ax]
+        assert n % PS == 0
+        s = np.empty((n // PS, NP), dtype=np.int64)
+        f = np.zeros((n // PS, NP), dtype=bool)
+        for b in range(n // PS):
+            for l in range(NP):
+                c = b * PS + l - NG
+                if 0 <= c < n:
+                    s[b, l] = c
+                    continue
+                kind = bc[ax][0] if c < 0 else bc[ax][1]
+                if kind == PERIODIC:
+                    s[b, l] = c % n
+                elif kind == OUTFLOW:
+                    s[b, l] = 0 if c < 0 else n - 1
+                elif kind == REFLECTING:
+                    s[b, l] = -1 - c if c < 0 else 2 * n - 1 - c
+                    f[b, l] = True
+                else:
+                    raise ValueError("unknown boundary condition")
+        src[ax], flip[ax] = s, f
+    gz, gy, gx = nz // PS, ny // PS, nx // PS
+    out = np.empty((gz * gy * gx, nv, NP, NP, NP), dtype=field.dtype)
+    for bz in range(gz):
+        for by in range(gy):
+            for bx in range(gx):
+                blk = field[:, src[2][bz]][:, :, src[1][by]][:, :, :, src[0][bx]].copy()
+                blk[1][:, :, flip[0][bx]] *= -1.0          # x momentum in cells mirrored across an x face
+                blk[2][:, flip[1][by], :] *= -1.0
+                blk[3][flip[2][bz], :, :] *= -1.0
+                out[(bz * gy + by) * gx + bx] = blk
+    return out
