@@ -102,6 +102,16 @@ int gamer_cfl_from_group_speed(const void* group_speed, int64_t n_groups, double
 int gamer_refresh_ghosts_periodic(const void* u, void* in, int gz, int gy, int gx, int nvar,
                                   int precision, void* stream);
 
+/* The same for a uniform level with the standard boundary conditions of PAPER.md L98, set per face:
+ * bc[6] = {x_lo, x_hi, y_lo, y_hi, z_lo, z_hi} (host ints), GAMER_BC_PERIODIC (ghost cell c takes cell c mod n),
+ * GAMER_BC_OUTFLOW (zero gradient: the nearest cell inside) or GAMER_BC_REFLECTING (the mirror cell -1-c / 2n-1-c
+ * with the momentum normal to that face negated).  Inflow (user-defined) boundaries are the caller's own fill. */
+#define GAMER_BC_PERIODIC   0
+#define GAMER_BC_OUTFLOW    1
+#define GAMER_BC_REFLECTING 2
+int gamer_refresh_ghosts(const void* u, void* in, int gz, int gy, int gx, int nvar, const int* bc,
+                         int precision, void* stream);
+
 /* Device-resident step with the same-level ghost refresh FUSED into the staging loads (SURVEY 8(f) NEXT-1,
  * PAPER.md L248 "preparation" + L274 Fig. 3): `u` is the UNPADDED state of the whole batch,
  * u[n_groups][NVAR][16][16][16] (the `out` layout), and nbr[n_groups][27] (device int32) names, for every group,

@@ -14,13 +14,14 @@ PLM, PPM = 1, 2
 ROE, HLLC, HLLE = 1, 2, 3
 FP32, FP64 = 4, 8
 GMINMOD, VANLEER, VANALBADA = 1, 2, 3
+BC_PERIODIC, BC_OUTFLOW, BC_REFLECTING = 0, 1, 2
 PS, NG, NP = 16, 3, 22
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libgamerhydro.so")
 
 EXPORTS = ["gamer_fluid_advance", "gamer_fluid_advance_ex", "gamer_cfl_dt", "gamer_cfl_dt_ex",
-           "gamer_cfl_from_group_speed", "gamer_refresh_ghosts_periodic", "gamer_fluid_advance_resident",
+           "gamer_cfl_from_group_speed", "gamer_refresh_ghosts_periodic", "gamer_refresh_ghosts", "gamer_fluid_advance_resident",
            "gamer_neighbors_periodic", "gamer_restrict", "gamer_flux_accumulate", "gamer_flux_correct",
            "gamer_fluid_advance_host",
            "gamer_launch_count", "gamer_strerror", "gamer_version"]
@@ -69,6 +70,7 @@ def lib():
         L.gamer_cfl_dt_ex.argtypes = cfl + [ctypes.POINTER(gamer_opts)]
         L.gamer_cfl_from_group_speed.argtypes = [vp, i64, dbl, dbl, ci, vp, vp]
         L.gamer_refresh_ghosts_periodic.argtypes = [vp, vp, ci, ci, ci, ci, ci, vp]
+        L.gamer_refresh_ghosts.argtypes = [vp, vp, ci, ci, ci, ci, ctypes.POINTER(ci), ci, vp]
         L.gamer_fluid_advance_resident.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, ci, ci, ctypes.POINTER(gamer_opts)]
         L.gamer_neighbors_periodic.argtypes = [vp, ci, ci, ci, vp]
         L.gamer_restrict.argtypes = [vp, vp, vp, i64, ci, ci, vp]
@@ -158,6 +160,13 @@ def gamer_cfl_from_group_speed(group_speed, dh, cfl, dt_out, stream=None):
 def gamer_refresh_ghosts_periodic(u, u_in, gz, gy, gx, stream=None):
     _check(lib().gamer_refresh_ghosts_periodic(_ptr(u), _ptr(u_in), gz, gy, gx, u.shape[1], _precision(u),
                                                _stream_handle(stream)), "gamer_refresh_ghosts_periodic")
+
+
+def gamer_refresh_ghosts(u, u_in, gz, gy, gx, bc, stream=None):
+    """bc = (x_lo, x_hi, y_lo, y_hi, z_lo, z_hi) of BC_PERIODIC / BC_OUTFLOW / BC_REFLECTING."""
+    arr = (ctypes.c_int * 6)(*[int(b) for b in bc])
+    _check(lib().gamer_refresh_ghosts(_ptr(u), _ptr(u_in), gz, gy, gx, u.shape[1], arr, _precision(u),
+                                      _stream_handle(stream)), "gamer_refresh_ghosts")
 
 
 def gamer_fluid_advance_resident(u, nbr, out, flux_out, dt, dh, gamma, scheme, recon, riemann, opts=None):

@@ -217,6 +217,29 @@ extern "C" int gamer_refresh_ghosts_periodic(const void* u, void* in, int gz, in
     return cudaGetLastError() == cudaSuccess ? GAMER_OK : GAMER_ECUDA;
 }
 
+extern "C" int gamer_refresh_ghosts(const void* u, void* in, int gz, int gy, int gx, int nvar, const int* bc,
+                                    int precision, void* stream) {
+    if (!u || !in || !bc || gz < 1 || gy < 1 || gx < 1 || nvar < 5 || nvar > 6) return GAMER_EINVAL;
+    if (precision != GAMER_FP32 && precision != GAMER_FP64) return GAMER_EINVAL;
+    BcSet b;
+    for (int i = 0; i < 6; ++i) {
+        if (bc[i] < GAMER_BC_PERIODIC || bc[i] > GAMER_BC_REFLECTING) return GAMER_EINVAL;
+        b.v[i] = bc[i];
+    }
+    for (int a = 0; a < 3; ++a)      // a periodic axis is periodic on both faces
+        if ((bc[2 * a] == GAMER_BC_PERIODIC) != (bc[2 * a + 1] == GAMER_BC_PERIODIC)) return GAMER_EINVAL;
+    const long long ng = (long long)gz * gy * gx;
+    if (ng * nvar > 0x7fffffff) return GAMER_EUNSUPPORTED;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const unsigned grid = (unsigned)(ng * nvar);
+    if (precision == GAMER_FP32)
+        refresh_bc_kernel<float><<<grid, 256, 0, st>>>(static_cast<const float*>(u), static_cast<float*>(in), gz, gy, gx, nvar, b);
+    else
+        refresh_bc_kernel<double><<<grid, 256, 0, st>>>(static_cast<const double*>(u), static_cast<double*>(in), gz, gy, gx, nvar, b);
+    g_launches += 1;
+    return cudaGetLastError() == cudaSuccess ? GAMER_OK : GAMER_ECUDA;
+}
+
 // ------------------------------------------------------------------------------------------ coarse-fine fix-up
 extern "C" int gamer_restrict(const void* fine, void* coarse, const int32_t* parent, int64_t n_fine, int nvar,
                               int precision, void* stream) {

@@ -130,6 +130,57 @@ __global__ void __launch_bounds__(256) refresh_periodic_kernel(const T* __restri
     }
 }
 
+// Same-level ghost refresh of a uniform level with the boundary conditions of PAPER.md L98 per face:
+// 0 periodic, 1 outflow (zero gradient: nearest cell inside), 2 reflecting (mirror cell, normal momentum negated).
+// One CTA per (group, variable) as refresh_periodic_kernel; bc = {x_lo, x_hi, y_lo, y_hi, z_lo, z_hi}.
+struct BcSet { int v[6]; };
+
+// global cell index c (may lie outside [0, n)) -> source cell; *flip is set when the cell is a mirror image
+__device__ __forceinline__ int bc_source(int c, int n, int lo, int hi, bool* flip) {
+    *flip = false;
+    if (c >= 0 && c < n) return c;
+    const int kind = c < 0 ? lo : hi;
+    if (kind == 1) return c < 0 ? 0 : n - 1;
+    if (kind == 2) { *flip = true; return c < 0 ? -1 - c : 2 * n - 1 - c; }
+    return c < 0 ? c + n : c - n;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) refresh_bc_kernel(const T* __restrict__ u, T* __restrict__ in, int gz, int gy,
+                                                         int gx, int nvar, BcSet bc) {
+    const long long gv = blockIdx.x;
+    const long long g = gv / nvar;
+    const int v = (int)(gv - g * nvar);
+    const int bx = (int)(g % gx), by = (int)((g / gx) % gy), bz = (int)(g / ((long long)gx * gy));
+    const size_t gstride = (size_t)nvar * (PS * PS * PS);
+    size_t offxy[2];
+    bool live[2], neg[2];
+#pragma unroll
+    for (int r = 0; r < 2; ++r) {
+        const int t = threadIdx.x + r * 256;
+        live[r] = t < NP * NP;
+        const int pj = t / NP, pi = t - pj * NP;
+        bool fx, fy;
+        const int cx = bc_source(bx * PS + pi - NGH, gx * PS, bc.v[0], bc.v[1], &fx);
+        const int cy = bc_source(by * PS + pj - NGH, gy * PS, bc.v[2], bc.v[3], &fy);
+        neg[r] = (v == 1 && fx) != (v == 2 && fy);      // at most one of the two can be true for a given v
+        offxy[r] = ((size_t)(cy / PS) * gx + cx / PS) * gstride + (size_t)v * (PS * PS * PS) + (cy % PS) * PS + (cx % PS);
+    }
+    T* dst = in + ((size_t)g * nvar + v) * NPC;
+    for (int pk = 0; pk < NP; ++pk) {
+        bool fz;
+        const int cz = bc_source(bz * PS + pk - NGH, gz * PS, bc.v[4], bc.v[5], &fz);
+        const size_t offz = (size_t)(cz / PS) * gy * gx * gstride + (size_t)(cz % PS) * (PS * PS);
+        const bool nz = (v == 3 && fz);
+#pragma unroll
+        for (int r = 0; r < 2; ++r)
+            if (live[r]) {
+                const T val = __ldg(u + offz + offxy[r]);
+                dst[pk * (NP * NP) + threadIdx.x + r * 256] = (neg[r] != nz) ? -val : val;
+            }
+    }
+}
+
 // neighbour table of a periodic box of gz x gy x gx groups: nbr[g][(dz+1)*9 + (dy+1)*3 + (dx+1)]
 __global__ void neighbors_periodic_kernel(int* __restrict__ nbr, int gz, int gy, int gx) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;

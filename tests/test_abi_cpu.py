@@ -65,6 +65,10 @@ def test_argument_validation_needs_no_gpu(built_lib):
     o.remedy_first_order = 1
     assert L.gamer_fluid_advance_resident(ok[0], vp(16384), ok[1], None, 1, 0.1, 0.1, 1.4, 2, 1, 1, 4, ctypes.byref(o)) == -2
     assert L.gamer_fluid_advance_resident(ok[0], vp(16384), ok[0], None, 1, 0.1, 0.1, 1.4, 1, 1, 1, 4, None) == -1
+    L.gamer_refresh_ghosts.argtypes = [vp, vp, ci, ci, ci, ci, ctypes.POINTER(ci), ci, vp]
+    assert L.gamer_refresh_ghosts(ok[0], ok[1], 1, 1, 1, 5, (ci * 6)(0, 0, 0, 0, 0, 3), 4, None) == -1     # unknown kind
+    assert L.gamer_refresh_ghosts(ok[0], ok[1], 1, 1, 1, 5, (ci * 6)(0, 1, 0, 0, 0, 0), 4, None) == -1     # half-periodic axis
+    assert L.gamer_refresh_ghosts(ok[0], ok[1], 1, 1, 1, 5, None, 4, None) == -1
     L.gamer_restrict.argtypes = [vp, vp, vp, i64, ci, ci, vp]
     assert L.gamer_restrict(None, ok[1], vp(64), 1, 5, 4, None) == -1
     assert L.gamer_restrict(ok[0], ok[1], vp(64), 1, 7, 4, None) == -1
