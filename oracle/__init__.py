@@ -13,7 +13,7 @@ from . import build as _build
 
 MHM, CTU = 1, 2
 PLM, PPM = 1, 2
-ROE, HLLC, HLLE = 1, 2, 3
+ROE, HLLC, HLLE, EXACT = 1, 2, 3, 4
 GMINMOD, VANLEER, VANALBADA = 1, 2, 3
 
 PS, NG, NP = 16, 3, 22

@@ -53,7 +53,7 @@
 
 enum { SCHEME_MHM = 1, SCHEME_CTU = 2 };
 enum { RECON_PLM = 1, RECON_PPM = 2 };
-enum { RSOLVER_ROE = 1, RSOLVER_HLLC = 2, RSOLVER_HLLE = 3 };
+enum { RSOLVER_ROE = 1, RSOLVER_HLLC = 2, RSOLVER_HLLE = 3, RSOLVER_EXACT = 4 };
 enum { LIMITER_GMINMOD = 1, LIMITER_VANLEER = 2, LIMITER_VANALBADA = 3 };
 
 typedef struct {
@@ -327,6 +327,96 @@ static int solve_roe(const ctx_t *c, const rstate_t *L, const rstate_t *R, const
     return 0;
 }
 
+/* Exact Riemann solver ("exact solver based on Toro (2009)"; Toro ch. 4), reading R21 of DESIGN.md:
+ *  - pressure function f_K(p) of Toro eqs. 4.6-4.7 (shock branch for p > p_K, rarefaction branch otherwise) and its
+ *    derivative (eq. 4.37), star pressure from Newton-Raphson on f_L + f_R + (u_R - u_L) = 0 (eq. 4.5);
+ *  - first guess: the two-rarefaction value p_TR (eq. 4.46), exact when both waves are rarefactions and always
+ *    positive; if its numerator is not positive the data generate vacuum (eq. 4.40) and the solver reports failure
+ *    (the caller falls back to HLLE, as for remedy (i));
+ *  - iterate until 2|p_new - p_old| / (p_new + p_old) < 1e-6 (Toro's TOL), then ONE more step, at most 30 steps;
+ *    a negative iterate is reset to 1e-6 of the guess;
+ *  - u* from eq. 4.9, state at x/t = 0 sampled as in Toro section 4.5, transverse velocities taken from the side
+ *    of the contact the axis lies on (u* >= 0: left), flux = physical flux of that state. */
+static void pressure_fn(double p, double rho, double pk, double ck, double gamma, double *f, double *df)
+{
+    if (p > pk) {
+        double A = 2.0 / ((gamma + 1.0) * rho), B = (gamma - 1.0) / (gamma + 1.0) * pk;
+        double q = sqrt(A / (p + B));
+        *f = (p - pk) * q;
+        *df = q * (1.0 - 0.5 * (p - pk) / (B + p));
+    } else {
+        double pr = p / pk;
+        *f = 2.0 * ck / (gamma - 1.0) * (pow(pr, (gamma - 1.0) / (2.0 * gamma)) - 1.0);
+        *df = pow(pr, -(gamma + 1.0) / (2.0 * gamma)) / (rho * ck);
+    }
+}
+
+static int solve_exact(const ctx_t *c, const rstate_t *L, const rstate_t *R, double *F)
+{
+    const double g = c->gamma, gm1 = g - 1.0, gp1 = g + 1.0, z = gm1 / (2.0 * g);
+    const double du = R->u - L->u;
+    const double num = L->c + R->c - 0.5 * gm1 * du;
+    if (!(num > 0.0)) return 1;                                   /* vacuum is generated */
+    const double p0 = pow(num / (L->c / pow(L->P, z) + R->c / pow(R->P, z)), 1.0 / z);
+    double p = p0, fl, dfl, fr, dfr;
+    int extra = 0;
+    for (int it = 0; it < 30; ++it) {
+        pressure_fn(p, L->rho, L->P, L->c, g, &fl, &dfl);
+        pressure_fn(p, R->rho, R->P, R->c, g, &fr, &dfr);
+        double pn = p - (fl + fr + du) / (dfl + dfr);
+        if (!(pn > 0.0)) pn = 1e-6 * p0;
+        const double change = 2.0 * fabs(pn - p) / (pn + p);
+        p = pn;
+        if (extra) break;
+        if (change < 1e-6) extra = 1;
+    }
+    pressure_fn(p, L->rho, L->P, L->c, g, &fl, &dfl);
+    pressure_fn(p, R->rho, R->P, R->c, g, &fr, &dfr);
+    const double us = 0.5 * (L->u + R->u) + 0.5 * (fr - fl);
+    double rho, u, P;
+    const rstate_t *K = us >= 0.0 ? L : R;
+    if (us >= 0.0) {                                              /* x/t = 0 lies left of the contact */
+        if (p > L->P) {                                           /* left shock */
+            double sl = L->u - L->c * sqrt(gp1 / (2.0 * g) * p / L->P + gm1 / (2.0 * g));
+            if (0.0 <= sl) { rho = L->rho; u = L->u; P = L->P; }
+            else { rho = L->rho * ((p / L->P + gm1 / gp1) / (gm1 / gp1 * p / L->P + 1.0)); u = us; P = p; }
+        } else {                                                  /* left rarefaction */
+            double shl = L->u - L->c, stl = us - L->c * pow(p / L->P, z);
+            if (0.0 <= shl) { rho = L->rho; u = L->u; P = L->P; }
+            else if (0.0 >= stl) { rho = L->rho * pow(p / L->P, 1.0 / g); u = us; P = p; }
+            else {
+                double cf = 2.0 / gp1 + gm1 / (gp1 * L->c) * L->u;
+                rho = L->rho * pow(cf, 2.0 / gm1);
+                u = 2.0 / gp1 * (L->c + 0.5 * gm1 * L->u);
+                P = L->P * pow(cf, 2.0 * g / gm1);
+            }
+        }
+    } else {
+        if (p > R->P) {                                           /* right shock */
+            double sr = R->u + R->c * sqrt(gp1 / (2.0 * g) * p / R->P + gm1 / (2.0 * g));
+            if (0.0 >= sr) { rho = R->rho; u = R->u; P = R->P; }
+            else { rho = R->rho * ((p / R->P + gm1 / gp1) / (gm1 / gp1 * p / R->P + 1.0)); u = us; P = p; }
+        } else {                                                  /* right rarefaction */
+            double shr = R->u + R->c, str_ = us + R->c * pow(p / R->P, z);
+            if (0.0 >= shr) { rho = R->rho; u = R->u; P = R->P; }
+            else if (0.0 <= str_) { rho = R->rho * pow(p / R->P, 1.0 / g); u = us; P = p; }
+            else {
+                double cf = 2.0 / gp1 - gm1 / (gp1 * R->c) * R->u;
+                rho = R->rho * pow(cf, 2.0 / gm1);
+                u = 2.0 / gp1 * (-R->c + 0.5 * gm1 * R->u);
+                P = R->P * pow(cf, 2.0 * g / gm1);
+            }
+        }
+    }
+    const double E = P / gm1 + 0.5 * rho * (u * u + K->v * K->v + K->w * K->w);
+    F[0] = rho * u;
+    F[1] = rho * u * u + P;
+    F[2] = rho * u * K->v;
+    F[3] = rho * u * K->w;
+    F[4] = u * (E + P);
+    return 0;
+}
+
 /* flux through a face normal to axis d;  UL/UR full conserved states in x,y,z order */
 static void riemann(const ctx_t *c, int solver, int d, const double *UL, const double *UR, double *F,
                     orc_stats *st)
@@ -348,6 +438,11 @@ static void riemann(const ctx_t *c, int solver, int d, const double *UL, const d
         }
     } else if (solver == RSOLVER_HLLC) {
         solve_hllc(&L, &R, &r, ul, ur, f);
+    } else if (solver == RSOLVER_EXACT) {
+        if (solve_exact(c, &L, &R, f)) {
+            st->n_roe_fallback++;
+            solve_hlle(&L, &R, &r, ul, ur, f); /* R21: vacuum-generating data fall back to HLLE */
+        }
     } else {
         solve_hlle(&L, &R, &r, ul, ur, f);
     }
@@ -786,7 +881,7 @@ int oracle_fluid_advance(const double *in, double *out, double *flux_out, double
     if (!in || !out || n_groups < 0 || !(dt > 0.0) || !(dh > 0.0) || !(gamma > 1.0)) return -1;
     if (scheme != SCHEME_MHM && scheme != SCHEME_CTU) return -1;
     if (recon != RECON_PLM && recon != RECON_PPM) return -1;
-    if (riemann_solver < RSOLVER_ROE || riemann_solver > RSOLVER_HLLE) return -1;
+    if (riemann_solver < RSOLVER_ROE || riemann_solver > RSOLVER_EXACT) return -1;
     ctx_t c;
     make_ctx(&c, gamma, recon, opts);
     if (c.o.n_scalar < 0 || c.o.n_scalar > 1) return -1;

@@ -31,7 +31,7 @@ def test_exact_solver_matches_printed_sod_values():
     assert np.allclose(f, [gold["flux_mass"], gold["flux_momx"], 0, 0, gold["flux_ener"]], atol=2e-10)
 
 
-@pytest.mark.parametrize("solver", [1, 2, 3])
+@pytest.mark.parametrize("solver", [1, 2, 3, 4])
 def test_consistency_is_bitwise_for_identical_states(oracle_mod, solver):
     rng = np.random.default_rng(3)
     for _ in range(20):
@@ -67,7 +67,7 @@ def test_roe_identities(oracle_mod):
             assert np.all(np.abs(F - one_sided) <= 1e-13 * fscale)
 
 
-@pytest.mark.parametrize("solver", [1, 2, 3])
+@pytest.mark.parametrize("solver", [1, 2, 3, 4])
 def test_supersonic_upwinding(oracle_mod, solver):
     l, r = (1.0, 5.0, 0.3, -0.2, 1.0), (0.7, 4.5, -0.1, 0.4, 0.8)
     F, _ = oracle_mod.riemann(solver, 0, cons(*l), cons(*r), G)
@@ -125,7 +125,7 @@ def test_sod_flux_near_exact(oracle_mod, solver):
     assert F[2] == 0 and F[3] == 0
 
 
-@pytest.mark.parametrize("solver", [1, 2, 3])
+@pytest.mark.parametrize("solver", [1, 2, 3, 4])
 def test_axis_rotation(oracle_mod, solver):
     """Flux through a y- (z-) face = x-face flux of the cyclically permuted states, permuted back."""
     l, r = (1.0, 0.3, -0.4, 0.25, 0.9), (0.6, -0.2, 0.5, 0.1, 0.5)
@@ -141,7 +141,7 @@ def test_axis_rotation(oracle_mod, solver):
     assert np.array_equal(Fz[[0, 3, 1, 2, 4]], Fx)
 
 
-@pytest.mark.parametrize("solver", [1, 2, 3])
+@pytest.mark.parametrize("solver", [1, 2, 3, 4])
 def test_mirror_symmetry(oracle_mod, solver):
     l, r = (1.0, 0.3, -0.4, 0.25, 0.9), (0.6, -0.2, 0.5, 0.1, 0.5)
     F, _ = oracle_mod.riemann(solver, 0, cons(*l), cons(*r), G)
@@ -150,7 +150,7 @@ def test_mirror_symmetry(oracle_mod, solver):
     assert np.allclose(Fm * np.array([-1, 1, -1, -1, -1]), F, rtol=1e-13, atol=1e-15)
 
 
-@pytest.mark.parametrize("solver", [1, 2, 3])
+@pytest.mark.parametrize("solver", [1, 2, 3, 4])
 def test_scalar_flux_is_upwinded_on_mass_flux(oracle_mod, solver):
     UL = np.append(cons(1.0, 0.3, 0, 0, 0.9), 1.0 * 2.0)     # q_L = 2
     UR = np.append(cons(0.6, 0.2, 0, 0, 0.5), 0.6 * 5.0)     # q_R = 5
@@ -173,3 +173,30 @@ def test_remedy_i_roe_falls_back_to_hlle_on_strong_rarefaction(oracle_mod):
     # a mild problem must not take the fallback
     _, fb = oracle_mod.riemann(1, 0, cons(1, 0, 0, 0, 1), cons(0.125, 0, 0, 0, 0.1), G)
     assert fb == 0
+
+
+def test_exact_solver_of_the_oracle_matches_the_test_side_solver(oracle_mod):
+    """Solver 4 (Toro ch. 4) against tests/exact_riemann.py -- an independent implementation with another
+    first guess and a 1e-15 stopping rule, itself pinned to the printed Sod values: the printed Godunov flux of the Sod
+    problem to 1e-9, and the flux of random subsonic / supersonic / strong-shock / strong-rarefaction data, transverse
+    components included, to 1e-9 of its scale (the oracle stops one Newton step after a 1e-6 change)."""
+    gold = load_golden("sod_exact.txt")
+    F, fb = oracle_mod.riemann(4, 0, cons(1, 0, 0, 0, 1), cons(0.125, 0, 0, 0, 0.1), G)
+    assert fb == 0
+    assert np.allclose(F, [gold["flux_mass"], gold["flux_momx"], 0, 0, gold["flux_ener"]], atol=1e-9)
+    rng = np.random.default_rng(11)
+    for k in range(300):
+        rl, rr = rng.uniform(0.05, 5, size=2)
+        pl, pr = 10 ** rng.uniform(-2, 2, size=2)
+        ul, ur = rng.normal(size=2) * rng.choice([0.3, 3.0])
+        vl, wl, vr, wr = rng.normal(size=4)
+        if 2 * (math.sqrt(G * pl / rl) + math.sqrt(G * pr / rr)) / (G - 1) <= ur - ul:
+            continue                                      # vacuum: covered below
+        F, fb = oracle_mod.riemann(4, 0, cons(rl, ul, vl, wl, pl), cons(rr, ur, vr, wr, pr), G)
+        Fe = er.godunov_flux(rl, ul, vl, wl, pl, rr, ur, vr, wr, pr, G)
+        assert fb == 0
+        assert np.abs(F - Fe).max() <= 1e-9 * (np.abs(Fe).max() + 1.0), (k, F, Fe)
+    # data that generate vacuum (Toro eq. 4.40) are reported and handed to HLLE
+    F, fb = oracle_mod.riemann(4, 0, cons(1, -20, 0, 0, 0.4), cons(1, 20, 0, 0, 0.4), G)
+    Fh, _ = oracle_mod.riemann(3, 0, cons(1, -20, 0, 0, 0.4), cons(1, 20, 0, 0, 0.4), G)
+    assert fb == 1 and np.array_equal(F, Fh)

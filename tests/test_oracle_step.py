@@ -13,7 +13,8 @@ from paper_1712_07070_b200 import inputs
 MHM, CTU = 1, 2
 PLM, PPM = 1, 2
 ROE, HLLC, HLLE = 1, 2, 3
-COMBOS = list(itertools.product((MHM, CTU), (PLM, PPM), (ROE, HLLC, HLLE)))
+EXACT = 4
+COMBOS = list(itertools.product((MHM, CTU), (PLM, PPM), (ROE, HLLC, HLLE))) + [(MHM, PLM, EXACT), (CTU, PPM, EXACT)]
 G53 = 5.0 / 3.0
 
 
