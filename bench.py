@@ -27,7 +27,7 @@ sys.path.insert(0, ROOT)
 
 SCHEMES = {"mhm": 1, "ctu": 2}
 RECONS = {"plm": 1, "ppm": 2}
-SOLVERS = {"roe": 1, "hllc": 2, "hlle": 3}
+SOLVERS = {"roe": 1, "hllc": 2, "hlle": 3, "exact": 4}
 CELLS = 4096
 
 # algorithmic HBM bytes per cell update: padded read + interior write + 9 flux planes

@@ -39,7 +39,9 @@ extern "C" {
 
 enum { GAMER_MHM = 1, GAMER_CTU = 2 };                      /* scheme   (L90)            */
 enum { GAMER_PLM = 1, GAMER_PPM = 2 };                      /* recon    (L94)            */
-enum { GAMER_ROE = 1, GAMER_HLLC = 2, GAMER_HLLE = 3 };     /* riemann  (L94)            */
+enum { GAMER_ROE = 1, GAMER_HLLC = 2, GAMER_HLLE = 3,
+       GAMER_EXACT = 4 };   /* riemann (L94); EXACT = Toro (2009) ch. 4, iterative: Newton on the pressure function
+                               from the two-rarefaction guess, vacuum-generating data handled by HLLE */
 enum { GAMER_FP32 = 4, GAMER_FP64 = 8 };                    /* precision = sizeof(real), L244 */
 enum { GAMER_LIMITER_GMINMOD = 1, GAMER_LIMITER_VANLEER = 2, GAMER_LIMITER_VANALBADA = 3 }; /* L94 */
 

@@ -11,7 +11,7 @@ import torch
 
 MHM, CTU = 1, 2
 PLM, PPM = 1, 2
-ROE, HLLC, HLLE = 1, 2, 3
+ROE, HLLC, HLLE, EXACT = 1, 2, 3, 4
 FP32, FP64 = 4, 8
 GMINMOD, VANLEER, VANALBADA = 1, 2, 3
 BC_PERIODIC, BC_OUTFLOW, BC_REFLECTING = 0, 1, 2

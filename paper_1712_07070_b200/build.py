@@ -39,7 +39,7 @@ def build(force=False, verbose=False):
     jobs = []
     for s in (1, 2):
         for r in (1, 2):
-            for v in (1, 2, 3):
+            for v in (1, 2, 3, 4):
                 o = os.path.join(OBJ, "inst_%d_%d_%d.o" % (s, r, v))
                 cmd = [NVCC, *FLAGS, "-DG_SCHEME=%d" % s, "-DG_RECON=%d" % r, "-DG_SOLVER=%d" % v]
                 if have_ctu:

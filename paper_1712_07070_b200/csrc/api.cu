@@ -9,13 +9,15 @@
 
 namespace gamer {
 #define G_DECL(s, r, v) cudaError_t gamer_launch_##s##_##r##_##v(int, int, int, const void*, cudaStream_t, int*);
-G_DECL(1, 1, 1) G_DECL(1, 1, 2) G_DECL(1, 1, 3) G_DECL(1, 2, 1) G_DECL(1, 2, 2) G_DECL(1, 2, 3)
-G_DECL(2, 1, 1) G_DECL(2, 1, 2) G_DECL(2, 1, 3) G_DECL(2, 2, 1) G_DECL(2, 2, 2) G_DECL(2, 2, 3)
+G_DECL(1, 1, 1) G_DECL(1, 1, 2) G_DECL(1, 1, 3) G_DECL(1, 1, 4) G_DECL(1, 2, 1) G_DECL(1, 2, 2) G_DECL(1, 2, 3) G_DECL(1, 2, 4)
+G_DECL(2, 1, 1) G_DECL(2, 1, 2) G_DECL(2, 1, 3) G_DECL(2, 1, 4) G_DECL(2, 2, 1) G_DECL(2, 2, 2) G_DECL(2, 2, 3) G_DECL(2, 2, 4)
 #undef G_DECL
 typedef cudaError_t (*launch_fn)(int, int, int, const void*, cudaStream_t, int*);
-static const launch_fn TABLE[2][2][3] = {
-    {{gamer_launch_1_1_1, gamer_launch_1_1_2, gamer_launch_1_1_3}, {gamer_launch_1_2_1, gamer_launch_1_2_2, gamer_launch_1_2_3}},
-    {{gamer_launch_2_1_1, gamer_launch_2_1_2, gamer_launch_2_1_3}, {gamer_launch_2_2_1, gamer_launch_2_2_2, gamer_launch_2_2_3}}};
+static const launch_fn TABLE[2][2][4] = {
+    {{gamer_launch_1_1_1, gamer_launch_1_1_2, gamer_launch_1_1_3, gamer_launch_1_1_4},
+     {gamer_launch_1_2_1, gamer_launch_1_2_2, gamer_launch_1_2_3, gamer_launch_1_2_4}},
+    {{gamer_launch_2_1_1, gamer_launch_2_1_2, gamer_launch_2_1_3, gamer_launch_2_1_4},
+     {gamer_launch_2_2_1, gamer_launch_2_2_2, gamer_launch_2_2_3, gamer_launch_2_2_4}}};
 static std::atomic<long long> g_launches{0};
 }  // namespace gamer
 
@@ -29,7 +31,7 @@ static int check_common(const void* in, const void* out, int64_t n_groups, doubl
     if (!(dh > 0.0) || !std::isfinite(dh) || !(gamma > 1.0) || !std::isfinite(gamma)) return GAMER_EINVAL;
     if (scheme != GAMER_MHM && scheme != GAMER_CTU) return GAMER_EINVAL;
     if (recon != GAMER_PLM && recon != GAMER_PPM) return GAMER_EINVAL;
-    if (riemann < GAMER_ROE || riemann > GAMER_HLLE) return GAMER_EINVAL;
+    if (riemann < GAMER_ROE || riemann > GAMER_EXACT) return GAMER_EINVAL;
     if (precision != GAMER_FP32 && precision != GAMER_FP64) return GAMER_EINVAL;
     if (!aligned16(in) || !aligned16(out)) return GAMER_EINVAL;
     return GAMER_OK;

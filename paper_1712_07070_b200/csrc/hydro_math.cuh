@@ -13,7 +13,7 @@ namespace gamer {
 
 enum { MHM = 1, CTU = 2 };
 enum { PLM = 1, PPM = 2 };
-enum { ROE = 1, HLLC = 2, HLLE = 3 };
+enum { ROE = 1, HLLC = 2, HLLE = 3, EXACT = 4 };
 enum { LIM_GMINMOD = 1, LIM_VANLEER = 2, LIM_VANALBADA = 3 };
 
 // ---------------------------------------------------------------------------------------------

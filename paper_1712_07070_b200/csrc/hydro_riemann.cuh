@@ -138,6 +138,78 @@ __device__ __forceinline__ bool solve_roe(const Side<T>& L, const Side<T>& R, co
     return false;
 }
 
+// Exact solver ("exact solver based on Toro (2009)", reading R21): star pressure by Newton-Raphson on
+// Toro's pressure function from the two-rarefaction guess, until a relative change below 1e-6 plus one more step
+// (at most 30), sampling at x/t = 0, transverse velocities from the side of the contact.  Returns true when the
+// data generate vacuum (Toro eq. 4.40); the caller then uses HLLE.  IEEE division / sqrt / pow throughout: this
+// solver is iterative and not on the fast path.
+template <typename T>
+__device__ __forceinline__ void pressure_fn(T p, T rho, T pk, T ck, T gamma, T& f, T& df) {
+    if (p > pk) {
+        const T A = T(2) / ((gamma + T(1)) * rho), B = (gamma - T(1)) / (gamma + T(1)) * pk;
+        const T q = ::sqrt(A / (p + B));
+        f = (p - pk) * q;
+        df = q * (T(1) - T(0.5) * (p - pk) / (B + p));
+    } else {
+        const T pr = p / pk;
+        f = T(2) * ck / (gamma - T(1)) * (Ops<T>::pow(pr, (gamma - T(1)) / (T(2) * gamma)) - T(1));
+        df = Ops<T>::pow(pr, -(gamma + T(1)) / (T(2) * gamma)) / (rho * ck);
+    }
+}
+
+template <typename T>
+__device__ __noinline__ bool solve_exact(const Side<T>& L, const Side<T>& R, T* F, const Phys<T>& ph) {
+    const T g = ph.gamma, gm1 = g - T(1), gp1 = g + T(1), z = gm1 / (T(2) * g);
+    const T cl = ::sqrt(g * L.P / L.rho), cr = ::sqrt(g * R.P / R.rho);
+    const T du = R.u - L.u;
+    const T num = cl + cr - T(0.5) * gm1 * du;
+    if (!(num > T(0))) return true;
+    const T p0 = Ops<T>::pow(num / (cl / Ops<T>::pow(L.P, z) + cr / Ops<T>::pow(R.P, z)), T(1) / z);
+    T p = p0, fl, dfl, fr, dfr;
+    bool extra = false;
+    for (int it = 0; it < 30; ++it) {
+        pressure_fn(p, L.rho, L.P, cl, g, fl, dfl);
+        pressure_fn(p, R.rho, R.P, cr, g, fr, dfr);
+        T pn = p - (fl + fr + du) / (dfl + dfr);
+        if (!(pn > T(0))) pn = T(1e-6) * p0;
+        const T change = T(2) * Ops<T>::abs(pn - p) / (pn + p);
+        p = pn;
+        if (extra) break;
+        if (change < T(1e-6)) extra = true;
+    }
+    pressure_fn(p, L.rho, L.P, cl, g, fl, dfl);
+    pressure_fn(p, R.rho, R.P, cr, g, fr, dfr);
+    const T us = T(0.5) * (L.u + R.u) + T(0.5) * (fr - fl);
+    T rho, u, P;
+    const bool left = us >= T(0);
+    const Side<T>& K = left ? L : R;
+    const T ck = left ? cl : cr;
+    const T sg = left ? T(1) : T(-1);          // mirror the right-hand formulas onto the left-hand ones
+    const T uk = sg * K.u, usk = sg * us;
+    if (p > K.P) {                             // shock on this side
+        const T sk = uk - ck * ::sqrt(gp1 / (T(2) * g) * p / K.P + gm1 / (T(2) * g));
+        if (T(0) <= sk) { rho = K.rho; u = K.u; P = K.P; }
+        else { rho = K.rho * ((p / K.P + gm1 / gp1) / (gm1 / gp1 * p / K.P + T(1))); u = us; P = p; }
+    } else {                                   // rarefaction on this side
+        const T sh = uk - ck, st = usk - ck * Ops<T>::pow(p / K.P, z);
+        if (T(0) <= sh) { rho = K.rho; u = K.u; P = K.P; }
+        else if (T(0) >= st) { rho = K.rho * Ops<T>::pow(p / K.P, T(1) / g); u = us; P = p; }
+        else {
+            const T cf = T(2) / gp1 + gm1 / (gp1 * ck) * uk;
+            rho = K.rho * Ops<T>::pow(cf, T(2) / gm1);
+            u = sg * (T(2) / gp1 * (ck + T(0.5) * gm1 * uk));
+            P = K.P * Ops<T>::pow(cf, T(2) * g / gm1);
+        }
+    }
+    const T E = P / gm1 + T(0.5) * rho * (u * u + K.v * K.v + K.w * K.w);
+    F[0] = rho * u;
+    F[1] = rho * u * u + P;
+    F[2] = rho * u * K.v;
+    F[3] = rho * u * K.w;
+    F[4] = u * (E + P);
+    return false;
+}
+
 // Flux through a face from rotated primitive states.  Returns true if Roe fell back to HLLE.
 template <typename T, int SOLVER, int NV>
 __device__ __forceinline__ bool riemann_flux(const T* WL, const T* WR, T* F, const Phys<T>& ph) {
@@ -152,6 +224,9 @@ __device__ __forceinline__ bool riemann_flux(const T* WL, const T* WR, T* F, con
         if (fb) solve_hlle(L, R, r, F, ph);
     } else if (SOLVER == HLLC) {
         solve_hllc(L, R, r, F, ph);
+    } else if (SOLVER == EXACT) {
+        fb = solve_exact(L, R, F, ph);
+        if (fb) solve_hlle(L, R, r, F, ph);
     } else {
         solve_hlle(L, R, r, F, ph);
     }

@@ -54,7 +54,7 @@ def test_argument_validation_needs_no_gpu(built_lib):
     assert L.gamer_fluid_advance(ok[0], ok[1], None, 1, 0.1, 0.1, 1.0, 1, 1, 1, 4) == -1
     assert L.gamer_fluid_advance(ok[0], ok[1], None, 1, 0.1, 0.1, 1.4, 3, 1, 1, 4) == -1
     assert L.gamer_fluid_advance(ok[0], ok[1], None, 1, 0.1, 0.1, 1.4, 1, 0, 1, 4) == -1
-    assert L.gamer_fluid_advance(ok[0], ok[1], None, 1, 0.1, 0.1, 1.4, 1, 1, 4, 4) == -1
+    assert L.gamer_fluid_advance(ok[0], ok[1], None, 1, 0.1, 0.1, 1.4, 1, 1, 5, 4) == -1
     assert L.gamer_fluid_advance(ok[0], ok[1], None, 1, 0.1, 0.1, 1.4, 1, 1, 1, 2) == -1
     assert L.gamer_fluid_advance(vp(4100), ok[1], None, 1, 0.1, 0.1, 1.4, 1, 1, 1, 4) == -1     # misaligned
     # fused-refresh entry: no neighbour table, remedy (ii) (needs the padded slab), in-place update

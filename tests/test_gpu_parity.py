@@ -17,7 +17,8 @@ pytestmark = pytest.mark.gpu
 G53 = 5.0 / 3.0
 TOL = {torch.float64: 1e-12, torch.float32: 1e-5}
 SCHEMES = [gb.MHM, gb.CTU]
-COMBOS = list(itertools.product(SCHEMES, (gb.PLM, gb.PPM), (gb.ROE, gb.HLLC, gb.HLLE)))
+COMBOS = list(itertools.product(SCHEMES, (gb.PLM, gb.PPM), (gb.ROE, gb.HLLC, gb.HLLE))) + \
+    [(gb.MHM, gb.PLM, gb.EXACT), (gb.CTU, gb.PPM, gb.EXACT), (gb.MHM, gb.PPM, gb.EXACT), (gb.CTU, gb.PLM, gb.EXACT)]
 
 
 @pytest.fixture(scope="module")
