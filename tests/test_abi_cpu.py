@@ -57,6 +57,9 @@ def test_argument_validation_needs_no_gpu(built_lib):
     assert L.gamer_fluid_advance(ok[0], ok[1], None, 1, 0.1, 0.1, 1.4, 1, 1, 5, 4) == -1
     assert L.gamer_fluid_advance(ok[0], ok[1], None, 1, 0.1, 0.1, 1.4, 1, 1, 1, 2) == -1
     assert L.gamer_fluid_advance(vp(4100), ok[1], None, 1, 0.1, 0.1, 1.4, 1, 1, 1, 4) == -1     # misaligned
+    # sizes beyond what the launch grid / 32-bit offsets cover are refused, not truncated
+    assert L.gamer_fluid_advance(ok[0], ok[1], None, 1 << 30, 0.1, 0.1, 1.4, 1, 1, 1, 4) == -2
+    assert L.gamer_fluid_advance(ok[0], ok[1], None, 0, 0.1, 0.1, 1.4, 1, 1, 1, 4) == 0          # empty batch: no-op
     # fused-refresh entry: no neighbour table, remedy (ii) (needs the padded slab), in-place update
     from paper_1712_07070_b200 import binding as gb
     L.gamer_fluid_advance_resident.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, ci, ci, ctypes.POINTER(gb.gamer_opts)]
