@@ -30,6 +30,7 @@ class Opts(ctypes.Structure):
         ("min_pres", ctypes.c_double),
         ("min_temp", ctypes.c_double),
         ("remedy_first_order", ctypes.c_int),
+        ("char_limiting", ctypes.c_int),
     ]
 
 
@@ -57,9 +58,9 @@ def lib():
 
 
 def make_opts(limiter=GMINMOD, theta=0.0, n_scalar=0, dual_energy=False, de_xi=1e-2,
-              min_dens=0.0, min_pres=0.0, min_temp=0.0, remedy_first_order=False):
+              min_dens=0.0, min_pres=0.0, min_temp=0.0, remedy_first_order=False, char_limiting=False):
     return Opts(limiter, theta, n_scalar, int(dual_energy), de_xi, min_dens, min_pres, min_temp,
-                int(remedy_first_order))
+                int(remedy_first_order), int(char_limiting))
 
 
 def _p(a):
@@ -222,4 +223,13 @@ def fill_ghosts(field, bc=((PERIODIC, PERIODIC),) * 3):
                 blk[2][:, flip[1][by], :] *= -1.0
                 blk[3][flip[2][bz], :, :] *= -1.0
                 out[(bz * gy + by) * gx + bx] = blk
+    return out
+
+
+def char_slope(Wl, Wc, Wr, gamma, limiter=GMINMOD, theta=1.0):
+    """Characteristic-limited slope vector of one cell (rotated primitive states of cells j-1, j, j+1)."""
+    Wl, Wc, Wr = _c64(Wl), _c64(Wc), _c64(Wr)
+    out = np.zeros_like(Wc)
+    lib().oracle_char_slope(int(limiter), ctypes.c_double(theta), ctypes.c_double(gamma), int(Wc.shape[0] - 5),
+                            _p(Wl), _p(Wc), _p(Wr), _p(out))
     return out

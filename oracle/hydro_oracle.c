@@ -64,6 +64,7 @@ typedef struct {
     double de_xi;              /* switch E_the/E_kin < xi (L100)                         */
     double min_dens, min_pres, min_temp;   /* floors; 0 = off                            */
     int    remedy_first_order; /* remedy (ii), L105                                      */
+    int    char_limiting;      /* 0: slopes limited in primitive variables; 1: in characteristic ones (L94) */
 } orc_opts;
 
 typedef struct {
@@ -601,10 +602,77 @@ typedef struct {
 
 static const int STEP[3] = {1, NP, NP * NP};
 
+/* Limited slope vector of one cell in CHARACTERISTIC variables (L94 "applied to either primitive or characteristic
+ * variables"; Stone et al. 2008 sect. 4.2.1, reading R22): the left and right differences of the rotated primitive
+ * state are projected on the left eigenvectors evaluated at the cell itself (project), each characteristic amplitude
+ * is limited by the same limiter as in the primitive case, and the limited amplitudes are multiplied back by the
+ * right eigenvectors (add_wave).  Wl, Wc, Wr: rotated (rho, vn, vt1, vt2, P [, q]) of cells j-1, j, j+1. */
+static void add_wave(double *T, int alpha, double amp, double rho, double cs);
+static void project(const double *dW, double rho, double cs, int nv, double *amp);
+
+static void char_slope(const ctx_t *c, const double *Wl, const double *Wc, const double *Wr, double *slope)
+{
+    int nv = c->nv;
+    double dL[NVMAX], dR[NVMAX], aL[NVMAX], aR[NVMAX];
+    double rho = Wc[0], cs = sqrt(c->gamma * Wc[4] / Wc[0]);
+    for (int v = 0; v < nv; ++v) {
+        dL[v] = Wc[v] - Wl[v];
+        dR[v] = Wr[v] - Wc[v];
+        slope[v] = 0.0;
+    }
+    project(dL, rho, cs, nv, aL);
+    project(dR, rho, cs, nv, aR);
+    for (int a = 0; a < nv; ++a) add_wave(slope, a, limited_slope(c, aL[a], aR[a]), rho, cs);
+}
+
 static void gather_face_values(const ctx_t *c, int recon, const double *W, int n, int d, double *wm,
                                double *wp)
 {
     int nv = c->nv;
+    if (c->o.char_limiting) {
+        /* rotated copies of cells n-2 .. n+2 along d (PLM uses n-1 .. n+1 only) */
+        int cn = 1 + d, c1 = 1 + (d + 1) % 3, c2 = 1 + (d + 2) % 3;
+        int R = recon == RECON_PPM ? 2 : 1;
+        double Wr[5][NVMAX], sl[3][NVMAX], rm[NVMAX], rp[NVMAX];
+        for (int m = -R; m <= R; ++m) {
+            const double *q = W + n + m * STEP[d];
+            Wr[m + 2][0] = q[0];
+            Wr[m + 2][1] = q[(size_t)cn * NPC];
+            Wr[m + 2][2] = q[(size_t)c1 * NPC];
+            Wr[m + 2][3] = q[(size_t)c2 * NPC];
+            Wr[m + 2][4] = q[(size_t)4 * NPC];
+            if (nv > 5) Wr[m + 2][5] = q[(size_t)5 * NPC];
+        }
+        if (recon == RECON_PLM) {
+            char_slope(c, Wr[1], Wr[2], Wr[3], sl[1]);
+            for (int v = 0; v < nv; ++v) {
+                rm[v] = Wr[2][v] - 0.5 * sl[1][v];
+                rp[v] = Wr[2][v] + 0.5 * sl[1][v];
+            }
+        } else {
+            for (int j = 0; j < 3; ++j) char_slope(c, Wr[j], Wr[j + 1], Wr[j + 2], sl[j]);   /* cells n-1, n, n+1 */
+            for (int v = 0; v < nv; ++v) {
+                double q0 = Wr[2][v];
+                double m = 0.5 * (Wr[1][v] + q0) - (sl[1][v] - sl[0][v]) / 6.0;
+                double p = 0.5 * (q0 + Wr[3][v]) - (sl[2][v] - sl[1][v]) / 6.0;
+                if ((p - q0) * (q0 - m) <= 0.0) {
+                    m = q0;
+                    p = q0;
+                } else {
+                    double D = p - m, C = q0 - 0.5 * (m + p);
+                    if (D * C > D * D / 6.0) m = 3.0 * q0 - 2.0 * p;
+                    else if (D * C < -D * D / 6.0) p = 3.0 * q0 - 2.0 * m;
+                }
+                rm[v] = m;
+                rp[v] = p;
+            }
+        }
+        /* back to the natural component order */
+        wm[0] = rm[0]; wm[cn] = rm[1]; wm[c1] = rm[2]; wm[c2] = rm[3]; wm[4] = rm[4];
+        wp[0] = rp[0]; wp[cn] = rp[1]; wp[c1] = rp[2]; wp[c2] = rp[3]; wp[4] = rp[4];
+        if (nv > 5) { wm[5] = rm[5]; wp[5] = rp[5]; }
+        return;
+    }
     for (int v = 0; v < nv; ++v) {
         double w[5];
         const double *q = W + (size_t)v * NPC + n;
@@ -1047,6 +1115,22 @@ int oracle_close_cell(double *U, double gamma, const orc_opts *opts, orc_stats *
     if (floors_set(&c)) floor_cons(&c, U, &st);
     if (st_out) *st_out = st;
     return is_physical(&c, U);
+}
+
+/* test hook: characteristic-limited slope vector of one cell from the rotated primitive states of cells j-1, j, j+1 */
+void oracle_char_slope(int limiter, double theta, double gamma, int n_scalar, const double *Wl, const double *Wc,
+                       const double *Wr, double *slope)
+{
+    orc_opts o;
+    memset(&o, 0, sizeof(o));
+    o.limiter = limiter;
+    o.theta = theta;
+    o.n_scalar = n_scalar;
+    ctx_t c;
+    make_ctx(&c, gamma, RECON_PLM, &o);
+    c.o.limiter = limiter;
+    c.o.theta = theta;
+    char_slope(&c, Wl, Wc, Wr, slope);
 }
 
 int oracle_sizeof_opts(void) { return (int)sizeof(orc_opts); }

@@ -113,3 +113,55 @@ def test_single_wave_tracing_is_domain_of_dependence_average(oracle_mod, recon, 
         exp_m = W + r * (mean(0.0, ym) if ym > 0 else prof(0.0))
         assert np.allclose(tp, exp_p, atol=1e-10), (a, tp, exp_p)
         assert np.allclose(tm, exp_m, atol=1e-10), (a, tm, exp_m)
+
+
+def _eig_lr(rho, cs):
+    """Left (rows) and right (columns) eigenvectors of the primitive-variable Euler system along n, written out from
+    the literature (e.g. Stone et al. 2008, appendix A) -- independent of the oracle's project / add_wave."""
+    L = np.array([[0, -rho / (2 * cs), 0, 0, 1 / (2 * cs * cs)],
+                  [1, 0, 0, 0, -1 / (cs * cs)],
+                  [0, 0, 1, 0, 0],
+                  [0, 0, 0, 1, 0],
+                  [0, rho / (2 * cs), 0, 0, 1 / (2 * cs * cs)]])
+    R = np.array([[1, 1, 0, 0, 1],
+                  [-cs / rho, 0, 0, 0, cs / rho],
+                  [0, 0, 1, 0, 0],
+                  [0, 0, 0, 1, 0],
+                  [cs * cs, 0, 0, 0, cs * cs]])
+    return L, R
+
+
+def test_characteristic_limiting_is_R_minmod_L(oracle_mod):
+    """Reading R22 (Stone et al. 2008 sect. 4.2.1): slope = R . limiter(L . dW_left, L . dW_right) with the
+    eigenvectors of the cell itself.  Pins: L R = 1; random data against the matrix formula; linear data are kept
+    exactly; a jump carried by one wave only (a contact: only rho differs) is limited like the scalar; and a case
+    where every primitive difference keeps its sign but one characteristic amplitude changes sign, so that the
+    primitive- and characteristic-limited slopes differ."""
+    g = 1.4
+    rng = np.random.default_rng(8)
+    for _ in range(50):
+        Wc = np.array([rng.uniform(0.2, 3), *rng.normal(size=3), rng.uniform(0.2, 3)])
+        Wl = Wc + 0.2 * rng.normal(size=5) * np.array([0.2, 1, 1, 1, 0.2])
+        Wr = Wc + 0.2 * rng.normal(size=5) * np.array([0.2, 1, 1, 1, 0.2])
+        cs = math.sqrt(g * Wc[4] / Wc[0])
+        L, R = _eig_lr(Wc[0], cs)
+        assert np.abs(L @ R - np.eye(5)).max() < 1e-14
+        aL, aR = L @ (Wc - Wl), L @ (Wr - Wc)
+        lim = np.array([oracle_mod.limited_slope(oracle_mod.GMINMOD, 1.0, a, b) for a, b in zip(aL, aR)])
+        got = oracle_mod.char_slope(Wl, Wc, Wr, g)
+        assert np.abs(got - R @ lim).max() <= 1e-13 * (np.abs(R @ lim).max() + 1.0)
+    Wc = np.array([1.3, 0.4, -0.2, 0.7, 2.1])
+    d = np.array([0.05, -0.02, 0.03, 0.01, 0.08])
+    assert np.abs(oracle_mod.char_slope(Wc - d, Wc, Wc + d, g) - d).max() <= 1e-15          # linear data
+    sl = oracle_mod.char_slope(Wc - np.array([0.3, 0, 0, 0, 0]), Wc, Wc + np.array([0.1, 0, 0, 0, 0]), g)
+    assert np.allclose(sl, [0.1, 0, 0, 0, 0], atol=1e-16)                                   # contact only
+    # all primitive differences positive on both sides, but the (v - c) amplitude changes sign
+    cs = math.sqrt(g * Wc[4] / Wc[0])
+    dl = np.array([0.10, 0.30, 0.0, 0.0, 0.10])
+    dr = np.array([0.10, 0.02, 0.0, 0.0, 0.10])
+    L, R = _eig_lr(Wc[0], cs)
+    assert (L @ dl)[0] * (L @ dr)[0] < 0 and (dl[[0, 1, 4]] > 0).all() and (dr[[0, 1, 4]] > 0).all()
+    ch = oracle_mod.char_slope(Wc - dl, Wc, Wc + dr, g)
+    pr = np.array([oracle_mod.limited_slope(oracle_mod.GMINMOD, 1.0, a, b) for a, b in zip(dl, dr)])
+    assert np.abs(ch - pr).max() > 1e-3
+    assert abs((L @ ch)[0]) <= 1e-15                                                         # that wave got no slope
