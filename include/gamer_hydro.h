@@ -69,6 +69,8 @@ typedef struct gamer_opts {
                                      the caller applies remedy (iv) (retry with 0.8 dt, L107)       */
     int32_t* diag_out;            /* nullable device int[4], set by the call: {remedy (i) faces,
                                      reverted predictor states, remedy (ii) cells, dual-energy fixes} */
+    int      char_limiting;       /* 1: slopes limited in characteristic variables (L94): R . limiter(L dW-, L dW+)
+                                     with the eigenvectors of the cell; 0: in primitive variables (default)    */
 } gamer_opts;
 
 /* One step for n_groups patch groups.  flux_out may be NULL.  n_groups == 0 is a successful no-op.

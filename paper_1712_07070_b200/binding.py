@@ -43,6 +43,7 @@ class gamer_opts(ctypes.Structure):
         ("group_speed_out", ctypes.c_void_p),
         ("n_unphysical_out", ctypes.c_void_p),
         ("diag_out", ctypes.c_void_p),
+        ("char_limiting", ctypes.c_int),
     ]
 
 
@@ -115,7 +116,7 @@ def _stream_handle(stream=None):
 
 def make_opts(stream=None, limiter=0, minmod_theta=0.0, n_scalar=0, dual_energy=False, de_xi=0.0, min_dens=0.0,
               min_pres=0.0, min_temp=0.0, remedy_first_order=False, dt_dev=None, group_speed_out=None,
-              n_unphysical_out=None, diag_out=None, on_device=True):
+              n_unphysical_out=None, diag_out=None, on_device=True, char_limiting=False):
     o = gamer_opts()
     o.stream = _stream_handle(stream) if on_device else None
     o.limiter, o.minmod_theta, o.n_scalar = int(limiter), float(minmod_theta), int(n_scalar)
@@ -126,6 +127,7 @@ def make_opts(stream=None, limiter=0, minmod_theta=0.0, n_scalar=0, dual_energy=
     o.group_speed_out = _ptr(group_speed_out)
     o.n_unphysical_out = _ptr(n_unphysical_out)
     o.diag_out = _ptr(diag_out)
+    o.char_limiting = int(bool(char_limiting))
     return o
 
 

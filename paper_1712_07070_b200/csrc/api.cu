@@ -60,14 +60,14 @@ static int advance_typed(const void* in, void* out, void* flux_out, int64_t n_gr
         if (o->minmod_theta > 0.0) a.theta = o->minmod_theta;
         if (o->de_xi > 0.0) a.xi = o->de_xi;
         a.min_dens = o->min_dens; a.min_pres = o->min_pres; a.min_temp = o->min_temp;
-        a.dual = o->dual_energy; a.remedy2 = o->remedy_first_order;
+        a.dual = o->dual_energy; a.remedy2 = o->remedy_first_order; a.char_limit = o->char_limiting ? 1 : 0;
         a.dt_dev = o->dt_dev;
         a.speed = static_cast<T*>(o->group_speed_out);
         a.n_unphys = o->n_unphysical_out;
         a.diag = o->diag_out;
         nsc = o->n_scalar;
         const bool custom_theta = a.theta != (recon == GAMER_PPM ? 2.0 : 1.0);   // fast kernels fix theta at compile time
-        ext = (nsc || a.dual || a.remedy2 || a.limiter != LIM_GMINMOD || custom_theta || a.min_dens > 0 || a.min_pres > 0 ||
+        ext = (nsc || a.dual || a.remedy2 || a.limiter != LIM_GMINMOD || custom_theta || a.char_limit || a.min_dens > 0 || a.min_pres > 0 ||
                a.min_temp > 0 || a.n_unphys || a.diag) ? 1 : 0;
     }
     if (a.n_unphys && cudaMemsetAsync(a.n_unphys, 0, sizeof(int), st) != cudaSuccess) return GAMER_ECUDA;

@@ -69,27 +69,41 @@ __device__ __forceinline__ void ctu_trace_dir(const T* const* Pz, int t, T* tcur
     constexpr int cn = 1 + D, c1 = 1 + (D + 1) % 3, c2 = 1 + (D + 2) % 3;
     const int ej = t / EW, ei = t - ej * EW;
     const int c = (ej + 2) * NP + (ei + 2);
-    T wm[NV], wp[NV], Wc[NV];
-#pragma unroll
-    for (int v = 0; v < NV; ++v) {
-        const T* q = Pz[R] + v * G::PLN + c;
-        Wc[v] = q[0];
-        if (D == 0) face_values<T, RECON, EXT, fixed_theta(EXT, RECON)>(q, 1, wm[v], wp[v], ph);
-        else if (D == 1) face_values<T, RECON, EXT, fixed_theta(EXT, RECON)>(q, NP, wm[v], wp[v], ph);
-        else {
-            const int o = v * G::PLN + c;
-            if (RECON == PPM)
-                face_values5<T, RECON, EXT>(Pz[0][o], Pz[R - 1][o], Pz[R][o], Pz[R + 1][o], Pz[2 * R][o], wm[v], wp[v], ph);
-            else
-                face_values5<T, RECON, EXT>(T(0), Pz[R - 1][o], Pz[R][o], Pz[R + 1][o], T(0), wm[v], wp[v], ph);
-        }
-    }
-    // rotate so that the traced axis is "n"
     T Wr[NV], rm[NV], rp[NV], tm[NV], tp[NV];
-    Wr[0] = Wc[0]; Wr[1] = Wc[cn]; Wr[2] = Wc[c1]; Wr[3] = Wc[c2]; Wr[4] = Wc[4];
-    rm[0] = wm[0]; rm[1] = wm[cn]; rm[2] = wm[c1]; rm[3] = wm[c2]; rm[4] = wm[4];
-    rp[0] = wp[0]; rp[1] = wp[cn]; rp[2] = wp[c1]; rp[3] = wp[c2]; rp[4] = wp[4];
-    if (NV > 5) { Wr[NV - 1] = Wc[NV - 1]; rm[NV - 1] = wm[NV - 1]; rp[NV - 1] = wp[NV - 1]; }
+    if (EXT && ph.char_limit) {      // slopes limited in characteristic variables (R22): all variables together
+        T W5[5][NV];
+#pragma unroll
+        for (int m = -R; m <= R; ++m) {
+            const T* q = (D == 2) ? Pz[R + m] + c : Pz[R] + c + m * (D == 0 ? 1 : NP);
+            W5[m + 2][0] = q[0]; W5[m + 2][1] = q[cn * G::PLN]; W5[m + 2][2] = q[c1 * G::PLN]; W5[m + 2][3] = q[c2 * G::PLN];
+            W5[m + 2][4] = q[4 * G::PLN];
+            if (NV > 5) W5[m + 2][NV - 1] = q[(NV - 1) * G::PLN];
+        }
+#pragma unroll
+        for (int k = 0; k < NV; ++k) Wr[k] = W5[2][k];
+        face_values_char<T, RECON, NV, EXT>(W5, rm, rp, ph);
+    } else {
+        T wm[NV], wp[NV], Wc[NV];
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+            const T* q = Pz[R] + v * G::PLN + c;
+            Wc[v] = q[0];
+            if (D == 0) face_values<T, RECON, EXT, fixed_theta(EXT, RECON)>(q, 1, wm[v], wp[v], ph);
+            else if (D == 1) face_values<T, RECON, EXT, fixed_theta(EXT, RECON)>(q, NP, wm[v], wp[v], ph);
+            else {
+                const int o = v * G::PLN + c;
+                if (RECON == PPM)
+                    face_values5<T, RECON, EXT>(Pz[0][o], Pz[R - 1][o], Pz[R][o], Pz[R + 1][o], Pz[2 * R][o], wm[v], wp[v], ph);
+                else
+                    face_values5<T, RECON, EXT>(T(0), Pz[R - 1][o], Pz[R][o], Pz[R + 1][o], T(0), wm[v], wp[v], ph);
+            }
+        }
+        // rotate so that the traced axis is "n"
+        Wr[0] = Wc[0]; Wr[1] = Wc[cn]; Wr[2] = Wc[c1]; Wr[3] = Wc[c2]; Wr[4] = Wc[4];
+        rm[0] = wm[0]; rm[1] = wm[cn]; rm[2] = wm[c1]; rm[3] = wm[c2]; rm[4] = wm[4];
+        rp[0] = wp[0]; rp[1] = wp[cn]; rp[2] = wp[c1]; rp[3] = wp[c2]; rp[4] = wp[4];
+        if (NV > 5) { Wr[NV - 1] = Wc[NV - 1]; rm[NV - 1] = wm[NV - 1]; rp[NV - 1] = wp[NV - 1]; }
+    }
     trace_cell<T, RECON, NV>(Wr, rm, rp, tm, tp, ph);
     if (EXT && ph.floors) { floor_prim(tm, ph); floor_prim(tp, ph); }
     if (!(tm[0] > T(0) && tm[4] > T(0) && tp[0] > T(0) && tp[4] > T(0))) {

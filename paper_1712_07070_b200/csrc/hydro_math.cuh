@@ -77,7 +77,7 @@ template <typename T> struct Phys {
     int limiter;    // LIM_*
     // extended mode only
     T xi, min_dens, min_pres, min_temp;
-    int floors, dual, remedy2;
+    int floors, dual, remedy2, char_limit;
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -166,6 +166,67 @@ __device__ __forceinline__ void face_values(const T* q, int s, T& wm, T& wp, con
         const T ap = Ops<T>::minabs_same_sign(dp, dm + dm);
         wm = c - Ops<T>::copysign(am, dm);
         wp = c + Ops<T>::copysign(ap, dp);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// slope limiting in characteristic variables (L94; DESIGN R22): rotated primitive states of cells j-1, j, j+1 ->
+// slope vector of cell j = R . limiter(L (W_j - W_j-1), L (W_j+1 - W_j)), eigenvectors evaluated at cell j
+// ---------------------------------------------------------------------------------------------
+template <typename T, int NV, bool EXT>
+__device__ __forceinline__ void char_slope(const T* Wl, const T* Wc, const T* Wr, T* slope, const Phys<T>& ph) {
+    const T rho = Wc[0];
+    const T c2 = ph.gamma * Wc[4] / rho;
+    const T cs = ::sqrt(c2);
+    T aL[NV], aR[NV];
+    {
+        const T d0 = Wc[0] - Wl[0], d1 = Wc[1] - Wl[1], d4 = Wc[4] - Wl[4];
+        aL[0] = (d4 - rho * cs * d1) / (T(2) * c2); aL[1] = d0 - d4 / c2; aL[2] = Wc[2] - Wl[2]; aL[3] = Wc[3] - Wl[3];
+        aL[4] = (d4 + rho * cs * d1) / (T(2) * c2);
+        if (NV > 5) aL[NV - 1] = Wc[NV - 1] - Wl[NV - 1];
+    }
+    {
+        const T d0 = Wr[0] - Wc[0], d1 = Wr[1] - Wc[1], d4 = Wr[4] - Wc[4];
+        aR[0] = (d4 - rho * cs * d1) / (T(2) * c2); aR[1] = d0 - d4 / c2; aR[2] = Wr[2] - Wc[2]; aR[3] = Wr[3] - Wc[3];
+        aR[4] = (d4 + rho * cs * d1) / (T(2) * c2);
+        if (NV > 5) aR[NV - 1] = Wr[NV - 1] - Wc[NV - 1];
+    }
+    T s[NV];
+#pragma unroll
+    for (int a = 0; a < NV; ++a) s[a] = limited_slope<T, EXT, 0>(aL[a], aR[a], ph);
+    slope[0] = (s[0] + s[1]) + s[4];
+    slope[1] = s[4] * cs / rho - s[0] * cs / rho;
+    slope[2] = s[2];
+    slope[3] = s[3];
+    slope[4] = s[0] * cs * cs + s[4] * cs * cs;
+    if (NV > 5) slope[NV - 1] = s[NV - 1];
+}
+
+// face values of cell j from the rotated primitive states Wr[0..4] = cells j-2 .. j+2 (PLM reads 1..3 only)
+template <typename T, int RECON, int NV, bool EXT>
+__device__ __forceinline__ void face_values_char(const T (*Wr)[NV], T* rm, T* rp, const Phys<T>& ph) {
+    if (RECON == PLM) {
+        T sl[NV];
+        char_slope<T, NV, EXT>(Wr[1], Wr[2], Wr[3], sl, ph);
+#pragma unroll
+        for (int v = 0; v < NV; ++v) { rm[v] = Wr[2][v] - T(0.5) * sl[v]; rp[v] = Wr[2][v] + T(0.5) * sl[v]; }
+    } else {
+        T sm[NV], s0[NV], sp[NV];
+        char_slope<T, NV, EXT>(Wr[0], Wr[1], Wr[2], sm, ph);
+        char_slope<T, NV, EXT>(Wr[1], Wr[2], Wr[3], s0, ph);
+        char_slope<T, NV, EXT>(Wr[2], Wr[3], Wr[4], sp, ph);
+        const T sixth = T(1.0 / 6.0);
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+            const T c = Wr[2][v];
+            const T m = T(0.5) * (Wr[1][v] + c) - (s0[v] - sm[v]) * sixth;
+            const T p = T(0.5) * (c + Wr[3][v]) - (sp[v] - s0[v]) * sixth;
+            const T dm = c - m, dp = p - c;      // monotonisation as in face_values
+            const T am = Ops<T>::minabs_same_sign(dm, dp + dp);
+            const T ap = Ops<T>::minabs_same_sign(dp, dm + dm);
+            rm[v] = c - Ops<T>::copysign(am, dm);
+            rp[v] = c + Ops<T>::copysign(ap, dp);
+        }
     }
 }
 

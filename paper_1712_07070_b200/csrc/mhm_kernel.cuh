@@ -79,6 +79,18 @@ __device__ __forceinline__ void mhm_face_states(const T* const* Pz, const Phys<T
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
         T Wm[NV], Wp[NV];
+        if (EXT && ph.char_limit) {      // slopes limited in characteristic variables (R22): all variables together
+            T Wr[5][NV], rm[NV], rp[NV];
+#pragma unroll
+            for (int m = -R; m <= R; ++m) {
+                const T* q = (d == 2) ? Pz[R + m] : Pz[R] + m * (d == 0 ? 1 : NP);
+#pragma unroll
+                for (int k = 0; k < NV; ++k) Wr[m + 2][k] = q[nat_index(d, k) * PLN];
+            }
+            face_values_char<T, RECON, NV, EXT>(Wr, rm, rp, ph);
+#pragma unroll
+            for (int k = 0; k < NV; ++k) { Wm[nat_index(d, k)] = rm[k]; Wp[nat_index(d, k)] = rp[k]; }
+        } else
 #pragma unroll
         for (int v = 0; v < NV; ++v) {
             const T* q = Pz[R] + v * PLN;
