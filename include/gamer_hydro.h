@@ -165,12 +165,15 @@ int gamer_flux_correct(void* coarse, const void* coarse_flux, const void* fine_f
 /* End-to-end form with HOST buffers (pinned or pageable): copies `in` to the device in chunks,
  * runs the solver, copies `out`, `flux_out` (nullable) and `group_speed_out` (nullable) back,
  * overlapping copies and kernels on internal streams as the paper does with CUDA streams (L242),
- * and synchronises before returning.  Device scratch is allocated and freed inside the call. */
+ * and synchronises before returning.  Three device buffer sets of one chunk (592 groups, about 0.6 GB in fp32) and three
+ * streams are created on first use and kept for later calls (gamer_release_scratch frees them); calls are serialised. */
 int gamer_fluid_advance_host(const void* in_host, void* out_host, void* flux_out_host,
                              void* group_speed_out_host, int64_t n_groups,
                              double dt, double dh, double gamma,
                              int scheme, int recon, int riemann, int precision,
                              const gamer_opts* opts /* nullable; device pointers inside are ignored */);
+
+void gamer_release_scratch(void);
 
 /* Number of kernel launches the library has issued in this process (all entry points). */
 int64_t gamer_launch_count(void);

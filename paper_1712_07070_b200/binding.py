@@ -23,7 +23,7 @@ LIB_PATH = os.path.join(_HERE, "libgamerhydro.so")
 EXPORTS = ["gamer_fluid_advance", "gamer_fluid_advance_ex", "gamer_cfl_dt", "gamer_cfl_dt_ex",
            "gamer_cfl_from_group_speed", "gamer_refresh_ghosts_periodic", "gamer_refresh_ghosts", "gamer_fluid_advance_resident",
            "gamer_neighbors_periodic", "gamer_restrict", "gamer_flux_accumulate", "gamer_flux_correct",
-           "gamer_fluid_advance_host",
+           "gamer_fluid_advance_host", "gamer_release_scratch",
            "gamer_launch_count", "gamer_strerror", "gamer_version"]
 
 
@@ -222,6 +222,10 @@ def gamer_fluid_advance_host(in_host, out_host, flux_out_host, group_speed_out_h
                                           _ptr(group_speed_out_host, "cpu"), n, float(dt), float(dh), float(gamma),
                                           int(scheme), int(recon), int(riemann), _precision(in_host),
                                           ctypes.byref(opts)), "gamer_fluid_advance_host")
+
+
+def gamer_release_scratch():
+    lib().gamer_release_scratch()
 
 
 def gamer_launch_count():

@@ -3,6 +3,7 @@
 #include <atomic>
 #include <cmath>
 #include <cstring>
+#include <mutex>
 
 #include "../../include/gamer_hydro.h"
 #include "aux_kernels.cuh"
@@ -293,6 +294,57 @@ extern "C" int gamer_flux_correct(void* coarse, const void* coarse_flux, const v
 }
 
 // ------------------------------------------------------------------------------------------ host-buffer entry
+// scratch of the host entry (3 streams, 3 sets of device buffers), kept between calls: allocating and freeing
+// ~0.6 GB per call cost more than the copies of a small batch.  Freed by gamer_release_scratch() or at exit.
+namespace {
+struct HostScratch {
+    static constexpr int NBUF = 3;
+    cudaStream_t st[NBUF] = {nullptr, nullptr, nullptr};
+    char* d_in[NBUF] = {};
+    char* d_out[NBUF] = {};
+    char* d_fl[NBUF] = {};
+    char* d_sp[NBUF] = {};
+    size_t cap_in = 0, cap_out = 0, cap_fl = 0, cap_sp = 0;
+    int device = -1;
+    std::mutex mu;
+    void release() {
+        for (int b = 0; b < NBUF; ++b) {
+            if (d_in[b]) cudaFree(d_in[b]);
+            if (d_out[b]) cudaFree(d_out[b]);
+            if (d_fl[b]) cudaFree(d_fl[b]);
+            if (d_sp[b]) cudaFree(d_sp[b]);
+            if (st[b]) cudaStreamDestroy(st[b]);
+            d_in[b] = d_out[b] = d_fl[b] = d_sp[b] = nullptr;
+            st[b] = nullptr;
+        }
+        cap_in = cap_out = cap_fl = cap_sp = 0;
+        device = -1;
+    }
+    bool ensure(size_t in_b, size_t out_b, size_t fl_b, size_t sp_b) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess) return false;
+        if (dev != device || in_b > cap_in || out_b > cap_out || fl_b > cap_fl || sp_b > cap_sp) {
+            release();
+            for (int b = 0; b < NBUF; ++b) {
+                if (cudaStreamCreateWithFlags(&st[b], cudaStreamNonBlocking) != cudaSuccess) return false;
+                if (cudaMalloc(&d_in[b], in_b) != cudaSuccess || cudaMalloc(&d_out[b], out_b) != cudaSuccess ||
+                    cudaMalloc(&d_fl[b], fl_b) != cudaSuccess || cudaMalloc(&d_sp[b], sp_b) != cudaSuccess)
+                    return false;
+            }
+            cap_in = in_b; cap_out = out_b; cap_fl = fl_b; cap_sp = sp_b;
+            device = dev;
+        }
+        return true;
+    }
+};
+HostScratch g_scratch;
+}  // namespace
+
+extern "C" void gamer_release_scratch(void) {
+    std::lock_guard<std::mutex> lock(g_scratch.mu);
+    g_scratch.release();
+}
+
 extern "C" int gamer_fluid_advance_host(const void* in_host, void* out_host, void* flux_out_host,
                                         void* group_speed_out_host, int64_t n_groups, double dt, double dh,
                                         double gamma, int scheme, int recon, int riemann, int precision,
@@ -304,17 +356,16 @@ extern "C" int gamer_fluid_advance_host(const void* in_host, void* out_host, voi
     const int nv = 5 + (opts ? opts->n_scalar : 0);
     const size_t sz = (size_t)precision;
     const size_t in_g = (size_t)nv * NPC * sz, out_g = (size_t)nv * PS * PS * PS * sz, fl_g = (size_t)9 * nv * PS * PS * sz;
-    constexpr int NBUF = 3;
-    const int64_t chunk = n_groups < 592 ? n_groups : 592;   // 4 waves of 148 CTAs; ~1e6 cells saturate (L321)
-    cudaStream_t st[NBUF] = {nullptr, nullptr, nullptr};
-    char *d_in[NBUF] = {}, *d_out[NBUF] = {}, *d_fl[NBUF] = {}, *d_sp[NBUF] = {};
-    int rc = GAMER_OK;
-    for (int b = 0; b < NBUF && rc == GAMER_OK; ++b) {
-        if (cudaStreamCreateWithFlags(&st[b], cudaStreamNonBlocking) != cudaSuccess) rc = GAMER_ECUDA;
-        else if (cudaMalloc(&d_in[b], in_g * chunk) != cudaSuccess || cudaMalloc(&d_out[b], out_g * chunk) != cudaSuccess ||
-                 cudaMalloc(&d_fl[b], fl_g * chunk) != cudaSuccess || cudaMalloc(&d_sp[b], sz * chunk) != cudaSuccess)
-            rc = GAMER_ECUDA;
+    constexpr int NBUF = HostScratch::NBUF;
+    const int64_t chunk = n_groups < 592 ? n_groups : 592;   // 2 waves of 296 CTAs; ~1e6 cells saturate (L321)
+    std::lock_guard<std::mutex> lock(g_scratch.mu);
+    if (!g_scratch.ensure(in_g * chunk, out_g * chunk, fl_g * chunk, sz * chunk)) {
+        g_scratch.release();
+        return GAMER_ECUDA;
     }
+    cudaStream_t* st = g_scratch.st;
+    char **d_in = g_scratch.d_in, **d_out = g_scratch.d_out, **d_fl = g_scratch.d_fl, **d_sp = g_scratch.d_sp;
+    int rc = GAMER_OK;
     int64_t done = 0;
     for (int it = 0; done < n_groups && rc == GAMER_OK; ++it) {
         const int b = it % NBUF;
@@ -337,11 +388,8 @@ extern "C" int gamer_fluid_advance_host(const void* in_host, void* out_host, voi
         if (cudaGetLastError() != cudaSuccess) rc = GAMER_ECUDA;
         done += n;
     }
-    for (int b = 0; b < NBUF; ++b) {
-        if (st[b]) { if (cudaStreamSynchronize(st[b]) != cudaSuccess) rc = GAMER_ECUDA; }
-        cudaFree(d_in[b]); cudaFree(d_out[b]); cudaFree(d_fl[b]); cudaFree(d_sp[b]);
-        if (st[b]) cudaStreamDestroy(st[b]);
-    }
+    for (int b = 0; b < NBUF; ++b)
+        if (cudaStreamSynchronize(st[b]) != cudaSuccess) rc = GAMER_ECUDA;
     return rc;
 }
 
