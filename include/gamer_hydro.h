@@ -116,6 +116,12 @@ int gamer_refresh_ghosts_periodic(const void* u, void* in, int gz, int gy, int g
 int gamer_refresh_ghosts(const void* u, void* in, int gz, int gy, int gx, int nvar, const int* bc,
                          int precision, void* stream);
 
+/* The sibling copy for any same-level topology: nbr[n_groups][27] (device int32) as in gamer_fluid_advance_resident,
+ * except that an entry may be -1 = "no same-level neighbour there" (a coarse-fine or domain boundary): those slabs of
+ * `in` are left as they are, for the caller to fill (interpolation from the parent level, user-defined inflow). */
+int gamer_refresh_ghosts_table(const void* u, void* in, const int32_t* nbr, int64_t n_groups, int nvar,
+                               int precision, void* stream);
+
 /* Device-resident step with the same-level ghost refresh FUSED into the staging loads (SURVEY 8(f) NEXT-1,
  * PAPER.md L248 "preparation" + L274 Fig. 3): `u` is the UNPADDED state of the whole batch,
  * u[n_groups][NVAR][16][16][16] (the `out` layout), and nbr[n_groups][27] (device int32) names, for every group,

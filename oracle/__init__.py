@@ -233,3 +233,21 @@ def char_slope(Wl, Wc, Wr, gamma, limiter=GMINMOD, theta=1.0):
     lib().oracle_char_slope(int(limiter), ctypes.c_double(theta), ctypes.c_double(gamma), int(Wc.shape[0] - 5),
                             _p(Wl), _p(Wc), _p(Wr), _p(out))
     return out
+
+
+def fill_ghosts_table(u, nbr, padded):
+    """Sibling copy of PAPER.md L248 driven by a same-level neighbour table: u [G,NV,16,16,16], nbr [G,27]
+    (index (dz+1)*9 + (dy+1)*3 + (dx+1), entry 13 = the group itself, -1 = no same-level neighbour), padded
+    [G,NV,22,22,22] modified in place: each of the 27 slabs of a padded group is copied from the group the table names;
+    slabs with entry -1 (coarse-fine boundaries, to be interpolated by the caller) are left as they are."""
+    u = np.asarray(u)
+    rng = {0: (slice(0, NG), slice(PS - NG, PS)), 1: (slice(NG, NG + PS), slice(0, PS)), 2: (slice(NG + PS, NP), slice(0, NG))}
+    for g in range(u.shape[0]):
+        for dz in range(3):
+            for dy in range(3):
+                for dx in range(3):
+                    s = int(nbr[g, (dz * 3 + dy) * 3 + dx])
+                    if s < 0:
+                        continue
+                    padded[g][:, rng[dz][0], rng[dy][0], rng[dx][0]] = u[s][:, rng[dz][1], rng[dy][1], rng[dx][1]]
+    return padded

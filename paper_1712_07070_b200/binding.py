@@ -21,7 +21,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libgamerhydro.so")
 
 EXPORTS = ["gamer_fluid_advance", "gamer_fluid_advance_ex", "gamer_cfl_dt", "gamer_cfl_dt_ex",
-           "gamer_cfl_from_group_speed", "gamer_refresh_ghosts_periodic", "gamer_refresh_ghosts", "gamer_fluid_advance_resident",
+           "gamer_cfl_from_group_speed", "gamer_refresh_ghosts_periodic", "gamer_refresh_ghosts", "gamer_refresh_ghosts_table", "gamer_fluid_advance_resident",
            "gamer_neighbors_periodic", "gamer_restrict", "gamer_flux_accumulate", "gamer_flux_correct",
            "gamer_fluid_advance_host", "gamer_release_scratch",
            "gamer_launch_count", "gamer_strerror", "gamer_version"]
@@ -72,6 +72,7 @@ def lib():
         L.gamer_cfl_from_group_speed.argtypes = [vp, i64, dbl, dbl, ci, vp, vp]
         L.gamer_refresh_ghosts_periodic.argtypes = [vp, vp, ci, ci, ci, ci, ci, vp]
         L.gamer_refresh_ghosts.argtypes = [vp, vp, ci, ci, ci, ci, ctypes.POINTER(ci), ci, vp]
+        L.gamer_refresh_ghosts_table.argtypes = [vp, vp, vp, i64, ci, ci, vp]
         L.gamer_fluid_advance_resident.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, ci, ci, ctypes.POINTER(gamer_opts)]
         L.gamer_neighbors_periodic.argtypes = [vp, ci, ci, ci, vp]
         L.gamer_restrict.argtypes = [vp, vp, vp, i64, ci, ci, vp]
@@ -169,6 +170,14 @@ def gamer_refresh_ghosts(u, u_in, gz, gy, gx, bc, stream=None):
     arr = (ctypes.c_int * 6)(*[int(b) for b in bc])
     _check(lib().gamer_refresh_ghosts(_ptr(u), _ptr(u_in), gz, gy, gx, u.shape[1], arr, _precision(u),
                                       _stream_handle(stream)), "gamer_refresh_ghosts")
+
+
+def gamer_refresh_ghosts_table(u, u_in, nbr, stream=None):
+    """Sibling copy through a [G, 27] int32 neighbour table; slabs whose entry is -1 are left untouched."""
+    if nbr.dtype != torch.int32 or tuple(nbr.shape) != (u.shape[0], 27):
+        raise GamerError("nbr must be an int32 tensor of shape [n_groups, 27]")
+    _check(lib().gamer_refresh_ghosts_table(_ptr(u), _ptr(u_in), _ptr(nbr), u.shape[0], u.shape[1], _precision(u),
+                                            _stream_handle(stream)), "gamer_refresh_ghosts_table")
 
 
 def gamer_fluid_advance_resident(u, nbr, out, flux_out, dt, dh, gamma, scheme, recon, riemann, opts=None):

@@ -243,6 +243,20 @@ extern "C" int gamer_refresh_ghosts(const void* u, void* in, int gz, int gy, int
     return cudaGetLastError() == cudaSuccess ? GAMER_OK : GAMER_ECUDA;
 }
 
+extern "C" int gamer_refresh_ghosts_table(const void* u, void* in, const int32_t* nbr, int64_t n_groups, int nvar,
+                                          int precision, void* stream) {
+    if (n_groups < 0 || nvar < 5 || nvar > 6 || (precision != GAMER_FP32 && precision != GAMER_FP64)) return GAMER_EINVAL;
+    if (n_groups > 0 && (!u || !in || !nbr)) return GAMER_EINVAL;
+    if (n_groups == 0) return GAMER_OK;
+    if (n_groups * nvar > 0x7fffffff) return GAMER_EUNSUPPORTED;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const unsigned grid = (unsigned)(n_groups * nvar);
+    if (precision == GAMER_FP32) refresh_table_kernel<float><<<grid, 256, 0, st>>>(static_cast<const float*>(u), static_cast<float*>(in), nbr, nvar);
+    else refresh_table_kernel<double><<<grid, 256, 0, st>>>(static_cast<const double*>(u), static_cast<double*>(in), nbr, nvar);
+    g_launches += 1;
+    return cudaGetLastError() == cudaSuccess ? GAMER_OK : GAMER_ECUDA;
+}
+
 // ------------------------------------------------------------------------------------------ coarse-fine fix-up
 extern "C" int gamer_restrict(const void* fine, void* coarse, const int32_t* parent, int64_t n_fine, int nvar,
                               int precision, void* stream) {

@@ -181,6 +181,42 @@ __global__ void __launch_bounds__(256) refresh_bc_kernel(const T* __restrict__ u
     }
 }
 
+// Same-level ghost refresh driven by a neighbour table (any topology): one CTA per (group, variable); padded cell
+// (pk, pj, pi) comes from the group nbr[g][(dz*3 + dy)*3 + dx] named for its slab, or is left untouched if that entry
+// is -1 (coarse-fine boundary, filled by the caller's interpolation).
+template <typename T>
+__global__ void __launch_bounds__(256) refresh_table_kernel(const T* __restrict__ u, T* __restrict__ in,
+                                                            const int* __restrict__ nbr, int nvar) {
+    __shared__ int nb[27];
+    const long long gv = blockIdx.x;
+    const long long g = gv / nvar;
+    const int v = (int)(gv - g * nvar);
+    if (threadIdx.x < 27) nb[threadIdx.x] = nbr[g * 27 + threadIdx.x];
+    __syncthreads();
+    int offxy[2], sxy[2];
+    bool live[2];
+#pragma unroll
+    for (int r = 0; r < 2; ++r) {
+        const int t = threadIdx.x + r * 256;
+        live[r] = t < NP * NP;
+        const int pj = t / NP, pi = t - pj * NP;
+        const int dx = pi < NGH ? 0 : (pi < NGH + PS ? 1 : 2), dy = pj < NGH ? 0 : (pj < NGH + PS ? 1 : 2);
+        sxy[r] = dy * 3 + dx;
+        offxy[r] = ((pj + PS - NGH) & (PS - 1)) * PS + ((pi + PS - NGH) & (PS - 1));
+    }
+    T* dst = in + ((size_t)g * nvar + v) * NPC;
+    for (int pk = 0; pk < NP; ++pk) {
+        const int dz = pk < NGH ? 0 : (pk < NGH + PS ? 1 : 2);
+        const int offz = ((pk + PS - NGH) & (PS - 1)) * (PS * PS);
+#pragma unroll
+        for (int r = 0; r < 2; ++r)
+            if (live[r]) {
+                const int s = nb[dz * 9 + sxy[r]];
+                if (s >= 0) dst[pk * (NP * NP) + threadIdx.x + r * 256] = __ldg(u + ((size_t)s * nvar + v) * (PS * PS * PS) + offz + offxy[r]);
+            }
+    }
+}
+
 // neighbour table of a periodic box of gz x gy x gx groups: nbr[g][(dz+1)*9 + (dy+1)*3 + (dx+1)]
 __global__ void neighbors_periodic_kernel(int* __restrict__ nbr, int gz, int gy, int gx) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;

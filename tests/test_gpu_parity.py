@@ -279,3 +279,22 @@ def test_config1_sod_with_outflow_in_x_as_stated(dev, oracle_mod, dtype):
     new = inputs.unpack(inputs.interior(u_gpu).cpu().to(torch.float64).contiguous(), 4, 4, 4)
     assert (new[0, :, :, 0] - 1.0).abs().max() <= 1e-6 and (new[0, :, :, -1] - 0.125).abs().max() <= 1e-6
     assert (new[0] - new[0, :1, :1, :]).abs().max() <= 1e-6
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+def test_table_driven_ghost_refresh_matches_oracle(dev, oracle_mod, dtype):
+    """gamer_refresh_ghosts_table (sibling copy of L248 for any same-level topology) against oracle.fill_ghosts_table,
+    bit for bit, including slabs without a same-level neighbour (-1), which must keep their previous content."""
+    f = inputs.turbulence_field(16, 5, kmax=4, gamma=G53, shape=(32, 48, 16)).to(dtype)
+    u = inputs.interior(inputs.pack_periodic(f)).contiguous()
+    nbr = gb.gamer_neighbors_periodic(2, 3, 1, dev).cpu()
+    nbr[:, 14] = -1
+    nbr[3, 4] = -1
+    nbr[5, 0] = -1
+    before = torch.randn((6, 5, 22, 22, 22), generator=torch.Generator().manual_seed(1), dtype=torch.float64).to(dtype)
+    ref = oracle_mod.fill_ghosts_table(u.numpy(), nbr.numpy(), before.numpy().copy())
+    padded = before.to(dev).clone()
+    gb.gamer_refresh_ghosts_table(u.to(dev), padded, nbr.to(dev))
+    torch.cuda.synchronize()
+    assert np.array_equal(padded.cpu().numpy(), ref)
+    assert not np.array_equal(ref, before.numpy())

@@ -78,3 +78,27 @@ def test_reflecting_box_is_closed_and_outflow_lets_a_pulse_leave(oracle_mod):
     opened = run(((O, O),) * 3)
     assert abs(opened[0].sum() - u[0].sum()) > 1e-7 * u[0].sum()       # in- and outflow nearly cancel, but not to round-off
     assert np.abs(opened[0] - closed[0]).max() > 1e-3                  # and the walls do matter
+
+
+def test_table_driven_sibling_copy(oracle_mod):
+    """oracle.fill_ghosts_table: with the periodic table of a 2 x 3 x 1 box it is pack_periodic; with some entries
+    set to -1 exactly those slabs keep their previous content."""
+    f = _field()
+    gz, gy, gx = 2, 3, 1
+    u = inputs.interior(inputs.pack_periodic(torch.from_numpy(f))).contiguous().numpy()
+    nbr = np.empty((6, 27), dtype=np.int32)
+    for g in range(6):
+        bz, by, bx = g // (gy * gx), (g // gx) % gy, g % gx
+        for k in range(27):
+            dz, dy, dx = k // 9 - 1, (k // 3) % 3 - 1, k % 3 - 1
+            nbr[g, k] = (((bz + dz) % gz) * gy + (by + dy) % gy) * gx + (bx + dx) % gx
+    full = oracle_mod.fill_ghosts_table(u, nbr, np.full((6, 5, 22, 22, 22), np.nan))
+    assert np.array_equal(full, inputs.pack_periodic(torch.from_numpy(f)).numpy())
+    nbr2 = nbr.copy()
+    nbr2[:, 14] = -1                       # no +x neighbour anywhere
+    nbr2[3, 4] = -1                        # group 3: no (dz, dy, dx) = (-1, 0, 0) neighbour
+    part = oracle_mod.fill_ghosts_table(u, nbr2, np.full((6, 5, 22, 22, 22), np.nan))
+    hole = np.isnan(part)
+    assert hole[:, :, 3:19, 3:19, 19:22].all() and hole[3, :, 0:3, 3:19, 3:19].all()
+    assert hole.sum() == 6 * 5 * 16 * 16 * 3 + 5 * 3 * 16 * 16
+    assert np.array_equal(part[~hole], full[~hole])
