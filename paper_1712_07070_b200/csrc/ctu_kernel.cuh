@@ -21,42 +21,96 @@ template <typename T, int RECON, int NV, int TY, bool FUSED = false> struct CtuS
     using G = Geo<TY>;
     static constexpr int R = RECON == PPM ? 2 : 1;
     static constexpr int PR = 2 * R + 1;
+    // every face-state / flux array is [Vec4 n | (NV-4) scalars n] in the rotated order of its axis
+    // (rho, v_d, v_d+1, v_d+2, P [, q]); n is rounded up to a multiple of 4 to keep the Vec4 parts 16-byte aligned
+    static constexpr int pad4(int n) { return (n + 3) / 4 * 4; }
     static constexpr int NF1X = 17 * G::EH, NF1Y = 18 * (G::EH - 1);
+    static constexpr int NF1XP = pad4(NF1X), NF1YP = pad4(NF1Y);
     static constexpr int RAW = 0;                                   // [2][NV][PLN]
     static constexpr int RSTG = NV * (FUSED ? G::NR * FW : G::PLN); // one landing stage (fused refresh: 24-wide rows)
     static constexpr int PRIM = RAW + 2 * RSTG;                     // [PR][NV][PLN]
-    static constexpr int TS = PRIM + PR * NV * G::PLN;              // [2][6][NV][EPL]
-    static constexpr int F1X = TS + 2 * 6 * NV * G::EPL;            // [NV][NF1X]
-    static constexpr int F1Y = F1X + NV * NF1X;                     // [NV][NF1Y]
-    static constexpr int F1Z = F1Y + NV * NF1Y;                     // [2][NV][EPL]
-    static constexpr int ZP = F1Z + 2 * NV * G::EPL;                // [2][NV][NFZ]
+    static constexpr int TS = PRIM + PR * NV * G::PLN;              // [2][6] x state array of EPL
+    static constexpr int F1X = TS + 2 * 6 * NV * G::EPL;            // flux array of NF1XP
+    static constexpr int F1Y = F1X + NV * NF1XP;                    // flux array of NF1YP
+    static constexpr int F1Z = F1Y + NV * NF1YP;                    // [2] x flux array of EPL
+    static constexpr int ZP = F1Z + 2 * NV * G::EPL;                // [2] x state array of NFZ
     static constexpr int FX = ZP + 2 * NV * G::NFZ;
     static constexpr int FY = FX + NV * G::NFX;
     static constexpr int FZ = FY + NV * G::NFY;
     static constexpr int END = FZ + NV * G::NFZ;
+    static_assert(RSTG % 4 == 0 && (NV * G::PLN) % 4 == 0 && G::EPL % 4 == 0 && G::NFX % 4 == 0 && G::NFY % 4 == 0 && G::NFZ % 4 == 0,
+                  "16-byte alignment of the Vec4 arrays");
     static constexpr size_t BYTES = 16 + (size_t)END * sizeof(T) + (FUSED ? 128 : 0);   // + neighbour table
 };
 
-// one first-pass Riemann solve: rotated loads from two state arrays, unrotated store
+// one first-pass Riemann solve: states and flux are stored in the rotated order of the axis, nothing to rotate here
 template <typename T, int SOLVER, int NV>
-__device__ __forceinline__ int first_pass_face(const T* lp, int lidx, const T* rp, int ridx, int sstr, T* fp,
-                                               int fidx, int fstr, int d, const Phys<T>& ph) {
-    const int cn = 1 + d, c1 = 1 + (d + 1) % 3, c2 = 1 + (d + 2) % 3;
+__device__ __forceinline__ int first_pass_face(const T* lblk, int lidx, const T* rblk, int ridx, int sn, T* fblk,
+                                               int fidx, int fn, const Phys<T>& ph) {
     T WL[NV], WR[NV], F[NV];
-    WL[0] = lp[lidx];               WR[0] = rp[ridx];
-    WL[1] = lp[cn * sstr + lidx];   WR[1] = rp[cn * sstr + ridx];
-    WL[2] = lp[c1 * sstr + lidx];   WR[2] = rp[c1 * sstr + ridx];
-    WL[3] = lp[c2 * sstr + lidx];   WR[3] = rp[c2 * sstr + ridx];
-    WL[4] = lp[4 * sstr + lidx];    WR[4] = rp[4 * sstr + ridx];
-    if (NV > 5) { WL[NV - 1] = lp[(NV - 1) * sstr + lidx]; WR[NV - 1] = rp[(NV - 1) * sstr + ridx]; }
+    get_state<T, NV>(lblk, sn, lidx, WL);
+    get_state<T, NV>(rblk, sn, ridx, WR);
     const int fb = riemann_flux<T, SOLVER, NV>(WL, WR, F, ph) ? 1 : 0;
-    fp[fidx] = F[0];
-    fp[cn * fstr + fidx] = F[1];
-    fp[c1 * fstr + fidx] = F[2];
-    fp[c2 * fstr + fidx] = F[3];
-    fp[4 * fstr + fidx] = F[4];
-    if (NV > 5) fp[(NV - 1) * fstr + fidx] = F[NV - 1];
+    put_state<T, NV>(fblk, fn, fidx, F);
     return fb;
+}
+
+// final Riemann pass over the faces of one plane of the tile (x- and y-faces of plane kk, z-faces between planes kk-1 and
+// kk): es = the six corrected state arrays of the plane, zprev = corrected z+ of plane kk-1; fluxes go to fx/fy/fz in the
+// rotated order of their axis and, on patch boundaries, to flux_out in natural order
+template <typename T, int SOLVER, int NV, int TY, int NT>
+__device__ __forceinline__ int ctu_final_pass(const T* es, const T* zprev, T* fx, T* fy, T* fz, T* gflux, int kk, int j0,
+                                              const Phys<T>& ph, int tid) {
+    using G = Geo<TY>;
+    constexpr int SB = NV * G::EPL;      // one state array
+    int nfb = 0;
+    const int f_lo = (kk >= 0 && kk < PS) ? 0 : G::NFX + G::NFY;
+    const int f_hi = (kk >= 0 && kk <= PS) ? G::NF : 0;
+    for (int f = f_lo + tid; f < f_hi; f += NT) {
+        int d, lidx, ridx, ln, fidx, fn, gp, ga, gb;
+        const T *lp, *rp;
+        T* fp;
+        if (f < G::NFX) {
+            const int jj = f / 17, ii = f - jj * 17;
+            d = 0;
+            lp = es + 1 * SB; lidx = (jj + 1) * G::EW + ii; ln = G::EPL;
+            rp = es + 0 * SB; ridx = lidx + 1;
+            fp = fx; fidx = f; fn = G::NFX;
+            gp = ii; ga = j0 + jj; gb = kk;
+        } else if (f < G::NFX + G::NFY) {
+            const int g = f - G::NFX;
+            const int jj = g >> 4, ii = g & 15;
+            d = 1;
+            lp = es + 3 * SB; lidx = jj * G::EW + ii + 1; ln = G::EPL;
+            rp = es + 2 * SB; ridx = lidx + G::EW;
+            fp = fy; fidx = g; fn = G::NFY;
+            gp = j0 + jj; ga = ii; gb = kk;
+        } else {
+            const int g = f - G::NFX - G::NFY;
+            const int jj = g >> 4, ii = g & 15;
+            d = 2;
+            lp = zprev; lidx = g; ln = G::NFZ;
+            rp = es + 4 * SB; ridx = (jj + 1) * G::EW + ii + 1;
+            fp = fz; fidx = g; fn = G::NFZ;
+            gp = kk; ga = ii; gb = j0 + jj;
+        }
+        T WL[NV], WR[NV], F[NV];
+        get_state<T, NV>(lp, ln, lidx, WL);
+        get_state<T, NV>(rp, G::EPL, ridx, WR);
+        nfb += riemann_flux<T, SOLVER, NV>(WL, WR, F, ph) ? 1 : 0;
+        put_state<T, NV>(fp, fn, fidx, F);
+        if (gflux != nullptr && (gp & 7) == 0) {   // faces 0, 8, 16 of the axis: patch boundaries (L112)
+            const int cn = 1 + d, c1 = 1 + (d + 1) % 3, c2 = 1 + (d + 2) % 3;
+            T* q = gflux + ((size_t)(d * 3 + (gp >> 3)) * NV) * (PS * PS) + gb * PS + ga;
+            q[0] = F[0];
+            q[(size_t)cn * (PS * PS)] = F[1];
+            q[(size_t)c1 * (PS * PS)] = F[2];
+            q[(size_t)c2 * (PS * PS)] = F[3];
+            q[(size_t)4 * (PS * PS)] = F[4];
+            if (NV > 5) q[(size_t)(NV - 1) * (PS * PS)] = F[NV - 1];
+        }
+    }
+    return nfb;
 }
 
 // T stage for one cell t of the 18 x (TY+2) face-state plane and one direction D: PLM/PPM face values of
@@ -111,14 +165,8 @@ __device__ __forceinline__ void ctu_trace_dir(const T* const* Pz, int t, T* tcur
 #pragma unroll
         for (int v = 0; v < NV; ++v) { tm[v] = rm[v]; tp[v] = rp[v]; }
     }
-    T* sm_ = tcur + (2 * D) * NV * EPL + t;
-    T* sp_ = tcur + (2 * D + 1) * NV * EPL + t;
-    sm_[0] = tm[0];        sp_[0] = tp[0];
-    sm_[cn * EPL] = tm[1]; sp_[cn * EPL] = tp[1];
-    sm_[c1 * EPL] = tm[2]; sp_[c1 * EPL] = tp[2];
-    sm_[c2 * EPL] = tm[3]; sp_[c2 * EPL] = tp[3];
-    sm_[4 * EPL] = tm[4];  sp_[4 * EPL] = tp[4];
-    if (NV > 5) { sm_[(NV - 1) * EPL] = tm[NV - 1]; sp_[(NV - 1) * EPL] = tp[NV - 1]; }
+    put_state<T, NV>(tcur + (2 * D) * NV * EPL, EPL, t, tm);          // rotated for axis D, as traced
+    put_state<T, NV>(tcur + (2 * D + 1) * NV * EPL, EPL, t, tp);
 }
 
 template <typename T, int RECON, int SOLVER, int NV, bool EXT, int TY, int NT, bool FUSED>
@@ -220,7 +268,7 @@ __global__ void __launch_bounds__(NT) ctu_kernel(const AdvArgs<T> a) {
         if (kk >= 0 && kk <= PS) {
             T* hz = f1z + (kk & 1) * NV * EPL;
             for (int t = tid; t < EPL; t += NT)
-                cnt.roe_fb += first_pass_face<T, SOLVER, NV>(tprev + 5 * NV * EPL, t, tcur + 4 * NV * EPL, t, EPL, hz, t, EPL, 2, ph);
+                cnt.roe_fb += first_pass_face<T, SOLVER, NV>(tprev + 5 * NV * EPL, t, tcur + 4 * NV * EPL, t, EPL, hz, t, EPL, ph);
         }
         {
             const int n = kk + 2 + 2 * R;
@@ -246,12 +294,29 @@ __global__ void __launch_bounds__(NT) ctu_kernel(const AdvArgs<T> a) {
                 else { const int u = t - 18 * TY; ej = (u < 16) ? 0 : TY + 1; ei = 1 + (u & 15); }
                 const int e = ej * EW + ei;
                 const bool rowin = (ej >= 1 && ej <= TY), colin = (ei >= 1 && ei <= 16);
-                T gx[NV], gy[NV], gz[NV];     // flux differences across the cell in x, y, z
+                T gx[NV], gy[NV], gz[NV];     // flux differences across the cell in x, y, z (natural variable order)
 #pragma unroll
-                for (int v = 0; v < NV; ++v) {
-                    gx[v] = colin ? f1x[v * S::NF1X + ej * 17 + ei] - f1x[v * S::NF1X + ej * 17 + ei - 1] : T(0);
-                    gy[v] = rowin ? f1y[v * S::NF1Y + ej * 18 + ei] - f1y[v * S::NF1Y + (ej - 1) * 18 + ei] : T(0);
-                    gz[v] = mid ? hhi[v * EPL + e] - hlo[v * EPL + e] : T(0);
+                for (int v = 0; v < NV; ++v) gx[v] = gy[v] = gz[v] = T(0);
+                if (colin) {
+                    T A[NV], B[NV];
+                    get_state<T, NV>(f1x, S::NF1XP, ej * 17 + ei, A);
+                    get_state<T, NV>(f1x, S::NF1XP, ej * 17 + ei - 1, B);
+#pragma unroll
+                    for (int k = 0; k < NV; ++k) gx[nat_index(0, k)] = A[k] - B[k];
+                }
+                if (rowin) {
+                    T A[NV], B[NV];
+                    get_state<T, NV>(f1y, S::NF1YP, ej * 18 + ei, A);
+                    get_state<T, NV>(f1y, S::NF1YP, (ej - 1) * 18 + ei, B);
+#pragma unroll
+                    for (int k = 0; k < NV; ++k) gy[nat_index(1, k)] = A[k] - B[k];
+                }
+                if (mid) {
+                    T A[NV], B[NV];
+                    get_state<T, NV>(hhi, EPL, e, A);
+                    get_state<T, NV>(hlo, EPL, e, B);
+#pragma unroll
+                    for (int k = 0; k < NV; ++k) gz[nat_index(2, k)] = A[k] - B[k];
                 }
 #pragma unroll
                 for (int d = 0; d < 3; ++d) {
@@ -261,10 +326,11 @@ __global__ void __launch_bounds__(NT) ctu_kernel(const AdvArgs<T> a) {
                     const T* g2 = (d == 0) ? gz : (d == 1) ? gx : gy;     // d2 = (d+2)%3
 #pragma unroll
                     for (int s = 0; s < 2; ++s) {
-                        T* sp_ = tprev + (2 * d + s) * NV * EPL + e;
-                        T W[NV], U[NV], Wn[NV];
+                        T* sblk = tprev + (2 * d + s) * NV * EPL;
+                        T W[NV], U[NV], Wn[NV], Wrot[NV];
+                        get_state<T, NV>(sblk, EPL, e, Wrot);
 #pragma unroll
-                        for (int v = 0; v < NV; ++v) W[v] = sp_[v * EPL];
+                        for (int k = 0; k < NV; ++k) W[nat_index(d, k)] = Wrot[k];
                         prim2cons<T, NV>(W, U, ph);
 #pragma unroll
                         for (int v = 0; v < NV; ++v) U[v] = U[v] - ph.hlam * g1[v] - ph.hlam * g2[v];
@@ -273,11 +339,9 @@ __global__ void __launch_bounds__(NT) ctu_kernel(const AdvArgs<T> a) {
                         const bool ok = Wn[0] > T(0) && Wn[4] > T(0);
                         if (!ok) cnt.reverted++;
 #pragma unroll
-                        for (int v = 0; v < NV; ++v) {
-                            const T val = ok ? Wn[v] : W[v];
-                            if (d == 2 && s == 1) zsave[v * G::NFZ + (ej - 1) * 16 + (ei - 1)] = val;
-                            else sp_[v * EPL] = val;
-                        }
+                        for (int k = 0; k < NV; ++k) Wrot[k] = ok ? Wn[nat_index(d, k)] : W[nat_index(d, k)];
+                        if (d == 2 && s == 1) put_state<T, NV>(zsave, G::NFZ, (ej - 1) * 16 + (ei - 1), Wrot);
+                        else put_state<T, NV>(sblk, EPL, e, Wrot);
                     }
                 }
             }
@@ -289,14 +353,14 @@ __global__ void __launch_bounds__(NT) ctu_kernel(const AdvArgs<T> a) {
                 if (t < S::NF1X) {
                     const int ej = t / 17, ei = t - ej * 17;
                     const int l = ej * EW + ei;
-                    cnt.roe_fb += first_pass_face<T, SOLVER, NV>(tcur + 1 * NV * EPL, l, tcur + 0 * NV * EPL, l + 1, EPL, f1x, t, S::NF1X, 0, ph);
+                    cnt.roe_fb += first_pass_face<T, SOLVER, NV>(tcur + 1 * NV * EPL, l, tcur + 0 * NV * EPL, l + 1, EPL, f1x, t, S::NF1XP, ph);
                 } else {
                     const int u = t - S::NF1X;      // = ej*18 + ei, ej in [0, EH-1)
-                    cnt.roe_fb += first_pass_face<T, SOLVER, NV>(tcur + 3 * NV * EPL, u, tcur + 2 * NV * EPL, u + EW, EPL, f1y, u, S::NF1Y, 1, ph);
+                    cnt.roe_fb += first_pass_face<T, SOLVER, NV>(tcur + 3 * NV * EPL, u, tcur + 2 * NV * EPL, u + EW, EPL, f1y, u, S::NF1YP, ph);
                 }
             }
         }
-        if (m >= 0) cnt.roe_fb += riemann_plane<T, SOLVER, NV, TY, NT>(tprev, zp + ((m + 1) & 1) * NV * G::NFZ, fx, fy, fz, gflux, m, j0, ph, tid);
+        if (m >= 0) cnt.roe_fb += ctu_final_pass<T, SOLVER, NV, TY, NT>(tprev, zp + ((m + 1) & 1) * NV * G::NFZ, fx, fy, fz, gflux, m, j0, ph, tid);
         __syncthreads();
         // ------------------------------------------------------------------ U(kk-2)
         {
@@ -311,10 +375,11 @@ __global__ void __launch_bounds__(NT) ctu_kernel(const AdvArgs<T> a) {
                 const int k = m - 1;
                 const T* gcell = FUSED ? gin + (size_t)g * NV * (PS * PS * PS) + (size_t)k * (PS * PS) + (j0 + cj) * PS + ci
                                        : gin + (size_t)(k + NGH) * (NP * NP) + (j0 + cj + NGH) * NP + (ci + NGH);
-                T U[NV];
+                T U[NV], Fz[NV];
+                get_state<T, NV>(fz, G::NFZ, tid, Fz);
 #pragma unroll
                 for (int v = 0; v < NV; ++v) {
-                    const T dfz = fz[v * G::NFZ + tid] - fzm[v];
+                    const T dfz = Fz[rot_index(2, v)] - fzm[v];
                     U[v] = __ldg(gcell + (size_t)v * (FUSED ? PS * PS * PS : NPC)) - ph.lam * (sxy[v] + dfz);
                 }
                 close_cell<T, SOLVER, NV, EXT>(U, gcell, cnt, ph);
@@ -326,12 +391,18 @@ __global__ void __launch_bounds__(NT) ctu_kernel(const AdvArgs<T> a) {
                 }
             }
             if (m >= 0 && m < PS) {
+                T Xr[NV], Xl[NV], Yu[NV], Yd[NV], Fz[NV];
+                get_state<T, NV>(fx, G::NFX, cj * 17 + ci + 1, Xr);
+                get_state<T, NV>(fx, G::NFX, cj * 17 + ci, Xl);
+                get_state<T, NV>(fy, G::NFY, (cj + 1) * 16 + ci, Yu);
+                get_state<T, NV>(fy, G::NFY, cj * 16 + ci, Yd);
+                get_state<T, NV>(fz, G::NFZ, tid, Fz);
 #pragma unroll
                 for (int v = 0; v < NV; ++v) {
-                    const T dfx = fx[v * G::NFX + cj * 17 + ci + 1] - fx[v * G::NFX + cj * 17 + ci];
-                    const T dfy = fy[v * G::NFY + (cj + 1) * 16 + ci] - fy[v * G::NFY + cj * 16 + ci];
+                    const T dfx = Xr[rot_index(0, v)] - Xl[rot_index(0, v)];
+                    const T dfy = Yu[rot_index(1, v)] - Yd[rot_index(1, v)];
                     sxy[v] = dfx + dfy;
-                    fzm[v] = fz[v * G::NFZ + tid];
+                    fzm[v] = Fz[rot_index(2, v)];
                 }
             }
         }

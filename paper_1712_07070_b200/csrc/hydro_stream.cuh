@@ -308,6 +308,31 @@ __device__ __forceinline__ int riemann_plane(const T* es, const T* zprev, T* fx,
 }
 
 // ---------------------------------------------------------------------------------------------
+// face states / fluxes in shared memory as one 16-byte vector + NV-4 scalars
+// ---------------------------------------------------------------------------------------------
+template <typename T> struct alignas(16) Vec4 {
+    T a, b, c, d;
+};
+
+// five (six) values of one face <-> shared memory: one Vec4 + NV-4 scalars; n = entries of the array
+template <typename T, int NV>
+__device__ __forceinline__ void put_state(T* blk, int n, int idx, const T* W) {
+    Vec4<T> q;
+    q.a = W[0]; q.b = W[1]; q.c = W[2]; q.d = W[3];
+    reinterpret_cast<Vec4<T>*>(blk)[idx] = q;
+#pragma unroll
+    for (int v = 4; v < NV; ++v) blk[v * n + idx] = W[v];
+}
+template <typename T, int NV>
+__device__ __forceinline__ void get_state(const T* blk, int n, int idx, T* W) {
+    const Vec4<T> q = reinterpret_cast<const Vec4<T>*>(blk)[idx];
+    W[0] = q.a; W[1] = q.b; W[2] = q.c; W[3] = q.d;
+#pragma unroll
+    for (int v = 4; v < NV; ++v) W[v] = blk[v * n + idx];
+}
+
+
+// ---------------------------------------------------------------------------------------------
 // Rotated storage (used by the MHM kernel): a face-state array of axis d holds (rho, v_d, v_{d+1},
 // v_{d+2}, P [, q]) -- the producer rotates at compile time -- and the flux array holds the rotated flux,
 // so the Riemann stage needs no per-face rotation arithmetic.  Face f of the flat list (x: 17*TY, y:

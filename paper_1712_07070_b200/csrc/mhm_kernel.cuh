@@ -23,10 +23,6 @@
 
 namespace gamer {
 
-template <typename T> struct alignas(16) Vec4 {
-    T a, b, c, d;
-};
-
 template <typename T, int RECON, int NV, int TY, int NSTG = 2, bool FUSED = false> struct MhmGeo {
     static constexpr int R = RECON == PPM ? 2 : 1;
     static constexpr int RING = 2 * R + 2;
@@ -49,24 +45,6 @@ template <typename T, int RECON, int NV, int TY, int NSTG = 2, bool FUSED = fals
                                                                 // first; neighbour table and copy list last
     static_assert((NV * PLN) % 4 == 0 && NSX % 4 == 0 && NSY % 4 == 0, "16-byte alignment of the Vec4 arrays");
 };
-
-// five (six) values of one face <-> shared memory: one Vec4 + NV-4 scalars; n = entries of the array
-template <typename T, int NV>
-__device__ __forceinline__ void put_state(T* blk, int n, int idx, const T* W) {
-    Vec4<T> q;
-    q.a = W[0]; q.b = W[1]; q.c = W[2]; q.d = W[3];
-    reinterpret_cast<Vec4<T>*>(blk)[idx] = q;
-#pragma unroll
-    for (int v = 4; v < NV; ++v) blk[v * n + idx] = W[v];
-}
-template <typename T, int NV>
-__device__ __forceinline__ void get_state(const T* blk, int n, int idx, T* W) {
-    const Vec4<T> q = reinterpret_cast<const Vec4<T>*>(blk)[idx];
-    W[0] = q.a; W[1] = q.b; W[2] = q.c; W[3] = q.d;
-#pragma unroll
-    for (int v = 4; v < NV; ++v) W[v] = blk[v * n + idx];
-}
-
 
 // ---------------------------------------------------------------------------------------------
 // predictor pieces (DESIGN R6)
