@@ -240,74 +240,6 @@ __device__ __forceinline__ void face_values5(T l2, T l1, T c, T r1, T r2, T& wm,
 }
 
 // ---------------------------------------------------------------------------------------------
-// final Riemann pass over the faces of one plane of the tile (x- and y-faces of plane kk, z-faces
-// between planes kk-1 and kk).  States are primitive; es = [5][NV][EPL] (x-,x+,y-,y+,z-),
-// zprev = [NV][16*TY] (z+ of plane kk-1).  Writes fx/fy/fz and the patch-boundary planes of flux_out.
-// ---------------------------------------------------------------------------------------------
-template <typename T, int SOLVER, int NV, int TY, int NT = Geo<TY>::NT>
-__device__ __forceinline__ int riemann_plane(const T* es, const T* zprev, T* fx, T* fy, T* fz, T* gflux,
-                                             int kk, int j0, const Phys<T>& ph, int tid) {
-    using G = Geo<TY>;
-    int nfb = 0;
-    const int f_lo = (kk >= 0 && kk < PS) ? 0 : G::NFX + G::NFY;
-    const int f_hi = (kk >= 0 && kk <= PS) ? G::NF : 0;
-    for (int f = f_lo + tid; f < f_hi; f += NT) {
-        int d, lidx, ridx, lstr, fidx, fstr, gp, ga, gb;
-        const T *lp, *rp;
-        T* fp;
-        if (f < G::NFX) {
-            const int jj = f / 17, ii = f - jj * 17;
-            d = 0;
-            lp = es + 1 * NV * G::EPL; lidx = (jj + 1) * G::EW + ii; lstr = G::EPL;
-            rp = es + 0 * NV * G::EPL; ridx = lidx + 1;
-            fp = fx; fidx = f; fstr = G::NFX;
-            gp = ii; ga = j0 + jj; gb = kk;
-        } else if (f < G::NFX + G::NFY) {
-            const int g = f - G::NFX;
-            const int jj = g >> 4, ii = g & 15;
-            d = 1;
-            lp = es + 3 * NV * G::EPL; lidx = jj * G::EW + ii + 1; lstr = G::EPL;
-            rp = es + 2 * NV * G::EPL; ridx = lidx + G::EW;
-            fp = fy; fidx = g; fstr = G::NFY;
-            gp = j0 + jj; ga = ii; gb = kk;
-        } else {
-            const int g = f - G::NFX - G::NFY;
-            const int jj = g >> 4, ii = g & 15;
-            d = 2;
-            lp = zprev; lidx = g; lstr = G::NFZ;
-            rp = es + 4 * NV * G::EPL; ridx = (jj + 1) * G::EW + ii + 1;
-            fp = fz; fidx = g; fstr = G::NFZ;
-            gp = kk; ga = ii; gb = j0 + jj;
-        }
-        const int cn = 1 + d, c1 = 1 + (d + 1) % 3, c2 = 1 + (d + 2) % 3;
-        T WL[NV], WR[NV], F[NV];
-        WL[0] = lp[lidx];                 WR[0] = rp[ridx];
-        WL[1] = lp[cn * lstr + lidx];     WR[1] = rp[cn * G::EPL + ridx];
-        WL[2] = lp[c1 * lstr + lidx];     WR[2] = rp[c1 * G::EPL + ridx];
-        WL[3] = lp[c2 * lstr + lidx];     WR[3] = rp[c2 * G::EPL + ridx];
-        WL[4] = lp[4 * lstr + lidx];      WR[4] = rp[4 * G::EPL + ridx];
-        if (NV > 5) { WL[NV - 1] = lp[(NV - 1) * lstr + lidx]; WR[NV - 1] = rp[(NV - 1) * G::EPL + ridx]; }
-        nfb += riemann_flux<T, SOLVER, NV>(WL, WR, F, ph) ? 1 : 0;
-        fp[fidx] = F[0];
-        fp[cn * fstr + fidx] = F[1];
-        fp[c1 * fstr + fidx] = F[2];
-        fp[c2 * fstr + fidx] = F[3];
-        fp[4 * fstr + fidx] = F[4];
-        if (NV > 5) fp[(NV - 1) * fstr + fidx] = F[NV - 1];
-        if (gflux != nullptr && (gp & 7) == 0) {   // faces 0, 8, 16 of the axis: patch boundaries (L112)
-            T* q = gflux + ((size_t)(d * 3 + (gp >> 3)) * NV) * (PS * PS) + gb * PS + ga;
-            q[0] = F[0];
-            q[(size_t)cn * (PS * PS)] = F[1];
-            q[(size_t)c1 * (PS * PS)] = F[2];
-            q[(size_t)c2 * (PS * PS)] = F[3];
-            q[(size_t)4 * (PS * PS)] = F[4];
-            if (NV > 5) q[(size_t)(NV - 1) * (PS * PS)] = F[NV - 1];
-        }
-    }
-    return nfb;
-}
-
-// ---------------------------------------------------------------------------------------------
 // face states / fluxes in shared memory as one 16-byte vector + NV-4 scalars
 // ---------------------------------------------------------------------------------------------
 template <typename T> struct alignas(16) Vec4 {
@@ -333,68 +265,11 @@ __device__ __forceinline__ void get_state(const T* blk, int n, int idx, T* W) {
 
 
 // ---------------------------------------------------------------------------------------------
-// Rotated storage (used by the MHM kernel): a face-state array of axis d holds (rho, v_d, v_{d+1},
-// v_{d+2}, P [, q]) -- the producer rotates at compile time -- and the flux array holds the rotated flux,
-// so the Riemann stage needs no per-face rotation arithmetic.  Face f of the flat list (x: 17*TY, y:
-// 16*(TY+1), z: 16*TY) reads its left / right state at offsets lo / ro from `es` (variable stride EPL)
-// and writes F[k*NF + f].  rot_index(d, v) = position of natural variable v in the rotation of axis d.
+// Rotated storage: a face-state array of axis d holds (rho, v_d, v_{d+1}, v_{d+2}, P [, q]) -- the producer rotates
+// at compile time -- so the Riemann stage needs no per-face rotation arithmetic.
+// rot_index(d, v) = position of natural variable v in the rotation of axis d; nat_index is its inverse.
 // ---------------------------------------------------------------------------------------------
 __host__ __device__ constexpr int rot_index(int d, int v) { return (v >= 1 && v <= 3) ? 1 + ((v - 1 - d + 3) % 3) : v; }
 __host__ __device__ constexpr int nat_index(int d, int k) { return (k >= 1 && k <= 3) ? 1 + ((k - 1 + d) % 3) : k; }
-
-// packed (lo | ro << 16) descriptor of face f; z faces get lo relative to the z+ buffer of parity 0
-template <int NV, int TY>
-__device__ __forceinline__ unsigned face_descriptor(int f, int zp_off) {
-    using G = Geo<TY>;
-    int lo, ro;
-    if (f < G::NFX) {
-        const int jj = f / 17, ii = f - jj * 17;
-        lo = 1 * NV * G::EPL + (jj + 1) * G::EW + ii;
-        ro = 0 * NV * G::EPL + (jj + 1) * G::EW + ii + 1;
-    } else if (f < G::NFX + G::NFY) {
-        const int g = f - G::NFX;
-        const int jj = g >> 4, ii = g & 15;
-        lo = 3 * NV * G::EPL + jj * G::EW + ii + 1;
-        ro = 2 * NV * G::EPL + (jj + 1) * G::EW + ii + 1;
-    } else {
-        const int g = f - G::NFX - G::NFY;
-        const int jj = g >> 4, ii = g & 15;
-        lo = zp_off + (jj + 1) * G::EW + ii + 1;
-        ro = 4 * NV * G::EPL + (jj + 1) * G::EW + ii + 1;
-    }
-    return (unsigned)lo | ((unsigned)ro << 16);
-}
-
-template <typename T, int SOLVER, int NV, int TY>
-__device__ __forceinline__ int riemann_face_rot(const T* es, T* fl, T* gflux, unsigned desc, int f, int zpar_off,
-                                                int kk, int j0, const Phys<T>& ph) {
-    using G = Geo<TY>;
-    const bool isz = f >= G::NFX + G::NFY;
-    const int lo = (int)(desc & 0xffffu) + (isz ? zpar_off : 0);
-    const int ro = (int)(desc >> 16);
-    T WL[NV], WR[NV], F[NV];
-#pragma unroll
-    for (int k = 0; k < NV; ++k) { WL[k] = es[k * G::EPL + lo]; WR[k] = es[k * G::EPL + ro]; }
-    const int fb = riemann_flux<T, SOLVER, NV>(WL, WR, F, ph) ? 1 : 0;
-#pragma unroll
-    for (int k = 0; k < NV; ++k) fl[k * G::NF + f] = F[k];
-    if (gflux != nullptr) {   // faces 0, 8, 16 of the axis are patch boundaries
-        int d, gp, ga, gb;
-        if (f < G::NFX) { const int jj = f / 17, ii = f - jj * 17; d = 0; gp = ii; ga = j0 + jj; gb = kk; }
-        else if (!isz) { const int g = f - G::NFX; d = 1; gp = j0 + (g >> 4); ga = g & 15; gb = kk; }
-        else { const int g = f - G::NFX - G::NFY; d = 2; gp = kk; ga = g & 15; gb = j0 + (g >> 4); }
-        if ((gp & 7) == 0) {
-            T* q = gflux + ((size_t)(d * 3 + (gp >> 3)) * NV) * (PS * PS) + gb * PS + ga;
-            const int cn = 1 + d, c1 = 1 + (d + 1) % 3, c2 = 1 + (d + 2) % 3;
-            q[0] = F[0];
-            q[(size_t)cn * (PS * PS)] = F[1];
-            q[(size_t)c1 * (PS * PS)] = F[2];
-            q[(size_t)c2 * (PS * PS)] = F[3];
-            q[(size_t)4 * (PS * PS)] = F[4];
-            if (NV > 5) q[(size_t)(NV - 1) * (PS * PS)] = F[NV - 1];
-        }
-    }
-    return fb;
-}
 
 }  // namespace gamer
