@@ -21,6 +21,7 @@
 #pragma once
 #include "hydro_close.cuh"
 
+
 namespace gamer {
 
 template <typename T, int RECON, int NV, int TY, int NSTG = 2, bool FUSED = false> struct MhmGeo {
@@ -102,22 +103,19 @@ __device__ __forceinline__ void mhm_face_states(const T* const* Pz, const Phys<T
     }
 }
 
-// Hancock half step of one face state.  full: evolved primitives -> We (floors applied in extended mode);
-// !full: only the positivity of the evolved state is tested (no division), We is left untouched.  A state
-// that no Riemann solver of this thread consumes still decides the revert of R6.  floors = false in the
-// reverting pass (the un-evolved face values are taken as they are).
+// Hancock half step of one face state: evolved primitives -> We (floors applied in extended mode, not in the
+// reverting pass, where the un-evolved face values are taken as they are); returns whether rho and P are positive.
+// Every thread evolves all six states of its cell, also the ones it hands to no Riemann solver: any bad state
+// reverts the cell (R6), the halo copy of a cell must decide exactly as its owner in the neighbouring group does, and
+// six straight-line conversions without per-state branches are faster than division-free tests of the unused ones.
 template <typename T, int NV, bool EXT>
-__device__ __forceinline__ bool mhm_evolve(const T* Uf, const T* dU, T* We, bool full, bool floors, const Phys<T>& ph) {
+__device__ __forceinline__ bool mhm_evolve(const T* Uf, const T* dU, T* We, bool floors, const Phys<T>& ph) {
     T Ue[NV];
 #pragma unroll
     for (int v = 0; v < NV; ++v) Ue[v] = Uf[v] - ph.hlam * dU[v];
-    if (full || (EXT && ph.floors)) {
-        cons2prim<T, NV>(Ue, We, ph);
-        if (EXT && ph.floors && floors) floor_prim(We, ph);
-        return (We[0] > T(0)) && (We[4] > T(0));
-    }
-    const T pe = Ue[0] * Ue[4] - T(0.5) * (Ue[1] * Ue[1] + Ue[2] * Ue[2] + Ue[3] * Ue[3]);
-    return (Ue[0] > T(0)) && (pe > T(0));
+    cons2prim<T, NV>(Ue, We, ph);
+    if (EXT && ph.floors && floors) floor_prim(We, ph);
+    return (We[0] > T(0)) && (We[4] > T(0));
 }
 
 // per-thread constants of the cell column this thread owns
@@ -262,30 +260,30 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED>::NT), M
                     for (int v = 0; v < NV; ++v) dU[v] = T(0);
                 }
                 const bool fl_ok = pass == 0;
-                bool ok = mhm_evolve<T, NV, EXT>(Uf[0][1], dU, We, mid && pub_x, fl_ok, ph);
+                bool ok = mhm_evolve<T, NV, EXT>(Uf[0][1], dU, We, fl_ok, ph);
                 if (mid && pub_x) {
                     T rot[NV];
 #pragma unroll
                     for (int k = 0; k < NV; ++k) rot[k] = We[nat_index(0, k)];
                     put_state<T, NV>(st_x, G::NSX, c.sx_own + 1, rot);
                 }
-                ok = mhm_evolve<T, NV, EXT>(Uf[1][1], dU, We, mid && pub_y, fl_ok, ph) && ok;
+                ok = mhm_evolve<T, NV, EXT>(Uf[1][1], dU, We, fl_ok, ph) && ok;
                 if (mid && pub_y) {
                     T rot[NV];
 #pragma unroll
                     for (int k = 0; k < NV; ++k) rot[k] = We[nat_index(1, k)];
                     put_state<T, NV>(st_y, G::NSY, c.sy_own + 16, rot);
                 }
-                ok = mhm_evolve<T, NV, EXT>(Uf[0][0], dU, We, mid && own_x, fl_ok, ph) && ok;
+                ok = mhm_evolve<T, NV, EXT>(Uf[0][0], dU, We, fl_ok, ph) && ok;
 #pragma unroll
                 for (int k = 0; k < NV; ++k) xminus[k] = We[nat_index(0, k)];
-                ok = mhm_evolve<T, NV, EXT>(Uf[1][0], dU, We, mid && own_y, fl_ok, ph) && ok;
+                ok = mhm_evolve<T, NV, EXT>(Uf[1][0], dU, We, fl_ok, ph) && ok;
 #pragma unroll
                 for (int k = 0; k < NV; ++k) yminus[k] = We[nat_index(1, k)];
-                ok = mhm_evolve<T, NV, EXT>(Uf[2][0], dU, We, interior && kk >= 0, fl_ok, ph) && ok;
+                ok = mhm_evolve<T, NV, EXT>(Uf[2][0], dU, We, fl_ok, ph) && ok;
 #pragma unroll
                 for (int k = 0; k < NV; ++k) zminus[k] = We[nat_index(2, k)];
-                ok = mhm_evolve<T, NV, EXT>(Uf[2][1], dU, We, interior && kk < PS, fl_ok, ph) && ok;
+                ok = mhm_evolve<T, NV, EXT>(Uf[2][1], dU, We, fl_ok, ph) && ok;
 #pragma unroll
                 for (int k = 0; k < NV; ++k) znew[k] = We[nat_index(2, k)];
                 if (ok || pass) break;
