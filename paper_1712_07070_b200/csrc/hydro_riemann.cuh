@@ -73,24 +73,29 @@ __device__ __forceinline__ void solve_hllc(const Side<T>& L, const Side<T>& R, c
     const T cr = Ops<T>::sqrt(ph.gamma * R.P * Ops<T>::rcp(R.rho));
     const T SL = Ops<T>::min(r.u - r.a, L.u - cl);
     const T SR = Ops<T>::max(r.u + r.a, R.u + cr);
-    if (SL >= T(0)) { side_flux(L, F); return; }
-    if (SR <= T(0)) { side_flux(R, F); return; }
+    // branch-free: the star-region flux of the side the axis lies on is always formed; in the supersonic cases
+    // (S_L >= 0: side L, S_R <= 0: side R) its correction term is switched off, which leaves F = F_K exactly
     const T ml = L.rho * (SL - L.u), mr = R.rho * (SR - R.u);
     const T SS = (R.P - L.P + L.u * ml - R.u * mr) * Ops<T>::rcp(ml - mr);
-    const bool left = SS >= T(0);
-    const Side<T>& K = left ? L : R;
+    const bool supl = SL >= T(0), supr = SR <= T(0);
+    const bool left = supl || (!supr && SS >= T(0));
+    const T rho = left ? L.rho : R.rho, u = left ? L.u : R.u, v = left ? L.v : R.v, w = left ? L.w : R.w;
+    const T P = left ? L.P : R.P, E = left ? L.E : R.E;
+    const T m1 = left ? L.m1 : R.m1, m2 = left ? L.m2 : R.m2, m3 = left ? L.m3 : R.m3;
     const T SK = left ? SL : SR;
-    T FK[5];
-    side_flux(K, FK);
-    const T dk = SK - K.u;
-    const T fac = K.rho * dk * Ops<T>::rcp(SK - SS);
-    const T ir = Ops<T>::rcp(K.rho);
-    const T es = K.E * ir + (SS - K.u) * (SS + K.P * ir * Ops<T>::rcp(dk));
-    F[0] = FK[0] + SK * (fac - K.rho);
-    F[1] = FK[1] + SK * (fac * SS - K.m1);
-    F[2] = FK[2] + SK * (fac * K.v - K.m2);
-    F[3] = FK[3] + SK * (fac * K.w - K.m3);
-    F[4] = FK[4] + SK * (fac * es - K.E);
+    const T dk = SK - u;
+    const T fac = rho * dk * Ops<T>::rcp(SK - SS);
+    const T ir = Ops<T>::rcp(rho);
+    const T es = E * ir + (SS - u) * (SS + P * ir * Ops<T>::rcp(dk));
+    const T sk = (supl || supr) ? T(0) : SK;
+    const T c0 = (supl || supr) ? T(0) : fac - rho, c1 = (supl || supr) ? T(0) : fac * SS - m1;
+    const T c2 = (supl || supr) ? T(0) : fac * v - m2, c3 = (supl || supr) ? T(0) : fac * w - m3;
+    const T c4 = (supl || supr) ? T(0) : fac * es - E;
+    F[0] = m1 + sk * c0;
+    F[1] = (m1 * u + P) + sk * c1;
+    F[2] = m2 * u + sk * c2;
+    F[3] = m3 * u + sk * c3;
+    F[4] = u * (E + P) + sk * c4;
 }
 
 // Roe (1981), no entropy fix.  Returns true if remedy (i) (L104) must be taken.
@@ -102,7 +107,9 @@ __device__ __forceinline__ void solve_hllc(const Side<T>& L, const Side<T>& R, c
 template <typename T>
 __device__ __forceinline__ bool solve_roe(const Side<T>& L, const Side<T>& R, const RoeAvg<T>& r, T* F,
                                           const Phys<T>& ph) {
-    if (!(r.a2 > T(0))) return true;
+    // no early exit: the flux is formed unconditionally (garbage where the solver does not apply, then replaced by
+    // the caller), which leaves one branch per solve instead of three
+    bool bad = !(r.a2 > T(0));
     const T d0 = R.rho - L.rho, d1 = R.m1 - L.m1, d2 = R.m2 - L.m2, d3 = R.m3 - L.m3, d4 = R.E - L.E;
     const T u = r.u, v = r.v, w = r.w, H = r.H, a = r.a;
     const T a3 = d2 - v * d0;
@@ -121,7 +128,7 @@ __device__ __forceinline__ bool solve_roe(const Side<T>& L, const Side<T>& R, co
         // P > 0  <=>  rho*E - |m|^2/2 > 0 when rho > 0
         const T p1 = r1 * e1 - T(0.5) * (n1 * n1 + s1 * s1 + t1 * t1);
         const T p5 = r5 * e5 - T(0.5) * (n5 * n5 + s5 * s5 + t5 * t5);
-        if (!(r1 > T(0)) || !(r5 > T(0)) || !(p1 > T(0)) || !(p5 > T(0))) return true;
+        bad = bad || !(r1 > T(0)) || !(r5 > T(0)) || !(p1 > T(0)) || !(p5 > T(0));
     }
     const bool pos = u >= T(0);
     const T rho = pos ? L.rho : R.rho, un = pos ? L.u : R.u, P = pos ? L.P : R.P, E = pos ? L.E : R.E;
@@ -135,7 +142,7 @@ __device__ __forceinline__ bool solve_roe(const Side<T>& L, const Side<T>& R, co
     F[2] = m2 * un + cf * v;
     F[3] = m3 * un + cf * w;
     F[4] = un * (E + P) + cf * K4;
-    return false;
+    return bad;
 }
 
 // Exact solver ("exact solver based on Toro (2009)", reading R21): star pressure by Newton-Raphson on
