@@ -113,6 +113,83 @@ __device__ __forceinline__ int ctu_final_pass(const T* es, const T* zprev, T* fx
     return nfb;
 }
 
+// One work list for the two Riemann passes that share a phase: the first-pass x / y faces of plane kk (states tcur ->
+// f1x, f1y) followed by the final-pass faces of plane m = kk-1 (corrected states tprev, zprev -> fx, fy, fz and flux_out).
+// A single list keeps all threads busy for ceil(total / NT) rounds instead of ceil(n1 / NT) + ceil(n2 / NT), and a single
+// call site keeps one copy of the solver in the instruction stream.
+template <typename T, int RECON, int SOLVER, int NV, int TY, int NT, bool FUSED>
+__device__ __forceinline__ int ctu_riemann_phase(const T* tcur, const T* tprev, const T* zprev, T* f1x, T* f1y, T* fx, T* fy,
+                                                 T* fz, T* gflux, int kk, int j0, const Phys<T>& ph, int tid) {
+    using G = Geo<TY>;
+    using S = CtuSmem<T, RECON, NV, TY, FUSED>;
+    constexpr int SB = NV * G::EPL, EW = G::EW;
+    const int m = kk - 1;
+    const int n1 = kk <= PS ? S::NF1X + S::NF1Y : 0;
+    const int f_lo = (m >= 0 && m < PS) ? 0 : G::NFX + G::NFY;
+    const int f_hi = (m >= 0 && m <= PS) ? G::NF : f_lo;
+    int nfb = 0;
+    for (int it = tid; it < n1 + (f_hi - f_lo); it += NT) {
+        int d, lidx, ridx, ln, fidx, fn, gp = 1, ga = 0, gb = 0;
+        const T *lp, *rp;
+        T* fp;
+        if (it < S::NF1X && it < n1) {                      // first pass, x face of plane kk
+            const int ej = it / 17, ei = it - ej * 17;
+            d = 0;
+            lp = tcur + 1 * SB; lidx = ej * EW + ei; ln = G::EPL;
+            rp = tcur + 0 * SB; ridx = lidx + 1;
+            fp = f1x; fidx = it; fn = S::NF1XP;
+        } else if (it < n1) {                               // first pass, y face
+            const int u = it - S::NF1X;
+            d = 1;
+            lp = tcur + 3 * SB; lidx = u; ln = G::EPL;
+            rp = tcur + 2 * SB; ridx = u + EW;
+            fp = f1y; fidx = u; fn = S::NF1YP;
+        } else {                                            // final pass of plane m
+            const int f = it - n1 + f_lo;
+            if (f < G::NFX) {
+                const int jj = f / 17, ii = f - jj * 17;
+                d = 0;
+                lp = tprev + 1 * SB; lidx = (jj + 1) * EW + ii; ln = G::EPL;
+                rp = tprev + 0 * SB; ridx = lidx + 1;
+                fp = fx; fidx = f; fn = G::NFX;
+                gp = ii; ga = j0 + jj; gb = m;
+            } else if (f < G::NFX + G::NFY) {
+                const int g = f - G::NFX;
+                const int jj = g >> 4, ii = g & 15;
+                d = 1;
+                lp = tprev + 3 * SB; lidx = jj * EW + ii + 1; ln = G::EPL;
+                rp = tprev + 2 * SB; ridx = lidx + EW;
+                fp = fy; fidx = g; fn = G::NFY;
+                gp = j0 + jj; ga = ii; gb = m;
+            } else {
+                const int g = f - G::NFX - G::NFY;
+                const int jj = g >> 4, ii = g & 15;
+                d = 2;
+                lp = zprev; lidx = g; ln = G::NFZ;
+                rp = tprev + 4 * SB; ridx = (jj + 1) * EW + ii + 1;
+                fp = fz; fidx = g; fn = G::NFZ;
+                gp = m; ga = ii; gb = j0 + jj;
+            }
+        }
+        T WL[NV], WR[NV], F[NV];
+        get_state<T, NV>(lp, ln, lidx, WL);
+        get_state<T, NV>(rp, G::EPL, ridx, WR);
+        nfb += riemann_flux<T, SOLVER, NV>(WL, WR, F, ph) ? 1 : 0;
+        put_state<T, NV>(fp, fn, fidx, F);
+        if (gflux != nullptr && it >= n1 && (gp & 7) == 0) {   // final pass on faces 0, 8, 16: patch boundaries (L112)
+            const int cn = 1 + d, c1 = 1 + (d + 1) % 3, c2 = 1 + (d + 2) % 3;
+            T* q = gflux + ((size_t)(d * 3 + (gp >> 3)) * NV) * (PS * PS) + gb * PS + ga;
+            q[0] = F[0];
+            q[(size_t)cn * (PS * PS)] = F[1];
+            q[(size_t)c1 * (PS * PS)] = F[2];
+            q[(size_t)c2 * (PS * PS)] = F[3];
+            q[(size_t)4 * (PS * PS)] = F[4];
+            if (NV > 5) q[(size_t)(NV - 1) * (PS * PS)] = F[NV - 1];
+        }
+    }
+    return nfb;
+}
+
 // T stage for one cell t of the 18 x (TY+2) face-state plane and one direction D: PLM/PPM face values of
 // every variable along D, characteristic tracing over dt/2 (R7), revert of an unphysical pair (R8), store.
 template <typename T, int RECON, int NV, bool EXT, int TY, int D>
@@ -348,19 +425,25 @@ __global__ void __launch_bounds__(NT) ctu_kernel(const AdvArgs<T> a) {
         }
         __syncthreads();
         // ------------------------------------------------------------------ R1xy(kk) + R2(kk-1)
-        if (kk <= PS) {
-            for (int t = tid; t < S::NF1X + S::NF1Y; t += NT) {
-                if (t < S::NF1X) {
-                    const int ej = t / 17, ei = t - ej * 17;
-                    const int l = ej * EW + ei;
-                    cnt.roe_fb += first_pass_face<T, SOLVER, NV>(tcur + 1 * NV * EPL, l, tcur + 0 * NV * EPL, l + 1, EPL, f1x, t, S::NF1XP, ph);
-                } else {
-                    const int u = t - S::NF1X;      // = ej*18 + ei, ej in [0, EH-1)
-                    cnt.roe_fb += first_pass_face<T, SOLVER, NV>(tcur + 3 * NV * EPL, u, tcur + 2 * NV * EPL, u + EW, EPL, f1y, u, S::NF1YP, ph);
+        if constexpr (sizeof(T) == 8) {
+            // fp64 (fewer threads per CTA): one work list for both passes, see ctu_riemann_phase (+8 %; -1 % in fp32)
+            cnt.roe_fb += ctu_riemann_phase<T, RECON, SOLVER, NV, TY, NT, FUSED>(tcur, tprev, zp + ((m + 1) & 1) * NV * G::NFZ, f1x,
+                                                                               f1y, fx, fy, fz, gflux, kk, j0, ph, tid);
+        } else {
+            if (kk <= PS) {
+                for (int t = tid; t < S::NF1X + S::NF1Y; t += NT) {
+                    if (t < S::NF1X) {
+                        const int ej = t / 17, ei = t - ej * 17;
+                        const int l = ej * EW + ei;
+                        cnt.roe_fb += first_pass_face<T, SOLVER, NV>(tcur + 1 * NV * EPL, l, tcur + 0 * NV * EPL, l + 1, EPL, f1x, t, S::NF1XP, ph);
+                    } else {
+                        const int u = t - S::NF1X;      // = ej*18 + ei, ej in [0, EH-1)
+                        cnt.roe_fb += first_pass_face<T, SOLVER, NV>(tcur + 3 * NV * EPL, u, tcur + 2 * NV * EPL, u + EW, EPL, f1y, u, S::NF1YP, ph);
+                    }
                 }
             }
+            if (m >= 0) cnt.roe_fb += ctu_final_pass<T, SOLVER, NV, TY, NT>(tprev, zp + ((m + 1) & 1) * NV * G::NFZ, fx, fy, fz, gflux, m, j0, ph, tid);
         }
-        if (m >= 0) cnt.roe_fb += ctu_final_pass<T, SOLVER, NV, TY, NT>(tprev, zp + ((m + 1) & 1) * NV * G::NFZ, fx, fy, fz, gflux, m, j0, ph, tid);
         __syncthreads();
         // ------------------------------------------------------------------ U(kk-2)
         {
