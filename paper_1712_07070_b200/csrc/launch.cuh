@@ -1,4 +1,6 @@
 // launch.cuh -- host-side launch helpers: tile height selection by shared-memory fit, attribute setup.
+// MHM_TY_OVERRIDE, MHM_FORCE_NSTG2, CTU_TY_OVERRIDE, CTU_NT_OVERRIDE are tuning hooks for experiments
+// (GAMER_EXTRA_DEFS of build.py); the shipped library is built without them.
 #pragma once
 #include <cstdlib>
 #include "mhm_kernel.cuh"
