@@ -95,6 +95,9 @@ def reference_arm(args):
     """The fp64 CPU oracle, as it stands, on a bounded sample of the same workload (rank 0 only)."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
+    # torchrun pins OMP_NUM_THREADS=1 for its workers; only this rank works, so it takes all host cores (set before
+    # the OpenMP runtime is loaded with torch / the oracle library)
+    os.environ["OMP_NUM_THREADS"] = str(os.cpu_count())
     import numpy as np
     import torch
     import oracle
@@ -108,7 +111,7 @@ def reference_arm(args):
     p = padded.numpy()
     dh = 1.0 / 512
     dt = oracle.cfl_dt(inputs.interior(padded).contiguous().numpy(), dh, 5.0 / 3.0, 0.4, scheme)[0]
-    cores = os.cpu_count()
+    cores = int(os.environ["OMP_NUM_THREADS"])
     for _ in range(max(1, min(args.warmup, 1))):
         oracle.fluid_advance(p, dt, dh, 5.0 / 3.0, scheme, recon, solver)
     t0 = time.perf_counter()
@@ -352,7 +355,7 @@ def main():
     roofline["kernel_ms"] = kern_ms
 
     cpu = None
-    if not args.no_cpu:
+    if not args.no_cpu and world == 1:       # the oracle beside it: rank 0 at N = 1 only
         import oracle
         ns = 1024
         sample = u_in[:ns].to(torch.float64).cpu().numpy()
@@ -365,7 +368,8 @@ def main():
             oracle.cfl_dt(r["out"], dh, gamma, cfl, scheme)
             reps += 1
         el = time.perf_counter() - t0
-        cpu = {"value": ns * CELLS * reps / el, "unit": "cells/s", "cores": os.cpu_count(), "kind": "oracle",
+        cpu = {"value": ns * CELLS * reps / el, "unit": "cells/s", "cores": int(os.environ.get("OMP_NUM_THREADS") or os.cpu_count()),
+               "kind": "oracle",
                "sample": f"first {ns} of {args.groups} patch groups, {reps} passes, OpenMP over groups"}
 
     line = {"metric": "hydro cell-updates/sec", "value": value, "unit": "cells/s", "n_gpus": world,
