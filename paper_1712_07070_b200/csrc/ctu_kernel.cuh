@@ -431,15 +431,14 @@ __global__ void __launch_bounds__(NT) ctu_kernel(const AdvArgs<T> a) {
                                                                                f1y, fx, fy, fz, gflux, kk, j0, ph, tid);
         } else {
             if (kk <= PS) {
-                for (int t = tid; t < S::NF1X + S::NF1Y; t += NT) {
-                    if (t < S::NF1X) {
-                        const int ej = t / 17, ei = t - ej * 17;
-                        const int l = ej * EW + ei;
-                        cnt.roe_fb += first_pass_face<T, SOLVER, NV>(tcur + 1 * NV * EPL, l, tcur + 0 * NV * EPL, l + 1, EPL, f1x, t, S::NF1XP, ph);
-                    } else {
-                        const int u = t - S::NF1X;      // = ej*18 + ei, ej in [0, EH-1)
-                        cnt.roe_fb += first_pass_face<T, SOLVER, NV>(tcur + 3 * NV * EPL, u, tcur + 2 * NV * EPL, u + EW, EPL, f1y, u, S::NF1YP, ph);
-                    }
+                for (int t = tid; t < S::NF1X + S::NF1Y; t += NT) {      // one call site for x and y faces
+                    const bool isx = t < S::NF1X;
+                    const int u = isx ? t : t - S::NF1X;              // x: ej*17 + ei;  y: ej*18 + ei, ej in [0, EH-1)
+                    const int ej = u / 17, ei = u - ej * 17;
+                    const int l = isx ? ej * EW + ei : u;
+                    cnt.roe_fb += first_pass_face<T, SOLVER, NV>(tcur + (isx ? 1 : 3) * NV * EPL, l, tcur + (isx ? 0 : 2) * NV * EPL,
+                                                                 isx ? l + 1 : l + EW, EPL, isx ? f1x : f1y, u,
+                                                                 isx ? S::NF1XP : S::NF1YP, ph);
                 }
             }
             if (m >= 0) cnt.roe_fb += ctu_final_pass<T, SOLVER, NV, TY, NT>(tprev, zp + ((m + 1) & 1) * NV * G::NFZ, fx, fy, fz, gflux, m, j0, ph, tid);
