@@ -50,7 +50,8 @@ enum {
     GAMER_EINVAL = -1,        /* NULL in/out, n_groups < 0, dt <= 0 or non-finite, dh <= 0, gamma <= 1,
                                  unknown enum, misaligned pointer                                  */
     GAMER_EUNSUPPORTED = -2,  /* valid arguments, combination not built                            */
-    GAMER_ECUDA = -3          /* CUDA runtime / launch error (cudaGetLastError)                    */
+    GAMER_ECUDA = -3,         /* CUDA runtime / launch error (cudaGetLastError)                    */
+    GAMER_EUNPHYSICAL = -4    /* gamer_fluid_advance_retry only: remedy (v) of L108 gave up at dt_min */
 };
 
 /* Everything the 11-argument form fixes by default.  Zero-initialise, then set what you need. */
@@ -85,6 +86,21 @@ int gamer_fluid_advance_ex(const void* in, void* out, void* flux_out, int64_t n_
                            double dt, double dh, double gamma,
                            int scheme, int recon, int riemann, int precision,
                            const gamer_opts* opts);
+
+/* Remedies (iv) and (v) of PAPER.md L107-108 around gamer_fluid_advance_ex: run the step; while the count of cells still
+ * unphysical after the in-kernel remedies (i), (ii) and the floors is not zero, "reduce the time-step by a fixed ratio
+ * (0.8 by default) and recalculate all patches" -- the whole batch again from the same `in` with dt <- dt * dt_ratio --
+ * "until no unphysical results are detected or reaching a given minimum time-step threshold": when the reduced dt falls
+ * below dt_min (or after 200 reductions) the call returns GAMER_EUNPHYSICAL, the caller's abort, with `out` holding the
+ * last attempt.  opts must be non-NULL with n_unphysical_out set (device int32; holds the last attempt's count on return)
+ * and dt_dev NULL; dt_ratio in (0,1), <= 0 = 0.8; dt_min >= 0.  *dt_used_host (nullable, HOST double) = the step of the
+ * last attempt = dt multiplied *n_retries_host (nullable, HOST int32) times by dt_ratio.  Unlike the other device entry
+ * points this one synchronises opts->stream after every attempt (it reads the count back). */
+int gamer_fluid_advance_retry(const void* in, void* out, void* flux_out, int64_t n_groups,
+                              double dt, double dh, double gamma,
+                              int scheme, int recon, int riemann, int precision,
+                              const gamer_opts* opts, double dt_ratio, double dt_min,
+                              double* dt_used_host, int32_t* n_retries_host);
 
 /* CFL time-step of an UNPADDED state u (the `out` layout): Eq. (2) for MHM, Eq. (1) for CTU.
  * *dt_out (device double) = cfl * dh / max speed.  group_speed_out nullable.

@@ -251,3 +251,25 @@ def fill_ghosts_table(u, nbr, padded):
                         continue
                     padded[g][:, rng[dz][0], rng[dy][0], rng[dx][0]] = u[s][:, rng[dz][1], rng[dy][1], rng[dx][1]]
     return padded
+
+
+def fluid_advance_retry(u_in, dt, dh, gamma, scheme, recon, riemann, opts=None, dt_ratio=0.8, dt_min=0.0,
+                        want_flux=True):
+    """Remedies (iv) and (v) of PAPER.md L107-108 around fluid_advance, in the paper's order: if any cell of the batch
+    is still unphysical after the in-solver remedies, "reduce the time-step by a fixed ratio (0.8 by default) and
+    recalculate all patches ... with this reduced time-step" (iv); "repeat step (iv) until no unphysical results are
+    detected or reaching a given minimum time-step threshold, for which the program is aborted" (v).  The whole batch is
+    recomputed from the same u_in each time.  Returns fluid_advance's dict plus "dt_used" and "n_retries"; raises
+    FloatingPointError (the abort) when the next reduced step would be below dt_min; after max 200 reductions too.
+    Reading (R23): the step of retry k is dt multiplied k times by dt_ratio (not dt * ratio**k), the
+    threshold test is dt_k < dt_min, taken before the attempt."""
+    n = 0
+    while True:
+        r = fluid_advance(u_in, dt, dh, gamma, scheme, recon, riemann, opts, want_flux)
+        if r["stats"]["n_unphysical"] == 0:
+            r["dt_used"], r["n_retries"] = dt, n
+            return r
+        dt = dt * dt_ratio
+        n += 1
+        if dt < dt_min or n > 200:
+            raise FloatingPointError(f"unphysical cells remain and the reduced time-step {dt} is below dt_min {dt_min}")

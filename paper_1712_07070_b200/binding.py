@@ -20,7 +20,7 @@ PS, NG, NP = 16, 3, 22
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libgamerhydro.so")
 
-EXPORTS = ["gamer_fluid_advance", "gamer_fluid_advance_ex", "gamer_cfl_dt", "gamer_cfl_dt_ex",
+EXPORTS = ["gamer_fluid_advance", "gamer_fluid_advance_ex", "gamer_fluid_advance_retry", "gamer_cfl_dt", "gamer_cfl_dt_ex",
            "gamer_cfl_from_group_speed", "gamer_refresh_ghosts_periodic", "gamer_refresh_ghosts", "gamer_refresh_ghosts_table", "gamer_fluid_advance_resident",
            "gamer_neighbors_periodic", "gamer_restrict", "gamer_flux_accumulate", "gamer_flux_correct",
            "gamer_fluid_advance_host", "gamer_release_scratch",
@@ -66,6 +66,8 @@ def lib():
         adv = [vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, ci, ci]
         L.gamer_fluid_advance.argtypes = adv
         L.gamer_fluid_advance_ex.argtypes = adv + [ctypes.POINTER(gamer_opts)]
+        L.gamer_fluid_advance_retry.argtypes = adv + [ctypes.POINTER(gamer_opts), dbl, dbl, ctypes.POINTER(dbl),
+                                                      ctypes.POINTER(ctypes.c_int32)]
         cfl = [vp, i64, dbl, dbl, dbl, ci, ci, vp, vp]
         L.gamer_cfl_dt.argtypes = cfl
         L.gamer_cfl_dt_ex.argtypes = cfl + [ctypes.POINTER(gamer_opts)]
@@ -144,6 +146,17 @@ def gamer_fluid_advance_ex(u_in, out, flux_out, dt, dh, gamma, scheme, recon, ri
     _check(lib().gamer_fluid_advance_ex(_ptr(u_in), _ptr(out), _ptr(flux_out), n, float(dt), float(dh), float(gamma),
                                         int(scheme), int(recon), int(riemann), _precision(u_in), ctypes.byref(opts)),
            "gamer_fluid_advance_ex")
+
+
+def gamer_fluid_advance_retry(u_in, out, flux_out, dt, dh, gamma, scheme, recon, riemann, opts, dt_ratio=0.8, dt_min=0.0):
+    """Remedies (iv)-(v).  Returns (dt_used, n_retries); GamerError(GAMER_EUNPHYSICAL) = the abort."""
+    n = u_in.shape[0]
+    dt_used, n_retries = ctypes.c_double(0.0), ctypes.c_int32(0)
+    _check(lib().gamer_fluid_advance_retry(_ptr(u_in), _ptr(out), _ptr(flux_out), n, float(dt), float(dh), float(gamma),
+                                           int(scheme), int(recon), int(riemann), _precision(u_in), ctypes.byref(opts),
+                                           float(dt_ratio), float(dt_min), ctypes.byref(dt_used),
+                                           ctypes.byref(n_retries)), "gamer_fluid_advance_retry")
+    return dt_used.value, n_retries.value
 
 
 def gamer_cfl_dt(u, dh, gamma, cfl, scheme, group_speed_out, dt_out, opts=None):

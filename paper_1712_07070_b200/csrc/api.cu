@@ -107,6 +107,33 @@ extern "C" int gamer_fluid_advance(const void* in, void* out, void* flux_out, in
                                   nullptr);
 }
 
+extern "C" int gamer_fluid_advance_retry(const void* in, void* out, void* flux_out, int64_t n_groups, double dt,
+                                         double dh, double gamma, int scheme, int recon, int riemann, int precision,
+                                         const gamer_opts* opts, double dt_ratio, double dt_min, double* dt_used_host,
+                                         int32_t* n_retries_host) {
+    if (!opts || !opts->n_unphysical_out || opts->dt_dev) return GAMER_EINVAL;
+    if (!(dt > 0.0) || !std::isfinite(dt) || !(dt_min >= 0.0) || !(dt_ratio < 1.0)) return GAMER_EINVAL;
+    if (!(dt_ratio > 0.0)) dt_ratio = 0.8;   // L107 "0.8 by default"
+    cudaStream_t st = static_cast<cudaStream_t>(opts->stream);
+    int32_t retries = 0;
+    for (;;) {
+        const int rc = gamer_fluid_advance_ex(in, out, flux_out, n_groups, dt, dh, gamma, scheme, recon, riemann,
+                                              precision, opts);
+        if (rc) return rc;
+        int32_t bad = 0;
+        if (n_groups > 0 &&
+            (cudaMemcpyAsync(&bad, opts->n_unphysical_out, sizeof(bad), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+             cudaStreamSynchronize(st) != cudaSuccess))
+            return GAMER_ECUDA;
+        if (dt_used_host) *dt_used_host = dt;
+        if (n_retries_host) *n_retries_host = retries;
+        if (bad == 0) return GAMER_OK;
+        dt *= dt_ratio;                      // remedy (iv): the whole batch again with the reduced step
+        ++retries;
+        if (dt < dt_min || retries > 200) return GAMER_EUNPHYSICAL;   // remedy (v): the caller's abort
+    }
+}
+
 extern "C" int gamer_fluid_advance_resident(const void* u, const int32_t* nbr, void* out, void* flux_out, int64_t n_groups,
                                             double dt, double dh, double gamma, int scheme, int recon, int riemann,
                                             int precision, const gamer_opts* opts) {
@@ -415,6 +442,7 @@ extern "C" const char* gamer_strerror(int code) {
     case GAMER_EINVAL: return "invalid argument";
     case GAMER_EUNSUPPORTED: return "unsupported combination or size";
     case GAMER_ECUDA: return "CUDA runtime or launch error";
+    case GAMER_EUNPHYSICAL: return "unphysical cells remain at the minimum time-step";
     default: return "unknown error code";
     }
 }

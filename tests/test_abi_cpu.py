@@ -85,6 +85,22 @@ def test_argument_validation_needs_no_gpu(built_lib):
     L.gamer_neighbors_periodic.argtypes = [vp, ci, ci, ci, vp]
     assert L.gamer_neighbors_periodic(None, 1, 1, 1, None) == -1
     assert L.gamer_neighbors_periodic(vp(4096), 0, 1, 1, None) == -1
+    # remedy (iv)/(v) driver: needs opts with the device counter, a host dt, a ratio below 1, dt_min >= 0
+    L.gamer_fluid_advance_retry.argtypes = [vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, ci, ci, ctypes.POINTER(gb.gamer_opts),
+                                            dbl, dbl, ctypes.POINTER(dbl), ctypes.POINTER(ctypes.c_int32)]
+    retry = lambda opts, ratio=0.8, dt_min=0.0, dt=0.1: L.gamer_fluid_advance_retry(
+        ok[0], ok[1], None, 1, dt, 0.1, 1.4, 1, 1, 1, 4, opts, ratio, dt_min, None, None)
+    assert retry(None) == -1
+    o2 = gb.gamer_opts()
+    assert retry(ctypes.byref(o2)) == -1                       # no n_unphysical_out
+    o2.n_unphysical_out = 32768
+    assert retry(ctypes.byref(o2), ratio=1.0) == -1
+    assert retry(ctypes.byref(o2), dt_min=-1.0) == -1
+    assert retry(ctypes.byref(o2), dt=0.0) == -1
+    o2.dt_dev = 65536
+    assert retry(ctypes.byref(o2)) == -1                       # dt must live on the host here
+    built_lib.gamer_strerror.restype = ctypes.c_char_p
+    assert b"unphysical" in built_lib.gamer_strerror(-4)
 
 
 def test_opts_struct_layout_matches_header():

@@ -384,3 +384,37 @@ def test_characteristic_variable_limiting(dev, oracle_mod, scheme, recon, solver
     assert fe <= 2 * tol
     base = gpu_ex(padded.to(dev), dt, dh, G53, scheme, recon, solver, **kw)[0]
     assert (base - out).abs().max().item() > 1e-3          # and it is not the primitive-variable result
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+def test_remedy_iv_v_retry_matches_oracle(dev, oracle_mod, dtype):
+    """gamer_fluid_advance_retry (remedies (iv), (v), L107-108) against oracle.fluid_advance_retry: Mach-3 turbulence with
+    5x the Eq. (2) step on 8 groups; the same number of reductions, the same accepted dt (bitwise: repeated
+    multiplication by 0.8 in double on both sides), the accepted result within the one-step tolerance; and the abort."""
+    f = inputs.turbulence_field(32, 3, kmax=6, gamma=G53, mach=3.0, sigma=1.0)
+    padded = inputs.pack_periodic(f).to(dtype)
+    p64 = padded.to(torch.float64)
+    dh = 1 / 32
+    dt0 = 5.0 * oracle_mod.cfl_dt(inputs.interior(p64).contiguous().numpy(), dh, G53, 0.5, gb.MHM)[0]
+    ref = oracle_mod.fluid_advance_retry(p64.numpy(), dt0, dh, G53, gb.MHM, gb.PLM, gb.ROE)
+    assert ref["n_retries"] >= 2
+    pd = padded.to(dev)
+    out, flux, speed = gb.alloc_outputs(pd)
+    nun = torch.zeros(1, dtype=torch.int32, device=dev)
+    o = gb.make_opts(group_speed_out=speed, n_unphysical_out=nun)
+    before = gb.gamer_launch_count()
+    dt_used, k = gb.gamer_fluid_advance_retry(pd, out, flux, dt0, dh, G53, gb.MHM, gb.PLM, gb.ROE, o)
+    assert gb.gamer_launch_count() - before >= k + 1            # every attempt is a kernel launch
+    assert int(nun.item()) == 0 and torch.isfinite(out).all()
+    assert k == ref["n_retries"] and dt_used == ref["dt_used"]
+    err = rel_l1(out.cpu().numpy(), ref["out"], G53)
+    assert max(err.values()) <= (1e-12 if dtype == torch.float64 else 1e-5), err
+    fe = np.abs(flux.cpu().numpy() - ref["flux"]).sum() / np.abs(ref["flux"]).sum()
+    assert fe <= (1e-12 if dtype == torch.float64 else 1e-5)
+    # remedy (v): threshold above the accepted step -> GAMER_EUNPHYSICAL, as the oracle's abort
+    with pytest.raises(FloatingPointError):
+        oracle_mod.fluid_advance_retry(p64.numpy(), dt0, dh, G53, gb.MHM, gb.PLM, gb.ROE, dt_min=1.01 * dt_used)
+    with pytest.raises(gb.GamerError, match="-4"):
+        gb.gamer_fluid_advance_retry(pd, out, flux, dt0, dh, G53, gb.MHM, gb.PLM, gb.ROE, o, dt_min=1.01 * dt_used)
+    assert int(nun.item()) > 0

@@ -169,3 +169,43 @@ def test_dual_energy_step_on_cold_supersonic_flow(oracle_mod):
     # entropy advected as a passive scalar of a pure contact: P from s stays 1 up to the scheme's
     # truncation error in rho^(gamma-1) q, far below the 1e-2 the ripple itself would give
     assert np.abs(pres_s - 1.0).max() < 5e-3
+
+
+def _retry_case(oracle_mod):
+    """Mach-3 turbulence advanced with 5x the CFL-0.5 step of Eq. (2): the first attempts leave negative pressures."""
+    f = inputs.turbulence_field(16, 3, kmax=6, gamma=G, mach=3.0, sigma=1.0)
+    p = inputs.pack_periodic(f).numpy()
+    dh = 1 / 16
+    dt0 = 5.0 * oracle_mod.cfl_dt(inputs.interior(inputs.pack_periodic(f)).contiguous().numpy(), dh, G, 0.5, MHM)[0]
+    return p, dt0, dh
+
+
+def test_remedy_iv_v_retry_loop(oracle_mod):
+    """Remedies (iv), (v) (L107-108), pinned by what the text fixes: the accepted step is dt0 * 0.8^k with k the SMALLEST
+    count whose attempt has no unphysical cell (every earlier attempt, recomputed here by direct calls, has some); the
+    result is the direct call at that step, from the same input; a physical first attempt is returned untouched with
+    k = 0; and the loop aborts once the reduced step falls below dt_min."""
+    p, dt0, dh = _retry_case(oracle_mod)
+    r = oracle_mod.fluid_advance_retry(p, dt0, dh, G, MHM, PLM, ROE)
+    k = r["n_retries"]
+    assert k >= 2 and r["stats"]["n_unphysical"] == 0
+    dt = dt0
+    for _ in range(k):
+        assert oracle_mod.fluid_advance(p, dt, dh, G, MHM, PLM, ROE)["stats"]["n_unphysical"] > 0
+        dt = dt * 0.8
+    assert r["dt_used"] == dt and abs(dt / dt0 - 0.8 ** k) < 1e-14
+    direct = oracle_mod.fluid_advance(p, dt, dh, G, MHM, PLM, ROE)
+    assert np.array_equal(direct["out"], r["out"]) and np.array_equal(direct["flux"], r["flux"])
+    uo = r["out"][0]
+    assert uo[0].min() > 0 and (uo[4] - 0.5 * (uo[1] ** 2 + uo[2] ** 2 + uo[3] ** 2) / uo[0]).min() > 0
+    # another ratio: fewer, larger reductions
+    r2 = oracle_mod.fluid_advance_retry(p, dt0, dh, G, MHM, PLM, ROE, dt_ratio=0.5)
+    assert 1 <= r2["n_retries"] < k and r2["dt_used"] == dt0 * 0.5 ** r2["n_retries"]
+    # physical first attempt
+    r0 = oracle_mod.fluid_advance_retry(p, dt0 / 5.0, dh, G, MHM, PLM, ROE)
+    assert r0["n_retries"] == 0 and r0["dt_used"] == dt0 / 5.0
+    assert np.array_equal(r0["out"], oracle_mod.fluid_advance(p, dt0 / 5.0, dh, G, MHM, PLM, ROE)["out"])
+    # (v): abort at the threshold -- the last allowed attempt is the largest dt0 * 0.8^j >= dt_min
+    with pytest.raises(FloatingPointError):
+        oracle_mod.fluid_advance_retry(p, dt0, dh, G, MHM, PLM, ROE, dt_min=dt * 1.01)
+    assert oracle_mod.fluid_advance_retry(p, dt0, dh, G, MHM, PLM, ROE, dt_min=dt * 0.99)["n_retries"] == k
