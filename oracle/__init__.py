@@ -273,3 +273,51 @@ def fluid_advance_retry(u_in, dt, dh, gamma, scheme, recon, riemann, opts=None, 
         n += 1
         if dt < dt_min or n > 200:
             raise FloatingPointError(f"unphysical cells remain and the reduced time-step {dt} is below dt_min {dt_min}")
+
+
+def interpolate_ghosts(coarse_padded, parent, nbr, fine_padded, coarse_padded_new=None, w=0.0, monotonic=False):
+    """Ghost zones of refined patch groups at coarse-fine boundaries, "interpolating from coarse patches",
+    with the "temporal interpolation" between the coarse level's two stored times (L482).  The paper names no spatial
+    scheme for the fluid; reading R24: conservative piecewise-linear interpolation of the conserved variables,
+        child = U_c + 1/4 * ((+-s_z) + (+-s_y)) + (+-s_x)),  sign + for the upper child along that axis,
+    s_d = (U_{c+e_d} - U_{c-e_d}) / 2 (monotonic=False) or minmod(U_c - U_{c-e_d}, U_{c+e_d} - U_c) (monotonic=True), so
+    that complete 2x2x2 sets of children average to U_c; U = (1-w) * coarse_padded + w * coarse_padded_new (linear in
+    time), or coarse_padded alone when coarse_padded_new is None.
+    coarse_padded [Gc,NV,22,22,22] (ghosts already filled); parent[g] = coarse group * 8 + octant (oz*4 + oy*2 + ox) that
+    fine group g refines; nbr [Gf,27] the fine level's same-level table: only slabs whose entry is < 0 are written;
+    fine_padded [Gf,NV,22,22,22] is modified in place and returned.  Fine cell i (= padded index - 3) along an axis lies
+    in coarse cell 8*o + floor(i/2) of the parent group and is its child number i mod 2."""
+    cp = np.asarray(coarse_padded, dtype=np.float64)
+    if coarse_padded_new is not None:
+        cp = (1.0 - w) * cp + w * np.asarray(coarse_padded_new, dtype=np.float64)
+    edges = {0: range(0, NG), 1: range(NG, NG + PS), 2: range(NG + PS, NP)}
+
+    def slope(lo, mid, hi):
+        if not monotonic:
+            return 0.5 * (hi - lo)
+        a, b = mid - lo, hi - mid
+        return np.where(a * b > 0.0, np.where(np.abs(a) < np.abs(b), a, b), 0.0)
+
+    for g in range(fine_padded.shape[0]):
+        cg, o = int(parent[g]) >> 3, int(parent[g]) & 7
+        oz, oy, ox = o >> 2, (o >> 1) & 1, o & 1
+        C = cp[cg]
+        for dz in range(3):
+            for dy in range(3):
+                for dx in range(3):
+                    s = (dz * 3 + dy) * 3 + dx
+                    if s == 13 or int(nbr[g, s]) >= 0:
+                        continue
+                    for pk in edges[dz]:
+                        qk, ak = 8 * oz + (pk - NG) // 2 + NG, (pk - NG) % 2
+                        for pj in edges[dy]:
+                            qj, aj = 8 * oy + (pj - NG) // 2 + NG, (pj - NG) % 2
+                            for pi in edges[dx]:
+                                qi, ai = 8 * ox + (pi - NG) // 2 + NG, (pi - NG) % 2
+                                u = C[:, qk, qj, qi]
+                                sz = slope(C[:, qk - 1, qj, qi], u, C[:, qk + 1, qj, qi])
+                                sy = slope(C[:, qk, qj - 1, qi], u, C[:, qk, qj + 1, qi])
+                                sx = slope(C[:, qk, qj, qi - 1], u, C[:, qk, qj, qi + 1])
+                                fine_padded[g, :, pk, pj, pi] = u + 0.25 * (((2 * ak - 1) * sz + (2 * aj - 1) * sy)
+                                                                            + (2 * ai - 1) * sx)
+    return fine_padded

@@ -220,3 +220,21 @@ def fixup_in_group_layout(restrict_fn, accumulate_fn, correct_fn):
         cg = correct_fn(cg, flux_c, acc, table.to(uc1.device), lam)
         return inputs.unpack(cg, *cdims)
     return fixup
+
+
+def region_neighbors(region):
+    """Same-level neighbour table [Gf, 27] (int32) of the fine groups of a box-shaped refined region: the group at
+    offset (dz, dy, dx), or -1 where that offset leaves the region (a coarse-fine boundary)."""
+    z0, z1, y0, y1, x0, x1 = region
+    fz, fy, fx = (z1 - z0) // 8, (y1 - y0) // 8, (x1 - x0) // 8
+    nbr = torch.full((fz * fy * fx, 27), -1, dtype=torch.int32)
+    for a in range(fz):
+        for b in range(fy):
+            for c in range(fx):
+                for dz in (-1, 0, 1):
+                    for dy in (-1, 0, 1):
+                        for dx in (-1, 0, 1):
+                            A, B, C = a + dz, b + dy, c + dx
+                            if 0 <= A < fz and 0 <= B < fy and 0 <= C < fx:
+                                nbr[(a * fy + b) * fx + c, (dz + 1) * 9 + (dy + 1) * 3 + dx + 1] = (A * fy + B) * fx + C
+    return nbr
