@@ -138,6 +138,22 @@ int gamer_refresh_ghosts(const void* u, void* in, int gz, int gy, int gx, int nv
 int gamer_refresh_ghosts_table(const void* u, void* in, const int32_t* nbr, int64_t n_groups, int nvar,
                                int precision, void* stream);
 
+/* Ghost zones at coarse-fine boundaries, "interpolating from coarse patches", with the temporal interpolation
+ * between the coarse level's two stored times (L482): the companion of gamer_refresh_ghosts_table, it fills exactly the slabs
+ * of fine_in[n_fine][nvar][22][22][22] whose entry in nbr[n_fine][27] (the FINE level's same-level table) is negative and
+ * touches nothing else.  coarse_in[..][nvar][22][22][22] is the PADDED coarse batch (ghosts filled: the stencil reaches one
+ * coarse cell beyond the two that 3 fine ghost cells cover); parent[g] (device int32) = coarse group * 8 + octant
+ * (oz*4 + oy*2 + ox) refined by fine group g, as in gamer_restrict.  The paper names no spatial scheme for the fluid; this is
+ * conservative piecewise-linear interpolation of the conserved variables (R24):
+ *   child = U_c + ((+-s_z) + (+-s_y) + (+-s_x)) / 4,   + for the upper child along that axis,
+ *   s_d = (U_{c+e_d} - U_{c-e_d}) / 2 (monotonic = 0) or minmod(U_c - U_{c-e_d}, U_{c+e_d} - U_c) (monotonic = 1),
+ * so that the 8 children of a coarse cell average to it.  U = coarse_in, or (1-w) * coarse_in + w * coarse_in_new when
+ * coarse_in_new is non-NULL (w in [0,1]: the fine sub-step's time between the two coarse states).  fp64 results are
+ * bit-identical to the oracle's loops.  n_fine == 0 is a successful no-op. */
+int gamer_interpolate_ghosts(const void* coarse_in, const void* coarse_in_new, double w, void* fine_in,
+                             const int32_t* parent, const int32_t* nbr, int64_t n_fine, int nvar,
+                             int monotonic, int precision, void* stream);
+
 /* Device-resident step with the same-level ghost refresh FUSED into the staging loads (SURVEY 8(f) NEXT-1,
  * PAPER.md L248 "preparation" + L274 Fig. 3): `u` is the UNPADDED state of the whole batch,
  * u[n_groups][NVAR][16][16][16] (the `out` layout), and nbr[n_groups][27] (device int32) names, for every group,

@@ -21,7 +21,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libgamerhydro.so")
 
 EXPORTS = ["gamer_fluid_advance", "gamer_fluid_advance_ex", "gamer_fluid_advance_retry", "gamer_cfl_dt", "gamer_cfl_dt_ex",
-           "gamer_cfl_from_group_speed", "gamer_refresh_ghosts_periodic", "gamer_refresh_ghosts", "gamer_refresh_ghosts_table", "gamer_fluid_advance_resident",
+           "gamer_cfl_from_group_speed", "gamer_refresh_ghosts_periodic", "gamer_refresh_ghosts", "gamer_refresh_ghosts_table", "gamer_interpolate_ghosts", "gamer_fluid_advance_resident",
            "gamer_neighbors_periodic", "gamer_restrict", "gamer_flux_accumulate", "gamer_flux_correct",
            "gamer_fluid_advance_host", "gamer_release_scratch",
            "gamer_launch_count", "gamer_strerror", "gamer_version"]
@@ -77,6 +77,7 @@ def lib():
         L.gamer_refresh_ghosts_table.argtypes = [vp, vp, vp, i64, ci, ci, vp]
         L.gamer_fluid_advance_resident.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, ci, ci, ctypes.POINTER(gamer_opts)]
         L.gamer_neighbors_periodic.argtypes = [vp, ci, ci, ci, vp]
+        L.gamer_interpolate_ghosts.argtypes = [vp, vp, dbl, vp, vp, vp, i64, ci, ci, ci, vp]
         L.gamer_restrict.argtypes = [vp, vp, vp, i64, ci, ci, vp]
         L.gamer_flux_accumulate.argtypes = [vp, vp, dbl, i64, ci, ci, ci, vp]
         L.gamer_flux_correct.argtypes = [vp, vp, vp, vp, i64, ci, dbl, ci, vp]
@@ -191,6 +192,17 @@ def gamer_refresh_ghosts_table(u, u_in, nbr, stream=None):
         raise GamerError("nbr must be an int32 tensor of shape [n_groups, 27]")
     _check(lib().gamer_refresh_ghosts_table(_ptr(u), _ptr(u_in), _ptr(nbr), u.shape[0], u.shape[1], _precision(u),
                                             _stream_handle(stream)), "gamer_refresh_ghosts_table")
+
+
+def gamer_interpolate_ghosts(coarse_in, fine_in, parent, nbr, coarse_in_new=None, w=0.0, monotonic=False, stream=None):
+    """Coarse->fine ghost interpolation into the slabs of fine_in whose nbr entry is negative."""
+    if parent.dtype != torch.int32 or nbr.dtype != torch.int32 or tuple(nbr.shape) != (fine_in.shape[0], 27):
+        raise GamerError("parent / nbr must be int32 tensors of shapes [n_fine] and [n_fine, 27]")
+    if coarse_in.dtype != fine_in.dtype or (coarse_in_new is not None and coarse_in_new.shape != coarse_in.shape):
+        raise GamerError("coarse and fine batches must share dtype; the two coarse batches must share shape")
+    _check(lib().gamer_interpolate_ghosts(_ptr(coarse_in), _ptr(coarse_in_new), float(w), _ptr(fine_in), _ptr(parent),
+                                          _ptr(nbr), fine_in.shape[0], fine_in.shape[1], int(bool(monotonic)),
+                                          _precision(fine_in), _stream_handle(stream)), "gamer_interpolate_ghosts")
 
 
 def gamer_fluid_advance_resident(u, nbr, out, flux_out, dt, dh, gamma, scheme, recon, riemann, opts=None):

@@ -285,6 +285,38 @@ extern "C" int gamer_refresh_ghosts_table(const void* u, void* in, const int32_t
 }
 
 // ------------------------------------------------------------------------------------------ coarse-fine fix-up
+template <typename T>
+static void launch_interp(const void* c0, const void* c1, double w, void* fine, const int32_t* parent, const int32_t* nbr,
+                          unsigned grid, int nvar, int monotonic, cudaStream_t st) {
+    const T* a0 = static_cast<const T*>(c0);
+    const T* a1 = static_cast<const T*>(c1);
+    T* f = static_cast<T*>(fine);
+    const T w0 = T(1.0 - w), w1 = T(w);
+    if (a1) {
+        if (monotonic) interpolate_ghosts_kernel<T, true, true><<<grid, 256, 0, st>>>(a0, a1, w0, w1, f, parent, nbr, nvar);
+        else interpolate_ghosts_kernel<T, true, false><<<grid, 256, 0, st>>>(a0, a1, w0, w1, f, parent, nbr, nvar);
+    } else {
+        if (monotonic) interpolate_ghosts_kernel<T, false, true><<<grid, 256, 0, st>>>(a0, a1, w0, w1, f, parent, nbr, nvar);
+        else interpolate_ghosts_kernel<T, false, false><<<grid, 256, 0, st>>>(a0, a1, w0, w1, f, parent, nbr, nvar);
+    }
+}
+
+extern "C" int gamer_interpolate_ghosts(const void* coarse_in, const void* coarse_in_new, double w, void* fine_in,
+                                        const int32_t* parent, const int32_t* nbr, int64_t n_fine, int nvar,
+                                        int monotonic, int precision, void* stream) {
+    if (n_fine < 0 || nvar < 1 || nvar > 6 || (precision != GAMER_FP32 && precision != GAMER_FP64)) return GAMER_EINVAL;
+    if (coarse_in_new && (!std::isfinite(w) || w < 0.0 || w > 1.0)) return GAMER_EINVAL;
+    if (n_fine > 0 && (!coarse_in || !fine_in || !parent || !nbr || coarse_in == fine_in)) return GAMER_EINVAL;
+    if (n_fine == 0) return GAMER_OK;
+    if (n_fine * nvar > 0x7fffffff) return GAMER_EUNSUPPORTED;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const unsigned grid = (unsigned)(n_fine * nvar);
+    if (precision == GAMER_FP32) launch_interp<float>(coarse_in, coarse_in_new, w, fine_in, parent, nbr, grid, nvar, monotonic, st);
+    else launch_interp<double>(coarse_in, coarse_in_new, w, fine_in, parent, nbr, grid, nvar, monotonic, st);
+    g_launches += 1;
+    return cudaGetLastError() == cudaSuccess ? GAMER_OK : GAMER_ECUDA;
+}
+
 extern "C" int gamer_restrict(const void* fine, void* coarse, const int32_t* parent, int64_t n_fine, int nvar,
                               int precision, void* stream) {
     if (n_fine < 0 || nvar < 1 || nvar > 6 || (precision != GAMER_FP32 && precision != GAMER_FP64)) return GAMER_EINVAL;

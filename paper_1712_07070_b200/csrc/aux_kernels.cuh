@@ -217,6 +217,62 @@ __global__ void __launch_bounds__(256) refresh_table_kernel(const T* __restrict_
     }
 }
 
+// Ghost zones at coarse-fine boundaries "interpolat[ed] from coarse patches", linear in time between the
+// coarse level's two stored states (L482); R24: conservative piecewise-linear interpolation of the conserved
+// variables, child = U_c + ((+-s_z) + (+-s_y) + (+-s_x)) / 4 with central or minmod slopes.  One CTA per (fine group,
+// variable); only the slabs whose entry of the fine level's neighbour table is negative are written.  Fine padded index p
+// along an axis -> fine cell i = p - 3 -> coarse cell 8 o + floor(i / 2) of the parent group (padded index + 3), child i & 1.
+__device__ __forceinline__ double blend_rn(double w0, double a, double w1, double b) { return __dadd_rn(__dmul_rn(w0, a), __dmul_rn(w1, b)); }
+__device__ __forceinline__ float blend_rn(float w0, float a, float w1, float b) { return __fadd_rn(__fmul_rn(w0, a), __fmul_rn(w1, b)); }
+
+template <typename T, bool BLEND, bool MONO>
+__global__ void __launch_bounds__(256) interpolate_ghosts_kernel(const T* __restrict__ c0, const T* __restrict__ c1, T w0, T w1,
+                                                                 T* __restrict__ fine, const int* __restrict__ parent,
+                                                                 const int* __restrict__ nbr, int nvar) {
+    __shared__ int nb[27];
+    const long long gv = blockIdx.x;
+    const long long g = gv / nvar;
+    const int v = (int)(gv - g * nvar);
+    if (threadIdx.x < 27) nb[threadIdx.x] = nbr[g * 27 + threadIdx.x];
+    __syncthreads();
+    const int par = parent[g];
+    const int oz = (par >> 2) & 1, oy = (par >> 1) & 1, ox = par & 1;
+    const size_t cbase = ((size_t)(par >> 3) * nvar + v) * NPC;
+    const T* a0 = c0 + cbase;
+    const T* a1 = BLEND ? c1 + cbase : nullptr;
+    T* dst = fine + ((size_t)g * nvar + v) * NPC;
+    auto coarse = [&](int q) -> T {
+        const T x = __ldg(a0 + q);
+        if (!BLEND) return x;
+        return blend_rn(w0, x, w1, __ldg(a1 + q));
+    };
+    auto slope = [&](T lo, T mid, T hi) -> T {
+        if (!MONO) return T(0.5) * (hi - lo);
+        const T a = mid - lo, b = hi - mid;
+        return a * b > T(0) ? (fabs(a) < fabs(b) ? a : b) : T(0);
+    };
+    for (int t = threadIdx.x; t < NP * NP; t += 256) {
+        const int pj = t / NP, pi = t - pj * NP;
+        const int dx = pi < NGH ? 0 : (pi < NGH + PS ? 1 : 2), dy = pj < NGH ? 0 : (pj < NGH + PS ? 1 : 2);
+        // floor((p - 3) / 2) = ((p + 1) >> 1) - 2 for p >= 0; child parity = (p + 1) & 1
+        const int qj = 8 * oy + ((pj + 1) >> 1) - 2 + NGH, qi = 8 * ox + ((pi + 1) >> 1) - 2 + NGH;
+        const bool uj = (pj + 1) & 1, ui = (pi + 1) & 1;
+        for (int pk = 0; pk < NP; ++pk) {
+            const int dz = pk < NGH ? 0 : (pk < NGH + PS ? 1 : 2);
+            const int s = dz * 9 + dy * 3 + dx;
+            if (s == 13 || nb[s] >= 0) continue;
+            const int qk = 8 * oz + ((pk + 1) >> 1) - 2 + NGH;
+            const bool uk = (pk + 1) & 1;
+            const int q = (qk * NP + qj) * NP + qi;
+            const T u = coarse(q);
+            const T sz = slope(coarse(q - NP * NP), u, coarse(q + NP * NP));
+            const T sy = slope(coarse(q - NP), u, coarse(q + NP));
+            const T sx = slope(coarse(q - 1), u, coarse(q + 1));
+            dst[(pk * NP + pj) * NP + pi] = u + T(0.25) * (((uk ? sz : -sz) + (uj ? sy : -sy)) + (ui ? sx : -sx));
+        }
+    }
+}
+
 // neighbour table of a periodic box of gz x gy x gx groups: nbr[g][(dz+1)*9 + (dy+1)*3 + (dx+1)]
 __global__ void neighbors_periodic_kernel(int* __restrict__ nbr, int gz, int gy, int gx) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;

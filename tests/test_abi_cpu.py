@@ -85,6 +85,14 @@ def test_argument_validation_needs_no_gpu(built_lib):
     L.gamer_neighbors_periodic.argtypes = [vp, ci, ci, ci, vp]
     assert L.gamer_neighbors_periodic(None, 1, 1, 1, None) == -1
     assert L.gamer_neighbors_periodic(vp(4096), 0, 1, 1, None) == -1
+    L.gamer_interpolate_ghosts.argtypes = [vp, vp, dbl, vp, vp, vp, i64, ci, ci, ci, vp]
+    interp = lambda c0=ok[0], c1=None, w=0.0, f=ok[1], par=vp(64), nb=vp(128), n=1, nv=5, prec=4: \
+        L.gamer_interpolate_ghosts(c0, c1, w, f, par, nb, n, nv, 0, prec, None)
+    assert interp(c0=None) == -1 and interp(f=None) == -1 and interp(par=None) == -1 and interp(nb=None) == -1
+    assert interp(nv=7) == -1 and interp(prec=2) == -1 and interp(n=-1) == -1
+    assert interp(c1=vp(16384), w=1.5) == -1 and interp(c1=vp(16384), w=float("nan")) == -1
+    assert interp(f=ok[0]) == -1                                # in place
+    assert interp(n=0) == 0
     # remedy (iv)/(v) driver: needs opts with the device counter, a host dt, a ratio below 1, dt_min >= 0
     L.gamer_fluid_advance_retry.argtypes = [vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, ci, ci, ctypes.POINTER(gb.gamer_opts),
                                             dbl, dbl, ctypes.POINTER(dbl), ctypes.POINTER(ctypes.c_int32)]

@@ -418,3 +418,69 @@ def test_remedy_iv_v_retry_matches_oracle(dev, oracle_mod, dtype):
     with pytest.raises(gb.GamerError, match="-4"):
         gb.gamer_fluid_advance_retry(pd, out, flux, dt0, dh, G53, gb.MHM, gb.PLM, gb.ROE, o, dt_min=1.01 * dt_used)
     assert int(nun.item()) > 0
+
+
+@pytest.mark.parametrize("monotonic", [False, True])
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+def test_interpolated_ghosts_match_oracle(dev, oracle_mod, dtype, monotonic):
+    """gamer_interpolate_ghosts (L248 "interpolating from coarse patches", L482 temporal interpolation; R24) against
+    oracle.interpolate_ghosts: a refined box that touches the periodic wrap of a 32 x 32 x 48 coarse level (parents in several
+    coarse groups, all 8 octants), 6 variables, two coarse states blended at w = 0.25; after gamer_refresh_ghosts_table has
+    copied the sibling slabs.  fp64: identical bits; fp32: 1e-6 of the scale.  Slabs with a sibling and the interior keep
+    their values; a second call without the time blend is checked too."""
+    import amr_harness as amr
+    region = (0, 16, 8, 24, 24, 48)
+    cshape = (32, 32, 48)
+    parent, _ = amr.region_tables(region, cshape)
+    nbr = amr.region_neighbors(region)
+    n_f = parent.shape[0]
+    assert n_f == 2 * 2 * 3 and sorted(set((parent % 8).tolist())) == list(range(8))
+    g = torch.Generator().manual_seed(5)
+    uc0 = torch.randn((6, *cshape), generator=g, dtype=torch.float64)
+    uc1 = uc0 + 0.3 * torch.randn((6, *cshape), generator=g, dtype=torch.float64)
+    c0, c1 = inputs.pack_periodic(uc0).to(dtype), inputs.pack_periodic(uc1).to(dtype)
+    uf = torch.randn((n_f, 6, 16, 16, 16), generator=g, dtype=torch.float64).to(dtype)
+    for blend in (True, False):
+        ref = np.full((n_f, 6, 22, 22, 22), -7.0)
+        ref[:, :, 3:19, 3:19, 3:19] = uf.double().numpy()
+        oracle_mod.fill_ghosts_table(uf.double().numpy(), nbr.numpy(), ref)
+        sibling_only = ref.copy()
+        oracle_mod.interpolate_ghosts(c0.double().numpy(), parent.numpy(), nbr.numpy(), ref,
+                                      coarse_padded_new=c1.double().numpy() if blend else None, w=0.25, monotonic=monotonic)
+        assert (ref != -7.0).all() and (sibling_only == -7.0).any()
+        fine = torch.full((n_f, 6, 22, 22, 22), -7.0, dtype=dtype, device=dev)
+        fine[:, :, 3:19, 3:19, 3:19] = uf.to(dev)
+        gb.gamer_refresh_ghosts_table(uf.to(dev), fine, nbr.to(dev))
+        before = gb.gamer_launch_count()
+        gb.gamer_interpolate_ghosts(c0.to(dev), fine, parent.to(dev), nbr.to(dev), coarse_in_new=c1.to(dev) if blend else None,
+                                    w=0.25, monotonic=monotonic)
+        torch.cuda.synchronize()
+        assert gb.gamer_launch_count() == before + 1
+        got = fine.cpu().double().numpy()
+        if dtype == torch.float64:
+            assert np.array_equal(got, ref)
+        else:
+            assert np.abs(got - ref).max() <= 1e-6 * np.abs(ref).max()
+        keep = sibling_only != -7.0
+        assert np.array_equal(got[keep], sibling_only[keep])
+
+
+def test_config3_ghosts_filled_on_the_gpu(dev):
+    """Config 3's fine-level preparation done entirely by the library (gamer_refresh_ghosts_table for siblings +
+    gamer_interpolate_ghosts for the coarse-fine slabs, linear in time) equals the harness's global-array packing
+    (amr.pack_fine) of the same two levels to round-off, at both sub-step times."""
+    import amr_harness as amr
+    uc, uf, region, dh_c = amr.sedov_two_level(32, 64, 64, gamma=G53, device=dev, e_blast=5.7e-5, p_amb=1.0)
+    uc1 = uc * (1.0 + 0.05 * torch.sin(torch.arange(uc.shape[-1], device=dev) * 0.3))
+    parent, _ = amr.region_tables(region, uc.shape[1:])
+    nbr = amr.region_neighbors(region).to(dev)
+    ug = amr.to_groups(uf)
+    c0, c1 = inputs.pack_periodic(uc), inputs.pack_periodic(uc1)
+    for w in (0.0, 0.5):
+        ref, _ = amr.pack_fine(uf, (1.0 - w) * uc + w * uc1, region)
+        fine = torch.zeros_like(ref)
+        fine[:, :, 3:19, 3:19, 3:19] = ug
+        gb.gamer_refresh_ghosts_table(ug, fine, nbr)
+        gb.gamer_interpolate_ghosts(c0, fine, parent.to(dev), nbr, coarse_in_new=c1, w=w)
+        torch.cuda.synchronize()
+        assert (fine - ref).abs().max().item() <= 1e-14 * ref.abs().max().item()
