@@ -289,7 +289,25 @@ def main():
         fixup = {"restrict_GBs": rb * 5 / (b0.elapsed_time(b1) * 1e-3) / 1e9, "restrict_bytes": rb,
                  "flux_accumulate_GBs": ab * 5 / (b1.elapsed_time(b2) * 1e-3) / 1e9, "flux_accumulate_bytes": ab,
                  "hbm_peak_GBs": peaks()[0]}
-        del coarse, acc, parent
+        # coarse->fine ghost interpolation (gamer_interpolate_ghosts, R24): up to 4096 isolated fine groups (all 26 slabs
+        # at a coarse-fine boundary) under the padded batch taken as the coarse level; bytes = ghost cells written +
+        # the 14^3 coarse cells each octant's stencil covers, read once
+        nfi = min(nf, 4096)
+        fine_pad = torch.zeros((nfi,) + tuple(u_in.shape[1:]), dtype=dtype, device=dev)
+        nbr_cf = torch.full((nfi, 27), -1, dtype=torch.int32, device=dev)
+        nbr_cf[:, 13] = torch.arange(nfi, dtype=torch.int32, device=dev)
+        gb.gamer_interpolate_ghosts(u_in, fine_pad, parent[:nfi].contiguous(), nbr_cf, monotonic=True, stream=stream)
+        b3, b4 = (torch.cuda.Event(enable_timing=True) for _ in range(2))
+        b3.record(stream)
+        for _ in range(5):
+            gb.gamer_interpolate_ghosts(u_in, fine_pad, parent[:nfi].contiguous(), nbr_cf, monotonic=True, stream=stream)
+        b4.record(stream)
+        torch.cuda.synchronize()
+        ib = nfi * u_in.shape[1] * (22 ** 3 - 16 ** 3 + 14 ** 3) * sz
+        fixup["interpolate_ghosts_GBs"] = ib * 5 / (b3.elapsed_time(b4) * 1e-3) / 1e9
+        fixup["interpolate_ghosts_bytes"] = ib
+        finite = finite and bool(torch.isfinite(fine_pad).all().item())
+        del coarse, acc, parent, fine_pad, nbr_cf
 
     # ---- e2e: host buffers through the C ABI, copies inside the timed region
     e2e = None

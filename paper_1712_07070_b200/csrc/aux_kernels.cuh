@@ -235,17 +235,27 @@ __global__ void __launch_bounds__(256) interpolate_ghosts_kernel(const T* __rest
     const int v = (int)(gv - g * nvar);
     if (threadIdx.x < 27) nb[threadIdx.x] = nbr[g * 27 + threadIdx.x];
     __syncthreads();
+    bool any = false;
+#pragma unroll
+    for (int s = 0; s < 27; ++s) any = any || (s != 13 && nb[s] < 0);
+    if (!any) return;                                  // no coarse-fine slab in this group (uniform over the CTA)
     const int par = parent[g];
     const int oz = (par >> 2) & 1, oy = (par >> 1) & 1, ox = par & 1;
     const size_t cbase = ((size_t)(par >> 3) * nvar + v) * NPC;
     const T* a0 = c0 + cbase;
     const T* a1 = BLEND ? c1 + cbase : nullptr;
     T* dst = fine + ((size_t)g * nvar + v) * NPC;
-    auto coarse = [&](int q) -> T {
+    // the 14^3 coarse cells under this octant's ghost zones (+1 for the slopes), blended in time once: padded coarse
+    // indices 8 o .. 8 o + 13 along each axis
+    constexpr int CB = 14;
+    __shared__ T cs[CB * CB * CB];
+    for (int t = threadIdx.x; t < CB * CB * CB; t += 256) {
+        const int k = t / (CB * CB), r = t - k * (CB * CB), j = r / CB, i = r - j * CB;
+        const int q = ((8 * oz + k) * NP + 8 * oy + j) * NP + 8 * ox + i;
         const T x = __ldg(a0 + q);
-        if (!BLEND) return x;
-        return blend_rn(w0, x, w1, __ldg(a1 + q));
-    };
+        cs[t] = BLEND ? blend_rn(w0, x, w1, __ldg(a1 + q)) : x;
+    }
+    __syncthreads();
     auto slope = [&](T lo, T mid, T hi) -> T {
         if (!MONO) return T(0.5) * (hi - lo);
         const T a = mid - lo, b = hi - mid;
@@ -254,20 +264,21 @@ __global__ void __launch_bounds__(256) interpolate_ghosts_kernel(const T* __rest
     for (int t = threadIdx.x; t < NP * NP; t += 256) {
         const int pj = t / NP, pi = t - pj * NP;
         const int dx = pi < NGH ? 0 : (pi < NGH + PS ? 1 : 2), dy = pj < NGH ? 0 : (pj < NGH + PS ? 1 : 2);
-        // floor((p - 3) / 2) = ((p + 1) >> 1) - 2 for p >= 0; child parity = (p + 1) & 1
-        const int qj = 8 * oy + ((pj + 1) >> 1) - 2 + NGH, qi = 8 * ox + ((pi + 1) >> 1) - 2 + NGH;
+        // floor((p - 3) / 2) = ((p + 1) >> 1) - 2 for p >= 0, i.e. index ((p + 1) >> 1) + 1 of the staged block;
+        // child parity = (p + 1) & 1
+        const int lj = ((pj + 1) >> 1) + 1, li = ((pi + 1) >> 1) + 1;
         const bool uj = (pj + 1) & 1, ui = (pi + 1) & 1;
         for (int pk = 0; pk < NP; ++pk) {
             const int dz = pk < NGH ? 0 : (pk < NGH + PS ? 1 : 2);
             const int s = dz * 9 + dy * 3 + dx;
             if (s == 13 || nb[s] >= 0) continue;
-            const int qk = 8 * oz + ((pk + 1) >> 1) - 2 + NGH;
+            const int lk = ((pk + 1) >> 1) + 1;
             const bool uk = (pk + 1) & 1;
-            const int q = (qk * NP + qj) * NP + qi;
-            const T u = coarse(q);
-            const T sz = slope(coarse(q - NP * NP), u, coarse(q + NP * NP));
-            const T sy = slope(coarse(q - NP), u, coarse(q + NP));
-            const T sx = slope(coarse(q - 1), u, coarse(q + 1));
+            const int q = (lk * CB + lj) * CB + li;
+            const T u = cs[q];
+            const T sz = slope(cs[q - CB * CB], u, cs[q + CB * CB]);
+            const T sy = slope(cs[q - CB], u, cs[q + CB]);
+            const T sx = slope(cs[q - 1], u, cs[q + 1]);
             dst[(pk * NP + pj) * NP + pi] = u + T(0.25) * (((uk ? sz : -sz) + (uj ? sy : -sy)) + (ui ? sx : -sx));
         }
     }

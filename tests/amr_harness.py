@@ -69,11 +69,13 @@ def restrict(uf):
     return 0.125 * sum(uf[:, a::2, b::2, d::2] for a in (0, 1) for b in (0, 1) for d in (0, 1))
 
 
-def two_level_step(solver, uc, uf, region, dh_c, dt_c, fixup=None):
+def two_level_step(solver, uc, uf, region, dh_c, dt_c, fixup=None, pack_fine_fn=None):
     """Returns (uc_new after fix-up, uf_new, records) where records holds every padded batch / output for parity.
     fixup = None: restriction and flux correction are done right here on the global arrays (torch); otherwise
     fixup(uc1, uf, flux_c, [flux_f of each sub-step], region, dt_c / dh_c) -> corrected uc1 (group-layout
-    implementations: the oracle's C functions or the CUDA library, see fixup_in_group_layout)."""
+    implementations: the oracle's C functions or the CUDA library, see fixup_in_group_layout).
+    pack_fine_fn(uf, uc0, uc1, w, region) -> (padded fine batch, fine group dims) replaces the global-array packing of the
+    fine level (sibling copy + interpolation from the coarse level at time weight w between uc0 and uc1)."""
     z0, z1, y0, y1, x0, x1 = region
     rec = {}
     cdims = inputs.group_dims(uc)
@@ -86,8 +88,11 @@ def two_level_step(solver, uc, uf, region, dh_c, dt_c, fixup=None):
     fine_fluxes = []
     for sub in (0, 1):
         w = 0.5 * sub
-        uc_t = (1.0 - w) * uc + w * uc1                      # linear in time
-        pf, fdims = pack_fine(uf, uc_t, region)
+        if pack_fine_fn is None:
+            uc_t = (1.0 - w) * uc + w * uc1                  # linear in time
+            pf, fdims = pack_fine(uf, uc_t, region)
+        else:
+            pf, fdims = pack_fine_fn(uf, uc, uc1, w, region)
         out_f, flux_f = solver(pf, 0.5 * dt_c, 0.5 * dh_c)
         rec["fine%d" % sub] = (pf, out_f, flux_f)
         fine_fluxes.append(flux_f)

@@ -484,3 +484,39 @@ def test_config3_ghosts_filled_on_the_gpu(dev):
         gb.gamer_interpolate_ghosts(c0, fine, parent.to(dev), nbr, coarse_in_new=c1, w=w)
         torch.cuda.synchronize()
         assert (fine - ref).abs().max().item() <= 1e-14 * ref.abs().max().item()
+
+
+def test_config3_step_with_library_preparation_and_fixup(dev):
+    """One whole two-level step of config 3 (reduced size) in which every stage outside the harness's bookkeeping is a
+    library call: sibling copy + coarse-fine interpolation in space and time for the fine level's ghosts, the solver, the
+    restriction, flux averaging and flux correction.  Same result as the harness's own global-array preparation and fix-up
+    to round-off, composite grid conserved to 1e-12."""
+    import amr_harness as amr
+    uc, uf, region, dh_c = amr.sedov_two_level(64, 128, 128, gamma=G53, device=dev)
+    parent, _ = amr.region_tables(region, uc.shape[1:])
+    parent, nbr = parent.to(dev), amr.region_neighbors(region).to(dev)
+    z0, z1, y0, y1, x0, x1 = region
+    fdims = ((z1 - z0) // 8, (y1 - y0) // 8, (x1 - x0) // 8)
+
+    def gpu_solver(p, dt, dh):
+        out, flux, speed, nun, diag = gpu_ex(p.contiguous(), dt, dh, G53, gb.MHM, gb.PLM, gb.HLLE, min_pres=1e-10)
+        return out, flux
+
+    def gpu_pack(uf_, uc0, uc1, w, region_):
+        ug = amr.to_groups(uf_)
+        fine = torch.empty((ug.shape[0], ug.shape[1], 22, 22, 22), dtype=ug.dtype, device=dev)
+        fine[:, :, 3:19, 3:19, 3:19] = ug
+        gb.gamer_refresh_ghosts_table(ug, fine, nbr)
+        gb.gamer_interpolate_ghosts(inputs.pack_periodic(uc0), fine, parent, nbr, coarse_in_new=inputs.pack_periodic(uc1), w=w)
+        return fine, fdims
+
+    pb = (G53 - 1.0) / (8 * (0.5 * dh_c) ** 3)
+    dt_c = 2 * 0.4 * (0.5 * dh_c) / (3.0 * math.sqrt(G53 * pb))
+    tot0 = amr.composite_total(uc, uf, region, dh_c)
+    ua, fa, _ = amr.two_level_step(gpu_solver, uc, uf, region, dh_c, dt_c)
+    ub, fb, _ = amr.two_level_step(gpu_solver, uc, uf, region, dh_c, dt_c, fixup=_gpu_fixup(), pack_fine_fn=gpu_pack)
+    torch.cuda.synchronize()
+    for a, b in ((ua, ub), (fa, fb)):
+        assert ((a - b).abs().amax(dim=(1, 2, 3)) <= 1e-12 * (a.abs().amax(dim=(1, 2, 3)) + 1e-30)).all()
+    tot1 = amr.composite_total(ub, fb, region, dh_c)
+    assert ((tot1 - tot0).abs() / (tot0.abs() + 1e-6)).max().item() <= 1e-12
