@@ -18,3 +18,31 @@ def global_dt(dt: torch.Tensor) -> torch.Tensor:
     if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
         dist.all_reduce(dt, op=dist.ReduceOp.MIN)
     return dt
+
+
+def global_count(n: int) -> int:
+    """SUM all-reduce of one integer (e.g. the unphysical-cell count of a rank's shard)."""
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        t = torch.tensor([int(n)], dtype=torch.int64)
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        return int(t.item())
+    return int(n)
+
+
+def retry_level(step_fn, dt: float, dt_ratio: float = 0.8, dt_min: float = 0.0, max_retries: int = 200):
+    """Remedies (iv), (v) of PAPER.md L107-108 for a level sharded over ranks: "recalculate ALL patches on the currently
+    targeted level with this reduced time-step" -- a rank whose own shard came out physical must redo it too, so the
+    decision is taken on the SUM of the ranks' counts.  step_fn(dt) advances this rank's shard from its unchanged input
+    (e.g. binding.gamer_fluid_advance_ex with n_unphysical_out) and returns its count of unphysical cells.
+    Returns (dt_used, n_retries), identical on every rank and to gamer_fluid_advance_retry on the unsharded batch;
+    raises ArithmeticError on every rank when the reduced step falls below dt_min (the paper's abort)."""
+    if not (0.0 < dt_ratio < 1.0) or not dt > 0.0 or dt_min < 0.0:
+        raise ValueError("need dt > 0, 0 < dt_ratio < 1, dt_min >= 0")
+    n = 0
+    while True:
+        if global_count(step_fn(dt)) == 0:
+            return dt, n
+        dt = dt * dt_ratio
+        n += 1
+        if dt < dt_min or n > max_retries:
+            raise ArithmeticError(f"unphysical cells remain and the reduced time-step {dt} is below dt_min {dt_min}")

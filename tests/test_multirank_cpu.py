@@ -52,3 +52,69 @@ def test_two_ranks_shard_groups_and_reduce_dt():
     assert (res[0][1], res[0][2], res[1][1], res[1][2]) == (0, 4, 4, 8)
     full = oracle.fluid_advance(padded.numpy(), dt_all, 1 / 32, 5 / 3, 1, 1, 1)["out"]
     assert np.array_equal(np.concatenate([res[0][5], res[1][5]]), full)
+
+
+def _retry_worker(rank, world, port, q):
+    sys.path.insert(0, ROOT)
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    import oracle
+    from paper_1712_07070_b200 import inputs, sharding
+    oracle.set_threads(2)
+    padded, dt0, dh = _retry_inputs(oracle, inputs)
+    lo, hi = sharding.shard_range(padded.shape[0], rank, world)
+    mine = padded[lo:hi].contiguous().numpy()
+    last, counts = {}, []
+
+    def step(dt):
+        last["r"] = oracle.fluid_advance(mine, dt, dh, 5 / 3, 1, 1, 1)
+        counts.append(last["r"]["stats"]["n_unphysical"])
+        return counts[-1]
+
+    dt_used, k = sharding.retry_level(step, dt0)
+    aborted = False
+    try:
+        sharding.retry_level(step, dt0, dt_min=1.01 * dt_used)
+    except ArithmeticError:
+        aborted = True
+    q.put((rank, dt_used, k, counts[:k + 1], last["r"]["out"] if not aborted else None, aborted,
+           oracle.fluid_advance(mine, dt_used, dh, 5 / 3, 1, 1, 1)["out"]))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def _retry_inputs(oracle, inputs):
+    # groups are independent given their padded inputs: rank 0's half comes from Mach-3 turbulence, rank 1's from a calm field
+    rough = inputs.pack_periodic(inputs.turbulence_field(32, 3, kmax=6, gamma=5 / 3, mach=3.0, sigma=1.0))
+    calm = inputs.pack_periodic(inputs.turbulence_field(32, 4, kmax=4, gamma=5 / 3, mach=0.3, sigma=0.2))
+    padded = torch.cat([rough[:4], calm[4:]]).contiguous()
+    dh = 1 / 32
+    dt0 = 5.0 * oracle.cfl_dt(inputs.interior(padded).contiguous().numpy(), dh, 5 / 3, 0.5, 1)[0]
+    return padded, dt0, dh
+
+
+def test_two_ranks_retry_the_level_together():
+    """Remedy (iv) is level-wide (L107): both ranks take the same number of reductions and the same dt as the unsharded
+    oracle loop, also in attempts where one rank's own shard had no unphysical cell; both abort together."""
+    sys.path.insert(0, ROOT)
+    import oracle
+    from paper_1712_07070_b200 import inputs
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 31500 + os.getpid() % 2000
+    procs = [ctx.Process(target=_retry_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted([q.get(timeout=600) for _ in range(2)], key=lambda x: x[0])
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    padded, dt0, dh = _retry_inputs(oracle, inputs)
+    ref = oracle.fluid_advance_retry(padded.numpy(), dt0, dh, 5 / 3, 1, 1, 1)
+    assert ref["n_retries"] >= 2
+    for r in res:
+        assert (r[1], r[2]) == (ref["dt_used"], ref["n_retries"]) and r[5]
+    assert np.array_equal(np.concatenate([res[0][6], res[1][6]]), ref["out"])
+    c0, c1 = res[0][3], res[1][3]
+    assert all(a + b > 0 for a, b in zip(c0[:-1], c1[:-1])) and c0[-1] == c1[-1] == 0
+    assert all(b == 0 for b in c1), (c0, c1)          # rank 1 alone would never have retried: the decision is the level's
