@@ -321,3 +321,34 @@ def interpolate_ghosts(coarse_padded, parent, nbr, fine_padded, coarse_padded_ne
                                 fine_padded[g, :, pk, pj, pi] = u + 0.25 * (((2 * ak - 1) * sz + (2 * aj - 1) * sy)
                                                                             + (2 * ai - 1) * sx)
     return fine_padded
+
+
+def poisson_sor(phi, rho, dh, coeff, omega, n_iter, want_acc=True):
+    """The refined-level Poisson solver of PAPER.md L126-128 / L236: every patch is relaxed on its own
+    (8 + 2*5)^3 = 18^3 grid "with the outermost cells being fixed during the iterations", Laplacian = "its second-order finite
+    difference equivalent", method = SOR (Press et al. 2007).  Reading R25: odd-even (red-black) ordering with a
+    constant over-relaxation parameter omega and a fixed number of iterations; one iteration = the half-sweep over the
+    cells with (i+j+k) even, then the one over the odd cells (i, j, k = indices in the 18^3 array):
+        r = phi(i-1) + phi(i+1) + phi(j-1) + phi(j+1) + phi(k-1) + phi(k+1) - 6 phi - coeff dh^2 rho,   phi += omega r / 6
+    for  laplacian(phi) = coeff * rho  (coeff = 4 pi G, times the scale factor in comoving coordinates).
+    phi [N,18,18,18]: initial guess inside (L238), boundary condition on the outermost layer; rho [N,16,16,16] on the
+    relaxed cells.  Returns (phi after n_iter iterations, acc [N,3,8,8,8] or None): acc = -grad(phi) by central
+    differences on the 8^3 active zones (cells 5..12 of the 18^3 array, Fig. 2), components ordered (x, y, z)."""
+    phi = np.array(phi, dtype=np.float64)
+    rho = np.asarray(rho, dtype=np.float64)
+    k, j, i = np.meshgrid(np.arange(1, 17), np.arange(1, 17), np.arange(1, 17), indexing="ij")
+    src = coeff * dh * dh * rho
+    for _ in range(int(n_iter)):
+        for colour in (0, 1):
+            m = ((k + j + i) % 2 == colour)[None]
+            c = phi[:, 1:17, 1:17, 1:17]
+            r = (phi[:, 1:17, 1:17, 0:16] + phi[:, 1:17, 1:17, 2:18] + phi[:, 1:17, 0:16, 1:17] + phi[:, 1:17, 2:18, 1:17]
+                 + phi[:, 0:16, 1:17, 1:17] + phi[:, 2:18, 1:17, 1:17] - 6.0 * c - src)
+            phi[:, 1:17, 1:17, 1:17] = np.where(m, c + omega * r / 6.0, c)
+    acc = None
+    if want_acc:
+        a = slice(5, 13)
+        acc = np.stack([-(phi[:, a, a, 6:14] - phi[:, a, a, 4:12]) / (2.0 * dh),
+                        -(phi[:, a, 6:14, a] - phi[:, a, 4:12, a]) / (2.0 * dh),
+                        -(phi[:, 6:14, a, a] - phi[:, 4:12, a, a]) / (2.0 * dh)], axis=1)
+    return phi, acc

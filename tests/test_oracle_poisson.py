@@ -1,0 +1,82 @@
+"""Pins for the oracle's SOR Poisson solver.  CPU only."""
+import numpy as np
+import scipy.sparse as sp
+import scipy.sparse.linalg as spla
+
+
+def _problem(seed, n=3):
+    rng = np.random.default_rng(seed)
+    phi = rng.standard_normal((n, 18, 18, 18))
+    rho = rng.standard_normal((n, 16, 16, 16)) + 2.0
+    return phi, rho
+
+
+def _direct(phi, rho, dh, coeff):
+    """The discrete Dirichlet problem solved without any relaxation: 7-point matrix on the 16^3 unknowns, boundary
+    values moved to the right-hand side, sparse LU."""
+    n = 16
+    e = sp.eye(n)
+    d = sp.diags([1.0, -2.0, 1.0], [-1, 0, 1], shape=(n, n))
+    A = (sp.kron(sp.kron(d, e), e) + sp.kron(sp.kron(e, d), e) + sp.kron(sp.kron(e, e), d)).tocsc()
+    lu = spla.splu(A)
+    out = phi.copy()
+    for p in range(phi.shape[0]):
+        b = coeff * dh * dh * rho[p].copy()
+        b[0] -= phi[p, 0, 1:17, 1:17]
+        b[-1] -= phi[p, 17, 1:17, 1:17]
+        b[:, 0] -= phi[p, 1:17, 0, 1:17]
+        b[:, -1] -= phi[p, 1:17, 17, 1:17]
+        b[:, :, 0] -= phi[p, 1:17, 1:17, 0]
+        b[:, :, -1] -= phi[p, 1:17, 1:17, 17]
+        out[p, 1:17, 1:17, 1:17] = lu.solve(b.ravel()).reshape(n, n, n)
+    return out
+
+
+def test_sor_converges_to_the_direct_solution_of_the_discrete_problem(oracle_mod):
+    """"solve the discretized Poisson equation to machine precision" (L126): enough SOR iterations reach the sparse-LU solution
+    of the same 7-point Dirichlet problem; the boundary layer never changes; fewer iterations are further away."""
+    phi0, rho = _problem(1)
+    dh, coeff = 0.37, 4 * np.pi * 0.8
+    omega = 2.0 / (1.0 + np.sin(np.pi / 17))                    # optimal SOR parameter of a 16-cell Dirichlet box (Press et al.)
+    want = _direct(phi0, rho, dh, coeff)
+    phi, _ = oracle_mod.poisson_sor(phi0, rho, dh, coeff, omega, 200)
+    scale = np.abs(want).max()
+    assert np.abs(phi - want).max() <= 1e-12 * scale
+    edge = np.ones((18, 18, 18), bool)
+    edge[1:17, 1:17, 1:17] = False
+    assert np.array_equal(phi[:, edge], phi0[:, edge])
+    e10 = np.abs(oracle_mod.poisson_sor(phi0, rho, dh, coeff, omega, 10)[0] - want).max()
+    e40 = np.abs(oracle_mod.poisson_sor(phi0, rho, dh, coeff, omega, 40)[0] - want).max()
+    assert e10 > e40 > 1e-9 * scale
+    # omega = 1 is Gauss-Seidel: converges too, far more slowly (the reason for over-relaxation)
+    gs = np.abs(oracle_mod.poisson_sor(phi0, rho, dh, coeff, 1.0, 40)[0] - want).max()
+    assert gs > 100 * e40
+
+
+def test_sor_fixed_point_sweep_definition_and_acceleration(oracle_mod):
+    """(a) A quadratic potential is an exact solution of the 7-point equation (laplacian of x^2 + 2 y^2 - z^2 = 4): with
+    rho = 4 / coeff it is a fixed point of every sweep, and its central-difference acceleration is the exact gradient.
+    (b) One iteration written out cell by cell in plain loops (red cells first, each using the latest neighbours)."""
+    dh, coeff, omega = 0.5, 2.5, 1.6
+    x = (np.arange(18) - 8.5) * dh
+    Z, Y, X = np.meshgrid(x, x, x, indexing="ij")
+    quad = (X ** 2 + 2 * Y ** 2 - Z ** 2 + 0.3 * X - 0.7 * Z + 1.0)[None]
+    rho = np.full((1, 16, 16, 16), 4.0 / coeff)
+    phi, acc = oracle_mod.poisson_sor(quad, rho, dh, coeff, omega, 7)
+    assert np.abs(phi - quad).max() <= 1e-12 * np.abs(quad).max()
+    a = slice(5, 13)
+    assert np.abs(acc[0, 0] + (2 * X + 0.3)[a, a, a]).max() <= 1e-12
+    assert np.abs(acc[0, 1] + (4 * Y)[a, a, a]).max() <= 1e-12
+    assert np.abs(acc[0, 2] + (-2 * Z - 0.7)[a, a, a]).max() <= 1e-12
+    phi0, rho = _problem(2, n=1)
+    p = phi0[0].copy()
+    for colour in (0, 1):
+        for k in range(1, 17):
+            for j in range(1, 17):
+                for i in range(1, 17):
+                    if (i + j + k) % 2 == colour:
+                        r = (p[k, j, i - 1] + p[k, j, i + 1] + p[k, j - 1, i] + p[k, j + 1, i] + p[k - 1, j, i] + p[k + 1, j, i]
+                             - 6 * p[k, j, i] - coeff * dh * dh * rho[0, k - 1, j - 1, i - 1])
+                        p[k, j, i] += omega * r / 6
+    got, _ = oracle_mod.poisson_sor(phi0, rho, dh, coeff, omega, 1, want_acc=False)
+    assert np.abs(got[0] - p).max() <= 1e-14 * np.abs(p).max()
