@@ -200,6 +200,19 @@ int gamer_flux_accumulate(void* acc, const void* flux, double weight, int64_t n_
 int gamer_flux_correct(void* coarse, const void* coarse_flux, const void* fine_flux_avg, const int32_t* table,
                        int64_t n_entries, int nvar, double lam, int precision, void* stream);
 
+/* ---- The paper's other GPU solver: the refined-level Poisson solver of PAPER.md L126-128, L236.
+ * Every patch is relaxed independently on its (8 + 2*5)^3 = 18^3 grid (8^3 active zones + 5 buffer zones per side, Fig. 2)
+ * "with the outermost cells being fixed during the iterations", 7-point Laplacian, successive over-relaxation in red-black
+ * order (R25): n_iter iterations, each = the half-sweep over cells with (i+j+k) even, then odd,
+ *   phi += omega / 6 * (sum of the 6 neighbours - 6 phi - coeff * dh^2 * rho),      for laplacian(phi) = coeff * rho.
+ * phi[n_patches][18][18][18] (device, in place): initial guess inside (L238: interpolated from the coarse level by the caller)
+ * and the boundary condition on the outermost layer, which is returned unchanged; rho[n_patches][16][16][16]: the density on
+ * the relaxed cells; acc (nullable) [n_patches][3][8][8][8] = -grad(phi) on the active zones (cells 5..12) by central
+ * differences, components (x, y, z) (L238: "the cell-centered gravitational acceleration ... immediately after solving the
+ * potential").  0 < omega < 2; n_iter >= 0; the potential lives in shared memory for the whole solve (46.7 KB in fp64). */
+int gamer_poisson_sor(void* phi, const void* rho, void* acc, int64_t n_patches, double dh, double coeff,
+                      double omega, int n_iter, int precision, void* stream);
+
 /* End-to-end form with HOST buffers (pinned or pageable): copies `in` to the device in chunks,
  * runs the solver, copies `out`, `flux_out` (nullable) and `group_speed_out` (nullable) back,
  * overlapping copies and kernels on internal streams as the paper does with CUDA streams (L242),

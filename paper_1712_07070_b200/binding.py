@@ -23,7 +23,7 @@ LIB_PATH = os.path.join(_HERE, "libgamerhydro.so")
 EXPORTS = ["gamer_fluid_advance", "gamer_fluid_advance_ex", "gamer_fluid_advance_retry", "gamer_cfl_dt", "gamer_cfl_dt_ex",
            "gamer_cfl_from_group_speed", "gamer_refresh_ghosts_periodic", "gamer_refresh_ghosts", "gamer_refresh_ghosts_table", "gamer_interpolate_ghosts", "gamer_fluid_advance_resident",
            "gamer_neighbors_periodic", "gamer_restrict", "gamer_flux_accumulate", "gamer_flux_correct",
-           "gamer_fluid_advance_host", "gamer_release_scratch",
+           "gamer_poisson_sor", "gamer_fluid_advance_host", "gamer_release_scratch",
            "gamer_launch_count", "gamer_strerror", "gamer_version"]
 
 
@@ -77,6 +77,7 @@ def lib():
         L.gamer_refresh_ghosts_table.argtypes = [vp, vp, vp, i64, ci, ci, vp]
         L.gamer_fluid_advance_resident.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, ci, ci, ctypes.POINTER(gamer_opts)]
         L.gamer_neighbors_periodic.argtypes = [vp, ci, ci, ci, vp]
+        L.gamer_poisson_sor.argtypes = [vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, vp]
         L.gamer_interpolate_ghosts.argtypes = [vp, vp, dbl, vp, vp, vp, i64, ci, ci, ci, vp]
         L.gamer_restrict.argtypes = [vp, vp, vp, i64, ci, ci, vp]
         L.gamer_flux_accumulate.argtypes = [vp, vp, dbl, i64, ci, ci, ci, vp]
@@ -244,6 +245,16 @@ def gamer_flux_correct(coarse, coarse_flux, fine_flux_avg, table, lam, stream=No
     _check(lib().gamer_flux_correct(_ptr(coarse), _ptr(coarse_flux), _ptr(fine_flux_avg), _ptr(table), table.shape[0],
                                     coarse.shape[1], float(lam), _precision(coarse), _stream_handle(stream)),
            "gamer_flux_correct")
+
+
+def gamer_poisson_sor(phi, rho, acc, dh, coeff, omega, n_iter, stream=None):
+    """Red-black SOR on every patch's 18^3 potential, in place; acc (nullable) [N,3,8,8,8]."""
+    if tuple(phi.shape[1:]) != (18, 18, 18) or tuple(rho.shape) != (phi.shape[0], 16, 16, 16) or rho.dtype != phi.dtype:
+        raise GamerError("phi must be [N,18,18,18] and rho [N,16,16,16] of the same dtype")
+    if acc is not None and (tuple(acc.shape) != (phi.shape[0], 3, 8, 8, 8) or acc.dtype != phi.dtype):
+        raise GamerError("acc must be [N,3,8,8,8] of phi's dtype")
+    _check(lib().gamer_poisson_sor(_ptr(phi), _ptr(rho), _ptr(acc), phi.shape[0], float(dh), float(coeff), float(omega),
+                                   int(n_iter), _precision(phi), _stream_handle(stream)), "gamer_poisson_sor")
 
 
 def gamer_fluid_advance_host(in_host, out_host, flux_out_host, group_speed_out_host, dt, dh, gamma, scheme, recon,

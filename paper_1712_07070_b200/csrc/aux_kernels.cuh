@@ -284,6 +284,52 @@ __global__ void __launch_bounds__(256) interpolate_ghosts_kernel(const T* __rest
     }
 }
 
+// Refined-level Poisson solver (R25): one CTA relaxes one patch's
+// (8 + 2*5)^3 = 18^3 potential, held entirely in shared memory as the paper does (46.7 KB in fp64), by red-black SOR with
+// the outermost cells fixed; thread (k, j) owns row (k, j) of the 16^3 relaxed cells: 8 cells per colour, source term in
+// registers.  Then the potential goes back and, optionally, -grad(phi) of the 8^3 active zones by central differences.
+constexpr int PN = 18, PR = 16, PA0 = 5, PAN = 8;
+template <typename T>
+__global__ void __launch_bounds__(256) poisson_sor_kernel(T* __restrict__ phi, const T* __restrict__ rho, T* __restrict__ acc,
+                                                          T src_scale, T w6, T inv_2dh, int n_iter) {
+    __shared__ T p[PN * PN * PN];
+    const size_t n = blockIdx.x;
+    T* gp = phi + n * (PN * PN * PN);
+    for (int t = threadIdx.x; t < PN * PN * PN; t += 256) p[t] = gp[t];
+    const int k = 1 + threadIdx.x / PR, j = 1 + threadIdx.x % PR;
+    T src[PR];
+    const T* gr = rho + n * (PR * PR * PR) + (size_t)((k - 1) * PR + (j - 1)) * PR;
+#pragma unroll
+    for (int i = 0; i < PR; ++i) src[i] = src_scale * gr[i];
+    __syncthreads();
+    T* row = p + (k * PN + j) * PN;
+    for (int it = 0; it < n_iter; ++it) {
+#pragma unroll
+        for (int colour = 0; colour < 2; ++colour) {
+            const int odd = (colour + j + k + 1) & 1;          // first cell of this colour in the row: i = 1 + odd
+#pragma unroll
+            for (int m = 0; m < PR / 2; ++m) {
+                const int i = 1 + 2 * m;                       // cell i + odd, source index i - 1 + odd
+                T* c = row + i + odd;
+                const T r = c[-1] + c[1] + c[-PN] + c[PN] + c[-PN * PN] + c[PN * PN] - T(6) * c[0] - (odd ? src[i] : src[i - 1]);
+                c[0] += w6 * r;
+            }
+            __syncthreads();
+        }
+    }
+    for (int t = threadIdx.x; t < PN * PN * PN; t += 256) gp[t] = p[t];
+    if (acc) {
+        T* ga = acc + n * (3 * PAN * PAN * PAN);
+        for (int t = threadIdx.x; t < PAN * PAN * PAN; t += 256) {
+            const int ak = t / (PAN * PAN), aj = (t / PAN) % PAN, ai = t % PAN;
+            const T* c = p + ((ak + PA0) * PN + aj + PA0) * PN + ai + PA0;
+            ga[t] = -(c[1] - c[-1]) * inv_2dh;
+            ga[t + PAN * PAN * PAN] = -(c[PN] - c[-PN]) * inv_2dh;
+            ga[t + 2 * PAN * PAN * PAN] = -(c[PN * PN] - c[-PN * PN]) * inv_2dh;
+        }
+    }
+}
+
 // neighbour table of a periodic box of gz x gy x gx groups: nbr[g][(dz+1)*9 + (dy+1)*3 + (dx+1)]
 __global__ void neighbors_periodic_kernel(int* __restrict__ nbr, int gz, int gy, int gx) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
