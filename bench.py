@@ -17,6 +17,7 @@ is the max-reduction of one scalar for dt).
 """
 import argparse
 import json
+import math
 import os
 import sys
 import threading
@@ -309,6 +310,30 @@ def main():
         finite = finite and bool(torch.isfinite(fine_pad).all().item())
         del coarse, acc, parent, fine_pad, nbr_cf
 
+    # ---- extra: the paper's other GPU solver (NEXT-4), SOR Poisson on 18^3 per 8^3 patch, 60 red-black iterations (what fp32
+    # needs to reach round-off from a random guess); "cells" = the 8^3 active zones, as in the paper's Fig. 5
+    poisson = None
+    if world == 1 and args.groups >= 64:
+        npatch = min(8 * args.groups, 65536)
+        gsor = torch.Generator(device=dev).manual_seed(1712)
+        phi = torch.randn((npatch, 18, 18, 18), generator=gsor, dtype=dtype, device=dev)
+        rho_p = torch.randn((npatch, 16, 16, 16), generator=gsor, dtype=dtype, device=dev) + 2.0
+        acc_p = torch.empty((npatch, 3, 8, 8, 8), dtype=dtype, device=dev)
+        om, nit = 2.0 / (1.0 + math.sin(math.pi / 17)), 60
+        gb.gamer_poisson_sor(phi, rho_p, acc_p, dh, 1.0, om, nit, stream)
+        p0, p1 = (torch.cuda.Event(enable_timing=True) for _ in range(2))
+        p0.record(stream)
+        for _ in range(3):
+            gb.gamer_poisson_sor(phi, rho_p, acc_p, dh, 1.0, om, nit, stream)
+        p1.record(stream)
+        torch.cuda.synchronize()
+        tsor = p0.elapsed_time(p1) * 1e-3 / 3
+        poisson = {"cells_per_s": npatch * 512 / tsor, "patches": npatch, "n_iter": nit, "ms": tsor * 1e3,
+                   "relaxations_per_s": npatch * 4096 * nit / tsor,
+                   "hbm_GBs": npatch * (2 * 18 ** 3 + 16 ** 3 + 3 * 512) * sz / tsor / 1e9}
+        finite = finite and bool(torch.isfinite(phi).all().item()) and bool(torch.isfinite(acc_p).all().item())
+        del phi, rho_p, acc_p
+
     # ---- e2e: host buffers through the C ABI, copies inside the timed region
     e2e = None
     if not args.no_e2e:
@@ -396,7 +421,7 @@ def main():
             "dtype": "f32" if sz == 4 else "f64", "data": "synthetic",
             "config": workload_config(args, args.groups), "clocks": sampler.summary(), "e2e": e2e,
             "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
-            "with_ghost_refresh": refresh_value, "with_fused_ghost_refresh": fused_value, "fixup_kernels": fixup, "outputs_finite": finite,
+            "with_ghost_refresh": refresh_value, "with_fused_ghost_refresh": fused_value, "fixup_kernels": fixup, "poisson_sor": poisson, "outputs_finite": finite,
             "paper_context": "P100-PCIe fp32 ~2e8 cells/s incl. PCIe (PAPER.md L318-320); other hardware, not a target"}
     print(json.dumps(line), flush=True)
     if world > 1:
