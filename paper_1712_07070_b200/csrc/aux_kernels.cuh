@@ -289,43 +289,65 @@ __global__ void __launch_bounds__(256) interpolate_ghosts_kernel(const T* __rest
 // the outermost cells fixed; thread (k, j) owns row (k, j) of the 16^3 relaxed cells: 8 cells per colour, source term in
 // registers.  Then the potential goes back and, optionally, -grad(phi) of the 8^3 active zones by central differences.
 constexpr int PN = 18, PR = 16, PA0 = 5, PAN = 8;
+constexpr int PPL = PN * PN + 1;   // plane stride in shared memory: = 1 (mod 4), see the bank note below
+
+// One half-sweep over the cells i = 2 - IP, 4 - IP, ... of the thread's row: x-neighbours from the row's registers, the four
+// others from shared memory, the new value to both.  Same order of additions as the oracle.
+template <typename T, int IP>
+__device__ __forceinline__ void sor_half_sweep(T (&me)[PN], const T (&src)[PR], T* row, T w6) {
+#pragma unroll
+    for (int m = 0; m < PR / 2; ++m) {
+        constexpr int dummy = 0; (void)dummy;
+        const int i = 2 - IP + 2 * m;
+        const T r = me[i - 1] + me[i + 1] + row[i - PN] + row[i + PN] + row[i - PPL] + row[i + PPL] - T(6) * me[i] - src[i - 1];
+        me[i] += w6 * r;
+        row[i] = me[i];
+    }
+}
+
+// Thread layout: warps 0-3 own the rows with (j + k) even, warps 4-7 those with (j + k) odd, so the x-parity of a colour's
+// cells is uniform over a warp and the row can live in registers with static indices.  Lane -> (k, j): r = (warp & 3) * 32 + lane,
+// k = 1 + r / 8, j = 1 + 2 (r % 8) + s with s fixing the parity.  Banks (fp32): 4 k + 4 (r % 8) + 18 s + i with the padded plane
+// stride (= 1 mod 4) puts the 32 lanes of a warp on 32 different banks.
 template <typename T>
 __global__ void __launch_bounds__(256) poisson_sor_kernel(T* __restrict__ phi, const T* __restrict__ rho, T* __restrict__ acc,
                                                           T src_scale, T w6, T inv_2dh, int n_iter) {
-    __shared__ T p[PN * PN * PN];
+    __shared__ T p[PN * PPL];
     const size_t n = blockIdx.x;
     T* gp = phi + n * (PN * PN * PN);
-    for (int t = threadIdx.x; t < PN * PN * PN; t += 256) p[t] = gp[t];
-    const int k = 1 + threadIdx.x / PR, j = 1 + threadIdx.x % PR;
-    T src[PR];
+    for (int t = threadIdx.x; t < PN * PN * PN; t += 256) {
+        const int kk = t / (PN * PN);
+        p[kk * PPL + t - kk * (PN * PN)] = gp[t];
+    }
+    const int par = threadIdx.x >> 7, r = threadIdx.x & 127;
+    const int k = 1 + (r >> 3), j = 1 + 2 * (r & 7) + ((par + k + 1) & 1);
+    T src[PR], me[PN];
     const T* gr = rho + n * (PR * PR * PR) + (size_t)((k - 1) * PR + (j - 1)) * PR;
 #pragma unroll
     for (int i = 0; i < PR; ++i) src[i] = src_scale * gr[i];
     __syncthreads();
-    T* row = p + (k * PN + j) * PN;
+    T* row = p + k * PPL + j * PN;
+#pragma unroll
+    for (int i = 0; i < PN; ++i) me[i] = row[i];
     for (int it = 0; it < n_iter; ++it) {
-#pragma unroll
-        for (int colour = 0; colour < 2; ++colour) {
-            const int odd = (colour + j + k + 1) & 1;          // first cell of this colour in the row: i = 1 + odd
-#pragma unroll
-            for (int m = 0; m < PR / 2; ++m) {
-                const int i = 1 + 2 * m;                       // cell i + odd, source index i - 1 + odd
-                T* c = row + i + odd;
-                const T r = c[-1] + c[1] + c[-PN] + c[PN] + c[-PN * PN] + c[PN * PN] - T(6) * c[0] - (odd ? src[i] : src[i - 1]);
-                c[0] += w6 * r;
-            }
-            __syncthreads();
-        }
+        // colour 0 = cells with (i + j + k) even: i even in the even rows, odd in the odd rows; then colour 1
+        if (par) sor_half_sweep<T, 1>(me, src, row, w6); else sor_half_sweep<T, 0>(me, src, row, w6);
+        __syncthreads();
+        if (par) sor_half_sweep<T, 0>(me, src, row, w6); else sor_half_sweep<T, 1>(me, src, row, w6);
+        __syncthreads();
     }
-    for (int t = threadIdx.x; t < PN * PN * PN; t += 256) gp[t] = p[t];
+    for (int t = threadIdx.x; t < PN * PN * PN; t += 256) {
+        const int kk = t / (PN * PN);
+        gp[t] = p[kk * PPL + t - kk * (PN * PN)];
+    }
     if (acc) {
         T* ga = acc + n * (3 * PAN * PAN * PAN);
         for (int t = threadIdx.x; t < PAN * PAN * PAN; t += 256) {
             const int ak = t / (PAN * PAN), aj = (t / PAN) % PAN, ai = t % PAN;
-            const T* c = p + ((ak + PA0) * PN + aj + PA0) * PN + ai + PA0;
+            const T* c = p + (ak + PA0) * PPL + (aj + PA0) * PN + ai + PA0;
             ga[t] = -(c[1] - c[-1]) * inv_2dh;
             ga[t + PAN * PAN * PAN] = -(c[PN] - c[-PN]) * inv_2dh;
-            ga[t + 2 * PAN * PAN * PAN] = -(c[PN * PN] - c[-PN * PN]) * inv_2dh;
+            ga[t + 2 * PAN * PAN * PAN] = -(c[PPL] - c[-PPL]) * inv_2dh;
         }
     }
 }
