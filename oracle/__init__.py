@@ -2,7 +2,10 @@
 
 Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
 this package.  It never imports paper_1712_07070_b200 (and is never imported by it).
-The arithmetic lives in hydro_oracle.c (plain C, gcc); this file only marshals numpy arrays.
+The solver's arithmetic lives in hydro_oracle.c (plain C, gcc) and is only marshalled here; the operations around it are
+written out in this file in plain numpy / Python loops: ghost filling (fill_ghosts, fill_ghosts_table), the coarse->fine
+ghost interpolation (interpolate_ghosts), the time-step retry loop (fluid_advance_retry) and the SOR Poisson solver
+(poisson_sor).  Every function is pinned by tests/test_oracle_*.py; none is "parity unpinned".
 """
 import ctypes
 import os
