@@ -355,3 +355,14 @@ def poisson_sor(phi, rho, dh, coeff, omega, n_iter, want_acc=True):
                         -(phi[:, a, 6:14, a] - phi[:, a, 4:12, a]) / (2.0 * dh),
                         -(phi[:, 6:14, a, a] - phi[:, 4:12, a, a]) / (2.0 * dh)], axis=1)
     return phi, acc
+
+
+def poisson_residual(phi, rho, dh, coeff):
+    """Per patch, the largest |phi(i-1) + phi(i+1) + phi(j-1) + phi(j+1) + phi(k-1) + phi(k+1) - 6 phi - coeff dh^2 rho| over
+    the 16^3 relaxed cells: dh^2 times the defect of the discretised Poisson equation of PAPER.md L126 (zero "to machine
+    precision" once the relaxation has converged).  phi [N,18,18,18], rho [N,16,16,16] -> [N]."""
+    phi = np.asarray(phi, dtype=np.float64)
+    c = phi[:, 1:17, 1:17, 1:17]
+    r = (phi[:, 1:17, 1:17, 0:16] + phi[:, 1:17, 1:17, 2:18] + phi[:, 1:17, 0:16, 1:17] + phi[:, 1:17, 2:18, 1:17]
+         + phi[:, 0:16, 1:17, 1:17] + phi[:, 2:18, 1:17, 1:17] - 6.0 * c - coeff * dh * dh * np.asarray(rho, dtype=np.float64))
+    return np.abs(r).reshape(phi.shape[0], -1).max(axis=1)

@@ -80,3 +80,27 @@ def test_sor_fixed_point_sweep_definition_and_acceleration(oracle_mod):
                         p[k, j, i] += omega * r / 6
     got, _ = oracle_mod.poisson_sor(phi0, rho, dh, coeff, omega, 1, want_acc=False)
     assert np.abs(got[0] - p).max() <= 1e-14 * np.abs(p).max()
+
+
+def test_residual_definition_and_decay(oracle_mod):
+    """poisson_residual: zero for the quadratic exact solution and (to round-off) for the sparse-LU solution; equal to the defect
+    of one cell written out by hand when a single cell of an exact solution is perturbed (the cell itself sees -6 eps, its six
+    neighbours +eps); monotonically smaller as SOR proceeds."""
+    dh, coeff = 0.5, 2.5
+    x = (np.arange(18) - 8.5) * dh
+    Z, Y, X = np.meshgrid(x, x, x, indexing="ij")
+    quad = (X ** 2 + 2 * Y ** 2 - Z ** 2)[None]
+    rho = np.full((1, 16, 16, 16), 4.0 / coeff)
+    assert oracle_mod.poisson_residual(quad, rho, dh, coeff)[0] <= 1e-12
+    bumped = quad.copy()
+    bumped[0, 7, 9, 4] += 0.125
+    assert abs(oracle_mod.poisson_residual(bumped, rho, dh, coeff)[0] - 6 * 0.125) <= 1e-12
+    bumped = quad.copy()
+    bumped[0, 0, 9, 4] += 0.125                                   # a boundary cell: only its one inner neighbour sees it
+    assert abs(oracle_mod.poisson_residual(bumped, rho, dh, coeff)[0] - 0.125) <= 1e-12
+    phi0, rho = _problem(3)
+    omega = 2.0 / (1.0 + np.sin(np.pi / 17))
+    res = [oracle_mod.poisson_residual(oracle_mod.poisson_sor(phi0, rho, dh, coeff, omega, n, want_acc=False)[0], rho, dh, coeff).max()
+           for n in (0, 5, 20, 60, 200)]
+    assert all(a > b for a, b in zip(res, res[1:])) and res[-1] <= 1e-12 * np.abs(phi0).max()
+    assert oracle_mod.poisson_residual(_direct(phi0, rho, dh, coeff), rho, dh, coeff).max() <= 1e-12 * np.abs(phi0).max()
