@@ -209,8 +209,11 @@ int gamer_flux_correct(void* coarse, const void* coarse_flux, const void* fine_f
  * and the boundary condition on the outermost layer, which is returned unchanged; rho[n_patches][16][16][16]: the density on
  * the relaxed cells; acc (nullable) [n_patches][3][8][8][8] = -grad(phi) on the active zones (cells 5..12) by central
  * differences, components (x, y, z) (L238: "the cell-centered gravitational acceleration ... immediately after solving the
- * potential").  0 < omega < 2; n_iter >= 0; the potential lives in shared memory for the whole solve (46.7 KB in fp64). */
-int gamer_poisson_sor(void* phi, const void* rho, void* acc, int64_t n_patches, double dh, double coeff,
+ * potential").  resid_out (nullable) real[n_patches] = max over the relaxed cells of |sum of the 6 neighbours - 6 phi -
+ * coeff * dh^2 * rho| after the last iteration: dh^2 times the defect of the discretised equation, for the caller to judge "to
+ * machine precision" (L126) and iterate on.  0 < omega < 2; n_iter >= 0; the potential lives in shared memory for the whole
+ * solve (46.8 KB in fp64). */
+int gamer_poisson_sor(void* phi, const void* rho, void* acc, void* resid_out, int64_t n_patches, double dh, double coeff,
                       double omega, int n_iter, int precision, void* stream);
 
 /* End-to-end form with HOST buffers (pinned or pageable): copies `in` to the device in chunks,

@@ -77,7 +77,7 @@ def lib():
         L.gamer_refresh_ghosts_table.argtypes = [vp, vp, vp, i64, ci, ci, vp]
         L.gamer_fluid_advance_resident.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, ci, ci, ctypes.POINTER(gamer_opts)]
         L.gamer_neighbors_periodic.argtypes = [vp, ci, ci, ci, vp]
-        L.gamer_poisson_sor.argtypes = [vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, vp]
+        L.gamer_poisson_sor.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, vp]
         L.gamer_interpolate_ghosts.argtypes = [vp, vp, dbl, vp, vp, vp, i64, ci, ci, ci, vp]
         L.gamer_restrict.argtypes = [vp, vp, vp, i64, ci, ci, vp]
         L.gamer_flux_accumulate.argtypes = [vp, vp, dbl, i64, ci, ci, ci, vp]
@@ -247,13 +247,15 @@ def gamer_flux_correct(coarse, coarse_flux, fine_flux_avg, table, lam, stream=No
            "gamer_flux_correct")
 
 
-def gamer_poisson_sor(phi, rho, acc, dh, coeff, omega, n_iter, stream=None):
+def gamer_poisson_sor(phi, rho, acc, dh, coeff, omega, n_iter, stream=None, resid_out=None):
     """Red-black SOR on every patch's 18^3 potential, in place; acc (nullable) [N,3,8,8,8]."""
     if tuple(phi.shape[1:]) != (18, 18, 18) or tuple(rho.shape) != (phi.shape[0], 16, 16, 16) or rho.dtype != phi.dtype:
         raise GamerError("phi must be [N,18,18,18] and rho [N,16,16,16] of the same dtype")
     if acc is not None and (tuple(acc.shape) != (phi.shape[0], 3, 8, 8, 8) or acc.dtype != phi.dtype):
         raise GamerError("acc must be [N,3,8,8,8] of phi's dtype")
-    _check(lib().gamer_poisson_sor(_ptr(phi), _ptr(rho), _ptr(acc), phi.shape[0], float(dh), float(coeff), float(omega),
+    if resid_out is not None and (tuple(resid_out.shape) != (phi.shape[0],) or resid_out.dtype != phi.dtype):
+        raise GamerError("resid_out must be [N] of phi's dtype")
+    _check(lib().gamer_poisson_sor(_ptr(phi), _ptr(rho), _ptr(acc), _ptr(resid_out), phi.shape[0], float(dh), float(coeff), float(omega),
                                    int(n_iter), _precision(phi), _stream_handle(stream)), "gamer_poisson_sor")
 
 

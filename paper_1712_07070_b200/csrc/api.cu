@@ -317,8 +317,8 @@ extern "C" int gamer_interpolate_ghosts(const void* coarse_in, const void* coars
     return cudaGetLastError() == cudaSuccess ? GAMER_OK : GAMER_ECUDA;
 }
 
-extern "C" int gamer_poisson_sor(void* phi, const void* rho, void* acc, int64_t n_patches, double dh, double coeff,
-                                 double omega, int n_iter, int precision, void* stream) {
+extern "C" int gamer_poisson_sor(void* phi, const void* rho, void* acc, void* resid_out, int64_t n_patches, double dh,
+                                 double coeff, double omega, int n_iter, int precision, void* stream) {
     if (n_patches < 0 || n_iter < 0 || (precision != GAMER_FP32 && precision != GAMER_FP64)) return GAMER_EINVAL;
     if (!(dh > 0.0) || !std::isfinite(dh) || !std::isfinite(coeff) || !(omega > 0.0) || !(omega < 2.0)) return GAMER_EINVAL;
     if (n_patches > 0 && (!phi || !rho || !aligned16(phi) || !aligned16(rho))) return GAMER_EINVAL;
@@ -329,10 +329,11 @@ extern "C" int gamer_poisson_sor(void* phi, const void* rho, void* acc, int64_t 
     const double ss = coeff * dh * dh, w6 = omega / 6.0, i2 = 1.0 / (2.0 * dh);
     if (precision == GAMER_FP32)
         poisson_sor_kernel<float><<<grid, 256, 0, st>>>(static_cast<float*>(phi), static_cast<const float*>(rho),
-                                                        static_cast<float*>(acc), (float)ss, (float)w6, (float)i2, n_iter);
+                                                        static_cast<float*>(acc), static_cast<float*>(resid_out), (float)ss, (float)w6,
+                                                        (float)i2, n_iter);
     else
         poisson_sor_kernel<double><<<grid, 256, 0, st>>>(static_cast<double*>(phi), static_cast<const double*>(rho),
-                                                         static_cast<double*>(acc), ss, w6, i2, n_iter);
+                                                         static_cast<double*>(acc), static_cast<double*>(resid_out), ss, w6, i2, n_iter);
     g_launches += 1;
     return cudaGetLastError() == cudaSuccess ? GAMER_OK : GAMER_ECUDA;
 }

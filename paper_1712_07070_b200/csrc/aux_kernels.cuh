@@ -311,7 +311,7 @@ __device__ __forceinline__ void sor_half_sweep(T (&me)[PN], const T (&src)[PR], 
 // stride (= 1 mod 4) puts the 32 lanes of a warp on 32 different banks.
 template <typename T>
 __global__ void __launch_bounds__(256) poisson_sor_kernel(T* __restrict__ phi, const T* __restrict__ rho, T* __restrict__ acc,
-                                                          T src_scale, T w6, T inv_2dh, int n_iter) {
+                                                          T* __restrict__ resid, T src_scale, T w6, T inv_2dh, int n_iter) {
     __shared__ T p[PN * PPL];
     const size_t n = blockIdx.x;
     T* gp = phi + n * (PN * PN * PN);
@@ -335,6 +335,23 @@ __global__ void __launch_bounds__(256) poisson_sor_kernel(T* __restrict__ phi, c
         __syncthreads();
         if (par) sor_half_sweep<T, 0>(me, src, row, w6); else sor_half_sweep<T, 1>(me, src, row, w6);
         __syncthreads();
+    }
+    if (resid) {
+        // defect of the discretised equation after the last iteration, max over the patch (order-independent: reproducible)
+        __shared__ T wmax[8];
+        T m = T(0);
+#pragma unroll
+        for (int i = 1; i <= PR; ++i)
+            m = fmax(m, fabs(me[i - 1] + me[i + 1] + row[i - PN] + row[i + PN] + row[i - PPL] + row[i + PPL] - T(6) * me[i] - src[i - 1]));
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+        if ((threadIdx.x & 31) == 0) wmax[threadIdx.x >> 5] = m;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+#pragma unroll
+            for (int w = 1; w < 8; ++w) m = fmax(m, wmax[w]);
+            resid[n] = m;
+        }
     }
     for (int t = threadIdx.x; t < PN * PN * PN; t += 256) {
         const int kk = t / (PN * PN);

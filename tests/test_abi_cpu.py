@@ -93,9 +93,9 @@ def test_argument_validation_needs_no_gpu(built_lib):
     assert interp(c1=vp(16384), w=1.5) == -1 and interp(c1=vp(16384), w=float("nan")) == -1
     assert interp(f=ok[0]) == -1                                # in place
     assert interp(n=0) == 0
-    L.gamer_poisson_sor.argtypes = [vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, vp]
+    L.gamer_poisson_sor.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, vp]
     sor = lambda phi=ok[0], rho=ok[1], n=1, dh=0.1, coeff=1.0, omega=1.5, it=10, prec=8: \
-        L.gamer_poisson_sor(phi, rho, None, n, dh, coeff, omega, it, prec, None)
+        L.gamer_poisson_sor(phi, rho, None, None, n, dh, coeff, omega, it, prec, None)
     assert sor(phi=None) == -1 and sor(rho=None) == -1 and sor(phi=vp(4100)) == -1
     assert sor(omega=2.0) == -1 and sor(omega=0.0) == -1 and sor(dh=0.0) == -1 and sor(it=-1) == -1 and sor(prec=2) == -1
     assert sor(coeff=float("inf")) == -1 and sor(n=-1) == -1

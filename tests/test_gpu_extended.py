@@ -541,12 +541,17 @@ def test_poisson_sor_matches_oracle(dev, oracle_mod, dtype):
         ref_phi, ref_acc = oracle_mod.poisson_sor(phi0.double().numpy(), rho.double().numpy(), dh, coeff, omega, n_iter)
         phi = phi0.to(dev).clone()
         acc = torch.full((n, 3, 8, 8, 8), float("nan"), dtype=dtype, device=dev)
-        gb.gamer_poisson_sor(phi, rho.to(dev), acc, dh, coeff, omega, n_iter)
+        res = torch.full((n,), float("nan"), dtype=dtype, device=dev)
+        gb.gamer_poisson_sor(phi, rho.to(dev), acc, dh, coeff, omega, n_iter, resid_out=res)
         torch.cuda.synchronize()
         got = phi.cpu().double().numpy()
         assert np.abs(got - ref_phi).max() <= tol * np.abs(ref_phi).max(), n_iter
         assert np.array_equal(got[:, edge], phi0.double().numpy()[:, edge])
         assert np.abs(acc.cpu().double().numpy() - ref_acc).max() <= 10 * tol * np.abs(ref_acc).max(), n_iter
+        ref_res = oracle_mod.poisson_residual(ref_phi, rho.double().numpy(), dh, coeff)
+        assert np.abs(res.cpu().double().numpy() - ref_res).max() <= 50 * tol * np.abs(ref_phi).max(), n_iter
+        if n_iter == 200:
+            assert res.max().item() <= 50 * tol * np.abs(ref_phi).max()        # converged: defect at round-off
     phi2 = phi0.to(dev).clone()
     gb.gamer_poisson_sor(phi2, rho.to(dev), None, dh, coeff, omega, 200)
     assert torch.equal(phi2, phi)                                     # acc = NULL: same potential, bitwise (run to run too)
