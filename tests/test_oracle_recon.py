@@ -165,3 +165,80 @@ def test_characteristic_limiting_is_R_minmod_L(oracle_mod):
     pr = np.array([oracle_mod.limited_slope(oracle_mod.GMINMOD, 1.0, a, b) for a, b in zip(dl, dr)])
     assert np.abs(ch - pr).max() > 1e-3
     assert abs((L @ ch)[0]) <= 1e-15                                                         # that wave got no slope
+
+
+def test_ppm_monotonisation_overshoot_branches_hand_computed(oracle_mod):
+    """Colella & Woodward (1984) eq. 1.10, the two overshoot branches, on steep monotone data worked out by hand
+    (PAPER.md L94 names PPM after that paper; R5: limited slopes with theta = 2, no steepening / flattening).
+
+    Cell values a = (0, 0, 1/10, 1, 1), centre a_j = 1/10:
+      slopes (gen. minmod, theta = 2; CW84 eq. 1.8): da_{j-1} = 0 (left difference is 0), da_{j+1} = 0,
+        da_j = min(2*(1/10), |1 - 0|/2, 2*(9/10)) = 1/5;
+      interface values (eq. 1.6): a_{j-1/2} = (0 + 1/10)/2 - (1/5 - 0)/6 = 1/20 - 1/30 = 1/60,
+                                  a_{j+1/2} = (1/10 + 1)/2 - (0 - 1/5)/6 = 11/20 + 1/30 = 7/12;
+      (a_R - a)(a - a_L) = (29/60)(1/12) > 0, so the cell is not an extremum;
+      D = a_R - a_L = 17/30, C = a - (a_L + a_R)/2 = 1/10 - 3/10 = -1/5:  D*C = -17/150 < -D^2/6 = -289/5400,
+      third line of eq. 1.10:  a_R <- 3a - 2a_L = 3/10 - 1/30 = 4/15.    Result (1/60, 4/15).
+    The mirrored data (1, 1, 1/10, 0, 0) take the second line of eq. 1.10 (D*C = +17/150 > D^2/6):
+      a_L <- 3a - 2a_R = 4/15, a_R = 1/60.
+    Cell values (0, 0, 9/10, 1, 1): da_j = min(9/5, 1/2, 1/5) = 1/5, a_L = 9/20 - 1/30 = 5/12,
+      a_R = 19/20 + 1/30 = 59/60, D = 17/30, C = 9/10 - 7/10 = 1/5, D*C = 17/150 > D^2/6:
+      a_L <- 3a - 2a_R = 27/10 - 59/30 = 11/15.                       Result (11/15, 59/60); mirror (59/60, 11/15).
+    A formula such as 2a - a_R in place of 3a - 2a_R (which also removes the overshoot and keeps |a_6| <= |a_R - a_L|)
+    gives 11/60 / 49/60 here and fails."""
+    from fractions import Fraction as Fr
+    cases = [((0, 0, Fr(1, 10), 1, 1), (Fr(1, 60), Fr(4, 15))),
+             ((1, 1, Fr(1, 10), 0, 0), (Fr(4, 15), Fr(1, 60))),
+             ((0, 0, Fr(9, 10), 1, 1), (Fr(11, 15), Fr(59, 60))),
+             ((1, 1, Fr(9, 10), 0, 0), (Fr(59, 60), Fr(11, 15)))]
+    for w, (em, ep) in cases:
+        wm, wp = oracle_mod.face_values(PPM, np.array([float(x) for x in w]))
+        assert abs(wm - float(em)) <= 1e-15 and abs(wp - float(ep)) <= 1e-15, (w, wm, wp)
+        # the monotonised parabola touches zero slope exactly at the far edge: |a_6| = |a_R - a_L|
+        assert abs(abs(6 * (float(w[2]) - 0.5 * (wm + wp))) - abs(wp - wm)) <= 1e-15
+    # shifted and scaled copies of the first case (the operation is affine-equivariant)
+    for shift, scale in ((2.5, 1.0), (-1.0, 3.0), (0.25, -2.0)):
+        w = np.array([shift + scale * float(x) for x in cases[0][0]])
+        wm, wp = oracle_mod.face_values(PPM, w)
+        assert wm == pytest.approx(shift + scale / 60.0, abs=4e-15) and wp == pytest.approx(shift + scale * 4.0 / 15.0, abs=4e-15)
+
+
+@pytest.mark.parametrize("scheme", [1, 2])
+def test_ppm_overshoot_branches_in_the_characteristic_limited_step(oracle_mod, scheme):
+    """The step keeps a second copy of the PPM monotonisation for slopes limited in characteristic variables
+    (R22).  On a pure contact (uniform velocity and pressure) the characteristic amplitudes of a density
+    jump are (0, d rho, 0, 0, 0), so that copy must reproduce the primitive-variable face values, which the test above
+    pins -- on data made of the hand-computed steep steps, so that both overshoot branches are taken.  Reference:
+    the 1-D closed forms of tests/test_oracle_step.py (CTU: average over the domain of dependence; MHM: Hancock half
+    step), built from oracle.face_values."""
+    import torch
+    from helpers import oracle_step
+    from paper_1712_07070_b200 import inputs
+    n = 32
+    rho1 = np.full(n, 1.0)
+    rho1[4:9] = 1.0 + np.array([0.0, 0.0, 0.1, 1.0, 1.0])      # the four hand-computed patterns, on a pedestal of 1
+    rho1[9:12] = 2.0
+    rho1[12:17] = 1.0 + np.array([1.0, 1.0, 0.1, 0.0, 0.0])
+    rho1[20:25] = 1.0 + np.array([0.0, 0.0, 0.9, 1.0, 1.0])
+    rho1[25:27] = 2.0
+    rho1[27:32] = 1.0 + np.array([1.0, 1.0, 0.9, 0.0, 0.0])
+    rho = torch.from_numpy(rho1)[None, None, :].expand(16, 16, n).contiguous()
+    one = torch.ones_like(rho)
+    v = 0.7
+    f = inputs.prim_to_cons(rho, v * one, 0 * one, 0 * one, one, 1.4)
+    dh, dt = 1.0 / n, 0.4 / n
+    nu = v * dt / dh
+    new, _ = oracle_step(oracle_mod, f, dt, dh, 1.4, scheme, PPM, 2, opts=oracle_mod.make_opts(char_limiting=True))
+    face, hit = np.empty(n), 0
+    for i in range(n):
+        w5 = np.array([rho1[(i + m) % n] for m in range(-2, 3)])
+        wm, wp = oracle_mod.face_values(PPM, w5)
+        d, w6 = wp - wm, 6 * (rho1[i] - 0.5 * (wm + wp))
+        hit += abs(abs(w6) - abs(d)) < 1e-14 and abs(d) > 0.1
+        if scheme == 2:      # CTU: average of the parabola over [x_f - v dt, x_f]
+            face[i] = wp - 0.5 * nu * (d - (1 - 2.0 / 3.0 * nu) * w6)
+        else:                # MHM: face value minus half the flux difference across the cell
+            face[i] = wp - 0.5 * nu * d
+    assert hit >= 4                                           # the overshoot branches were taken
+    ref = rho1 - nu * (face - np.roll(face, 1))
+    assert np.abs(new[0, 2, 7].numpy() - ref).max() <= 5e-14
