@@ -152,6 +152,8 @@ def main():
     ap.add_argument("--groups", type=int, default=32768, help="patch groups per GPU (must be a cube of an integer)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-variants", action="store_true", help="skip the other three configs[3] variants")
+    ap.add_argument("--no-extras", action="store_true", help="skip the NEXT-row extras (refresh, fix-up, Poisson)")
     args = ap.parse_args()
     if args.impl == "reference":
         if args.steps > 5:
@@ -184,60 +186,69 @@ def main():
     # ---- synthetic input, built on the device (seed differs per rank: every rank owns its own box)
     field = inputs.turbulence_field(n, 7070 + rank, kmax=16, gamma=gamma, device=dev)
     u_in = inputs.pack_periodic(field, dtype=dtype)
-    del field
+    if world > 1 or args.no_variants:
+        del field
     torch.cuda.empty_cache()
     out, flux, speed = gb.alloc_outputs(u_in)
     dt_dev = torch.zeros(1, dtype=torch.float64, device=dev)
-    gb.gamer_cfl_dt(inputs.interior(u_in[:64]).contiguous(), dh, gamma, cfl, scheme, None, dt_dev)   # a valid first dt
     stream = torch.cuda.current_stream()
-    opts = gb.make_opts(stream=stream, dt_dev=dt_dev, group_speed_out=speed)
-
-    def step():
-        gb.gamer_fluid_advance_ex(u_in, out, flux, 1.0, dh, gamma, scheme, recon, solver, opts)
-        gb.gamer_cfl_from_group_speed(speed, dh, cfl, dt_dev, stream)
-        if world > 1:
-            dist.all_reduce(dt_dev, op=dist.ReduceOp.MIN)        # the one exchange: 1 scalar
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(args.warmup, 3)):
-        step()
-    barrier()
+    def time_variant(u, o, fl, sp, sch, rec, sol, c, nsteps, nwarm):
+        """nwarm untimed + nsteps timed passes of the hot path (advance + dt) on one resident batch; CUDA events on the
+        launching stream: whole loop and each advance launch."""
+        gb.gamer_cfl_dt(inputs.interior(u[:64]).contiguous(), dh, gamma, c, sch, None, dt_dev)   # a valid first dt
+        o_ = gb.make_opts(stream=stream, dt_dev=dt_dev, group_speed_out=sp)
+
+        def one():
+            gb.gamer_fluid_advance_ex(u, o, fl, 1.0, dh, gamma, sch, rec, sol, o_)
+            gb.gamer_cfl_from_group_speed(sp, dh, c, dt_dev, stream)
+            if world > 1:
+                dist.all_reduce(dt_dev, op=dist.ReduceOp.MIN)        # the one exchange: 1 scalar
+
+        for _ in range(nwarm):
+            one()
+        barrier()
+        l0 = gb.gamer_launch_count()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        kev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(nsteps)]
+        barrier()
+        ev0.record(stream)
+        for i in range(nsteps):
+            kev[i][0].record(stream)
+            gb.gamer_fluid_advance_ex(u, o, fl, 1.0, dh, gamma, sch, rec, sol, o_)
+            kev[i][1].record(stream)
+            gb.gamer_cfl_from_group_speed(sp, dh, c, dt_dev, stream)
+            if world > 1:
+                dist.all_reduce(dt_dev, op=dist.ReduceOp.MIN)
+        ev1.record(stream)
+        barrier()
+        nl = gb.gamer_launch_count() - l0
+        tot = ev0.elapsed_time(ev1)
+        kms = sum(a.elapsed_time(b) for a, b in kev) / nsteps
+        t = torch.tensor([tot], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ok = bool(torch.isfinite(o).all().item()) and bool(torch.isfinite(dt_dev).all().item())
+        return t.item(), kms, nl, ok, one
+
+    opts = gb.make_opts(stream=stream, dt_dev=dt_dev, group_speed_out=speed)
     sampler = ClockSampler(local)
     sampler.start()
-    l0 = gb.gamer_launch_count()
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
-    kev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    barrier()
-    ev[0].record(stream)
-    for i in range(args.steps):
-        kev[i][0].record(stream)
-        gb.gamer_fluid_advance_ex(u_in, out, flux, 1.0, dh, gamma, scheme, recon, solver, opts)
-        kev[i][1].record(stream)
-        gb.gamer_cfl_from_group_speed(speed, dh, cfl, dt_dev, stream)
-        if world > 1:
-            dist.all_reduce(dt_dev, op=dist.ReduceOp.MIN)
-        ev[i + 1].record(stream)
-    barrier()
-    launches = gb.gamer_launch_count() - l0
+    total_ms, kern_ms, launches, finite, step = time_variant(u_in, out, flux, speed, scheme, recon, solver, cfl,
+                                                            args.steps, max(args.warmup, 3))
     sampler.stop_flag = True
-    total_ms = ev[0].elapsed_time(ev[-1])
-    kern_ms = sum(a.elapsed_time(b) for a, b in kev) / args.steps
-    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms = t.item()
     cells = args.groups * CELLS
     value = world * cells * args.steps / (total_ms * 1e-3)
-    finite = bool(torch.isfinite(out).all().item()) and bool(torch.isfinite(dt_dev).all().item())
 
     # ---- extra: the same loop with the device-side periodic ghost refresh included (NEXT-1 row)
     refresh_value = None
-    if world == 1:
-        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if world == 1 and not args.no_extras:
         nref = max(2, min(5, args.steps))
         a0.record(stream)
         for _ in range(nref):
@@ -250,7 +261,7 @@ def main():
     # ---- extra: the fused form of the same loop (gamer_fluid_advance_resident: unpadded state + neighbour table,
     # ghost zones gathered inside the solver) -- two unpadded buffers ping-pong, no padded batch is touched
     fused_value = None
-    if world == 1:
+    if world == 1 and not args.no_extras:
         nbr = gb.gamer_neighbors_periodic(gside, gside, gside, dev)
         ua, ub = out, torch.empty_like(out)
         nref = max(2, min(5, args.steps))
@@ -269,7 +280,7 @@ def main():
     # ---- extra: the L112 fix-up kernels (NEXT-2) on this batch taken as a fine level: restriction of all groups into
     # groups/8 parent groups, and the time-averaging pass over flux_out; both are pure HBM streams
     fixup = None
-    if world == 1 and args.groups >= 64:
+    if world == 1 and args.groups >= 64 and not args.no_extras:
         nf = (args.groups // 8) * 8
         parent = torch.arange(nf, dtype=torch.int32, device=dev)          # fine g -> octant g % 8 of coarse g // 8
         coarse = torch.empty((nf // 8,) + tuple(out.shape[1:]), dtype=dtype, device=dev)
@@ -313,7 +324,7 @@ def main():
     # ---- extra: the paper's other GPU solver (NEXT-4), SOR Poisson on 18^3 per 8^3 patch, 60 red-black iterations (what fp32
     # needs to reach round-off from a random guess); "cells" = the 8^3 active zones, as in the paper's Fig. 5
     poisson = None
-    if world == 1 and args.groups >= 64:
+    if world == 1 and args.groups >= 64 and not args.no_extras:
         npatch = min(8 * args.groups, 65536)
         gsor = torch.Generator(device=dev).manual_seed(1712)
         phi = torch.randn((npatch, 18, 18, 18), generator=gsor, dtype=dtype, device=dev)
@@ -368,34 +379,84 @@ def main():
             dist.destroy_process_group()
         return
 
+    # ---- measured plain-ALU peaks (gamer_alu_peak: dependent-free streams, same process, same clocks)
     hbm_peak, sm_max, which = peaks()
-    bpc = algorithmic_bytes_per_cell(recon, sz)
-    key = f"{args.scheme}_{args.recon}_{args.riemann}_{args.precision}"
-    fpc = FLOPS_PER_CELL.get(key)
-    lanes = 128 if sz == 4 else 64
-    alu_peak = 148 * lanes * 2 * sm_max * 1e6 / 1e12          # TFLOP/s, DESIGN.md "Rooflines"
-    hbm_ach = bpc * cells / (kern_ms * 1e-3) / 1e9
-    roofline = {"kernel": "mhm_kernel" if scheme == 1 else "ctu_kernel"}
-    if fpc:
-        ach = fpc * cells / (kern_ms * 1e-3) / 1e12
-        roofline.update({"bound": "alu", "achieved": ach, "peak": alu_peak, "unit": "TFLOP/s", "frac": ach / alu_peak,
-                         "flops_per_cell": fpc, "peak_source": f"148 SMs x {lanes} lanes x 2 x {sm_max} MHz"})
-    else:
-        roofline.update({"bound": "hbm", "achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_ach / hbm_peak})
-    ipc = FLOPS_PER_CELL.get(key + "_inst_per_cell")
-    if ipc:      # instruction-issue view of the same launch: warp instructions per second against 1 / clock / SM sub-partition
-        issue_peak = 148 * 4 * sm_max * 1e6 / 1e9
-        issue_ach = ipc / 32.0 * cells / (kern_ms * 1e-3) / 1e9
-        roofline["issue"] = {"achieved": issue_ach, "peak": issue_peak, "unit": "G warp-inst/s", "frac": issue_ach / issue_peak,
-                             "warp_inst_x32_per_cell": ipc,
-                             "note": "FP32 adds/multiplies count 1 FLOP but take the same issue slot as an FMA, and compares, "
-                                     "selects, min/max and shared-memory traffic take slots too: the FMA-only peak is not "
-                                     "reachable by this instruction mix (DESIGN.md section 6)"}
-    tr = FLOPS_PER_CELL.get(key + "_dram_bytes_per_cell")
-    roofline["traffic"] = tr * cells if tr else None
-    roofline["hbm"] = {"achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_ach / hbm_peak,
-                       "bytes_per_cell": bpc, "peak_source": which}
-    roofline["kernel_ms"] = kern_ms
+    alu = {}
+    for name, kind in (("ffma", gb.ALU_FFMA), ("dfma", gb.ALU_DFMA), ("fmul_fadd", gb.ALU_FMUL_FADD),
+                       ("ffma_fmnmx", gb.ALU_FFMA_FMNMX), ("ffma2", gb.ALU_FFMA2), ("ffma2_fmnmx", gb.ALU_FFMA2_FMNMX),
+                       ("ffma_mufu", gb.ALU_FFMA_MUFU)):
+        tf, gi = gb.gamer_alu_peak(kind, stream)
+        alu[name] = {"tflops": tf, "gwarpinst_per_s": gi}
+    alu["issue_slots_gwarpinst_per_s"] = 148 * 4 * sm_max * 1e6 / 1e9
+    alu["capture_commit"] = FLOPS_PER_CELL.get("capture_commit")
+
+    def roofline_of(sch_name, rec_name, sol_name, prec, kms):
+        szv = 4 if prec == "fp32" else 8
+        bpc = algorithmic_bytes_per_cell(RECONS[rec_name], szv)
+        key = f"{sch_name}_{rec_name}_{sol_name}_{prec}"
+        fpc = FLOPS_PER_CELL.get(key)
+        lanes = 128 if szv == 4 else 64
+        derived = 148 * lanes * 2 * sm_max * 1e6 / 1e12          # TFLOP/s, DESIGN.md "Rooflines"
+        measured = alu["ffma" if szv == 4 else "dfma"]["tflops"]
+        hbm_ach = bpc * cells / (kms * 1e-3) / 1e9
+        r = {"kernel": "mhm_kernel" if sch_name == "mhm" else "ctu_kernel"}
+        if fpc:
+            ach = fpc * cells / (kms * 1e-3) / 1e12
+            r.update({"bound": "alu", "achieved": ach, "peak": measured, "unit": "TFLOP/s", "frac": ach / measured,
+                      "flops_per_cell": fpc,
+                      "peak_source": f"measured {'FFMA' if szv == 4 else 'DFMA'} stream (gamer_alu_peak), {measured:.2f} TFLOP/s "
+                                     f"at {sm_max:.0f} MHz max SM clock; derived 148 SMs x {lanes} lanes x 2 x clock = {derived:.2f}",
+                      "peak_derived": derived, "frac_of_derived": ach / derived,
+                      "flops_capture_commit": FLOPS_PER_CELL.get("capture_commit")})
+        else:
+            r.update({"bound": "hbm", "achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_ach / hbm_peak})
+        ipc = FLOPS_PER_CELL.get(key + "_inst_per_cell")
+        if ipc:      # instruction-issue view of the same launch: warp instructions per second against 1 / clock / SM sub-partition
+            issue_peak = alu["issue_slots_gwarpinst_per_s"]
+            issue_ach = ipc / 32.0 * cells / (kms * 1e-3) / 1e9
+            r["issue"] = {"achieved": issue_ach, "peak": issue_peak, "unit": "G warp-inst/s", "frac": issue_ach / issue_peak,
+                          "warp_inst_x32_per_cell": ipc}
+        tr = FLOPS_PER_CELL.get(key + "_dram_bytes_per_cell")
+        r["traffic"] = tr * cells if tr else None
+        r["hbm"] = {"achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_ach / hbm_peak,
+                    "bytes_per_cell": bpc, "peak_source": which}
+        r["kernel_ms"] = kms
+        return r
+
+    roofline = roofline_of(args.scheme, args.recon, args.riemann, args.precision, kern_ms)
+
+    # ---- the four variants BASELINE.json configs[3] names, on the same batch (fp64: the same field packed in fp64)
+    variants = None
+    if world == 1 and not args.no_variants:
+        variants = []
+        vsteps = max(3, min(10, args.steps))
+        bufs = {"fp32": (u_in, out, flux, speed) if sz == 4 else None, "fp64": (u_in, out, flux, speed) if sz == 8 else None}
+        for sch_name, rec_name, sol_name, prec in (("mhm", "plm", "roe", "fp32"), ("ctu", "ppm", "hllc", "fp32"),
+                                                   ("mhm", "plm", "roe", "fp64"), ("ctu", "ppm", "hllc", "fp64")):
+            if (sch_name, rec_name, sol_name, prec) == (args.scheme, args.recon, args.riemann, args.precision):
+                v_total, v_kms, v_steps, v_ok = total_ms, kern_ms, args.steps, finite
+            else:
+                if bufs[prec] is None:
+                    for other in list(bufs):      # free the other precision's batch first
+                        if other != prec and bufs[other] is not None and bufs[other][0] is not u_in:
+                            bufs[other] = None
+                    torch.cuda.empty_cache()
+                    vt = torch.float32 if prec == "fp32" else torch.float64
+                    vu = inputs.pack_periodic(field, dtype=vt)
+                    bufs[prec] = (vu,) + gb.alloc_outputs(vu)
+                vu, vo, vf, vs = bufs[prec]
+                sch = SCHEMES[sch_name]
+                v_total, v_kms, _, v_ok, _ = time_variant(vu, vo, vf, vs, sch, RECONS[rec_name], SOLVERS[sol_name],
+                                                          0.4 if sch == 2 else 0.5, vsteps, 3)
+                v_steps = vsteps
+            variants.append({"scheme": sch_name.upper(), "recon": rec_name.upper(), "riemann": sol_name.upper(), "precision": prec,
+                             "value": cells * v_steps / (v_total * 1e-3), "unit": "cells/s", "steps": v_steps,
+                             "ms_per_step": v_total / v_steps, "kernel_ms": v_kms, "outputs_finite": v_ok,
+                             "roofline": roofline_of(sch_name, rec_name, sol_name, prec, v_kms)})
+            finite = finite and v_ok
+        del bufs
+        del field
+        torch.cuda.empty_cache()
 
     cpu = None
     if not args.no_cpu and world == 1:       # the oracle beside it: rank 0 at N = 1 only
@@ -420,7 +481,7 @@ def main():
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32" if sz == 4 else "f64", "data": "synthetic",
             "config": workload_config(args, args.groups), "clocks": sampler.summary(), "e2e": e2e,
-            "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
+            "gpu_launches": launches, "roofline": roofline, "variants": variants, "alu_peaks": alu, "cpu_baseline": cpu,
             "with_ghost_refresh": refresh_value, "with_fused_ghost_refresh": fused_value, "fixup_kernels": fixup, "poisson_sor": poisson, "outputs_finite": finite,
             "paper_context": "P100-PCIe fp32 ~2e8 cells/s incl. PCIe (PAPER.md L318-320); other hardware, not a target"}
     print(json.dumps(line), flush=True)

@@ -229,6 +229,22 @@ int gamer_fluid_advance_host(const void* in_host, void* out_host, void* flux_out
 
 void gamer_release_scratch(void);
 
+/* Measurement helper, not part of the solver (SURVEY 8(d) "ALU peaks to verify on the box"): runs a dependent-free
+ * instruction stream of the given kind on every SM (2 x 1024 threads per SM, 8 independent chains per thread), times it with
+ * CUDA events on `stream` (best of 5; the call synchronises) and returns the plain-ALU rate it reached:
+ * *tflops_out (nullable, HOST double) in TFLOP/s with FMA = 2 FLOPs, *gwarpinst_out (nullable, HOST double) in 1e9 warp
+ * instructions per second.  bench.py uses GAMER_ALU_FFMA / GAMER_ALU_DFMA as the measured peaks of the fp32 / fp64 "alu"
+ * roofline of the hydro kernels; the mixed streams show how issue slots are shared between the FMA pipe, the ALU pipe
+ * (min/max, compares, selects) and the special-function unit.  Allocates and frees 1.2 MB of device scratch. */
+enum { GAMER_ALU_FFMA = 0,         /* fp32 FMA, three register operands                                   */
+       GAMER_ALU_FMUL_FADD = 1,    /* fp32 multiply and add kept apart: 1 FLOP per issue slot             */
+       GAMER_ALU_FFMA_FMNMX = 2,   /* fp32 FMA + min, alternating: FMA pipe + ALU pipe                    */
+       GAMER_ALU_FFMA2 = 3,        /* packed fma.rn.f32x2: two FMAs per instruction                       */
+       GAMER_ALU_FFMA2_FMNMX = 4,  /* packed FMA + two min                                                */
+       GAMER_ALU_DFMA = 5,         /* fp64 FMA                                                            */
+       GAMER_ALU_FFMA_MUFU = 6 };  /* fp32 FMA with one rcp.approx in every 9 instructions                */
+int gamer_alu_peak(int kind, double* tflops_out, double* gwarpinst_out, void* stream);
+
 /* Number of kernel launches the library has issued in this process (all entry points). */
 int64_t gamer_launch_count(void);
 

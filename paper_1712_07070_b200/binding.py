@@ -23,7 +23,7 @@ LIB_PATH = os.path.join(_HERE, "libgamerhydro.so")
 EXPORTS = ["gamer_fluid_advance", "gamer_fluid_advance_ex", "gamer_fluid_advance_retry", "gamer_cfl_dt", "gamer_cfl_dt_ex",
            "gamer_cfl_from_group_speed", "gamer_refresh_ghosts_periodic", "gamer_refresh_ghosts", "gamer_refresh_ghosts_table", "gamer_interpolate_ghosts", "gamer_fluid_advance_resident",
            "gamer_neighbors_periodic", "gamer_restrict", "gamer_flux_accumulate", "gamer_flux_correct",
-           "gamer_poisson_sor", "gamer_fluid_advance_host", "gamer_release_scratch",
+           "gamer_poisson_sor", "gamer_fluid_advance_host", "gamer_release_scratch", "gamer_alu_peak",
            "gamer_launch_count", "gamer_strerror", "gamer_version"]
 
 
@@ -84,6 +84,7 @@ def lib():
         L.gamer_flux_correct.argtypes = [vp, vp, vp, vp, i64, ci, dbl, ci, vp]
         L.gamer_fluid_advance_host.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, ci, ci,
                                                ctypes.POINTER(gamer_opts)]
+        L.gamer_alu_peak.argtypes = [ci, ctypes.POINTER(dbl), ctypes.POINTER(dbl), vp]
         L.gamer_launch_count.restype = ctypes.c_int64
         L.gamer_strerror.restype = ctypes.c_char_p
         L.gamer_strerror.argtypes = [ci]
@@ -269,6 +270,16 @@ def gamer_fluid_advance_host(in_host, out_host, flux_out_host, group_speed_out_h
                                           _ptr(group_speed_out_host, "cpu"), n, float(dt), float(dh), float(gamma),
                                           int(scheme), int(recon), int(riemann), _precision(in_host),
                                           ctypes.byref(opts)), "gamer_fluid_advance_host")
+
+
+ALU_FFMA, ALU_FMUL_FADD, ALU_FFMA_FMNMX, ALU_FFMA2, ALU_FFMA2_FMNMX, ALU_DFMA, ALU_FFMA_MUFU = range(7)
+
+
+def gamer_alu_peak(kind, stream=None):
+    """Measurement helper: (TFLOP/s, 1e9 warp instructions/s) of a dependent-free instruction stream of the given kind."""
+    tf, gi = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    _check(lib().gamer_alu_peak(int(kind), ctypes.byref(tf), ctypes.byref(gi), _stream_handle(stream)), "gamer_alu_peak")
+    return tf.value, gi.value
 
 
 def gamer_release_scratch():

@@ -49,8 +49,9 @@ def build(force=False, verbose=False):
                 if verbose:
                     cmd += ["-Xptxas", "-v"]
                 jobs.append((cmd + ["-c", os.path.join(CSRC, "inst.cu"), "-o", o], o))
-    o = os.path.join(OBJ, "api.o")
-    jobs.append(([NVCC, *FLAGS, "-c", os.path.join(CSRC, "api.cu"), "-o", o], o))
+    for unit in ("api", "alu_peak"):
+        o = os.path.join(OBJ, unit + ".o")
+        jobs.append(([NVCC, *FLAGS, "-c", os.path.join(CSRC, unit + ".cu"), "-o", o], o))
     with concurrent.futures.ThreadPoolExecutor(max_workers=os.cpu_count() or 4) as ex:
         outs = list(ex.map(lambda j: _run(j[0]), jobs))
     if verbose:

@@ -21,6 +21,16 @@ __device__ __forceinline__ void make_side(const T* W, Side<T>& s, const Phys<T>&
     s.H = (s.E + s.P) * Ops<T>::rcp(s.rho);
 }
 
+// the same from a rotated CONSERVED state (rho, m_n, m_t1, m_t2, E): one reciprocal serves the velocities and H
+template <typename T>
+__device__ __forceinline__ void make_side_cons(const T* U, Side<T>& s, const Phys<T>& ph) {
+    s.rho = U[0]; s.m1 = U[1]; s.m2 = U[2]; s.m3 = U[3]; s.E = U[4];
+    const T ir = Ops<T>::rcp(s.rho);
+    s.u = s.m1 * ir; s.v = s.m2 * ir; s.w = s.m3 * ir;
+    s.P = ph.gm1 * (s.E - T(0.5) * (s.m1 * s.u + s.m2 * s.v + s.m3 * s.w));
+    s.H = (s.E + s.P) * ir;
+}
+
 template <typename T>
 __device__ __forceinline__ void side_flux(const Side<T>& s, T* F) {
     F[0] = s.m1;
@@ -215,6 +225,37 @@ __device__ __noinline__ bool solve_exact(const Side<T>& L, const Side<T>& R, T* 
     F[3] = rho * u * K.w;
     F[4] = u * (E + P);
     return false;
+}
+
+// Flux through a face from the two sides.  Returns true if Roe (or the exact solver) fell back to HLLE.
+template <typename T, int SOLVER>
+__device__ __forceinline__ bool riemann_sides(const Side<T>& L, const Side<T>& R, T* F, const Phys<T>& ph) {
+    RoeAvg<T> r;
+    roe_average(L, R, r, ph);
+    bool fb = false;
+    if (SOLVER == ROE) {
+        fb = solve_roe(L, R, r, F, ph);
+        if (fb) solve_hlle(L, R, r, F, ph);
+    } else if (SOLVER == HLLC) {
+        solve_hllc(L, R, r, F, ph);
+    } else if (SOLVER == EXACT) {
+        fb = solve_exact(L, R, F, ph);
+        if (fb) solve_hlle(L, R, r, F, ph);
+    } else {
+        solve_hlle(L, R, r, F, ph);
+    }
+    return fb;
+}
+
+// Flux through a face from rotated CONSERVED states (rho, m_n, m_t1, m_t2, E [, s]).
+template <typename T, int SOLVER, int NV>
+__device__ __forceinline__ bool riemann_flux_cons(const T* UL, const T* UR, T* F, const Phys<T>& ph) {
+    Side<T> L, R;
+    make_side_cons(UL, L, ph);
+    make_side_cons(UR, R, ph);
+    const bool fb = riemann_sides<T, SOLVER>(L, R, F, ph);
+    if (NV > 5) F[NV - 1] = F[0] >= T(0) ? F[0] * (UL[NV - 1] * Ops<T>::rcp(UL[0])) : F[0] * (UR[NV - 1] * Ops<T>::rcp(UR[0]));
+    return fb;
 }
 
 // Flux through a face from rotated primitive states.  Returns true if Roe fell back to HLLE.

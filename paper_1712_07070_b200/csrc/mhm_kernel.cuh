@@ -103,19 +103,27 @@ __device__ __forceinline__ void mhm_face_states(const T* const* Pz, const Phys<T
     }
 }
 
-// Hancock half step of one face state: evolved primitives -> We (floors applied in extended mode, not in the
-// reverting pass, where the un-evolved face values are taken as they are); returns whether rho and P are positive.
+// Hancock half step of one conserved face state: Ue = Uf - hdU (hdU = dt/(2 dh) * dU, or 0 in the reverting pass,
+// where the un-evolved face values are taken as they are); returns whether rho and P of the result are positive.
+// The evolved state stays in conserved variables all the way to the Riemann solver, which derives the velocities,
+// P and H it needs from them with one reciprocal (make_side_cons): no conserved -> primitive -> conserved round
+// trip per state.  P > 0 is tested without a division: for rho > 0, P > 0 <=> rho E - |m|^2 / 2 > 0.
+// With floors (extended mode) the state goes through primitives, as in the oracle: floor, back to conserved.
 // Every thread evolves all six states of its cell, also the ones it hands to no Riemann solver: any bad state
-// reverts the cell (R6), the halo copy of a cell must decide exactly as its owner in the neighbouring group does, and
-// six straight-line conversions without per-state branches are faster than division-free tests of the unused ones.
+// reverts the cell (R6) and the halo copy of a cell must decide exactly as its owner in the neighbouring group does.
 template <typename T, int NV, bool EXT>
-__device__ __forceinline__ bool mhm_evolve(const T* Uf, const T* dU, T* We, bool floors, const Phys<T>& ph) {
-    T Ue[NV];
+__device__ __forceinline__ bool mhm_evolve(const T* Uf, const T* hdU, T* Ue, bool floors, const Phys<T>& ph) {
 #pragma unroll
-    for (int v = 0; v < NV; ++v) Ue[v] = Uf[v] - ph.hlam * dU[v];
-    cons2prim<T, NV>(Ue, We, ph);
-    if (EXT && ph.floors && floors) floor_prim(We, ph);
-    return (We[0] > T(0)) && (We[4] > T(0));
+    for (int v = 0; v < NV; ++v) Ue[v] = Uf[v] - hdU[v];
+    if (EXT && ph.floors && floors) {
+        T We[NV];
+        cons2prim<T, NV>(Ue, We, ph);
+        floor_prim(We, ph);
+        prim2cons<T, NV>(We, Ue, ph);
+        return (We[0] > T(0)) && (We[4] > T(0));
+    }
+    const T pe = Ue[0] * Ue[4] - T(0.5) * (Ue[1] * Ue[1] + Ue[2] * Ue[2] + Ue[3] * Ue[3]);
+    return (Ue[0] > T(0)) && (pe > T(0));
 }
 
 // per-thread constants of the cell column this thread owns
@@ -221,7 +229,7 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED>::NT), M
         }
     }
 
-    T zplus[NV];                    // z+ state of the plane below (rotated for z)
+    T zplus[NV];                    // evolved conserved z+ state of the plane below (rotated for z)
     T fzl[NV];                      // z flux at kk-3/2 (natural variable order)
 #pragma unroll
     for (int v = 0; v < NV; ++v) { zplus[v] = T(1); fzl[v] = T(0); }
@@ -253,39 +261,37 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED>::NT), M
             T zminus[NV], znew[NV];
 #pragma unroll 1
             for (int pass = 0; pass < 2; ++pass) {
-                T Uf[3][2][NV], dU[NV], We[NV];
+                T Uf[3][2][NV], dU[NV], Ue[NV];
                 mhm_face_states<T, RECON, NV, EXT, PLN>(Pz, ph, Uf, dU);
-                if (pass) {
 #pragma unroll
-                    for (int v = 0; v < NV; ++v) dU[v] = T(0);
-                }
+                for (int v = 0; v < NV; ++v) dU[v] = pass ? T(0) : ph.hlam * dU[v];
                 const bool fl_ok = pass == 0;
-                bool ok = mhm_evolve<T, NV, EXT>(Uf[0][1], dU, We, fl_ok, ph);
+                bool ok = mhm_evolve<T, NV, EXT>(Uf[0][1], dU, Ue, fl_ok, ph);
                 if (mid && pub_x) {
                     T rot[NV];
 #pragma unroll
-                    for (int k = 0; k < NV; ++k) rot[k] = We[nat_index(0, k)];
+                    for (int k = 0; k < NV; ++k) rot[k] = Ue[nat_index(0, k)];
                     put_state<T, NV>(st_x, G::NSX, c.sx_own + 1, rot);
                 }
-                ok = mhm_evolve<T, NV, EXT>(Uf[1][1], dU, We, fl_ok, ph) && ok;
+                ok = mhm_evolve<T, NV, EXT>(Uf[1][1], dU, Ue, fl_ok, ph) && ok;
                 if (mid && pub_y) {
                     T rot[NV];
 #pragma unroll
-                    for (int k = 0; k < NV; ++k) rot[k] = We[nat_index(1, k)];
+                    for (int k = 0; k < NV; ++k) rot[k] = Ue[nat_index(1, k)];
                     put_state<T, NV>(st_y, G::NSY, c.sy_own + 16, rot);
                 }
-                ok = mhm_evolve<T, NV, EXT>(Uf[0][0], dU, We, fl_ok, ph) && ok;
+                ok = mhm_evolve<T, NV, EXT>(Uf[0][0], dU, Ue, fl_ok, ph) && ok;
 #pragma unroll
-                for (int k = 0; k < NV; ++k) xminus[k] = We[nat_index(0, k)];
-                ok = mhm_evolve<T, NV, EXT>(Uf[1][0], dU, We, fl_ok, ph) && ok;
+                for (int k = 0; k < NV; ++k) xminus[k] = Ue[nat_index(0, k)];
+                ok = mhm_evolve<T, NV, EXT>(Uf[1][0], dU, Ue, fl_ok, ph) && ok;
 #pragma unroll
-                for (int k = 0; k < NV; ++k) yminus[k] = We[nat_index(1, k)];
-                ok = mhm_evolve<T, NV, EXT>(Uf[2][0], dU, We, fl_ok, ph) && ok;
+                for (int k = 0; k < NV; ++k) yminus[k] = Ue[nat_index(1, k)];
+                ok = mhm_evolve<T, NV, EXT>(Uf[2][0], dU, Ue, fl_ok, ph) && ok;
 #pragma unroll
-                for (int k = 0; k < NV; ++k) zminus[k] = We[nat_index(2, k)];
-                ok = mhm_evolve<T, NV, EXT>(Uf[2][1], dU, We, fl_ok, ph) && ok;
+                for (int k = 0; k < NV; ++k) zminus[k] = Ue[nat_index(2, k)];
+                ok = mhm_evolve<T, NV, EXT>(Uf[2][1], dU, Ue, fl_ok, ph) && ok;
 #pragma unroll
-                for (int k = 0; k < NV; ++k) znew[k] = We[nat_index(2, k)];
+                for (int k = 0; k < NV; ++k) znew[k] = Ue[nat_index(2, k)];
                 if (ok || pass) break;
                 cnt.reverted++;
             }
@@ -293,7 +299,7 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED>::NT), M
                 // ------------------------------------------------------------ z face kk-1/2
                 if (kk >= 0) {
                     T F[NV];
-                    cnt.roe_fb += riemann_flux<T, SOLVER, NV>(zplus, zminus, F, ph) ? 1 : 0;
+                    cnt.roe_fb += riemann_flux_cons<T, SOLVER, NV>(zplus, zminus, F, ph) ? 1 : 0;
 #pragma unroll
                     for (int v = 0; v < NV; ++v) fzn[v] = F[rot_index(2, v)];
                     if (gflux != nullptr && (kk & 7) == 0) {      // block-uniform: a real branch
@@ -341,7 +347,7 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED>::NT), M
         if (mid && own_x) {
             T WL[NV], F[NV], fn[NV];
             get_state<T, NV>(st_x, G::NSX, c.sx_own, WL);
-            cnt.roe_fb += riemann_flux<T, SOLVER, NV>(WL, xminus, F, ph) ? 1 : 0;
+            cnt.roe_fb += riemann_flux_cons<T, SOLVER, NV>(WL, xminus, F, ph) ? 1 : 0;
 #pragma unroll
             for (int v = 0; v < NV; ++v) fn[v] = F[rot_index(0, v)];
             put_state<T, NV>(fl_x, G::NSX, c.sx_own, fn);
@@ -349,7 +355,7 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED>::NT), M
         if (mid && own_y) {
             T WL[NV], F[NV], fn[NV];
             get_state<T, NV>(st_y, G::NSY, c.sy_own, WL);
-            cnt.roe_fb += riemann_flux<T, SOLVER, NV>(WL, yminus, F, ph) ? 1 : 0;
+            cnt.roe_fb += riemann_flux_cons<T, SOLVER, NV>(WL, yminus, F, ph) ? 1 : 0;
 #pragma unroll
             for (int v = 0; v < NV; ++v) fn[v] = F[rot_index(1, v)];
             put_state<T, NV>(fl_y, G::NSY, c.sy_own, fn);
