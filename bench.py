@@ -384,7 +384,7 @@ def main():
     alu = {}
     for name, kind in (("ffma", gb.ALU_FFMA), ("dfma", gb.ALU_DFMA), ("fmul_fadd", gb.ALU_FMUL_FADD),
                        ("ffma_fmnmx", gb.ALU_FFMA_FMNMX), ("ffma2", gb.ALU_FFMA2), ("ffma2_fmnmx", gb.ALU_FFMA2_FMNMX),
-                       ("ffma_mufu", gb.ALU_FFMA_MUFU)):
+                       ("ffma_mufu", gb.ALU_FFMA_MUFU), ("ffma2_ffma", gb.ALU_FFMA2_FFMA), ("ffma2_iadd", gb.ALU_FFMA2_IADD)):
         tf, gi = gb.gamer_alu_peak(kind, stream)
         alu[name] = {"tflops": tf, "gwarpinst_per_s": gi}
     alu["issue_slots_gwarpinst_per_s"] = 148 * 4 * sm_max * 1e6 / 1e9

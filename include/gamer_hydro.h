@@ -242,7 +242,9 @@ enum { GAMER_ALU_FFMA = 0,         /* fp32 FMA, three register operands         
        GAMER_ALU_FFMA2 = 3,        /* packed fma.rn.f32x2: two FMAs per instruction                       */
        GAMER_ALU_FFMA2_FMNMX = 4,  /* packed FMA + two min                                                */
        GAMER_ALU_DFMA = 5,         /* fp64 FMA                                                            */
-       GAMER_ALU_FFMA_MUFU = 6 };  /* fp32 FMA with one rcp.approx in every 9 instructions                */
+       GAMER_ALU_FFMA_MUFU = 6,    /* fp32 FMA with one rcp.approx in every 9 instructions                */
+       GAMER_ALU_FFMA2_FFMA = 7,   /* one packed FMA to two plain ones                                    */
+       GAMER_ALU_FFMA2_IADD = 8 }; /* packed FMA + integer add, alternating                               */
 int gamer_alu_peak(int kind, double* tflops_out, double* gwarpinst_out, void* stream);
 
 /* Number of kernel launches the library has issued in this process (all entry points). */

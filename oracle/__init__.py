@@ -14,7 +14,7 @@ import numpy as np
 
 from . import build as _build
 
-MHM, CTU = 1, 2
+MHM, CTU, VL = 1, 2, 3
 PLM, PPM = 1, 2
 ROE, HLLC, HLLE, EXACT = 1, 2, 3, 4
 GMINMOD, VANLEER, VANALBADA = 1, 2, 3

@@ -11,6 +11,8 @@
  * What it follows (PAPER.md = /root/reference/PAPER.md, section 2.2 unless noted):
  *   - Euler equations, ideal gas, conserved (rho, mom, E); definitions of P, E_kin, E_the: L100
  *   - MHM (MUSCL-Hancock) and CTU ("6 Riemann solvers per cell per time-step"): L90
+ *   - VL ("a variant of the MUSCL-Hancock scheme (VL; Falle 1991; van Leer 2006)", L90; Eq. (2) applies to it, L168):
+ *     the half-step predictor is a first-order Godunov update of the cell averages (reading R26 of DESIGN.md)
  *   - PLM / PPM reconstruction on primitive variables, slope limiters: L94
  *   - Roe / HLLC / HLLE Riemann solvers: L94
  *   - dual-energy formalism with entropy s = P/rho^(gamma-1) and switch xi: L100
@@ -51,7 +53,7 @@
 #define NVMAX 6
 #define IDX(i, j, k) ((((k) * NP) + (j)) * NP + (i))
 
-enum { SCHEME_MHM = 1, SCHEME_CTU = 2 };
+enum { SCHEME_MHM = 1, SCHEME_CTU = 2, SCHEME_VL = 3 };
 enum { RECON_PLM = 1, RECON_PPM = 2 };
 enum { RSOLVER_ROE = 1, RSOLVER_HLLC = 2, RSOLVER_HLLE = 3, RSOLVER_EXACT = 4 };
 enum { LIMITER_GMINMOD = 1, LIMITER_VANLEER = 2, LIMITER_VANALBADA = 3 };
@@ -580,7 +582,7 @@ static double signal_speed(const ctx_t *c, int scheme, const double *U)
     floor_prim(c, W);
     double cs = sqrt(c->gamma * W[4] / W[0]);
     double ax = fabs(W[1]), ay = fabs(W[2]), az = fabs(W[3]);
-    if (scheme == SCHEME_MHM) return ax + ay + az + 3.0 * cs;
+    if (scheme != SCHEME_CTU) return ax + ay + az + 3.0 * cs;   /* Eq. (2): MHM and VL (L168) */
     double m = ax > ay ? ax : ay;
     if (az > m) m = az;
     return m + cs;
@@ -595,6 +597,7 @@ typedef struct {
     double *TS;   /* [3][2][nv][NPC]     CTU traced states (conserved)                */
     double *F1;   /* [3][nv][NPC]        CTU first-pass flux at face c + e_d/2        */
     double *FX;   /* [3][nv][NPC]        final flux at face c + e_d/2                 */
+    double *WH;   /* [nv][NPC]           VL: primitives of the half-step state        */
 } work_t;
 
 #define FSI(d, s, v, n) ((((size_t)(d) * 2 + (s)) * nv + (v)) * NPC + (n))
@@ -820,6 +823,61 @@ static void advance_group(const ctx_t *c, int scheme, int recon, int solver, dou
         for (int k = lo; k <= hi; ++k)
             for (int j = lo; j <= hi; ++j)
                 for (int i = lo; i <= hi; ++i) mhm_predict_cell(c, recon, lam_r, wk, IDX(i, j, k), st);
+    } else if (scheme == SCHEME_VL) {
+        /* O4-VL (van Leer 2006; Falle 1991; Stone & Gardiner 2009 sect. 3; reading R26):
+         * (a) first-order fluxes: the Riemann solver on the piecewise-constant cell averages U^n, at every face of
+         *     the cells [-2,17]^3 (padded [1,20]) */
+        const int l1 = lo - 1, h1 = hi + 1;
+        for (int d = 0; d < 3; ++d)
+            for (int k = l1 - (d == 2); k <= h1; ++k)
+                for (int j = l1 - (d == 1); j <= h1; ++j)
+                    for (int i = l1 - (d == 0); i <= h1; ++i) {
+                        int n = IDX(i, j, k);
+                        double UL[NVMAX] = {0}, UR[NVMAX] = {0}, F[NVMAX];
+                        for (int v = 0; v < nv; ++v) {
+                            UL[v] = in[(size_t)v * NPC + n];
+                            UR[v] = in[(size_t)v * NPC + n + STEP[d]];
+                        }
+                        riemann(c, solver, d, UL, UR, F, st);
+                        for (int v = 0; v < nv; ++v) wk->F1[FLI(d, v, n)] = F[v];
+                    }
+        /* (b) half-step state U^{n+1/2} = U^n - dt/(2 dh) sum_d [F1_d(+) - F1_d(-)] of the cells [-2,17]^3, as
+         *     primitives; floors if set; an unphysical half-step state falls back to the cell's own U^n */
+        for (int k = l1; k <= h1; ++k)
+            for (int j = l1; j <= h1; ++j)
+                for (int i = l1; i <= h1; ++i) {
+                    int n = IDX(i, j, k);
+                    double U[NVMAX], W[NVMAX];
+                    for (int v = 0; v < nv; ++v) {
+                        double dfx = wk->F1[FLI(0, v, n)] - wk->F1[FLI(0, v, n - STEP[0])];
+                        double dfy = wk->F1[FLI(1, v, n)] - wk->F1[FLI(1, v, n - STEP[1])];
+                        double dfz = wk->F1[FLI(2, v, n)] - wk->F1[FLI(2, v, n - STEP[2])];
+                        U[v] = in[(size_t)v * NPC + n] - 0.5 * lam_r * ((dfx + dfy) + dfz);
+                    }
+                    cons2prim(c, U, W);
+                    floor_prim(c, W);
+                    if (!state_ok(W)) {
+                        st->n_pred_revert++;
+                        for (int v = 0; v < nv; ++v) W[v] = wk->W[(size_t)v * NPC + n];
+                    }
+                    for (int v = 0; v < nv; ++v) wk->WH[(size_t)v * NPC + n] = W[v];
+                }
+        /* (c) face values of the half-step primitives (O2, O3) for every cell of [-1,16]^3, as conserved states */
+        for (int k = lo; k <= hi; ++k)
+            for (int j = lo; j <= hi; ++j)
+                for (int i = lo; i <= hi; ++i) {
+                    int n = IDX(i, j, k);
+                    for (int d = 0; d < 3; ++d) {
+                        double wm[NVMAX], wp[NVMAX], Um[NVMAX], Up[NVMAX];
+                        gather_face_values(c, recon, wk->WH, n, d, wm, wp);
+                        prim2cons(c, wm, Um);
+                        prim2cons(c, wp, Up);
+                        for (int v = 0; v < nv; ++v) {
+                            wk->FS[FSI(d, 0, v, n)] = Um[v];
+                            wk->FS[FSI(d, 1, v, n)] = Up[v];
+                        }
+                    }
+                }
     } else {
         /* (a) traced states */
         for (int k = lo; k <= hi; ++k)
@@ -947,7 +1005,8 @@ int oracle_fluid_advance(const double *in, double *out, double *flux_out, double
                          int riemann_solver, const orc_opts *opts, orc_stats *stats_out)
 {
     if (!in || !out || n_groups < 0 || !(dt > 0.0) || !(dh > 0.0) || !(gamma > 1.0)) return -1;
-    if (scheme != SCHEME_MHM && scheme != SCHEME_CTU) return -1;
+    if (scheme != SCHEME_MHM && scheme != SCHEME_CTU && scheme != SCHEME_VL) return -1;
+    if (scheme == SCHEME_VL && recon != RECON_PLM) return -2;   /* VL + PPM needs a fourth ghost zone (L300 fixes three) */
     if (recon != RECON_PLM && recon != RECON_PPM) return -1;
     if (riemann_solver < RSOLVER_ROE || riemann_solver > RSOLVER_EXACT) return -1;
     ctx_t c;
@@ -966,9 +1025,10 @@ int oracle_fluid_advance(const double *in, double *out, double *flux_out, double
         wk.TS = (double *)malloc(sizeof(double) * 6 * nv * NPC);
         wk.F1 = (double *)malloc(sizeof(double) * 3 * nv * NPC);
         wk.FX = (double *)malloc(sizeof(double) * 3 * nv * NPC);
+        wk.WH = (double *)malloc(sizeof(double) * nv * NPC);
         orc_stats st;
         memset(&st, 0, sizeof(st));
-        if (!wk.W || !wk.FS || !wk.TS || !wk.F1 || !wk.FX) {
+        if (!wk.W || !wk.FS || !wk.TS || !wk.F1 || !wk.FX || !wk.WH) {
 #pragma omp atomic write
             fail = 1;
         } else {
@@ -991,7 +1051,7 @@ int oracle_fluid_advance(const double *in, double *out, double *flux_out, double
             tot.n_floor += st.n_floor;
             tot.n_unphysical += st.n_unphysical;
         }
-        free(wk.W); free(wk.FS); free(wk.TS); free(wk.F1); free(wk.FX);
+        free(wk.W); free(wk.FS); free(wk.TS); free(wk.F1); free(wk.FX); free(wk.WH);
     }
     if (fail) return -4;
     if (stats_out) *stats_out = tot;

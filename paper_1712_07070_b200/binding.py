@@ -272,7 +272,7 @@ def gamer_fluid_advance_host(in_host, out_host, flux_out_host, group_speed_out_h
                                           ctypes.byref(opts)), "gamer_fluid_advance_host")
 
 
-ALU_FFMA, ALU_FMUL_FADD, ALU_FFMA_FMNMX, ALU_FFMA2, ALU_FFMA2_FMNMX, ALU_DFMA, ALU_FFMA_MUFU = range(7)
+ALU_FFMA, ALU_FMUL_FADD, ALU_FFMA_FMNMX, ALU_FFMA2, ALU_FFMA2_FMNMX, ALU_DFMA, ALU_FFMA_MUFU, ALU_FFMA2_FFMA, ALU_FFMA2_IADD = range(9)
 
 
 def gamer_alu_peak(kind, stream=None):

@@ -61,6 +61,25 @@ template <> struct Stream<GAMER_ALU_FFMA2_FMNMX> {
         a.y = fminf(a.y, b.y);
     }
 };
+// one packed FMA to two plain ones: 4 FMAs in 3 issue slots
+template <> struct Stream<GAMER_ALU_FFMA2_FFMA> {
+    typedef float2 T;
+    static constexpr double FLOPS = 8.0, INSTS = 3.0;
+    static __device__ __forceinline__ void op(float2& a, float2 b, float2 c) {
+        Stream<GAMER_ALU_FFMA2>::op(a, b, c);
+        a.x = fmaf(a.x, b.x, c.x);
+        a.y = fmaf(a.y, b.y, c.y);
+    }
+};
+// packed FMA + one integer add (IADD3 on the ALU pipe) on a side chain
+template <> struct Stream<GAMER_ALU_FFMA2_IADD> {
+    typedef float2 T;
+    static constexpr double FLOPS = 4.0, INSTS = 2.0;
+    static __device__ __forceinline__ void op(float2& a, float2 b, float2 c) {
+        Stream<GAMER_ALU_FFMA2>::op(a, b, c);
+        a.y = __int_as_float(__float_as_int(a.y) + __float_as_int(b.y));      // the .y lane carries integer garbage: only rates matter
+    }
+};
 // fp64 FMA
 template <> struct Stream<GAMER_ALU_DFMA> {
     typedef double T;
@@ -170,6 +189,8 @@ extern "C" int gamer_alu_peak(int kind, double* tflops_out, double* gwarpinst_ou
     case GAMER_ALU_FFMA2_FMNMX: return run_stream<GAMER_ALU_FFMA2_FMNMX>(tflops_out, gwarpinst_out, st);
     case GAMER_ALU_DFMA: return run_stream<GAMER_ALU_DFMA>(tflops_out, gwarpinst_out, st);
     case GAMER_ALU_FFMA_MUFU: return run_stream<GAMER_ALU_FFMA_MUFU>(tflops_out, gwarpinst_out, st);
+    case GAMER_ALU_FFMA2_FFMA: return run_stream<GAMER_ALU_FFMA2_FFMA>(tflops_out, gwarpinst_out, st);
+    case GAMER_ALU_FFMA2_IADD: return run_stream<GAMER_ALU_FFMA2_IADD>(tflops_out, gwarpinst_out, st);
     default: return GAMER_EINVAL;
     }
 }

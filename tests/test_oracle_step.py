@@ -10,11 +10,12 @@ import torch
 from helpers import oracle_run, oracle_step
 from paper_1712_07070_b200 import inputs
 
-MHM, CTU = 1, 2
+MHM, CTU, VL = 1, 2, 3
 PLM, PPM = 1, 2
 ROE, HLLC, HLLE = 1, 2, 3
 EXACT = 4
-COMBOS = list(itertools.product((MHM, CTU), (PLM, PPM), (ROE, HLLC, HLLE))) + [(MHM, PLM, EXACT), (CTU, PPM, EXACT)]
+COMBOS = list(itertools.product((MHM, CTU), (PLM, PPM), (ROE, HLLC, HLLE))) + [(MHM, PLM, EXACT), (CTU, PPM, EXACT)] + \
+    [(VL, PLM, ROE), (VL, PLM, HLLC), (VL, PLM, HLLE)]
 G53 = 5.0 / 3.0
 
 
@@ -42,7 +43,7 @@ def test_conservation_on_periodic_box(oracle_mod, scheme, recon, solver):
     assert (new - f).abs().max() > 1e-3       # and something did happen
 
 
-@pytest.mark.parametrize("scheme,recon,solver", [(MHM, PLM, ROE), (CTU, PPM, HLLC), (MHM, PPM, HLLE)])
+@pytest.mark.parametrize("scheme,recon,solver", [(MHM, PLM, ROE), (CTU, PPM, HLLC), (MHM, PPM, HLLE), (VL, PLM, ROE)])
 def test_boundary_fluxes_of_neighbouring_groups_are_bitwise_equal(oracle_mod, scheme, recon, solver):
     """the flux through a face shared by two groups is computed twice and must agree
     bit for bit; also the mid-plane (p=1) equals the difference form of the update."""
@@ -57,7 +58,7 @@ def test_boundary_fluxes_of_neighbouring_groups_are_bitwise_equal(oracle_mod, sc
         assert np.array_equal(fl[gz, gy, gx, 2, 2], fl[(gz + 1) % 2, gy, gx, 2, 0])
 
 
-@pytest.mark.parametrize("scheme,recon,solver", [(MHM, PLM, HLLE), (CTU, PLM, ROE)])
+@pytest.mark.parametrize("scheme,recon,solver", [(MHM, PLM, HLLE), (CTU, PLM, ROE), (VL, PLM, HLLC)])
 def test_flux_out_reproduces_update_of_a_boundary_slab(oracle_mod, scheme, recon, solver):
     """Sum over a half-group slab: d(sum U)/dt = -(flux through its faces)/dh.  With periodic y,z
     sums over a whole x-slab [0,8) of the 32^3 box, only the x-planes 0 and 8 contribute."""
@@ -99,7 +100,7 @@ def test_cyclic_permutation_symmetry(oracle_mod, scheme, recon, solver):
     assert (newP - ref).abs().max().item() <= 1e-13 * ref.abs().max().item()
 
 
-@pytest.mark.parametrize("scheme,recon,solver", [(MHM, PLM, ROE), (CTU, PPM, HLLC), (CTU, PLM, HLLE), (MHM, PPM, HLLC)])
+@pytest.mark.parametrize("scheme,recon,solver", [(MHM, PLM, ROE), (CTU, PPM, HLLC), (CTU, PLM, HLLE), (MHM, PPM, HLLC), (VL, PLM, HLLE)])
 def test_mirror_symmetry(oracle_mod, scheme, recon, solver):
     f = _turb(seed=5)
     dh, dt = 1.0 / 32, 0.004
@@ -228,7 +229,7 @@ def test_sod_converges_to_exact_solution(oracle_mod, scheme, recon, solver):
     assert errs[1] < 1.2e-2 and order >= 0.7, (errs, order)
 
 
-@pytest.mark.parametrize("scheme,recon,cfl", [(MHM, PLM, 1.0), (MHM, PPM, 1.0), (CTU, PLM, 0.5), (CTU, PPM, 0.5)])
+@pytest.mark.parametrize("scheme,recon,cfl", [(MHM, PLM, 1.0), (MHM, PPM, 1.0), (CTU, PLM, 0.5), (CTU, PPM, 0.5), (VL, PLM, 1.0)])
 def test_stable_at_the_stated_cfl_limit(oracle_mod, scheme, recon, cfl):
     """CTU needs C_CFL <= 0.5, the others support C_CFL <= 1.0 (with their own Eq. 1 / 2)."""
     f = inputs.blob_field(16, G53)
@@ -238,10 +239,11 @@ def test_stable_at_the_stated_cfl_limit(oracle_mod, scheme, recon, cfl):
     assert out[0].min().item() >= lo - 0.02 and out[0].max().item() <= hi + 0.02
 
 
-@pytest.mark.parametrize("scheme,recon", [(MHM, PLM), (CTU, PLM), (MHM, PPM), (CTU, PPM)])
+@pytest.mark.parametrize("scheme,recon", [(MHM, PLM), (CTU, PLM), (MHM, PPM), (CTU, PPM), (VL, PLM)])
 def test_ghost_footprint(oracle_mod, scheme, recon):
-    """CTU+PPM needs 3 ghost zones.  PLM variants must ignore ghost layer 3; no variant
-    reads the triple-corner ghosts; PPM must read layer 3."""
+    """CTU+PPM needs 3 ghost zones.  MHM/CTU + PLM must ignore ghost layer 3; no variant's result depends on
+    the triple-corner ghosts; PPM must read layer 3, and so must VL + PLM (its half-step predictor reaches one cell
+    further than the reconstruction: that is why VL + PPM would need a fourth zone)."""
     f = _turb(n=16, seed=3)
     p = inputs.pack_periodic(f).numpy()
     dt, dh = 0.002, 1.0 / 16
@@ -252,7 +254,7 @@ def test_ghost_footprint(oracle_mod, scheme, recon):
     q[:, :, outer] *= 1.5                      # outermost ghost layer (layer 3)
     r = oracle_mod.fluid_advance(q, dt, dh, G53, scheme, recon, HLLC)
     same = np.array_equal(r["out"], base["out"]) and np.array_equal(r["flux"], base["flux"])
-    assert same == (recon == PLM)
+    assert same == (recon == PLM and scheme != VL)
     q = p.copy()
     idx = np.arange(22)
     gh = (idx < 3) | (idx >= 19)
@@ -273,6 +275,10 @@ def test_riemann_solves_per_cell(oracle_mod):
     assert 3 * 16 ** 3 * 16 // 17 <= 3 * 16 ** 3                      # shared faces: 16 of 17 unique
     assert b["n_riemann_final"] == 3 * 17 * 16 * 16
     assert b["n_riemann"] - b["n_riemann_final"] == 3 * 17 * 18 * 18
+    # VL: 3 + 3 per cell too (first-order pass on the faces of the cells [-2,17]^3, then the final pass)
+    v = oracle_mod.fluid_advance(p, 0.002, 1.0 / 16, G53, VL, PLM, HLLC)["stats"]
+    assert v["n_riemann_final"] == 3 * 17 * 16 * 16
+    assert v["n_riemann"] - v["n_riemann_final"] == 3 * 21 * 20 * 20
 
 
 @pytest.mark.parametrize("scheme,recon,solver", [(MHM, PLM, ROE), (CTU, PPM, HLLC), (MHM, PPM, HLLE), (CTU, PLM, ROE)])
@@ -492,3 +498,121 @@ def test_ctu_diagonal_advection_is_second_order(oracle_mod, recon):
     order = math.log(errs[1] / errs[2], 2.0)
     assert order >= 1.8, (errs, order)
     assert errs[2] < 1e-3
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# VL scheme ("a variant of the MUSCL-Hancock scheme (VL; Falle 1991; van Leer 2006)"; R26)
+# ---------------------------------------------------------------------------------------------------------------
+def _vl_contact_reference(rho, vel, lam_r):
+    """The VL scheme written out for linear advection of rho (uniform velocity and pressure, exact upwinding by Roe /
+    HLLC): first-order upwind half step  rho_h = rho - 1/2 sum_d nu_d (rho - rho_upwind-neighbour),  minmod slopes of
+    rho_h, second-order upwind fluxes  v_d (rho_h +- 1/2 slope)  from the upwind cell, full step from rho.
+    (van Leer 2006 sect. 5; Stone & Gardiner 2009 sect. 3 steps 1-6 without magnetic field.)"""
+    ax = {0: 2, 1: 1, 2: 0}
+    rh = rho.copy()
+    for d in range(3):
+        nu = vel[d] * lam_r
+        up = np.roll(rho, 1, ax[d]) if vel[d] > 0 else np.roll(rho, -1, ax[d])
+        rh -= 0.5 * abs(nu) * (rho - up)
+    new = rho.copy()
+    for d in range(3):
+        s = _minmod(rh - np.roll(rh, 1, ax[d]), np.roll(rh, -1, ax[d]) - rh)
+        face = rh + 0.5 * s if vel[d] > 0 else np.roll(rh - 0.5 * s, -1, ax[d])      # at c + e_d/2
+        new -= vel[d] * lam_r * (face - np.roll(face, 1, ax[d]))
+    return new
+
+
+@pytest.mark.parametrize("solver", [ROE, HLLC])
+@pytest.mark.parametrize("vel", [(0.9, -0.6, 0.4), (-0.5, 0.8, -0.7), (0.8, 0.0, 0.0)])
+def test_vl_contact_advection_closed_form(oracle_mod, solver, vel):
+    """1-D (third velocity) and oblique 3-D contact advection: VL + PLM equals the scheme above to round-off.
+    Kills: a predictor over dt instead of dt/2, slopes taken from U^n instead of the half-step state, a final update
+    from the half-step state instead of U^n, Hancock-type evolution left in, wrong upwind side."""
+    n = 16
+    z, y, x = np.meshgrid(*(((np.arange(n) + 0.5) / n,) * 3), indexing="ij")
+    rho = (1.0 + 0.4 * np.sin(2 * np.pi * x) * np.cos(2 * np.pi * y) + 0.25 * np.cos(2 * np.pi * (y - 2 * z))
+           + 0.3 * (np.abs(x - 0.5) + np.abs(y - 0.4) + np.abs(z - 0.6) < 0.45))
+    t = torch.from_numpy(rho)
+    one = torch.ones_like(t)
+    f0 = inputs.prim_to_cons(t, vel[0] * one, vel[1] * one, vel[2] * one, one.clone(), G53)
+    dh, dt = 1.0 / n, 0.3 / n
+    new, r = oracle_step(oracle_mod, f0, dt, dh, G53, VL, PLM, solver)
+    assert r["stats"]["n_pred_revert"] == 0 and r["stats"]["n_roe_fallback"] == 0
+    ref = _vl_contact_reference(rho, vel, dt / dh)
+    assert np.abs(new[0].numpy() - ref).max() <= 5e-14
+    mhm, _ = oracle_step(oracle_mod, f0, dt, dh, G53, MHM, PLM, solver)
+    assert (new[0] - mhm[0]).abs().max().item() > 1e-4       # and it is not the Hancock predictor
+
+
+def test_vl_smooth_advection_is_second_order(oracle_mod):
+    """L1 order >= 1.8 on a diagonally advected density wave (theta = 2 as in the CTU convergence pin): a predictor
+    that is missing or taken over the wrong interval leaves a first-order error in time."""
+    vel, t_end = (1.0, 0.75, 0.0), 0.25
+    opts = oracle_mod.make_opts(theta=2.0)
+    errs = []
+    for n in (32, 64):
+        x = ((np.arange(n) + 0.5) / n)[None, None, :]
+        y = ((np.arange(n) + 0.5) / n)[None, :, None]
+        rho_fn = lambda xx, yy: 1.0 + 0.3 * np.sin(2 * np.pi * (xx + yy))
+        t = torch.from_numpy(np.broadcast_to(rho_fn(x, y), (16, n, n)).copy())
+        one = torch.ones_like(t)
+        f = inputs.prim_to_cons(t, vel[0] * one, vel[1] * one, 0.0 * one, one.clone(), 1.4)
+        out, _ = oracle_run(oracle_mod, f, t_end, 1.0 / n, 1.4, 0.8, VL, PLM, HLLC, opts)
+        exact = np.broadcast_to(rho_fn(x - vel[0] * t_end, y - vel[1] * t_end), (16, n, n))
+        errs.append(np.abs(out[0].numpy() - exact).mean())
+    assert math.log(errs[0] / errs[1], 2.0) >= 1.8, errs
+
+
+def test_vl_with_ppm_is_refused(oracle_mod):
+    """VL + PPM needs a fourth ghost zone; the boundary fixes three."""
+    p = inputs.pack_periodic(_turb(n=16)).numpy()
+    with pytest.raises(ValueError):
+        oracle_mod.fluid_advance(p, 0.002, 1.0 / 16, G53, VL, PPM, HLLC)
+
+
+def test_vl_cell_rebuilt_from_single_face_solves(oracle_mod):
+    """General data, all five variables: the VL update of sampled cells rebuilt from oracle.riemann (pinned in
+    tests/test_oracle_riemann.py) and oracle.face_values with the wiring written independently:
+    first-order fluxes -> half-step state -> PLM face values of its primitives -> final fluxes -> update of U^n."""
+    gamma = G53
+    gm1 = gamma - 1.0
+    f = _turb(n=16, seed=21)
+    p = inputs.pack_periodic(f).numpy()[0]
+    dh = 1.0 / 16
+    dt = _dt(oracle_mod, f, dh, gamma, 0.6, VL)
+    lam = dt / dh
+    r = oracle_mod.fluid_advance(p[None], dt, dh, gamma, VL, PLM, HLLE)
+    step = {0: (1, 0, 0), 1: (0, 1, 0), 2: (0, 0, 1)}
+    sh = lambda c, d, m: tuple(c[a] + m * step[d][a] for a in range(3))
+    U = lambda c: p[:, c[2], c[1], c[0]]
+    memo = {}
+
+    def f1(c, d):
+        if (c, d) not in memo:
+            memo[(c, d)] = oracle_mod.riemann(HLLE, d, U(c), U(sh(c, d, 1)), gamma)[0]
+        return memo[(c, d)]
+
+    def half_prim(c):
+        u = U(c).copy()
+        for d in range(3):
+            u -= 0.5 * lam * (f1(c, d) - f1(sh(c, d, -1), d))
+        v = u[1:4] / u[0]
+        return np.array([u[0], v[0], v[1], v[2], gm1 * (u[4] - 0.5 * u[0] * (v ** 2).sum())])
+
+    def face_state(c, d, side):
+        strip = np.array([half_prim(sh(c, d, m)) for m in (-1, 0, 1)])
+        w = np.empty(5)
+        for v in range(5):
+            w[v] = oracle_mod.face_values(PLM, np.array([0.0, strip[0, v], strip[1, v], strip[2, v], 0.0]))[side]
+        return np.array([w[0], w[0] * w[1], w[0] * w[2], w[0] * w[3], w[4] / gm1 + 0.5 * w[0] * (w[1:4] ** 2).sum()])
+
+    def f2(c, d):
+        return oracle_mod.riemann(HLLE, d, face_state(c, d, 1), face_state(sh(c, d, 1), d, 0), gamma)[0]
+
+    for (i, j, k) in ((0, 0, 0), (15, 7, 3), (8, 15, 12)):
+        c = (i + 3, j + 3, k + 3)
+        ref = U(c).copy()
+        for d in range(3):
+            ref -= lam * (f2(c, d) - f2(sh(c, d, -1), d))
+        got = r["out"][0, :, k, j, i]
+        assert np.abs(got - ref).max() <= 1e-13 * np.abs(ref).max(), (i, j, k)
