@@ -26,7 +26,7 @@ import time
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-SCHEMES = {"mhm": 1, "ctu": 2}
+SCHEMES = {"mhm": 1, "ctu": 2, "vl": 3}
 RECONS = {"plm": 1, "ppm": 2}
 SOLVERS = {"roe": 1, "hllc": 2, "hlle": 3, "exact": 4}
 CELLS = 4096

@@ -5,7 +5,7 @@
  * One call advances a batch of AMR patch groups (8 sibling patches of 8^3 cells
  * = 16^3 cells), each padded with 3 ghost zones per side (L300), by one step of an unsplit
  * Godunov scheme for the ideal-gas Euler equations (section 2.2): MUSCL-Hancock (MHM)
- * or corner-transport-upwind (CTU, 6 Riemann solves per cell), PLM or PPM reconstruction on
+ * or its VL variant, or corner-transport-upwind (CTU, 6 Riemann solves per cell), PLM or PPM reconstruction on
  * primitive variables, Roe / HLLC / HLLE Riemann solver, conservative update.  It also emits
  * the patch-boundary fluxes the AMR flux fix-up needs (L112) and the per-group CFL maximum
  * (Eqs. 1-2; the paper computes time-steps on the GPU too, L240).
@@ -22,7 +22,7 @@
  *             index 8p of that axis (faces of the 8^3 patches); the two 16-long dims are the two
  *             other axes, the lower-numbered axis fastest (x-faces: [z][y]; y: [z][x]; z: [y][x]).
  *             Values are the time-centred flux densities F_d, not multiplied by dt or area.
- *   group_speed_out [n_groups]   max over the 16^3 UPDATED cells of |vx|+|vy|+|vz|+3c (MHM, Eq. 2)
+ *   group_speed_out [n_groups]   max over the 16^3 UPDATED cells of |vx|+|vy|+|vz|+3c (MHM and VL, Eq. 2)
  *                                or max(|vx|,|vy|,|vz|)+c (CTU, Eq. 1)
  *   NVAR = 5 + n_scalar (n_scalar = 1 carries the entropy s = P/rho^(gamma-1) of L100).
  * Ownership: every pointer is a DEVICE pointer owned by the caller, 16-byte aligned and
@@ -37,7 +37,12 @@
 extern "C" {
 #endif
 
-enum { GAMER_MHM = 1, GAMER_CTU = 2 };                      /* scheme   (L90)            */
+enum { GAMER_MHM = 1, GAMER_CTU = 2,
+       GAMER_VL = 3 };      /* scheme (L90).  VL = "a variant of the MUSCL-Hancock scheme (VL; Falle 1991; van Leer 2006)":
+                               the half-step predictor is a first-order Godunov update of the cell averages (the same Riemann
+                               solver on piecewise-constant data), the face values are then reconstructed from that half-step
+                               state; 6 Riemann solves per cell; CFL by Eq. (2) like MHM (L168).  PLM only: with PPM the scheme
+                               would read a fourth ghost zone, the layout fixes three (L300) -> GAMER_EUNSUPPORTED */
 enum { GAMER_PLM = 1, GAMER_PPM = 2 };                      /* recon    (L94)            */
 enum { GAMER_ROE = 1, GAMER_HLLC = 2, GAMER_HLLE = 3,
        GAMER_EXACT = 4 };   /* riemann (L94); EXACT = Toro (2009) ch. 4, iterative: Newton on the pressure function

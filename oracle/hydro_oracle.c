@@ -825,19 +825,22 @@ static void advance_group(const ctx_t *c, int scheme, int recon, int solver, dou
                 for (int i = lo; i <= hi; ++i) mhm_predict_cell(c, recon, lam_r, wk, IDX(i, j, k), st);
     } else if (scheme == SCHEME_VL) {
         /* O4-VL (van Leer 2006; Falle 1991; Stone & Gardiner 2009 sect. 3; reading R26):
-         * (a) first-order fluxes: the Riemann solver on the piecewise-constant cell averages U^n, at every face of
-         *     the cells [-2,17]^3 (padded [1,20]) */
+         * (a) first-order fluxes: the Riemann solver on the piecewise-constant cell averages, at every face of
+         *     the cells [-2,17]^3 (padded [1,20]).  The predictor works on the same floored primitives W as the
+         *     reconstruction of the other schemes does (R14): its input states are prim2cons(W). */
         const int l1 = lo - 1, h1 = hi + 1;
         for (int d = 0; d < 3; ++d)
             for (int k = l1 - (d == 2); k <= h1; ++k)
                 for (int j = l1 - (d == 1); j <= h1; ++j)
                     for (int i = l1 - (d == 0); i <= h1; ++i) {
                         int n = IDX(i, j, k);
-                        double UL[NVMAX] = {0}, UR[NVMAX] = {0}, F[NVMAX];
+                        double WL[NVMAX], WR[NVMAX], UL[NVMAX] = {0}, UR[NVMAX] = {0}, F[NVMAX];
                         for (int v = 0; v < nv; ++v) {
-                            UL[v] = in[(size_t)v * NPC + n];
-                            UR[v] = in[(size_t)v * NPC + n + STEP[d]];
+                            WL[v] = wk->W[(size_t)v * NPC + n];
+                            WR[v] = wk->W[(size_t)v * NPC + n + STEP[d]];
                         }
+                        prim2cons(c, WL, UL);
+                        prim2cons(c, WR, UR);
                         riemann(c, solver, d, UL, UR, F, st);
                         for (int v = 0; v < nv; ++v) wk->F1[FLI(d, v, n)] = F[v];
                     }
@@ -847,18 +850,20 @@ static void advance_group(const ctx_t *c, int scheme, int recon, int solver, dou
             for (int j = l1; j <= h1; ++j)
                 for (int i = l1; i <= h1; ++i) {
                     int n = IDX(i, j, k);
-                    double U[NVMAX], W[NVMAX];
+                    double U0[NVMAX], W0[NVMAX], U[NVMAX], W[NVMAX];
+                    for (int v = 0; v < nv; ++v) W0[v] = wk->W[(size_t)v * NPC + n];
+                    prim2cons(c, W0, U0);
                     for (int v = 0; v < nv; ++v) {
                         double dfx = wk->F1[FLI(0, v, n)] - wk->F1[FLI(0, v, n - STEP[0])];
                         double dfy = wk->F1[FLI(1, v, n)] - wk->F1[FLI(1, v, n - STEP[1])];
                         double dfz = wk->F1[FLI(2, v, n)] - wk->F1[FLI(2, v, n - STEP[2])];
-                        U[v] = in[(size_t)v * NPC + n] - 0.5 * lam_r * ((dfx + dfy) + dfz);
+                        U[v] = U0[v] - 0.5 * lam_r * ((dfx + dfy) + dfz);
                     }
                     cons2prim(c, U, W);
                     floor_prim(c, W);
                     if (!state_ok(W)) {
                         st->n_pred_revert++;
-                        for (int v = 0; v < nv; ++v) W[v] = wk->W[(size_t)v * NPC + n];
+                        for (int v = 0; v < nv; ++v) W[v] = W0[v];
                     }
                     for (int v = 0; v < nv; ++v) wk->WH[(size_t)v * NPC + n] = W[v];
                 }

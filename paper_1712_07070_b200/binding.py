@@ -9,7 +9,7 @@ import os
 
 import torch
 
-MHM, CTU = 1, 2
+MHM, CTU, VL = 1, 2, 3
 PLM, PPM = 1, 2
 ROE, HLLC, HLLE, EXACT = 1, 2, 3, 4
 FP32, FP64 = 4, 8

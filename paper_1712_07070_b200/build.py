@@ -37,8 +37,10 @@ def build(force=False, verbose=False):
     os.makedirs(OBJ, exist_ok=True)
     have_ctu = os.path.exists(os.path.join(CSRC, "ctu_kernel.cuh"))
     jobs = []
-    for s in (1, 2):
+    for s in (1, 2, 3):
         for r in (1, 2):
+            if s == 3 and r == 2:      # VL + PPM is not built (fourth ghost zone)
+                continue
             for v in (1, 2, 3, 4):
                 o = os.path.join(OBJ, "inst_%d_%d_%d.o" % (s, r, v))
                 cmd = [NVCC, *FLAGS, "-DG_SCHEME=%d" % s, "-DG_RECON=%d" % r, "-DG_SOLVER=%d" % v]

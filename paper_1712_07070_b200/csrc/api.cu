@@ -12,13 +12,16 @@ namespace gamer {
 #define G_DECL(s, r, v) cudaError_t gamer_launch_##s##_##r##_##v(int, int, int, const void*, cudaStream_t, int*);
 G_DECL(1, 1, 1) G_DECL(1, 1, 2) G_DECL(1, 1, 3) G_DECL(1, 1, 4) G_DECL(1, 2, 1) G_DECL(1, 2, 2) G_DECL(1, 2, 3) G_DECL(1, 2, 4)
 G_DECL(2, 1, 1) G_DECL(2, 1, 2) G_DECL(2, 1, 3) G_DECL(2, 1, 4) G_DECL(2, 2, 1) G_DECL(2, 2, 2) G_DECL(2, 2, 3) G_DECL(2, 2, 4)
+G_DECL(3, 1, 1) G_DECL(3, 1, 2) G_DECL(3, 1, 3) G_DECL(3, 1, 4)
 #undef G_DECL
 typedef cudaError_t (*launch_fn)(int, int, int, const void*, cudaStream_t, int*);
-static const launch_fn TABLE[2][2][4] = {
+static const launch_fn TABLE[3][2][4] = {
     {{gamer_launch_1_1_1, gamer_launch_1_1_2, gamer_launch_1_1_3, gamer_launch_1_1_4},
      {gamer_launch_1_2_1, gamer_launch_1_2_2, gamer_launch_1_2_3, gamer_launch_1_2_4}},
     {{gamer_launch_2_1_1, gamer_launch_2_1_2, gamer_launch_2_1_3, gamer_launch_2_1_4},
-     {gamer_launch_2_2_1, gamer_launch_2_2_2, gamer_launch_2_2_3, gamer_launch_2_2_4}}};
+     {gamer_launch_2_2_1, gamer_launch_2_2_2, gamer_launch_2_2_3, gamer_launch_2_2_4}},
+    {{gamer_launch_3_1_1, gamer_launch_3_1_2, gamer_launch_3_1_3, gamer_launch_3_1_4},
+     {nullptr, nullptr, nullptr, nullptr}}};      // VL + PPM: needs a fourth ghost zone
 static std::atomic<long long> g_launches{0};
 }  // namespace gamer
 
@@ -30,11 +33,12 @@ static int check_common(const void* in, const void* out, int64_t n_groups, doubl
                         int recon, int riemann, int precision) {
     if (n_groups < 0 || (n_groups > 0 && (!in || !out))) return GAMER_EINVAL;
     if (!(dh > 0.0) || !std::isfinite(dh) || !(gamma > 1.0) || !std::isfinite(gamma)) return GAMER_EINVAL;
-    if (scheme != GAMER_MHM && scheme != GAMER_CTU) return GAMER_EINVAL;
+    if (scheme != GAMER_MHM && scheme != GAMER_CTU && scheme != GAMER_VL) return GAMER_EINVAL;
     if (recon != GAMER_PLM && recon != GAMER_PPM) return GAMER_EINVAL;
     if (riemann < GAMER_ROE || riemann > GAMER_EXACT) return GAMER_EINVAL;
     if (precision != GAMER_FP32 && precision != GAMER_FP64) return GAMER_EINVAL;
     if (!aligned16(in) || !aligned16(out)) return GAMER_EINVAL;
+    if (scheme == GAMER_VL && recon != GAMER_PLM) return GAMER_EUNSUPPORTED;
     return GAMER_OK;
 }
 
@@ -182,7 +186,7 @@ static int cfl_typed(const void* u, int64_t n_groups, double dh, double gamma, d
     if (cudaMemsetAsync(dt_out, 0, sizeof(double), st) != cudaSuccess) return GAMER_ECUDA;
     if (n_groups > 0) {
         const unsigned grid = (unsigned)n_groups;
-        if (scheme == GAMER_MHM) {
+        if (scheme != GAMER_CTU) {      // Eq. (2): MHM and VL (L168)
             if (nsc) cfl_kernel<T, 6, MHM><<<grid, 256, 0, st>>>(a); else cfl_kernel<T, 5, MHM><<<grid, 256, 0, st>>>(a);
         } else {
             if (nsc) cfl_kernel<T, 6, CTU><<<grid, 256, 0, st>>>(a); else cfl_kernel<T, 5, CTU><<<grid, 256, 0, st>>>(a);
@@ -197,7 +201,7 @@ static int cfl_typed(const void* u, int64_t n_groups, double dh, double gamma, d
 extern "C" int gamer_cfl_dt_ex(const void* u, int64_t n_groups, double dh, double gamma, double cfl, int scheme,
                                int precision, void* group_speed_out, double* dt_out, const gamer_opts* opts) {
     if (!u || !dt_out || n_groups < 0 || !(dh > 0.0) || !(gamma > 1.0) || !(cfl > 0.0)) return GAMER_EINVAL;
-    if (scheme != GAMER_MHM && scheme != GAMER_CTU) return GAMER_EINVAL;
+    if (scheme != GAMER_MHM && scheme != GAMER_CTU && scheme != GAMER_VL) return GAMER_EINVAL;
     if (precision != GAMER_FP32 && precision != GAMER_FP64) return GAMER_EINVAL;
     if (!aligned16(u)) return GAMER_EINVAL;
     if (opts && (opts->n_scalar < 0 || opts->n_scalar > 1)) return GAMER_EINVAL;

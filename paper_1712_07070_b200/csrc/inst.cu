@@ -3,7 +3,7 @@
 #include "launch.cuh"
 
 #ifndef G_SCHEME
-#error "compile with -DG_SCHEME=1|2 -DG_RECON=1|2 -DG_SOLVER=1|2|3"
+#error "compile with -DG_SCHEME=1|2|3 -DG_RECON=1|2 -DG_SOLVER=1|2|3|4 (scheme 3 = VL: recon 1 only)"
 #endif
 
 #define G_CAT2(a, b, c, d) a##b##_##c##_##d
@@ -17,6 +17,8 @@ static cudaError_t go(const void* args, cudaStream_t st, int* launches) {
     const AdvArgs<T>& a = *static_cast<const AdvArgs<T>*>(args);
 #if G_SCHEME == 1
     return launch_mhm<T, G_RECON, G_SOLVER, NV, EXT>(a, st, launches);
+#elif G_SCHEME == 3
+    return launch_mhm<T, G_RECON, G_SOLVER, NV, EXT, true>(a, st, launches);
 #elif defined(GAMER_HAVE_CTU)
     return launch_ctu<T, G_RECON, G_SOLVER, NV, EXT>(a, st, launches);
 #else

@@ -12,32 +12,32 @@ namespace gamer {
 
 constexpr size_t SMEM_LIMIT = 232448;   // 227 KB opt-in maximum per CTA on sm_100
 
-template <typename T, int RECON, int NV>
+template <typename T, int RECON, int NV, bool VLS>
 constexpr int mhm_tile() {
-    return MhmGeo<T, RECON, NV, 16>::BYTES <= SMEM_LIMIT ? 16 : (MhmGeo<T, RECON, NV, 8>::BYTES <= SMEM_LIMIT ? 8 : 4);
+    return MhmGeo<T, RECON, NV, 16, 2, false, VLS>::BYTES <= SMEM_LIMIT ? 16 : (MhmGeo<T, RECON, NV, 8, 2, false, VLS>::BYTES <= SMEM_LIMIT ? 8 : 4);
 }
 
 constexpr size_t SM_SMEM = 233472;      // 228 KB of shared memory per SM, 1 KB of it reserved per resident CTA
 constexpr int ctas_by_smem(size_t bytes) { return (int)(SM_SMEM / (bytes + 1024)); }
 
-template <typename T, int RECON, int SOLVER, int NV, bool EXT, bool FUSED>
+template <typename T, int RECON, int SOLVER, int NV, bool EXT, bool FUSED, bool VLS>
 cudaError_t launch_mhm_f(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
 #ifdef MHM_TY_OVERRIDE
     constexpr int TY = MHM_TY_OVERRIDE;
 #else
-    constexpr int TY = mhm_tile<T, RECON, NV>();
+    constexpr int TY = mhm_tile<T, RECON, NV, VLS>();
 #endif
     // two landing stages unless dropping to one lets a second CTA share the SM
-    constexpr int C2 = ctas_by_smem(MhmGeo<T, RECON, NV, TY, 2, FUSED>::BYTES), C1 = ctas_by_smem(MhmGeo<T, RECON, NV, TY, 1, FUSED>::BYTES);
+    constexpr int C2 = ctas_by_smem(MhmGeo<T, RECON, NV, TY, 2, FUSED, VLS>::BYTES), C1 = ctas_by_smem(MhmGeo<T, RECON, NV, TY, 1, FUSED, VLS>::BYTES);
 #ifdef MHM_FORCE_NSTG2
     constexpr int NSTG = 2;
 #else
     constexpr int NSTG = (!FUSED && C1 >= 2 && C2 < 2) ? 1 : 2;      // the fused gather is pipelined over two stages
 #endif
-    using G = MhmGeo<T, RECON, NV, TY, NSTG, FUSED>;
+    using G = MhmGeo<T, RECON, NV, TY, NSTG, FUSED, VLS>;
     static_assert(G::BYTES <= SMEM_LIMIT, "tile does not fit in shared memory");
     constexpr int MINB = ctas_by_smem(G::BYTES) >= 2 ? 2 : 1;
-    auto kern = mhm_kernel<T, RECON, SOLVER, NV, EXT, TY, NSTG, MINB, FUSED>;
+    auto kern = mhm_kernel<T, RECON, SOLVER, NV, EXT, TY, NSTG, MINB, FUSED, VLS>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::BYTES);
     if (e != cudaSuccess) return e;
     if (G::NTILE > 1 && a.speed) {
@@ -51,10 +51,10 @@ cudaError_t launch_mhm_f(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
 }
 
 // a.nbr set => `in` is the unpadded state and the ghost refresh is fused into the staging loads
-template <typename T, int RECON, int SOLVER, int NV, bool EXT>
+template <typename T, int RECON, int SOLVER, int NV, bool EXT, bool VLS = false>
 cudaError_t launch_mhm(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
-    return a.nbr ? launch_mhm_f<T, RECON, SOLVER, NV, EXT, true>(a, st, launches)
-                 : launch_mhm_f<T, RECON, SOLVER, NV, EXT, false>(a, st, launches);
+    return a.nbr ? launch_mhm_f<T, RECON, SOLVER, NV, EXT, true, VLS>(a, st, launches)
+                 : launch_mhm_f<T, RECON, SOLVER, NV, EXT, false, VLS>(a, st, launches);
 }
 
 #ifdef GAMER_HAVE_CTU

@@ -24,8 +24,9 @@
 
 namespace gamer {
 
-template <typename T, int RECON, int NV, int TY, int NSTG = 2, bool FUSED = false> struct MhmGeo {
+template <typename T, int RECON, int NV, int TY, int NSTG = 2, bool FUSED = false, bool VLS = false> struct MhmGeo {
     static constexpr int R = RECON == PPM ? 2 : 1;
+    static constexpr int RSTAGE = VLS ? R + 1 : R;              // planes staged beyond the tile: the VL half-step predictor reaches one cell further
     static constexpr int RING = 2 * R + 2;
     static constexpr int NI = 16 * TY;                          // interior threads
     static constexpr int NXH = 2 * TY, NYH = 32;                // halo threads
@@ -37,10 +38,18 @@ template <typename T, int RECON, int NV, int TY, int NSTG = 2, bool FUSED = fals
     static constexpr int BLK = (NSX + NSY) * NV;                // one buffer of states (or of fluxes)
     static constexpr int RSTG = NV * (FUSED ? NR * FW : PLN);   // one landing stage (fused refresh: 24-wide rows)
     static constexpr int RAW = 0;                               // [NSTG][RSTG]  TMA / cp.async landing stages
-    static constexpr int PRIM = RAW + NSTG * RSTG;              // [RING][NV][PLN]
+    static constexpr int PRIM = RAW + NSTG * RSTG;              // [RING][NV][PLN]  (VL: primitives of the half-step state)
     static constexpr int ST = PRIM + RING * NV * PLN;           // [2] x [Vec4 NSX | (NV-4) NSX | Vec4 NSY | (NV-4) NSY]
     static constexpr int FL = ST + 2 * BLK;                     // same shape, fluxes in natural variable order
-    static constexpr int END = FL + 2 * BLK;
+    static constexpr int END0 = FL + 2 * BLK;
+    // VL scheme only: primitives of U^n (3 planes) and the first-order fluxes of the half-step predictor, [NV][n] each
+    static constexpr int NRH = TY + 4;                          // rows of half-step cells: -2 .. TY+1
+    static constexpr int NF1X = 21 * NRH, NF1Y = 20 * (NRH + 1), NF1Z = 20 * NRH;
+    static constexpr int WN = END0;                             // [3][NV][PLN]
+    static constexpr int F1X = WN + 3 * NV * PLN;
+    static constexpr int F1Y = F1X + NV * NF1X;
+    static constexpr int F1Z = F1Y + NV * NF1Y;                 // [2][NV][NF1Z]: faces below planes of even / odd padded index
+    static constexpr int END = VLS ? F1Z + 2 * NV * NF1Z : END0;
     static constexpr int NCOPY = FUSED ? FusedCopies<T, NV, TY>::N : 0;                   // fused refresh: copy list
     static constexpr size_t BYTES = 16 + (size_t)END * sizeof(T) + (FUSED ? 128 + 8 * (size_t)NCOPY : 0);   // 2 mbarriers
                                                                 // first; neighbour table and copy list last
@@ -126,6 +135,74 @@ __device__ __forceinline__ bool mhm_evolve(const T* Uf, const T* hdU, T* Ue, boo
     return (Ue[0] > T(0)) && (pe > T(0));
 }
 
+// ---------------------------------------------------------------------------------------------
+// VL scheme (DESIGN R26): the half-step predictor is a first-order Godunov update of the cell
+// averages.  Two cooperative stages per plane, work items spread over all threads of the tile:
+//   vl_faces : first-order fluxes from the piecewise-constant primitives W^n -- x and y faces of padded plane pm and
+//              the z faces between planes pm and pm+1 -- on the 20 x (TY+4) cells the reconstruction will read;
+//   vl_cells : U^{n+1/2} = U^n - dt/(2 dh) sum_d dF1_d  ->  primitives (floors; an unphysical state falls back to
+//              W^n) into the ring of half-step primitive planes, which the PLM face values are then taken from.
+// ---------------------------------------------------------------------------------------------
+template <typename T, int SOLVER, int NV, class G, int NT>
+__device__ __forceinline__ void vl_faces(const T* wlo, const T* whi, T* f1x, T* f1y, T* f1z, bool xy, const Phys<T>& ph, int tid,
+                                         Counters& cnt) {
+    constexpr int PLN = G::PLN, NX = G::NF1X, NY = G::NF1Y, NZ = G::NF1Z;
+    for (int it = (xy ? 0 : NX + NY) + tid; it < NX + NY + NZ; it += NT) {
+        int d, l, rr, n, o;
+        const T* pr = wlo;
+        T* fo;
+        if (it < NX) {                    // x face ii (between staged columns ii, ii+1) of half-step row r
+            const int r = it / 21, ii = it - r * 21;
+            d = 0; l = (r + 1) * NP + ii; rr = l + 1; fo = f1x; n = NX; o = it;
+        } else if (it < NX + NY) {        // y face between staged rows r, r+1, column ii+1
+            const int g = it - NX;
+            const int r = g / 20, ii = g - r * 20;
+            d = 1; l = r * NP + ii + 1; rr = l + NP; fo = f1y; n = NY; o = g;
+        } else {                          // z face between the two planes
+            const int g = it - NX - NY;
+            const int r = g / 20, ii = g - r * 20;
+            d = 2; l = (r + 1) * NP + ii + 1; rr = l; pr = whi; fo = f1z; n = NZ; o = g;
+        }
+        const int cn = 1 + d, c1 = d == 2 ? 1 : 2 + d, c2 = d == 0 ? 3 : d;      // 1 + (d+1)%3, 1 + (d+2)%3
+        T WL[NV], WR[NV], F[NV];
+        WL[0] = wlo[l]; WL[1] = wlo[cn * PLN + l]; WL[2] = wlo[c1 * PLN + l]; WL[3] = wlo[c2 * PLN + l]; WL[4] = wlo[4 * PLN + l];
+        WR[0] = pr[rr]; WR[1] = pr[cn * PLN + rr]; WR[2] = pr[c1 * PLN + rr]; WR[3] = pr[c2 * PLN + rr]; WR[4] = pr[4 * PLN + rr];
+#pragma unroll
+        for (int v = 5; v < NV; ++v) { WL[v] = wlo[v * PLN + l]; WR[v] = pr[v * PLN + rr]; }
+        cnt.roe_fb += riemann_flux<T, SOLVER, NV>(WL, WR, F, ph) ? 1 : 0;
+        fo[o] = F[0]; fo[cn * n + o] = F[1]; fo[c1 * n + o] = F[2]; fo[c2 * n + o] = F[3]; fo[4 * n + o] = F[4];
+#pragma unroll
+        for (int v = 5; v < NV; ++v) fo[v * n + o] = F[v];
+    }
+}
+
+template <typename T, int NV, bool EXT, class G, int NT>
+__device__ __forceinline__ void vl_cells(const T* wn, const T* f1x, const T* f1y, const T* fzlo, const T* fzhi, T* wh,
+                                         const Phys<T>& ph, int tid, Counters& cnt) {
+    constexpr int PLN = G::PLN, NX = G::NF1X, NY = G::NF1Y, NZ = G::NF1Z;
+    for (int c = tid; c < NZ; c += NT) {
+        const int r = c / 20, ii = c - r * 20;
+        const int s = (r + 1) * NP + ii + 1;
+        T W0[NV], U[NV], W[NV];
+#pragma unroll
+        for (int v = 0; v < NV; ++v) W0[v] = wn[v * PLN + s];
+        prim2cons<T, NV>(W0, U, ph);
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+            const T dfx = f1x[v * NX + r * 21 + ii + 1] - f1x[v * NX + r * 21 + ii];
+            const T dfy = f1y[v * NY + (r + 1) * 20 + ii] - f1y[v * NY + r * 20 + ii];
+            const T dfz = fzhi[v * NZ + c] - fzlo[v * NZ + c];
+            U[v] = U[v] - ph.hlam * ((dfx + dfy) + dfz);
+        }
+        cons2prim<T, NV>(U, W, ph);
+        if (EXT && ph.floors) floor_prim(W, ph);
+        const bool ok = (W[0] > T(0)) && (W[4] > T(0));
+        if (!ok) cnt.reverted++;
+#pragma unroll
+        for (int v = 0; v < NV; ++v) wh[v * PLN + s] = ok ? W[v] : W0[v];
+    }
+}
+
 // per-thread constants of the cell column this thread owns
 template <typename T> struct MhmCell {
     int cidx;            // cell inside a staged plane
@@ -134,13 +211,15 @@ template <typename T> struct MhmCell {
     int out_off;         // cell (ei, ej) inside a 16 x 16 plane of `out` (also of a z plane of flux_out)
 };
 
-template <typename T, int RECON, int SOLVER, int NV, bool EXT, int TY, int NSTG, int MINB, bool FUSED>
-__global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED>::NT), MINB) mhm_kernel(const AdvArgs<T> a) {
-    using G = MhmGeo<T, RECON, NV, TY, NSTG, FUSED>;
+template <typename T, int RECON, int SOLVER, int NV, bool EXT, int TY, int NSTG, int MINB, bool FUSED, bool VLS>
+__global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED, VLS>::NT), MINB) mhm_kernel(const AdvArgs<T> a) {
+    using G = MhmGeo<T, RECON, NV, TY, NSTG, FUSED, VLS>;
     constexpr int RS = G::RSTG;
     constexpr int R = G::R, RING = G::RING, NT = G::NT, NI = G::NI, PLN = G::PLN, S = NV * G::PLN;
-    constexpr int NPL = 18 + 2 * R;      // staged planes: padded PF .. PF+NPL-1
-    constexpr int PF = 2 - R;
+    constexpr int NPL = 18 + 2 * G::RSTAGE;      // staged planes: padded PF .. PF+NPL-1
+    constexpr int PF = 2 - G::RSTAGE;
+    constexpr int CV = VLS ? 7 : 2 + 2 * R;      // staged plane kk+CV is converted in iteration kk
+    static_assert(!VLS || RECON == PLM, "VL + PPM would need a fourth ghost zone");
     constexpr int PSQ = PS * PS;
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -212,20 +291,47 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED>::NT), M
         issue_plane<T, NV, TY>(gin, j0, PF + 0, raw, &bars[0]);
         if (NSTG > 1) issue_plane<T, NV, TY>(gin, j0, PF + 1, raw + RS, &bars[1]);
     }
-    // prologue: staged planes n = 0 .. 2R (what the predictor of plane -1 reads), all threads convert
-    for (int n = 0; n <= 2 * R; ++n) {
+    // prologue: all threads convert staged plane n into dst, then the freed landing stage is refilled
+    auto convert_all = [&](int n, T* dst) {
         if (FUSED) {
             cp_async_wait<0>();
             __syncthreads();
-            convert_plane_fused<T, NV, EXT, TY, NT>(raw + (n % NSTG) * RS, prim + n * S, ph, tid);
+            convert_plane_fused<T, NV, EXT, TY, NT>(raw + (n % NSTG) * RS, dst, ph, tid);
         } else {
             mbar_wait(&bars[n % NSTG], (n / NSTG) & 1);
-            convert_plane<T, NV, EXT, TY, NT>(raw + (n % NSTG) * RS, prim + n * S, ph, tid);
+            convert_plane<T, NV, EXT, TY, NT>(raw + (n % NSTG) * RS, dst, ph, tid);
         }
         __syncthreads();
         if (n + NSTG < NPL) {
             if (FUSED) stage_plane_fused<T, NV, TY>(gin, nb, ctab, j0, PF + n + NSTG, raw + (n % NSTG) * RS, tid, NT);
             else if (tid == NI) issue_plane<T, NV, TY>(gin, j0, PF + n + NSTG, raw + (n % NSTG) * RS, &bars[n % NSTG]);
+        }
+    };
+    Counters cnt = {0, 0, 0, 0, 0};
+    T* wn = sm + G::WN;                              // VL: primitives of U^n, padded plane p in slot p % 3
+    T* f1x = sm + G::F1X;
+    T* f1y = sm + G::F1Y;
+    T* f1z = sm + G::F1Z;                            // faces below padded plane p in buffer p & 1
+    constexpr int FZB = NV * G::NF1Z;
+    if constexpr (!VLS) {
+        // staged planes n = 0 .. 2R: what the predictor of plane -1 reads
+        for (int n = 0; n <= 2 * R; ++n) convert_all(n, prim + n * S);
+    } else {
+        // half-step primitives of the cell planes -2, -1, 0 (what the predictor of plane -1 reads) from padded planes 0 .. 4
+        for (int n = 0; n < 3; ++n) convert_all(n, wn + n * S);
+        vl_faces<T, SOLVER, NV, G, NT>(wn, wn + S, f1x, f1y, f1z + FZB, false, ph, tid, cnt);            // z faces below plane 1
+        vl_faces<T, SOLVER, NV, G, NT>(wn + S, wn + 2 * S, f1x, f1y, f1z, true, ph, tid, cnt);           // plane 1, z faces below plane 2
+        __syncthreads();
+        for (int m = -2; m <= 0; ++m) {
+            const int pm = m + NGH;
+            vl_cells<T, NV, EXT, G, NT>(wn + (pm % 3) * S, f1x, f1y, f1z + (pm & 1) * FZB, f1z + ((pm + 1) & 1) * FZB,
+                                        prim + (m + 2) * S, ph, tid, cnt);
+            convert_all(pm + 2, wn + ((pm + 2) % 3) * S);
+            if (m < 0) {
+                vl_faces<T, SOLVER, NV, G, NT>(wn + ((pm + 1) % 3) * S, wn + ((pm + 2) % 3) * S, f1x, f1y, f1z + (pm & 1) * FZB, true, ph,
+                                               tid, cnt);
+                __syncthreads();
+            }
         }
     }
 
@@ -234,7 +340,6 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED>::NT), M
 #pragma unroll
     for (int v = 0; v < NV; ++v) { zplus[v] = T(1); fzl[v] = T(0); }
     T smax = T(0);
-    Counters cnt = {0, 0, 0, 0, 0};
     // Q[m] = ring slot (offset into prim) of staged plane kk+1+m; Q[2R+1] is the slot the next plane goes to
     int Q[RING];
 #pragma unroll
@@ -260,7 +365,7 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED>::NT), M
             // as it has been evolved; x+ / y+ go to shared memory at once, pass 1 simply overwrites them.
             T zminus[NV], znew[NV];
 #pragma unroll 1
-            for (int pass = 0; pass < 2; ++pass) {
+            for (int pass = VLS ? 1 : 0; pass < 2; ++pass) {      // VL: plain face values of the half-step state, nothing to evolve
                 T Uf[3][2][NV], dU[NV], Ue[NV];
                 mhm_face_states<T, RECON, NV, EXT, PLN>(Pz, ph, Uf, dU);
 #pragma unroll
@@ -312,22 +417,29 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED>::NT), M
                 for (int k = 0; k < NV; ++k) zplus[k] = znew[k];
             }
         }
+        // ------------------------------------------------------------------ VL: first-order fluxes of the plane two above
+        if constexpr (VLS) {
+            const int pm = kk + 2 + NGH;
+            if (pm <= PS + 1 + NGH)
+                vl_faces<T, SOLVER, NV, G, NT>(wn + (pm % 3) * S, wn + ((pm + 1) % 3) * S, f1x, f1y, f1z + ((pm + 1) & 1) * FZB, true, ph, tid, cnt);
+        }
         // ------------------------------------------------------------------ halo warps: next plane -> primitives
         {
-            const int n = kk + 2 + 2 * R;
+            const int n = kk + CV;
             if (!interior && n < NPL) {
+                T* dst = VLS ? wn + (n % 3) * S : prim + Q[2 * R + 1];
                 if (FUSED) {      // this plane's copies were waited for before the previous barrier
-                    convert_plane_fused<T, NV, EXT, TY, G::NCV>(raw + (n % NSTG) * RS, prim + Q[2 * R + 1], ph, tid - NI);
+                    convert_plane_fused<T, NV, EXT, TY, G::NCV>(raw + (n % NSTG) * RS, dst, ph, tid - NI);
                 } else {
                     mbar_wait(&bars[n % NSTG], (n / NSTG) & 1);
-                    convert_plane<T, NV, EXT, TY, G::NCV>(raw + (n % NSTG) * RS, prim + Q[2 * R + 1], ph, tid - NI);
+                    convert_plane<T, NV, EXT, TY, G::NCV>(raw + (n % NSTG) * RS, dst, ph, tid - NI);
                 }
             }
         }
         if (FUSED) cp_async_wait<0>();      // the plane issued one barrier ago: visible to the converting warps after this one
         __syncthreads();
         {      // the stage the plane above came from is free again
-            const int n = kk + 2 + 2 * R + NSTG;
+            const int n = kk + CV + NSTG;
             if (n < NPL) {
                 if (FUSED) stage_plane_fused<T, NV, TY>(gin, nb, ctab, j0, PF + n, raw + (n % NSTG) * RS, tid, NT);
                 else if (tid == NI) issue_plane<T, NV, TY>(gin, j0, PF + n, raw + (n % NSTG) * RS, &bars[n % NSTG]);
@@ -407,6 +519,13 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED>::NT), M
         if (interior && kk >= 0) {
 #pragma unroll
             for (int v = 0; v < NV; ++v) fzl[v] = fzn[v];
+        }
+        if constexpr (VLS) {      // half-step primitives of the plane two above into the spare ring slot; second barrier of the plane
+            const int pm = kk + 2 + NGH;
+            if (pm <= PS + 1 + NGH)
+                vl_cells<T, NV, EXT, G, NT>(wn + (pm % 3) * S, f1x, f1y, f1z + (pm & 1) * FZB, f1z + ((pm + 1) & 1) * FZB,
+                                            prim + Q[2 * R + 1], ph, tid, cnt);
+            __syncthreads();
         }
         // rotate the ring: the slot of the lowest plane is the one the plane after next is converted into
         {

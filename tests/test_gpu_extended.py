@@ -41,6 +41,8 @@ STRESS = [
     (gb.MHM, gb.PPM, gb.ROE, dict(remedy_first_order=True)),
     (gb.MHM, gb.PLM, gb.HLLE, dict(n_scalar=1, min_temp=1e-3)),
     (gb.CTU, gb.PLM, gb.ROE, dict()),
+    (gb.VL, gb.PLM, gb.ROE, dict(n_scalar=1, dual_energy=True, remedy_first_order=True, min_pres=1e-12, min_dens=1e-10)),
+    (gb.VL, gb.PLM, gb.HLLC, dict()),
 ]
 
 
@@ -65,8 +67,10 @@ def test_stress_modes_match_oracle(dev, oracle_mod, scheme, recon, solver, kw, d
         # per-cell decisions are counted exactly; per-face / per-state ones are counted once per tile, and the
         # fp64 variants that do not fit 227 KB split a group in 2 or 4 tiles whose halo faces overlap
         assert diag[2] == st["n_first_order"] and diag[3] == st["n_dual_fix"]
-        assert st["n_roe_fallback"] <= diag[0] <= 1.6 * st["n_roe_fallback"] + 2
-        assert 0.9 * st["n_pred_revert"] - 2 <= diag[1] <= 1.6 * st["n_pred_revert"] + 2
+        # (VL: the half-step predictor of a 4-row tile covers 8 rows, so its first-pass faces are counted twice)
+        over = 2.2 if scheme == gb.VL else 1.6
+        assert st["n_roe_fallback"] <= diag[0] <= over * st["n_roe_fallback"] + 2
+        assert 0.9 * st["n_pred_revert"] - 2 <= diag[1] <= over * st["n_pred_revert"] + 2
         assert max(err.values()) <= 1e-12, err
         fe = np.abs(flux.cpu().numpy() - ref["flux"]).sum() / np.abs(ref["flux"]).sum()
         assert fe <= 1e-12
@@ -226,7 +230,8 @@ def test_config3_two_level_sedov_flux_correction(dev, oracle_mod):
 @pytest.mark.parametrize("scheme,recon,solver,kw", [(gb.MHM, gb.PLM, gb.ROE, {}), (gb.MHM, gb.PPM, gb.HLLC, {}),
                                                     (gb.MHM, gb.PLM, gb.HLLE, dict(n_scalar=1, dual_energy=True, min_pres=1e-12)),
                                                     (gb.CTU, gb.PPM, gb.HLLC, {}), (gb.CTU, gb.PLM, gb.ROE, {}),
-                                                    (gb.CTU, gb.PPM, gb.HLLE, dict(n_scalar=1, dual_energy=True, min_pres=1e-12))])
+                                                    (gb.CTU, gb.PPM, gb.HLLE, dict(n_scalar=1, dual_energy=True, min_pres=1e-12)),
+                                                    (gb.VL, gb.PLM, gb.HLLC, {}), (gb.VL, gb.PLM, gb.ROE, dict(n_scalar=1, dual_energy=True, min_pres=1e-12))])
 def test_fused_ghost_refresh_entry_is_bitwise_the_padded_path(dev, scheme, recon, solver, kw, dtype):
     """SURVEY 8(f) NEXT-1, second half: gamer_fluid_advance_resident gathers the ghost zones from the neighbours'
     unpadded state inside the solver.  On a periodic 2 x 3 x 4 box of groups (so that -1 and +1 neighbours coincide

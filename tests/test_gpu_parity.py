@@ -18,7 +18,8 @@ G53 = 5.0 / 3.0
 TOL = {torch.float64: 1e-12, torch.float32: 1e-5}
 SCHEMES = [gb.MHM, gb.CTU]
 COMBOS = list(itertools.product(SCHEMES, (gb.PLM, gb.PPM), (gb.ROE, gb.HLLC, gb.HLLE))) + \
-    [(gb.MHM, gb.PLM, gb.EXACT), (gb.CTU, gb.PPM, gb.EXACT), (gb.MHM, gb.PPM, gb.EXACT), (gb.CTU, gb.PLM, gb.EXACT)]
+    [(gb.MHM, gb.PLM, gb.EXACT), (gb.CTU, gb.PPM, gb.EXACT), (gb.MHM, gb.PPM, gb.EXACT), (gb.CTU, gb.PLM, gb.EXACT)] + \
+    [(gb.VL, gb.PLM, s) for s in (gb.ROE, gb.HLLC, gb.HLLE, gb.EXACT)]      # VL scheme, PLM only
 
 
 @pytest.fixture(scope="module")
@@ -78,7 +79,7 @@ def test_one_step_matches_oracle(dev, oracle_mod, scheme, recon, solver, dtype):
         assert (np.abs(out.cpu().numpy() - ref["out"]) / scale).max() <= 1e-11
 
 
-@pytest.mark.parametrize("scheme,recon,solver", [(gb.MHM, gb.PLM, gb.ROE), (gb.CTU, gb.PPM, gb.HLLC)])
+@pytest.mark.parametrize("scheme,recon,solver", [(gb.MHM, gb.PLM, gb.ROE), (gb.CTU, gb.PPM, gb.HLLC), (gb.VL, gb.PLM, gb.HLLC)])
 def test_fp64_is_bitwise_reproducible_and_eleven_arg_form_agrees(dev, scheme, recon, solver):
     """bitwise reproducibility (run to run)."""
     f = inputs.turbulence_field(32, 7, kmax=4, gamma=G53)
@@ -101,7 +102,7 @@ def test_uniform_state_bitwise_invariant(dev, scheme, recon, solver, dtype):
     assert torch.equal(out, inputs.interior(padded))
 
 
-@pytest.mark.parametrize("scheme,recon,solver", [(gb.MHM, gb.PLM, gb.ROE), (gb.CTU, gb.PPM, gb.HLLC)])
+@pytest.mark.parametrize("scheme,recon,solver", [(gb.MHM, gb.PLM, gb.ROE), (gb.CTU, gb.PPM, gb.HLLC), (gb.VL, gb.PLM, gb.ROE)])
 def test_shared_faces_bitwise_equal_and_conservation(dev, scheme, recon, solver):
     f = inputs.turbulence_field(32, 1712, kmax=4, gamma=G53)
     padded = inputs.pack_periodic(f).to(dev)
@@ -298,3 +299,11 @@ def test_table_driven_ghost_refresh_matches_oracle(dev, oracle_mod, dtype):
     torch.cuda.synchronize()
     assert np.array_equal(padded.cpu().numpy(), ref)
     assert not np.array_equal(ref, before.numpy())
+
+
+def test_vl_with_ppm_is_unsupported(dev):
+    """VL + PPM would read a fourth ghost zone; the header promises GAMER_EUNSUPPORTED."""
+    padded = inputs.pack_periodic(inputs.turbulence_field(16, 3, kmax=2, gamma=G53)).to(dev)
+    out, flux, _ = gb.alloc_outputs(padded)
+    with pytest.raises(gb.GamerError, match="-2"):
+        gb.gamer_fluid_advance(padded, out, flux, 1e-3, 1 / 16, G53, gb.VL, gb.PPM, gb.ROE)
