@@ -34,6 +34,7 @@ class Opts(ctypes.Structure):
         ("min_temp", ctypes.c_double),
         ("remedy_first_order", ctypes.c_int),
         ("char_limiting", ctypes.c_int),
+        ("renormalize", ctypes.c_int),
     ]
 
 
@@ -61,9 +62,9 @@ def lib():
 
 
 def make_opts(limiter=GMINMOD, theta=0.0, n_scalar=0, dual_energy=False, de_xi=1e-2,
-              min_dens=0.0, min_pres=0.0, min_temp=0.0, remedy_first_order=False, char_limiting=False):
+              min_dens=0.0, min_pres=0.0, min_temp=0.0, remedy_first_order=False, char_limiting=False, renormalize=False):
     return Opts(limiter, theta, n_scalar, int(dual_energy), de_xi, min_dens, min_pres, min_temp,
-                int(remedy_first_order), int(char_limiting))
+                int(remedy_first_order), int(char_limiting), int(renormalize))
 
 
 def _p(a):

@@ -50,7 +50,8 @@
 #define NG   3               /* ghost cells per side (L300)                   */
 #define NP   (PS + 2 * NG)   /* padded edge = 22                              */
 #define NPC  (NP * NP * NP)  /* padded cells per group = 10648                */
-#define NVMAX 6
+#define NSMAX 8             /* passive scalars carried at most (L96 "an arbitrary number"; a compile-time bound here) */
+#define NVMAX (5 + NSMAX)
 #define IDX(i, j, k) ((((k) * NP) + (j)) * NP + (i))
 
 enum { SCHEME_MHM = 1, SCHEME_CTU = 2, SCHEME_VL = 3 };
@@ -61,12 +62,13 @@ enum { LIMITER_GMINMOD = 1, LIMITER_VANLEER = 2, LIMITER_VANALBADA = 3 };
 typedef struct {
     int    limiter;            /* LIMITER_*                                              */
     double theta;              /* generalized-minmod parameter                           */
-    int    n_scalar;           /* 0 or 1 passively advected scalar (the entropy, L100)   */
+    int    n_scalar;           /* 0..NSMAX passively advected scalars (L96); with dual_energy the LAST one is the entropy (L100) */
     int    dual_energy;        /* 0/1                                                    */
     double de_xi;              /* switch E_the/E_kin < xi (L100)                         */
     double min_dens, min_pres, min_temp;   /* floors; 0 = off                            */
     int    remedy_first_order; /* remedy (ii), L105                                      */
     int    char_limiting;      /* 0: slopes limited in primitive variables; 1: in characteristic ones (L94) */
+    int    renormalize;        /* 1: after the update rescale the passive scalars (not the entropy) so that they sum to rho (L96) */
 } orc_opts;
 
 typedef struct {
@@ -99,7 +101,7 @@ static void cons2prim(const ctx_t *c, const double *U, double *W)
     W[3] = U[3] / rho;
     double ekin = 0.5 * (U[1] * U[1] + U[2] * U[2] + U[3] * U[3]) / rho;
     W[4] = c->gm1 * (U[4] - ekin);
-    if (c->nv > 5) W[5] = U[5] / rho;
+    for (int v = 5; v < c->nv; ++v) W[v] = U[v] / rho;   /* q_k = s_k / rho */
 }
 
 static void prim2cons(const ctx_t *c, const double *W, double *U)
@@ -110,7 +112,7 @@ static void prim2cons(const ctx_t *c, const double *W, double *U)
     U[2] = rho * W[2];
     U[3] = rho * W[3];
     U[4] = W[4] / c->gm1 + 0.5 * rho * (W[1] * W[1] + W[2] * W[2] + W[3] * W[3]);
-    if (c->nv > 5) U[5] = rho * W[5];
+    for (int v = 5; v < c->nv; ++v) U[v] = rho * W[v];
 }
 
 static int floors_set(const ctx_t *c)
@@ -138,7 +140,7 @@ static void phys_flux(const ctx_t *c, int d, const double *W, const double *U, d
     F[3] = U[3] * vn;
     F[1 + d] += W[4];
     F[4] = vn * (U[4] + W[4]);
-    if (c->nv > 5) F[5] = U[5] * vn;
+    for (int v = 5; v < c->nv; ++v) F[v] = U[v] * vn;
 }
 
 /* ------------------------------------------------------------------------------------------
@@ -454,9 +456,9 @@ static void riemann(const ctx_t *c, int solver, int d, const double *UL, const d
     F[t1] = f[2];
     F[t2] = f[3];
     F[4] = f[4];
-    if (c->nv > 5) { /* R12: passive scalar rides the mass flux, upwinded */
-        double ql = UL[5] / UL[0], qr = UR[5] / UR[0];
-        F[5] = f[0] >= 0.0 ? f[0] * ql : f[0] * qr;
+    for (int v = 5; v < c->nv; ++v) { /* R12: every passive scalar rides the mass flux, upwinded */
+        double ql = UL[v] / UL[0], qr = UR[v] / UR[0];
+        F[v] = f[0] >= 0.0 ? f[0] * ql : f[0] * qr;
     }
 }
 
@@ -474,7 +476,7 @@ static void project(const double *dW, double rho, double cs, int nv, double *amp
     amp[2] = dW[2];                                    /* shear        */
     amp[3] = dW[3];                                    /* shear        */
     amp[4] = (dW[4] + rho * cs * dW[1]) / (2.0 * c2);  /* v + c        */
-    if (nv > 5) amp[5] = dW[5];                        /* scalar       */
+    for (int v = 5; v < nv; ++v) amp[v] = dW[v];       /* scalars      */
 }
 
 static void add_wave(double *T, int alpha, double amp, double rho, double cs)
@@ -485,7 +487,7 @@ static void add_wave(double *T, int alpha, double amp, double rho, double cs)
     case 2: T[2] += amp; break;
     case 3: T[3] += amp; break;
     case 4: T[0] += amp; T[1] += amp * cs / rho; T[4] += amp * cs * cs; break;
-    default: T[5] += amp; break;
+    default: T[alpha] += amp; break;   /* passive scalar alpha: its own characteristic field, speed vn */
     }
 }
 
@@ -494,7 +496,8 @@ static void trace_cell(const ctx_t *c, int recon, const double *W, const double 
 {
     int nv = c->nv;
     double rho = W[0], vn = W[1], cs = sqrt(c->gamma * W[4] / W[0]);
-    double lam[NVMAX] = {vn - cs, vn, vn, vn, vn + cs, vn};
+    double lam[NVMAX] = {vn - cs, vn, vn, vn, vn + cs};
+    for (int a = 5; a < nv; ++a) lam[a] = vn;
     double chi[NVMAX];
     for (int a = 0; a < nv; ++a) chi[a] = lam[a] * lam_r;
     double chi5p = chi[4] > 0.0 ? chi[4] : 0.0;
@@ -547,11 +550,11 @@ static void dual_energy_fix(const ctx_t *c, double *U, orc_stats *st)
     double ethe = U[4] - ekin;
     double rg = pow(U[0], c->gm1);
     if (ethe < c->o.de_xi * ekin) {
-        double P = U[5] * rg;
+        double P = U[c->nv - 1] * rg;
         U[4] = ekin + P / c->gm1;
         st->n_dual_fix++;
     } else {
-        U[5] = c->gm1 * ethe / rg;
+        U[c->nv - 1] = c->gm1 * ethe / rg;
     }
 }
 
@@ -568,10 +571,24 @@ static void floor_cons(const ctx_t *c, double *U, orc_stats *st)
     if (pt > pf) pf = pt;
     if (pf > 0.0 && P < pf) {
         U[4] = ekin + pf / c->gm1;
-        if (c->o.dual_energy) U[5] = pf / pow(U[0], c->gm1);
+        if (c->o.dual_energy) U[c->nv - 1] = pf / pow(U[0], c->gm1);
         touched = 1;
     }
     st->n_floor += touched;
+}
+
+/* L96: "an arbitrary number of chemical species, which can be renormalized after every update to ensure that the sum
+ * of their mass fractions equals unity": s_k <- s_k * rho / sum_k s_k over the passive scalars -- all of them, except the
+ * last one when it is the entropy of the dual-energy formalism (reading R27).  A non-positive sum is left alone. */
+static void renormalize_scalars(const ctx_t *c, double *U)
+{
+    if (!c->o.renormalize) return;
+    int last = c->nv - (c->o.dual_energy ? 1 : 0);
+    double sum = 0.0;
+    for (int v = 5; v < last; ++v) sum = sum + U[v];
+    if (!(sum > 0.0)) return;
+    double f = U[0] / sum;
+    for (int v = 5; v < last; ++v) U[v] = U[v] * f;
 }
 
 /* O9: CFL signal speed of one cell (Eq. 1 for CTU, Eq. 2 for MHM; L158-168) */
@@ -644,7 +661,7 @@ static void gather_face_values(const ctx_t *c, int recon, const double *W, int n
             Wr[m + 2][2] = q[(size_t)c1 * NPC];
             Wr[m + 2][3] = q[(size_t)c2 * NPC];
             Wr[m + 2][4] = q[(size_t)4 * NPC];
-            if (nv > 5) Wr[m + 2][5] = q[(size_t)5 * NPC];
+            for (int v = 5; v < nv; ++v) Wr[m + 2][v] = q[(size_t)v * NPC];
         }
         if (recon == RECON_PLM) {
             char_slope(c, Wr[1], Wr[2], Wr[3], sl[1]);
@@ -673,7 +690,7 @@ static void gather_face_values(const ctx_t *c, int recon, const double *W, int n
         /* back to the natural component order */
         wm[0] = rm[0]; wm[cn] = rm[1]; wm[c1] = rm[2]; wm[c2] = rm[3]; wm[4] = rm[4];
         wp[0] = rp[0]; wp[cn] = rp[1]; wp[c1] = rp[2]; wp[c2] = rp[3]; wp[4] = rp[4];
-        if (nv > 5) { wm[5] = rm[5]; wp[5] = rp[5]; }
+        for (int v = 5; v < nv; ++v) { wm[v] = rm[v]; wp[v] = rp[v]; }
         return;
     }
     for (int v = 0; v < nv; ++v) {
@@ -738,7 +755,8 @@ static void ctu_trace_cell(const ctx_t *c, int recon, double lam_r, const work_t
         gather_face_values(c, recon, wk->W, n, d, wm, wp);
         /* rotate so that the traced axis is "n" */
         double Wr[NVMAX], rm[NVMAX], rp[NVMAX], tm[NVMAX], tp[NVMAX];
-        int map[NVMAX] = {0, in_, it1, it2, 4, 5};
+        int map[NVMAX] = {0, in_, it1, it2, 4};
+        for (int v = 5; v < nv; ++v) map[v] = v;
         for (int v = 0; v < nv; ++v) {
             Wr[v] = Wc[map[v]];
             rm[v] = wm[map[v]];
@@ -959,6 +977,7 @@ static void advance_group(const ctx_t *c, int scheme, int recon, int solver, dou
                     dual_energy_fix(c, U, st);
                 }
                 if (floors_set(c)) floor_cons(c, U, st);
+                renormalize_scalars(c, U);
                 if (!is_physical(c, U)) st->n_unphysical++;
                 for (int v = 0; v < nv; ++v) out[(((size_t)v * PS + k) * PS + j) * PS + i] = U[v];
                 double s = signal_speed(c, scheme, U);
@@ -1016,8 +1035,8 @@ int oracle_fluid_advance(const double *in, double *out, double *flux_out, double
     if (riemann_solver < RSOLVER_ROE || riemann_solver > RSOLVER_EXACT) return -1;
     ctx_t c;
     make_ctx(&c, gamma, recon, opts);
-    if (c.o.n_scalar < 0 || c.o.n_scalar > 1) return -1;
-    if (c.o.dual_energy && c.o.n_scalar != 1) return -1;
+    if (c.o.n_scalar < 0 || c.o.n_scalar > NSMAX) return -1;
+    if (c.o.dual_energy && c.o.n_scalar < 1) return -1;
     const int nv = c.nv;
     orc_stats tot;
     memset(&tot, 0, sizeof(tot));
@@ -1178,6 +1197,7 @@ int oracle_close_cell(double *U, double gamma, const orc_opts *opts, orc_stats *
     memset(&st, 0, sizeof(st));
     dual_energy_fix(&c, U, &st);
     if (floors_set(&c)) floor_cons(&c, U, &st);
+    renormalize_scalars(&c, U);
     if (st_out) *st_out = st;
     return is_physical(&c, U);
 }
