@@ -24,7 +24,9 @@
  *             Values are the time-centred flux densities F_d, not multiplied by dt or area.
  *   group_speed_out [n_groups]   max over the 16^3 UPDATED cells of |vx|+|vy|+|vz|+3c (MHM and VL, Eq. 2)
  *                                or max(|vx|,|vy|,|vz|)+c (CTU, Eq. 1)
- *   NVAR = 5 + n_scalar (n_scalar = 1 carries the entropy s = P/rho^(gamma-1) of L100).
+ *   NVAR = 5 + n_scalar: conserved passive scalars s_k (chemical species as partial densities, L96) follow E; each
+ *   is reconstructed as q_k = s_k / rho and rides the mass flux, upwinded.  With dual_energy the last one carries the
+ *   entropy s = P/rho^(gamma-1) of L100.
  * Ownership: every pointer is a DEVICE pointer owned by the caller, 16-byte aligned and
  * non-overlapping, unless the name ends in _host.  The library keeps no state between calls.
  */
@@ -47,6 +49,7 @@ enum { GAMER_PLM = 1, GAMER_PPM = 2 };                      /* recon    (L94)   
 enum { GAMER_ROE = 1, GAMER_HLLC = 2, GAMER_HLLE = 3,
        GAMER_EXACT = 4 };   /* riemann (L94); EXACT = Toro (2009) ch. 4, iterative: Newton on the pressure function
                                from the two-rarefaction guess, vacuum-generating data handled by HLLE */
+#define GAMER_MAX_SCALARS 4   /* passive scalars the kernels are built for (the paper: "an arbitrary number", L96) */
 enum { GAMER_FP32 = 4, GAMER_FP64 = 8 };                    /* precision = sizeof(real), L244 */
 enum { GAMER_LIMITER_GMINMOD = 1, GAMER_LIMITER_VANLEER = 2, GAMER_LIMITER_VANALBADA = 3 }; /* L94 */
 
@@ -64,8 +67,8 @@ typedef struct gamer_opts {
     void*    stream;              /* cudaStream_t; NULL = default stream                            */
     int      limiter;             /* GAMER_LIMITER_*; 0 = generalized minmod                        */
     double   minmod_theta;        /* <= 0: 1 for PLM (plain minmod), 2 for PPM (Colella-Woodward)   */
-    int      n_scalar;            /* 0 | 1                                                          */
-    int      dual_energy;         /* 0 | 1 (needs n_scalar = 1): L100                               */
+    int      n_scalar;            /* 0 .. GAMER_MAX_SCALARS passively advected scalars (L96)        */
+    int      dual_energy;         /* 0 | 1 (needs n_scalar >= 1; the LAST scalar is the entropy): L100 */
     double   de_xi;               /* switch E_the/E_kin < xi; <= 0: 1e-2                            */
     double   min_dens, min_pres, min_temp;   /* floors, 0 = off; temperature = P/rho (L504)         */
     int      remedy_first_order;  /* 1: remedy (ii) of L105 on cells that come out unphysical       */
@@ -77,6 +80,9 @@ typedef struct gamer_opts {
                                      reverted predictor states, remedy (ii) cells, dual-energy fixes} */
     int      char_limiting;       /* 1: slopes limited in characteristic variables (L94): R . limiter(L dW-, L dW+)
                                      with the eigenvectors of the cell; 0: in primitive variables (default)    */
+    int      renormalize;         /* 1: after every update rescale the passive scalars so that they sum to rho, i.e. the
+                                     mass fractions to unity (L96): s_k <- s_k rho / sum_k s_k over all scalars except the
+                                     entropy of the dual-energy formalism; a cell whose sum is not positive is left alone   */
 } gamer_opts;
 
 /* One step for n_groups patch groups.  flux_out may be NULL.  n_groups == 0 is a successful no-op.

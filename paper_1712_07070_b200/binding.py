@@ -44,6 +44,7 @@ class gamer_opts(ctypes.Structure):
         ("n_unphysical_out", ctypes.c_void_p),
         ("diag_out", ctypes.c_void_p),
         ("char_limiting", ctypes.c_int),
+        ("renormalize", ctypes.c_int),
     ]
 
 
@@ -122,7 +123,7 @@ def _stream_handle(stream=None):
 
 def make_opts(stream=None, limiter=0, minmod_theta=0.0, n_scalar=0, dual_energy=False, de_xi=0.0, min_dens=0.0,
               min_pres=0.0, min_temp=0.0, remedy_first_order=False, dt_dev=None, group_speed_out=None,
-              n_unphysical_out=None, diag_out=None, on_device=True, char_limiting=False):
+              n_unphysical_out=None, diag_out=None, on_device=True, char_limiting=False, renormalize=False):
     o = gamer_opts()
     o.stream = _stream_handle(stream) if on_device else None
     o.limiter, o.minmod_theta, o.n_scalar = int(limiter), float(minmod_theta), int(n_scalar)
@@ -134,6 +135,7 @@ def make_opts(stream=None, limiter=0, minmod_theta=0.0, n_scalar=0, dual_energy=
     o.n_unphysical_out = _ptr(n_unphysical_out)
     o.diag_out = _ptr(diag_out)
     o.char_limiting = int(bool(char_limiting))
+    o.renormalize = int(bool(renormalize))
     return o
 
 

@@ -66,13 +66,14 @@ static int advance_typed(const void* in, void* out, void* flux_out, int64_t n_gr
         if (o->de_xi > 0.0) a.xi = o->de_xi;
         a.min_dens = o->min_dens; a.min_pres = o->min_pres; a.min_temp = o->min_temp;
         a.dual = o->dual_energy; a.remedy2 = o->remedy_first_order; a.char_limit = o->char_limiting ? 1 : 0;
+        a.renorm = (o->renormalize && o->n_scalar - (o->dual_energy ? 1 : 0) > 0) ? 1 : 0;
         a.dt_dev = o->dt_dev;
         a.speed = static_cast<T*>(o->group_speed_out);
         a.n_unphys = o->n_unphysical_out;
         a.diag = o->diag_out;
         nsc = o->n_scalar;
         const bool custom_theta = a.theta != (recon == GAMER_PPM ? 2.0 : 1.0);   // fast kernels fix theta at compile time
-        ext = (nsc || a.dual || a.remedy2 || a.limiter != LIM_GMINMOD || custom_theta || a.char_limit || a.min_dens > 0 || a.min_pres > 0 ||
+        ext = (nsc || a.renorm || a.dual || a.remedy2 || a.limiter != LIM_GMINMOD || custom_theta || a.char_limit || a.min_dens > 0 || a.min_pres > 0 ||
                a.min_temp > 0 || a.n_unphys || a.diag) ? 1 : 0;
     }
     if (a.n_unphys && cudaMemsetAsync(a.n_unphys, 0, sizeof(int), st) != cudaSuccess) return GAMER_ECUDA;
@@ -82,6 +83,7 @@ static int advance_typed(const void* in, void* out, void* flux_out, int64_t n_gr
     int launches = 0;
     const cudaError_t e = TABLE[scheme - 1][recon - 1][riemann - 1](sizeof(T), nsc, ext, &a, st, &launches);
     g_launches += launches;
+    if (e == cudaErrorNotSupported) return GAMER_EUNSUPPORTED;      // combination not built (e.g. a tile that cannot fit)
     return e == cudaSuccess ? GAMER_OK : GAMER_ECUDA;
 }
 
@@ -94,8 +96,8 @@ extern "C" int gamer_fluid_advance_ex(const void* in, void* out, void* flux_out,
     if (!dev_dt && (!(dt > 0.0) || !std::isfinite(dt))) return GAMER_EINVAL;
     if (flux_out && !aligned16(flux_out)) return GAMER_EINVAL;
     if (opts) {
-        if (opts->n_scalar < 0 || opts->n_scalar > 1) return GAMER_EINVAL;
-        if (opts->dual_energy && opts->n_scalar != 1) return GAMER_EINVAL;
+        if (opts->n_scalar < 0 || opts->n_scalar > GAMER_MAX_SCALARS) return GAMER_EINVAL;
+        if (opts->dual_energy && opts->n_scalar < 1) return GAMER_EINVAL;      // the entropy is the last scalar
         if (opts->limiter < 0 || opts->limiter > GAMER_LIMITER_VANALBADA) return GAMER_EINVAL;
         if (opts->min_dens < 0 || opts->min_pres < 0 || opts->min_temp < 0) return GAMER_EINVAL;
     }
@@ -148,8 +150,8 @@ extern "C" int gamer_fluid_advance_resident(const void* u, const int32_t* nbr, v
     if (!dev_dt && (!(dt > 0.0) || !std::isfinite(dt))) return GAMER_EINVAL;
     if (flux_out && !aligned16(flux_out)) return GAMER_EINVAL;
     if (opts) {
-        if (opts->n_scalar < 0 || opts->n_scalar > 1) return GAMER_EINVAL;
-        if (opts->dual_energy && opts->n_scalar != 1) return GAMER_EINVAL;
+        if (opts->n_scalar < 0 || opts->n_scalar > GAMER_MAX_SCALARS) return GAMER_EINVAL;
+        if (opts->dual_energy && opts->n_scalar < 1) return GAMER_EINVAL;      // the entropy is the last scalar
         if (opts->limiter < 0 || opts->limiter > GAMER_LIMITER_VANALBADA) return GAMER_EINVAL;
         if (opts->min_dens < 0 || opts->min_pres < 0 || opts->min_temp < 0) return GAMER_EINVAL;
         if (opts->remedy_first_order) return GAMER_EUNSUPPORTED;   // remedy (ii) re-reads the padded slab
@@ -182,14 +184,14 @@ static int cfl_typed(const void* u, int64_t n_groups, double dh, double gamma, d
     a.gamma = gamma;
     a.min_dens = o ? o->min_dens : 0.0; a.min_pres = o ? o->min_pres : 0.0; a.min_temp = o ? o->min_temp : 0.0;
     a.n_groups = n_groups;
-    const int nsc = o ? o->n_scalar : 0;
+    a.nvar = 5 + (o ? o->n_scalar : 0);
     if (cudaMemsetAsync(dt_out, 0, sizeof(double), st) != cudaSuccess) return GAMER_ECUDA;
     if (n_groups > 0) {
         const unsigned grid = (unsigned)n_groups;
         if (scheme != GAMER_CTU) {      // Eq. (2): MHM and VL (L168)
-            if (nsc) cfl_kernel<T, 6, MHM><<<grid, 256, 0, st>>>(a); else cfl_kernel<T, 5, MHM><<<grid, 256, 0, st>>>(a);
+            cfl_kernel<T, MHM><<<grid, 256, 0, st>>>(a);
         } else {
-            if (nsc) cfl_kernel<T, 6, CTU><<<grid, 256, 0, st>>>(a); else cfl_kernel<T, 5, CTU><<<grid, 256, 0, st>>>(a);
+            cfl_kernel<T, CTU><<<grid, 256, 0, st>>>(a);
         }
         g_launches += 1;
     }
@@ -204,7 +206,7 @@ extern "C" int gamer_cfl_dt_ex(const void* u, int64_t n_groups, double dh, doubl
     if (scheme != GAMER_MHM && scheme != GAMER_CTU && scheme != GAMER_VL) return GAMER_EINVAL;
     if (precision != GAMER_FP32 && precision != GAMER_FP64) return GAMER_EINVAL;
     if (!aligned16(u)) return GAMER_EINVAL;
-    if (opts && (opts->n_scalar < 0 || opts->n_scalar > 1)) return GAMER_EINVAL;
+    if (opts && (opts->n_scalar < 0 || opts->n_scalar > GAMER_MAX_SCALARS)) return GAMER_EINVAL;
     if (n_groups > 0x7fffffff) return GAMER_EUNSUPPORTED;
     return precision == GAMER_FP32 ? cfl_typed<float>(u, n_groups, dh, gamma, cfl, scheme, group_speed_out, dt_out, opts)
                                    : cfl_typed<double>(u, n_groups, dh, gamma, cfl, scheme, group_speed_out, dt_out, opts);
@@ -237,7 +239,7 @@ extern "C" int gamer_cfl_from_group_speed(const void* group_speed, int64_t n_gro
 // ------------------------------------------------------------------------------------------ ghost refresh
 extern "C" int gamer_refresh_ghosts_periodic(const void* u, void* in, int gz, int gy, int gx, int nvar, int precision,
                                              void* stream) {
-    if (!u || !in || gz < 1 || gy < 1 || gx < 1 || nvar < 5 || nvar > 6) return GAMER_EINVAL;
+    if (!u || !in || gz < 1 || gy < 1 || gx < 1 || nvar < 5 || nvar > 5 + GAMER_MAX_SCALARS) return GAMER_EINVAL;
     if (precision != GAMER_FP32 && precision != GAMER_FP64) return GAMER_EINVAL;
     const long long ng = (long long)gz * gy * gx;
     if (ng * nvar > 0x7fffffff) return GAMER_EUNSUPPORTED;
@@ -253,7 +255,7 @@ extern "C" int gamer_refresh_ghosts_periodic(const void* u, void* in, int gz, in
 
 extern "C" int gamer_refresh_ghosts(const void* u, void* in, int gz, int gy, int gx, int nvar, const int* bc,
                                     int precision, void* stream) {
-    if (!u || !in || !bc || gz < 1 || gy < 1 || gx < 1 || nvar < 5 || nvar > 6) return GAMER_EINVAL;
+    if (!u || !in || !bc || gz < 1 || gy < 1 || gx < 1 || nvar < 5 || nvar > 5 + GAMER_MAX_SCALARS) return GAMER_EINVAL;
     if (precision != GAMER_FP32 && precision != GAMER_FP64) return GAMER_EINVAL;
     BcSet b;
     for (int i = 0; i < 6; ++i) {
@@ -276,7 +278,7 @@ extern "C" int gamer_refresh_ghosts(const void* u, void* in, int gz, int gy, int
 
 extern "C" int gamer_refresh_ghosts_table(const void* u, void* in, const int32_t* nbr, int64_t n_groups, int nvar,
                                           int precision, void* stream) {
-    if (n_groups < 0 || nvar < 5 || nvar > 6 || (precision != GAMER_FP32 && precision != GAMER_FP64)) return GAMER_EINVAL;
+    if (n_groups < 0 || nvar < 5 || nvar > 5 + GAMER_MAX_SCALARS || (precision != GAMER_FP32 && precision != GAMER_FP64)) return GAMER_EINVAL;
     if (n_groups > 0 && (!u || !in || !nbr)) return GAMER_EINVAL;
     if (n_groups == 0) return GAMER_OK;
     if (n_groups * nvar > 0x7fffffff) return GAMER_EUNSUPPORTED;
@@ -308,7 +310,7 @@ static void launch_interp(const void* c0, const void* c1, double w, void* fine, 
 extern "C" int gamer_interpolate_ghosts(const void* coarse_in, const void* coarse_in_new, double w, void* fine_in,
                                         const int32_t* parent, const int32_t* nbr, int64_t n_fine, int nvar,
                                         int monotonic, int precision, void* stream) {
-    if (n_fine < 0 || nvar < 1 || nvar > 6 || (precision != GAMER_FP32 && precision != GAMER_FP64)) return GAMER_EINVAL;
+    if (n_fine < 0 || nvar < 1 || nvar > 5 + GAMER_MAX_SCALARS || (precision != GAMER_FP32 && precision != GAMER_FP64)) return GAMER_EINVAL;
     if (coarse_in_new && (!std::isfinite(w) || w < 0.0 || w > 1.0)) return GAMER_EINVAL;
     if (n_fine > 0 && (!coarse_in || !fine_in || !parent || !nbr || coarse_in == fine_in)) return GAMER_EINVAL;
     if (n_fine == 0) return GAMER_OK;
@@ -344,7 +346,7 @@ extern "C" int gamer_poisson_sor(void* phi, const void* rho, void* acc, void* re
 
 extern "C" int gamer_restrict(const void* fine, void* coarse, const int32_t* parent, int64_t n_fine, int nvar,
                               int precision, void* stream) {
-    if (n_fine < 0 || nvar < 1 || nvar > 6 || (precision != GAMER_FP32 && precision != GAMER_FP64)) return GAMER_EINVAL;
+    if (n_fine < 0 || nvar < 1 || nvar > 5 + GAMER_MAX_SCALARS || (precision != GAMER_FP32 && precision != GAMER_FP64)) return GAMER_EINVAL;
     if (n_fine > 0 && (!fine || !coarse || !parent)) return GAMER_EINVAL;
     if (n_fine == 0) return GAMER_OK;
     if (n_fine * nvar > 0x7fffffff) return GAMER_EUNSUPPORTED;
@@ -358,7 +360,7 @@ extern "C" int gamer_restrict(const void* fine, void* coarse, const int32_t* par
 
 extern "C" int gamer_flux_accumulate(void* acc, const void* flux, double weight, int64_t n_groups, int nvar, int init,
                                      int precision, void* stream) {
-    if (n_groups < 0 || nvar < 1 || nvar > 6 || (precision != GAMER_FP32 && precision != GAMER_FP64)) return GAMER_EINVAL;
+    if (n_groups < 0 || nvar < 1 || nvar > 5 + GAMER_MAX_SCALARS || (precision != GAMER_FP32 && precision != GAMER_FP64)) return GAMER_EINVAL;
     if (n_groups > 0 && (!acc || !flux)) return GAMER_EINVAL;
     if (!std::isfinite(weight)) return GAMER_EINVAL;
     if (n_groups == 0) return GAMER_OK;
@@ -373,7 +375,7 @@ extern "C" int gamer_flux_accumulate(void* acc, const void* flux, double weight,
 
 extern "C" int gamer_flux_correct(void* coarse, const void* coarse_flux, const void* fine_flux_avg, const int32_t* table,
                                   int64_t n_entries, int nvar, double lam, int precision, void* stream) {
-    if (n_entries < 0 || nvar < 1 || nvar > 6 || (precision != GAMER_FP32 && precision != GAMER_FP64)) return GAMER_EINVAL;
+    if (n_entries < 0 || nvar < 1 || nvar > 5 + GAMER_MAX_SCALARS || (precision != GAMER_FP32 && precision != GAMER_FP64)) return GAMER_EINVAL;
     if (n_entries > 0 && (!coarse || !coarse_flux || !fine_flux_avg || !table)) return GAMER_EINVAL;
     if (!std::isfinite(lam)) return GAMER_EINVAL;
     if (n_entries == 0) return GAMER_OK;

@@ -17,10 +17,11 @@ template <typename T> struct CflArgs {
     double* acc;     // device double holding the running max (bits), zeroed before the launch
     double gamma, min_dens, min_pres, min_temp;
     long long n_groups;
+    int nvar;        // variables per cell in u (5 + passive scalars); only the first five enter the signal speed
 };
 
 // one CTA per patch group, 256 threads, 16 cells per thread, 16-byte loads
-template <typename T, int NV, int SCHEME>
+template <typename T, int SCHEME>
 __global__ void __launch_bounds__(256) cfl_kernel(const CflArgs<T> a) {
     constexpr int NC = PS * PS * PS;
     constexpr int VEC = 16 / sizeof(T);
@@ -29,7 +30,8 @@ __global__ void __launch_bounds__(256) cfl_kernel(const CflArgs<T> a) {
     ph.min_dens = T(a.min_dens); ph.min_pres = T(a.min_pres); ph.min_temp = T(a.min_temp);
     ph.floors = (a.min_dens > 0.0 || a.min_pres > 0.0 || a.min_temp > 0.0) ? 1 : 0;
     const long long g = blockIdx.x;
-    const T* base = a.u + (size_t)g * NV * NC;
+    constexpr int NV = 5;
+    const T* base = a.u + (size_t)g * a.nvar * NC;
     T smax = T(0);
     for (int c = threadIdx.x * VEC; c < NC; c += 256 * VEC) {
         T U[NV][VEC];

@@ -107,7 +107,8 @@ __device__ __forceinline__ int ctu_final_pass(const T* es, const T* zprev, T* fx
             q[(size_t)c1 * (PS * PS)] = F[2];
             q[(size_t)c2 * (PS * PS)] = F[3];
             q[(size_t)4 * (PS * PS)] = F[4];
-            if (NV > 5) q[(size_t)(NV - 1) * (PS * PS)] = F[NV - 1];
+#pragma unroll
+            for (int v = 5; v < NV; ++v) q[(size_t)v * (PS * PS)] = F[v];
         }
     }
     return nfb;
@@ -184,7 +185,8 @@ __device__ __forceinline__ int ctu_riemann_phase(const T* tcur, const T* tprev, 
             q[(size_t)c1 * (PS * PS)] = F[2];
             q[(size_t)c2 * (PS * PS)] = F[3];
             q[(size_t)4 * (PS * PS)] = F[4];
-            if (NV > 5) q[(size_t)(NV - 1) * (PS * PS)] = F[NV - 1];
+#pragma unroll
+            for (int v = 5; v < NV; ++v) q[(size_t)v * (PS * PS)] = F[v];
         }
     }
     return nfb;
@@ -208,7 +210,8 @@ __device__ __forceinline__ void ctu_trace_dir(const T* const* Pz, int t, T* tcur
             const T* q = (D == 2) ? Pz[R + m] + c : Pz[R] + c + m * (D == 0 ? 1 : NP);
             W5[m + 2][0] = q[0]; W5[m + 2][1] = q[cn * G::PLN]; W5[m + 2][2] = q[c1 * G::PLN]; W5[m + 2][3] = q[c2 * G::PLN];
             W5[m + 2][4] = q[4 * G::PLN];
-            if (NV > 5) W5[m + 2][NV - 1] = q[(NV - 1) * G::PLN];
+#pragma unroll
+            for (int v = 5; v < NV; ++v) W5[m + 2][v] = q[v * G::PLN];
         }
 #pragma unroll
         for (int k = 0; k < NV; ++k) Wr[k] = W5[2][k];
@@ -233,7 +236,8 @@ __device__ __forceinline__ void ctu_trace_dir(const T* const* Pz, int t, T* tcur
         Wr[0] = Wc[0]; Wr[1] = Wc[cn]; Wr[2] = Wc[c1]; Wr[3] = Wc[c2]; Wr[4] = Wc[4];
         rm[0] = wm[0]; rm[1] = wm[cn]; rm[2] = wm[c1]; rm[3] = wm[c2]; rm[4] = wm[4];
         rp[0] = wp[0]; rp[1] = wp[cn]; rp[2] = wp[c1]; rp[3] = wp[c2]; rp[4] = wp[4];
-        if (NV > 5) { Wr[NV - 1] = Wc[NV - 1]; rm[NV - 1] = wm[NV - 1]; rp[NV - 1] = wp[NV - 1]; }
+#pragma unroll
+        for (int v = 5; v < NV; ++v) { Wr[v] = Wc[v]; rm[v] = wm[v]; rp[v] = wp[v]; }
     }
     trace_cell<T, RECON, NV>(Wr, rm, rp, tm, tp, ph);
     if (EXT && ph.floors) { floor_prim(tm, ph); floor_prim(tp, ph); }

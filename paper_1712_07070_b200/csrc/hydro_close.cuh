@@ -43,6 +43,23 @@ __device__ __forceinline__ void floor_cons(T* U, const Phys<T>& ph) {
     }
 }
 
+// L96: the passive scalars (all but the entropy of the dual-energy formalism, which is the last one) rescaled so that they
+// sum to rho; a non-positive sum is left alone (DESIGN R27)
+template <typename T, int NV>
+__device__ __forceinline__ void renormalize_scalars(T* U, const Phys<T>& ph) {
+    if (NV < 6 || !ph.renorm) return;
+    const int last = NV - (ph.dual ? 1 : 0);
+    T sum = T(0);
+#pragma unroll
+    for (int v = 5; v < NV; ++v)
+        if (v < last) sum = sum + U[v];
+    if (!(sum > T(0))) return;
+    const T f = U[0] / sum;
+#pragma unroll
+    for (int v = 5; v < NV; ++v)
+        if (v < last) U[v] = U[v] * f;
+}
+
 template <typename T, int NV, int SCHEME, bool EXT>
 __device__ __forceinline__ T signal_speed(const T* U, const Phys<T>& ph) {
     T W[NV];
@@ -68,7 +85,8 @@ __device__ __noinline__ void first_order_cell(const T* gin, T* Unew, int* nfb, c
         const int cn = 1 + d, c1 = 1 + (d + 1) % 3, c2 = 1 + (d + 2) % 3;
         T Wr[NV] ;
         Wr[0] = Wc[0]; Wr[1] = Wc[cn]; Wr[2] = Wc[c1]; Wr[3] = Wc[c2]; Wr[4] = Wc[4];
-        if (NV > 5) Wr[NV - 1] = Wc[NV - 1];
+#pragma unroll
+        for (int v = 5; v < NV; ++v) Wr[v] = Wc[v];
         T Fd[NV];
 #pragma unroll
         for (int v = 0; v < NV; ++v) Fd[v] = T(0);
@@ -80,7 +98,8 @@ __device__ __noinline__ void first_order_cell(const T* gin, T* Unew, int* nfb, c
             for (int v = 0; v < NV; ++v) Un[v] = gin[(size_t)v * NPC + off];
             cons2prim<T, NV>(Un, Wn, ph);
             Wq[0] = Wn[0]; Wq[1] = Wn[cn]; Wq[2] = Wn[c1]; Wq[3] = Wn[c2]; Wq[4] = Wn[4];
-            if (NV > 5) Wq[NV - 1] = Wn[NV - 1];
+#pragma unroll
+            for (int v = 5; v < NV; ++v) Wq[v] = Wn[v];
             const bool fb = s ? riemann_flux<T, SOLVER, NV>(Wr, Wq, F, ph) : riemann_flux<T, SOLVER, NV>(Wq, Wr, F, ph);
             *nfb += fb ? 1 : 0;
             const T sg = s ? T(1) : T(-1);
@@ -89,7 +108,8 @@ __device__ __noinline__ void first_order_cell(const T* gin, T* Unew, int* nfb, c
             Fd[c1] += sg * F[2];
             Fd[c2] += sg * F[3];
             Fd[4] += sg * F[4];
-            if (NV > 5) Fd[NV - 1] += sg * F[NV - 1];
+#pragma unroll
+            for (int v = 5; v < NV; ++v) Fd[v] += sg * F[v];
         }
 #pragma unroll
         for (int v = 0; v < NV; ++v) acc[v] += Fd[v];
@@ -113,6 +133,7 @@ __device__ __forceinline__ void close_cell(T* U, const T* gin_cell, Counters& cn
         cnt.dual_fix += dual_energy_fix<T, NV>(U, ph);
     }
     if (ph.floors) floor_cons<T, NV>(U, ph);
+    renormalize_scalars<T, NV>(U, ph);
     if (!is_physical<T, NV>(U)) cnt.unphys++;
 }
 

@@ -77,7 +77,7 @@ template <typename T> struct Phys {
     int limiter;    // LIM_*
     // extended mode only
     T xi, min_dens, min_pres, min_temp;
-    int floors, dual, remedy2, char_limit;
+    int floors, dual, remedy2, char_limit, renorm;
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -92,7 +92,8 @@ __device__ __forceinline__ void cons2prim(const T* U, T* W, const Phys<T>& ph) {
     W[3] = U[3] * ir;
     const T ek = T(0.5) * (U[1] * W[1] + U[2] * W[2] + U[3] * W[3]);
     W[4] = ph.gm1 * (U[4] - ek);
-    if (NV > 5) W[NV - 1] = U[NV - 1] * ir;
+#pragma unroll
+    for (int v = 5; v < NV; ++v) W[v] = U[v] * ir;      // passive scalars: q_k = s_k / rho (L96)
 }
 
 template <typename T, int NV>
@@ -102,7 +103,8 @@ __device__ __forceinline__ void prim2cons(const T* W, T* U, const Phys<T>& ph) {
     U[2] = W[0] * W[2];
     U[3] = W[0] * W[3];
     U[4] = W[4] * ph.inv_gm1 + T(0.5) * (U[1] * W[1] + U[2] * W[2] + U[3] * W[3]);
-    if (NV > 5) U[NV - 1] = W[0] * W[NV - 1];
+#pragma unroll
+    for (int v = 5; v < NV; ++v) U[v] = W[0] * W[v];
 }
 
 template <typename T>
@@ -183,13 +185,15 @@ __device__ __forceinline__ void char_slope(const T* Wl, const T* Wc, const T* Wr
         const T d0 = Wc[0] - Wl[0], d1 = Wc[1] - Wl[1], d4 = Wc[4] - Wl[4];
         aL[0] = (d4 - rho * cs * d1) / (T(2) * c2); aL[1] = d0 - d4 / c2; aL[2] = Wc[2] - Wl[2]; aL[3] = Wc[3] - Wl[3];
         aL[4] = (d4 + rho * cs * d1) / (T(2) * c2);
-        if (NV > 5) aL[NV - 1] = Wc[NV - 1] - Wl[NV - 1];
+#pragma unroll
+        for (int v = 5; v < NV; ++v) aL[v] = Wc[v] - Wl[v];
     }
     {
         const T d0 = Wr[0] - Wc[0], d1 = Wr[1] - Wc[1], d4 = Wr[4] - Wc[4];
         aR[0] = (d4 - rho * cs * d1) / (T(2) * c2); aR[1] = d0 - d4 / c2; aR[2] = Wr[2] - Wc[2]; aR[3] = Wr[3] - Wc[3];
         aR[4] = (d4 + rho * cs * d1) / (T(2) * c2);
-        if (NV > 5) aR[NV - 1] = Wr[NV - 1] - Wc[NV - 1];
+#pragma unroll
+        for (int v = 5; v < NV; ++v) aR[v] = Wr[v] - Wc[v];
     }
     T s[NV];
 #pragma unroll
@@ -199,7 +203,8 @@ __device__ __forceinline__ void char_slope(const T* Wl, const T* Wc, const T* Wr
     slope[2] = s[2];
     slope[3] = s[3];
     slope[4] = s[0] * cs * cs + s[4] * cs * cs;
-    if (NV > 5) slope[NV - 1] = s[NV - 1];
+#pragma unroll
+    for (int v = 5; v < NV; ++v) slope[v] = s[v];
 }
 
 // face values of cell j from the rotated primitive states Wr[0..4] = cells j-2 .. j+2 (PLM reads 1..3 only)
@@ -240,7 +245,8 @@ __device__ __forceinline__ void phys_flux(const T* W, const T* U, T* F) {
     F[3] = U[3] * vn;
     F[1 + D] += W[4];
     F[4] = vn * (U[4] + W[4]);
-    if (NV > 5) F[NV - 1] = U[NV - 1] * vn;
+#pragma unroll
+    for (int v = 5; v < NV; ++v) F[v] = U[v] * vn;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -288,7 +294,8 @@ __device__ __forceinline__ void trace_cell(const T* W, const T* wm, const T* wp,
         tp[0] += vR - vP * ic2;
         tp[2] += A * (d[2] - w6[2]) + B * w6[2];
         tp[3] += A * (d[3] - w6[3]) + B * w6[3];
-        if (NV > 5) tp[NV - 1] += A * (d[NV - 1] - w6[NV - 1]) + B * w6[NV - 1];
+#pragma unroll
+        for (int v = 5; v < NV; ++v) tp[v] += A * (d[v] - w6[v]) + B * w6[v];
     }
     // ---- minus face: waves with lambda < 0
     if (l5 < T(0)) {
@@ -307,7 +314,8 @@ __device__ __forceinline__ void trace_cell(const T* W, const T* wm, const T* wp,
         tm[0] += vR - vP * ic2;
         tm[2] += C * (d[2] + w6[2]) + D * w6[2];
         tm[3] += C * (d[3] + w6[3]) + D * w6[3];
-        if (NV > 5) tm[NV - 1] += C * (d[NV - 1] + w6[NV - 1]) + D * w6[NV - 1];
+#pragma unroll
+        for (int v = 5; v < NV; ++v) tm[v] += C * (d[v] + w6[v]) + D * w6[v];
     }
 }
 

@@ -254,7 +254,12 @@ __device__ __forceinline__ bool riemann_flux_cons(const T* UL, const T* UR, T* F
     make_side_cons(UL, L, ph);
     make_side_cons(UR, R, ph);
     const bool fb = riemann_sides<T, SOLVER>(L, R, F, ph);
-    if (NV > 5) F[NV - 1] = F[0] >= T(0) ? F[0] * (UL[NV - 1] * Ops<T>::rcp(UL[0])) : F[0] * (UR[NV - 1] * Ops<T>::rcp(UR[0]));
+    if (NV > 5) {      // every passive scalar rides the mass flux, upwinded (R12)
+        const bool up = F[0] >= T(0);
+        const T fq = F[0] * Ops<T>::rcp(up ? UL[0] : UR[0]);
+#pragma unroll
+        for (int v = 5; v < NV; ++v) F[v] = fq * (up ? UL[v] : UR[v]);
+    }
     return fb;
 }
 
@@ -278,7 +283,8 @@ __device__ __forceinline__ bool riemann_flux(const T* WL, const T* WR, T* F, con
     } else {
         solve_hlle(L, R, r, F, ph);
     }
-    if (NV > 5) F[NV - 1] = F[0] >= T(0) ? F[0] * WL[NV - 1] : F[0] * WR[NV - 1];
+#pragma unroll
+    for (int v = 5; v < NV; ++v) F[v] = F[0] >= T(0) ? F[0] * WL[v] : F[0] * WR[v];
     return fb;
 }
 

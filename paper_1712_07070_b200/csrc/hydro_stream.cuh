@@ -27,7 +27,7 @@ template <typename T> struct AdvArgs {
     const double* dt_dev;
     const int* nbr;   // nullable: [n_groups][27] same-level neighbour table => `in` is the UNPADDED state (fused refresh)
     double dt, dh, gamma, theta, xi, min_dens, min_pres, min_temp;
-    int limiter, dual, remedy2, char_limit;
+    int limiter, dual, remedy2, char_limit, renorm;
     long long n_groups;
     Phys<T> ph;       // the run-time constants in the kernel's precision, filled on the host (fill_phys)
 };
@@ -53,6 +53,7 @@ inline void fill_phys(AdvArgs<T>& a) {
     ph.dual = a.dual;
     ph.remedy2 = a.remedy2;
     ph.char_limit = a.char_limit;
+    ph.renorm = a.renorm;
 }
 
 // device side: the host-filled constants; only dt/dh comes from memory when dt lives on the device

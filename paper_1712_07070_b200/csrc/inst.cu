@@ -27,14 +27,21 @@ static cudaError_t go(const void* args, cudaStream_t st, int* launches) {
 #endif
 }
 
-// prec = 4|8, nsc = 0|1, ext = 0|1 (nsc = 1 implies ext)
-cudaError_t G_NAME(int prec, int nsc, int ext, const void* args, cudaStream_t st, int* launches) {
-    if (prec == 4) {
-        if (nsc) return go<float, 6, true>(args, st, launches);
-        return ext ? go<float, 5, true>(args, st, launches) : go<float, 5, false>(args, st, launches);
+template <typename T>
+static cudaError_t by_scalars(int nsc, int ext, const void* args, cudaStream_t st, int* launches) {
+    switch (nsc) {
+    case 0: return ext ? go<T, 5, true>(args, st, launches) : go<T, 5, false>(args, st, launches);
+    case 1: return go<T, 6, true>(args, st, launches);
+    case 2: return go<T, 7, true>(args, st, launches);
+    case 3: return go<T, 8, true>(args, st, launches);
+    case 4: return go<T, 9, true>(args, st, launches);
+    default: return cudaErrorNotSupported;
     }
-    if (nsc) return go<double, 6, true>(args, st, launches);
-    return ext ? go<double, 5, true>(args, st, launches) : go<double, 5, false>(args, st, launches);
+}
+
+// prec = 4|8, nsc = 0..4 passive scalars, ext = 0|1 (nsc > 0 implies ext)
+cudaError_t G_NAME(int prec, int nsc, int ext, const void* args, cudaStream_t st, int* launches) {
+    return prec == 4 ? by_scalars<float>(nsc, ext, args, st, launches) : by_scalars<double>(nsc, ext, args, st, launches);
 }
 
 }  // namespace gamer

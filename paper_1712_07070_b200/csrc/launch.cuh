@@ -35,7 +35,10 @@ cudaError_t launch_mhm_f(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
     constexpr int NSTG = (!FUSED && C1 >= 2 && C2 < 2) ? 1 : 2;      // the fused gather is pipelined over two stages
 #endif
     using G = MhmGeo<T, RECON, NV, TY, NSTG, FUSED, VLS>;
-    static_assert(G::BYTES <= SMEM_LIMIT, "tile does not fit in shared memory");
+    if constexpr (G::BYTES > SMEM_LIMIT) {      // not even the 4-row tile fits (many scalars in fp64): not built
+        (void)a; (void)st; (void)launches;
+        return cudaErrorNotSupported;
+    } else {
     constexpr int MINB = ctas_by_smem(G::BYTES) >= 2 ? 2 : 1;
     auto kern = mhm_kernel<T, RECON, SOLVER, NV, EXT, TY, NSTG, MINB, FUSED, VLS>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::BYTES);
@@ -48,6 +51,7 @@ cudaError_t launch_mhm_f(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
     kern<<<(unsigned)grid, G::NT, G::BYTES, st>>>(a);
     *launches += 1;
     return cudaGetLastError();
+    }
 }
 
 // a.nbr set => `in` is the unpadded state and the ghost refresh is fused into the staging loads
@@ -72,7 +76,10 @@ cudaError_t launch_ctu_f(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
     constexpr int NT = CTU_NT_OVERRIDE > 0 ? CTU_NT_OVERRIDE : ((sizeof(T) == 8 ? 48 : 32) * TY < 128 ? 128 : (sizeof(T) == 8 ? 48 : 32) * TY);
     using G = Geo<TY>;
     using S = CtuSmem<T, RECON, NV, TY, FUSED>;
-    static_assert(S::BYTES <= SMEM_LIMIT, "tile does not fit in shared memory");
+    if constexpr (S::BYTES > SMEM_LIMIT) {      // not even the 4-row tile fits (many scalars in fp64): not built
+        (void)a; (void)st; (void)launches;
+        return cudaErrorNotSupported;
+    } else {
     auto kern = ctu_kernel<T, RECON, SOLVER, NV, EXT, TY, NT, FUSED>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::BYTES);
     if (e != cudaSuccess) return e;
@@ -84,6 +91,7 @@ cudaError_t launch_ctu_f(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
     kern<<<(unsigned)grid, NT, S::BYTES, st>>>(a);
     *launches += 1;
     return cudaGetLastError();
+    }
 }
 
 // a.nbr set => `in` is the unpadded state and the ghost refresh is fused into the staging loads

@@ -52,7 +52,8 @@ def test_argument_validation_needs_no_gpu(built_lib):
     assert L.gamer_fluid_advance(ok[0], ok[1], None, 1, float("nan"), 0.1, 1.4, 1, 1, 1, 4) == -1
     assert L.gamer_fluid_advance(ok[0], ok[1], None, 1, 0.1, -1.0, 1.4, 1, 1, 1, 4) == -1
     assert L.gamer_fluid_advance(ok[0], ok[1], None, 1, 0.1, 0.1, 1.0, 1, 1, 1, 4) == -1
-    assert L.gamer_fluid_advance(ok[0], ok[1], None, 1, 0.1, 0.1, 1.4, 3, 1, 1, 4) == -1
+    assert L.gamer_fluid_advance(ok[0], ok[1], None, 1, 0.1, 0.1, 1.4, 4, 1, 1, 4) == -1
+    assert L.gamer_fluid_advance(ok[0], ok[1], None, 1, 0.1, 0.1, 1.4, 3, 2, 1, 4) == -2      # VL + PPM: fourth ghost zone
     assert L.gamer_fluid_advance(ok[0], ok[1], None, 1, 0.1, 0.1, 1.4, 1, 0, 1, 4) == -1
     assert L.gamer_fluid_advance(ok[0], ok[1], None, 1, 0.1, 0.1, 1.4, 1, 1, 5, 4) == -1
     assert L.gamer_fluid_advance(ok[0], ok[1], None, 1, 0.1, 0.1, 1.4, 1, 1, 1, 2) == -1
@@ -74,7 +75,7 @@ def test_argument_validation_needs_no_gpu(built_lib):
     assert L.gamer_refresh_ghosts(ok[0], ok[1], 1, 1, 1, 5, None, 4, None) == -1
     L.gamer_restrict.argtypes = [vp, vp, vp, i64, ci, ci, vp]
     assert L.gamer_restrict(None, ok[1], vp(64), 1, 5, 4, None) == -1
-    assert L.gamer_restrict(ok[0], ok[1], vp(64), 1, 7, 4, None) == -1
+    assert L.gamer_restrict(ok[0], ok[1], vp(64), 1, 10, 4, None) == -1
     assert L.gamer_restrict(ok[0], ok[1], vp(64), 0, 5, 4, None) == 0
     L.gamer_flux_accumulate.argtypes = [vp, vp, dbl, i64, ci, ci, ci, vp]
     assert L.gamer_flux_accumulate(ok[0], None, 0.5, 1, 5, 1, 4, None) == -1
@@ -89,7 +90,7 @@ def test_argument_validation_needs_no_gpu(built_lib):
     interp = lambda c0=ok[0], c1=None, w=0.0, f=ok[1], par=vp(64), nb=vp(128), n=1, nv=5, prec=4: \
         L.gamer_interpolate_ghosts(c0, c1, w, f, par, nb, n, nv, 0, prec, None)
     assert interp(c0=None) == -1 and interp(f=None) == -1 and interp(par=None) == -1 and interp(nb=None) == -1
-    assert interp(nv=7) == -1 and interp(prec=2) == -1 and interp(n=-1) == -1
+    assert interp(nv=10) == -1 and interp(prec=2) == -1 and interp(n=-1) == -1
     assert interp(c1=vp(16384), w=1.5) == -1 and interp(c1=vp(16384), w=float("nan")) == -1
     assert interp(f=ok[0]) == -1                                # in place
     assert interp(n=0) == 0

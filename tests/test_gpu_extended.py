@@ -562,3 +562,47 @@ def test_poisson_sor_matches_oracle(dev, oracle_mod, dtype):
     assert torch.equal(phi2, phi)                                     # acc = NULL: same potential, bitwise (run to run too)
     empty = torch.empty((0, 18, 18, 18), dtype=dtype, device=dev)
     gb.gamer_poisson_sor(empty, torch.empty((0, 16, 16, 16), dtype=dtype, device=dev), None, dh, coeff, omega, 5)
+
+
+def _species_field(ns, n=32, seed=1712, entropy=False):
+    """Mach-1 turbulence + ns species s_k = X_k rho (smooth positive X_k summing to one) [+ the entropy as last scalar]"""
+    f = inputs.turbulence_field(n, seed, kmax=4, gamma=G53, entropy=entropy)
+    rho = f[0]
+    raw = [torch.exp(0.5 * inputs.random_field(rho.shape, seed + 31 * (k + 1), 4, "cpu")) for k in range(ns)]
+    tot = sum(raw)
+    spec = torch.stack([r / tot * rho for r in raw])
+    return torch.cat([f[:5], spec, f[5:]], dim=0)
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("ns", [2, 3, 4])
+@pytest.mark.parametrize("scheme,recon,solver", [(gb.MHM, gb.PLM, gb.ROE), (gb.CTU, gb.PPM, gb.HLLC), (gb.VL, gb.PLM, gb.HLLC)])
+def test_passive_scalars_match_oracle(dev, oracle_mod, scheme, recon, solver, ns, dtype):
+    """N passive scalars, with and without renormalisation; ns = 3 also runs as 2 species + the entropy of
+    the dual-energy formalism (the entropy is the last scalar and is not renormalised)."""
+    for kw in (dict(), dict(renormalize=True)) + ((dict(renormalize=True, dual_energy=True),) if ns == 3 else ()):
+        dual = bool(kw.get("dual_energy"))
+        f = _species_field(ns - 1 if dual else ns, entropy=dual)
+        padded = inputs.pack_periodic(f).to(dtype)
+        p64 = padded.to(torch.float64)
+        dh = 1 / 32
+        dt = oracle_mod.cfl_dt(inputs.interior(p64).contiguous().numpy(), dh, G53, 0.4, scheme, oracle_mod.make_opts(n_scalar=ns))[0]
+        ref = oracle_mod.fluid_advance(p64.numpy(), dt, dh, G53, scheme, recon, solver, oracle_mod.make_opts(n_scalar=ns, **kw))
+        try:
+            out, flux, speed, nun, diag = gpu_ex(padded.to(dev), dt, dh, G53, scheme, recon, solver, n_scalar=ns, **kw)
+        except gb.GamerError as e:      # a tile that cannot fit in shared memory is refused, never computed wrongly
+            assert "-2" in str(e) and dtype == torch.float64 and ns == 4, e
+            continue
+        tol = 1e-12 if dtype == torch.float64 else 1e-5
+        err = rel_l1(out.cpu().numpy(), ref["out"], G53)
+        assert max(err.values()) <= tol, (kw, err)
+        o, r = out.cpu().numpy().astype(np.float64), ref["out"]
+        for k in range(5, 5 + ns):
+            assert np.abs(o[:, k] - r[:, k]).sum() <= tol * np.abs(r[:, k]).sum(), (kw, k)
+        fe = np.abs(flux.cpu().numpy() - ref["flux"]).sum() / np.abs(ref["flux"]).sum()
+        assert fe <= 2 * tol
+        assert nun == ref["stats"]["n_unphysical"] == 0
+        if kw.get("renormalize"):
+            last = 5 + ns - (1 if dual else 0)
+            ssum = o[:, 5:last].sum(axis=1)
+            assert np.abs(ssum / o[:, 0] - 1.0).max() <= (1e-14 if dtype == torch.float64 else 1e-6)
