@@ -1,11 +1,12 @@
 // launch.cuh -- host-side launch helpers: tile height selection by shared-memory fit, attribute setup.
-// MHM_TY_OVERRIDE, MHM_FORCE_NSTG2, CTU_TY_OVERRIDE, CTU_NT_OVERRIDE are tuning hooks for experiments
+// MHM_TY_OVERRIDE, MHM_FORCE_NSTG2, CTU_TY_OVERRIDE are tuning hooks for experiments
 // (GAMER_EXTRA_DEFS of build.py); the shipped library is built without them.
 #pragma once
 #include <cstdlib>
 #include "mhm_kernel.cuh"
 #ifdef GAMER_HAVE_CTU
 #include "ctu_kernel.cuh"
+#include "ctu_wl_kernel.cuh"
 #endif
 
 namespace gamer {
@@ -62,33 +63,48 @@ cudaError_t launch_mhm(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
 }
 
 #ifdef GAMER_HAVE_CTU
-#ifndef CTU_NT_OVERRIDE
-#define CTU_NT_OVERRIDE 0
-#endif
+// fp32: the thread-owned kernel (ctu_kernel.cuh); fp64: the work-list kernel (ctu_wl_kernel.cuh), see its header
+template <typename T, int RECON, int NV, int TY, bool FUSED>
+struct CtuPick {
+    using S32 = CtuSmem<T, RECON, NV, TY, FUSED>;
+    using S64 = CtuWlSmem<T, RECON, NV, TY, FUSED>;
+    static constexpr bool WL = sizeof(T) == 8;
+    static constexpr size_t BYTES = WL ? S64::BYTES : S32::BYTES;
+    static constexpr int NT = WL ? (48 * TY < 128 ? 128 : 48 * TY) : S32::NT;
+};
+
 template <typename T, int RECON, int NV, bool FUSED>
 constexpr int ctu_tile() {
-    return CtuSmem<T, RECON, NV, 16, FUSED>::BYTES <= SMEM_LIMIT ? 16 : (CtuSmem<T, RECON, NV, 8, FUSED>::BYTES <= SMEM_LIMIT ? 8 : 4);
+    return CtuPick<T, RECON, NV, 16, FUSED>::BYTES <= SMEM_LIMIT ? 16 : (CtuPick<T, RECON, NV, 8, FUSED>::BYTES <= SMEM_LIMIT ? 8 : 4);
 }
 
 template <typename T, int RECON, int SOLVER, int NV, bool EXT, bool FUSED>
 cudaError_t launch_ctu_f(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
+#ifdef CTU_TY_OVERRIDE
+    constexpr int TY = CTU_TY_OVERRIDE;
+#else
     constexpr int TY = ctu_tile<T, RECON, NV, FUSED>();
-    constexpr int NT = CTU_NT_OVERRIDE > 0 ? CTU_NT_OVERRIDE : ((sizeof(T) == 8 ? 48 : 32) * TY < 128 ? 128 : (sizeof(T) == 8 ? 48 : 32) * TY);
+#endif
     using G = Geo<TY>;
-    using S = CtuSmem<T, RECON, NV, TY, FUSED>;
+    using S = CtuPick<T, RECON, NV, TY, FUSED>;
     if constexpr (S::BYTES > SMEM_LIMIT) {      // not even the 4-row tile fits (many scalars in fp64): not built
         (void)a; (void)st; (void)launches;
         return cudaErrorNotSupported;
     } else {
-    auto kern = ctu_kernel<T, RECON, SOLVER, NV, EXT, TY, NT, FUSED>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::BYTES);
+    cudaError_t (*set)(const void*, cudaFuncAttribute, int) = cudaFuncSetAttribute;
+    const void* kern;
+    if constexpr (S::WL) kern = (const void*)ctu_wl_kernel<T, RECON, SOLVER, NV, EXT, TY, S::NT, FUSED>;
+    else kern = (const void*)ctu_kernel<T, RECON, SOLVER, NV, EXT, TY, FUSED>;
+    cudaError_t e = set(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)S::BYTES);
     if (e != cudaSuccess) return e;
     if (G::NTILE > 1 && a.speed) {
         e = cudaMemsetAsync(a.speed, 0, sizeof(T) * a.n_groups, st);
         if (e != cudaSuccess) return e;
     }
     const long long grid = a.n_groups * G::NTILE;
-    kern<<<(unsigned)grid, NT, S::BYTES, st>>>(a);
+    void* args[] = {const_cast<AdvArgs<T>*>(&a)};
+    e = cudaLaunchKernel(kern, dim3((unsigned)grid), dim3(S::NT), args, S::BYTES, st);
+    if (e != cudaSuccess) return e;
     *launches += 1;
     return cudaGetLastError();
     }
