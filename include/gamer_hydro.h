@@ -28,7 +28,8 @@
  *   is reconstructed as q_k = s_k / rho and rides the mass flux, upwinded.  With dual_energy the last one carries the
  *   entropy s = P/rho^(gamma-1) of L100.
  * Ownership: every pointer is a DEVICE pointer owned by the caller, 16-byte aligned and
- * non-overlapping, unless the name ends in _host.  The library keeps no state between calls.
+ * non-overlapping, unless the name ends in _host.  The device entries keep no state between calls; the two *_host entries
+ * keep their streams and device scratch buffers until gamer_release_scratch() and serialise their callers on a mutex.
  */
 #ifndef GAMER_HYDRO_H
 #define GAMER_HYDRO_H
@@ -236,7 +237,24 @@ int gamer_fluid_advance_host(const void* in_host, void* out_host, void* flux_out
                              void* group_speed_out_host, int64_t n_groups,
                              double dt, double dh, double gamma,
                              int scheme, int recon, int riemann, int precision,
-                             const gamer_opts* opts /* nullable; device pointers inside are ignored */);
+                             const gamer_opts* opts /* nullable; stream is ignored; n_unphysical_out / diag_out / dt_dev
+                                                       set => GAMER_EUNSUPPORTED; invalid fields => GAMER_EINVAL before any copy */);
+
+/* The same from the UNPADDED state: u_host[n_groups][NVAR][16][16][16] and the same-level table nbr_host[n_groups][27]
+ * (HOST int32; as in gamer_fluid_advance_resident: entry 13 = the group itself, every entry in [0, n_groups)).  No padded
+ * batch exists anywhere: the state crosses PCIe once (1 / 2.6 of the padded bytes), in chunks of 1024 groups on a copy
+ * stream; the kernel of output chunk k (gamer_fluid_advance_resident's fused ghost gather, on one of three streams) starts as
+ * soon as the input chunks its table entries point into have landed, and its out / flux_out / group_speed_out chunk is copied
+ * back behind it -- the paper's preparation step (its stated bottleneck, L681-687) and its stream overlap (L242) without the
+ * CPU gather.  The call keeps a device copy of the whole state (n_groups x NVAR x 16 KB in fp32) plus three output chunks
+ * between calls (gamer_release_scratch frees them), serialises callers on a mutex and synchronises before returning.
+ * fp64 results are bit-identical to gamer_fluid_advance_resident.  Not with remedy_first_order (GAMER_EUNSUPPORTED);
+ * opts->n_unphysical_out / diag_out / dt_dev set => GAMER_EUNSUPPORTED (device outputs belong to the device entries). */
+int gamer_fluid_advance_host_resident(const void* u_host, const int32_t* nbr_host, void* out_host, void* flux_out_host,
+                                      void* group_speed_out_host, int64_t n_groups,
+                                      double dt, double dh, double gamma,
+                                      int scheme, int recon, int riemann, int precision,
+                                      const gamer_opts* opts /* nullable */);
 
 void gamer_release_scratch(void);
 

@@ -23,7 +23,7 @@ LIB_PATH = os.path.join(_HERE, "libgamerhydro.so")
 EXPORTS = ["gamer_fluid_advance", "gamer_fluid_advance_ex", "gamer_fluid_advance_retry", "gamer_cfl_dt", "gamer_cfl_dt_ex",
            "gamer_cfl_from_group_speed", "gamer_refresh_ghosts_periodic", "gamer_refresh_ghosts", "gamer_refresh_ghosts_table", "gamer_interpolate_ghosts", "gamer_fluid_advance_resident",
            "gamer_neighbors_periodic", "gamer_restrict", "gamer_flux_accumulate", "gamer_flux_correct",
-           "gamer_poisson_sor", "gamer_fluid_advance_host", "gamer_release_scratch", "gamer_alu_peak",
+           "gamer_poisson_sor", "gamer_fluid_advance_host", "gamer_fluid_advance_host_resident", "gamer_release_scratch", "gamer_alu_peak",
            "gamer_launch_count", "gamer_strerror", "gamer_version"]
 
 
@@ -85,6 +85,8 @@ def lib():
         L.gamer_flux_correct.argtypes = [vp, vp, vp, vp, i64, ci, dbl, ci, vp]
         L.gamer_fluid_advance_host.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, ci, ci,
                                                ctypes.POINTER(gamer_opts)]
+        L.gamer_fluid_advance_host_resident.argtypes = [vp, vp, vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, ci, ci,
+                                                        ctypes.POINTER(gamer_opts)]
         L.gamer_alu_peak.argtypes = [ci, ctypes.POINTER(dbl), ctypes.POINTER(dbl), vp]
         L.gamer_launch_count.restype = ctypes.c_int64
         L.gamer_strerror.restype = ctypes.c_char_p
@@ -272,6 +274,20 @@ def gamer_fluid_advance_host(in_host, out_host, flux_out_host, group_speed_out_h
                                           _ptr(group_speed_out_host, "cpu"), n, float(dt), float(dh), float(gamma),
                                           int(scheme), int(recon), int(riemann), _precision(in_host),
                                           ctypes.byref(opts)), "gamer_fluid_advance_host")
+
+
+def gamer_fluid_advance_host_resident(u_host, nbr_host, out_host, flux_out_host, group_speed_out_host, dt, dh, gamma, scheme,
+                                      recon, riemann, opts=None):
+    """Host-buffer entry on the UNPADDED state + neighbour table (CPU tensors, pinned preferably); copies happen inside."""
+    n = u_host.shape[0]
+    if nbr_host.dtype != torch.int32 or tuple(nbr_host.shape) != (n, 27):
+        raise GamerError("nbr_host must be an int32 tensor of shape [n_groups, 27]")
+    if opts is None:
+        opts = make_opts(on_device=False, n_scalar=u_host.shape[1] - 5)
+    _check(lib().gamer_fluid_advance_host_resident(_ptr(u_host, "cpu"), _ptr(nbr_host, "cpu"), _ptr(out_host, "cpu"),
+                                                   _ptr(flux_out_host, "cpu"), _ptr(group_speed_out_host, "cpu"), n, float(dt),
+                                                   float(dh), float(gamma), int(scheme), int(recon), int(riemann),
+                                                   _precision(u_host), ctypes.byref(opts)), "gamer_fluid_advance_host_resident")
 
 
 ALU_FFMA, ALU_FMUL_FADD, ALU_FFMA_FMNMX, ALU_FFMA2, ALU_FFMA2_FMNMX, ALU_DFMA, ALU_FFMA_MUFU, ALU_FFMA2_FFMA, ALU_FFMA2_IADD = range(9)

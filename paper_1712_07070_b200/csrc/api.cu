@@ -3,7 +3,9 @@
 #include <atomic>
 #include <cmath>
 #include <cstring>
+#include <algorithm>
 #include <mutex>
+#include <vector>
 
 #include "../../include/gamer_hydro.h"
 #include "aux_kernels.cuh"
@@ -396,6 +398,8 @@ extern "C" int gamer_flux_correct(void* coarse, const void* coarse_flux, const v
 // ------------------------------------------------------------------------------------------ host-buffer entry
 // scratch of the host entry (3 streams, 3 sets of device buffers), kept between calls: allocating and freeing
 // ~0.6 GB per call cost more than the copies of a small batch.  Freed by gamer_release_scratch() or at exit.
+static void gamer_release_resident_scratch();
+static int check_host_opts(const gamer_opts* opts);
 namespace {
 struct HostScratch {
     static constexpr int NBUF = 3;
@@ -441,8 +445,11 @@ HostScratch g_scratch;
 }  // namespace
 
 extern "C" void gamer_release_scratch(void) {
-    std::lock_guard<std::mutex> lock(g_scratch.mu);
-    g_scratch.release();
+    {
+        std::lock_guard<std::mutex> lock(g_scratch.mu);
+        g_scratch.release();
+    }
+    gamer_release_resident_scratch();
 }
 
 extern "C" int gamer_fluid_advance_host(const void* in_host, void* out_host, void* flux_out_host,
@@ -452,6 +459,10 @@ extern "C" int gamer_fluid_advance_host(const void* in_host, void* out_host, voi
     if (!in_host || !out_host || n_groups < 0) return GAMER_EINVAL;
     if (precision != GAMER_FP32 && precision != GAMER_FP64) return GAMER_EINVAL;
     if (!(dt > 0.0) || !std::isfinite(dt)) return GAMER_EINVAL;
+    {
+        const int vrc = check_host_opts(opts);      // before anything is sized from opts
+        if (vrc) return vrc;
+    }
     if (n_groups == 0) return GAMER_OK;
     const int nv = 5 + (opts ? opts->n_scalar : 0);
     const size_t sz = (size_t)precision;
@@ -491,6 +502,159 @@ extern "C" int gamer_fluid_advance_host(const void* in_host, void* out_host, voi
     for (int b = 0; b < NBUF; ++b)
         if (cudaStreamSynchronize(st[b]) != cudaSuccess) rc = GAMER_ECUDA;
     return rc;
+}
+
+// ------------------------------------------------------------------------------------------ host entry, unpadded state
+// Validation shared by the two host entries: everything that sizes an allocation or a copy is checked BEFORE it is used.
+static int check_host_opts(const gamer_opts* opts) {
+    if (!opts) return GAMER_OK;
+    if (opts->n_scalar < 0 || opts->n_scalar > GAMER_MAX_SCALARS) return GAMER_EINVAL;
+    if (opts->dual_energy && opts->n_scalar < 1) return GAMER_EINVAL;
+    if (opts->limiter < 0 || opts->limiter > GAMER_LIMITER_VANALBADA) return GAMER_EINVAL;
+    if (opts->min_dens < 0 || opts->min_pres < 0 || opts->min_temp < 0) return GAMER_EINVAL;
+    if (opts->n_unphysical_out || opts->diag_out || opts->dt_dev) return GAMER_EUNSUPPORTED;   // device outputs: use the device entries
+    return GAMER_OK;
+}
+
+namespace {
+struct ResidentScratch {      // device copy of the whole unpadded state + table, and a ring of output chunks
+    static constexpr int NBUF = 3;
+    cudaStream_t st_in = nullptr, st[NBUF] = {nullptr, nullptr, nullptr};
+    char* d_u = nullptr;
+    int32_t* d_nbr = nullptr;
+    char* d_out[NBUF] = {};
+    char* d_fl[NBUF] = {};
+    char* d_sp[NBUF] = {};
+    std::vector<cudaEvent_t> ev;      // one per input chunk
+    size_t cap_u = 0, cap_nbr = 0, cap_out = 0, cap_fl = 0, cap_sp = 0;
+    int device = -1;
+    std::mutex mu;
+    void release() {
+        if (d_u) cudaFree(d_u);
+        if (d_nbr) cudaFree(d_nbr);
+        for (int b = 0; b < NBUF; ++b) {
+            if (d_out[b]) cudaFree(d_out[b]);
+            if (d_fl[b]) cudaFree(d_fl[b]);
+            if (d_sp[b]) cudaFree(d_sp[b]);
+            if (st[b]) cudaStreamDestroy(st[b]);
+            d_out[b] = d_fl[b] = d_sp[b] = nullptr;
+            st[b] = nullptr;
+        }
+        if (st_in) cudaStreamDestroy(st_in);
+        for (cudaEvent_t e : ev) cudaEventDestroy(e);
+        ev.clear();
+        d_u = nullptr; d_nbr = nullptr; st_in = nullptr;
+        cap_u = cap_nbr = cap_out = cap_fl = cap_sp = 0;
+        device = -1;
+    }
+    bool ensure(size_t u_b, size_t nbr_b, size_t out_b, size_t fl_b, size_t sp_b, size_t n_ev) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess) return false;
+        if (dev != device || u_b > cap_u || nbr_b > cap_nbr || out_b > cap_out || fl_b > cap_fl || sp_b > cap_sp) {
+            release();
+            if (cudaStreamCreateWithFlags(&st_in, cudaStreamNonBlocking) != cudaSuccess) return false;
+            if (cudaMalloc(&d_u, u_b) != cudaSuccess || cudaMalloc(&d_nbr, nbr_b) != cudaSuccess) return false;
+            for (int b = 0; b < NBUF; ++b) {
+                if (cudaStreamCreateWithFlags(&st[b], cudaStreamNonBlocking) != cudaSuccess) return false;
+                if (cudaMalloc(&d_out[b], out_b) != cudaSuccess || cudaMalloc(&d_fl[b], fl_b) != cudaSuccess ||
+                    cudaMalloc(&d_sp[b], sp_b) != cudaSuccess)
+                    return false;
+            }
+            cap_u = u_b; cap_nbr = nbr_b; cap_out = out_b; cap_fl = fl_b; cap_sp = sp_b;
+            device = dev;
+        }
+        while (ev.size() < n_ev) {
+            cudaEvent_t e;
+            if (cudaEventCreateWithFlags(&e, cudaEventDisableTiming) != cudaSuccess) return false;
+            ev.push_back(e);
+        }
+        return true;
+    }
+};
+ResidentScratch g_resident;
+}  // namespace
+
+extern "C" int gamer_fluid_advance_host_resident(const void* u_host, const int32_t* nbr_host, void* out_host,
+                                                 void* flux_out_host, void* group_speed_out_host, int64_t n_groups,
+                                                 double dt, double dh, double gamma, int scheme, int recon, int riemann,
+                                                 int precision, const gamer_opts* opts) {
+    if (!u_host || !nbr_host || !out_host || n_groups < 0 || u_host == out_host) return GAMER_EINVAL;
+    if (precision != GAMER_FP32 && precision != GAMER_FP64) return GAMER_EINVAL;
+    if (!(dt > 0.0) || !std::isfinite(dt)) return GAMER_EINVAL;
+    int rc = check_host_opts(opts);
+    if (rc) return rc;
+    if (opts && opts->remedy_first_order) return GAMER_EUNSUPPORTED;      // remedy (ii) re-reads the padded slab
+    if (n_groups > 0x3fffffff / 27) return GAMER_EUNSUPPORTED;
+    if (n_groups == 0) return GAMER_OK;
+    const int nv = 5 + (opts ? opts->n_scalar : 0);
+    const size_t sz = (size_t)precision;
+    const size_t u_g = (size_t)nv * PS * PS * PS * sz, fl_g = (size_t)9 * nv * PS * PS * sz;
+    const int64_t chunk = n_groups < 1024 ? n_groups : 1024;      // input and output granularity
+    const int64_t n_chunks = (n_groups + chunk - 1) / chunk;
+    // which input chunks each output chunk needs: those that hold one of its groups' 27 table entries
+    std::vector<std::vector<int>> need((size_t)n_chunks);
+    {
+        std::vector<char> mark((size_t)n_chunks);
+        for (int64_t k = 0; k < n_chunks; ++k) {
+            std::fill(mark.begin(), mark.end(), 0);
+            const int64_t g1 = (k + 1) * chunk < n_groups ? (k + 1) * chunk : n_groups;
+            for (int64_t i = k * chunk * 27; i < g1 * 27; ++i) {
+                const int32_t s = nbr_host[i];
+                if (s < 0 || s >= n_groups) return GAMER_EINVAL;
+                mark[(size_t)(s / chunk)] = 1;
+            }
+            for (int64_t c = 0; c < n_chunks; ++c)
+                if (mark[(size_t)c]) need[(size_t)k].push_back((int)c);
+        }
+    }
+    constexpr int NBUF = ResidentScratch::NBUF;
+    std::lock_guard<std::mutex> lock(g_resident.mu);
+    ResidentScratch& R = g_resident;
+    if (!R.ensure(u_g * n_groups, sizeof(int32_t) * 27 * n_groups, u_g * chunk, fl_g * chunk, sz * chunk, (size_t)n_chunks)) {
+        R.release();
+        return GAMER_ECUDA;
+    }
+    // the whole unpadded state goes to the device once, chunk by chunk on its own stream; the table first
+    if (cudaMemcpyAsync(R.d_nbr, nbr_host, sizeof(int32_t) * 27 * n_groups, cudaMemcpyHostToDevice, R.st_in) != cudaSuccess) return GAMER_ECUDA;
+    for (int64_t k = 0; k < n_chunks; ++k) {
+        const int64_t g0 = k * chunk, n = (n_groups - g0) < chunk ? (n_groups - g0) : chunk;
+        if (cudaMemcpyAsync(R.d_u + g0 * u_g, static_cast<const char*>(u_host) + g0 * u_g, u_g * n, cudaMemcpyHostToDevice, R.st_in) != cudaSuccess ||
+            cudaEventRecord(R.ev[(size_t)k], R.st_in) != cudaSuccess)
+            return GAMER_ECUDA;
+    }
+    rc = GAMER_OK;
+    for (int64_t k = 0; k < n_chunks && rc == GAMER_OK; ++k) {
+        const int b = (int)(k % NBUF);
+        const int64_t g0 = k * chunk, n = (n_groups - g0) < chunk ? (n_groups - g0) : chunk;
+        for (int c : need[(size_t)k])
+            if (cudaStreamWaitEvent(R.st[b], R.ev[(size_t)c], 0) != cudaSuccess) rc = GAMER_ECUDA;
+        if (rc != GAMER_OK) break;
+        gamer_opts o;
+        if (opts) o = *opts; else std::memset(&o, 0, sizeof(o));
+        o.stream = R.st[b];
+        o.dt_dev = nullptr; o.n_unphysical_out = nullptr; o.diag_out = nullptr;
+        o.group_speed_out = group_speed_out_host ? R.d_sp[b] : nullptr;
+        // the kernel indexes `in` by the table's (global) entries and out / flux / speed by the group's index in the launch
+        rc = precision == GAMER_FP32
+                 ? advance_typed<float>(R.d_u, R.d_out[b], flux_out_host ? R.d_fl[b] : nullptr, n, dt, dh, gamma, scheme, recon, riemann, &o, R.d_nbr + g0 * 27)
+                 : advance_typed<double>(R.d_u, R.d_out[b], flux_out_host ? R.d_fl[b] : nullptr, n, dt, dh, gamma, scheme, recon, riemann, &o, R.d_nbr + g0 * 27);
+        if (rc != GAMER_OK) break;
+        cudaMemcpyAsync(static_cast<char*>(out_host) + g0 * u_g, R.d_out[b], u_g * n, cudaMemcpyDeviceToHost, R.st[b]);
+        if (flux_out_host)
+            cudaMemcpyAsync(static_cast<char*>(flux_out_host) + g0 * fl_g, R.d_fl[b], fl_g * n, cudaMemcpyDeviceToHost, R.st[b]);
+        if (group_speed_out_host)
+            cudaMemcpyAsync(static_cast<char*>(group_speed_out_host) + g0 * sz, R.d_sp[b], sz * n, cudaMemcpyDeviceToHost, R.st[b]);
+        if (cudaGetLastError() != cudaSuccess) rc = GAMER_ECUDA;
+    }
+    if (cudaStreamSynchronize(R.st_in) != cudaSuccess) rc = GAMER_ECUDA;
+    for (int b = 0; b < NBUF; ++b)
+        if (cudaStreamSynchronize(R.st[b]) != cudaSuccess) rc = GAMER_ECUDA;
+    return rc;
+}
+
+static void gamer_release_resident_scratch() {
+    std::lock_guard<std::mutex> lock(g_resident.mu);
+    g_resident.release();
 }
 
 extern "C" int64_t gamer_launch_count(void) { return g_launches.load(); }

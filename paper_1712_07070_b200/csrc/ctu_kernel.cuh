@@ -270,7 +270,7 @@ __global__ void __launch_bounds__((CtuSmem<T, RECON, NV, TY, FUSED>::NT), 1) ctu
         // ------------------------------------------------------------------ P2
         T f1x[NV], f1y[NV], ffx[NV], ffy[NV], U0[NV];
         // conserved input of cell (ci, cj, kk-1): padded mode: cell of the padded slab; fused mode: of the group's own state
-        const T* gcell = FUSED ? gin + (size_t)g * NV * PS3 + (size_t)(kk - 1) * PSQ + gj * PS + ci
+        const T* gcell = FUSED ? gin + (size_t)nb[13] * NV * PS3 + (size_t)(kk - 1) * PSQ + gj * PS + ci
                                : gin + (size_t)(kk - 1 + NGH) * (NP * NP) + (gj + NGH) * NP + (ci + NGH);
         if (inner && kk >= 1) {      // loaded two phases ahead of its use
 #pragma unroll

@@ -463,7 +463,7 @@ __global__ void __launch_bounds__(NT) ctu_wl_kernel(const AdvArgs<T> a) {
         if (owner) {
             if (m >= 1) {
                 const int k = m - 1;
-                const T* gcell = FUSED ? gin + (size_t)g * NV * (PS * PS * PS) + (size_t)k * (PS * PS) + (j0 + cj) * PS + ci
+                const T* gcell = FUSED ? gin + (size_t)nb[13] * NV * (PS * PS * PS) + (size_t)k * (PS * PS) + (j0 + cj) * PS + ci
                                        : gin + (size_t)(k + NGH) * (NP * NP) + (j0 + cj + NGH) * NP + (ci + NGH);
                 T U[NV], Fz[NV];
                 get_state<T, NV>(fz, G::NFZ, tid, Fz);

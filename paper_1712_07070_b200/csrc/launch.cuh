@@ -13,9 +13,9 @@ namespace gamer {
 
 constexpr size_t SMEM_LIMIT = 232448;   // 227 KB opt-in maximum per CTA on sm_100
 
-template <typename T, int RECON, int NV, bool VLS>
+template <typename T, int RECON, int NV, bool VLS, bool FUSED>
 constexpr int mhm_tile() {
-    return MhmGeo<T, RECON, NV, 16, 2, false, VLS>::BYTES <= SMEM_LIMIT ? 16 : (MhmGeo<T, RECON, NV, 8, 2, false, VLS>::BYTES <= SMEM_LIMIT ? 8 : 4);
+    return MhmGeo<T, RECON, NV, 16, 2, FUSED, VLS>::BYTES <= SMEM_LIMIT ? 16 : (MhmGeo<T, RECON, NV, 8, 2, FUSED, VLS>::BYTES <= SMEM_LIMIT ? 8 : 4);
 }
 
 constexpr size_t SM_SMEM = 233472;      // 228 KB of shared memory per SM, 1 KB of it reserved per resident CTA
@@ -26,7 +26,7 @@ cudaError_t launch_mhm_f(const AdvArgs<T>& a, cudaStream_t st, int* launches) {
 #ifdef MHM_TY_OVERRIDE
     constexpr int TY = MHM_TY_OVERRIDE;
 #else
-    constexpr int TY = mhm_tile<T, RECON, NV, VLS>();
+    constexpr int TY = mhm_tile<T, RECON, NV, VLS, FUSED>();
 #endif
     // two landing stages unless dropping to one lets a second CTA share the SM
     constexpr int C2 = ctas_by_smem(MhmGeo<T, RECON, NV, TY, 2, FUSED, VLS>::BYTES), C1 = ctas_by_smem(MhmGeo<T, RECON, NV, TY, 1, FUSED, VLS>::BYTES);

@@ -448,7 +448,7 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED, VLS>::N
         // ------------------------------------------------------------------ conserved input of cell (ei, ej, kk-1)
         const bool upd = interior && kk >= 1;
         // padded mode: cell of the padded slab; fused mode: cell of this group's unpadded state
-        const T* gcell = FUSED ? gin + (size_t)g * NV * (PS * PSQ) + c.out_off + (kk - 1) * PSQ
+        const T* gcell = FUSED ? gin + (size_t)nb[13] * NV * (PS * PSQ) + c.out_off + (kk - 1) * PSQ
                                : gin + c.gin_off + (kk - 1) * (NP * NP);
         T U[NV];
         if (upd) {

@@ -606,3 +606,58 @@ def test_passive_scalars_match_oracle(dev, oracle_mod, scheme, recon, solver, ns
             last = 5 + ns - (1 if dual else 0)
             ssum = o[:, 5:last].sum(axis=1)
             assert np.abs(ssum / o[:, 0] - 1.0).max() <= (1e-14 if dtype == torch.float64 else 1e-6)
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+@pytest.mark.parametrize("scheme,recon,solver,kw,dims", [
+    (gb.MHM, gb.PLM, gb.ROE, {}, (2, 3, 4)),                                   # one ragged chunk
+    (gb.CTU, gb.PPM, gb.HLLC, {}, (2, 3, 4)),
+    (gb.VL, gb.PLM, gb.HLLC, dict(n_scalar=2, renormalize=True), (2, 3, 4)),
+    (gb.MHM, gb.PLM, gb.HLLE, {}, (11, 10, 10)),                               # 1100 groups: two chunks, the second ragged
+])
+def test_host_entry_on_the_unpadded_state_is_bitwise_the_resident_entry(dev, scheme, recon, solver, kw, dims, dtype):
+    """gamer_fluid_advance_host_resident: unpadded host state + host neighbour table in, host out / flux_out / speeds out,
+    chunked copies overlapped with the fused-ghost kernels.  Must carry the bits of gamer_fluid_advance_resident on the
+    whole batch (the same kernels on sub-ranges of the same device state), and of the padded host entry in fp64."""
+    gz, gy, gx = dims
+    ns = kw.get("n_scalar", 0)
+    if gz * gy * gx > 100:
+        gen = torch.Generator().manual_seed(5)
+        rho = 1.0 + 0.3 * torch.rand((gz * 16, gy * 16, gx * 16), generator=gen, dtype=torch.float64)
+        vel = [0.3 * (torch.rand(rho.shape, generator=gen, dtype=torch.float64) - 0.5) for _ in range(3)]
+        f = inputs.prim_to_cons(rho, vel[0], vel[1], vel[2], torch.ones_like(rho), G53)
+    else:
+        f = _species_field(ns, n=16, seed=77)[:5 + ns] if ns else inputs.turbulence_field(16, 77, kmax=4, gamma=G53, shape=(gz * 16, gy * 16, gx * 16))
+        if ns:
+            f = torch.cat([f] * 1, dim=0)
+            f = f.repeat(1, gz, gy, gx)
+    padded = inputs.pack_periodic(f).to(dtype)
+    u = inputs.interior(padded).contiguous()
+    dt, dh = 0.002, 1.0 / 64
+    nbr = gb.gamer_neighbors_periodic(gz, gy, gx, dev)
+    ud = u.to(dev)
+    out1, flux1, speed1 = gb.alloc_outputs(padded.to(dev))
+    gb.gamer_fluid_advance_resident(ud, nbr, out1, flux1, dt, dh, G53, scheme, recon, solver, gb.make_opts(group_speed_out=speed1, **kw))
+    torch.cuda.synchronize()
+    h_u, h_nbr = u.pin_memory(), nbr.cpu().pin_memory()
+    h_out, h_flux, h_speed = torch.empty_like(h_u).pin_memory(), torch.empty(flux1.shape, dtype=dtype).pin_memory(), torch.empty(speed1.shape, dtype=dtype).pin_memory()
+    for _ in range(2):      # second call: scratch reused
+        h_out.zero_()
+        gb.gamer_fluid_advance_host_resident(h_u, h_nbr, h_out, h_flux, h_speed, dt, dh, G53, scheme, recon, solver,
+                                             gb.make_opts(on_device=False, **kw))
+        assert torch.equal(h_out, out1.cpu()) and torch.equal(h_flux, flux1.cpu()) and torch.equal(h_speed, speed1.cpu())
+    if dtype == torch.float64 and not kw:
+        p_out, p_flux, p_speed = torch.empty_like(h_out), torch.empty_like(h_flux), torch.empty_like(h_speed)
+        gb.gamer_fluid_advance_host(padded.contiguous(), p_out, p_flux, p_speed, dt, dh, G53, scheme, recon, solver)
+        assert (p_out - h_out).abs().max().item() <= 1e-13 * h_out.abs().max().item()
+    # bad table entries and unsupported options are refused before any copy
+    bad = h_nbr.clone()
+    bad[0, 5] = gz * gy * gx
+    with pytest.raises(gb.GamerError, match="-1"):
+        gb.gamer_fluid_advance_host_resident(h_u, bad, h_out, h_flux, h_speed, dt, dh, G53, scheme, recon, solver, gb.make_opts(on_device=False, **kw))
+    with pytest.raises(gb.GamerError, match="-1"):
+        gb.gamer_fluid_advance_host_resident(h_u, h_nbr, h_out, h_flux, h_speed, dt, dh, G53, scheme, recon, solver, gb.make_opts(on_device=False, n_scalar=7))
+    with pytest.raises(gb.GamerError, match="-2"):
+        gb.gamer_fluid_advance_host_resident(h_u, h_nbr, h_out, h_flux, h_speed, dt, dh, G53, scheme, recon, solver,
+                                             gb.make_opts(on_device=False, remedy_first_order=True, **kw))
+    gb.gamer_release_scratch()
