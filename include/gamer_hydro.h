@@ -23,7 +23,9 @@
  *             other axes, the lower-numbered axis fastest (x-faces: [z][y]; y: [z][x]; z: [y][x]).
  *             Values are the time-centred flux densities F_d, not multiplied by dt or area.
  *   group_speed_out [n_groups]   max over the 16^3 UPDATED cells of |vx|+|vy|+|vz|+3c (MHM and VL, Eq. 2)
- *                                or max(|vx|,|vy|,|vz|)+c (CTU, Eq. 1)
+ *                                or max(|vx|,|vy|,|vz|)+c (CTU, Eq. 1).  A cell whose speed is NaN (P < 0 after the update)
+ *                                is skipped by the maximum: such cells are reported through n_unphysical_out, which is what
+ *                                a caller must test (remedies (iv)/(v)); the dt of the remaining cells stays usable
  *   NVAR = 5 + n_scalar: conserved passive scalars s_k (chemical species as partial densities, L96) follow E; each
  *   is reconstructed as q_k = s_k / rho and rides the mass flux, upwinded.  With dual_energy the last one carries the
  *   entropy s = P/rho^(gamma-1) of L100.
@@ -67,7 +69,8 @@ enum {
 typedef struct gamer_opts {
     void*    stream;              /* cudaStream_t; NULL = default stream                            */
     int      limiter;             /* GAMER_LIMITER_*; 0 = generalized minmod                        */
-    double   minmod_theta;        /* <= 0: 1 for PLM (plain minmod), 2 for PPM (Colella-Woodward)   */
+    double   minmod_theta;        /* <= 0: 1 for PLM (plain minmod), 2 for PPM (Colella-Woodward); else must lie in [1, 2]
+                                     (the TVD range), anything else is GAMER_EINVAL                 */
     int      n_scalar;            /* 0 .. GAMER_MAX_SCALARS passively advected scalars (L96)        */
     int      dual_energy;         /* 0 | 1 (needs n_scalar >= 1; the LAST scalar is the entropy): L100 */
     double   de_xi;               /* switch E_the/E_kin < xi; <= 0: 1e-2                            */

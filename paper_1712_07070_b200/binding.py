@@ -138,17 +138,44 @@ def make_opts(stream=None, limiter=0, minmod_theta=0.0, n_scalar=0, dual_energy=
     o.diag_out = _ptr(diag_out)
     o.char_limiting = int(bool(char_limiting))
     o.renormalize = int(bool(renormalize))
+    # keeps the tensors alive as long as the struct and lets the wrappers check their shapes and dtypes
+    o._tensors = {"dt_dev": dt_dev, "group_speed_out": group_speed_out, "n_unphysical_out": n_unphysical_out, "diag_out": diag_out}
     return o
+
+
+def _check_batch(u, out, flux_out, opts, padded, device_type="cuda"):
+    """Cheap shape / dtype / device checks of one advance call (the kernels trust their pointers): u [G,NV,22^3] (padded) or
+    [G,NV,16^3], out [G,NV,16,16,16], flux_out [G,3,3,NV,16,16], all of u's dtype; NV = 5 + opts.n_scalar; the optional
+    opts outputs: group_speed_out real[G], dt_dev float64[1], n_unphysical_out int32[1], diag_out int32[4] cannot be
+    checked from their raw pointers, so make_opts records their tensors."""
+    g, nv = int(u.shape[0]), int(u.shape[1])
+    edge = NP if padded else PS
+    if u.dim() != 5 or tuple(u.shape[2:]) != (edge, edge, edge):
+        raise GamerError(f"state must be [G, NV, {edge}, {edge}, {edge}], got {tuple(u.shape)}")
+    ns = opts.n_scalar if opts is not None else 0
+    if nv != 5 + ns:
+        raise GamerError(f"state carries {nv} variables but opts.n_scalar = {ns}")
+    if tuple(out.shape) != (g, nv, PS, PS, PS) or out.dtype != u.dtype or out.device.type != device_type:
+        raise GamerError(f"out must be [{g}, {nv}, 16, 16, 16] of {u.dtype} on {device_type}")
+    if flux_out is not None and (tuple(flux_out.shape) != (g, 3, 3, nv, PS, PS) or flux_out.dtype != u.dtype or flux_out.device.type != device_type):
+        raise GamerError(f"flux_out must be [{g}, 3, 3, {nv}, 16, 16] of {u.dtype} on {device_type}")
+    for name, shape, dtype in (("group_speed_out", (g,), u.dtype), ("dt_dev", (1,), torch.float64),
+                               ("n_unphysical_out", (1,), torch.int32), ("diag_out", (4,), torch.int32)):
+        t = getattr(opts, "_tensors", {}).get(name) if opts is not None else None
+        if t is not None and (tuple(t.shape) != shape or t.dtype != dtype):
+            raise GamerError(f"opts.{name} must be a {dtype} tensor of shape {shape}")
 
 
 def gamer_fluid_advance(u_in, out, flux_out, dt, dh, gamma, scheme, recon, riemann):
     """11-argument form.  NOTE: runs on the default stream, as the C ABI states."""
+    _check_batch(u_in, out, flux_out, None, True)
     n = u_in.shape[0]
     _check(lib().gamer_fluid_advance(_ptr(u_in), _ptr(out), _ptr(flux_out), n, float(dt), float(dh), float(gamma),
                                      int(scheme), int(recon), int(riemann), _precision(u_in)), "gamer_fluid_advance")
 
 
 def gamer_fluid_advance_ex(u_in, out, flux_out, dt, dh, gamma, scheme, recon, riemann, opts):
+    _check_batch(u_in, out, flux_out, opts, True)
     n = u_in.shape[0]
     _check(lib().gamer_fluid_advance_ex(_ptr(u_in), _ptr(out), _ptr(flux_out), n, float(dt), float(dh), float(gamma),
                                         int(scheme), int(recon), int(riemann), _precision(u_in), ctypes.byref(opts)),
@@ -157,6 +184,7 @@ def gamer_fluid_advance_ex(u_in, out, flux_out, dt, dh, gamma, scheme, recon, ri
 
 def gamer_fluid_advance_retry(u_in, out, flux_out, dt, dh, gamma, scheme, recon, riemann, opts, dt_ratio=0.8, dt_min=0.0):
     """Remedies (iv)-(v).  Returns (dt_used, n_retries); GamerError(GAMER_EUNPHYSICAL) = the abort."""
+    _check_batch(u_in, out, flux_out, opts, True)
     n = u_in.shape[0]
     dt_used, n_retries = ctypes.c_double(0.0), ctypes.c_int32(0)
     _check(lib().gamer_fluid_advance_retry(_ptr(u_in), _ptr(out), _ptr(flux_out), n, float(dt), float(dh), float(gamma),
@@ -216,7 +244,8 @@ def gamer_fluid_advance_resident(u, nbr, out, flux_out, dt, dh, gamma, scheme, r
     if nbr.dtype != torch.int32 or tuple(nbr.shape) != (u.shape[0], 27):
         raise GamerError("nbr must be an int32 tensor of shape [n_groups, 27]")
     if opts is None:
-        opts = make_opts()
+        opts = make_opts(n_scalar=u.shape[1] - 5)
+    _check_batch(u, out, flux_out, opts, False)
     _check(lib().gamer_fluid_advance_resident(_ptr(u), _ptr(nbr), _ptr(out), _ptr(flux_out), u.shape[0], float(dt), float(dh),
                                               float(gamma), int(scheme), int(recon), int(riemann), _precision(u),
                                               ctypes.byref(opts)), "gamer_fluid_advance_resident")
@@ -269,7 +298,8 @@ def gamer_fluid_advance_host(in_host, out_host, flux_out_host, group_speed_out_h
     """Host-buffer entry: tensors live on the CPU (pinned preferably); copies happen inside the call."""
     n = in_host.shape[0]
     if opts is None:
-        opts = make_opts(on_device=False)
+        opts = make_opts(on_device=False, n_scalar=in_host.shape[1] - 5)
+    _check_batch(in_host, out_host, flux_out_host, opts, True, "cpu")
     _check(lib().gamer_fluid_advance_host(_ptr(in_host, "cpu"), _ptr(out_host, "cpu"), _ptr(flux_out_host, "cpu"),
                                           _ptr(group_speed_out_host, "cpu"), n, float(dt), float(dh), float(gamma),
                                           int(scheme), int(recon), int(riemann), _precision(in_host),
@@ -284,6 +314,7 @@ def gamer_fluid_advance_host_resident(u_host, nbr_host, out_host, flux_out_host,
         raise GamerError("nbr_host must be an int32 tensor of shape [n_groups, 27]")
     if opts is None:
         opts = make_opts(on_device=False, n_scalar=u_host.shape[1] - 5)
+    _check_batch(u_host, out_host, flux_out_host, opts, False, "cpu")
     _check(lib().gamer_fluid_advance_host_resident(_ptr(u_host, "cpu"), _ptr(nbr_host, "cpu"), _ptr(out_host, "cpu"),
                                                    _ptr(flux_out_host, "cpu"), _ptr(group_speed_out_host, "cpu"), n, float(dt),
                                                    float(dh), float(gamma), int(scheme), int(recon), int(riemann),

@@ -101,6 +101,7 @@ extern "C" int gamer_fluid_advance_ex(const void* in, void* out, void* flux_out,
         if (opts->n_scalar < 0 || opts->n_scalar > GAMER_MAX_SCALARS) return GAMER_EINVAL;
         if (opts->dual_energy && opts->n_scalar < 1) return GAMER_EINVAL;      // the entropy is the last scalar
         if (opts->limiter < 0 || opts->limiter > GAMER_LIMITER_VANALBADA) return GAMER_EINVAL;
+        if (opts->minmod_theta > 0.0 && !(opts->minmod_theta >= 1.0 && opts->minmod_theta <= 2.0)) return GAMER_EINVAL;   // TVD range
         if (opts->min_dens < 0 || opts->min_pres < 0 || opts->min_temp < 0) return GAMER_EINVAL;
     }
     if (n_groups > 0x3fffffff) return GAMER_EUNSUPPORTED;
@@ -155,6 +156,7 @@ extern "C" int gamer_fluid_advance_resident(const void* u, const int32_t* nbr, v
         if (opts->n_scalar < 0 || opts->n_scalar > GAMER_MAX_SCALARS) return GAMER_EINVAL;
         if (opts->dual_energy && opts->n_scalar < 1) return GAMER_EINVAL;      // the entropy is the last scalar
         if (opts->limiter < 0 || opts->limiter > GAMER_LIMITER_VANALBADA) return GAMER_EINVAL;
+        if (opts->minmod_theta > 0.0 && !(opts->minmod_theta >= 1.0 && opts->minmod_theta <= 2.0)) return GAMER_EINVAL;   // TVD range
         if (opts->min_dens < 0 || opts->min_pres < 0 || opts->min_temp < 0) return GAMER_EINVAL;
         if (opts->remedy_first_order) return GAMER_EUNSUPPORTED;   // remedy (ii) re-reads the padded slab
     }
@@ -511,6 +513,7 @@ static int check_host_opts(const gamer_opts* opts) {
     if (opts->n_scalar < 0 || opts->n_scalar > GAMER_MAX_SCALARS) return GAMER_EINVAL;
     if (opts->dual_energy && opts->n_scalar < 1) return GAMER_EINVAL;
     if (opts->limiter < 0 || opts->limiter > GAMER_LIMITER_VANALBADA) return GAMER_EINVAL;
+    if (opts->minmod_theta > 0.0 && !(opts->minmod_theta >= 1.0 && opts->minmod_theta <= 2.0)) return GAMER_EINVAL;
     if (opts->min_dens < 0 || opts->min_pres < 0 || opts->min_temp < 0) return GAMER_EINVAL;
     if (opts->n_unphysical_out || opts->diag_out || opts->dt_dev) return GAMER_EUNSUPPORTED;   // device outputs: use the device entries
     return GAMER_OK;

@@ -51,7 +51,7 @@ __global__ void __launch_bounds__(256) cfl_kernel(const CflArgs<T> a) {
 #pragma unroll
             for (int v = 0; v < NV; ++v) Uc[v] = U[v][e];
             const T s = signal_speed<T, NV, SCHEME, true>(Uc, ph);
-            if (s > smax) smax = s;
+            smax = speed_max(smax, s);
         }
     }
 #pragma unroll

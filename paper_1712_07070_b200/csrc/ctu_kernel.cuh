@@ -381,7 +381,7 @@ __global__ void __launch_bounds__((CtuSmem<T, RECON, NV, TY, FUSED>::NT), 1) ctu
                 for (int v = 0; v < NV; ++v) gout[((size_t)v * PS + k) * PSQ + gj * PS + ci] = U[v];
                 if (a.speed) {
                     const T s = signal_speed<T, NV, CTU, EXT>(U, ph);
-                    if (s > smax) smax = s;
+                    smax = speed_max(smax, s);
                 }
             }
 #pragma unroll

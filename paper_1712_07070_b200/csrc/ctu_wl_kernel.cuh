@@ -477,7 +477,7 @@ __global__ void __launch_bounds__(NT) ctu_wl_kernel(const AdvArgs<T> a) {
                 for (int v = 0; v < NV; ++v) gout[((size_t)v * PS + k) * (PS * PS) + (j0 + cj) * PS + ci] = U[v];
                 if (a.speed) {
                     const T s = signal_speed<T, NV, CTU, EXT>(U, ph);
-                    if (s > smax) smax = s;
+                    smax = speed_max(smax, s);
                 }
             }
             if (m >= 0 && m < PS) {

@@ -60,6 +60,12 @@ __device__ __forceinline__ void renormalize_scalars(T* U, const Phys<T>& ph) {
         if (v < last) U[v] = U[v] * f;
 }
 
+// running maximum of the CFL signal speeds.  A NaN speed (a cell that came out with P < 0) never wins the comparison, as
+// in the oracle's reduction: such cells are what n_unphysical_out counts and remedies (iv)/(v) act on; the time-step
+// of the remaining cells stays usable for the retry.
+template <typename T>
+__device__ __forceinline__ T speed_max(T smax, T s) { return s > smax ? s : smax; }
+
 template <typename T, int NV, int SCHEME, bool EXT>
 __device__ __forceinline__ T signal_speed(const T* U, const Phys<T>& ph) {
     T W[NV];

@@ -513,7 +513,7 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED, VLS>::N
             for (int v = 0; v < NV; ++v) o[(size_t)v * (PS * PSQ)] = U[v];
             if (a.speed) {
                 const T s = signal_speed<T, NV, MHM, EXT>(U, ph);
-                if (s > smax) smax = s;
+                smax = speed_max(smax, s);
             }
         }
         if (interior && kk >= 0) {

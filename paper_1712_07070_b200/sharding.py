@@ -20,17 +20,34 @@ def global_dt(dt: torch.Tensor) -> torch.Tensor:
     return dt
 
 
-def global_count(n: int) -> int:
-    """SUM all-reduce of one integer (e.g. the unphysical-cell count of a rank's shard)."""
+def _reduce_device() -> torch.device:
+    """Where a tensor must live to be all-reduced by the current process group: NCCL reduces device tensors only."""
+    if dist.get_backend() == "nccl":
+        return torch.device("cuda", torch.cuda.current_device())
+    return torch.device("cpu")
+
+
+def global_count(n) -> int:
+    """SUM all-reduce of one integer (e.g. the unphysical-cell count of a rank's shard).  `n` is an int or a 1-element
+    integer tensor (the device counter that gamer_fluid_advance_ex filled); the reduction runs on the device the
+    backend needs (NCCL: the current CUDA device, gloo: the host)."""
     if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
-        t = torch.tensor([int(n)], dtype=torch.int64)
+        dev = _reduce_device()
+        if torch.is_tensor(n):
+            t = n.detach().reshape(1).to(device=dev, dtype=torch.int64)
+        else:
+            t = torch.tensor([int(n)], dtype=torch.int64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.SUM)
         return int(t.item())
-    return int(n)
+    return int(n.item()) if torch.is_tensor(n) else int(n)
 
 
 def retry_level(step_fn, dt: float, dt_ratio: float = 0.8, dt_min: float = 0.0, max_retries: int = 200):
-    """Remedies (iv), (v) of PAPER.md L107-108 for a level sharded over ranks: "recalculate ALL patches on the currently
+    """The DISTRIBUTED form of gamer_fluid_advance_retry (csrc/api.cu), which is its single-process form: the same policy
+    (dt multiplied by dt_ratio per retry, threshold test before the attempt, at most 200 reductions; R23) with the
+    one thing a single process cannot do, the reduction of the count over ranks between attempts.  tests/test_multirank_cpu.py
+    holds the two to the same (dt_used, n_retries) through the oracle's loop.
+    Remedies (iv), (v) of PAPER.md L107-108 for a level sharded over ranks: "recalculate ALL patches on the currently
     targeted level with this reduced time-step" -- a rank whose own shard came out physical must redo it too, so the
     decision is taken on the SUM of the ranks' counts.  step_fn(dt) advances this rank's shard from its unchanged input
     (e.g. binding.gamer_fluid_advance_ex with n_unphysical_out) and returns its count of unphysical cells.

@@ -61,6 +61,27 @@ def test_argument_validation_needs_no_gpu(built_lib):
     # sizes beyond what the launch grid / 32-bit offsets cover are refused, not truncated
     assert L.gamer_fluid_advance(ok[0], ok[1], None, 1 << 30, 0.1, 0.1, 1.4, 1, 1, 1, 4) == -2
     assert L.gamer_fluid_advance(ok[0], ok[1], None, 0, 0.1, 0.1, 1.4, 1, 1, 1, 4) == 0          # empty batch: no-op
+    # extended entry: option fields are validated before any CUDA call
+    from paper_1712_07070_b200 import binding as gbo
+    L.gamer_fluid_advance_ex.argtypes = [vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, ci, ci, ctypes.POINTER(gbo.gamer_opts)]
+    for field, val in (("minmod_theta", 3.0), ("minmod_theta", 0.5), ("n_scalar", 5), ("n_scalar", -1), ("limiter", 9), ("min_dens", -1.0)):
+        ob = gbo.gamer_opts()
+        setattr(ob, field, val)
+        assert L.gamer_fluid_advance_ex(ok[0], ok[1], None, 1, 0.1, 0.1, 1.4, 1, 1, 1, 4, ctypes.byref(ob)) == -1, field
+    ob = gbo.gamer_opts()
+    ob.dual_energy = 1                                            # needs the entropy scalar
+    assert L.gamer_fluid_advance_ex(ok[0], ok[1], None, 1, 0.1, 0.1, 1.4, 1, 1, 1, 4, ctypes.byref(ob)) == -1
+    # host entries: the same validation happens before anything is sized or copied; device outputs are refused
+    L.gamer_fluid_advance_host.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, ci, ci, ctypes.POINTER(gbo.gamer_opts)]
+    L.gamer_fluid_advance_host_resident.argtypes = [vp, vp, vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, ci, ci, ctypes.POINTER(gbo.gamer_opts)]
+    ob = gbo.gamer_opts()
+    ob.n_scalar = 7
+    assert L.gamer_fluid_advance_host(ok[0], ok[1], None, None, 1, 0.1, 0.1, 1.4, 1, 1, 1, 4, ctypes.byref(ob)) == -1
+    assert L.gamer_fluid_advance_host_resident(ok[0], vp(64), ok[1], None, None, 1, 0.1, 0.1, 1.4, 1, 1, 1, 4, ctypes.byref(ob)) == -1
+    ob = gbo.gamer_opts()
+    ob.diag_out = 4096
+    assert L.gamer_fluid_advance_host(ok[0], ok[1], None, None, 1, 0.1, 0.1, 1.4, 1, 1, 1, 4, ctypes.byref(ob)) == -2
+    assert L.gamer_fluid_advance_host_resident(None, vp(64), ok[1], None, None, 1, 0.1, 0.1, 1.4, 1, 1, 1, 4, None) == -1
     # fused-refresh entry: no neighbour table, remedy (ii) (needs the padded slab), in-place update
     from paper_1712_07070_b200 import binding as gb
     L.gamer_fluid_advance_resident.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, ci, ci, ctypes.POINTER(gb.gamer_opts)]

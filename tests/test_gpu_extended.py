@@ -76,10 +76,31 @@ def test_stress_modes_match_oracle(dev, oracle_mod, scheme, recon, solver, kw, d
         assert fe <= 1e-12
         assert np.abs(speed.cpu().numpy() - ref["speed"]).max() <= 1e-11 * ref["speed"].max()
     else:
-        # marginal decisions may flip in fp32: report through a looser bound, still far below O(1)
-        assert abs(nun - st["n_unphysical"]) <= 2 + 0.02 * st["n_unphysical"]
-        assert abs(diag[2] - st["n_first_order"]) <= 3 + 0.05 * st["n_first_order"]
-        assert max(err.values()) <= 2e-4, err
+        # fp32: the continuous arithmetic must meet the contract's 1e-5; what may differ from the fp64 oracle are the
+        # DISCONTINUOUS decisions on marginal data (remedy (i) fallback, predictor / correction reverts, remedy (ii), the
+        # dual-energy switch): SURVEY 8(c) asks for their number.  A cell counts as "decided differently" when it is off by
+        # more than 1e-3 of the variable's scale (three orders above fp32 round-off, the size of a flipped decision);
+        # the 1e-5 bound is asserted on all other cells, the differing cells are counted, bounded and reported.
+        o, r = out.cpu().numpy().astype(np.float64), ref["out"]
+        scale = np.abs(r).mean(axis=(0, 2, 3, 4), keepdims=True) + 1e-300
+        scale[:, 1:4] = np.sqrt((r[:, 1:4] ** 2).sum(axis=1, keepdims=True)).mean() + np.abs(r[:, 0:1]).mean() * math.sqrt(G53)
+        cell_err = (np.abs(o - r) / scale).max(axis=1)                   # [G,16,16,16]
+        differ = cell_err > 1e-3
+        n_diff, n_cells = int(differ.sum()), differ.size
+        keep = ~differ
+        agree = {name: np.abs(o[:, v][keep] - r[:, v][keep]).sum() / np.abs(r[:, v][keep]).sum() for v, name in ((0, "rho"), (4, "E"))}
+        agree["mom"] = sum(np.abs(o[:, d][keep] - r[:, d][keep]).sum() for d in (1, 2, 3)) / (scale[0, 1, 0, 0, 0] * keep.sum())
+        counts = {"cells_decided_differently": n_diff, "of": n_cells,
+                  "remedy_i_faces": (diag[0], st["n_roe_fallback"]), "reverted_states": (diag[1], st["n_pred_revert"]),
+                  "remedy_ii_cells": (diag[2], st["n_first_order"]), "dual_energy_cells": (diag[3], st["n_dual_fix"]),
+                  "unphysical": (nun, st["n_unphysical"])}
+        print("fp32 decisions (gpu, oracle):", counts, "L1 on agreeing cells:", agree)
+        assert max(agree.values()) <= 1e-5, (agree, counts)
+        assert n_diff <= 2e-3 * n_cells, counts                          # measured: a few 1e-4 of the cells at Mach 10
+        assert abs(nun - st["n_unphysical"]) <= 2 + 0.02 * st["n_unphysical"], counts
+        assert abs(diag[2] - st["n_first_order"]) <= 3 + 0.05 * st["n_first_order"], counts
+        assert abs(diag[3] - st["n_dual_fix"]) <= 3 + 0.02 * st["n_dual_fix"], counts
+        assert max(err.values()) <= 2e-4, err                            # and the flipped cells stay far below O(1) in the norm
     assert torch.isfinite(out).all()
 
 
@@ -164,9 +185,12 @@ def test_config4_full_size_sampled_fp32(dev, oracle_mod, scheme, recon, solver, 
     _sampled_parity(dev, oracle_mod, f, torch.float32, scheme, recon, solver, cfl, 1e-5)
 
 
-def test_config4_sampled_fp64_8192_groups(dev, oracle_mod):
-    f = inputs.turbulence_field(320, 7070, kmax=16, gamma=G53, device=dev)        # 20^3 = 8000 groups
-    _sampled_parity(dev, oracle_mod, f, torch.float64, gb.MHM, gb.PLM, gb.ROE, 0.5, 1e-12, n_sample=24)
+@pytest.mark.parametrize("scheme,recon,solver,cfl", [(gb.MHM, gb.PLM, gb.ROE, 0.5), (gb.CTU, gb.PPM, gb.HLLC, 0.4)])
+def test_config4_full_size_sampled_fp64(dev, oracle_mod, scheme, recon, solver, cfl):
+    """BASELINE.json config 4 in fp64 at its full 32,768 groups (in + out + flux_out = 22 GB of the 180), both variants the
+    bench times; oracle on sampled groups, conservation over the whole box."""
+    f = inputs.turbulence_field(512, 7070, kmax=16, gamma=G53, device=dev)
+    _sampled_parity(dev, oracle_mod, f, torch.float64, scheme, recon, solver, cfl, 1e-12, n_sample=24)
 
 
 def test_config5_full_size_sampled(dev, oracle_mod):
@@ -232,7 +256,7 @@ def test_config3_two_level_sedov_flux_correction(dev, oracle_mod):
                                                     (gb.CTU, gb.PPM, gb.HLLC, {}), (gb.CTU, gb.PLM, gb.ROE, {}),
                                                     (gb.CTU, gb.PPM, gb.HLLE, dict(n_scalar=1, dual_energy=True, min_pres=1e-12)),
                                                     (gb.VL, gb.PLM, gb.HLLC, {}), (gb.VL, gb.PLM, gb.ROE, dict(n_scalar=1, dual_energy=True, min_pres=1e-12))])
-def test_fused_ghost_refresh_entry_is_bitwise_the_padded_path(dev, scheme, recon, solver, kw, dtype):
+def test_fused_ghost_refresh_entry_matches_the_padded_path(dev, scheme, recon, solver, kw, dtype):
     """SURVEY 8(f) NEXT-1, second half: gamer_fluid_advance_resident gathers the ghost zones from the neighbours'
     unpadded state inside the solver.  On a periodic 2 x 3 x 4 box of groups (so that -1 and +1 neighbours coincide
     along z and differ along x) it must reproduce host packing + gamer_fluid_advance_ex for out, flux_out and the
@@ -655,7 +679,7 @@ def test_host_entry_on_the_unpadded_state_is_bitwise_the_resident_entry(dev, sch
     bad[0, 5] = gz * gy * gx
     with pytest.raises(gb.GamerError, match="-1"):
         gb.gamer_fluid_advance_host_resident(h_u, bad, h_out, h_flux, h_speed, dt, dh, G53, scheme, recon, solver, gb.make_opts(on_device=False, **kw))
-    with pytest.raises(gb.GamerError, match="-1"):
+    with pytest.raises(gb.GamerError):      # the binding's own shape check catches it before the C entry would (-1)
         gb.gamer_fluid_advance_host_resident(h_u, h_nbr, h_out, h_flux, h_speed, dt, dh, G53, scheme, recon, solver, gb.make_opts(on_device=False, n_scalar=7))
     with pytest.raises(gb.GamerError, match="-2"):
         gb.gamer_fluid_advance_host_resident(h_u, h_nbr, h_out, h_flux, h_speed, dt, dh, G53, scheme, recon, solver,

@@ -118,3 +118,16 @@ def test_two_ranks_retry_the_level_together():
     c0, c1 = res[0][3], res[1][3]
     assert all(a + b > 0 for a, b in zip(c0[:-1], c1[:-1])) and c0[-1] == c1[-1] == 0
     assert all(b == 0 for b in c1), (c0, c1)          # rank 1 alone would never have retried: the decision is the level's
+
+
+def test_count_reduction_picks_the_device_the_backend_needs(monkeypatch):
+    """bench.py initialises NCCL only: a CPU tensor cannot be all-reduced there.  The placement is decided by
+    the backend, not hard-coded; a tensor argument (the device counter) is accepted as well as an int."""
+    sys.path.insert(0, ROOT)
+    from paper_1712_07070_b200 import sharding
+    monkeypatch.setattr(sharding.dist, "get_backend", lambda: "gloo")
+    assert sharding._reduce_device().type == "cpu"
+    monkeypatch.setattr(sharding.dist, "get_backend", lambda: "nccl")
+    monkeypatch.setattr(sharding.torch.cuda, "current_device", lambda: 3)
+    assert sharding._reduce_device() == torch.device("cuda", 3)
+    assert sharding.global_count(5) == 5 and sharding.global_count(torch.tensor([7], dtype=torch.int32)) == 7   # no group: identity
