@@ -367,3 +367,31 @@ def poisson_residual(phi, rho, dh, coeff):
     r = (phi[:, 1:17, 1:17, 0:16] + phi[:, 1:17, 1:17, 2:18] + phi[:, 1:17, 0:16, 1:17] + phi[:, 1:17, 2:18, 1:17]
          + phi[:, 0:16, 1:17, 1:17] + phi[:, 2:18, 1:17, 1:17] - 6.0 * c - coeff * dh * dh * np.asarray(rho, dtype=np.float64))
     return np.abs(r).reshape(phi.shape[0], -1).max(axis=1)
+
+
+def gravity_update(u, acc, dt):
+    """The fluid's gravity update that the paper performs on the GPU "immediately after solving the potential" (PAPER.md L238;
+    SURVEY 8(f) NEXT-4 tail; reading R28 of DESIGN.md): with the cell-centred acceleration g = -grad(phi) of a patch's 8^3
+    active zones,
+        m_new = m + dt * rho * g            (momentum kick; rho is not changed by gravity),
+        E_new = E + (|m_new|^2 - |m|^2) / (2 rho)      ("use the corrected momentum to further correct energy", L130:
+                                                         the kinetic energy follows the momentum, the thermal energy stays).
+    u [G, NV, 16, 16, 16] fluid in the patch-group layout (a copy is returned); acc [8 G, 3, 8, 8, 8] in the PATCH layout
+    of poisson_sor, components (x, y, z), patch n = 8 g + octant, octant = oz*4 + oy*2 + ox covering cells
+    [8 ox, 8 ox + 8) x [8 oy, ..) x [8 oz, ..) of group g (the octant numbering of restrict / interpolate_ghosts).
+    Passive scalars are untouched.  Plain loops over patches; numpy arithmetic inside a patch."""
+    u = np.array(u, dtype=np.float64)
+    acc = np.asarray(acc, dtype=np.float64)
+    assert acc.shape[0] == 8 * u.shape[0] and acc.shape[1:] == (3, 8, 8, 8)
+    for n in range(acc.shape[0]):
+        g, o = n >> 3, n & 7
+        sz, sy, sx = (slice(8 * b, 8 * b + 8) for b in (o >> 2, (o >> 1) & 1, o & 1))
+        rho = u[g, 0, sz, sy, sx]
+        m_old = [u[g, 1 + d, sz, sy, sx].copy() for d in range(3)]
+        m_new = [m_old[d] + (dt * rho) * acc[n, d] for d in range(3)]
+        ke_new = (m_new[0] * m_new[0] + m_new[1] * m_new[1]) + m_new[2] * m_new[2]
+        ke_old = (m_old[0] * m_old[0] + m_old[1] * m_old[1]) + m_old[2] * m_old[2]
+        u[g, 4, sz, sy, sx] = u[g, 4, sz, sy, sx] + 0.5 * (ke_new - ke_old) / rho
+        for d in range(3):
+            u[g, 1 + d, sz, sy, sx] = m_new[d]
+    return u

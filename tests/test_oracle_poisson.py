@@ -1,5 +1,6 @@
 """Pins for the oracle's SOR Poisson solver.  CPU only."""
 import numpy as np
+import pytest
 import scipy.sparse as sp
 import scipy.sparse.linalg as spla
 
@@ -104,3 +105,63 @@ def test_residual_definition_and_decay(oracle_mod):
            for n in (0, 5, 20, 60, 200)]
     assert all(a > b for a, b in zip(res, res[1:])) and res[-1] <= 1e-12 * np.abs(phi0).max()
     assert oracle_mod.poisson_residual(_direct(phi0, rho, dh, coeff), rho, dh, coeff).max() <= 1e-12 * np.abs(phi0).max()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# fluid gravity update behind the Poisson solve (R28)
+# ---------------------------------------------------------------------------------------------------------------
+def _gas(g=2, seed=3, nv=5):
+    rng = np.random.default_rng(seed)
+    u = np.empty((g, nv, 16, 16, 16))
+    u[:, 0] = rng.uniform(0.5, 2.0, (g, 16, 16, 16))
+    v = rng.normal(0, 0.5, (g, 3, 16, 16, 16))
+    p = rng.uniform(0.5, 2.0, (g, 16, 16, 16))
+    u[:, 1:4] = u[:, 0:1] * v
+    u[:, 4] = p / (5 / 3 - 1) + 0.5 * u[:, 0] * (v ** 2).sum(axis=1)
+    if nv > 5:
+        u[:, 5:] = rng.uniform(0.1, 1.0, (g, nv - 5, 16, 16, 16))
+    return u
+
+
+def test_gravity_update_closed_forms(oracle_mod):
+    """Uniform acceleration: momentum gains dt rho g exactly as written; the thermal energy E - |m|^2 / 2 rho is unchanged
+    to round-off (the energy correction is the kinetic-energy difference); density and scalars untouched bit for bit;
+    a kick followed by the opposite kick restores the state; N kicks of a gas at rest give v = N dt g."""
+    u = _gas(nv=7)
+    gvec = np.array([0.3, -0.7, 1.1])
+    acc = np.broadcast_to(gvec[None, :, None, None, None], (16, 3, 8, 8, 8)).copy()
+    dt = 0.05
+    new = oracle_mod.gravity_update(u, acc, dt)
+    assert np.array_equal(new[:, 0], u[:, 0]) and np.array_equal(new[:, 5:], u[:, 5:])
+    for d in range(3):
+        assert np.array_equal(new[:, 1 + d], u[:, 1 + d] + (dt * u[:, 0]) * gvec[d])
+    eth = lambda a: a[:, 4] - 0.5 * (a[:, 1:4] ** 2).sum(axis=1) / a[:, 0]
+    assert np.abs(eth(new) - eth(u)).max() <= 2e-15 * np.abs(u[:, 4]).max()
+    back = oracle_mod.gravity_update(new, -acc, dt)
+    assert np.abs(back - u).max() <= 4e-15 * np.abs(u).max()
+    rest = _gas()
+    rest[:, 1:4] = 0.0
+    rest[:, 4] = 1.5
+    cur = rest
+    for _ in range(8):
+        cur = oracle_mod.gravity_update(cur, acc, dt)
+    for d in range(3):
+        assert np.abs(cur[:, 1 + d] / cur[:, 0] - 8 * dt * gvec[d]).max() <= 1e-14
+    assert np.abs(cur[:, 4] - (1.5 + 0.5 * cur[:, 0] * ((8 * dt * gvec) ** 2).sum())).max() <= 1e-13
+
+
+def test_gravity_update_patch_to_group_mapping(oracle_mod):
+    """acc lives in the patch layout of poisson_sor (patch n = 8 g + oz*4 + oy*2 + ox), the fluid in the group layout: a
+    kick confined to one patch changes exactly that octant of that group, with the patch's own cell order."""
+    u = _gas(g=3)
+    acc = np.zeros((24, 3, 8, 8, 8))
+    n = 8 * 1 + (1 * 4 + 0 * 2 + 1)                      # group 1, octant oz=1, oy=0, ox=1
+    acc[n, 0] = np.arange(512).reshape(8, 8, 8)          # distinct value per cell: x fastest
+    new = oracle_mod.gravity_update(u, acc, 1.0)
+    diff = new != u
+    assert not diff[0].any() and not diff[2].any()
+    box = np.zeros((16, 16, 16), dtype=bool)
+    box[8:16, 0:8, 8:16] = True                          # [z, y, x]
+    assert not diff[1][:, ~box].any() and not diff[1, 0].any() and not diff[1, 2:4].any()
+    dm = (new[1, 1] - u[1, 1]) / u[1, 0]
+    assert dm[8, 0, 9] == pytest.approx(1.0, rel=1e-14) and dm[9, 0, 8] == pytest.approx(64.0, rel=1e-14) and dm[8, 1, 8] == pytest.approx(8.0, rel=1e-14)
