@@ -231,6 +231,20 @@ int gamer_flux_correct(void* coarse, const void* coarse_flux, const void* fine_f
 int gamer_poisson_sor(void* phi, const void* rho, void* acc, void* resid_out, int64_t n_patches, double dh, double coeff,
                       double omega, int n_iter, int precision, void* stream);
 
+/* The fluid's gravity update, which the paper performs on the GPU "immediately after solving the potential" to save a round
+ * trip of the acceleration (L130 "correct momentum and then use the corrected momentum to further correct
+ * energy"; R28).  For every cell of the 8^3 active zones of every patch, with g = -grad(phi):
+ *   m <- m + dt * rho * g,      E <- E + (|m_new|^2 - |m_old|^2) / (2 rho)      (density, thermal energy and scalars unchanged).
+ * flu[n_patches / 8][nvar][16][16][16] is the fluid in the PATCH-GROUP layout (`out` of the solver), updated in place; patch
+ * n = 8 g + oz*4 + oy*2 + ox is the octant (ox, oy, oz) of group g (the numbering of gamer_restrict), so n_patches must be a
+ * multiple of 8.  gamer_poisson_sor_gravity = gamer_poisson_sor with this update fused behind the solve in the same kernel
+ * (the acceleration never leaves the SM; acc may be NULL); gamer_gravity_update applies a given acc[n_patches][3][8][8][8]
+ * (e.g. the root level's, or an external acceleration).  A caller builds the second-order corrector of L130 from two
+ * half kicks with the old and the new acceleration.  dt may be negative (undoing a kick). */
+int gamer_poisson_sor_gravity(void* phi, const void* rho, void* acc, void* resid_out, void* flu, int nvar, double dt,
+                              int64_t n_patches, double dh, double coeff, double omega, int n_iter, int precision, void* stream);
+int gamer_gravity_update(void* flu, const void* acc, int64_t n_patches, int nvar, double dt, int precision, void* stream);
+
 /* End-to-end form with HOST buffers (pinned or pageable): copies `in` to the device in chunks,
  * runs the solver, copies `out`, `flux_out` (nullable) and `group_speed_out` (nullable) back,
  * overlapping copies and kernels on internal streams as the paper does with CUDA streams (L242),

@@ -23,7 +23,7 @@ LIB_PATH = os.path.join(_HERE, "libgamerhydro.so")
 EXPORTS = ["gamer_fluid_advance", "gamer_fluid_advance_ex", "gamer_fluid_advance_retry", "gamer_cfl_dt", "gamer_cfl_dt_ex",
            "gamer_cfl_from_group_speed", "gamer_refresh_ghosts_periodic", "gamer_refresh_ghosts", "gamer_refresh_ghosts_table", "gamer_interpolate_ghosts", "gamer_fluid_advance_resident",
            "gamer_neighbors_periodic", "gamer_restrict", "gamer_flux_accumulate", "gamer_flux_correct",
-           "gamer_poisson_sor", "gamer_fluid_advance_host", "gamer_fluid_advance_host_resident", "gamer_release_scratch", "gamer_alu_peak",
+           "gamer_poisson_sor", "gamer_poisson_sor_gravity", "gamer_gravity_update", "gamer_fluid_advance_host", "gamer_fluid_advance_host_resident", "gamer_release_scratch", "gamer_alu_peak",
            "gamer_launch_count", "gamer_strerror", "gamer_version"]
 
 
@@ -79,6 +79,8 @@ def lib():
         L.gamer_fluid_advance_resident.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, ci, ci, ctypes.POINTER(gamer_opts)]
         L.gamer_neighbors_periodic.argtypes = [vp, ci, ci, ci, vp]
         L.gamer_poisson_sor.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, vp]
+        L.gamer_poisson_sor_gravity.argtypes = [vp, vp, vp, vp, vp, ci, dbl, i64, dbl, dbl, dbl, ci, ci, vp]
+        L.gamer_gravity_update.argtypes = [vp, vp, i64, ci, dbl, ci, vp]
         L.gamer_interpolate_ghosts.argtypes = [vp, vp, dbl, vp, vp, vp, i64, ci, ci, ci, vp]
         L.gamer_restrict.argtypes = [vp, vp, vp, i64, ci, ci, vp]
         L.gamer_flux_accumulate.argtypes = [vp, vp, dbl, i64, ci, ci, ci, vp]
@@ -291,6 +293,32 @@ def gamer_poisson_sor(phi, rho, acc, dh, coeff, omega, n_iter, stream=None, resi
         raise GamerError("resid_out must be [N] of phi's dtype")
     _check(lib().gamer_poisson_sor(_ptr(phi), _ptr(rho), _ptr(acc), _ptr(resid_out), phi.shape[0], float(dh), float(coeff), float(omega),
                                    int(n_iter), _precision(phi), _stream_handle(stream)), "gamer_poisson_sor")
+
+
+def _check_gravity(flu, n_patches):
+    if flu.dim() != 5 or tuple(flu.shape[2:]) != (PS, PS, PS) or flu.shape[0] * 8 != n_patches:
+        raise GamerError("flu must be [n_patches / 8, NV, 16, 16, 16] (patch n = 8 g + octant)")
+
+
+def gamer_poisson_sor_gravity(phi, rho, acc, flu, dt, dh, coeff, omega, n_iter, stream=None, resid_out=None):
+    """gamer_poisson_sor with the fluid's gravity update fused behind the solve; flu in the group layout."""
+    if tuple(phi.shape[1:]) != (18, 18, 18) or tuple(rho.shape) != (phi.shape[0], 16, 16, 16) or rho.dtype != phi.dtype or flu.dtype != phi.dtype:
+        raise GamerError("phi must be [N,18,18,18], rho [N,16,16,16], flu of the same dtype")
+    if acc is not None and (tuple(acc.shape) != (phi.shape[0], 3, 8, 8, 8) or acc.dtype != phi.dtype):
+        raise GamerError("acc must be [N,3,8,8,8] of phi's dtype")
+    _check_gravity(flu, phi.shape[0])
+    _check(lib().gamer_poisson_sor_gravity(_ptr(phi), _ptr(rho), _ptr(acc), _ptr(resid_out), _ptr(flu), flu.shape[1], float(dt),
+                                           phi.shape[0], float(dh), float(coeff), float(omega), int(n_iter), _precision(phi),
+                                           _stream_handle(stream)), "gamer_poisson_sor_gravity")
+
+
+def gamer_gravity_update(flu, acc, dt, stream=None):
+    """m += dt rho g, E += kinetic-energy difference, for acc [N,3,8,8,8] in the patch layout and flu in the group layout."""
+    if tuple(acc.shape[1:]) != (3, 8, 8, 8) or acc.dtype != flu.dtype:
+        raise GamerError("acc must be [N,3,8,8,8] of flu's dtype")
+    _check_gravity(flu, acc.shape[0])
+    _check(lib().gamer_gravity_update(_ptr(flu), _ptr(acc), acc.shape[0], flu.shape[1], float(dt), _precision(flu),
+                                      _stream_handle(stream)), "gamer_gravity_update")
 
 
 def gamer_fluid_advance_host(in_host, out_host, flux_out_host, group_speed_out_host, dt, dh, gamma, scheme, recon,

@@ -327,11 +327,12 @@ extern "C" int gamer_interpolate_ghosts(const void* coarse_in, const void* coars
     return cudaGetLastError() == cudaSuccess ? GAMER_OK : GAMER_ECUDA;
 }
 
-extern "C" int gamer_poisson_sor(void* phi, const void* rho, void* acc, void* resid_out, int64_t n_patches, double dh,
-                                 double coeff, double omega, int n_iter, int precision, void* stream) {
+static int poisson_sor_impl(void* phi, const void* rho, void* acc, void* resid_out, void* flu, int nvar, double dt,
+                            int64_t n_patches, double dh, double coeff, double omega, int n_iter, int precision, void* stream) {
     if (n_patches < 0 || n_iter < 0 || (precision != GAMER_FP32 && precision != GAMER_FP64)) return GAMER_EINVAL;
     if (!(dh > 0.0) || !std::isfinite(dh) || !std::isfinite(coeff) || !(omega > 0.0) || !(omega < 2.0)) return GAMER_EINVAL;
     if (n_patches > 0 && (!phi || !rho || !aligned16(phi) || !aligned16(rho))) return GAMER_EINVAL;
+    if (flu && (nvar < 5 || nvar > 5 + GAMER_MAX_SCALARS || !std::isfinite(dt) || (n_patches & 7) != 0)) return GAMER_EINVAL;
     if (n_patches == 0) return GAMER_OK;
     if (n_patches > 0x7fffffff) return GAMER_EUNSUPPORTED;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
@@ -340,10 +341,38 @@ extern "C" int gamer_poisson_sor(void* phi, const void* rho, void* acc, void* re
     if (precision == GAMER_FP32)
         poisson_sor_kernel<float><<<grid, 256, 0, st>>>(static_cast<float*>(phi), static_cast<const float*>(rho),
                                                         static_cast<float*>(acc), static_cast<float*>(resid_out), (float)ss, (float)w6,
-                                                        (float)i2, n_iter);
+                                                        (float)i2, n_iter, static_cast<float*>(flu), nvar, (float)dt);
     else
         poisson_sor_kernel<double><<<grid, 256, 0, st>>>(static_cast<double*>(phi), static_cast<const double*>(rho),
-                                                         static_cast<double*>(acc), static_cast<double*>(resid_out), ss, w6, i2, n_iter);
+                                                         static_cast<double*>(acc), static_cast<double*>(resid_out), ss, w6, i2, n_iter,
+                                                         static_cast<double*>(flu), nvar, dt);
+    g_launches += 1;
+    return cudaGetLastError() == cudaSuccess ? GAMER_OK : GAMER_ECUDA;
+}
+
+extern "C" int gamer_poisson_sor(void* phi, const void* rho, void* acc, void* resid_out, int64_t n_patches, double dh,
+                                 double coeff, double omega, int n_iter, int precision, void* stream) {
+    return poisson_sor_impl(phi, rho, acc, resid_out, nullptr, 0, 0.0, n_patches, dh, coeff, omega, n_iter, precision, stream);
+}
+
+extern "C" int gamer_poisson_sor_gravity(void* phi, const void* rho, void* acc, void* resid_out, void* flu, int nvar, double dt,
+                                         int64_t n_patches, double dh, double coeff, double omega, int n_iter, int precision,
+                                         void* stream) {
+    if (n_patches > 0 && !flu) return GAMER_EINVAL;
+    return poisson_sor_impl(phi, rho, acc, resid_out, flu, nvar, dt, n_patches, dh, coeff, omega, n_iter, precision, stream);
+}
+
+extern "C" int gamer_gravity_update(void* flu, const void* acc, int64_t n_patches, int nvar, double dt, int precision, void* stream) {
+    if (n_patches < 0 || (n_patches & 7) != 0 || nvar < 5 || nvar > 5 + GAMER_MAX_SCALARS || !std::isfinite(dt)) return GAMER_EINVAL;
+    if (precision != GAMER_FP32 && precision != GAMER_FP64) return GAMER_EINVAL;
+    if (n_patches > 0 && (!flu || !acc)) return GAMER_EINVAL;
+    if (n_patches == 0) return GAMER_OK;
+    if (n_patches > 0x7fffffff) return GAMER_EUNSUPPORTED;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (precision == GAMER_FP32)
+        gravity_update_kernel<float><<<(unsigned)n_patches, 256, 0, st>>>(static_cast<float*>(flu), static_cast<const float*>(acc), nvar, (float)dt);
+    else
+        gravity_update_kernel<double><<<(unsigned)n_patches, 256, 0, st>>>(static_cast<double*>(flu), static_cast<const double*>(acc), nvar, dt);
     g_launches += 1;
     return cudaGetLastError() == cudaSuccess ? GAMER_OK : GAMER_ECUDA;
 }

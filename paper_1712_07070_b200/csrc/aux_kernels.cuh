@@ -311,9 +311,40 @@ __device__ __forceinline__ void sor_half_sweep(T (&me)[PN], const T (&src)[PR], 
 // cells is uniform over a warp and the row can live in registers with static indices.  Lane -> (k, j): r = (warp & 3) * 32 + lane,
 // k = 1 + r / 8, j = 1 + 2 (r % 8) + s with s fixing the parity.  Banks (fp32): 4 k + 4 (r % 8) + 18 s + i with the padded plane
 // stride (= 1 mod 4) puts the 32 lanes of a warp on 32 different banks.
+// (poisson_sor_kernel below, after the gravity helpers it calls.)
+
+// Fluid gravity update of one cell (DESIGN R28): U points at variable 0 of the cell in the patch-group
+// layout (variable stride 16^3); momentum kick dt * rho * g, energy by the kinetic-energy difference.
+template <typename T>
+__device__ __forceinline__ void gravity_kick(T* U, T ax, T ay, T az, T dt) {
+    constexpr int VS = PS * PS * PS;
+    const T rho = U[0], mx = U[VS], my = U[2 * VS], mz = U[3 * VS];
+    const T k = dt * rho;
+    const T nx = mx + k * ax, ny = my + k * ay, nz = mz + k * az;
+    const T ke_new = (nx * nx + ny * ny) + nz * nz, ke_old = (mx * mx + my * my) + mz * mz;
+    U[4 * VS] = U[4 * VS] + T(0.5) * (ke_new - ke_old) / rho;
+    U[VS] = nx; U[2 * VS] = ny; U[3 * VS] = nz;
+}
+
+// the cell (ai, aj, ak) of patch n's 8^3 active zones inside the patch-group batch: patch n = 8 g + oz*4 + oy*2 + ox
+__device__ __forceinline__ size_t patch_cell_in_group(size_t n, int nvar, int ak, int aj, int ai) {
+    const size_t g = n >> 3;
+    const int o = (int)(n & 7);
+    return g * nvar * (PS * PS * PS) + (size_t)(((o >> 2) * 8 + ak) * PS + (((o >> 1) & 1) * 8 + aj)) * PS + ((o & 1) * 8 + ai);
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) gravity_update_kernel(T* __restrict__ flu, const T* __restrict__ acc, int nvar, T dt) {
+    const size_t n = blockIdx.x;
+    const T* ga = acc + n * (3 * 512);
+    for (int t = threadIdx.x; t < 512; t += 256)
+        gravity_kick(flu + patch_cell_in_group(n, nvar, t >> 6, (t >> 3) & 7, t & 7), ga[t], ga[t + 512], ga[t + 1024], dt);
+}
+
 template <typename T>
 __global__ void __launch_bounds__(256) poisson_sor_kernel(T* __restrict__ phi, const T* __restrict__ rho, T* __restrict__ acc,
-                                                          T* __restrict__ resid, T src_scale, T w6, T inv_2dh, int n_iter) {
+                                                          T* __restrict__ resid, T src_scale, T w6, T inv_2dh, int n_iter,
+                                                          T* __restrict__ flu = nullptr, int nvar = 0, T dt_g = T(0)) {
     __shared__ T p[PN * PPL];
     const size_t n = blockIdx.x;
     T* gp = phi + n * (PN * PN * PN);
@@ -359,14 +390,18 @@ __global__ void __launch_bounds__(256) poisson_sor_kernel(T* __restrict__ phi, c
         const int kk = t / (PN * PN);
         gp[t] = p[kk * PPL + t - kk * (PN * PN)];
     }
-    if (acc) {
-        T* ga = acc + n * (3 * PAN * PAN * PAN);
+    if (acc || flu) {      // acceleration of the active zones; the fluid's gravity update straight from it (L238)
+        T* ga = acc ? acc + n * (3 * PAN * PAN * PAN) : nullptr;
         for (int t = threadIdx.x; t < PAN * PAN * PAN; t += 256) {
             const int ak = t / (PAN * PAN), aj = (t / PAN) % PAN, ai = t % PAN;
             const T* c = p + (ak + PA0) * PPL + (aj + PA0) * PN + ai + PA0;
-            ga[t] = -(c[1] - c[-1]) * inv_2dh;
-            ga[t + PAN * PAN * PAN] = -(c[PN] - c[-PN]) * inv_2dh;
-            ga[t + 2 * PAN * PAN * PAN] = -(c[PPL] - c[-PPL]) * inv_2dh;
+            const T ax = -(c[1] - c[-1]) * inv_2dh, ay = -(c[PN] - c[-PN]) * inv_2dh, az = -(c[PPL] - c[-PPL]) * inv_2dh;
+            if (ga) {
+                ga[t] = ax;
+                ga[t + PAN * PAN * PAN] = ay;
+                ga[t + 2 * PAN * PAN * PAN] = az;
+            }
+            if (flu) gravity_kick(flu + patch_cell_in_group(n, nvar, ak, aj, ai), ax, ay, az, dt_g);
         }
     }
 }

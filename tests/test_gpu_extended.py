@@ -685,3 +685,50 @@ def test_host_entry_on_the_unpadded_state_is_bitwise_the_resident_entry(dev, sch
         gb.gamer_fluid_advance_host_resident(h_u, h_nbr, h_out, h_flux, h_speed, dt, dh, G53, scheme, recon, solver,
                                              gb.make_opts(on_device=False, remedy_first_order=True, **kw))
     gb.gamer_release_scratch()
+
+
+@pytest.mark.parametrize("dtype", [torch.float64, torch.float32])
+def test_gravity_update_fused_and_standalone_match_oracle(dev, oracle_mod, dtype):
+    """the fluid's gravity update right behind the Poisson solve.  gamer_poisson_sor_gravity (fused: the
+    acceleration never leaves the SM) and gamer_poisson_sor + gamer_gravity_update must both equal the oracle's
+    poisson_sor -> gravity_update composition; group 1's octants are checked against the patch numbering."""
+    gen = torch.Generator().manual_seed(12)
+    ng, nv = 3, 6
+    npatch = 8 * ng
+    phi = torch.randn((npatch, 18, 18, 18), generator=gen, dtype=torch.float64)
+    rho_p = torch.rand((npatch, 16, 16, 16), generator=gen, dtype=torch.float64) + 0.5
+    flu = torch.empty((ng, nv, 16, 16, 16), dtype=torch.float64)
+    flu[:, 0] = torch.rand((ng, 16, 16, 16), generator=gen, dtype=torch.float64) + 0.5
+    flu[:, 1:4] = flu[:, 0:1] * 0.4 * torch.randn((ng, 3, 16, 16, 16), generator=gen, dtype=torch.float64)
+    flu[:, 4] = 1.5 + 0.5 * (flu[:, 1:4] ** 2).sum(dim=1) / flu[:, 0]
+    flu[:, 5] = torch.rand((ng, 16, 16, 16), generator=gen, dtype=torch.float64)
+    phi, rho_p, flu = phi.to(dtype), rho_p.to(dtype), flu.to(dtype)
+    dh, coeff, om, nit, dt = 0.1, 1.3, 1.6, 12, 0.07
+    rphi, racc = oracle_mod.poisson_sor(phi.double().numpy(), rho_p.double().numpy(), dh, coeff, om, nit)
+    ref = oracle_mod.gravity_update(flu.double().numpy(), racc, dt)
+    tol = 1e-13 if dtype == torch.float64 else 2e-5
+    # fused
+    p1, f1 = phi.clone().to(dev), flu.clone().to(dev)
+    acc1 = torch.empty((npatch, 3, 8, 8, 8), dtype=dtype, device=dev)
+    gb.gamer_poisson_sor_gravity(p1, rho_p.to(dev), acc1, f1, dt, dh, coeff, om, nit)
+    # two calls
+    p2, f2 = phi.clone().to(dev), flu.clone().to(dev)
+    acc2 = torch.empty_like(acc1)
+    gb.gamer_poisson_sor(p2, rho_p.to(dev), acc2, dh, coeff, om, nit)
+    gb.gamer_gravity_update(f2, acc2, dt)
+    # fused without the acceleration output
+    p3, f3 = phi.clone().to(dev), flu.clone().to(dev)
+    gb.gamer_poisson_sor_gravity(p3, rho_p.to(dev), None, f3, dt, dh, coeff, om, nit)
+    torch.cuda.synchronize()
+    assert torch.equal(p1, p2) and torch.equal(acc1, acc2) and torch.equal(f1, f2) and torch.equal(f1, f3)
+    scale = np.abs(ref).max(axis=(0, 2, 3, 4), keepdims=True)
+    assert (np.abs(f1.cpu().numpy() - ref) / scale).max() <= tol
+    assert torch.equal(f1[:, 0], flu[:, 0].to(dev)) and torch.equal(f1[:, 5], flu[:, 5].to(dev))      # density, scalar untouched
+    assert (f1[:, 1:5] - flu[:, 1:5].to(dev)).abs().max().item() > 1e-3
+    # a kick and its opposite
+    gb.gamer_gravity_update(f2, acc2, -dt)
+    torch.cuda.synchronize()
+    assert ((f2.cpu() - flu).abs().max().item()) <= (1e-13 if dtype == torch.float64 else 1e-5) * flu.abs().max().item()
+    # n_patches must be whole groups
+    with pytest.raises(gb.GamerError):
+        gb.gamer_gravity_update(f2, acc2[:7].contiguous(), dt)
