@@ -53,8 +53,13 @@ template <typename T, int RECON, int NV, int TY, bool FUSED = false> struct CtuS
 
 // PLM/PPM face values of every variable of cell c along direction D, characteristic tracing over dt/2 (R7), revert of an
 // unphysical pair (R8), result as CONSERVED states in the rotated order of D: um at the lower face, up at the upper one.
-template <typename T, int RECON, int NV, bool EXT, int PLN, int D>
-__device__ __forceinline__ void ctu_trace(const T* const* Pz, int c, T* um, T* up, const Phys<T>& ph, Counters& cnt) {
+// CARRY (z direction, PPM, slopes limited in primitive variables): the thread traces plane after plane of its own column,
+// so of the three limited slopes a plane needs two were computed for the plane below.  cs0 / csp hold the slopes of the
+// cells at planes p and p+1 (rotated order) from the last call: 0 = none yet (compute all three, fill them), 1 = use them
+// as the slopes of p-1 and p, compute only the one of p+1 (one shared-memory load per variable less, too).
+template <typename T, int RECON, int NV, bool EXT, int PLN, int D, int CARRY = -1>
+__device__ __forceinline__ void ctu_trace(const T* const* Pz, int c, T* um, T* up, const Phys<T>& ph, Counters& cnt,
+                                          T* cs0 = nullptr, T* csp = nullptr) {
     constexpr int R = RECON == PPM ? 2 : 1;
     T Wr[NV], rm[NV], rp[NV], tm[NV], tp[NV];
     if (EXT && ph.char_limit) {      // slopes limited in characteristic variables (R22): all variables together
@@ -78,7 +83,22 @@ __device__ __forceinline__ void ctu_trace(const T* const* Pz, int c, T* um, T* u
             else if (D == 1) face_values<T, RECON, EXT, fixed_theta(EXT, RECON)>(q, NP, rm[k], rp[k], ph);
             else {
                 const int o = v * PLN + c;
-                if (RECON == PPM)
+                if (RECON == PPM && CARRY >= 0) {
+                    const T l1 = Pz[R - 1][o], r1 = Pz[R + 1][o], r2 = Pz[2 * R][o];
+                    T sm, s0;
+                    if (CARRY == 0) {
+                        const T l2 = Pz[0][o];
+                        sm = limited_slope<T, EXT, fixed_theta(EXT, RECON)>(l1 - l2, Wr[k] - l1, ph);
+                        s0 = limited_slope<T, EXT, fixed_theta(EXT, RECON)>(Wr[k] - l1, r1 - Wr[k], ph);
+                    } else {
+                        sm = cs0[k];
+                        s0 = csp[k];
+                    }
+                    const T sp = limited_slope<T, EXT, fixed_theta(EXT, RECON)>(r1 - Wr[k], r2 - r1, ph);
+                    ppm_faces<T>(l1, Wr[k], r1, sm, s0, sp, rm[k], rp[k]);
+                    cs0[k] = s0;
+                    csp[k] = sp;
+                } else if (RECON == PPM)
                     face_values5<T, RECON, EXT>(Pz[0][o], Pz[R - 1][o], Pz[R][o], Pz[R + 1][o], Pz[2 * R][o], rm[k], rp[k], ph);
                 else
                     face_values5<T, RECON, EXT>(T(0), Pz[R - 1][o], Pz[R][o], Pz[R + 1][o], T(0), rm[k], rp[k], ph);
@@ -236,11 +256,16 @@ __global__ void __launch_bounds__((CtuSmem<T, RECON, NV, TY, FUSED>::NT), 1) ctu
     T cxm[NV], cym[NV];        // corrected x-, y- of plane kk-1
 #pragma unroll
     for (int v = 0; v < NV; ++v) { zmT[v] = zpT[v] = czp[v] = cxm[v] = cym[v] = T(1); hlo[v] = fzlo[v] = T(0); }
+    // z slopes carried from plane to plane (fast kernels; the extended ones may limit in characteristic variables)
+    constexpr bool ZC = RECON == PPM && !EXT;
+    T zs0[NV], zsp[NV];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) zs0[v] = zsp[v] = T(0);
     if (plus) {                // z trace of plane -1
         const T* Pz[2 * R + 1];
 #pragma unroll
         for (int m = 0; m <= 2 * R; ++m) Pz[m] = prim + slot(-1 - R + m);
-        ctu_trace<T, RECON, NV, EXT, PLN, 2>(Pz, c, zmT, zpT, ph, cnt);
+        ctu_trace<T, RECON, NV, EXT, PLN, 2, ZC ? 0 : -1>(Pz, c, zmT, zpT, ph, cnt, zs0, zsp);
     }
 
 #pragma unroll 1
@@ -253,7 +278,7 @@ __global__ void __launch_bounds__((CtuSmem<T, RECON, NV, TY, FUSED>::NT), 1) ctu
             const T* Pz[2 * R + 1];
 #pragma unroll
             for (int m = 0; m <= 2 * R; ++m) Pz[m] = prim + slot(kk + 1 - R + m);
-            ctu_trace<T, RECON, NV, EXT, PLN, 2>(Pz, c, zmN, zpN, ph, cnt);
+            ctu_trace<T, RECON, NV, EXT, PLN, 2, ZC ? 1 : -1>(Pz, c, zmN, zpN, ph, cnt, zs0, zsp);
             ctu_solve<T, SOLVER, NV, 2>(zpT, zmN, hhi, ph, cnt);
         }
         if (cell && (mid || plus)) {      // planes -1 and 16 feed the z correction of interior cells only: no corners

@@ -142,6 +142,25 @@ __device__ __forceinline__ T limited_slope(T dL, T dR, const Phys<T>& ph) {
 // compile-time theta of the fast (non-extended) kernels: the 11-argument defaults, theta = 1 (PLM) / 2 (PPM)
 __host__ __device__ constexpr int fixed_theta(bool ext, int recon) { return ext ? 0 : (recon == PLM ? 1 : 2); }
 
+// PPM face values of a cell from its value c, its neighbours l1, r1 and the limited slopes sm, s0, sp of the three cells
+// (Colella & Woodward 1984 eqs. 1.6, 1.10)
+template <typename T>
+__device__ __forceinline__ void ppm_faces(T l1, T c, T r1, T sm, T s0, T sp, T& wm, T& wp) {
+    const T sixth = T(1.0 / 6.0);
+    const T m = T(0.5) * (l1 + c) - (s0 - sm) * sixth;
+    const T p = T(0.5) * (c + r1) - (sp - s0) * sixth;
+    // Monotonisation (CW84 eq. 1.10) written without branches.  With dm = c - m, dp = p - c:
+    //   (p-c)(c-m) <= 0                      <=>  dm, dp of opposite sign (or one is 0)  ->  dm = dp = 0
+    //   (p-m)(c-(m+p)/2) >  (p-m)^2/6        <=>  |dm| > 2|dp|                            ->  dm = 2 dp
+    //   (p-m)(c-(m+p)/2) < -(p-m)^2/6        <=>  |dp| > 2|dm|                            ->  dp = 2 dm
+    // i.e. dm <- sign * min(|dm|, 2|dp|), dp <- sign * min(|dp|, 2|dm|), both 0 for opposite signs.
+    const T dm = c - m, dp = p - c;
+    const T am = Ops<T>::minabs_same_sign(dm, dp + dp);
+    const T ap = Ops<T>::minabs_same_sign(dp, dm + dm);
+    wm = c - Ops<T>::copysign(am, dm);
+    wp = c + Ops<T>::copysign(ap, dp);
+}
+
 // face values of the centre cell of a strip: q points at the centre, neighbours at q[+-s], q[+-2s]
 template <typename T, int RECON, bool EXT, int THETA = 0>
 __device__ __forceinline__ void face_values(const T* q, int s, T& wm, T& wp, const Phys<T>& ph) {
@@ -155,19 +174,7 @@ __device__ __forceinline__ void face_values(const T* q, int s, T& wm, T& wp, con
         const T sm = limited_slope<T, EXT, THETA>(l1 - l2, c - l1, ph);
         const T s0 = limited_slope<T, EXT, THETA>(c - l1, r1 - c, ph);
         const T sp = limited_slope<T, EXT, THETA>(r1 - c, r2 - r1, ph);
-        const T sixth = T(1.0 / 6.0);
-        const T m = T(0.5) * (l1 + c) - (s0 - sm) * sixth;
-        const T p = T(0.5) * (c + r1) - (sp - s0) * sixth;
-        // Monotonisation (CW84 eq. 1.10) written without branches.  With dm = c - m, dp = p - c:
-        //   (p-c)(c-m) <= 0                      <=>  dm, dp of opposite sign (or one is 0)  ->  dm = dp = 0
-        //   (p-m)(c-(m+p)/2) >  (p-m)^2/6        <=>  |dm| > 2|dp|                            ->  dm = 2 dp
-        //   (p-m)(c-(m+p)/2) < -(p-m)^2/6        <=>  |dp| > 2|dm|                            ->  dp = 2 dm
-        // i.e. dm <- sign * min(|dm|, 2|dp|), dp <- sign * min(|dp|, 2|dm|), both 0 for opposite signs.
-        const T dm = c - m, dp = p - c;
-        const T am = Ops<T>::minabs_same_sign(dm, dp + dp);
-        const T ap = Ops<T>::minabs_same_sign(dp, dm + dm);
-        wm = c - Ops<T>::copysign(am, dm);
-        wp = c + Ops<T>::copysign(ap, dp);
+        ppm_faces<T>(l1, c, r1, sm, s0, sp, wm, wp);
     }
 }
 
