@@ -62,7 +62,8 @@ enum {
                                  unknown enum, misaligned pointer                                  */
     GAMER_EUNSUPPORTED = -2,  /* valid arguments, combination not built                            */
     GAMER_ECUDA = -3,         /* CUDA runtime / launch error (cudaGetLastError)                    */
-    GAMER_EUNPHYSICAL = -4    /* gamer_fluid_advance_retry only: remedy (v) of L108 gave up at dt_min */
+    GAMER_EUNPHYSICAL = -4,   /* gamer_fluid_advance_retry only: remedy (v) of L108 gave up at dt_min */
+    GAMER_ETOOLARGE = -5      /* gamer_fluid_advance_table_noalloc only: the batch exceeds the static scratch array */
 };
 
 /* Everything the 11-argument form fixes by default.  Zero-initialise, then set what you need. */
@@ -272,6 +273,28 @@ int gamer_fluid_advance_host_resident(const void* u_host, const int32_t* nbr_hos
                                       double dt, double dh, double gamma,
                                       int scheme, int recon, int riemann, int precision,
                                       const gamer_opts* opts /* nullable */);
+
+/* Allocation-free step from the UNPADDED state, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid allocation): u[n_groups][NVAR][16][16][16] and the same-level table nbr[n_groups][27]
+ * (device int32, as in gamer_fluid_advance_resident: every entry in [0, n_groups)) in, out / flux_out as everywhere.  The
+ * padded batch that gamer_refresh_ghosts_table + gamer_fluid_advance_ex need as caller-allocated scratch lives here in a
+ * file-scope static device array of GAMER_NOALLOC_SCRATCH_BYTES (64 MiB; every GPU that loads the library holds it until the
+ * process exits): the call runs those same two kernels on it -- results are bit-identical to that pair -- and calls no
+ * cudaMalloc, cudaFree or allocating library routine.  Because the padded slab stays in memory, remedy_first_order (remedy
+ * (ii), which gamer_fluid_advance_resident cannot offer) works.  All opts as gamer_fluid_advance_ex; work is enqueued on
+ * opts->stream, nothing synchronises.
+ * Limit: n_groups <= gamer_noalloc_max_groups(NVAR, precision) = 64 MiB / (NVAR * 22^3 * sizeof(real)) -- 315 groups in fp32
+ * and 157 in fp64 at NVAR = 5; more returns GAMER_ETOOLARGE and enqueues nothing.
+ * ALL CALLS SHARE THE ONE ARRAY per GPU: two calls that overlap on the GPU (different streams, different host threads) race
+ * on it; order them on one stream or with events.  The array keeps the last call's contents, so the part a call uses is
+ * cleared first: a slab whose table entry is -1 (no same-level neighbour; the allocating path leaves it for the caller's
+ * interpolation) is zero here, and cells that depend on it come out non-finite, the same way on every call. */
+#define GAMER_NOALLOC_SCRATCH_BYTES (64u << 20)
+int gamer_fluid_advance_table_noalloc(const void* u, const int32_t* nbr, void* out, void* flux_out, int64_t n_groups,
+                                      double dt, double dh, double gamma,
+                                      int scheme, int recon, int riemann, int precision,
+                                      const gamer_opts* opts /* nullable */);
+int64_t gamer_noalloc_max_groups(int nvar, int precision);
 
 void gamer_release_scratch(void);
 

@@ -23,7 +23,7 @@ LIB_PATH = os.path.join(_HERE, "libgamerhydro.so")
 EXPORTS = ["gamer_fluid_advance", "gamer_fluid_advance_ex", "gamer_fluid_advance_retry", "gamer_cfl_dt", "gamer_cfl_dt_ex",
            "gamer_cfl_from_group_speed", "gamer_refresh_ghosts_periodic", "gamer_refresh_ghosts", "gamer_refresh_ghosts_table", "gamer_interpolate_ghosts", "gamer_fluid_advance_resident",
            "gamer_neighbors_periodic", "gamer_restrict", "gamer_flux_accumulate", "gamer_flux_correct",
-           "gamer_poisson_sor", "gamer_poisson_sor_gravity", "gamer_gravity_update", "gamer_fluid_advance_host", "gamer_fluid_advance_host_resident", "gamer_release_scratch", "gamer_alu_peak",
+           "gamer_poisson_sor", "gamer_poisson_sor_gravity", "gamer_gravity_update", "gamer_fluid_advance_host", "gamer_fluid_advance_host_resident", "gamer_release_scratch", "gamer_alu_peak", "gamer_fluid_advance_table_noalloc", "gamer_noalloc_max_groups",
            "gamer_launch_count", "gamer_strerror", "gamer_version"]
 
 
@@ -89,6 +89,9 @@ def lib():
                                                ctypes.POINTER(gamer_opts)]
         L.gamer_fluid_advance_host_resident.argtypes = [vp, vp, vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, ci, ci,
                                                         ctypes.POINTER(gamer_opts)]
+        L.gamer_fluid_advance_table_noalloc.argtypes = [vp, vp, vp, vp, i64, dbl, dbl, dbl, ci, ci, ci, ci, ctypes.POINTER(gamer_opts)]
+        L.gamer_noalloc_max_groups.argtypes = [ci, ci]
+        L.gamer_noalloc_max_groups.restype = ctypes.c_int64
         L.gamer_alu_peak.argtypes = [ci, ctypes.POINTER(dbl), ctypes.POINTER(dbl), vp]
         L.gamer_launch_count.restype = ctypes.c_int64
         L.gamer_strerror.restype = ctypes.c_char_p
@@ -251,6 +254,23 @@ def gamer_fluid_advance_resident(u, nbr, out, flux_out, dt, dh, gamma, scheme, r
     _check(lib().gamer_fluid_advance_resident(_ptr(u), _ptr(nbr), _ptr(out), _ptr(flux_out), u.shape[0], float(dt), float(dh),
                                               float(gamma), int(scheme), int(recon), int(riemann), _precision(u),
                                               ctypes.byref(opts)), "gamer_fluid_advance_resident")
+
+
+def gamer_noalloc_max_groups(nvar, precision):
+    return int(lib().gamer_noalloc_max_groups(int(nvar), int(precision)))
+
+
+def gamer_fluid_advance_table_noalloc(u, nbr, out, flux_out, dt, dh, gamma, scheme, recon, riemann, opts=None):
+    """Allocation-free step from the unpadded state + neighbour table: the padded batch lives in the library's static
+    64 MiB device array (GAMER_ETOOLARGE = -5 beyond gamer_noalloc_max_groups); overlapping calls race on it."""
+    if nbr.dtype != torch.int32 or tuple(nbr.shape) != (u.shape[0], 27):
+        raise GamerError("nbr must be an int32 tensor of shape [n_groups, 27]")
+    if opts is None:
+        opts = make_opts(n_scalar=u.shape[1] - 5)
+    _check_batch(u, out, flux_out, opts, False)
+    _check(lib().gamer_fluid_advance_table_noalloc(_ptr(u), _ptr(nbr), _ptr(out), _ptr(flux_out), u.shape[0], float(dt), float(dh),
+                                                   float(gamma), int(scheme), int(recon), int(riemann), _precision(u),
+                                                   ctypes.byref(opts)), "gamer_fluid_advance_table_noalloc")
 
 
 def gamer_neighbors_periodic(gz, gy, gx, device, stream=None):

@@ -51,7 +51,7 @@ def build(force=False, verbose=False):
                 if verbose:
                     cmd += ["-Xptxas", "-v"]
                 jobs.append((cmd + ["-c", os.path.join(CSRC, "inst.cu"), "-o", o], o))
-    for unit in ("api", "alu_peak"):
+    for unit in ("api", "alu_peak", "noalloc"):
         o = os.path.join(OBJ, unit + ".o")
         jobs.append(([NVCC, *FLAGS, "-c", os.path.join(CSRC, unit + ".cu"), "-o", o], o))
     with concurrent.futures.ThreadPoolExecutor(max_workers=os.cpu_count() or 4) as ex:

@@ -698,6 +698,7 @@ extern "C" const char* gamer_strerror(int code) {
     case GAMER_EUNSUPPORTED: return "unsupported combination or size";
     case GAMER_ECUDA: return "CUDA runtime or launch error";
     case GAMER_EUNPHYSICAL: return "unphysical cells remain at the minimum time-step";
+    case GAMER_ETOOLARGE: return "batch exceeds the static scratch array of the allocation-free entry";
     default: return "unknown error code";
     }
 }
