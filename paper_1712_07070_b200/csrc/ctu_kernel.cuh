@@ -188,22 +188,28 @@ __global__ void __launch_bounds__((CtuSmem<T, RECON, NV, TY, FUSED>::NT), 1) ctu
 
     // ---- the cell column this thread owns.  Interior cells first, a warp holding rows w and w + TY/2 (its two 16-lane
     // halves then fall in disjoint shared-memory banks: 8 x 22 words = 16 mod 32); then the two x-halo columns
-    // (ci = -1, 16; stride 22 words: 16 lanes on 16 different banks), then the two y-halo rows.  Halo warps skip what only
+    // (ci = -1, 16, interleaved row by row), then the two y-halo rows.  Halo warps skip what only
     // interior cells do (final z solve, update) instead of idling through it in every warp.
     constexpr int NI = PS * TY, NXH = 2 * (TY + 2);
-    const bool cell = tid < NC;
+    // the x-halo threads get whole warps when the CTA has spare threads for it, so that the y-halo rows start a warp
+    constexpr int XS = (NI + (NXH + 31) / 32 * 32 + 2 * PS <= NT) ? (NXH + 31) / 32 * 32 : NXH;
+    bool cell = true;
     int ci = 0, cj = 0;
     if (tid < NI) {
         ci = tid & 15;
         cj = (tid >> 5) + ((tid >> 4) & 1) * (TY / 2);
-    } else if (tid < NI + NXH) {
-        const int u = tid - NI;
-        ci = u < TY + 2 ? -1 : PS;
-        cj = (u < TY + 2 ? u : u - (TY + 2)) - 1;
-    } else if (cell) {
-        const int u = tid - NI - NXH;
+    } else if (tid < NI + XS) {
+        const int u = tid - NI;      // the two columns interleaved: a quarter-warp holds 4 rows x 2 columns, whose 16-byte exchange
+        ci = (u & 1) ? PS : -1;      // entries (row stride 18 Vec4 = 8 banks, column offset 17 Vec4 = 4 banks) and whose
+        cj = (u >> 1) - 1;           // primitive cells (row stride 22 words, column offset 17) fall on distinct banks
+        cell = u < NXH;
+        if (!cell) { ci = 0; cj = 0; }
+    } else if (tid < NI + XS + 2 * PS) {
+        const int u = tid - NI - XS;
         ci = u & 15;
         cj = u < PS ? -1 : TY;
+    } else {
+        cell = false;
     }
     const bool rowin = cell && cj >= 0 && cj < TY, colin = cell && ci >= 0 && ci < PS;
     const bool inner = rowin && colin;

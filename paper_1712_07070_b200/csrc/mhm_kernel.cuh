@@ -112,7 +112,7 @@ __device__ __forceinline__ void mhm_face_states(const T* const* Pz, const Phys<T
     }
 }
 
-// Hancock half step of one conserved face state: Ue = Uf - hdU (hdU = dt/(2 dh) * dU, or 0 in the reverting pass,
+// Hancock half step of one conserved face state: Ue = Uf - hl * dU (hl = dt/(2 dh), or 0 in the reverting pass,
 // where the un-evolved face values are taken as they are); returns whether rho and P of the result are positive.
 // The evolved state stays in conserved variables all the way to the Riemann solver, which derives the velocities,
 // P and H it needs from them with one reciprocal (make_side_cons): no conserved -> primitive -> conserved round
@@ -121,9 +121,9 @@ __device__ __forceinline__ void mhm_face_states(const T* const* Pz, const Phys<T
 // Every thread evolves all six states of its cell, also the ones it hands to no Riemann solver: any bad state
 // reverts the cell (R6) and the halo copy of a cell must decide exactly as its owner in the neighbouring group does.
 template <typename T, int NV, bool EXT>
-__device__ __forceinline__ bool mhm_evolve(const T* Uf, const T* hdU, T* Ue, bool floors, const Phys<T>& ph) {
+__device__ __forceinline__ bool mhm_evolve(const T* Uf, const T* dU, T hl, T* Ue, bool floors, const Phys<T>& ph) {
 #pragma unroll
-    for (int v = 0; v < NV; ++v) Ue[v] = Uf[v] - hdU[v];
+    for (int v = 0; v < NV; ++v) Ue[v] = Uf[v] - hl * dU[v];      // one FMA per component
     if (EXT && ph.floors && floors) {
         T We[NV];
         cons2prim<T, NV>(Ue, We, ph);
@@ -368,33 +368,32 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED, VLS>::N
             for (int pass = VLS ? 1 : 0; pass < 2; ++pass) {      // VL: plain face values of the half-step state, nothing to evolve
                 T Uf[3][2][NV], dU[NV], Ue[NV];
                 mhm_face_states<T, RECON, NV, EXT, PLN>(Pz, ph, Uf, dU);
-#pragma unroll
-                for (int v = 0; v < NV; ++v) dU[v] = pass ? T(0) : ph.hlam * dU[v];
+                const T hl = pass ? T(0) : ph.hlam;
                 const bool fl_ok = pass == 0;
-                bool ok = mhm_evolve<T, NV, EXT>(Uf[0][1], dU, Ue, fl_ok, ph);
+                bool ok = mhm_evolve<T, NV, EXT>(Uf[0][1], dU, hl, Ue, fl_ok, ph);
                 if (mid && pub_x) {
                     T rot[NV];
 #pragma unroll
                     for (int k = 0; k < NV; ++k) rot[k] = Ue[nat_index(0, k)];
                     put_state<T, NV>(st_x, G::NSX, c.sx_own + 1, rot);
                 }
-                ok = mhm_evolve<T, NV, EXT>(Uf[1][1], dU, Ue, fl_ok, ph) && ok;
+                ok = mhm_evolve<T, NV, EXT>(Uf[1][1], dU, hl, Ue, fl_ok, ph) && ok;
                 if (mid && pub_y) {
                     T rot[NV];
 #pragma unroll
                     for (int k = 0; k < NV; ++k) rot[k] = Ue[nat_index(1, k)];
                     put_state<T, NV>(st_y, G::NSY, c.sy_own + 16, rot);
                 }
-                ok = mhm_evolve<T, NV, EXT>(Uf[0][0], dU, Ue, fl_ok, ph) && ok;
+                ok = mhm_evolve<T, NV, EXT>(Uf[0][0], dU, hl, Ue, fl_ok, ph) && ok;
 #pragma unroll
                 for (int k = 0; k < NV; ++k) xminus[k] = Ue[nat_index(0, k)];
-                ok = mhm_evolve<T, NV, EXT>(Uf[1][0], dU, Ue, fl_ok, ph) && ok;
+                ok = mhm_evolve<T, NV, EXT>(Uf[1][0], dU, hl, Ue, fl_ok, ph) && ok;
 #pragma unroll
                 for (int k = 0; k < NV; ++k) yminus[k] = Ue[nat_index(1, k)];
-                ok = mhm_evolve<T, NV, EXT>(Uf[2][0], dU, Ue, fl_ok, ph) && ok;
+                ok = mhm_evolve<T, NV, EXT>(Uf[2][0], dU, hl, Ue, fl_ok, ph) && ok;
 #pragma unroll
                 for (int k = 0; k < NV; ++k) zminus[k] = Ue[nat_index(2, k)];
-                ok = mhm_evolve<T, NV, EXT>(Uf[2][1], dU, Ue, fl_ok, ph) && ok;
+                ok = mhm_evolve<T, NV, EXT>(Uf[2][1], dU, hl, Ue, fl_ok, ph) && ok;
 #pragma unroll
                 for (int k = 0; k < NV; ++k) znew[k] = Ue[nat_index(2, k)];
                 if (ok || pass) break;
