@@ -34,7 +34,10 @@ template <typename T, int RECON, int NV, int TY, int NSTG = 2, bool FUSED = fals
     static constexpr int NCV = NT - NI;                         // threads that convert planes
     static constexpr int NTILE = PS / TY;
     static constexpr int NR = TY + 2 * NGH, PLN = NR * NP;      // staged plane
-    static constexpr int NSX = 17 * TY, NSY = 16 * (TY + 1);    // x+ states / x fluxes, y+ states / y fluxes
+    // row stride of the exchange arrays: 18 entries (17 x faces / 16 y faces used).  A warp holds rows w and w + TY/2; with
+    // 8 * 18 = 16 mod 32 the scalar fifth components of its two half-warps fall on disjoint banks (17 and 16 gave 2-way conflicts)
+    static constexpr int SW = 18;
+    static constexpr int NSX = (SW * TY + 3) / 4 * 4, NSY = (SW * (TY + 1) + 3) / 4 * 4;     // x+ states / x fluxes, y+ states / y fluxes
     static constexpr int BLK = (NSX + NSY) * NV;                // one buffer of states (or of fluxes)
     static constexpr int RSTG = NV * (FUSED ? NR * FW : PLN);   // one landing stage (fused refresh: 24-wide rows)
     static constexpr int RAW = 0;                               // [NSTG][RSTG]  TMA / cp.async landing stages
@@ -267,8 +270,8 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED, VLS>::N
     const int gj = j0 + ej;
     MhmCell<T> c;
     c.cidx = (ej + NGH) * NP + (ei + NGH);
-    c.sx_own = ej * 17 + ei;
-    c.sy_own = ej * 16 + ei;
+    c.sx_own = ej * G::SW + ei;
+    c.sy_own = ej * G::SW + ei;
     c.gin_off = NGH * (NP * NP) + (gj + NGH) * NP + (ei + NGH);
     c.out_off = gj * PS + ei;
     T* gout = a.out + (size_t)g * NV * (PS * PSQ);
@@ -382,7 +385,7 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED, VLS>::N
                     T rot[NV];
 #pragma unroll
                     for (int k = 0; k < NV; ++k) rot[k] = Ue[nat_index(1, k)];
-                    put_state<T, NV>(st_y, G::NSY, c.sy_own + 16, rot);
+                    put_state<T, NV>(st_y, G::NSY, c.sy_own + G::SW, rot);
                 }
                 ok = mhm_evolve<T, NV, EXT>(Uf[0][0], dU, hl, Ue, fl_ok, ph) && ok;
 #pragma unroll
@@ -481,13 +484,13 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED, VLS>::N
                 T* q;
                 if (f < NXF) {
                     const int p = f / TY, j = f - p * TY;
-                    get_state<T, NV>(pl_x, G::NSX, j * 17 + 8 * p, fn);
+                    get_state<T, NV>(pl_x, G::NSX, j * G::SW + 8 * p, fn);
                     q = gflux + ((0 * 3 + p) * NV) * PSQ + (kk - 1) * PS + (j0 + j);
                 } else {
                     const int h = f - NXF, r = h >> 4, i = h & 15;
                     const int j = yrow0 + 8 * r;
                     if (j > TY) continue;
-                    get_state<T, NV>(pl_y, G::NSY, j * 16 + i, fn);
+                    get_state<T, NV>(pl_y, G::NSY, j * G::SW + i, fn);
                     q = gflux + ((1 * 3 + ((j0 + j) >> 3)) * NV) * PSQ + (kk - 1) * PS + i;
                 }
 #pragma unroll
@@ -502,7 +505,7 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED, VLS>::N
             get_state<T, NV>(pl_x, G::NSX, c.sx_own, fl);
             get_state<T, NV>(pl_x, G::NSX, c.sx_own + 1, fr);
             get_state<T, NV>(pl_y, G::NSY, c.sy_own, fd);
-            get_state<T, NV>(pl_y, G::NSY, c.sy_own + 16, fu);
+            get_state<T, NV>(pl_y, G::NSY, c.sy_own + G::SW, fu);
 #pragma unroll
             for (int v = 0; v < NV; ++v)
                 U[v] = U[v] - ph.lam * (((fr[v] - fl[v]) + (fu[v] - fd[v])) + (fzn[v] - fzl[v]));
