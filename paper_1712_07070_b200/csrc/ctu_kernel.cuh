@@ -212,7 +212,8 @@ __global__ void __launch_bounds__((CtuSmem<T, RECON, NV, TY, FUSED>::NT), 1) ctu
         cell = false;
     }
     const bool rowin = cell && cj >= 0 && cj < TY, colin = cell && ci >= 0 && ci < PS;
-    const bool inner = rowin && colin;
+    // interior cells fill whole warps (NI is a multiple of 32): the flag through a warp vote is a uniform predicate
+    const bool inner = __all_sync(0xffffffffu, tid < NI);
     const bool plus = rowin || colin;                                // not a corner: its z states are needed
     const bool facex = cell && ci >= 0, facey = cell && cj >= 0;     // has a lower x / y face among the 18 x (TY+2) cells
     const int c = (cj + NGH) * NP + (ci + NGH);                      // the cell inside a staged plane

@@ -247,7 +247,9 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED, VLS>::N
 
     // ---- role of this thread: cell (ei, ej) of the tile, ei in -1..16, ej in -1..TY
     // role: 0 = interior, 1 = x-low, 2 = x-high, 4 = y-low, 8 = y-high, 16 = padding thread (conversion only)
-    const bool interior = tid < NI;
+    // NI is a multiple of 32: a warp is all interior or all halo.  Taking the flag through a warp vote tells the compiler so
+    // (uniform predicate, plain branches without convergence barriers around the role-dependent blocks).
+    const bool interior = __all_sync(0xffffffffu, tid < NI);
     int ei = 0, ej = 0, role = 16;
     if (interior) {
         // a warp holds rows w and w + TY/2: the two 16-lane halves then fall in disjoint shared-memory banks
