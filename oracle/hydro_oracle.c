@@ -37,9 +37,15 @@
  * Pins (tests/test_oracle_*.py): exact Riemann solution of Sod's tube, closed-form fluxes,
  * Roe identities, conservation on a periodic box, uniform-state invariance, x/y/z permutation
  * and mirror symmetry, 1-D reduction, exact reproduction of linear / parabolic data, single-wave
- * characteristic tracing, ghost-footprint, dual-energy / floor closed forms, CFL closed forms.
- * Parity unpinned: none of the functions exported here (the hybrid limiter, characteristic-
- * variable limiting and remedy (iii) are not implemented at all).
+ * characteristic tracing, ghost-footprint, dual-energy / floor closed forms, CFL closed forms;
+ * CTU transverse correction: 3-D contact advection against the 6-solve scheme written out, cells
+ * rebuilt from the pinned building blocks, second-order diagonal advection; PPM overshoot branches:
+ * hand-computed cases (both copies); characteristic limiting: R . limiter(L dW) with eigenvectors
+ * written out from the literature; VL scheme: contact-advection closed form, cell rebuilt from
+ * single-face solves; passive scalars: per-species conservation, bitwise independence, closed-form
+ * renormalisation (DESIGN.md section 2 lists which test kills which mutation).
+ * Parity unpinned: none of the functions exported here (the hybrid limiter and remedy (iii) are
+ * not implemented at all).
  */
 #include <math.h>
 #include <stdint.h>
