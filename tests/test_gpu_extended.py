@@ -255,7 +255,9 @@ def test_config3_two_level_sedov_flux_correction(dev, oracle_mod):
                                                     (gb.MHM, gb.PLM, gb.HLLE, dict(n_scalar=1, dual_energy=True, min_pres=1e-12)),
                                                     (gb.CTU, gb.PPM, gb.HLLC, {}), (gb.CTU, gb.PLM, gb.ROE, {}),
                                                     (gb.CTU, gb.PPM, gb.HLLE, dict(n_scalar=1, dual_energy=True, min_pres=1e-12)),
-                                                    (gb.VL, gb.PLM, gb.HLLC, {}), (gb.VL, gb.PLM, gb.ROE, dict(n_scalar=1, dual_energy=True, min_pres=1e-12))])
+                                                    (gb.VL, gb.PLM, gb.HLLC, {}), (gb.VL, gb.PLM, gb.ROE, dict(n_scalar=1, dual_energy=True, min_pres=1e-12)),
+                                                    (gb.CTU, gb.PPM, gb.HLLC, dict(n_scalar=3, renormalize=True)),
+                                                    (gb.MHM, gb.PPM, gb.ROE, dict(n_scalar=2))])
 def test_fused_ghost_refresh_entry_matches_the_padded_path(dev, scheme, recon, solver, kw, dtype):
     """SURVEY 8(f) NEXT-1, second half: gamer_fluid_advance_resident gathers the ghost zones from the neighbours'
     unpadded state inside the solver.  On a periodic 2 x 3 x 4 box of groups (so that -1 and +1 neighbours coincide
@@ -266,6 +268,10 @@ def test_fused_ghost_refresh_entry_matches_the_padded_path(dev, scheme, recon, s
     the neighbour table must be the periodic one."""
     gz, gy, gx = 2, 3, 4
     f = inputs.turbulence_field(16, 4242, kmax=4, gamma=G53, shape=(gz * 16, gy * 16, gx * 16), entropy=bool(kw.get("n_scalar")))
+    if kw.get("n_scalar", 0) > 1:      # species: smooth positive partial densities
+        extra = [f[0] * (0.2 + 0.1 * k + 0.05 * torch.sin(6.283185307179586 * (k + 1) * torch.arange(f.shape[-1], dtype=torch.float64) / f.shape[-1]))
+                 for k in range(kw["n_scalar"])]
+        f = torch.cat([f[:5], torch.stack([e.expand_as(f[0]).contiguous() for e in extra])], dim=0)
     padded = inputs.pack_periodic(f).to(dtype).to(dev)
     u = inputs.interior(padded).contiguous()
     dt, dh = 0.004, 1.0 / 64
