@@ -78,7 +78,7 @@ class ClockSampler(threading.Thread):
                 reasons = nv.nvmlDeviceGetCurrentClocksEventReasons(h) if hasattr(nv, "nvmlDeviceGetCurrentClocksEventReasons") \
                     else nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
                 self.samples.append((float(mhz), int(reasons)))
-                time.sleep(0.02)
+                time.sleep(0.01)
         except Exception as e:       # no NVML: report nothing rather than guess
             self.error = repr(e)
 

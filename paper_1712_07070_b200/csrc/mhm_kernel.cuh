@@ -64,6 +64,13 @@ template <typename T, int RECON, int NV, int TY, int NSTG = 2, bool FUSED = fals
 // ---------------------------------------------------------------------------------------------
 // Face values of one cell in all three directions -> conserved face states Uf[d][s] and the sum over d of
 // F_d(W+) - F_d(W-).  Pz[m] points at variable 0 of this cell in the primitive plane kk-R+m.
+// Packed form (fp32, Blackwell fma.rn.f32x2): the minus and plus state of one direction evolved and tested together,
+// two FMAs per instruction.  Same arithmetic per lane as mhm_evolve.
+__device__ __forceinline__ uint64_t pk2(float a, float b) { uint64_t r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b)); return r; }
+__device__ __forceinline__ void upk2(uint64_t r, float& a, float& b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(r)); }
+__device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c) { uint64_t r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
+__device__ __forceinline__ uint64_t mul2(uint64_t a, uint64_t b) { uint64_t r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+
 template <typename T, int RECON, int NV, bool EXT, int PLN>
 __device__ __forceinline__ void mhm_face_states(const T* const* Pz, const Phys<T>& ph, T (&Uf)[3][2][NV], T (&dU)[NV]) {
     constexpr int R = RECON == PPM ? 2 : 1;
@@ -136,6 +143,24 @@ __device__ __forceinline__ bool mhm_evolve(const T* Uf, const T* dU, T hl, T* Ue
     }
     const T pe = Ue[0] * Ue[4] - T(0.5) * (Ue[1] * Ue[1] + Ue[2] * Ue[2] + Ue[3] * Ue[3]);
     return (Ue[0] > T(0)) && (pe > T(0));
+}
+
+// (packed helpers pk2 / upk2 / fma2 / mul2: above mhm_face_states)
+template <int NV>
+__device__ __forceinline__ bool mhm_evolve_pair(const float* UfA, const float* UfB, const float* dU, float hl, float* UeA, float* UeB) {
+    const uint64_t mh = pk2(-hl, -hl);
+    uint64_t e[NV];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) e[v] = fma2(mh, pk2(dU[v], dU[v]), pk2(UfA[v], UfB[v]));
+    uint64_t q = mul2(e[1], e[1]);
+    q = fma2(e[2], e[2], q);
+    q = fma2(e[3], e[3], q);
+    const uint64_t pe = fma2(pk2(-0.5f, -0.5f), q, mul2(e[0], e[4]));
+#pragma unroll
+    for (int v = 0; v < NV; ++v) upk2(e[v], UeA[v], UeB[v]);
+    float pa, pb;
+    upk2(pe, pa, pb);
+    return (UeA[0] > 0.f) && (UeB[0] > 0.f) && (pa > 0.f) && (pb > 0.f);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -375,7 +400,32 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED, VLS>::N
                 mhm_face_states<T, RECON, NV, EXT, PLN>(Pz, ph, Uf, dU);
                 const T hl = pass ? T(0) : ph.hlam;
                 const bool fl_ok = pass == 0;
-                bool ok = mhm_evolve<T, NV, EXT>(Uf[0][1], dU, hl, Ue, fl_ok, ph);
+                bool ok;
+                if constexpr (sizeof(T) == 4 && !EXT) {
+                    T Um[NV], Up[NV];
+                    ok = mhm_evolve_pair<NV>(Uf[0][0], Uf[0][1], dU, hl, Um, Up);
+                    if (mid && pub_x) {
+                        T rot[NV];
+#pragma unroll
+                        for (int k = 0; k < NV; ++k) rot[k] = Up[nat_index(0, k)];
+                        put_state<T, NV>(st_x, G::NSX, c.sx_own + 1, rot);
+                    }
+#pragma unroll
+                    for (int k = 0; k < NV; ++k) xminus[k] = Um[nat_index(0, k)];
+                    ok = mhm_evolve_pair<NV>(Uf[1][0], Uf[1][1], dU, hl, Um, Up) && ok;
+                    if (mid && pub_y) {
+                        T rot[NV];
+#pragma unroll
+                        for (int k = 0; k < NV; ++k) rot[k] = Up[nat_index(1, k)];
+                        put_state<T, NV>(st_y, G::NSY, c.sy_own + G::SW, rot);
+                    }
+#pragma unroll
+                    for (int k = 0; k < NV; ++k) yminus[k] = Um[nat_index(1, k)];
+                    ok = mhm_evolve_pair<NV>(Uf[2][0], Uf[2][1], dU, hl, Um, Up) && ok;
+#pragma unroll
+                    for (int k = 0; k < NV; ++k) { zminus[k] = Um[nat_index(2, k)]; znew[k] = Up[nat_index(2, k)]; }
+                } else {
+                ok = mhm_evolve<T, NV, EXT>(Uf[0][1], dU, hl, Ue, fl_ok, ph);
                 if (mid && pub_x) {
                     T rot[NV];
 #pragma unroll
@@ -401,6 +451,7 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED, VLS>::N
                 ok = mhm_evolve<T, NV, EXT>(Uf[2][1], dU, hl, Ue, fl_ok, ph) && ok;
 #pragma unroll
                 for (int k = 0; k < NV; ++k) znew[k] = Ue[nat_index(2, k)];
+                }
                 if (ok || pass) break;
                 cnt.reverted++;
             }
