@@ -102,6 +102,10 @@ template <> struct Ops<double> {
         const double m = fabs(fabs(a) < fabs(b) ? a : b);
         return (__double2hiint(a) ^ __double2hiint(b)) < 0 ? 0.0 : m;
     }
+    // minmod(a, b): the one of smaller magnitude (it carries the common sign), 0 for opposite signs
+    static __device__ __forceinline__ bool opposite(double a, double b) { return (__double2hiint(a) ^ __double2hiint(b)) < 0; }
+    static __device__ __forceinline__ double minmag(double a, double b) { return fabs(a) < fabs(b) ? a : b; }
+    static __device__ __forceinline__ double minmod(double a, double b) { return opposite(a, b) ? 0.0 : minmag(a, b); }
 };
 
 // run-time constants shared by every stage (kept in registers / constant bank)
@@ -167,6 +171,14 @@ __device__ __forceinline__ T limited_slope(T dL, T dR, const Phys<T>& ph) {
         if (ph.limiter == LIM_VANLEER) return T(2) * prod * Ops<T>::rcp(dL + dR);
         return prod * (dL + dR) * Ops<T>::rcp(dL * dL + dR * dR);
     }
+    if constexpr (sizeof(T) == 8) {
+        // fp64 has no min/max/abs/copysign instructions: every one of them is a compare + two selects or a pair of
+        // moves.  Signed form of the lines below, same values: the smaller of dL, dR carries the sign already, and
+        // the centred difference has it too
+        T sl = Ops<T>::minmod(dL, dR);
+        if (THETA == 2 || (THETA == 0 && ph.theta != T(1))) sl = Ops<T>::minmag(THETA == 2 ? sl + sl : ph.theta * sl, T(0.5) * (dL + dR));
+        return sl;
+    }
     T m = Ops<T>::minabs_same_sign(dL, dR);
     // theta == 1 (plain minmod): |dL+dR|/2 >= min(|dL|,|dR|) holds exactly in floating point for equal
     // signs (rounding is monotonic), so the centred term can never win and is skipped
@@ -191,6 +203,12 @@ __device__ __forceinline__ void ppm_faces(T l1, T c, T r1, T sm, T s0, T sp, T& 
     //   (p-m)(c-(m+p)/2) < -(p-m)^2/6        <=>  |dp| > 2|dm|                            ->  dp = 2 dm
     // i.e. dm <- sign * min(|dm|, 2|dp|), dp <- sign * min(|dp|, 2|dm|), both 0 for opposite signs.
     const T dm = c - m, dp = p - c;
+    if constexpr (sizeof(T) == 8) {      // signed form (see limited_slope): one sign test serves both faces
+        const bool opp = Ops<T>::opposite(dm, dp);
+        wm = c - (opp ? T(0) : Ops<T>::minmag(dm, dp + dp));
+        wp = c + (opp ? T(0) : Ops<T>::minmag(dp, dm + dm));
+        return;
+    }
     const T am = Ops<T>::minabs_same_sign(dm, dp + dp);
     const T ap = Ops<T>::minabs_same_sign(dp, dm + dm);
     wm = c - Ops<T>::copysign(am, dm);
