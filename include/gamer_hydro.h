@@ -267,7 +267,10 @@ int gamer_fluid_advance_host(const void* in_host, void* out_host, void* flux_out
  * CPU gather.  The call keeps a device copy of the whole state (n_groups x NVAR x 16 KB in fp32) plus three output chunks
  * between calls (gamer_release_scratch frees them), serialises callers on a mutex and synchronises before returning.
  * fp64 results are bit-identical to gamer_fluid_advance_resident.  Not with remedy_first_order (GAMER_EUNSUPPORTED);
- * opts->n_unphysical_out / diag_out / dt_dev set => GAMER_EUNSUPPORTED (device outputs belong to the device entries). */
+ * opts->n_unphysical_out / diag_out / dt_dev set => GAMER_EUNSUPPORTED (device outputs belong to the device entries).
+ * The table is walked on the host while the input copies are already in flight, and output chunks are launched in the order
+ * in which their inputs land; a table entry outside [0, n_groups) => GAMER_EINVAL once those copies have drained, with the
+ * host outputs untouched. */
 int gamer_fluid_advance_host_resident(const void* u_host, const int32_t* nbr_host, void* out_host, void* flux_out_host,
                                       void* group_speed_out_host, int64_t n_groups,
                                       double dt, double dh, double gamma,

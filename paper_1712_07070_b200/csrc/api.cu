@@ -623,22 +623,6 @@ extern "C" int gamer_fluid_advance_host_resident(const void* u_host, const int32
     const size_t u_g = (size_t)nv * PS * PS * PS * sz, fl_g = (size_t)9 * nv * PS * PS * sz;
     const int64_t chunk = n_groups < 1024 ? n_groups : 1024;      // input and output granularity
     const int64_t n_chunks = (n_groups + chunk - 1) / chunk;
-    // which input chunks each output chunk needs: those that hold one of its groups' 27 table entries
-    std::vector<std::vector<int>> need((size_t)n_chunks);
-    {
-        std::vector<char> mark((size_t)n_chunks);
-        for (int64_t k = 0; k < n_chunks; ++k) {
-            std::fill(mark.begin(), mark.end(), 0);
-            const int64_t g1 = (k + 1) * chunk < n_groups ? (k + 1) * chunk : n_groups;
-            for (int64_t i = k * chunk * 27; i < g1 * 27; ++i) {
-                const int32_t s = nbr_host[i];
-                if (s < 0 || s >= n_groups) return GAMER_EINVAL;
-                mark[(size_t)(s / chunk)] = 1;
-            }
-            for (int64_t c = 0; c < n_chunks; ++c)
-                if (mark[(size_t)c]) need[(size_t)k].push_back((int)c);
-        }
-    }
     constexpr int NBUF = ResidentScratch::NBUF;
     std::lock_guard<std::mutex> lock(g_resident.mu);
     ResidentScratch& R = g_resident;
@@ -654,9 +638,41 @@ extern "C" int gamer_fluid_advance_host_resident(const void* u_host, const int32
             cudaEventRecord(R.ev[(size_t)k], R.st_in) != cudaSuccess)
             return GAMER_ECUDA;
     }
+    // which input chunks each output chunk needs: those that hold one of its groups' 27 table entries.  Walked while the
+    // copies above are in flight (885k entries for 32,768 groups: milliseconds of host time); a bad entry is reported after
+    // the streams have drained
+    std::vector<std::vector<int>> need((size_t)n_chunks);
+    bool bad_entry = false;
+    {
+        std::vector<char> mark((size_t)n_chunks);
+        const uint32_t ng = (uint32_t)n_groups, ch = (uint32_t)chunk;
+        for (int64_t k = 0; k < n_chunks; ++k) {
+            std::fill(mark.begin(), mark.end(), 0);
+            const int64_t g1 = (k + 1) * chunk < n_groups ? (k + 1) * chunk : n_groups;
+            for (int64_t i = k * chunk * 27; i < g1 * 27; ++i) {
+                const uint32_t sidx = (uint32_t)nbr_host[i];      // a negative entry wraps above n_groups
+                if (sidx >= ng) { bad_entry = true; continue; }
+                mark[(size_t)(sidx / ch)] = 1;
+            }
+            for (int64_t c = 0; c < n_chunks; ++c)
+                if (mark[(size_t)c]) need[(size_t)k].push_back((int)c);
+            if (need[(size_t)k].empty()) need[(size_t)k].push_back((int)k);
+        }
+    }
+    if (bad_entry) {
+        cudaStreamSynchronize(R.st_in);
+        return GAMER_EINVAL;
+    }
+    // Output chunks are launched in the order in which their inputs arrive (the last input chunk each needs), not in index
+    // order: in a periodic box chunk 0 needs the LAST input chunk, and launched first it would hold its stream -- a third of
+    // all output chunks queued behind it -- until the whole state is on the device.
+    std::vector<int64_t> order((size_t)n_chunks);
+    for (int64_t k = 0; k < n_chunks; ++k) order[(size_t)k] = k;
+    std::stable_sort(order.begin(), order.end(), [&](int64_t a, int64_t b) { return need[(size_t)a].back() < need[(size_t)b].back(); });
     rc = GAMER_OK;
-    for (int64_t k = 0; k < n_chunks && rc == GAMER_OK; ++k) {
-        const int b = (int)(k % NBUF);
+    for (int64_t pos = 0; pos < n_chunks && rc == GAMER_OK; ++pos) {
+        const int64_t k = order[(size_t)pos];
+        const int b = (int)(pos % NBUF);
         const int64_t g0 = k * chunk, n = (n_groups - g0) < chunk ? (n_groups - g0) : chunk;
         for (int c : need[(size_t)k])
             if (cudaStreamWaitEvent(R.st[b], R.ev[(size_t)c], 0) != cudaSuccess) rc = GAMER_ECUDA;

@@ -348,8 +348,10 @@ __device__ __forceinline__ void trace_cell(const T* W, const T* wm, const T* wp,
         tp[1] -= amp * cor;
         tp[4] += amp * c2;
     }
-    if (vn > T(0)) {
-        const T A = T(0.5) * (x5p - x0), B = third * (x5p * x5p - x0 * x0);
+    {   // the lambda = vn waves reach one face or the other in every cell, and neighbouring cells disagree: taken without a
+        // branch (zero coefficients on the far face); the acoustic corrections above and below apply to supersonic cells only
+        const bool on = vn > T(0);
+        const T A = on ? T(0.5) * (x5p - x0) : T(0), B = on ? third * (x5p * x5p - x0 * x0) : T(0);
         const T vR = A * (d[0] - w6[0]) + B * w6[0];
         const T vP = A * (d[4] - w6[4]) + B * w6[4];
         tp[0] += vR - vP * ic2;
@@ -368,8 +370,9 @@ __device__ __forceinline__ void trace_cell(const T* W, const T* wm, const T* wp,
         tm[1] += amp * cor;
         tm[4] += amp * c2;
     }
-    if (vn < T(0)) {
-        const T C = T(0.5) * (x1m - x0), D = third * (x1m * x1m - x0 * x0);
+    {
+        const bool on = vn < T(0);
+        const T C = on ? T(0.5) * (x1m - x0) : T(0), D = on ? third * (x1m * x1m - x0 * x0) : T(0);
         const T vR = C * (d[0] + w6[0]) + D * w6[0];
         const T vP = C * (d[4] + w6[4]) + D * w6[4];
         tm[0] += vR - vP * ic2;
