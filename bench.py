@@ -406,7 +406,8 @@ def main():
         derived = 148 * lanes * 2 * sm_max * 1e6 / 1e12          # TFLOP/s, DESIGN.md "Rooflines"
         measured = alu["ffma" if szv == 4 else "dfma"]["tflops"]
         hbm_ach = bpc * cells / (kms * 1e-3) / 1e9
-        r = {"kernel": "mhm_kernel" if sch_name == "mhm" else "ctu_kernel"}
+        # VL runs in mhm_kernel (its VLS instantiation); CTU is the thread-owned ctu_kernel in fp32, the work-list ctu_wl_kernel in fp64
+        r = {"kernel": "ctu_kernel" if (sch_name == "ctu" and szv == 4) else ("ctu_wl_kernel" if sch_name == "ctu" else "mhm_kernel")}
         if fpc:
             ach = fpc * cells / (kms * 1e-3) / 1e12
             r.update({"bound": "alu", "achieved": ach, "peak": measured, "unit": "TFLOP/s", "frac": ach / measured,
