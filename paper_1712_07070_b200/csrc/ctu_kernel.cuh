@@ -180,8 +180,16 @@ __global__ void __launch_bounds__((CtuSmem<T, RECON, NV, TY, FUSED>::NT), 1) ctu
     // from the same-level neighbours inside the kernel (hydro_stream.cuh "Fused ghost refresh")
     const T* gin = FUSED ? a.in : a.in + (size_t)g * NV * NPC;
     int* nb = reinterpret_cast<int*>(smem_raw + 16 + S::END * sizeof(T));
-    const int2* ctab = nullptr;      // copy list decoded on the fly
-    if (FUSED && tid < 27) nb[tid] = a.nbr[g * 27 + tid];
+    constexpr int NCD = FUSED ? (FusedCopies<T, NV, TY>::N + NT - 1) / NT : 1;      // fused mode: this thread's entries of the copy list
+    int2 cd[NCD];
+    if (FUSED) {
+        if (tid < 27) nb[tid] = a.nbr[g * 27 + tid];
+#pragma unroll
+        for (int i = 0; i < NCD; ++i) {
+            const int it = tid + i * NT;
+            cd[i] = it < FusedCopies<T, NV, TY>::N ? fused_copy_desc<T, NV, TY>(it, j0) : make_int2(-1, 0);
+        }
+    }
     T* gout = a.out + (size_t)g * NV * PS3;
     T* gflux = a.flux ? a.flux + (size_t)g * 9 * NV * PSQ : nullptr;
     const Phys<T> ph = make_phys<T>(a);
@@ -228,7 +236,7 @@ __global__ void __launch_bounds__((CtuSmem<T, RECON, NV, TY, FUSED>::NT), 1) ctu
     __syncthreads();
     auto issue = [&](int n) {      // stage padded plane PF + n into landing stage n & 1
         if (FUSED) {
-            if (n < NPL) stage_plane_fused<T, NV, TY>(gin, nb, ctab, j0, PF + n, raw + (n & 1) * RS, tid, NT);
+            if (n < NPL) stage_plane_fused_regs<T, NV, NCD>(gin, nb, cd, PF + n, raw + (n & 1) * RS);
             else cp_async_commit();      // keeps "all but the newest group" = "everything older than one barrier"
         } else if (tid == 0 && n < NPL) {
             issue_plane<T, NV, TY>(gin, j0, PF + n, raw + (n & 1) * RS, &bars[n & 1]);

@@ -286,8 +286,16 @@ __global__ void __launch_bounds__(NT) ctu_wl_kernel(const AdvArgs<T> a) {
     // from the same-level neighbours inside the kernel (hydro_stream.cuh "Fused ghost refresh")
     const T* gin = FUSED ? a.in : a.in + (size_t)g * NV * NPC;
     int* nb = reinterpret_cast<int*>(smem_raw + 16 + S::END * sizeof(T));
-    const int2* ctab = nullptr;      // copy list decoded on the fly: a table would cost the fp64 variants a tile size
-    if (FUSED && tid < 27) nb[tid] = a.nbr[g * 27 + tid];
+    constexpr int NCD = FUSED ? (FusedCopies<T, NV, TY>::N + NT - 1) / NT : 1;      // fused mode: this thread's entries of the copy list
+    int2 cd[NCD];
+    if (FUSED) {
+        if (tid < 27) nb[tid] = a.nbr[g * 27 + tid];
+#pragma unroll
+        for (int i = 0; i < NCD; ++i) {
+            const int it = tid + i * NT;
+            cd[i] = it < FusedCopies<T, NV, TY>::N ? fused_copy_desc<T, NV, TY>(it, j0) : make_int2(-1, 0);
+        }
+    }
     T* gout = a.out + (size_t)g * NV * (PS * PS * PS);
     T* gflux = a.flux ? a.flux + (size_t)g * 9 * NV * (PS * PS) : nullptr;
     const Phys<T> ph = make_phys<T>(a);
@@ -299,8 +307,8 @@ __global__ void __launch_bounds__(NT) ctu_wl_kernel(const AdvArgs<T> a) {
     }
     __syncthreads();
     if (FUSED) {
-        stage_plane_fused<T, NV, TY>(gin, nb, ctab, j0, PF + 0, raw, tid, NT);
-        stage_plane_fused<T, NV, TY>(gin, nb, ctab, j0, PF + 1, raw + RS, tid, NT);
+        stage_plane_fused_regs<T, NV, NCD>(gin, nb, cd, PF + 0, raw);
+        stage_plane_fused_regs<T, NV, NCD>(gin, nb, cd, PF + 1, raw + RS);
     } else if (tid == 0) {
         issue_plane<T, NV, TY>(gin, j0, PF + 0, raw, &bars[0]);
         issue_plane<T, NV, TY>(gin, j0, PF + 1, raw + RS, &bars[1]);
@@ -316,7 +324,7 @@ __global__ void __launch_bounds__(NT) ctu_wl_kernel(const AdvArgs<T> a) {
         }
         __syncthreads();
         if (n + 2 < NPL) {
-            if (FUSED) stage_plane_fused<T, NV, TY>(gin, nb, ctab, j0, PF + n + 2, raw + (n & 1) * RS, tid, NT);
+            if (FUSED) stage_plane_fused_regs<T, NV, NCD>(gin, nb, cd, PF + n + 2, raw + (n & 1) * RS);
             else if (tid == 0) issue_plane<T, NV, TY>(gin, j0, PF + n + 2, raw + (n & 1) * RS, &bars[n & 1]);
         }
     }
@@ -456,7 +464,7 @@ __global__ void __launch_bounds__(NT) ctu_wl_kernel(const AdvArgs<T> a) {
         {
             const int n = kk + 4 + 2 * R;
             if (n < NPL) {
-                if (FUSED) stage_plane_fused<T, NV, TY>(gin, nb, ctab, j0, PF + n, raw + (n & 1) * RS, tid, NT);
+                if (FUSED) stage_plane_fused_regs<T, NV, NCD>(gin, nb, cd, PF + n, raw + (n & 1) * RS);
                 else if (tid == 0) issue_plane<T, NV, TY>(gin, j0, PF + n, raw + (n & 1) * RS, &bars[n & 1]);
             }
         }

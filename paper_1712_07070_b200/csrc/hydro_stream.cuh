@@ -168,8 +168,7 @@ template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile(
 
 // One copy of the gather of a padded plane: destination element inside the landing stage, source element inside a
 // group's plane z (v*16^3 + y*16 + x), which in-plane neighbour (dy*3 + dx) holds it, and whether it is a 16-byte
-// copy.  The list is the same for every plane, so it is built once per CTA (fused_copy_table) and each thread
-// issues the same few entries for every plane.
+// copy.  The list is the same for every plane: each thread decodes its few entries once (stage_plane_fused_regs).
 template <typename T, int NV, int TY> struct FusedCopies {
     static constexpr int CE = 16 / (int)sizeof(T);          // elements per 16-byte copy
     static constexpr int GC = 4 / CE;                       // copies per ghost side: the 3 ghost cells travel as the
@@ -196,24 +195,21 @@ __device__ __forceinline__ int2 fused_copy_desc(int it, int j0) {
     return make_int2((v * G::NR + r) * FW + col, (v * PS3 + yy * PS + xx) | ((dy * 3 + dx) << 20));
 }
 
-template <typename T, int NV, int TY>
-__device__ __forceinline__ void fused_copy_table(int2* tab, int j0, int tid, int nthr) {
-    for (int it = tid; it < FusedCopies<T, NV, TY>::N; it += nthr) tab[it] = fused_copy_desc<T, NV, TY>(it, j0);
-}
-
-// every thread issues its entries of the list for padded plane p (0..21) and commits them as one group;
-// tab == nullptr: the entries are decoded on the fly (CTU, where the list would cost a tile size in shared memory)
-template <typename T, int NV, int TY>
-__device__ __forceinline__ void stage_plane_fused(const T* u, const int* nb, const int2* tab, int j0, int p, T* raw_stage, int tid, int nthr) {
-    using F = FusedCopies<T, NV, TY>;
+// Every thread issues its own entries of the list for padded plane p (0..21) and commits them as one cp.async group.  The
+// entries (NCP = ceil(N / nthr) per thread, .x < 0 = none) are the same for every plane, so each thread decodes its own once,
+// keeps them in registers, and the per-plane work is one table look-up (neighbour group), one 64-bit address and the copy per entry.
+template <typename T, int NV, int NCP>
+__device__ __forceinline__ void stage_plane_fused_regs(const T* u, const int* nb, const int2 (&cd)[NCP], int p, T* raw_stage) {
     constexpr int PS3 = PS * PS * PS;
     const int dz = p < NGH ? 0 : (p < NGH + PS ? 1 : 2);
     const int zoff = ((p + PS - NGH) & (PS - 1)) * (PS * PS);
     const int* nbz = nb + dz * 9;
-    for (int it = tid; it < F::N; it += nthr) {
-        const int2 d = tab ? tab[it] : fused_copy_desc<T, NV, TY>(it, j0);
-        const T* src = u + (size_t)nbz[d.y >> 20] * NV * PS3 + ((d.y & 0xfffff) + zoff);
-        cp_async_16(raw_stage + d.x, src);
+#pragma unroll
+    for (int i = 0; i < NCP; ++i) {
+        if (cd[i].x >= 0) {
+            const T* src = u + (size_t)nbz[cd[i].y >> 20] * NV * PS3 + ((cd[i].y & 0xfffff) + zoff);
+            cp_async_16(raw_stage + cd[i].x, src);
+        }
     }
     cp_async_commit();
 }

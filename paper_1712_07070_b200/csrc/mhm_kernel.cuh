@@ -54,8 +54,7 @@ template <typename T, int RECON, int NV, int TY, int NSTG = 2, bool FUSED = fals
     static constexpr int F1Z = F1Y + NV * NF1Y;                 // [2][NV][NF1Z]: faces below planes of even / odd padded index
     static constexpr int END = VLS ? F1Z + 2 * NV * NF1Z : END0;
     static constexpr int NCOPY = FUSED ? FusedCopies<T, NV, TY>::N : 0;                   // fused refresh: copy list
-    static constexpr size_t BYTES = 16 + (size_t)END * sizeof(T) + (FUSED ? 128 + 8 * (size_t)NCOPY : 0);   // 2 mbarriers
-                                                                // first; neighbour table and copy list last
+    static constexpr size_t BYTES = 16 + (size_t)END * sizeof(T) + (FUSED ? 128 : 0);   // 2 mbarriers first; neighbour table last
     static_assert((NV * PLN) % 4 == 0 && NSX % 4 == 0 && NSY % 4 == 0, "16-byte alignment of the Vec4 arrays");
 };
 
@@ -263,10 +262,15 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED, VLS>::N
     // padded mode: this group's padded slab; fused mode: the whole unpadded batch (neighbours are read too)
     const T* gin = FUSED ? a.in : a.in + (size_t)g * NV * NPC;
     int* nb = reinterpret_cast<int*>(smem_raw + 16 + G::END * sizeof(T));      // fused mode: 27 neighbour groups
-    int2* ctab = reinterpret_cast<int2*>(smem_raw + 16 + G::END * sizeof(T) + 128);
+    constexpr int NCP = FUSED ? (G::NCOPY + NT - 1) / NT : 1;      // fused mode: this thread's entries of the copy list, in registers
+    int2 cd[NCP];
     if (FUSED) {
         if (tid < 27) nb[tid] = a.nbr[g * 27 + tid];
-        fused_copy_table<T, NV, TY>(ctab, j0, tid, NT);
+#pragma unroll
+        for (int i = 0; i < NCP; ++i) {
+            const int it = tid + i * NT;
+            cd[i] = it < G::NCOPY ? fused_copy_desc<T, NV, TY>(it, j0) : make_int2(-1, 0);
+        }
     }
     const Phys<T> ph = make_phys<T>(a);
 
@@ -315,8 +319,8 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED, VLS>::N
     }
     __syncthreads();
     if (FUSED) {      // every thread issues a few copies of each plane (cp.async groups are per thread)
-        stage_plane_fused<T, NV, TY>(gin, nb, ctab, j0, PF + 0, raw, tid, NT);
-        stage_plane_fused<T, NV, TY>(gin, nb, ctab, j0, PF + 1, raw + RS, tid, NT);
+        stage_plane_fused_regs<T, NV, NCP>(gin, nb, cd, PF + 0, raw);
+        stage_plane_fused_regs<T, NV, NCP>(gin, nb, cd, PF + 1, raw + RS);
     } else if (tid == NI) {
         issue_plane<T, NV, TY>(gin, j0, PF + 0, raw, &bars[0]);
         if (NSTG > 1) issue_plane<T, NV, TY>(gin, j0, PF + 1, raw + RS, &bars[1]);
@@ -333,7 +337,7 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED, VLS>::N
         }
         __syncthreads();
         if (n + NSTG < NPL) {
-            if (FUSED) stage_plane_fused<T, NV, TY>(gin, nb, ctab, j0, PF + n + NSTG, raw + (n % NSTG) * RS, tid, NT);
+            if (FUSED) stage_plane_fused_regs<T, NV, NCP>(gin, nb, cd, PF + n + NSTG, raw + (n % NSTG) * RS);
             else if (tid == NI) issue_plane<T, NV, TY>(gin, j0, PF + n + NSTG, raw + (n % NSTG) * RS, &bars[n % NSTG]);
         }
     };
@@ -496,7 +500,7 @@ __global__ void __launch_bounds__((MhmGeo<T, RECON, NV, TY, NSTG, FUSED, VLS>::N
         {      // the stage the plane above came from is free again
             const int n = kk + CV + NSTG;
             if (n < NPL) {
-                if (FUSED) stage_plane_fused<T, NV, TY>(gin, nb, ctab, j0, PF + n, raw + (n % NSTG) * RS, tid, NT);
+                if (FUSED) stage_plane_fused_regs<T, NV, NCP>(gin, nb, cd, PF + n, raw + (n % NSTG) * RS);
                 else if (tid == NI) issue_plane<T, NV, TY>(gin, j0, PF + n, raw + (n % NSTG) * RS, &bars[n % NSTG]);
             }
         }
