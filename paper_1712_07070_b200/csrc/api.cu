@@ -303,11 +303,11 @@ static void launch_interp(const void* c0, const void* c1, double w, void* fine, 
     T* f = static_cast<T*>(fine);
     const T w0 = T(1.0 - w), w1 = T(w);
     if (a1) {
-        if (monotonic) interpolate_ghosts_kernel<T, true, true><<<grid, 256, 0, st>>>(a0, a1, w0, w1, f, parent, nbr, nvar);
-        else interpolate_ghosts_kernel<T, true, false><<<grid, 256, 0, st>>>(a0, a1, w0, w1, f, parent, nbr, nvar);
+        if (monotonic) interpolate_ghosts_kernel<T, true, true><<<grid, INTERP_NT, 0, st>>>(a0, a1, w0, w1, f, parent, nbr, nvar);
+        else interpolate_ghosts_kernel<T, true, false><<<grid, INTERP_NT, 0, st>>>(a0, a1, w0, w1, f, parent, nbr, nvar);
     } else {
-        if (monotonic) interpolate_ghosts_kernel<T, false, true><<<grid, 256, 0, st>>>(a0, a1, w0, w1, f, parent, nbr, nvar);
-        else interpolate_ghosts_kernel<T, false, false><<<grid, 256, 0, st>>>(a0, a1, w0, w1, f, parent, nbr, nvar);
+        if (monotonic) interpolate_ghosts_kernel<T, false, true><<<grid, INTERP_NT, 0, st>>>(a0, a1, w0, w1, f, parent, nbr, nvar);
+        else interpolate_ghosts_kernel<T, false, false><<<grid, INTERP_NT, 0, st>>>(a0, a1, w0, w1, f, parent, nbr, nvar);
     }
 }
 

@@ -227,10 +227,17 @@ __global__ void __launch_bounds__(256) refresh_table_kernel(const T* __restrict_
 __device__ __forceinline__ double blend_rn(double w0, double a, double w1, double b) { return __dadd_rn(__dmul_rn(w0, a), __dmul_rn(w1, b)); }
 __device__ __forceinline__ float blend_rn(float w0, float a, float w1, float b) { return __fadd_rn(__fmul_rn(w0, a), __fmul_rn(w1, b)); }
 
+// Work is organised by coarse cell in y and z and by FINE cell in x: u and the three limited slopes are formed once per
+// (coarse z, coarse y, fine x) item and serve its four (ck, cj) children, whose signs are compile-time constants of the
+// unrolled loops, and consecutive lanes write consecutive fine cells.  (The first version walked the 22^3 fine cells and
+// rebuilt the slopes for every one of them: 99 instructions per ghost value, issue-bound at 27 % of the HBM roof; a version
+// with all eight children per thread wrote every other cell of a row per store: 6.5 sectors per request.)
+constexpr int INTERP_NT = 288;
+
 template <typename T, bool BLEND, bool MONO>
-__global__ void __launch_bounds__(256) interpolate_ghosts_kernel(const T* __restrict__ c0, const T* __restrict__ c1, T w0, T w1,
-                                                                 T* __restrict__ fine, const int* __restrict__ parent,
-                                                                 const int* __restrict__ nbr, int nvar) {
+__global__ void __launch_bounds__(INTERP_NT) interpolate_ghosts_kernel(const T* __restrict__ c0, const T* __restrict__ c1, T w0, T w1,
+                                                                       T* __restrict__ fine, const int* __restrict__ parent,
+                                                                       const int* __restrict__ nbr, int nvar) {
     __shared__ int nb[27];
     const long long gv = blockIdx.x;
     const long long g = gv / nvar;
@@ -248,14 +255,17 @@ __global__ void __launch_bounds__(256) interpolate_ghosts_kernel(const T* __rest
     const T* a1 = BLEND ? c1 + cbase : nullptr;
     T* dst = fine + ((size_t)g * nvar + v) * NPC;
     // the 14^3 coarse cells under this octant's ghost zones (+1 for the slopes), blended in time once: padded coarse
-    // indices 8 o .. 8 o + 13 along each axis
+    // indices 8 o .. 8 o + 13 along each axis; a thread carries one (j, i) of the block through its 14 planes
     constexpr int CB = 14;
     __shared__ T cs[CB * CB * CB];
-    for (int t = threadIdx.x; t < CB * CB * CB; t += 256) {
-        const int k = t / (CB * CB), r = t - k * (CB * CB), j = r / CB, i = r - j * CB;
-        const int q = ((8 * oz + k) * NP + 8 * oy + j) * NP + 8 * ox + i;
-        const T x = __ldg(a0 + q);
-        cs[t] = BLEND ? blend_rn(w0, x, w1, __ldg(a1 + q)) : x;
+    for (int t = threadIdx.x; t < CB * CB; t += INTERP_NT) {
+        const int j = t / CB, i = t - j * CB;
+        const int q0 = ((8 * oz) * NP + 8 * oy + j) * NP + 8 * ox + i;
+#pragma unroll
+        for (int k = 0; k < CB; ++k) {
+            const T x = __ldg(a0 + q0 + k * (NP * NP));
+            cs[k * (CB * CB) + t] = BLEND ? blend_rn(w0, x, w1, __ldg(a1 + q0 + k * (NP * NP))) : x;
+        }
     }
     __syncthreads();
     auto slope = [&](T lo, T mid, T hi) -> T {
@@ -263,25 +273,53 @@ __global__ void __launch_bounds__(256) interpolate_ghosts_kernel(const T* __rest
         const T a = mid - lo, b = hi - mid;
         return a * b > T(0) ? (fabs(a) < fabs(b) ? a : b) : T(0);
     };
-    for (int t = threadIdx.x; t < NP * NP; t += 256) {
-        const int pj = t / NP, pi = t - pj * NP;
-        const int dx = pi < NGH ? 0 : (pi < NGH + PS ? 1 : 2), dy = pj < NGH ? 0 : (pj < NGH + PS ? 1 : 2);
-        // floor((p - 3) / 2) = ((p + 1) >> 1) - 2 for p >= 0, i.e. index ((p + 1) >> 1) + 1 of the staged block;
-        // child parity = (p + 1) & 1
-        const int lj = ((pj + 1) >> 1) + 1, li = ((pi + 1) >> 1) + 1;
-        const bool uj = (pj + 1) & 1, ui = (pi + 1) & 1;
-        for (int pk = 0; pk < NP; ++pk) {
-            const int dz = pk < NGH ? 0 : (pk < NGH + PS ? 1 : 2);
-            const int s = dz * 9 + dy * 3 + dx;
-            if (s == 13 || nb[s] >= 0) continue;
-            const int lk = ((pk + 1) >> 1) + 1;
-            const bool uk = (pk + 1) & 1;
-            const int q = (lk * CB + lj) * CB + li;
-            const T u = cs[q];
-            const T sz = slope(cs[q - CB * CB], u, cs[q + CB * CB]);
-            const T sy = slope(cs[q - CB], u, cs[q + CB]);
-            const T sx = slope(cs[q - 1], u, cs[q + 1]);
-            dst[(pk * NP + pj) * NP + pi] = u + T(0.25) * (((uk ? sz : -sz) + (uj ? sy : -sy)) + (ui ? sx : -sx));
+    // Staged coarse index l = 1..12 along an axis holds the fine padded cells p = 2l - 3 (child 0) and 2l - 2 (child 1):
+    // l = 1, 2 are the low ghost zones (p = 0 | 1, 2), l = 3..10 the interior, l = 11, 12 the high ones (p = 19, 20 | 21);
+    // p = -1 and p = 22 do not exist.  Both children of a coarse cell lie in the same slab of the neighbour table.
+    // Work items = (coarse z, coarse y, fine x) triples of the ghost shell only, in three segments: the four z-ghost
+    // coarse planes in full (4 x 12 x 22), the four y-ghost coarse rows of the eight inner planes (8 x 4 x 22), the six
+    // x-ghost fine columns of their inner rows (8 x 8 x 6).  2144 items of four children each (6552 ghost cells, plus the
+    // children at p = -1 / 22 that do not exist) instead of 12 x 12 x 22 with the interior masked out.
+    constexpr int NA = 4 * 12 * NP, NB = 8 * 4 * NP, NC = 8 * 8 * 6;
+    for (int it = threadIdx.x; it < NA + NB + NC; it += INTERP_NT) {
+        int lk, lj, pi;
+        if (it < NA) {
+            const int a = it / (12 * NP), r = it - a * (12 * NP);
+            lk = a < 2 ? a + 1 : a + 9;
+            lj = r / NP + 1;
+            pi = r - (lj - 1) * NP;
+        } else if (it < NA + NB) {
+            const int r = it - NA, a = r / (4 * NP), r2 = r - a * (4 * NP), c = r2 / NP;
+            lk = a + 3;
+            lj = c < 2 ? c + 1 : c + 9;
+            pi = r2 - c * NP;
+        } else {
+            const int r = it - NA - NB, a = r / 48, r2 = r - a * 48, c = r2 / 6, x = r2 - c * 6;
+            lk = a + 3;
+            lj = c + 3;
+            pi = x < 3 ? x : x + 16;
+        }
+        const int li = ((pi + 1) >> 1) + 1;
+        const bool ui = (pi + 1) & 1;
+        const int dz = lk < 3 ? 0 : (lk < 11 ? 1 : 2), dy = lj < 3 ? 0 : (lj < 11 ? 1 : 2), dx = li < 3 ? 0 : (li < 11 ? 1 : 2);
+        if (nb[dz * 9 + dy * 3 + dx] >= 0) continue;
+        const int q = (lk * CB + lj) * CB + li;
+        const T u = cs[q];
+        const T sz = slope(cs[q - CB * CB], u, cs[q + CB * CB]);
+        const T sy = slope(cs[q - CB], u, cs[q + CB]);
+        const T sx = slope(cs[q - 1], u, cs[q + 1]);
+        const T sxs = ui ? sx : -sx;
+        const int pk0 = 2 * lk - 3, pj0 = 2 * lj - 3;
+#pragma unroll
+        for (int ck = 0; ck < 2; ++ck) {
+            const int pk = pk0 + ck;
+            if (pk < 0 || pk >= NP) continue;
+#pragma unroll
+            for (int cj = 0; cj < 2; ++cj) {
+                const int pj = pj0 + cj;
+                if (pj < 0 || pj >= NP) continue;
+                dst[(pk * NP + pj) * NP + pi] = u + T(0.25) * (((ck ? sz : -sz) + (cj ? sy : -sy)) + sxs);
+            }
         }
     }
 }
