@@ -243,9 +243,24 @@ template <typename T> struct alignas(16) Vec4 {
     T a, b, c, d;
 };
 
-// five (six) values of one face <-> shared memory: one Vec4 + NV-4 scalars; n = entries of the array
+template <typename T> struct alignas(16) Vec2 {
+    T a, b;
+};
+
+// five (six) values of one face <-> shared memory: one Vec4 + NV-4 scalars; n = entries of the array.
+// fp64: a 32-byte Vec4 per lane is two 16-byte accesses at stride 32 -- every quarter-warp spans 256 bytes, a 2-way bank
+// conflict on each -- so the four values are kept as two arrays of 16-byte pairs [Vec2 n | Vec2 n | (NV-4) x n] in the same space.
 template <typename T, int NV>
 __device__ __forceinline__ void put_state(T* blk, int n, int idx, const T* W) {
+    if constexpr (sizeof(T) == 8) {
+        Vec2<T> lo, hi;
+        lo.a = W[0]; lo.b = W[1]; hi.a = W[2]; hi.b = W[3];
+        reinterpret_cast<Vec2<T>*>(blk)[idx] = lo;
+        reinterpret_cast<Vec2<T>*>(blk + 2 * n)[idx] = hi;
+#pragma unroll
+        for (int v = 4; v < NV; ++v) blk[v * n + idx] = W[v];
+        return;
+    }
     Vec4<T> q;
     q.a = W[0]; q.b = W[1]; q.c = W[2]; q.d = W[3];
     reinterpret_cast<Vec4<T>*>(blk)[idx] = q;
@@ -254,6 +269,14 @@ __device__ __forceinline__ void put_state(T* blk, int n, int idx, const T* W) {
 }
 template <typename T, int NV>
 __device__ __forceinline__ void get_state(const T* blk, int n, int idx, T* W) {
+    if constexpr (sizeof(T) == 8) {
+        const Vec2<T> lo = reinterpret_cast<const Vec2<T>*>(blk)[idx];
+        const Vec2<T> hi = reinterpret_cast<const Vec2<T>*>(blk + 2 * n)[idx];
+        W[0] = lo.a; W[1] = lo.b; W[2] = hi.a; W[3] = hi.b;
+#pragma unroll
+        for (int v = 4; v < NV; ++v) W[v] = blk[v * n + idx];
+        return;
+    }
     const Vec4<T> q = reinterpret_cast<const Vec4<T>*>(blk)[idx];
     W[0] = q.a; W[1] = q.b; W[2] = q.c; W[3] = q.d;
 #pragma unroll
