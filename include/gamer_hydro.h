@@ -228,7 +228,7 @@ int gamer_flux_correct(void* coarse, const void* coarse_flux, const void* fine_f
  * potential").  resid_out (nullable) real[n_patches] = max over the relaxed cells of |sum of the 6 neighbours - 6 phi -
  * coeff * dh^2 * rho| after the last iteration: dh^2 times the defect of the discretised equation, for the caller to judge "to
  * machine precision" (L126) and iterate on.  0 < omega < 2; n_iter >= 0; the potential lives in shared memory for the whole
- * solve (46.8 KB in fp64). */
+ * solve (49.2 KB in fp64). */
 int gamer_poisson_sor(void* phi, const void* rho, void* acc, void* resid_out, int64_t n_patches, double dh, double coeff,
                       double omega, int n_iter, int precision, void* stream);
 

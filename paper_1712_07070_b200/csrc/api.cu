@@ -338,12 +338,15 @@ static int poisson_sor_impl(void* phi, const void* rho, void* acc, void* resid_o
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const unsigned grid = (unsigned)n_patches;
     const double ss = coeff * dh * dh, w6 = omega / 6.0, i2 = 1.0 / (2.0 * dh);
+    if (precision == GAMER_FP64 &&      // 49.2 KB of dynamic shared memory: above the default limit
+        cudaFuncSetAttribute(poisson_sor_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SorGeo<double>::BYTES) != cudaSuccess)
+        return GAMER_ECUDA;
     if (precision == GAMER_FP32)
-        poisson_sor_kernel<float><<<grid, 256, 0, st>>>(static_cast<float*>(phi), static_cast<const float*>(rho),
+        poisson_sor_kernel<float><<<grid, 256, SorGeo<float>::BYTES, st>>>(static_cast<float*>(phi), static_cast<const float*>(rho),
                                                         static_cast<float*>(acc), static_cast<float*>(resid_out), (float)ss, (float)w6,
                                                         (float)i2, n_iter, static_cast<float*>(flu), nvar, (float)dt);
     else
-        poisson_sor_kernel<double><<<grid, 256, 0, st>>>(static_cast<double*>(phi), static_cast<const double*>(rho),
+        poisson_sor_kernel<double><<<grid, 256, SorGeo<double>::BYTES, st>>>(static_cast<double*>(phi), static_cast<const double*>(rho),
                                                          static_cast<double*>(acc), static_cast<double*>(resid_out), ss, w6, i2, n_iter,
                                                          static_cast<double*>(flu), nvar, dt);
     g_launches += 1;

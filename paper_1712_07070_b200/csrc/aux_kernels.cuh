@@ -325,11 +325,23 @@ __global__ void __launch_bounds__(INTERP_NT) interpolate_ghosts_kernel(const T* 
 }
 
 // Refined-level Poisson solver (R25): one CTA relaxes one patch's
-// (8 + 2*5)^3 = 18^3 potential, held entirely in shared memory as the paper does (46.7 KB in fp64), by red-black SOR with
+// (8 + 2*5)^3 = 18^3 potential, held entirely in shared memory as the paper does (49.2 KB in fp64 with its padded rows), by red-black SOR with
 // the outermost cells fixed; thread (k, j) owns row (k, j) of the 16^3 relaxed cells: 8 cells per colour, source term in
 // registers.  Then the potential goes back and, optionally, -grad(phi) of the 8^3 active zones by central differences.
 constexpr int PN = 18, PR = 16, PA0 = 5, PAN = 8;
-constexpr int PPL = PN * PN + 1;   // plane stride in shared memory: = 1 (mod 4), see the bank note below
+// Row and plane stride of the potential in shared memory.  fp32: rows of 18, planes of 18 * 18 + 1 (= 1 mod 4), see the bank
+// note below.  fp64: a lane's 8-byte access covers a pair of banks and a warp is served as two half-warps of 16 lanes = 2 plane
+// indices k x 8 row indices j (stride 2, parity alternating with k).  With rows of 18 doubles two j-rows are 72 words apart:
+// 72 m mod 32 takes only four values, rows m and m + 4 share their banks -- a 2-way conflict on every access (measured: 50 %
+// excess wavefronts with the shared-memory pipe 95 % busy).  Rows of 19 doubles: 76 m mod 32 = 12 m = 0, 12, 24, 4, 16, 28, 8, 20,
+// eight distinct bank pairs {4q, 4q+1}; the plane stride must then be EVEN (342): the next k is 684 +- 38 words on (its rows have
+// the other parity) = 18 or 6 mod 32, the pairs {4q+2, 4q+3} -- one wavefront per half-warp.  (Checked with a 32-lane
+// LDS.64 microbenchmark: 343 gives the 2-way conflict back.)
+template <typename T> struct SorGeo {
+    static constexpr int RS = sizeof(T) == 8 ? 19 : 18;                    // row stride
+    static constexpr int PL = PN * RS + (sizeof(T) == 8 ? 0 : 1);          // plane stride: 325 (fp32), 342 (fp64)
+    static constexpr size_t BYTES = (size_t)PN * PL * sizeof(T);
+};
 
 // One half-sweep over the cells i = 2 - IP, 4 - IP, ... of the thread's row: x-neighbours from the row's registers, the four
 // others from shared memory, the new value to both.  Same order of additions as the oracle.
@@ -339,7 +351,8 @@ __device__ __forceinline__ void sor_half_sweep(T (&me)[PN], const T (&src)[PR], 
     for (int m = 0; m < PR / 2; ++m) {
         constexpr int dummy = 0; (void)dummy;
         const int i = 2 - IP + 2 * m;
-        const T r = me[i - 1] + me[i + 1] + row[i - PN] + row[i + PN] + row[i - PPL] + row[i + PPL] - T(6) * me[i] - src[i - 1];
+        constexpr int RS = SorGeo<T>::RS, PL = SorGeo<T>::PL;
+        const T r = me[i - 1] + me[i + 1] + row[i - RS] + row[i + RS] + row[i - PL] + row[i + PL] - T(6) * me[i] - src[i - 1];
         me[i] += w6 * r;
         row[i] = me[i];
     }
@@ -383,12 +396,14 @@ template <typename T>
 __global__ void __launch_bounds__(256) poisson_sor_kernel(T* __restrict__ phi, const T* __restrict__ rho, T* __restrict__ acc,
                                                           T* __restrict__ resid, T src_scale, T w6, T inv_2dh, int n_iter,
                                                           T* __restrict__ flu = nullptr, int nvar = 0, T dt_g = T(0)) {
-    __shared__ T p[PN * PPL];
+    constexpr int RS = SorGeo<T>::RS, PL = SorGeo<T>::PL;
+    extern __shared__ __align__(16) unsigned char sor_smem[];      // SorGeo<T>::BYTES (fp64: 49.2 KB, above the static limit)
+    T* p = reinterpret_cast<T*>(sor_smem);
     const size_t n = blockIdx.x;
     T* gp = phi + n * (PN * PN * PN);
     for (int t = threadIdx.x; t < PN * PN * PN; t += 256) {
-        const int kk = t / (PN * PN);
-        p[kk * PPL + t - kk * (PN * PN)] = gp[t];
+        const int kk = t / (PN * PN), rr = t - kk * (PN * PN), jj = rr / PN;
+        p[kk * PL + jj * RS + (rr - jj * PN)] = gp[t];
     }
     const int par = threadIdx.x >> 7, r = threadIdx.x & 127;
     const int k = 1 + (r >> 3), j = 1 + 2 * (r & 7) + ((par + k + 1) & 1);
@@ -397,7 +412,7 @@ __global__ void __launch_bounds__(256) poisson_sor_kernel(T* __restrict__ phi, c
 #pragma unroll
     for (int i = 0; i < PR; ++i) src[i] = src_scale * gr[i];
     __syncthreads();
-    T* row = p + k * PPL + j * PN;
+    T* row = p + k * PL + j * RS;
 #pragma unroll
     for (int i = 0; i < PN; ++i) me[i] = row[i];
     for (int it = 0; it < n_iter; ++it) {
@@ -413,7 +428,7 @@ __global__ void __launch_bounds__(256) poisson_sor_kernel(T* __restrict__ phi, c
         T m = T(0);
 #pragma unroll
         for (int i = 1; i <= PR; ++i)
-            m = fmax(m, fabs(me[i - 1] + me[i + 1] + row[i - PN] + row[i + PN] + row[i - PPL] + row[i + PPL] - T(6) * me[i] - src[i - 1]));
+            m = fmax(m, fabs(me[i - 1] + me[i + 1] + row[i - RS] + row[i + RS] + row[i - PL] + row[i + PL] - T(6) * me[i] - src[i - 1]));
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
         if ((threadIdx.x & 31) == 0) wmax[threadIdx.x >> 5] = m;
@@ -425,15 +440,15 @@ __global__ void __launch_bounds__(256) poisson_sor_kernel(T* __restrict__ phi, c
         }
     }
     for (int t = threadIdx.x; t < PN * PN * PN; t += 256) {
-        const int kk = t / (PN * PN);
-        gp[t] = p[kk * PPL + t - kk * (PN * PN)];
+        const int kk = t / (PN * PN), rr = t - kk * (PN * PN), jj = rr / PN;
+        gp[t] = p[kk * PL + jj * RS + (rr - jj * PN)];
     }
     if (acc || flu) {      // acceleration of the active zones; the fluid's gravity update straight from it (L238)
         T* ga = acc ? acc + n * (3 * PAN * PAN * PAN) : nullptr;
         for (int t = threadIdx.x; t < PAN * PAN * PAN; t += 256) {
             const int ak = t / (PAN * PAN), aj = (t / PAN) % PAN, ai = t % PAN;
-            const T* c = p + (ak + PA0) * PPL + (aj + PA0) * PN + ai + PA0;
-            const T ax = -(c[1] - c[-1]) * inv_2dh, ay = -(c[PN] - c[-PN]) * inv_2dh, az = -(c[PPL] - c[-PPL]) * inv_2dh;
+            const T* c = p + (ak + PA0) * PL + (aj + PA0) * RS + ai + PA0;
+            const T ax = -(c[1] - c[-1]) * inv_2dh, ay = -(c[RS] - c[-RS]) * inv_2dh, az = -(c[PL] - c[-PL]) * inv_2dh;
             if (ga) {
                 ga[t] = ax;
                 ga[t + PAN * PAN * PAN] = ay;
