@@ -344,6 +344,18 @@ def main():
                    "hbm_GBs": npatch * (2 * 18 ** 3 + 16 ** 3 + 3 * 512) * sz / tsor / 1e9}
         finite = finite and bool(torch.isfinite(phi).all().item()) and bool(torch.isfinite(acc_p).all().item())
         del phi, rho_p, acc_p
+        if dtype == torch.float32:      # the same solve in fp64 (its own shared-memory layout), one timed call
+            phi = torch.randn((npatch, 18, 18, 18), generator=gsor, dtype=torch.float64, device=dev)
+            rho_p = torch.randn((npatch, 16, 16, 16), generator=gsor, dtype=torch.float64, device=dev) + 2.0
+            acc_p = torch.empty((npatch, 3, 8, 8, 8), dtype=torch.float64, device=dev)
+            gb.gamer_poisson_sor(phi, rho_p, acc_p, dh, 1.0, om, nit, stream)
+            p0.record(stream)
+            gb.gamer_poisson_sor(phi, rho_p, acc_p, dh, 1.0, om, nit, stream)
+            p1.record(stream)
+            torch.cuda.synchronize()
+            poisson["fp64_cells_per_s"] = npatch * 512 / (p0.elapsed_time(p1) * 1e-3)
+            finite = finite and bool(torch.isfinite(phi).all().item())
+            del phi, rho_p, acc_p
 
     # ---- e2e: host buffers through the C ABI, copies inside the timed region.  gamer_fluid_advance_host_resident ships the
     # UNPADDED state + neighbour table (no ghost bytes cross PCIe) for ALL groups of the workload; the two pinned state
